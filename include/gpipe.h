@@ -1,0 +1,174 @@
+/* gpipe.h - C ABI of the B200-native GPipe hot path (libgpipe_b200.so).
+ *
+ * What the library computes (citations: /root/reference/PAPER.md line numbers, arXiv 1811.06965):
+ *   A model is "a sequence of L layers" partitioned into K consecutive cells (2.1;
+ *   the user specifies "(i) the number of model partitions K, (ii) the number of micro-batches
+ *   M, and (iii) the sequence and definitions of L layers").  Every mini-batch of
+ *   N sequences is divided into M equal micro-batches which are pipelined through the K cells;
+ *   the backward pass of each micro-batch uses the same parameters as its forward pass;
+ *   gradients of all M micro-batches are accumulated and applied once per mini-batch
+ *   (2.2).  With re-materialization each cell stores only its boundary (input)
+ *   activation and recomputes its forward F_k just before its backward (2.3); the
+ *   recompute does not wait for the upstream gradient.
+ *   The layers are pre-LayerNorm self-attention + ReLU-FFN Transformer layers
+ *   (BASELINE.json north_star; readings A2-A8), the loss is the token-mean softmax
+ *   cross-entropy of the whole mini-batch.
+ *
+ * On one GPU the K cells are K CUDA streams with event dependencies F(k,m) <- F(k-1,m),
+ * B(k,m) <- B(k+1,m) (Fig. 2c).  All arithmetic runs in the library's own
+ * sm_100a kernels.  There is no CPU fallback: every call fails with GPIPE_ECUDA if no device
+ * is usable.
+ *
+ * Conventions
+ *   - Status: 0 = success, negative = error; gpipe_last_error() returns a thread-local,
+ *     NUL-terminated message for the last failing call on this thread.  Nothing aborts or
+ *     throws across this boundary.
+ *   - "host" / "device" is stated per pointer.  All matrices are row-major, y = x * W.
+ *   - The library never allocates device memory: the caller passes one arena and K streams
+ *     (PyTorch supplies both in the Python binding).  The arena must stay alive and untouched
+ *     until gpipe_destroy.
+ *   - Canonical tensor order (index i of gpipe_tensor_info / get / set):
+ *       emb [V,d];
+ *       per layer l: ln1_g [1,d], ln1_b [1,d], w_qkv [d,3*da] (column blocks q|k|v, head h owns
+ *       columns h*d_head.. of each block), b_qkv [1,3*da], w_o [da,d], b_o [1,d], ln2_g, ln2_b,
+ *       w_1 [d,H], b_1 [1,H], w_2 [H,d], b_2 [1,d];
+ *       lnf_g [1,d], lnf_b [1,d], w_out [d,V].     (da = n_heads * d_head)
+ */
+#ifndef GPIPE_H_
+#define GPIPE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+#if defined(__GNUC__)
+#pragma GCC visibility push(default)   /* the library is built with -fvisibility=hidden */
+#endif
+
+#define GPIPE_OK        0
+#define GPIPE_EINVAL   -1   /* bad argument / unsupported shape; message says which            */
+#define GPIPE_ECUDA    -2   /* CUDA runtime/driver error; message carries the CUDA error string */
+#define GPIPE_ENOMEM   -3   /* arena too small; message carries the needed byte count           */
+#define GPIPE_ENOTIMPL -4
+
+#define GPIPE_DTYPE_FP32 0  /* fp32 storage and arithmetic everywhere, TF32 off (SIMT FMA)      */
+#define GPIPE_DTYPE_BF16 1  /* bf16 weights/activations as tensor-core operands, fp32 residual
+                               stream, fp32 accumulation, fp32 master weights and gradients      */
+
+/* peak-HBM categories (index into by_category[]) */
+#define GPIPE_CAT_WEIGHTS   0   /* working copy of the parameters (bf16 in bf16 mode, else fp32) */
+#define GPIPE_CAT_MASTERS   1   /* fp32 master copy (bf16 mode only)                             */
+#define GPIPE_CAT_GRADS     2   /* fp32 gradient accumulators                                    */
+#define GPIPE_CAT_BOUNDARY  3   /* K*M cell-boundary activations + boundary-gradient ring        */
+#define GPIPE_CAT_INTERIOR  4   /* per-cell interior workspaces (x M when remat is off)          */
+#define GPIPE_CAT_HEAD      5   /* logits / dlogits workspace, loss partials                     */
+#define GPIPE_CAT_MISC      6   /* token ids, positional table, reduction scratch                */
+#define GPIPE_CAT_BWD       7   /* backward-pass scratch of a cell (activation gradients)        */
+#define GPIPE_NUM_CATS      8
+
+typedef struct gpipe gpipe_t;   /* opaque handle, owned by the library */
+
+/* "the sequence and definitions of L layers": n_layers identical Transformer
+ * layers that differ only in their attention mask. */
+typedef struct {
+  int32_t n_layers;     /* L >= 0                                                              */
+  int32_t d_model;      /* d, multiple of 4 (bf16 mode: multiple of 64)                        */
+  int32_t d_ffn;        /* H                                                                   */
+  int32_t n_heads;      /* A                                                                   */
+  int32_t d_head;       /* 0 -> d_model / n_heads.  Supported: 16, 32, 64, 128                 */
+  int32_t vocab;        /* V                                                                   */
+  int32_t seq_len;      /* S, every sequence has exactly S tokens (dense batches)              */
+  int32_t dtype;        /* GPIPE_DTYPE_*                                                       */
+  const uint8_t *causal;/* host, [n_layers] 0/1, read during gpipe_create only; NULL = all 1   */
+  float   ln_eps;       /* 0 -> 1e-5                                                           */
+} gpipe_layer_spec;
+
+typedef struct {
+  void   *arena;        /* device, >= gpipe_plan_bytes(), 1024-byte aligned                    */
+  size_t  arena_bytes;
+  void *const *streams; /* host array of n_streams cudaStream_t, one per cell (n_streams >= K) */
+  int32_t n_streams;
+} gpipe_env;
+
+/* One scheduled task of a traced step (gpipe_trace): kind 'F' forward, 'R' re-materialization
+ * replay, 'B' backward; start/end in milliseconds since the step's first enqueue (CUDA events
+ * on the cell's stream). */
+typedef struct {
+  int32_t kind, k, m, enqueue_index;
+  float   start_ms, end_ms;
+} gpipe_trace_event;
+
+/* Bytes of arena that gpipe_create needs for (spec, K, M, remat) and a mini-batch of n_seqs
+ * sequences (O(N + (L/K)(N/M)) activations with remat).  Host only, no CUDA. */
+int gpipe_plan_bytes(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs,
+                     size_t *bytes_out);
+
+/* gpipe_create(layer_spec, K, M, remat) of BASELINE.json.  1 <= K <= max(L,1); the first
+ * L mod K cells get one more layer; M >= 1; n_seqs % M == 0 ("M equal micro-batches",
+ * PAPER.md:67).  n_seqs fixes the mini-batch size the plan is built for.  Parameters start at
+ * zero (LayerNorm gains too): call gpipe_init_params or gpipe_set_param. */
+int gpipe_create(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs,
+                 const gpipe_env *env, gpipe_t **out);
+void gpipe_destroy(gpipe_t *g);
+
+/* N(0, std) for matrices and emb, from a counter-based generator on the device (Philox-4x32-10
+ * + Box-Muller); parity != 0 also draws biases / beta ~ N(0,std) and gamma = 1 + N(0,std)
+ * (reading A10), parity == 0 sets gamma = 1, beta = bias = 0.  bf16 mode: the master is the
+ * RNE-bf16-rounded draw (reading A12). */
+int gpipe_init_params(gpipe_t *g, uint64_t seed, float std, int parity);
+
+/* gpipe_step(tokens, labels) -> loss.  tokens, labels: HOST, int32 [n_seqs, seq_len] row-major,
+ * values in [0, V), read during the call only.  Runs the whole GPipe schedule (forward ticks,
+ * then backward ticks with replay), ADDS d(mean loss)/dw into the fp32 gradient buffers and
+ * writes the mini-batch mean loss to *loss_out (host).  Synchronous on return. */
+int gpipe_step(gpipe_t *g, const int32_t *tokens, const int32_t *labels, float *loss_out);
+
+/* Same with DEVICE-resident int32 ids (inputs already in HBM); loss still returned to host. */
+int gpipe_step_device(gpipe_t *g, const int32_t *tokens_dev, const int32_t *labels_dev,
+                      float *loss_out);
+
+/* w <- w - lr * g for every parameter, once per mini-batch, then g <- 0.
+ * bf16 mode updates the fp32 master and re-rounds the bf16 working copy. */
+int gpipe_apply_sgd(gpipe_t *g, float lr);
+int gpipe_zero_grads(gpipe_t *g);
+
+int gpipe_num_tensors(const gpipe_t *g);
+/* *name points into library-owned storage valid until gpipe_destroy. */
+int gpipe_tensor_info(const gpipe_t *g, int i, const char **name, int64_t *rows, int64_t *cols);
+/* host_out / host_in: HOST fp32 [rows*cols].  get_param returns the values the kernels use
+ * (bf16 mode: the bf16 working copy widened).  set_param in bf16 mode RNE-rounds into both the
+ * master and the working copy. */
+int gpipe_get_param(gpipe_t *g, int i, float *host_out);
+int gpipe_set_param(gpipe_t *g, int i, const float *host_in);
+int gpipe_get_grad(gpipe_t *g, int i, float *host_out);
+
+/* Peak-HBM tracker: bytes the engine holds at its high-water mark, total, by category
+ * (by_category[GPIPE_NUM_CATS], may be NULL) and by cell (by_cell[K], activations and scratch
+ * owned by that cell; may be NULL). */
+int gpipe_peak_bytes(const gpipe_t *g, size_t *total, size_t *by_category, size_t *by_cell);
+
+/* enable != 0: subsequent steps record one gpipe_trace_event per task.  With events_out != NULL
+ * copies up to *n_events events of the last step and sets *n_events to the number written;
+ * with events_out == NULL sets *n_events to the number available. */
+int gpipe_trace(gpipe_t *g, int enable, gpipe_trace_event *events_out, int64_t *n_events);
+
+/* Number of kernels the library launched since gpipe_create (for bench.py's gpu_launches). */
+int64_t gpipe_launch_count(const gpipe_t *g);
+
+/* Debug/verification taps for the per-kernel parity tests: copies a named device buffer of the
+ * LAST executed (cell k, micro-batch m) task to host as fp32.  Names: see DESIGN.md. */
+int gpipe_debug_read(gpipe_t *g, const char *what, int layer, float *host_out, int64_t max_elems,
+                     int64_t *n_elems);
+
+const char *gpipe_last_error(void);
+const char *gpipe_version(void);
+
+#if defined(__GNUC__)
+#pragma GCC visibility pop
+#endif
+#ifdef __cplusplus
+}
+#endif
+#endif /* GPIPE_H_ */

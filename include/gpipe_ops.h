@@ -1,0 +1,78 @@
+/* gpipe_ops.h - C ABI of the individual sm_100a kernels of the GPipe hot path, exported so that
+ * each one can be checked against the oracle's corresponding operator on identical inputs
+ * ("teacher-forced" per-kernel parity) and timed in isolation against its roofline.
+ * gpipe_step (gpipe.h) is built from exactly these launchers.
+ *
+ * All data pointers are DEVICE pointers; `stream` is a cudaStream_t (0 = default stream).
+ * `dtype` is GPIPE_DTYPE_FP32 or GPIPE_DTYPE_BF16 and selects the storage type of "lp" tensors
+ * (tensor-core operands: activations, activation gradients, weight matrices); residual stream,
+ * statistics, biases/gains, losses and parameter gradients are always fp32.  Calls are
+ * asynchronous on `stream`; status 0 / negative as in gpipe.h (message via gpipe_last_error).
+ * Layer math per BASELINE.json north_star and DESIGN.md readings A2-A8 (the paper cites [15]
+ * for the layer).
+ */
+#ifndef GPIPE_OPS_H_
+#define GPIPE_OPS_H_
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+#if defined(__GNUC__)
+#pragma GCC visibility push(default)   /* the library is built with -fvisibility=hidden */
+#endif
+
+/* epilogue flags of gpipe_op_gemm */
+#define GPIPE_EPI_BIAS    1   /* + bias[n]            (fp32 [N])                                  */
+#define GPIPE_EPI_RELU    2   /* max(v, 0)                                                        */
+#define GPIPE_EPI_MASK    4   /* v * [mask[m,n] > 0]  (lp [M, ldmask]; ReLU backward)             */
+#define GPIPE_EPI_RESID   8   /* + resid[m,n]         (fp32 [M, ldc], may alias C)                */
+#define GPIPE_EPI_ACCUM  16   /* C (fp32) += v        (wgrad accumulation across micro-batches)   */
+#define GPIPE_EPI_OUT_F32 32  /* C is fp32, else lp                                               */
+
+/* C[M,N] = epilogue(op(A)[M,K] op(B)[K,N]), fp32 accumulation.  transA = 0: A stored [M,K]
+ * row-major, 1: stored [K,M]; transB = 0: B stored [K,N], 1: stored [N,K].  backend: 0 = auto
+ * (tcgen05 tensor cores for bf16 when the shape is tile-aligned), 1 = fp32-FMA SIMT kernel,
+ * 2 = tcgen05 or fail with GPIPE_EINVAL. */
+int gpipe_op_gemm(void *stream, int dtype, int M, int N, int K, const void *A, int64_t lda, int transA,
+                  const void *B, int64_t ldb, int transB, void *C, int64_t ldc, const float *bias,
+                  const float *resid, const void *mask, int64_t ldmask, int flags, int backend);
+
+/* y = LayerNorm(x) * gamma + beta over the last axis (biased variance); y lp [n_tok,d]; x fp32. */
+int gpipe_op_ln_fwd(void *stream, int dtype, const float *x, const float *gamma, const float *beta,
+                    void *y, float *mean, float *rstd, int64_t n_tok, int d, float eps);
+/* dx_out = (dres_in ? dres_in : 0) + LN'(dy); dx_out_lp optional lp copy; dgamma/dbeta += .
+ * partials: fp32 scratch of gpipe_op_ln_bwd_scratch_floats(d) floats. */
+int64_t gpipe_op_ln_bwd_scratch_floats(int d);
+int gpipe_op_ln_bwd(void *stream, int dtype, const void *dy, const float *x, const float *mean,
+                    const float *rstd, const float *gamma, const float *dres_in, float *dx_out,
+                    void *dx_out_lp, float *partials, float *dgamma, float *dbeta, int64_t n_tok, int d);
+
+/* qkv lp [n_seq*S, 3*A*dh] (q|k|v blocks); o lp [n_seq*S, A*dh]; lse fp32 [n_seq, A, S].
+ * backend: 0 = auto, 1 = SIMT. */
+int gpipe_op_attn_fwd(void *stream, int dtype, const void *qkv, void *o, float *lse, int n_seq, int S,
+                      int A, int dh, int causal, int backend);
+int gpipe_op_attn_bwd(void *stream, int dtype, const void *qkv, const void *o, const void *d_o,
+                      const float *lse, void *dqkv, float *dvec, int n_seq, int S, int A, int dh,
+                      int causal, int backend);
+
+/* in place logits -> dlogits = (softmax - onehot) * inv_T; rowloss[t] = CE_t * inv_T */
+int gpipe_op_softmax_ce(void *stream, int dtype, void *logits, const int32_t *labels, float *rowloss,
+                        int64_t n_tok, int V, float inv_T);
+/* out[n] += sum_t dy[t,n] */
+int gpipe_op_colsum(void *stream, int dtype, const void *dy, int64_t ld, float *out, int64_t n_tok, int n);
+/* x[t,:] = emb[tok[t],:] + pe[t mod S,:];  gemb[tok[t],:] += dx[t,:] */
+int gpipe_op_embed_fwd(void *stream, int dtype, const int32_t *tok, const void *emb, const float *pe,
+                       float *x, int64_t n_tok, int S, int d);
+int gpipe_op_embed_bwd(void *stream, const int32_t *tok, const float *dx, float *gemb, int64_t n_tok, int d);
+int gpipe_op_positional(void *stream, float *pe, int S, int d);
+/* master -= lr*grad; w_lp = RNE(master) (bf16 mode, may be NULL); grad = 0.  n multiple of 4. */
+int gpipe_op_sgd(void *stream, int dtype, float *master, float *grad, void *w_lp, int64_t n, float lr);
+
+#if defined(__GNUC__)
+#pragma GCC visibility pop
+#endif
+#ifdef __cplusplus
+}
+#endif
+#endif

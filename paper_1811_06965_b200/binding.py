@@ -1,0 +1,289 @@
+"""ctypes binding of libgpipe_b200.so (include/gpipe.h, include/gpipe_ops.h).
+
+Argument marshalling only: every step of the path runs in the library's CUDA kernels.  PyTorch
+supplies device memory (one uint8 arena tensor) and the K CUDA streams; there is no CPU fallback -
+if the shared library is missing or no B200 is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, List, Optional, Sequence, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgpipe_b200.so")
+
+DTYPE_FP32, DTYPE_BF16 = 0, 1
+CATEGORIES = ["weights", "masters", "grads", "boundary", "interior", "head", "misc", "bwd_scratch"]
+EPI_BIAS, EPI_RELU, EPI_MASK, EPI_RESID, EPI_ACCUM, EPI_OUT_F32 = 1, 2, 4, 8, 16, 32
+
+
+class GPipeError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__("gpipe error %d: %s" % (code, msg))
+        self.code = code
+
+
+class LayerSpec(C.Structure):
+    _fields_ = [("n_layers", C.c_int32), ("d_model", C.c_int32), ("d_ffn", C.c_int32),
+                ("n_heads", C.c_int32), ("d_head", C.c_int32), ("vocab", C.c_int32),
+                ("seq_len", C.c_int32), ("dtype", C.c_int32), ("causal", C.POINTER(C.c_uint8)),
+                ("ln_eps", C.c_float)]
+
+
+class Env(C.Structure):
+    _fields_ = [("arena", C.c_void_p), ("arena_bytes", C.c_size_t),
+                ("streams", C.POINTER(C.c_void_p)), ("n_streams", C.c_int32)]
+
+
+class TraceEvent(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("k", C.c_int32), ("m", C.c_int32), ("enqueue_index", C.c_int32),
+                ("start_ms", C.c_float), ("end_ms", C.c_float)]
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Loads the shared library (once).  Fails loudly when it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("%s is missing: run `python -m paper_1811_06965_b200.build` "
+                          "(there is no CPU fallback)" % LIB_PATH)
+    L = C.CDLL(LIB_PATH)
+    vp, i32, i64, f32 = C.c_void_p, C.c_int, C.c_int64, C.c_float
+    sig = {
+        "gpipe_plan_bytes": (i32, [C.POINTER(LayerSpec), i32, i32, i32, i64, C.POINTER(C.c_size_t)]),
+        "gpipe_create": (i32, [C.POINTER(LayerSpec), i32, i32, i32, i64, C.POINTER(Env), C.POINTER(vp)]),
+        "gpipe_destroy": (None, [vp]),
+        "gpipe_init_params": (i32, [vp, C.c_uint64, f32, i32]),
+        "gpipe_step": (i32, [vp, vp, vp, C.POINTER(f32)]),
+        "gpipe_step_device": (i32, [vp, vp, vp, C.POINTER(f32)]),
+        "gpipe_apply_sgd": (i32, [vp, f32]),
+        "gpipe_zero_grads": (i32, [vp]),
+        "gpipe_num_tensors": (i32, [vp]),
+        "gpipe_tensor_info": (i32, [vp, i32, C.POINTER(C.c_char_p), C.POINTER(i64), C.POINTER(i64)]),
+        "gpipe_get_param": (i32, [vp, i32, vp]),
+        "gpipe_set_param": (i32, [vp, i32, vp]),
+        "gpipe_get_grad": (i32, [vp, i32, vp]),
+        "gpipe_peak_bytes": (i32, [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]),
+        "gpipe_trace": (i32, [vp, i32, C.POINTER(TraceEvent), C.POINTER(i64)]),
+        "gpipe_launch_count": (i64, [vp]),
+        "gpipe_debug_read": (i32, [vp, C.c_char_p, i32, vp, i64, C.POINTER(i64)]),
+        "gpipe_last_error": (C.c_char_p, []),
+        "gpipe_version": (C.c_char_p, []),
+        "gpipe_op_gemm": (i32, [vp, i32, i32, i32, i32, vp, i64, i32, vp, i64, i32, vp, i64, vp, vp, vp, i64, i32, i32]),
+        "gpipe_op_ln_fwd": (i32, [vp, i32, vp, vp, vp, vp, vp, vp, i64, i32, f32]),
+        "gpipe_op_ln_bwd_scratch_floats": (i64, [i32]),
+        "gpipe_op_ln_bwd": (i32, [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, i32]),
+        "gpipe_op_attn_fwd": (i32, [vp, i32, vp, vp, vp, i32, i32, i32, i32, i32, i32]),
+        "gpipe_op_attn_bwd": (i32, [vp, i32, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32]),
+        "gpipe_op_softmax_ce": (i32, [vp, i32, vp, vp, vp, i64, i32, f32]),
+        "gpipe_op_colsum": (i32, [vp, i32, vp, i64, vp, i64, i32]),
+        "gpipe_op_embed_fwd": (i32, [vp, i32, vp, vp, vp, vp, i64, i32, i32]),
+        "gpipe_op_embed_bwd": (i32, [vp, vp, vp, vp, i64, i32]),
+        "gpipe_op_positional": (i32, [vp, vp, i32, i32]),
+        "gpipe_op_sgd": (i32, [vp, i32, vp, vp, vp, i64, f32]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = L
+    return L
+
+
+EXPORTED_SYMBOLS = [
+    "gpipe_plan_bytes", "gpipe_create", "gpipe_destroy", "gpipe_init_params", "gpipe_step",
+    "gpipe_step_device", "gpipe_apply_sgd", "gpipe_zero_grads", "gpipe_num_tensors",
+    "gpipe_tensor_info", "gpipe_get_param", "gpipe_set_param", "gpipe_get_grad", "gpipe_peak_bytes",
+    "gpipe_trace", "gpipe_launch_count", "gpipe_debug_read", "gpipe_last_error", "gpipe_version",
+    "gpipe_op_gemm", "gpipe_op_ln_fwd", "gpipe_op_ln_bwd_scratch_floats", "gpipe_op_ln_bwd",
+    "gpipe_op_attn_fwd", "gpipe_op_attn_bwd", "gpipe_op_softmax_ce", "gpipe_op_colsum",
+    "gpipe_op_embed_fwd", "gpipe_op_embed_bwd", "gpipe_op_positional", "gpipe_op_sgd",
+]
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise GPipeError(rc, lib().gpipe_last_error().decode("utf-8", "replace"))
+
+
+def make_spec(n_layers, d_model, d_ffn, n_heads, d_head, vocab, seq_len, dtype, causal=None,
+              ln_eps=1e-5) -> Tuple[LayerSpec, object]:
+    """Returns (spec, keepalive) - keepalive owns the causal array the spec points to."""
+    dt = {"fp32": DTYPE_FP32, "bf16": DTYPE_BF16, 0: 0, 1: 1}[dtype]
+    keep = None
+    ptr = C.POINTER(C.c_uint8)()
+    if causal is not None:
+        if len(causal) != n_layers:
+            raise ValueError("causal must have n_layers entries")
+        keep = (C.c_uint8 * max(n_layers, 1))(*[1 if c else 0 for c in causal])
+        ptr = C.cast(keep, C.POINTER(C.c_uint8))
+    return LayerSpec(n_layers, d_model, d_ffn, n_heads, d_head, vocab, seq_len, dt, ptr, ln_eps), keep
+
+
+def plan_bytes(spec: LayerSpec, K: int, M: int, remat: bool, n_seqs: int) -> int:
+    """gpipe_plan_bytes: host-only, works without a GPU."""
+    out = C.c_size_t(0)
+    _check(lib().gpipe_plan_bytes(C.byref(spec), K, M, int(bool(remat)), n_seqs, C.byref(out)))
+    return int(out.value)
+
+
+class GPipe:
+    """gpipe_create / gpipe_step / gpipe_apply_sgd (BASELINE.json north_star) on one B200."""
+
+    def __init__(self, *, n_layers, d_model, d_ffn, n_heads, d_head, vocab, seq_len, dtype, K, M,
+                 remat=True, n_seqs, causal=None, ln_eps=1e-5, device="cuda:0"):
+        import torch
+        if not torch.cuda.is_available():
+            raise GPipeError(-2, "no CUDA device: the GPipe path has no CPU fallback")
+        self._torch = torch
+        self.device = torch.device(device)
+        self.spec, self._keep = make_spec(n_layers, d_model, d_ffn, n_heads, d_head, vocab, seq_len,
+                                          dtype, causal, ln_eps)
+        self.K, self.M, self.remat, self.n_seqs, self.seq_len = K, M, bool(remat), n_seqs, seq_len
+        self._h = C.c_void_p(None)
+        with torch.cuda.device(self.device):
+            nbytes = plan_bytes(self.spec, K, M, remat, n_seqs)
+            self.arena = torch.empty(nbytes + 1024, dtype=torch.uint8, device=self.device)
+            base = (self.arena.data_ptr() + 1023) // 1024 * 1024
+            self.streams = [torch.cuda.Stream(device=self.device) for _ in range(K)]
+            self._stream_arr = (C.c_void_p * K)(*[s.cuda_stream for s in self.streams])
+            env = Env(base, nbytes, C.cast(self._stream_arr, C.POINTER(C.c_void_p)), K)
+            torch.cuda.synchronize(self.device)
+            _check(lib().gpipe_create(C.byref(self.spec), K, M, int(self.remat), n_seqs, C.byref(env),
+                                      C.byref(self._h)))
+        self.names: List[str] = []
+        self.shapes: Dict[str, Tuple[int, int]] = {}
+        for i in range(lib().gpipe_num_tensors(self._h)):
+            nm, r, c = C.c_char_p(), C.c_int64(), C.c_int64()
+            _check(lib().gpipe_tensor_info(self._h, i, C.byref(nm), C.byref(r), C.byref(c)))
+            self.names.append(nm.value.decode())
+            self.shapes[self.names[-1]] = (r.value, c.value)
+        self._index = {n: i for i, n in enumerate(self.names)}
+
+    # -- life cycle ---------------------------------------------------------------------------
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().gpipe_destroy(self._h)
+            self._h = C.c_void_p(None)
+        self.arena = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    # -- the three calls ------------------------------------------------------------------------
+    def init_params(self, seed: int, std: float = 0.02, parity: bool = False):
+        with self._torch.cuda.device(self.device):
+            _check(lib().gpipe_init_params(self._h, seed, std, int(parity)))
+
+    def step(self, tokens, labels) -> float:
+        """tokens/labels: numpy int32 [N,S] or CPU torch tensors (host path, gpipe_step), or CUDA
+        int32 tensors (inputs resident in HBM, gpipe_step_device).  Returns the mean loss."""
+        torch = self._torch
+        loss = C.c_float(0)
+        with torch.cuda.device(self.device):
+            if isinstance(tokens, torch.Tensor) and tokens.is_cuda:
+                if tokens.dtype != torch.int32 or labels.dtype != torch.int32:
+                    raise ValueError("device ids must be int32")
+                t, l = tokens.contiguous(), labels.contiguous()
+                if t.numel() != self.n_seqs * self.seq_len or l.numel() != t.numel():
+                    raise ValueError("tokens/labels must be [n_seqs, seq_len]")
+                torch.cuda.current_stream(self.device).synchronize()
+                _check(lib().gpipe_step_device(self._h, t.data_ptr(), l.data_ptr(), C.byref(loss)))
+            else:
+                t = np.ascontiguousarray(tokens.numpy() if isinstance(tokens, torch.Tensor) else tokens, dtype=np.int32)
+                l = np.ascontiguousarray(labels.numpy() if isinstance(labels, torch.Tensor) else labels, dtype=np.int32)
+                if t.size != self.n_seqs * self.seq_len or l.size != t.size:
+                    raise ValueError("tokens/labels must be [n_seqs, seq_len]")
+                _check(lib().gpipe_step(self._h, t.ctypes.data, l.ctypes.data, C.byref(loss)))
+        return float(loss.value)
+
+    def apply_sgd(self, lr: float):
+        with self._torch.cuda.device(self.device):
+            _check(lib().gpipe_apply_sgd(self._h, lr))
+
+    def zero_grads(self):
+        with self._torch.cuda.device(self.device):
+            _check(lib().gpipe_zero_grads(self._h))
+
+    # -- parameters -----------------------------------------------------------------------------
+    def _idx(self, key) -> int:
+        return key if isinstance(key, int) else self._index[key]
+
+    def _get(self, fn, key) -> np.ndarray:
+        i = self._idx(key)
+        out = np.empty(self.shapes[self.names[i]], np.float32)
+        with self._torch.cuda.device(self.device):
+            _check(fn(self._h, i, out.ctypes.data))
+        return out
+
+    def get_param(self, key) -> np.ndarray:
+        return self._get(lib().gpipe_get_param, key)
+
+    def get_grad(self, key) -> np.ndarray:
+        return self._get(lib().gpipe_get_grad, key)
+
+    def set_param(self, key, value):
+        i = self._idx(key)
+        a = np.ascontiguousarray(value, dtype=np.float32)
+        if a.size != self.shapes[self.names[i]][0] * self.shapes[self.names[i]][1]:
+            raise ValueError("wrong size for %s" % self.names[i])
+        with self._torch.cuda.device(self.device):
+            _check(lib().gpipe_set_param(self._h, i, a.ctypes.data))
+
+    def set_params(self, params: Dict[str, np.ndarray]):
+        for n in self.names:
+            self.set_param(n, params[n])
+
+    def grads(self) -> Dict[str, np.ndarray]:
+        return {n: self.get_grad(n) for n in self.names}
+
+    # -- tracker / trace --------------------------------------------------------------------------
+    def peak_bytes(self) -> Dict[str, object]:
+        total = C.c_size_t(0)
+        cats = (C.c_size_t * len(CATEGORIES))()
+        cells = (C.c_size_t * self.K)()
+        _check(lib().gpipe_peak_bytes(self._h, C.byref(total), cats, cells))
+        return {"total": int(total.value), "by_category": {c: int(cats[i]) for i, c in enumerate(CATEGORIES)},
+                "by_cell": [int(cells[k]) for k in range(self.K)]}
+
+    def trace(self, enable: bool):
+        _check(lib().gpipe_trace(self._h, int(enable), None, None))
+
+    def trace_events(self) -> List[Tuple[str, int, int, int, float, float]]:
+        n = C.c_int64(0)
+        _check(lib().gpipe_trace(self._h, 1, None, C.byref(n)))
+        buf = (TraceEvent * max(n.value, 1))()
+        _check(lib().gpipe_trace(self._h, 1, buf, C.byref(n)))
+        return [(chr(e.kind), e.k, e.m, e.enqueue_index, e.start_ms, e.end_ms) for e in buf[:n.value]]
+
+    def launch_count(self) -> int:
+        return int(lib().gpipe_launch_count(self._h))
+
+    def debug_read(self, what: str, layer: int = -1, max_elems: Optional[int] = None) -> np.ndarray:
+        if max_elems is None:
+            T_mb = self.n_seqs // self.M * self.seq_len
+            s = self.spec
+            da = s.n_heads * (s.d_head or s.d_model // s.n_heads)
+            max_elems = T_mb * max(s.vocab, s.d_ffn, 3 * da, s.d_model)
+        out = np.empty(max_elems, np.float32)
+        n = C.c_int64(0)
+        with self._torch.cuda.device(self.device):
+            self._torch.cuda.synchronize(self.device)
+            _check(lib().gpipe_debug_read(self._h, what.encode(), layer, out.ctypes.data, max_elems, C.byref(n)))
+        return out[:n.value].copy()

@@ -1,0 +1,382 @@
+// api.cu - the C ABI of include/gpipe.h: argument validation, handle life cycle, parameter
+// access, tracker and trace read-out.  Never throws, never aborts across the boundary.
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <string>
+
+#include "engine.h"
+
+using namespace gp;
+
+static thread_local std::string g_err;
+
+struct gpipe {
+  Engine e;
+};
+
+void gpipe_set_error_(const std::string &s) { g_err = s; }
+
+static int fail(int code, const std::string &msg) {
+  g_err = msg;
+  return code;
+}
+static int cuda_fail(cudaError_t e, const char *where) {
+  g_err = std::string(where) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")";
+  return GPIPE_ECUDA;
+}
+#define API_CUDA(x, where)                            \
+  do {                                                \
+    cudaError_t e__ = (x);                            \
+    if (e__ != cudaSuccess) return cuda_fail(e__, where); \
+  } while (0)
+
+static int env_int(const char *name, int dflt) {
+  const char *v = getenv(name);
+  return v && *v ? atoi(v) : dflt;
+}
+
+// fills the shape fields of an Engine from the spec; no CUDA calls
+static int configure(Engine &e, const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs) {
+  if (!spec) return fail(GPIPE_EINVAL, "spec is NULL");
+  e.spec = *spec;
+  e.dt = spec->dtype;
+  if (e.dt != GPIPE_DTYPE_FP32 && e.dt != GPIPE_DTYPE_BF16) return fail(GPIPE_EINVAL, "dtype must be 0 (fp32) or 1 (bf16)");
+  e.d = spec->d_model; e.H = spec->d_ffn; e.A = spec->n_heads; e.V = spec->vocab; e.S = spec->seq_len;
+  if (spec->n_layers < 0 || e.d <= 0 || e.H <= 0 || e.A <= 0 || e.V <= 0 || e.S <= 0)
+    return fail(GPIPE_EINVAL, "n_layers >= 0 and d_model, d_ffn, n_heads, vocab, seq_len > 0 required");
+  e.dh = spec->d_head ? spec->d_head : e.d / e.A;
+  if (e.dh != 16 && e.dh != 32 && e.dh != 64 && e.dh != 128) return fail(GPIPE_EINVAL, "d_head must be 16, 32, 64 or 128");
+  e.da = e.A * e.dh;
+  if (e.d % 4 || e.H % 4 || e.V % 4 || e.d > 2048) return fail(GPIPE_EINVAL, "d_model, d_ffn, vocab must be multiples of 4 and d_model <= 2048");
+  if (e.dt == GPIPE_DTYPE_BF16 && (e.d % 8 || e.H % 8 || e.V % 8)) return fail(GPIPE_EINVAL, "bf16 mode needs d_model, d_ffn, vocab multiples of 8");
+  e.eps = spec->ln_eps > 0.f ? spec->ln_eps : 1e-5f;
+  int L = spec->n_layers;
+  if (K < 1 || K > (L > 1 ? L : 1)) return fail(GPIPE_EINVAL, "need 1 <= K <= max(L, 1)");
+  if (M < 1) return fail(GPIPE_EINVAL, "need M >= 1");
+  if (n_seqs < 1 || n_seqs % M) return fail(GPIPE_EINVAL, "n_seqs must split into M equal micro-batches (PAPER.md:67)");
+  e.K = K; e.M = M; e.remat = remat ? 1 : 0;
+  e.n_seqs = n_seqs; e.nb = n_seqs / M; e.T_mb = e.nb * e.S; e.T_total = n_seqs * e.S;
+  if (e.T_mb * (int64_t)(e.V > 3 * e.da ? e.V : 3 * e.da) >= ((int64_t)1 << 40)) return fail(GPIPE_EINVAL, "micro-batch too large");
+  e.causal.assign(L, 1);
+  if (spec->causal) for (int l = 0; l < L; ++l) e.causal[l] = spec->causal[l] ? 1 : 0;
+  e.cell_lo.resize(K); e.cell_hi.resize(K);
+  int base = L / K, extra = L % K;          // first L mod K cells get one more layer
+  for (int k = 0; k < K; ++k) {
+    e.cell_lo[k] = k * base + (k < extra ? k : extra);
+    e.cell_hi[k] = e.cell_lo[k] + base + (k < extra ? 1 : 0);
+  }
+  e.gemm_backend = env_int("GPIPE_GEMM_SIMT", 0);
+  e.replay_full = env_int("GPIPE_REPLAY_FULL", 0);
+  std::string err;
+  e.build_inventory(err);
+  return GPIPE_OK;
+}
+
+extern "C" {
+
+const char *gpipe_last_error(void) { return g_err.c_str(); }
+const char *gpipe_version(void) { return "gpipe-b200 0.1 (sm_100a)"; }
+
+int gpipe_plan_bytes(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs, size_t *bytes_out) {
+  if (!bytes_out) return fail(GPIPE_EINVAL, "bytes_out is NULL");
+  Engine e;
+  int rc = configure(e, spec, K, M, remat, n_seqs);
+  if (rc) return rc;
+  std::string err;
+  rc = e.build_plan(true, err);
+  if (rc) return fail(rc, err);
+  *bytes_out = e.arena.used;
+  return GPIPE_OK;
+}
+
+int gpipe_create(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs, const gpipe_env *env, gpipe_t **out) {
+  if (!out) return fail(GPIPE_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (!env || !env->arena || !env->streams) return fail(GPIPE_EINVAL, "env, env->arena and env->streams are required");
+  gpipe *g = new (std::nothrow) gpipe();
+  if (!g) return fail(GPIPE_ENOMEM, "host allocation failed");
+  Engine &e = g->e;
+  int rc = configure(e, spec, K, M, remat, n_seqs);
+  if (rc) { delete g; return rc; }
+  if (env->n_streams < K) { delete g; return fail(GPIPE_EINVAL, "need one stream per cell (n_streams >= K)"); }
+  if ((uintptr_t)env->arena % 1024) { delete g; return fail(GPIPE_EINVAL, "arena must be 1024-byte aligned"); }
+  int dev = 0;
+  cudaError_t ce = cudaGetDevice(&dev);
+  if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&e.sm_count, cudaDevAttrMultiProcessorCount, dev);
+  int cc_major = 0;
+  if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev);
+  if (ce != cudaSuccess) { delete g; return cuda_fail(ce, "gpipe_create: no usable CUDA device"); }
+  if (cc_major != 10) { delete g; return fail(GPIPE_ECUDA, "gpipe_create: this library is built for sm_100a (B200) only"); }
+  std::string err;
+  e.arena.base = (char *)env->arena;
+  e.arena.cap = env->arena_bytes;
+  rc = e.build_plan(true, err);
+  if (rc == GPIPE_OK && e.arena.used > e.arena.cap)
+    rc = fail(GPIPE_ENOMEM, "arena too small: need " + std::to_string(e.arena.used) + " bytes, have " + std::to_string(e.arena.cap));
+  if (rc == GPIPE_OK) { rc = e.build_plan(false, err); if (rc) fail(rc, err); }
+  if (rc) { delete g; return rc; }
+  e.streams.resize(K);
+  for (int k = 0; k < K; ++k) e.streams[k] = (cudaStream_t)env->streams[k];
+  e.ev_f.assign(K, std::vector<cudaEvent_t>(e.M, nullptr));
+  e.ev_b.assign(K, std::vector<cudaEvent_t>(e.M, nullptr));
+  e.ev_done.assign(K, nullptr);
+  for (int k = 0; k < K && ce == cudaSuccess; ++k) {
+    for (int m = 0; m < e.M && ce == cudaSuccess; ++m) {
+      ce = cudaEventCreateWithFlags(&e.ev_f[k][m], cudaEventDisableTiming);
+      if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&e.ev_b[k][m], cudaEventDisableTiming);
+    }
+    if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&e.ev_done[k], cudaEventDisableTiming);
+  }
+  if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&e.ev_in, cudaEventDisableTiming);
+  if (ce == cudaSuccess) ce = cudaEventCreate(&e.ev_t0);
+  if (ce == cudaSuccess) ce = cudaMallocHost((void **)&e.host_loss, sizeof(float) * (e.M + 1));
+  if (ce == cudaSuccess) ce = cudaMallocHost((void **)&e.host_flag, sizeof(int));
+  Ctx c = e.ctx(0);
+  // parameters, gradients start at zero; positional table is built once
+  if (ce == cudaSuccess) ce = cudaMemsetAsync(e.master, 0, (size_t)e.n_flat * 4, c.stream);
+  if (ce == cudaSuccess) ce = cudaMemsetAsync(e.grad, 0, (size_t)e.n_flat * 4, c.stream);
+  if (ce == cudaSuccess && e.dt == GP_BF16) ce = cudaMemsetAsync(e.w_lp, 0, (size_t)e.n_flat * 2, c.stream);
+  if (ce == cudaSuccess) ce = cudaMemsetAsync(e.flag_dev, 0, 4, c.stream);
+  if (ce == cudaSuccess) ce = positional_table(c, e.pe, e.S, e.d);
+  if (ce == cudaSuccess) ce = cudaStreamSynchronize(c.stream);
+  if (ce != cudaSuccess) { gpipe_destroy(g); return cuda_fail(ce, "gpipe_create"); }
+  *out = g;
+  return GPIPE_OK;
+}
+
+void gpipe_destroy(gpipe_t *g) {
+  if (!g) return;
+  Engine &e = g->e;
+  for (auto s : e.streams) cudaStreamSynchronize(s);
+  for (auto &v : e.ev_f) for (auto ev : v) if (ev) cudaEventDestroy(ev);
+  for (auto &v : e.ev_b) for (auto ev : v) if (ev) cudaEventDestroy(ev);
+  for (auto ev : e.ev_done) if (ev) cudaEventDestroy(ev);
+  for (auto ev : e.ev_pool) cudaEventDestroy(ev);
+  if (e.ev_in) cudaEventDestroy(e.ev_in);
+  if (e.ev_t0) cudaEventDestroy(e.ev_t0);
+  if (e.host_loss) cudaFreeHost(e.host_loss);
+  if (e.host_flag) cudaFreeHost(e.host_flag);
+  delete g;
+}
+
+int gpipe_init_params(gpipe_t *g, uint64_t seed, float std, int parity) {
+  if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
+  Engine &e = g->e;
+  Ctx c = e.ctx(0);
+  for (size_t i = 0; i < e.tensors.size(); ++i) {
+    const TensorInfo &t = e.tensors[i];
+    int64_t n = ((t.rows * t.cols + 63) / 64) * 64;
+    float *m = e.master + t.off;
+    void *w = e.dt == GP_BF16 ? (void *)((char *)e.w_lp + t.off * 2) : nullptr;
+    bool gamma = !t.matrix && t.name.size() >= 2 && t.name.compare(t.name.size() - 2, 2, "_g") == 0;
+    cudaError_t ce;
+    if (t.matrix || parity) {
+      ce = init_normal(c, e.dt, m, w, n, seed, (uint64_t)i, gamma ? 1.f : 0.f, std);
+    } else {
+      ce = fill_f32(c, m, n, gamma ? 1.f : 0.f);
+      if (ce == cudaSuccess) ce = master_to_lp(c, e.dt, m, w, n, 0);
+    }
+    if (ce != cudaSuccess) return cuda_fail(ce, "gpipe_init_params");
+    // padding elements beyond rows*cols stay harmless: nothing reads them
+  }
+  API_CUDA(cudaStreamSynchronize(c.stream), "gpipe_init_params");
+  return GPIPE_OK;
+}
+
+static int step_common(Engine &e, float *loss_out) {
+  if (!loss_out) return fail(GPIPE_EINVAL, "loss_out is NULL");
+  cudaError_t ce = e.run_step(loss_out);
+  if (ce != cudaSuccess) {
+    for (auto s : e.streams) cudaStreamSynchronize(s);
+    return cuda_fail(ce, "gpipe_step");
+  }
+  return GPIPE_OK;
+}
+
+int gpipe_step(gpipe_t *g, const int32_t *tokens, const int32_t *labels, float *loss_out) {
+  if (!g || !tokens || !labels) return fail(GPIPE_EINVAL, "handle, tokens and labels are required");
+  Engine &e = g->e;
+  for (int64_t i = 0; i < e.T_total; ++i)
+    if (tokens[i] < 0 || tokens[i] >= e.V || labels[i] < 0 || labels[i] >= e.V)
+      return fail(GPIPE_EINVAL, "token/label outside [0, V) at flat index " + std::to_string(i));
+  API_CUDA(cudaMemcpyAsync(e.tok_dev, tokens, (size_t)e.T_total * 4, cudaMemcpyHostToDevice, e.streams[0]), "gpipe_step H2D");
+  API_CUDA(cudaMemcpyAsync(e.lab_dev, labels, (size_t)e.T_total * 4, cudaMemcpyHostToDevice, e.streams[0]), "gpipe_step H2D");
+  return step_common(e, loss_out);
+}
+
+int gpipe_step_device(gpipe_t *g, const int32_t *tokens_dev, const int32_t *labels_dev, float *loss_out) {
+  if (!g || !tokens_dev || !labels_dev) return fail(GPIPE_EINVAL, "handle, tokens and labels are required");
+  Engine &e = g->e;
+  Ctx c = e.ctx(0);
+  API_CUDA(cudaMemsetAsync(e.flag_dev, 0, 4, c.stream), "gpipe_step_device");
+  API_CUDA(check_ids(c, tokens_dev, e.T_total, e.V, e.flag_dev), "gpipe_step_device");
+  API_CUDA(check_ids(c, labels_dev, e.T_total, e.V, e.flag_dev), "gpipe_step_device");
+  API_CUDA(cudaMemcpyAsync(e.host_flag, e.flag_dev, 4, cudaMemcpyDeviceToHost, c.stream), "gpipe_step_device");
+  API_CUDA(cudaMemcpyAsync(e.tok_dev, tokens_dev, (size_t)e.T_total * 4, cudaMemcpyDeviceToDevice, c.stream), "gpipe_step_device");
+  API_CUDA(cudaMemcpyAsync(e.lab_dev, labels_dev, (size_t)e.T_total * 4, cudaMemcpyDeviceToDevice, c.stream), "gpipe_step_device");
+  API_CUDA(cudaStreamSynchronize(c.stream), "gpipe_step_device");
+  if (*e.host_flag) return fail(GPIPE_EINVAL, "token/label outside [0, V)");
+  return step_common(e, loss_out);
+}
+
+int gpipe_apply_sgd(gpipe_t *g, float lr) {
+  if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
+  Engine &e = g->e;
+  Ctx c = e.ctx(0);
+  API_CUDA(sgd_apply(c, e.dt, e.master, e.grad, e.dt == GP_BF16 ? e.w_lp : nullptr, e.n_flat, lr), "gpipe_apply_sgd");
+  API_CUDA(cudaStreamSynchronize(c.stream), "gpipe_apply_sgd");
+  return GPIPE_OK;
+}
+
+int gpipe_zero_grads(gpipe_t *g) {
+  if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
+  Engine &e = g->e;
+  API_CUDA(cudaMemsetAsync(e.grad, 0, (size_t)e.n_flat * 4, e.streams[0]), "gpipe_zero_grads");
+  API_CUDA(cudaStreamSynchronize(e.streams[0]), "gpipe_zero_grads");
+  return GPIPE_OK;
+}
+
+int gpipe_num_tensors(const gpipe_t *g) { return g ? (int)g->e.tensors.size() : fail(GPIPE_EINVAL, "handle is NULL"); }
+
+int gpipe_tensor_info(const gpipe_t *g, int i, const char **name, int64_t *rows, int64_t *cols) {
+  if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
+  if (i < 0 || i >= (int)g->e.tensors.size()) return fail(GPIPE_EINVAL, "tensor index out of range");
+  const TensorInfo &t = g->e.tensors[i];
+  if (name) *name = t.name.c_str();
+  if (rows) *rows = t.rows;
+  if (cols) *cols = t.cols;
+  return GPIPE_OK;
+}
+
+static int tensor_check(gpipe_t *g, int i, const void *p) {
+  if (!g || !p) return fail(GPIPE_EINVAL, "handle and host pointer are required");
+  if (i < 0 || i >= (int)g->e.tensors.size()) return fail(GPIPE_EINVAL, "tensor index out of range");
+  return GPIPE_OK;
+}
+
+int gpipe_get_param(gpipe_t *g, int i, float *host_out) {
+  int rc = tensor_check(g, i, host_out);
+  if (rc) return rc;
+  Engine &e = g->e;
+  const TensorInfo &t = e.tensors[i];
+  int64_t n = t.rows * t.cols;
+  Ctx c = e.ctx(0);
+  if (e.dt == GP_BF16 && t.matrix) {
+    // widen the bf16 working copy through the gradient-free scratch of cell 0 (dh is the largest)
+    // -> simpler and always big enough: convert in chunks through ln_partials? use a temp on host:
+    std::string tmp((size_t)n * 2, '\0');
+    API_CUDA(cudaMemcpyAsync(&tmp[0], (const char *)e.w_lp + t.off * 2, (size_t)n * 2, cudaMemcpyDeviceToHost, c.stream), "gpipe_get_param");
+    API_CUDA(cudaStreamSynchronize(c.stream), "gpipe_get_param");
+    const uint16_t *u = (const uint16_t *)tmp.data();
+    for (int64_t j = 0; j < n; ++j) {
+      uint32_t w = (uint32_t)u[j] << 16;
+      memcpy(host_out + j, &w, 4);
+    }
+    return GPIPE_OK;
+  }
+  API_CUDA(cudaMemcpyAsync(host_out, e.master + t.off, (size_t)n * 4, cudaMemcpyDeviceToHost, c.stream), "gpipe_get_param");
+  API_CUDA(cudaStreamSynchronize(c.stream), "gpipe_get_param");
+  return GPIPE_OK;
+}
+
+int gpipe_set_param(gpipe_t *g, int i, const float *host_in) {
+  int rc = tensor_check(g, i, host_in);
+  if (rc) return rc;
+  Engine &e = g->e;
+  const TensorInfo &t = e.tensors[i];
+  int64_t n = t.rows * t.cols;
+  Ctx c = e.ctx(0);
+  API_CUDA(cudaMemcpyAsync(e.master + t.off, host_in, (size_t)n * 4, cudaMemcpyHostToDevice, c.stream), "gpipe_set_param");
+  if (e.dt == GP_BF16)   // RNE-round into the working copy; matrices also round the master (A12)
+    API_CUDA(master_to_lp(c, e.dt, e.master + t.off, (char *)e.w_lp + t.off * 2, n, t.matrix ? 1 : 0), "gpipe_set_param");
+  API_CUDA(cudaStreamSynchronize(c.stream), "gpipe_set_param");
+  return GPIPE_OK;
+}
+
+int gpipe_get_grad(gpipe_t *g, int i, float *host_out) {
+  int rc = tensor_check(g, i, host_out);
+  if (rc) return rc;
+  Engine &e = g->e;
+  const TensorInfo &t = e.tensors[i];
+  API_CUDA(cudaMemcpyAsync(host_out, e.grad + t.off, (size_t)(t.rows * t.cols) * 4, cudaMemcpyDeviceToHost, e.streams[0]), "gpipe_get_grad");
+  API_CUDA(cudaStreamSynchronize(e.streams[0]), "gpipe_get_grad");
+  return GPIPE_OK;
+}
+
+int gpipe_peak_bytes(const gpipe_t *g, size_t *total, size_t *by_category, size_t *by_cell) {
+  if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
+  const Engine &e = g->e;
+  if (total) *total = e.arena.used;
+  if (by_category) for (int i = 0; i < GPIPE_NUM_CATS; ++i) by_category[i] = e.arena.by_cat[i];
+  if (by_cell) for (int k = 0; k < e.K; ++k) by_cell[k] = e.arena.by_cell[k];
+  return GPIPE_OK;
+}
+
+int gpipe_trace(gpipe_t *g, int enable, gpipe_trace_event *events_out, int64_t *n_events) {
+  if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
+  Engine &e = g->e;
+  e.trace_on = enable ? 1 : 0;
+  if (!n_events) return GPIPE_OK;
+  if (!events_out) { *n_events = (int64_t)e.trace.size(); return GPIPE_OK; }
+  int64_t n = *n_events < (int64_t)e.trace.size() ? *n_events : (int64_t)e.trace.size();
+  for (int64_t i = 0; i < n; ++i) {
+    const TraceRec &r = e.trace[i];
+    gpipe_trace_event &o = events_out[i];
+    o.kind = r.kind; o.k = r.k; o.m = r.m; o.enqueue_index = r.idx;
+    API_CUDA(cudaEventElapsedTime(&o.start_ms, e.ev_t0, r.e0), "gpipe_trace");
+    API_CUDA(cudaEventElapsedTime(&o.end_ms, e.ev_t0, r.e1), "gpipe_trace");
+  }
+  *n_events = n;
+  return GPIPE_OK;
+}
+
+int64_t gpipe_launch_count(const gpipe_t *g) { return g ? g->e.launches : 0; }
+
+int gpipe_debug_read(gpipe_t *g, const char *what, int layer, float *host_out, int64_t max_elems, int64_t *n_elems) {
+  if (!g || !what || !host_out || !n_elems) return fail(GPIPE_EINVAL, "arguments are required");
+  Engine &e = g->e;
+  std::string w(what);
+  const void *src = nullptr;
+  int64_t n = 0;
+  bool is_lp = true;
+  int k = e.K - 1, li = 0;
+  if (layer >= 0) {
+    if (layer >= e.spec.n_layers) return fail(GPIPE_EINVAL, "layer out of range");
+    for (k = 0; k < e.K; ++k) if (layer >= e.cell_lo[k] && layer < e.cell_hi[k]) break;
+    li = layer - e.cell_lo[k];
+  }
+  Workspace &ws = e.wsp(k, 0);
+  int64_t T = e.T_mb;
+  if (layer >= 0) {
+    LayerBuf &b = ws.layers[li];
+    if (w == "a") { src = b.a; n = T * e.d; }
+    else if (w == "qkv") { src = b.qkv; n = T * 3 * e.da; }
+    else if (w == "o") { src = b.o; n = T * e.da; }
+    else if (w == "c") { src = b.c; n = T * e.d; }
+    else if (w == "h") { src = b.h; n = T * e.H; }
+    else if (w == "x1") { src = b.x1; n = T * e.d; is_lp = false; }
+    else if (w == "lse") { src = b.lse; n = T * e.A; is_lp = false; }
+  } else {
+    if (w == "y") { src = ws.y; n = T * e.d; }
+    else if (w == "dlogits") { src = ws.logits; n = T * e.V; }
+    else if (w == "x_out") { src = ws.x_out; n = T * e.d; is_lp = false; }
+  }
+  if (!src) return fail(GPIPE_EINVAL, "unknown debug buffer '" + w + "'");
+  if (n > max_elems) return fail(GPIPE_EINVAL, "host buffer too small: need " + std::to_string(n));
+  Ctx c = e.ctx(0);
+  if (is_lp && e.dt == GP_BF16) {
+    std::string tmp((size_t)n * 2, '\0');
+    API_CUDA(cudaMemcpy(&tmp[0], src, (size_t)n * 2, cudaMemcpyDeviceToHost), "gpipe_debug_read");
+    const uint16_t *u = (const uint16_t *)tmp.data();
+    for (int64_t j = 0; j < n; ++j) { uint32_t x = (uint32_t)u[j] << 16; memcpy(host_out + j, &x, 4); }
+  } else {
+    API_CUDA(cudaMemcpy(host_out, src, (size_t)n * 4, cudaMemcpyDeviceToHost), "gpipe_debug_read");
+  }
+  (void)c;
+  *n_elems = n;
+  return GPIPE_OK;
+}
+
+}  // extern "C"

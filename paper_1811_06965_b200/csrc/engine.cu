@@ -1,0 +1,394 @@
+// engine.cu - parameter inventory, memory plan / peak-HBM tracker, cell executor and the GPipe
+// scheduler (PAPER.md:59-67 cells and micro-batches; :87 boundary-only storage + replay; :89 early
+// replay).  Host code only: every arithmetic step is a launcher from ops.h.
+#include "engine.h"
+
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+namespace gp {
+
+#define GP_TRY(x)                       \
+  do {                                  \
+    cudaError_t e__ = (x);              \
+    if (e__ != cudaSuccess) return e__; \
+  } while (0)
+
+void *Arena::alloc(size_t bytes, int cat, int cell) {
+  size_t a = (bytes + 1023) & ~(size_t)1023;
+  size_t off = used;
+  used += a;
+  by_cat[cat] += a;
+  if (cell >= 0 && cell < (int)by_cell.size()) by_cell[cell] += a;
+  if (dry) return nullptr;
+  return used <= cap ? (void *)(base + off) : nullptr;
+}
+
+// Canonical tensor list (gpipe.h); every tensor padded to a multiple of 64 elements so that the
+// flat SGD / init kernels can run over one contiguous range with 16-byte vectors.
+int Engine::build_inventory(std::string &err) {
+  (void)err;
+  tensors.clear();
+  lp.clear();
+  int64_t off = 0;
+  auto add = [&](const std::string &name, int64_t r, int64_t c, bool matrix) {
+    TensorInfo t{name, r, c, off, matrix};
+    off += ((r * c + 63) / 64) * 64;
+    tensors.push_back(t);
+    return (int)tensors.size() - 1;
+  };
+  i_emb = add("emb", V, d, true);
+  for (int l = 0; l < spec.n_layers; ++l) {
+    std::string p = "l" + std::to_string(l) + ".";
+    LayerParams q;
+    q.ln1_g = add(p + "ln1_g", 1, d, false);
+    q.ln1_b = add(p + "ln1_b", 1, d, false);
+    q.w_qkv = add(p + "w_qkv", d, 3 * da, true);
+    q.b_qkv = add(p + "b_qkv", 1, 3 * da, false);
+    q.w_o = add(p + "w_o", da, d, true);
+    q.b_o = add(p + "b_o", 1, d, false);
+    q.ln2_g = add(p + "ln2_g", 1, d, false);
+    q.ln2_b = add(p + "ln2_b", 1, d, false);
+    q.w_1 = add(p + "w_1", d, H, true);
+    q.b_1 = add(p + "b_1", 1, H, false);
+    q.w_2 = add(p + "w_2", H, d, true);
+    q.b_2 = add(p + "b_2", 1, d, false);
+    lp.push_back(q);
+  }
+  i_lnf_g = add("lnf_g", 1, d, false);
+  i_lnf_b = add("lnf_b", 1, d, false);
+  i_w_out = add("w_out", d, V, true);
+  n_flat = off;
+  return GPIPE_OK;
+}
+
+// The memory plan.  Static: everything a step needs is carved once, so the arena high-water
+// mark IS the peak (with remat, K*M boundary activations ~ N plus one cell interior
+// ~ (L/K)(N/M) per cell; without remat M interiors per cell ~ N*L).
+int Engine::build_plan(bool dry, std::string &err) {
+  arena.dry = dry;
+  arena.used = 0;
+  memset(arena.by_cat, 0, sizeof(arena.by_cat));
+  arena.by_cell.assign(K, 0);
+  size_t lpb = lp_size(dt);
+  size_t Tm = (size_t)T_mb;
+  auto F32 = [&](size_t n, int cat, int cell) { return (float *)arena.alloc(n * 4, cat, cell); };
+  auto LP = [&](size_t n, int cat, int cell) { return arena.alloc(n * lpb, cat, cell); };
+
+  master = F32((size_t)n_flat, dt == GP_BF16 ? GPIPE_CAT_MASTERS : GPIPE_CAT_WEIGHTS, -1);
+  grad = F32((size_t)n_flat, GPIPE_CAT_GRADS, -1);
+  w_lp = dt == GP_BF16 ? arena.alloc((size_t)n_flat * 2, GPIPE_CAT_WEIGHTS, -1) : (void *)master;
+
+  tok_dev = (int32_t *)arena.alloc((size_t)T_total * 4, GPIPE_CAT_MISC, -1);
+  lab_dev = (int32_t *)arena.alloc((size_t)T_total * 4, GPIPE_CAT_MISC, -1);
+  pe = F32((size_t)S * d, GPIPE_CAT_MISC, -1);
+  loss_parts = F32((size_t)M + 1, GPIPE_CAT_HEAD, -1);
+  loss_dummy = loss_parts ? loss_parts + M : nullptr;
+  flag_dev = (int *)arena.alloc(4, GPIPE_CAT_MISC, -1);
+
+  slot.assign(K, std::vector<float *>(M, nullptr));
+  for (int k = 1; k < K; ++k)
+    for (int m = 0; m < M; ++m) slot[k][m] = F32(Tm * d, GPIPE_CAT_BOUNDARY, k);
+  for (int i = 0; i < 2; ++i) {
+    dbound[i].assign(K, nullptr);
+    dbound_lp[i].assign(K, nullptr);
+    for (int k = 1; k < K; ++k) {
+      dbound[i][k] = F32(Tm * d, GPIPE_CAT_BOUNDARY, k);
+      dbound_lp[i][k] = dt == GP_BF16 ? LP(Tm * d, GPIPE_CAT_BOUNDARY, k) : (void *)dbound[i][k];
+    }
+  }
+
+  ws.assign(K, std::vector<Workspace>());
+  bwd.assign(K, BwdScratch());
+  for (int k = 0; k < K; ++k) {
+    int n_ws = remat ? 1 : M;
+    ws[k].resize(n_ws);
+    for (int w = 0; w < n_ws; ++w) {
+      Workspace &W_ = ws[k][w];
+      const int cat = GPIPE_CAT_INTERIOR;
+      if (k == 0) W_.x_emb = F32(Tm * d, cat, k);
+      if (k == K - 1 || remat) W_.x_out = F32(Tm * d, cat, k);
+      int nl = cell_hi[k] - cell_lo[k];
+      W_.layers.resize(nl);
+      for (int i = 0; i < nl; ++i) {
+        LayerBuf &b = W_.layers[i];
+        b.a = LP(Tm * d, cat, k);
+        b.qkv = LP(Tm * 3 * da, cat, k);
+        b.o = LP(Tm * da, cat, k);
+        b.c = LP(Tm * d, cat, k);
+        b.h = LP(Tm * H, cat, k);
+        b.x1 = F32(Tm * d, cat, k);
+        b.x2 = i + 1 < nl ? F32(Tm * d, cat, k) : nullptr;
+        b.lse = F32(Tm * A, cat, k);
+        b.mean1 = F32(Tm, cat, k);
+        b.rstd1 = F32(Tm, cat, k);
+        b.mean2 = F32(Tm, cat, k);
+        b.rstd2 = F32(Tm, cat, k);
+      }
+      if (k == K - 1) {
+        W_.meanf = F32(Tm, GPIPE_CAT_HEAD, k);
+        W_.rstdf = F32(Tm, GPIPE_CAT_HEAD, k);
+        W_.rowloss = F32(Tm, GPIPE_CAT_HEAD, k);
+        W_.y = LP(Tm * d, GPIPE_CAT_HEAD, k);
+        W_.logits = LP(Tm * V, GPIPE_CAT_HEAD, k);
+      }
+    }
+    BwdScratch &s = bwd[k];
+    const int cat = GPIPE_CAT_BWD;
+    for (int i = 0; i < 2; ++i) {
+      s.dx[i] = F32(Tm * d, cat, k);
+      s.dx_lp[i] = dt == GP_BF16 ? LP(Tm * d, cat, k) : (void *)s.dx[i];
+    }
+    s.dh = LP(Tm * H, cat, k);
+    s.dc = LP(Tm * d, cat, k);
+    s.d_o = LP(Tm * da, cat, k);
+    s.dqkv = LP(Tm * 3 * da, cat, k);
+    s.dvec = F32(Tm * A, cat, k);
+    s.ln_partials = F32((size_t)ln_bwd_partial_rows(sm_count) * 2 * d, cat, k);
+  }
+  if (!dry && arena.used > arena.cap) {
+    err = "arena too small: need " + std::to_string(arena.used) + " bytes, have " +
+          std::to_string(arena.cap);
+    return GPIPE_ENOMEM;
+  }
+  return GPIPE_OK;
+}
+
+cudaEvent_t Engine::pool_event() {
+  if (ev_pool_used == ev_pool.size()) {
+    cudaEvent_t e;
+    cudaEventCreate(&e);
+    ev_pool.push_back(e);
+  }
+  return ev_pool[ev_pool_used++];
+}
+
+// ---------------------------------------------------------------------------------------------
+// F_k (and its replay): embedding (cell 0), the cell's layers, head + loss (cell K-1)
+// ---------------------------------------------------------------------------------------------
+cudaError_t Engine::forward_cell(int k, int m, bool replay) {
+  Ctx c = ctx(k);
+  Workspace &w = wsp(k, m);
+  const int32_t *tok = tok_dev + (int64_t)m * T_mb;
+  const int32_t *lab = lab_dev + (int64_t)m * T_mb;
+  float *x;
+  if (k == 0) {
+    GP_TRY(embed_fwd(c, dt, tok, W(i_emb), pe, w.x_emb, T_mb, S, d));
+    x = w.x_emb;
+  } else {
+    x = slot[k][m];
+  }
+  int nl = cell_hi[k] - cell_lo[k];
+  for (int i = 0; i < nl; ++i) {
+    int l = cell_lo[k] + i;
+    const LayerParams &q = lp[l];
+    LayerBuf &b = w.layers[i];
+    bool last = (i + 1 == nl);
+    // a = LN1(x)                                                             (a5)
+    GP_TRY(ln_fwd(c, dt, x, P(q.ln1_g), P(q.ln1_b), b.a, b.mean1, b.rstd1, T_mb, d, eps));
+    // [q|k|v] = a W_qkv + b_qkv                                              (a6)
+    GemmArgs g{};
+    g.M = (int)T_mb; g.N = 3 * da; g.K = d;
+    g.A = b.a; g.lda = d; g.B = W(q.w_qkv); g.ldb = 3 * da; g.C = b.qkv; g.ldc = 3 * da;
+    g.bias = P(q.b_qkv); g.flags = EPI_BIAS;
+    GP_TRY(gemm(c, dt, g));
+    // o = softmax(q k^T / sqrt(dh) + mask) v                                 (a7)
+    GP_TRY(attn_fwd(c, dt, b.qkv, b.o, b.lse, (int)nb, S, A, dh, causal[l]));
+    // x1 = x + o W_o + b_o                                                   (a8)
+    g = GemmArgs{};
+    g.M = (int)T_mb; g.N = d; g.K = da;
+    g.A = b.o; g.lda = da; g.B = W(q.w_o); g.ldb = d; g.C = b.x1; g.ldc = d;
+    g.bias = P(q.b_o); g.resid = x; g.flags = EPI_BIAS | EPI_RESID | EPI_OUT_F32;
+    GP_TRY(gemm(c, dt, g));
+    // c = LN2(x1)                                                            (a9)
+    GP_TRY(ln_fwd(c, dt, b.x1, P(q.ln2_g), P(q.ln2_b), b.c, b.mean2, b.rstd2, T_mb, d, eps));
+    // h = relu(c W_1 + b_1)                                                  (a10)
+    g = GemmArgs{};
+    g.M = (int)T_mb; g.N = H; g.K = d;
+    g.A = b.c; g.lda = d; g.B = W(q.w_1); g.ldb = H; g.C = b.h; g.ldc = H;
+    g.bias = P(q.b_1); g.flags = EPI_BIAS | EPI_RELU;
+    GP_TRY(gemm(c, dt, g));
+    // x2 = x1 + h W_2 + b_2                                                  (a11)
+    float *x2;
+    if (!last) x2 = b.x2;
+    else if (k == K - 1) x2 = w.x_out;
+    else if (!replay) x2 = slot[k + 1][m];            // boundary stash (a12)
+    else if (replay_full) x2 = w.x_out;               // replay output nobody reads
+    else x2 = nullptr;                                // skipped: B_k does not need F_k's output
+    if (x2) {
+      g = GemmArgs{};
+      g.M = (int)T_mb; g.N = d; g.K = H;
+      g.A = b.h; g.lda = H; g.B = W(q.w_2); g.ldb = d; g.C = x2; g.ldc = d;
+      g.bias = P(q.b_2); g.resid = b.x1; g.flags = EPI_BIAS | EPI_RESID | EPI_OUT_F32;
+      GP_TRY(gemm(c, dt, g));
+    }
+    x = x2;
+  }
+  if (k == K - 1) {
+    if (nl == 0 && K == 1) x = w.x_emb;
+    // y = LN_f(x_L); logits = y W_out; fused softmax-CE -> loss partial, dlogits   (a13, a14)
+    GP_TRY(ln_fwd(c, dt, x, P(i_lnf_g), P(i_lnf_b), w.y, w.meanf, w.rstdf, T_mb, d, eps));
+    GemmArgs g{};
+    g.M = (int)T_mb; g.N = V; g.K = d;
+    g.A = w.y; g.lda = d; g.B = W(i_w_out); g.ldb = V; g.C = w.logits; g.ldc = V;
+    g.flags = 0;
+    GP_TRY(gemm(c, dt, g));
+    GP_TRY(softmax_ce(c, dt, w.logits, lab, w.rowloss, T_mb, V, 1.f / (float)T_total));
+    GP_TRY(loss_reduce(c, w.rowloss, replay ? loss_dummy : loss_parts + m, T_mb));
+  }
+  return cudaSuccess;
+}
+
+// ---------------------------------------------------------------------------------------------
+// B_k: back-propagation through the cell, accumulating parameter gradients in fp32 (a16-a18)
+// ---------------------------------------------------------------------------------------------
+cudaError_t Engine::backward_cell(int k, int m) {
+  Ctx c = ctx(k);
+  Workspace &w = wsp(k, m);
+  BwdScratch &s = bwd[k];
+  const int32_t *tok = tok_dev + (int64_t)m * T_mb;
+  int nl = cell_hi[k] - cell_lo[k];
+  const float *dx;            // gradient of the residual stream at the current position
+  const void *dxo;            // its lp operand copy
+  int cur = 0;                // which ping-pong buffer the NEXT producer writes
+  auto wgrad = [&](const void *X, int64_t ldx, int Min, const void *dY, int64_t ldy, int Nout,
+                   int iw) -> cudaError_t {
+    GemmArgs g{};
+    g.M = Min; g.N = Nout; g.K = (int)T_mb;
+    g.A = X; g.lda = ldx; g.transA = 1; g.B = dY; g.ldb = ldy; g.transB = 0;
+    g.C = G(iw); g.ldc = Nout; g.flags = EPI_ACCUM | EPI_OUT_F32;
+    return gemm(c, dt, g);
+  };
+  auto dgrad = [&](const void *dY, int64_t ldy, int Kout, int iw, int Nin, void *dX,
+                   const void *mask) -> cudaError_t {
+    GemmArgs g{};
+    g.M = (int)T_mb; g.N = Nin; g.K = Kout;
+    g.A = dY; g.lda = ldy; g.transA = 0; g.B = W(iw); g.ldb = Kout; g.transB = 1;
+    g.C = dX; g.ldc = Nin; g.mask = mask; g.ldmask = Nin; g.flags = mask ? EPI_MASK : 0;
+    return gemm(c, dt, g);
+  };
+
+  if (k == K - 1) {
+    const float *xL = nl > 0 ? w.x_out : (K == 1 ? w.x_emb : slot[k][m]);
+    GP_TRY(wgrad(w.y, d, d, w.logits, V, V, i_w_out));                 // dW_out += y^T dlogits
+    GP_TRY(dgrad(w.logits, V, V, i_w_out, d, s.dc, nullptr));          // dy = dlogits W_out^T
+    GP_TRY(ln_bwd(c, dt, s.dc, xL, w.meanf, w.rstdf, P(i_lnf_g), nullptr, s.dx[cur],
+                  dt == GP_BF16 ? s.dx_lp[cur] : nullptr, s.ln_partials, G(i_lnf_g), G(i_lnf_b),
+                  T_mb, d));
+    dx = s.dx[cur];
+    dxo = s.dx_lp[cur];
+    cur ^= 1;
+  } else {
+    dx = dbound[m & 1][k + 1];
+    dxo = dbound_lp[m & 1][k + 1];
+  }
+  for (int i = nl - 1; i >= 0; --i) {
+    int l = cell_lo[k] + i;
+    const LayerParams &q = lp[l];
+    LayerBuf &b = w.layers[i];
+    const float *x_in = i > 0 ? w.layers[i - 1].x2 : (k == 0 ? w.x_emb : slot[k][m]);
+    // FFN: dh = (dx W_2^T) * [h > 0]; dW_2 += h^T dx; db_2 += sum_t dx
+    GP_TRY(dgrad(dxo, d, d, q.w_2, H, s.dh, b.h));
+    GP_TRY(wgrad(b.h, H, H, dxo, d, d, q.w_2));
+    GP_TRY(colsum_accum(c, dt, dxo, d, G(q.b_2), T_mb, d));
+    // dc = dh W_1^T; dW_1 += c^T dh; db_1 += sum_t dh
+    GP_TRY(dgrad(s.dh, H, H, q.w_1, d, s.dc, nullptr));
+    GP_TRY(wgrad(b.c, d, d, s.dh, H, H, q.w_1));
+    GP_TRY(colsum_accum(c, dt, s.dh, H, G(q.b_1), T_mb, H));
+    // LN2 backward; residual adds gradients: dx1 = dx + LN2'(dc)
+    GP_TRY(ln_bwd(c, dt, s.dc, b.x1, b.mean2, b.rstd2, P(q.ln2_g), dx, s.dx[cur],
+                  dt == GP_BF16 ? s.dx_lp[cur] : nullptr, s.ln_partials, G(q.ln2_g), G(q.ln2_b),
+                  T_mb, d));
+    dx = s.dx[cur];
+    dxo = s.dx_lp[cur];
+    cur ^= 1;
+    // attention block: do = dx1 W_o^T; dW_o += o^T dx1; db_o += sum_t dx1
+    GP_TRY(dgrad(dxo, d, d, q.w_o, da, s.d_o, nullptr));
+    GP_TRY(wgrad(b.o, da, da, dxo, d, d, q.w_o));
+    GP_TRY(colsum_accum(c, dt, dxo, d, G(q.b_o), T_mb, d));
+    GP_TRY(attn_bwd(c, dt, b.qkv, b.o, s.d_o, b.lse, s.dqkv, s.dvec, (int)nb, S, A, dh, causal[l]));
+    // da = dqkv W_qkv^T; dW_qkv += a^T dqkv; db_qkv += sum_t dqkv
+    GP_TRY(dgrad(s.dqkv, 3 * da, 3 * da, q.w_qkv, d, s.dc, nullptr));
+    GP_TRY(wgrad(b.a, d, d, s.dqkv, 3 * da, 3 * da, q.w_qkv));
+    GP_TRY(colsum_accum(c, dt, s.dqkv, 3 * da, G(q.b_qkv), T_mb, 3 * da));
+    // LN1 backward: dx_in = dx1 + LN1'(da); the cell's first layer writes the boundary gradient
+    float *out = s.dx[cur];
+    void *out_lp = s.dx_lp[cur];
+    if (i == 0 && k > 0) {
+      out = dbound[m & 1][k];
+      out_lp = dbound_lp[m & 1][k];
+    }
+    GP_TRY(ln_bwd(c, dt, s.dc, x_in, b.mean1, b.rstd1, P(q.ln1_g), dx, out,
+                  dt == GP_BF16 ? out_lp : nullptr, s.ln_partials, G(q.ln1_g), G(q.ln1_b), T_mb, d));
+    dx = out;
+    dxo = out_lp;
+    cur ^= 1;
+  }
+  if (k == 0) GP_TRY(embed_bwd(c, tok, dx, G(i_emb), T_mb, d));       // dE[tok] += dx0
+  return cudaSuccess;
+}
+
+// ---------------------------------------------------------------------------------------------
+// One mini-batch on the GPipe schedule.  Tasks are enqueued in global tick order (a topological
+// order of the dependency graph), cell k on stream k:
+//   forward ticks   F(k,m), m = tau - k                      F(k,m) <- F(k-1,m)
+//   backward ticks  [R(k,m)] B(k,m), m = M-1 - (tau-(K-1-k))  B(k,m) <- B(k+1,m);  R(k,m) <- slot only
+// ---------------------------------------------------------------------------------------------
+cudaError_t Engine::run_step(float *loss_out) {
+  ev_pool_used = 0;
+  trace.clear();
+  int idx = 0;
+  auto task = [&](int kind, int k, int m) -> cudaError_t {
+    TraceRec r{kind, k, m, idx++, nullptr, nullptr};
+    if (trace_on) {
+      r.e0 = pool_event();
+      r.e1 = pool_event();
+      GP_TRY(cudaEventRecord(r.e0, streams[k]));
+    }
+    cudaError_t e = kind == 'B' ? backward_cell(k, m) : forward_cell(k, m, kind == 'R');
+    if (e != cudaSuccess) return e;
+    if (trace_on) {
+      GP_TRY(cudaEventRecord(r.e1, streams[k]));
+      trace.push_back(r);
+    }
+    return cudaSuccess;
+  };
+  // inputs are on stream 0; every other cell waits for them
+  GP_TRY(cudaEventRecord(ev_in, streams[0]));
+  for (int k = 1; k < K; ++k) GP_TRY(cudaStreamWaitEvent(streams[k], ev_in, 0));
+  if (trace_on) GP_TRY(cudaEventRecord(ev_t0, streams[0]));
+
+  for (int tau = 0; tau < M + K - 1; ++tau)
+    for (int k = 0; k < K; ++k) {
+      int m = tau - k;
+      if (m < 0 || m >= M) continue;
+      if (k > 0) GP_TRY(cudaStreamWaitEvent(streams[k], ev_f[k - 1][m], 0));
+      GP_TRY(task('F', k, m));
+      if (k + 1 < K) GP_TRY(cudaEventRecord(ev_f[k][m], streams[k]));
+    }
+  for (int tau = 0; tau < M + K - 1; ++tau)
+    for (int k = K - 1; k >= 0; --k) {
+      int m = M - 1 - (tau - (K - 1 - k));
+      if (m < 0 || m >= M) continue;
+      if (remat) GP_TRY(task('R', k, m));                       // early: no wait on B(k+1,m)
+      if (k + 1 < K) GP_TRY(cudaStreamWaitEvent(streams[k], ev_b[k + 1][m], 0));
+      // the boundary-gradient ring has two entries: B(k,m) reuses the one B(k-1,m+2) read
+      if (k > 0 && m + 2 < M) GP_TRY(cudaStreamWaitEvent(streams[k], ev_b[k - 1][m + 2], 0));
+      GP_TRY(task('B', k, m));
+      GP_TRY(cudaEventRecord(ev_b[k][m], streams[k]));
+    }
+  // join: stream 0 waits for every cell, then the loss partials come back
+  for (int k = 1; k < K; ++k) {
+    GP_TRY(cudaEventRecord(ev_done[k], streams[k]));
+    GP_TRY(cudaStreamWaitEvent(streams[0], ev_done[k], 0));
+  }
+  GP_TRY(cudaMemcpyAsync(host_loss, loss_parts, sizeof(float) * M, cudaMemcpyDeviceToHost, streams[0]));
+  GP_TRY(cudaStreamSynchronize(streams[0]));
+  double s = 0.0;
+  for (int m = 0; m < M; ++m) s += (double)host_loss[m];
+  *loss_out = (float)s;
+  return cudaSuccess;
+}
+
+}  // namespace gp

@@ -1,0 +1,124 @@
+// engine.h - host-side state of one gpipe handle: parameter inventory, memory plan (arena carving
+// + peak-HBM tracker), cell workspaces, and the GPipe scheduler (K streams, events, replay).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/gpipe.h"
+#include "ops.h"
+
+namespace gp {
+
+struct TensorInfo {
+  std::string name;
+  int64_t rows, cols;
+  int64_t off;        // element offset into the flat master / grad / lp arrays
+  bool matrix;        // matrices are tensor-core operands (lp working copy); vectors stay fp32
+};
+
+struct LayerParams {  // indices into Engine::tensors
+  int ln1_g, ln1_b, w_qkv, b_qkv, w_o, b_o, ln2_g, ln2_b, w_1, b_1, w_2, b_2;
+};
+
+// Interior activations of one layer that the backward pass needs.
+struct LayerBuf {
+  void *a, *qkv, *o, *c, *h;             // lp
+  float *x1, *x2;                        // fp32 residual stream (x2 unused for the cell's last layer)
+  float *lse, *mean1, *rstd1, *mean2, *rstd2;
+};
+
+struct Workspace {                       // one per cell (remat) or per (cell, micro-batch)
+  float *x_emb = nullptr;                // cell 0: embedding output
+  float *x_out = nullptr;                // last cell: x_L; other cells: replay output scratch
+  std::vector<LayerBuf> layers;
+  float *meanf = nullptr, *rstdf = nullptr, *rowloss = nullptr;   // head (last cell)
+  void *y = nullptr, *logits = nullptr;
+};
+
+struct BwdScratch {                      // one per cell
+  float *dx[2];                          // residual-gradient ping-pong, fp32 [T_mb, d]
+  void *dx_lp[2];                        // lp operand copies (bf16 mode)
+  void *dh, *dc, *d_o, *dqkv;            // lp activation gradients
+  float *dvec;                           // attention D = rowsum(dO*O)
+  float *ln_partials;
+};
+
+struct Arena {
+  char *base = nullptr;
+  size_t cap = 0, used = 0;
+  bool dry = true;
+  size_t by_cat[GPIPE_NUM_CATS] = {0};
+  std::vector<size_t> by_cell;
+  void *alloc(size_t bytes, int cat, int cell);
+};
+
+struct TraceRec {
+  int kind, k, m, idx;
+  cudaEvent_t e0, e1;
+};
+
+struct Engine {
+  gpipe_layer_spec spec;
+  std::vector<uint8_t> causal;
+  int K = 1, M = 1, remat = 1, dt = GP_F32;
+  int64_t n_seqs = 0, nb = 0, T_mb = 0, T_total = 0;   // nb = sequences per micro-batch
+  int d = 0, H = 0, A = 0, dh = 0, da = 0, V = 0, S = 0;
+  float eps = 1e-5f;
+  int sm_count = 148;
+  int gemm_backend = 0;
+  int replay_full = 0;
+
+  std::vector<TensorInfo> tensors;
+  std::vector<LayerParams> lp;
+  int i_emb = 0, i_lnf_g = 0, i_lnf_b = 0, i_w_out = 0;
+  int64_t n_flat = 0;
+  float *master = nullptr, *grad = nullptr;
+  void *w_lp = nullptr;                                // bf16 working copy (bf16 mode), else = master
+
+  std::vector<int> cell_lo, cell_hi;                   // layers [lo, hi) of cell k
+  Arena arena;
+  std::vector<cudaStream_t> streams;
+  std::vector<std::vector<float *>> slot;              // slot[k][m], k = 1..K-1: input of cell k
+  std::vector<float *> dbound[2];                      // dbound[i][k]: gradient wrt input of cell k
+  std::vector<void *> dbound_lp[2];
+  std::vector<std::vector<Workspace>> ws;              // ws[k][remat ? 0 : m]
+  std::vector<BwdScratch> bwd;
+  int32_t *tok_dev = nullptr, *lab_dev = nullptr;
+  float *pe = nullptr, *loss_parts = nullptr, *loss_dummy = nullptr;
+  int *flag_dev = nullptr;
+  float *host_loss = nullptr;                          // pinned
+  int *host_flag = nullptr;                            // pinned
+
+  std::vector<std::vector<cudaEvent_t>> ev_f, ev_b;    // [k][m]
+  cudaEvent_t ev_in = nullptr;
+  std::vector<cudaEvent_t> ev_done;                    // per stream
+
+  int trace_on = 0;
+  std::vector<TraceRec> trace;
+  std::vector<cudaEvent_t> ev_pool;
+  size_t ev_pool_used = 0;
+  cudaEvent_t ev_t0 = nullptr;
+  int64_t launches = 0;
+
+  // -- construction --
+  int build_inventory(std::string &err);
+  int build_plan(bool dry, std::string &err);
+  // -- helpers --
+  Ctx ctx(int k) { return Ctx{streams[k], &launches, sm_count, gemm_backend}; }
+  float *P(int i) const { return master + tensors[i].off; }            // fp32 vector param
+  const void *W(int i) const {                                         // matrix operand
+    return dt == GP_BF16 ? (const void *)((const char *)w_lp + tensors[i].off * 2)
+                         : (const void *)(master + tensors[i].off);
+  }
+  float *G(int i) const { return grad + tensors[i].off; }
+  Workspace &wsp(int k, int m) { return ws[k][remat ? 0 : m]; }
+  // -- schedule --
+  cudaError_t forward_cell(int k, int m, bool replay);
+  cudaError_t backward_cell(int k, int m);
+  cudaError_t run_step(float *loss_out);
+  cudaEvent_t pool_event();
+};
+
+}  // namespace gp

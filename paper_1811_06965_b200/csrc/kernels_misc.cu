@@ -1,0 +1,314 @@
+// kernels_misc.cu - fused softmax cross-entropy over the vocabulary, loss reduction, SGD apply,
+// device-side parameter initialisation (Philox-4x32-10 + Box-Muller) and dtype conversions.
+#include "common.cuh"
+
+namespace gp {
+
+// ---------------------------------------------------------------------------------------------
+// Fused softmax cross-entropy (reading A8): one block per token row.
+//   rowloss[t] = (log sum_v exp(z_v - max) + max - z_label) * inv_T
+//   z_v <- (exp(z_v - max)/sum - [v == label]) * inv_T            (in place: logits -> dlogits)
+// The row is read once from HBM into registers (VPT vectors of 8 (bf16) / 4 (fp32) elements per
+// thread) when it fits, so HBM traffic is one read + one write of the row; longer rows fall
+// back to three passes over global memory (L2-resident row).
+// ---------------------------------------------------------------------------------------------
+template <typename T> struct VecIO;       // 16-byte vectors kept packed in registers
+template <> struct VecIO<float> {
+  static constexpr int W = 4;
+  __device__ static void unpack(const uint4 &u, float *v) {
+    v[0] = __uint_as_float(u.x); v[1] = __uint_as_float(u.y);
+    v[2] = __uint_as_float(u.z); v[3] = __uint_as_float(u.w);
+  }
+  __device__ static uint4 pack(const float *v) {
+    return make_uint4(__float_as_uint(v[0]), __float_as_uint(v[1]), __float_as_uint(v[2]),
+                      __float_as_uint(v[3]));
+  }
+};
+template <> struct VecIO<bf16> {
+  static constexpr int W = 8;
+  __device__ static void unpack(const uint4 &u, float *v) {
+    const __nv_bfloat162 *h = reinterpret_cast<const __nv_bfloat162 *>(&u);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      float2 f = __bfloat1622float2(h[i]);
+      v[2 * i] = f.x;
+      v[2 * i + 1] = f.y;
+    }
+  }
+  __device__ static uint4 pack(const float *v) {
+    uint4 u;
+    __nv_bfloat162 *h = reinterpret_cast<__nv_bfloat162 *>(&u);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) h[i] = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]);
+    return u;
+  }
+};
+
+template <typename T, int VPT>
+__global__ void __launch_bounds__(1024)
+softmax_ce_reg_kernel(T *__restrict__ logits, const int32_t *__restrict__ labels,
+                      float *__restrict__ rowloss, int V, float inv_T) {
+  constexpr int W = VecIO<T>::W;
+  __shared__ float red[33];
+  int64_t row = blockIdx.x;
+  uint4 *z = reinterpret_cast<uint4 *>(logits + row * (int64_t)V);
+  int nvec = V / W;
+  uint4 raw[VPT];
+  float mx = -INFINITY;
+#pragma unroll
+  for (int i = 0; i < VPT; ++i) {
+    int j = threadIdx.x + i * blockDim.x;
+    if (j < nvec) {
+      raw[i] = z[j];
+      float v[W];
+      VecIO<T>::unpack(raw[i], v);
+#pragma unroll
+      for (int e = 0; e < W; ++e) mx = fmaxf(mx, v[e]);
+    }
+  }
+  mx = block_max(mx, red);
+  float s = 0.f;
+#pragma unroll
+  for (int i = 0; i < VPT; ++i) {
+    int j = threadIdx.x + i * blockDim.x;
+    if (j < nvec) {
+      float v[W];
+      VecIO<T>::unpack(raw[i], v);
+#pragma unroll
+      for (int e = 0; e < W; ++e) s += expf(v[e] - mx);
+    }
+  }
+  s = block_sum(s, red);
+  int lab = labels[row];
+  float inv = 1.f / s;
+  if (threadIdx.x == 0) rowloss[row] = (logf(s) + mx - to_f<T>(logits[row * (int64_t)V + lab])) * inv_T;
+  __syncthreads();                       // z[lab] read before anyone overwrites it
+#pragma unroll
+  for (int i = 0; i < VPT; ++i) {
+    int j = threadIdx.x + i * blockDim.x;
+    if (j < nvec) {
+      float v[W];
+      VecIO<T>::unpack(raw[i], v);
+#pragma unroll
+      for (int e = 0; e < W; ++e) {
+        float p = expf(v[e] - mx) * inv;
+        if (j * W + e == lab) p -= 1.f;
+        v[e] = p * inv_T;
+      }
+      z[j] = VecIO<T>::pack(v);
+    }
+  }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(1024)
+softmax_ce_3pass_kernel(T *__restrict__ logits, const int32_t *__restrict__ labels,
+                        float *__restrict__ rowloss, int V, float inv_T) {
+  __shared__ float red[33];
+  int64_t row = blockIdx.x;
+  T *z = logits + row * (int64_t)V;
+  float mx = -INFINITY;
+  for (int j = threadIdx.x; j < V; j += blockDim.x) mx = fmaxf(mx, to_f<T>(z[j]));
+  mx = block_max(mx, red);
+  float s = 0.f;
+  for (int j = threadIdx.x; j < V; j += blockDim.x) s += expf(to_f<T>(z[j]) - mx);
+  s = block_sum(s, red);
+  int lab = labels[row];
+  float inv = 1.f / s;
+  if (threadIdx.x == 0) rowloss[row] = (logf(s) + mx - to_f<T>(z[lab])) * inv_T;
+  __syncthreads();
+  for (int j = threadIdx.x; j < V; j += blockDim.x) {
+    float p = expf(to_f<T>(z[j]) - mx) * inv;
+    if (j == lab) p -= 1.f;
+    z[j] = from_f<T>(p * inv_T);
+  }
+}
+
+template <typename T>
+static cudaError_t softmax_ce_t(const Ctx &c, T *logits, const int32_t *labels, float *rowloss,
+                                int64_t n_tok, int V, float inv_T) {
+  if (n_tok == 0) return cudaSuccess;
+  constexpr int W = VecIO<T>::W;
+  unsigned grid = (unsigned)n_tok;
+  int nvec = V / W;
+  bool vec_ok = (V % W == 0);
+  if (vec_ok && nvec <= 256)
+    softmax_ce_reg_kernel<T, 1><<<grid, 256, 0, c.stream>>>(logits, labels, rowloss, V, inv_T);
+  else if (vec_ok && nvec <= 1024 * 4)
+    softmax_ce_reg_kernel<T, 4><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T);
+  else if (vec_ok && nvec <= 1024 * 8)
+    softmax_ce_reg_kernel<T, 8><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T);
+  else
+    softmax_ce_3pass_kernel<T><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T);
+  GP_LAUNCH_CHECK(c);
+}
+
+cudaError_t softmax_ce(const Ctx &c, int dt, void *logits, const int32_t *labels, float *rowloss,
+                       int64_t n_tok, int V, float inv_T) {
+  return dt == GP_BF16 ? softmax_ce_t<bf16>(c, (bf16 *)logits, labels, rowloss, n_tok, V, inv_T)
+                       : softmax_ce_t<float>(c, (float *)logits, labels, rowloss, n_tok, V, inv_T);
+}
+
+// single block, fixed order: loss = sum_t rowloss[t]
+__global__ void __launch_bounds__(1024)
+loss_reduce_kernel(const float *__restrict__ rowloss, float *__restrict__ loss, int64_t n) {
+  __shared__ float red[33];
+  float s = 0.f;
+  for (int64_t i = threadIdx.x; i < n; i += blockDim.x) s += rowloss[i];
+  s = block_sum(s, red);
+  if (threadIdx.x == 0) *loss = s;
+}
+
+cudaError_t loss_reduce(const Ctx &c, const float *rowloss, float *loss, int64_t n_tok) {
+  loss_reduce_kernel<<<1, 1024, 0, c.stream>>>(rowloss, loss, n_tok);
+  GP_LAUNCH_CHECK(c);
+}
+
+// ---------------------------------------------------------------------------------------------
+// SGD apply: master -= lr*g; working copy = RNE(master); g = 0.  One pass.
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256)
+sgd_kernel(float *__restrict__ master, float *__restrict__ grad, T *__restrict__ w_lp, int64_t n4,
+           float lr) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    float4 m = load4(master + 4 * i), g = load4(grad + 4 * i);
+    m.x -= lr * g.x; m.y -= lr * g.y; m.z -= lr * g.z; m.w -= lr * g.w;
+    store4(master + 4 * i, m);
+    if (w_lp) store4(w_lp + 4 * i, m);
+    store4(grad + 4 * i, make_float4(0.f, 0.f, 0.f, 0.f));
+  }
+}
+
+cudaError_t sgd_apply(const Ctx &c, int dt, float *master, float *grad, void *w_lp, int64_t n,
+                      float lr) {
+  if (n == 0) return cudaSuccess;
+  int64_t n4 = n / 4;
+  int64_t want = (n4 + 255) / 256;
+  unsigned grid = (unsigned)(want < (int64_t)c.sm_count * 16 ? want : (int64_t)c.sm_count * 16);
+  if (dt == GP_BF16) sgd_kernel<bf16><<<grid, 256, 0, c.stream>>>(master, grad, (bf16 *)w_lp, n4, lr);
+  else sgd_kernel<float><<<grid, 256, 0, c.stream>>>(master, grad, (float *)nullptr, n4, lr);
+  GP_LAUNCH_CHECK(c);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Philox-4x32-10 counter RNG + Box-Muller; element i uses counter (i/4, stream_id), lane i%4
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void philox_round(uint32_t &c0, uint32_t &c1, uint32_t &c2, uint32_t &c3,
+                                             uint32_t k0, uint32_t k1) {
+  const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+  uint32_t hi0 = __umulhi(M0, c0), lo0 = M0 * c0;
+  uint32_t hi1 = __umulhi(M1, c2), lo1 = M1 * c2;
+  uint32_t n0 = hi1 ^ c1 ^ k0, n1 = lo1, n2 = hi0 ^ c3 ^ k1, n3 = lo0;
+  c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+init_normal_kernel(float *__restrict__ master, T *__restrict__ w_lp, int64_t n4, uint64_t seed,
+                   uint64_t stream_id, float mean, float std) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    uint32_t c0 = (uint32_t)i, c1 = (uint32_t)((uint64_t)i >> 32);
+    uint32_t c2 = (uint32_t)stream_id, c3 = (uint32_t)(stream_id >> 32);
+    uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+      philox_round(c0, c1, c2, c3, k0, k1);
+      k0 += 0x9E3779B9u;
+      k1 += 0xBB67AE85u;
+    }
+    const float two32 = 2.3283064365386963e-10f;
+    float u0 = ((float)c0 + 0.5f) * two32, u1 = ((float)c1 + 0.5f) * two32;
+    float u2 = ((float)c2 + 0.5f) * two32, u3 = ((float)c3 + 0.5f) * two32;
+    u0 = fminf(fmaxf(u0, 1e-12f), 1.f);
+    u2 = fminf(fmaxf(u2, 1e-12f), 1.f);
+    float r0 = sqrtf(-2.f * logf(u0)), r1 = sqrtf(-2.f * logf(u2));
+    float s0, c0f, s1, c1f;
+    sincospif(2.f * u1, &s0, &c0f);
+    sincospif(2.f * u3, &s1, &c1f);
+    float4 v = make_float4(mean + std * r0 * c0f, mean + std * r0 * s0, mean + std * r1 * c1f,
+                           mean + std * r1 * s1);
+    if (w_lp) {                      // bf16 mode: master = the RNE-rounded draw (reading A12)
+      store4(w_lp + 4 * i, v);
+      v = load4(w_lp + 4 * i);
+    }
+    store4(master + 4 * i, v);
+  }
+}
+
+cudaError_t init_normal(const Ctx &c, int dt, float *master, void *w_lp, int64_t n, uint64_t seed,
+                        uint64_t stream_id, float mean, float std) {
+  if (n == 0) return cudaSuccess;
+  int64_t n4 = n / 4;
+  int64_t want = (n4 + 255) / 256;
+  unsigned grid = (unsigned)(want < (int64_t)c.sm_count * 16 ? want : (int64_t)c.sm_count * 16);
+  if (dt == GP_BF16)
+    init_normal_kernel<bf16><<<grid, 256, 0, c.stream>>>(master, (bf16 *)w_lp, n4, seed, stream_id, mean, std);
+  else
+    init_normal_kernel<float><<<grid, 256, 0, c.stream>>>(master, (float *)nullptr, n4, seed, stream_id, mean, std);
+  GP_LAUNCH_CHECK(c);
+}
+
+__global__ void fill_kernel(float *p, int64_t n, float v) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+       i += (int64_t)gridDim.x * blockDim.x)
+    p[i] = v;
+}
+cudaError_t fill_f32(const Ctx &c, float *p, int64_t n, float v) {
+  if (n == 0) return cudaSuccess;
+  int64_t want = (n + 255) / 256;
+  unsigned grid = (unsigned)(want < (int64_t)c.sm_count * 16 ? want : (int64_t)c.sm_count * 16);
+  fill_kernel<<<grid, 256, 0, c.stream>>>(p, n, v);
+  GP_LAUNCH_CHECK(c);
+}
+
+// master (fp32) -> lp working copy; round_master != 0 also writes the rounded value back
+template <typename T>
+__global__ void master_to_lp_kernel(float *__restrict__ master, T *__restrict__ w_lp, int64_t n,
+                                    int round_master) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    T v = from_f<T>(master[i]);
+    w_lp[i] = v;
+    if (round_master) master[i] = to_f<T>(v);
+  }
+}
+cudaError_t master_to_lp(const Ctx &c, int dt, float *master, void *w_lp, int64_t n, int round_master) {
+  if (n == 0 || dt != GP_BF16) return cudaSuccess;
+  int64_t want = (n + 255) / 256;
+  unsigned grid = (unsigned)(want < (int64_t)c.sm_count * 16 ? want : (int64_t)c.sm_count * 16);
+  master_to_lp_kernel<bf16><<<grid, 256, 0, c.stream>>>(master, (bf16 *)w_lp, n, round_master);
+  GP_LAUNCH_CHECK(c);
+}
+
+template <typename T>
+__global__ void lp_to_f32_kernel(const T *__restrict__ src, float *__restrict__ dst, int64_t n) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+       i += (int64_t)gridDim.x * blockDim.x)
+    dst[i] = to_f<T>(src[i]);
+}
+cudaError_t lp_to_f32(const Ctx &c, int dt, const void *src, float *dst, int64_t n) {
+  if (n == 0) return cudaSuccess;
+  int64_t want = (n + 255) / 256;
+  unsigned grid = (unsigned)(want < (int64_t)c.sm_count * 16 ? want : (int64_t)c.sm_count * 16);
+  if (dt == GP_BF16) lp_to_f32_kernel<bf16><<<grid, 256, 0, c.stream>>>((const bf16 *)src, dst, n);
+  else lp_to_f32_kernel<float><<<grid, 256, 0, c.stream>>>((const float *)src, dst, n);
+  GP_LAUNCH_CHECK(c);
+}
+
+__global__ void check_ids_kernel(const int32_t *__restrict__ ids, int64_t n, int V, int *flag) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+       i += (int64_t)gridDim.x * blockDim.x)
+    if (ids[i] < 0 || ids[i] >= V) *flag = 1;
+}
+cudaError_t check_ids(const Ctx &c, const int32_t *ids, int64_t n, int V, int *flag) {
+  if (n == 0) return cudaSuccess;
+  int64_t want = (n + 255) / 256;
+  unsigned grid = (unsigned)(want < (int64_t)c.sm_count * 4 ? want : (int64_t)c.sm_count * 4);
+  check_ids_kernel<<<grid, 256, 0, c.stream>>>(ids, n, V, flag);
+  GP_LAUNCH_CHECK(c);
+}
+
+}  // namespace gp

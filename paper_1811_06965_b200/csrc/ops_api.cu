@@ -1,0 +1,116 @@
+// ops_api.cu - extern "C" wrappers of include/gpipe_ops.h and the backend dispatch of ops.h.
+#include <string>
+
+#include "../../include/gpipe.h"
+#include "../../include/gpipe_ops.h"
+#include "ops.h"
+
+namespace gp {
+cudaError_t gemm_simt(const Ctx &c, int dt, const GemmArgs &a);
+cudaError_t gemm_tc(const Ctx &c, const GemmArgs &a);
+cudaError_t attn_fwd_simt(const Ctx &c, int dt, const void *qkv, void *o, float *lse, int n_seq,
+                          int S, int A, int dh, int causal);
+cudaError_t attn_bwd_simt(const Ctx &c, int dt, const void *qkv, const void *o, const void *d_o,
+                          const float *lse, void *dqkv, float *dvec, int n_seq, int S, int A, int dh,
+                          int causal);
+
+cudaError_t gemm(const Ctx &c, int dt, const GemmArgs &a) {
+  if (c.gemm_backend != 1 && gemm_tc_supported(dt, a)) return gemm_tc(c, a);
+  if (c.gemm_backend == 2) return cudaErrorNotSupported;
+  return gemm_simt(c, dt, a);
+}
+cudaError_t attn_fwd(const Ctx &c, int dt, const void *qkv, void *o, float *lse, int n_seq, int S,
+                     int A, int dh, int causal) {
+  return attn_fwd_simt(c, dt, qkv, o, lse, n_seq, S, A, dh, causal);
+}
+cudaError_t attn_bwd(const Ctx &c, int dt, const void *qkv, const void *o, const void *d_o,
+                     const float *lse, void *dqkv, float *dvec, int n_seq, int S, int A, int dh,
+                     int causal) {
+  return attn_bwd_simt(c, dt, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal);
+}
+}  // namespace gp
+
+using namespace gp;
+void gpipe_set_error_(const std::string &s);
+
+static int sm_count_cached() {
+  static int n = 0;
+  if (!n) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+      n = 148;
+  }
+  return n;
+}
+static Ctx mk(void *stream, int backend = 0) {
+  return Ctx{(cudaStream_t)stream, nullptr, sm_count_cached(), backend};
+}
+static int ret(cudaError_t e, const char *where) {
+  if (e == cudaSuccess) return GPIPE_OK;
+  gpipe_set_error_(std::string(where) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")");
+  return e == cudaErrorInvalidValue || e == cudaErrorNotSupported ? GPIPE_EINVAL : GPIPE_ECUDA;
+}
+
+extern "C" {
+int gpipe_op_gemm(void *stream, int dtype, int M, int N, int K, const void *A, int64_t lda, int transA,
+                  const void *B, int64_t ldb, int transB, void *C, int64_t ldc, const float *bias,
+                  const float *resid, const void *mask, int64_t ldmask, int flags, int backend) {
+  GemmArgs g{};
+  g.M = M; g.N = N; g.K = K;
+  g.A = A; g.lda = lda; g.transA = transA;
+  g.B = B; g.ldb = ldb; g.transB = transB;
+  g.C = C; g.ldc = ldc;
+  g.bias = bias; g.resid = resid; g.mask = mask; g.ldmask = ldmask; g.flags = flags;
+  return ret(gemm(mk(stream, backend), dtype, g), "gpipe_op_gemm");
+}
+int gpipe_op_ln_fwd(void *stream, int dtype, const float *x, const float *gamma, const float *beta,
+                    void *y, float *mean, float *rstd, int64_t n_tok, int d, float eps) {
+  return ret(ln_fwd(mk(stream), dtype, x, gamma, beta, y, mean, rstd, n_tok, d, eps), "gpipe_op_ln_fwd");
+}
+int64_t gpipe_op_ln_bwd_scratch_floats(int d) {
+  return (int64_t)ln_bwd_partial_rows(sm_count_cached()) * 2 * d;
+}
+int gpipe_op_ln_bwd(void *stream, int dtype, const void *dy, const float *x, const float *mean,
+                    const float *rstd, const float *gamma, const float *dres_in, float *dx_out,
+                    void *dx_out_lp, float *partials, float *dgamma, float *dbeta, int64_t n_tok, int d) {
+  return ret(ln_bwd(mk(stream), dtype, dy, x, mean, rstd, gamma, dres_in, dx_out, dx_out_lp, partials,
+                    dgamma, dbeta, n_tok, d), "gpipe_op_ln_bwd");
+}
+int gpipe_op_attn_fwd(void *stream, int dtype, const void *qkv, void *o, float *lse, int n_seq, int S,
+                      int A, int dh, int causal, int backend) {
+  Ctx c = mk(stream);
+  return ret(backend == 1 ? attn_fwd_simt(c, dtype, qkv, o, lse, n_seq, S, A, dh, causal)
+                          : attn_fwd(c, dtype, qkv, o, lse, n_seq, S, A, dh, causal),
+             "gpipe_op_attn_fwd");
+}
+int gpipe_op_attn_bwd(void *stream, int dtype, const void *qkv, const void *o, const void *d_o,
+                      const float *lse, void *dqkv, float *dvec, int n_seq, int S, int A, int dh,
+                      int causal, int backend) {
+  Ctx c = mk(stream);
+  return ret(backend == 1
+                 ? attn_bwd_simt(c, dtype, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal)
+                 : attn_bwd(c, dtype, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal),
+             "gpipe_op_attn_bwd");
+}
+int gpipe_op_softmax_ce(void *stream, int dtype, void *logits, const int32_t *labels, float *rowloss,
+                        int64_t n_tok, int V, float inv_T) {
+  return ret(softmax_ce(mk(stream), dtype, logits, labels, rowloss, n_tok, V, inv_T), "gpipe_op_softmax_ce");
+}
+int gpipe_op_colsum(void *stream, int dtype, const void *dy, int64_t ld, float *out, int64_t n_tok, int n) {
+  return ret(colsum_accum(mk(stream), dtype, dy, ld, out, n_tok, n), "gpipe_op_colsum");
+}
+int gpipe_op_embed_fwd(void *stream, int dtype, const int32_t *tok, const void *emb, const float *pe,
+                       float *x, int64_t n_tok, int S, int d) {
+  return ret(embed_fwd(mk(stream), dtype, tok, emb, pe, x, n_tok, S, d), "gpipe_op_embed_fwd");
+}
+int gpipe_op_embed_bwd(void *stream, const int32_t *tok, const float *dx, float *gemb, int64_t n_tok, int d) {
+  return ret(embed_bwd(mk(stream), tok, dx, gemb, n_tok, d), "gpipe_op_embed_bwd");
+}
+int gpipe_op_positional(void *stream, float *pe, int S, int d) {
+  return ret(positional_table(mk(stream), pe, S, d), "gpipe_op_positional");
+}
+int gpipe_op_sgd(void *stream, int dtype, float *master, float *grad, void *w_lp, int64_t n, float lr) {
+  return ret(sgd_apply(mk(stream), dtype, master, grad, w_lp, n, lr), "gpipe_op_sgd");
+}
+}

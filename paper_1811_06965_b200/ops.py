@@ -1,0 +1,101 @@
+"""Thin wrappers of the per-kernel C entry points (include/gpipe_ops.h) on torch CUDA tensors.
+Marshalling only: pointers, sizes and the current stream are passed to the library."""
+from __future__ import annotations
+
+from typing import Optional
+
+from . import binding as B
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _dt(t) -> int:
+    torch = _torch()
+    if t.dtype == torch.bfloat16:
+        return B.DTYPE_BF16
+    if t.dtype == torch.float32:
+        return B.DTYPE_FP32
+    raise ValueError("lp tensors must be float32 or bfloat16")
+
+
+def _p(t):
+    return None if t is None else t.data_ptr()
+
+
+def _stream():
+    return _torch().cuda.current_stream().cuda_stream
+
+
+def gemm(A, B_, C, *, transA=False, transB=False, bias=None, resid=None, mask=None, relu=False,
+         accumulate=False, backend=0):
+    """C = epilogue(op(A) @ op(B)); shapes follow gpipe_op_gemm.  C is written in place."""
+    torch = _torch()
+    M, N = C.shape
+    K = A.shape[0] if transA else A.shape[1]
+    flags = 0
+    if bias is not None: flags |= B.EPI_BIAS
+    if relu: flags |= B.EPI_RELU
+    if mask is not None: flags |= B.EPI_MASK
+    if resid is not None: flags |= B.EPI_RESID
+    if accumulate: flags |= B.EPI_ACCUM
+    if C.dtype == torch.float32: flags |= B.EPI_OUT_F32
+    B._check(B.lib().gpipe_op_gemm(_stream(), _dt(A), M, N, K, _p(A), A.stride(0), int(transA), _p(B_),
+                                   B_.stride(0), int(transB), _p(C), C.stride(0), _p(bias), _p(resid),
+                                   _p(mask), mask.stride(0) if mask is not None else 0, flags, backend))
+    return C
+
+
+def ln_fwd(x, gamma, beta, y, mean, rstd, eps=1e-5):
+    n, d = x.shape
+    B._check(B.lib().gpipe_op_ln_fwd(_stream(), _dt(y), _p(x), _p(gamma), _p(beta), _p(y), _p(mean), _p(rstd), n, d, eps))
+
+
+def ln_bwd(dy, x, mean, rstd, gamma, dres_in, dx_out, dx_out_lp, dgamma, dbeta):
+    torch = _torch()
+    n, d = x.shape
+    scratch = torch.empty(B.lib().gpipe_op_ln_bwd_scratch_floats(d), dtype=torch.float32, device=x.device)
+    B._check(B.lib().gpipe_op_ln_bwd(_stream(), _dt(dy), _p(dy), _p(x), _p(mean), _p(rstd), _p(gamma), _p(dres_in),
+                                     _p(dx_out), _p(dx_out_lp), _p(scratch), _p(dgamma), _p(dbeta), n, d))
+    return scratch
+
+
+def attn_fwd(qkv, o, lse, n_seq, S, A, dh, causal, backend=0):
+    B._check(B.lib().gpipe_op_attn_fwd(_stream(), _dt(qkv), _p(qkv), _p(o), _p(lse), n_seq, S, A, dh, int(causal), backend))
+
+
+def attn_bwd(qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal, backend=0):
+    B._check(B.lib().gpipe_op_attn_bwd(_stream(), _dt(qkv), _p(qkv), _p(o), _p(d_o), _p(lse), _p(dqkv), _p(dvec),
+                                       n_seq, S, A, dh, int(causal), backend))
+
+
+def softmax_ce(logits, labels, rowloss, inv_T):
+    n, V = logits.shape
+    B._check(B.lib().gpipe_op_softmax_ce(_stream(), _dt(logits), _p(logits), _p(labels), _p(rowloss), n, V, inv_T))
+
+
+def colsum(dy, out):
+    n, c = dy.shape
+    B._check(B.lib().gpipe_op_colsum(_stream(), _dt(dy), _p(dy), dy.stride(0), _p(out), n, c))
+
+
+def embed_fwd(tok, emb, pe, x, S):
+    n, d = x.shape
+    B._check(B.lib().gpipe_op_embed_fwd(_stream(), _dt(emb), _p(tok), _p(emb), _p(pe), _p(x), n, S, d))
+
+
+def embed_bwd(tok, dx, gemb):
+    n, d = dx.shape
+    B._check(B.lib().gpipe_op_embed_bwd(_stream(), _p(tok), _p(dx), _p(gemb), n, d))
+
+
+def positional(pe):
+    S, d = pe.shape
+    B._check(B.lib().gpipe_op_positional(_stream(), _p(pe), S, d))
+
+
+def sgd(master, grad, w_lp, lr):
+    B._check(B.lib().gpipe_op_sgd(_stream(), B.DTYPE_BF16 if w_lp is not None else B.DTYPE_FP32, _p(master), _p(grad),
+                                  _p(w_lp), master.numel(), lr))

@@ -1,0 +1,91 @@
+"""CPU-side checks of the boundary: the shared library builds, loads and exports every symbol the
+headers declare; the host-only planner and argument validation work without a GPU."""
+import os
+import re
+
+import pytest
+
+import gpipe_inputs as gi
+import paper_1811_06965_b200 as gp
+from paper_1811_06965_b200 import binding, build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def built():
+    build.build()
+
+
+def _declared(header):
+    src = open(os.path.join(ROOT, "include", header)).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(gpipe_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported():
+    lib = gp.lib()
+    declared = _declared("gpipe.h") + _declared("gpipe_ops.h")
+    assert len(declared) >= 30
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert sorted(declared) == sorted(binding.EXPORTED_SYMBOLS)
+
+
+def test_version_and_error_string():
+    assert b"sm_100a" in gp.lib().gpipe_version()
+
+
+def _spec(w):
+    return gp.make_spec(w.n_layers, w.d_model, w.d_ffn, w.n_heads, w.d_head, w.vocab, w.seq_len, w.dtype,
+                        list(w.causal))
+
+
+def test_plan_bytes_follows_paper_memory_law():
+    """activations ~ N + (L/K)(N/M) with remat; ~ N*L without (tracker, no GPU)."""
+    w = gi.CONFIGS["T(12,8192,16)"]
+    spec, keep = _spec(w)
+    r = {M: gp.plan_bytes(spec, w.K, M, True, w.n_seqs) for M in (1, 4, 8, 16, 32)}
+    s = {M: gp.plan_bytes(spec, w.K, M, False, w.n_seqs) for M in (1, 4, 8, 16, 32)}
+    # a + b/M: successive differences are proportional to differences of 1/M
+    b1 = (r[1] - r[4]) / (1 - 1 / 4)
+    b2 = (r[8] - r[16]) / (1 / 8 - 1 / 16)
+    assert abs(b1 - b2) / b1 < 0.02
+    assert r[32] < r[1] / 5
+    assert max(s.values()) / min(s.values()) < 1.4          # ~ independent of M
+    assert s[32] > 5 * r[32]
+
+
+def test_config5_fits_180GB_with_remat():
+    w = gi.CONFIGS["T(64,16384,32)"]
+    spec, keep = _spec(w)
+    assert gp.plan_bytes(spec, w.K, w.M, True, w.n_seqs) < 180e9
+
+
+def test_invalid_arguments_are_rejected():
+    w = gi.CONFIGS["tiny"]
+    spec, keep = _spec(w)
+    with pytest.raises(gp.GPipeError) as e:
+        gp.plan_bytes(spec, 3, 4, True, 8)              # K > L
+    assert e.value.code == -1
+    with pytest.raises(gp.GPipeError):
+        gp.plan_bytes(spec, 2, 3, True, 8)              # 8 % 3 != 0: micro-batches must be equal
+    with pytest.raises(gp.GPipeError):
+        gp.plan_bytes(spec, 2, 0, True, 8)
+    bad, keep2 = gp.make_spec(2, 64, 256, 4, 24, 512, 16, "fp32")
+    with pytest.raises(gp.GPipeError):
+        gp.plan_bytes(bad, 2, 4, True, 8)               # unsupported d_head
+
+
+def test_product_does_not_import_oracle():
+    """The CUDA package must not reach into oracle/ (and vice versa)."""
+    pkg = os.path.join(ROOT, "paper_1811_06965_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, fn)).read()
+                assert "oracle" not in txt.replace("no oracle code", ""), fn
+    for fn in os.listdir(os.path.join(ROOT, "oracle")):
+        if fn.endswith(".py"):
+            assert "paper_1811_06965_b200" not in open(os.path.join(ROOT, "oracle", fn)).read().replace(
+                "CUDA path (paper_1811_06965_b200/)", "")

@@ -1,0 +1,279 @@
+"""End-to-end parity of the CUDA path (through the C ABI) against the CPU oracle, fp32 and bf16,
+plus the structural properties of the schedule, the tracker and the error paths.
+
+Tolerances (BASELINE.json north_star): fp32 - loss and per-tensor max-relative gradient error
+<= 1e-4 (TF32 off); bf16 - loss within 1e-2 relative, per-tensor gradient cosine >= 0.999.
+"""
+import numpy as np
+import pytest
+
+import gpipe_inputs as gi
+import paper_1811_06965_b200 as gp
+from oracle import schedule as sch
+from tests.util import cosine, maxrel, run_oracle
+
+pytestmark = pytest.mark.gpu
+
+FP32_TOL = 1e-4
+
+
+def _engine(w, **kw):
+    return gp.from_workload(w, **kw)
+
+
+def _tiny(causal=(1, 1), **kw):
+    return gi.CONFIGS["tiny"].replace(causal=tuple(causal), **kw)
+
+
+def _compare_fp32(w, K, M, remat, seed_p=1001, seed_t=2001):
+    params = gi.make_params(w, seed_p, round_bf16=False)
+    tok, lab = gi.make_tokens(w, seed_t)
+    o, loss_ref = run_oracle(w, params, tok, lab, K=K, M=M, remat=remat)
+    with _engine(w, K=K, M=M, remat=remat) as e:
+        e.set_params(params)
+        loss = e.step(tok, lab)
+        assert abs(loss - loss_ref) <= FP32_TOL * abs(loss_ref), (loss, loss_ref)
+        worst = 0.0
+        for n in e.names:
+            err = maxrel(e.get_grad(n), o.g[n])
+            worst = max(worst, err)
+            assert err <= FP32_TOL, (n, err)
+    return worst
+
+
+@pytest.mark.parametrize("causal", [(1, 1), (0, 1), (0, 0)])
+def test_config1_tiny_fp32_parity(causal):
+    """BASELINE.json configs[0]: 2 layers, d 64, FFN 256, 4 heads, vocab 512, seq 16, N 8, M 4, K 2."""
+    _compare_fp32(_tiny(causal), 2, 4, True)
+
+
+@pytest.mark.parametrize("K,M,remat", [(1, 1, False), (1, 8, True), (2, 1, True), (2, 2, False),
+                                         (2, 8, True), (2, 4, False)])
+def test_fp32_parity_over_K_M_remat(K, M, remat):
+    _compare_fp32(_tiny((0, 1)), K, M, remat)
+
+
+def test_fp32_parity_uneven_cells_and_ragged_shapes():
+    """L % K != 0 (first cells get the extra layer), S not a multiple of 32, d_head 32."""
+    w = gi.CONFIGS["tiny"].replace(n_layers=5, causal=(0, 1, 0, 1, 1), d_model=96, n_heads=3, d_head=32,
+                                   d_ffn=200, vocab=1000, seq_len=40, n_seqs=6, M=3, K=3)
+    _compare_fp32(w, 3, 3, True)
+    _compare_fp32(w, 2, 2, False)
+
+
+def test_zero_layer_model():
+    w = gi.CONFIGS["tiny"].replace(n_layers=0, causal=(), K=1, M=2)
+    _compare_fp32(w, 1, 2, True)
+
+
+def test_gradients_independent_of_K_M_remat_on_gpu():
+    """PAPER.md:45/:67/:209 on the GPU itself; dE uses float atomics so not bitwise."""
+    w = _tiny((0, 1))
+    params = gi.make_params(w, 1001, round_bf16=False)
+    tok, lab = gi.make_tokens(w, 2001)
+    ref = None
+    for K, M, remat in [(1, 1, False), (2, 4, True), (2, 8, False), (1, 2, True)]:
+        with _engine(w, K=K, M=M, remat=remat) as e:
+            e.set_params(params)
+            loss = e.step(tok, lab)
+            g = e.grads()
+        if ref is None:
+            ref = (loss, g)
+            continue
+        assert abs(loss - ref[0]) <= 1e-6 * abs(ref[0])
+        for n in g:
+            assert maxrel(g[n], ref[1][n]) <= 1e-5, (K, M, remat, n)
+
+
+def test_remat_equals_stored_bitwise_on_gpu():
+    """replayed activations are bit-identical, so every gradient that is summed in
+    a fixed order is bit-identical (everything except the atomically accumulated embedding)."""
+    w = _tiny((0, 1))
+    params = gi.make_params(w, 1001, round_bf16=False)
+    tok, lab = gi.make_tokens(w, 2001)
+    out = []
+    for remat in (True, False):
+        with _engine(w, remat=remat) as e:
+            e.set_params(params)
+            out.append((e.step(tok, lab), e.grads()))
+    assert out[0][0] == out[1][0]
+    for n in out[0][1]:
+        if n != "emb":
+            assert np.array_equal(out[0][1][n], out[1][1][n]), n
+
+
+def test_step_accumulates_and_sgd_applies():
+    w = _tiny()
+    params = gi.make_params(w, 1001, round_bf16=False)
+    tok, lab = gi.make_tokens(w, 2001)
+    with _engine(w) as e:
+        e.set_params(params)
+        l0 = e.step(tok, lab)
+        g1 = e.grads()
+        e.step(tok, lab)
+        g2 = e.grads()
+        for n in g1:
+            assert maxrel(g2[n], 2 * g1[n]) <= 1e-6, n
+        e.zero_grads()
+        assert not any(e.get_grad(n).any() for n in e.names)
+        e.step(tok, lab)
+        g = e.grads()
+        before = {n: e.get_param(n) for n in e.names}
+        e.apply_sgd(0.5)
+        for n in e.names:
+            assert np.array_equal(e.get_param(n), before[n] - np.float32(0.5) * g[n]), n
+            assert not e.get_grad(n).any()
+        assert e.step(tok, lab) < l0
+        # the oracle agrees on the updated parameters and the second loss
+        o, _ = run_oracle(w, params, tok, lab, dtype=np.float32)
+        o.apply_sgd(0.5)
+        for n in e.names:
+            assert maxrel(e.get_param(n), o.p[n]) <= 1e-5, n
+
+
+def test_device_resident_inputs_match_host_inputs():
+    import torch
+    w = _tiny()
+    params = gi.make_params(w, 1001, round_bf16=False)
+    tok, lab = gi.make_tokens(w, 2001)
+    with _engine(w) as e:
+        e.set_params(params)
+        l_host = e.step(tok, lab)
+        g_host = e.grads()
+        e.zero_grads()
+        l_dev = e.step(torch.tensor(tok, device="cuda"), torch.tensor(lab, device="cuda"))
+        assert l_dev == l_host
+        for n in e.names:
+            if n != "emb":
+                assert np.array_equal(e.get_grad(n), g_host[n])
+        bad = torch.tensor(tok, device="cuda").clone()
+        bad[0, 0] = w.vocab
+        with pytest.raises(gp.GPipeError):
+            e.step(bad, torch.tensor(lab, device="cuda"))
+
+
+def test_error_paths():
+    w = _tiny()
+    tok, lab = gi.make_tokens(w, 2001)
+    with _engine(w) as e:
+        bad = tok.copy()
+        bad[1, 2] = -1
+        with pytest.raises(gp.GPipeError) as err:
+            e.step(bad, lab)
+        assert err.value.code == -1
+        with pytest.raises(ValueError):
+            e.step(tok[:4], lab[:4])
+    with pytest.raises(gp.GPipeError):
+        _engine(w, K=3)
+    with pytest.raises(gp.GPipeError):
+        _engine(w, M=3)
+
+
+def test_trace_is_a_valid_gpipe_schedule():
+    """Every task of Fig. 2c appears once; per-cell program order and cross-cell dependencies
+    hold in device time; with M = 1 at most one cell is busy."""
+    w = _tiny()
+    params = gi.make_params(w, 1001, round_bf16=False)
+    tok, lab = gi.make_tokens(w, 2001)
+    for K, M, remat in [(2, 4, True), (2, 4, False), (2, 1, True)]:
+        with _engine(w, K=K, M=M, remat=remat) as e:
+            e.set_params(params)
+            e.trace(True)
+            e.step(tok, lab)
+            ev = e.trace_events()
+        tasks = {(kind, k, m): (s, t, idx) for kind, k, m, idx, s, t in ev}
+        want = set()
+        for k in range(K):
+            want |= set(sch.cell_program(k, K, M, remat))
+        assert set(tasks) == want and len(ev) == len(want)
+        for (kind, k, m), (s, t, idx) in tasks.items():
+            assert t >= s
+            for dep in sch.dependencies((kind, k, m), K, remat, early=True):
+                assert tasks[dep][1] <= s + 1e-3, ((kind, k, m), dep)
+        for k in range(K):
+            prog = sorted([(v[2], key) for key, v in tasks.items() if key[1] == k])
+            assert [key for _, key in prog] == sch.cell_program(k, K, M, remat)
+            times = [tasks[key] for _, key in prog]
+            for a, b in zip(times, times[1:]):
+                assert a[1] <= b[0] + 1e-3                  # a stream is an in-order queue
+        if M == 1:
+            spans = sorted((s, t) for s, t, _ in tasks.values())
+            for a, b in zip(spans, spans[1:]):
+                assert a[1] <= b[0] + 1e-3
+
+
+def test_peak_bytes_tracker():
+    w = _tiny(n_seqs=8)
+    peaks = {}
+    for M in (1, 2, 4, 8):
+        with _engine(w, M=M, remat=True) as e:
+            p = e.peak_bytes()
+            assert p["total"] == sum(p["by_category"].values())
+            assert p["total"] <= e.arena.numel()
+            peaks[M] = p["by_category"]["interior"]
+    assert peaks[1] > peaks[2] > peaks[4] > peaks[8]
+    with _engine(w, M=8, remat=False) as e:
+        assert e.peak_bytes()["by_category"]["interior"] > 4 * peaks[8]
+
+
+def test_device_init_params_statistics():
+    w = gi.CONFIGS["tiny"].replace(d_model=256, d_ffn=1024, n_heads=4, d_head=64, vocab=4096)
+    with _engine(w) as e:
+        e.init_params(seed=7, std=0.02, parity=False)
+        wq = e.get_param("l0.w_qkv")
+        assert abs(wq.std() - 0.02) < 5e-4 and abs(wq.mean()) < 2e-4
+        assert np.array_equal(e.get_param("l0.ln1_g"), np.ones((1, 256), np.float32))
+        assert not e.get_param("l0.b_1").any()
+        emb = e.get_param("emb")
+        assert abs(np.corrcoef(emb[0], emb[1])[0, 1]) < 0.2
+        e.init_params(seed=7, std=0.02, parity=True)
+        assert abs(e.get_param("l1.ln2_g").mean() - 1.0) < 5e-3
+        assert abs(e.get_param("l1.b_1").std() - 0.02) < 2e-3
+        tok, lab = gi.make_tokens(w, 5)
+        loss = e.step(tok, lab)
+        assert abs(loss - (np.log(w.vocab) + 0.5 * 0.02 ** 2 * w.d_model)) < 0.05   # P7 closed form
+
+
+# -------------------------------------------------------------------------------------------------
+# bf16
+# -------------------------------------------------------------------------------------------------
+def _bf16_small():
+    # a scaled-down T(L,H,A): same structure as configs[1], sized for the oracle (seconds)
+    return gi.CONFIGS["T(6,4096,16)"].replace(name="bf16-small", n_layers=2, d_model=256, d_ffn=1024, n_heads=4,
+                                              d_head=64, vocab=2048, seq_len=64, n_seqs=8, M=4, K=2,
+                                              causal=(0, 1))
+
+
+def test_bf16_end_to_end_parity_small():
+    w = _bf16_small()
+    params = gi.make_params(w, 1002)                        # bf16-representable (A12)
+    tok, lab = gi.make_tokens(w, 2002)
+    o, loss_ref = run_oracle(w, params, tok, lab)
+    with _engine(w) as e:
+        e.set_params(params)
+        for n in e.names:                                   # both sides start from identical values
+            assert np.array_equal(e.get_param(n), params[n]), n
+        loss = e.step(tok, lab)
+        assert abs(loss - loss_ref) <= 1e-2 * abs(loss_ref)
+        cos = {n: cosine(e.get_grad(n), o.g[n]) for n in e.names}
+    assert min(cos.values()) >= 0.999, sorted(cos.items(), key=lambda kv: kv[1])[:5]
+
+
+def test_bf16_invariance_over_M_and_remat():
+    """Per-token forward values do not depend on the micro-batch split (deterministic K-loop
+    order), so gradients agree to fp32 summation-order level across (K, M, remat)."""
+    w = _bf16_small()
+    params = gi.make_params(w, 1002)
+    tok, lab = gi.make_tokens(w, 2002)
+    ref = None
+    for K, M, remat in [(2, 4, True), (2, 4, False), (1, 2, True), (2, 8, True)]:
+        with _engine(w, K=K, M=M, remat=remat) as e:
+            e.set_params(params)
+            loss = e.step(tok, lab)
+            g = e.grads()
+        if ref is None:
+            ref = (loss, g)
+            continue
+        assert abs(loss - ref[0]) <= 1e-5 * abs(ref[0])
+        for n in g:
+            assert maxrel(g[n], ref[1][n]) <= 2e-3, (K, M, remat, n, maxrel(g[n], ref[1][n]))

@@ -1,0 +1,226 @@
+"""Per-kernel ("teacher-forced") parity: each CUDA kernel, called through the C ABI of
+include/gpipe_ops.h, against the oracle's operator on identical inputs.  fp32 kernels must agree to
+fp32 rounding; bf16 kernels get bf16-representable inputs and must agree to output rounding
+(<= 2^-7 max-rel, cosine >= 0.99999)."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import gpipe_inputs as gi
+from oracle import gpipe_oracle as go
+from paper_1811_06965_b200 import ops
+from tests.util import cosine, maxrel
+
+pytestmark = pytest.mark.gpu
+
+DEV = "cuda"
+
+
+def _rng(seed):
+    return np.random.Generator(np.random.PCG64(seed))
+
+
+def _lp(a, dtype):
+    """host fp array -> device lp tensor and the exact fp64 values it holds"""
+    if dtype == "bf16":
+        a = gi.bf16_round(a.astype(np.float32))
+        return torch.tensor(a, device=DEV).to(torch.bfloat16), a.astype(np.float64)
+    a = a.astype(np.float32)
+    return torch.tensor(a, device=DEV), a.astype(np.float64)
+
+
+def _np(t):
+    return t.detach().float().cpu().numpy().astype(np.float64)
+
+
+def _tol(dtype):
+    return (2e-5, 0.9999999) if dtype == "fp32" else (2 ** -7, 0.99999)
+
+
+# -------------------------------------------------------------------------------------------------
+# GEMM
+# -------------------------------------------------------------------------------------------------
+GEMM_SHAPES = [(32, 64, 48), (70, 130, 33), (128, 128, 64), (256, 192, 128), (1, 8, 8)]
+
+
+@pytest.mark.parametrize("dtype", ["fp32", "bf16"])
+@pytest.mark.parametrize("transA,transB", [(0, 0), (0, 1), (1, 0), (1, 1)])
+def test_gemm_simt_all_layouts(dtype, transA, transB):
+    for (M, N, K) in GEMM_SHAPES:
+        r = _rng(M * 1000 + N + K)
+        A = r.standard_normal((K, M) if transA else (M, K))
+        B = r.standard_normal((N, K) if transB else (K, N))
+        At, Aq = _lp(A, dtype)
+        Bt, Bq = _lp(B, dtype)
+        C = torch.empty((M, N), device=DEV, dtype=At.dtype)
+        ops.gemm(At, Bt, C, transA=bool(transA), transB=bool(transB), backend=1)
+        ref = (Aq.T if transA else Aq) @ (Bq.T if transB else Bq)
+        tol, cos = _tol(dtype)
+        assert maxrel(_np(C), ref) <= tol, (M, N, K)
+        assert cosine(_np(C), ref) >= cos
+
+
+@pytest.mark.parametrize("dtype", ["fp32", "bf16"])
+@pytest.mark.parametrize("backend", [1, 0])
+def test_gemm_epilogues(dtype, backend):
+    """bias+ReLU (a10), bias+residual fp32 out (a8/a11), ReLU-mask (a16 dh), fp32 accumulate (a18)."""
+    M, N, K = 256, 384, 128
+    r = _rng(5)
+    At, Aq = _lp(r.standard_normal((M, K)), dtype)
+    Bt, Bq = _lp(r.standard_normal((K, N)), dtype)
+    bias = r.standard_normal(N).astype(np.float32)
+    resid = r.standard_normal((M, N)).astype(np.float32)
+    maskt, maskq = _lp(np.maximum(r.standard_normal((M, N)), 0), dtype)
+    bt, rt = torch.tensor(bias, device=DEV), torch.tensor(resid, device=DEV)
+    tol, cos = _tol(dtype)
+    ref = Aq @ Bq
+    C = torch.empty((M, N), device=DEV, dtype=At.dtype)
+    ops.gemm(At, Bt, C, bias=bt, relu=True, backend=backend)
+    assert maxrel(_np(C), np.maximum(ref + bias, 0)) <= tol
+    Cf = torch.empty((M, N), device=DEV, dtype=torch.float32)
+    ops.gemm(At, Bt, Cf, bias=bt, resid=rt, backend=backend)
+    assert maxrel(_np(Cf), ref + bias + resid) <= 2e-5
+    ops.gemm(At, Bt, rt, bias=bt, resid=rt, backend=backend)            # residual aliasing the output
+    assert maxrel(_np(rt), ref + bias + resid) <= 2e-5
+    ops.gemm(At, Bt, C, mask=maskt, backend=backend)
+    assert maxrel(_np(C), ref * (maskq > 0)) <= tol
+    acc0 = r.standard_normal((K, N)).astype(np.float32)
+    acc = torch.tensor(acc0, device=DEV)
+    Xt, Xq = _lp(r.standard_normal((M, K)), dtype)
+    Yt, Yq = _lp(r.standard_normal((M, N)), dtype)
+    ops.gemm(Xt, Yt, acc, transA=True, accumulate=True, backend=backend)  # dW += X^T dY
+    ops.gemm(Xt, Yt, acc, transA=True, accumulate=True, backend=backend)
+    assert maxrel(_np(acc), acc0 + 2 * (Xq.T @ Yq)) <= 2e-5
+
+
+# -------------------------------------------------------------------------------------------------
+# LayerNorm
+# -------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["fp32", "bf16"])
+@pytest.mark.parametrize("n,d", [(7, 64), (130, 1024), (33, 96), (5, 2048)])
+def test_layernorm_fwd_bwd(dtype, n, d):
+    r = _rng(n * d)
+    x = (r.standard_normal((n, d)) * 2 + 0.5).astype(np.float32)
+    g = (1 + 0.1 * r.standard_normal((1, d))).astype(np.float32)
+    b = (0.1 * r.standard_normal((1, d))).astype(np.float32)
+    dyt, dyq = _lp(r.standard_normal((n, d)), dtype)
+    dres = r.standard_normal((n, d)).astype(np.float32)
+    y_ref, xhat, rstd = go.layernorm_fwd(x.astype(np.float64), g.astype(np.float64), b.astype(np.float64), 1e-5)
+    dx_ref, dg_ref, db_ref = go.layernorm_bwd(dyq, xhat, rstd, g.astype(np.float64))
+    xt, gt, bt = [torch.tensor(a, device=DEV) for a in (x, g, b)]
+    y = torch.empty((n, d), device=DEV, dtype=dyt.dtype)
+    mean = torch.empty(n, device=DEV)
+    rs = torch.empty(n, device=DEV)
+    ops.ln_fwd(xt, gt, bt, y, mean, rs)
+    tol, cos = _tol(dtype)
+    assert maxrel(_np(y), y_ref) <= tol
+    assert maxrel(_np(rs), rstd[:, 0]) <= 1e-5 and maxrel(_np(mean), x.astype(np.float64).mean(1)) <= 1e-5
+    dx = torch.empty((n, d), device=DEV)
+    dx_lp = torch.empty((n, d), device=DEV, dtype=dyt.dtype) if dtype == "bf16" else None
+    dg0 = r.standard_normal(d).astype(np.float32)
+    dgt, dbt = torch.tensor(dg0, device=DEV), torch.zeros(d, device=DEV)
+    ops.ln_bwd(dyt, xt, mean, rs, gt, torch.tensor(dres, device=DEV), dx, dx_lp, dgt, dbt)
+    assert maxrel(_np(dx), dx_ref + dres) <= 2e-5
+    if dx_lp is not None:
+        assert maxrel(_np(dx_lp), dx_ref + dres) <= 2 ** -7
+    assert maxrel(_np(dgt), dg0 + dg_ref[0]) <= 2e-5          # accumulates into dgamma
+    assert maxrel(_np(dbt), db_ref[0]) <= 2e-5
+    ops.ln_bwd(dyt, xt, mean, rs, gt, None, dx, None, dgt, dbt)   # no incoming residual gradient
+    assert maxrel(_np(dx), dx_ref) <= 2e-5
+
+
+# -------------------------------------------------------------------------------------------------
+# attention
+# -------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["fp32", "bf16"])
+@pytest.mark.parametrize("S,A,dh", [(16, 4, 16), (40, 3, 32), (256, 2, 64), (100, 2, 64)])
+@pytest.mark.parametrize("causal", [0, 1])
+def test_attention_fwd_bwd(dtype, S, A, dh, causal):
+    n_seq, da = 2, A * dh
+    r = _rng(S * A + dh + causal)
+    qkvt, qkvq = _lp(r.standard_normal((n_seq * S, 3 * da)), dtype)
+    dot, doq = _lp(r.standard_normal((n_seq * S, da)), dtype)
+    o = torch.empty((n_seq * S, da), device=DEV, dtype=qkvt.dtype)
+    lse = torch.empty((n_seq, A, S), device=DEV)
+    ops.attn_fwd(qkvt, o, lse, n_seq, S, A, dh, causal)
+    dqkv = torch.empty_like(qkvt)
+    dvec = torch.empty((n_seq, A, S), device=DEV)
+    ops.attn_bwd(qkvt, o, dot, lse, dqkv, dvec, n_seq, S, A, dh, causal)
+    tol, cos = _tol(dtype)
+    if dtype == "bf16":
+        tol = 2 ** -6                                   # P and dS are rounded to bf16 on tensor cores
+    for b in range(n_seq):
+        rows = slice(b * S, (b + 1) * S)
+        q, k, v = qkvq[rows, :da], qkvq[rows, da:2 * da], qkvq[rows, 2 * da:]
+        o_ref, ps = go.attention_fwd(q, k, v, A, dh, causal)
+        assert maxrel(_np(o[rows]), o_ref) <= tol
+        for h in range(A):
+            s = (q[:, h * dh:(h + 1) * dh] @ k[:, h * dh:(h + 1) * dh].T) / math.sqrt(dh)
+            if causal:
+                s = np.where(np.tril(np.ones((S, S), bool)), s, -np.inf)
+            lse_ref = np.log(np.exp(s - s.max(1, keepdims=True)).sum(1)) + s.max(1)
+            assert np.abs(_np(lse[b, h]) - lse_ref).max() <= 1e-4
+        # backward against the oracle with the kernel's own forward output as O (teacher-forced)
+        dq, dk, dv = go.attention_bwd(doq[rows], q, k, v, ps, A, dh)
+        got = _np(dqkv[rows])
+        for name, ref, blk in (("dq", dq, 0), ("dk", dk, 1), ("dv", dv, 2)):
+            assert maxrel(got[:, blk * da:(blk + 1) * da], ref) <= 4 * tol, name
+            assert cosine(got[:, blk * da:(blk + 1) * da], ref) >= (cos if dtype == "fp32" else 0.9999), name
+
+
+# -------------------------------------------------------------------------------------------------
+# softmax cross-entropy, column sums, embedding, SGD
+# -------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["fp32", "bf16"])
+@pytest.mark.parametrize("n,V", [(9, 512), (33, 32000), (4, 64000), (3, 1000)])
+def test_softmax_ce(dtype, n, V):
+    r = _rng(V + n)
+    zt, zq = _lp(r.standard_normal((n, V)) * 3, dtype)
+    labels = r.integers(0, V, size=n).astype(np.int32)
+    rowloss = torch.empty(n, device=DEV)
+    inv_T = 1.0 / 77
+    loss_ref, dl_ref = go.softmax_ce(zq, labels, 77)
+    ops.softmax_ce(zt, torch.tensor(labels, device=DEV), rowloss, inv_T)
+    assert abs(float(rowloss.double().sum()) - loss_ref) <= 2e-5 * abs(loss_ref)
+    tol, cos = _tol(dtype)
+    assert maxrel(_np(zt), dl_ref) <= tol
+    assert cosine(_np(zt), dl_ref) >= cos
+
+
+@pytest.mark.parametrize("dtype", ["fp32", "bf16"])
+def test_colsum_embedding_sgd(dtype):
+    r = _rng(11)
+    dyt, dyq = _lp(r.standard_normal((300, 200)), dtype)
+    out0 = r.standard_normal(200).astype(np.float32)
+    out = torch.tensor(out0, device=DEV)
+    ops.colsum(dyt, out)
+    assert maxrel(_np(out), out0 + dyq.sum(0)) <= 2e-5
+    # embedding forward/backward (reading A6)
+    V, d, S, n_seq = 50, 64, 10, 3
+    embt, embq = _lp(r.standard_normal((V, d)), dtype)
+    tok = r.integers(0, V, size=n_seq * S).astype(np.int32)
+    pe = torch.empty((S, d), device=DEV)
+    ops.positional(pe)
+    assert maxrel(_np(pe), go.positional_table(S, d, np.float64)) <= 1e-6
+    x = torch.empty((n_seq * S, d), device=DEV)
+    tt = torch.tensor(tok, device=DEV)
+    ops.embed_fwd(tt, embt, pe, x, S)
+    assert maxrel(_np(x), embq[tok] + np.tile(go.positional_table(S, d, np.float64), (n_seq, 1))) <= 1e-6
+    dx = r.standard_normal((n_seq * S, d)).astype(np.float32)
+    gemb = torch.zeros((V, d), device=DEV)
+    ops.embed_bwd(tt, torch.tensor(dx, device=DEV), gemb)
+    ref = np.zeros((V, d))
+    np.add.at(ref, tok, dx.astype(np.float64))
+    assert maxrel(_np(gemb), ref) <= 1e-5
+    # SGD apply
+    n = 4096
+    m0, g0 = r.standard_normal(n).astype(np.float32), r.standard_normal(n).astype(np.float32)
+    m, g = torch.tensor(m0, device=DEV), torch.tensor(g0, device=DEV)
+    wl = torch.empty(n, device=DEV, dtype=torch.bfloat16) if dtype == "bf16" else None
+    ops.sgd(m, g, wl, 0.25)
+    assert np.array_equal(m.cpu().numpy(), m0 - np.float32(0.25) * g0)
+    assert not g.any()
+    if wl is not None:
+        assert torch.equal(wl, m.to(torch.bfloat16))

@@ -1,0 +1,314 @@
+#!/usr/bin/env python
+"""bench.py - tokens/s of one GPipe mini-batch step (forward + re-materialized backward, fp32
+gradient accumulation) on B200, through the C ABI of libgpipe_b200.so.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl ours|reference]
+
+One "step" is one pass of the whole hot path (every row of SURVEY.md 8(a): micro-batch split,
+all forward ticks, all replay + backward ticks, gradient accumulation) over one synthetic
+mini-batch.  `value` is measured with the token ids already resident in HBM
+(gpipe_step_device); `e2e` is the same step called with HOST id buffers (gpipe_step: H2D of
+the ids and D2H of the loss partials inside the timed region).  The default workload is
+BASELINE.json's T(64,16384,32) configuration - the one its target is quoted on; it fits one GPU.
+Prints ONE JSON line on rank 0.  `--impl reference` times the CPU oracle on a bounded sample
+(see DESIGN.md "Measurement").  N > 1: independent replicas, no collective (the
+north star fixes "no sharding across GPUs and no collectives").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import gpipe_inputs as gi  # noqa: E402
+
+METRIC = "tokens_per_sec_fwd_bwd"
+UNIT = "tokens/s"
+DEFAULT_WORKLOAD = "T(64,16384,32)"
+
+
+# ---------------------------------------------------------------------------------------------
+# FLOP model
+# ---------------------------------------------------------------------------------------------
+def flops_per_step(w, replay_skips_last_ffn2=True):
+    d, H, da, V, S = w.d_model, w.d_ffn, w.d_attn, w.vocab, w.seq_len
+    T = w.tokens_per_step
+    f_qkv, f_o, f_1, f_2 = 2 * d * 3 * da, 2 * da * d, 2 * d * H, 2 * H * d
+    f_g = f_qkv + f_o + f_1 + f_2
+    f_v = 2 * d * V
+    fa = [4 * S * da * ((S + 1) / (2 * S) if c else 1.0) for c in w.causal]
+    fwd = sum(f_g + a for a in fa) + f_v
+    bwd = sum(2 * f_g + 2.5 * a for a in fa) + 2 * f_v
+    model = (fwd + bwd) * T
+    replay = 0.0
+    if w.remat:
+        replay = sum(f_g + a for a in fa) + f_v          # the head is replayed with its cell
+        if replay_skips_last_ffn2:
+            replay -= (w.K - 1) * f_2                     # cells 0..K-2 skip their last FFN2 in replay
+        replay *= T
+    return {"model": model, "executed": model + replay}
+
+
+# ---------------------------------------------------------------------------------------------
+# clocks
+# ---------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "200"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()                      # the exact PID we started
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except Exception:
+            self.p.kill()
+            out = ""
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        j = json.load(open(p))
+        return {"burst": j["bf16_tflops"], "sustained": j.get("bf16_tflops_sustained", j["bf16_tflops"]),
+                "hbm": j["hbm_gbs"], "src": "measured"}
+    return {"burst": 1590.0, "sustained": 1400.0, "hbm": 6650.0, "src": "fallback"}
+
+
+# ---------------------------------------------------------------------------------------------
+# the oracle arm (cpu_baseline and --impl reference)
+# ---------------------------------------------------------------------------------------------
+def oracle_sample(w, repeats=2):
+    """Times the CPU oracle, as it stands, on a bounded sample of the workload: ONE sequence
+    through a 2-layer / 2-cell model of the same d, H, A, d_head, V, S (forward, replay,
+    backward, head), and through the 0-layer model (embedding + head only); per-layer and head
+    costs are separated and extrapolated linearly to the full depth (gradients are sums of
+    independent per-sequence terms, so cost is linear in sequences and layers)."""
+    from oracle import gpipe_oracle as go
+    try:
+        from threadpoolctl import threadpool_info
+        cores = max([i.get("num_threads", 1) for i in threadpool_info()] + [1])
+    except Exception:
+        cores = os.cpu_count() or 1
+
+    def run(L):
+        causal = tuple(w.causal[i * len(w.causal) // L] for i in range(L)) if L else ()
+        ww = w.replace(n_layers=L, causal=causal, n_seqs=1, M=1, K=max(1, min(L, 2)))
+        params = gi.make_params(ww, 1, parity=False, round_bf16=False)
+        tok, lab = gi.make_tokens(ww, 2)
+        o = go.GPipeOracle(go.Spec(ww.n_layers, ww.d_model, ww.d_ffn, ww.n_heads, ww.d_head, ww.vocab,
+                                   ww.seq_len, ww.causal, ww.ln_eps), ww.K, 1, ww.remat, dtype=np.float32)
+        o.set_params(params)
+        o.step(tok, lab)                                    # BLAS thread pool / page-fault warm-up
+        best = 1e30
+        for _ in range(repeats):
+            t0 = time.perf_counter()
+            o.step(tok, lab)
+            best = min(best, time.perf_counter() - t0)
+        return best
+
+    nl = min(4, w.n_layers)
+    t_head = run(0)
+    t_some = run(nl) if nl else t_head
+    t_layer = max(t_some - t_head, 0.0) / max(nl, 1)
+    t_seq = t_head + w.n_layers * t_layer                   # one sequence through the full depth
+    value = w.seq_len / t_seq
+    return {"value": value, "unit": UNIT, "cores": int(cores), "kind": "oracle",
+            "sample": "fp32 numpy oracle step (forward, replay, backward) on 1 sequence of %d tokens: 0-layer model "
+                      "(embedding+head) %.3fs, %d-layer/2-cell model %.3fs; per-layer cost extrapolated linearly to "
+                      "%d layers" % (w.seq_len, t_head, nl, t_some, w.n_layers),
+            "seconds": t_head + t_some}
+
+
+def run_reference(args, w, rank, world):
+    if rank != 0:
+        return
+    times = []
+    res = None
+    for i in range(args.warmup + args.steps):
+        res = oracle_sample(w)
+        if i >= args.warmup:
+            times.append(res["value"])
+    value = float(np.mean(times))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * w.tokens_per_step / value,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "K": w.K, "M": w.M, "remat": w.remat, "n_seqs": w.n_seqs,
+                       "seq_len": w.seq_len},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": res["cores"], "kind": "oracle",
+                             "sample": res["sample"]},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------
+def run_ours(args, w, rank, world, local_rank):
+    import torch
+    import paper_1811_06965_b200 as gp
+    from paper_1811_06965_b200 import build
+    from paper_1811_06965_b200.dist_util import max_over_ranks, barrier
+
+    if rank == 0:
+        build.build()
+    barrier(world)
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    peaks = measured_peaks()
+    eng = gp.from_workload(w, device=dev)
+    eng.init_params(seed=1000 + rank, std=0.02, parity=False)
+    tok, lab = gi.make_tokens(w, 2000 + rank)
+    tok_d, lab_d = torch.tensor(tok, device=dev), torch.tensor(lab, device=dev)
+    tok_h = torch.tensor(tok).pin_memory().numpy()
+    lab_h = torch.tensor(lab).pin_memory().numpy()
+    s0 = eng.streams[0]
+
+    def timed(fn, steps):
+        barrier(world)
+        torch.cuda.synchronize(dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(s0)                       # the engine starts and joins every step on stream 0
+        for _ in range(steps):
+            fn()                            # gradients keep accumulating (no apply in fwd+bwd)
+        e1.record(s0)
+        torch.cuda.synchronize(dev)
+        barrier(world)
+        return max_over_ranks(e0.elapsed_time(e1), world)
+
+    loss = None
+    for _ in range(args.warmup):
+        loss = eng.step(tok_d, lab_d)
+        eng.zero_grads()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    l0 = eng.launch_count()
+    ms = timed(lambda: eng.step(tok_d, lab_d), args.steps)
+    launches = (eng.launch_count() - l0)
+    clocks = sampler.stop() if sampler else None
+    ms_e2e = timed(lambda: eng.step(tok_h, lab_h), args.steps)
+    # one extra step with per-launch CUDA events for the roofline of the dominant kernel class
+    eng.kernel_timing(True)
+    eng.step(tok_d, lab_d)
+    stats = eng.kernel_stats()
+    eng.kernel_timing(False)
+    eng.zero_grads()
+    peak_hbm = eng.peak_bytes()
+
+    tokens = w.tokens_per_step * world
+    value = tokens * args.steps / (ms / 1e3)
+    fl = flops_per_step(w, replay_skips_last_ffn2=not int(os.environ.get("GPIPE_REPLAY_FULL", "0")))
+    step_s = ms / 1e3 / args.steps
+    gem = {k: stats[k] for k in ("gemm_fwd", "gemm_dgrad", "gemm_wgrad")}
+    gem_ms = sum(v["ms"] for v in gem.values())
+    gem_fl = sum(v["flops"] for v in gem.values())
+    tot_ms = sum(v["ms"] for v in stats.values())
+    achieved = gem_fl / (gem_ms / 1e3) / 1e12 if gem_ms > 0 else 0.0
+    roofline = {"bound": "tensor", "kernel": "gemm_tcgen05_kernel (fwd + dgrad + wgrad launches)",
+                "achieved": achieved, "peak": peaks["sustained"], "unit": "TFLOP/s",
+                "frac": achieved / peaks["sustained"], "peak_src": peaks["src"] + " sustained bf16 (kernel timed inside a long step)",
+                "traffic": None, "launches": int(sum(v["launches"] for v in gem.values())),
+                "share_of_kernel_time": gem_ms / tot_ms if tot_ms else None,
+                "per_class": {k: {"launches": int(v["launches"]), "ms": round(v["ms"], 3),
+                                  "tflops": (v["flops"] / v["ms"] / 1e9) if v["ms"] > 0 and v["flops"] > 0 else None,
+                                  "gbs": (v["bytes"] / v["ms"] / 1e6) if v["ms"] > 0 else None}
+                              for k, v in stats.items()}}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "bf16" if w.dtype == "bf16" else "f32", "data": "synthetic",
+            "config": {"workload": w.name, "L": w.n_layers, "d_model": w.d_model, "d_ffn": w.d_ffn,
+                       "n_heads": w.n_heads, "d_head": w.d_head, "vocab": w.vocab, "seq_len": w.seq_len,
+                       "n_seqs": w.n_seqs, "K": w.K, "M": w.M, "remat": w.remat, "parallelism": "replicas" if world > 1 else "1 GPU, K streams",
+                       "l2": "inputs larger than L2 (activations+weights per step >> 126 MB)"},
+            "loss": loss,
+            "tflops_executed": fl["executed"] / step_s / 1e12, "tflops_model": fl["model"] / step_s / 1e12,
+            "frac_of_bf16_peak_executed": fl["executed"] / step_s / 1e12 / peaks["burst"],
+            "mfu_model_flops": fl["model"] / step_s / 1e12 / peaks["burst"],
+            "peak_tflops_burst": peaks["burst"], "peak_tflops_sustained": peaks["sustained"],
+            "peak_hbm_bytes": peak_hbm["total"], "peak_hbm_by_category": peak_hbm["by_category"],
+            "clocks": clocks, "roofline": roofline,
+            "e2e": {"value": tokens * args.steps / (ms_e2e / 1e3), "unit": UNIT,
+                    "h2d_bytes_per_step": int(tok.nbytes + lab.nbytes), "d2h_bytes_per_step": 4 * w.M},
+            "gpu_launches": int(launches)}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = {k: v for k, v in oracle_sample(w).items() if k != "seconds"}
+    eng.close()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=gi.CONFIG_ORDER)
+    ap.add_argument("--M", type=int, default=None)
+    ap.add_argument("--K", type=int, default=None)
+    ap.add_argument("--no-remat", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    w = gi.CONFIGS[args.workload]
+    if args.M:
+        w = w.replace(M=args.M)
+    if args.K:
+        w = w.replace(K=args.K)
+    if args.no_remat:
+        w = w.replace(remat=False)
+    if args.impl == "reference":
+        run_reference(args, w, rank, world)
+        return
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl")
+    try:
+        run_ours(args, w, rank, world, local_rank)
+    finally:
+        if world > 1:
+            import torch.distributed as dist
+            dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

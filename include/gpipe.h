@@ -154,6 +154,16 @@ int gpipe_peak_bytes(const gpipe_t *g, size_t *total, size_t *by_category, size_
  * with events_out == NULL sets *n_events to the number available. */
 int gpipe_trace(gpipe_t *g, int enable, gpipe_trace_event *events_out, int64_t *n_events);
 
+/* Per-launch timing for the roofline report: with enable != 0 every kernel launch of the following
+ * steps is bracketed by CUDA events on its stream and accumulated per kernel class (enabling
+ * resets the counters).  gpipe_kernel_stats returns, for class cls in [0, GPIPE_NUM_KCLASSES):
+ * its name, launches, summed device milliseconds, and summed ALGORITHMIC flops and bytes
+ * (2MNK per GEMM; operand + output bytes once). */
+#define GPIPE_NUM_KCLASSES 10
+int gpipe_kernel_timing(gpipe_t *g, int enable);
+int gpipe_kernel_stats(const gpipe_t *g, int cls, const char **name, int64_t *count, double *ms,
+                       double *flops, double *bytes);
+
 /* Number of kernels the library launched since gpipe_create (for bench.py's gpu_launches). */
 int64_t gpipe_launch_count(const gpipe_t *g);
 

@@ -73,6 +73,9 @@ def lib() -> C.CDLL:
         "gpipe_peak_bytes": (i32, [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]),
         "gpipe_trace": (i32, [vp, i32, C.POINTER(TraceEvent), C.POINTER(i64)]),
         "gpipe_launch_count": (i64, [vp]),
+        "gpipe_kernel_timing": (i32, [vp, i32]),
+        "gpipe_kernel_stats": (i32, [vp, i32, C.POINTER(C.c_char_p), C.POINTER(i64), C.POINTER(C.c_double),
+                                     C.POINTER(C.c_double), C.POINTER(C.c_double)]),
         "gpipe_debug_read": (i32, [vp, C.c_char_p, i32, vp, i64, C.POINTER(i64)]),
         "gpipe_last_error": (C.c_char_p, []),
         "gpipe_version": (C.c_char_p, []),
@@ -101,7 +104,7 @@ EXPORTED_SYMBOLS = [
     "gpipe_plan_bytes", "gpipe_create", "gpipe_destroy", "gpipe_init_params", "gpipe_step",
     "gpipe_step_device", "gpipe_apply_sgd", "gpipe_zero_grads", "gpipe_num_tensors",
     "gpipe_tensor_info", "gpipe_get_param", "gpipe_set_param", "gpipe_get_grad", "gpipe_peak_bytes",
-    "gpipe_trace", "gpipe_launch_count", "gpipe_debug_read", "gpipe_last_error", "gpipe_version",
+    "gpipe_trace", "gpipe_launch_count", "gpipe_kernel_timing", "gpipe_kernel_stats", "gpipe_debug_read", "gpipe_last_error", "gpipe_version",
     "gpipe_op_gemm", "gpipe_op_ln_fwd", "gpipe_op_ln_bwd_scratch_floats", "gpipe_op_ln_bwd",
     "gpipe_op_attn_fwd", "gpipe_op_attn_bwd", "gpipe_op_softmax_ce", "gpipe_op_colsum",
     "gpipe_op_embed_fwd", "gpipe_op_embed_bwd", "gpipe_op_positional", "gpipe_op_sgd",
@@ -271,6 +274,18 @@ class GPipe:
         buf = (TraceEvent * max(n.value, 1))()
         _check(lib().gpipe_trace(self._h, 1, buf, C.byref(n)))
         return [(chr(e.kind), e.k, e.m, e.enqueue_index, e.start_ms, e.end_ms) for e in buf[:n.value]]
+
+    def kernel_timing(self, enable: bool):
+        _check(lib().gpipe_kernel_timing(self._h, int(enable)))
+
+    def kernel_stats(self) -> Dict[str, Dict[str, float]]:
+        out = {}
+        for cls in range(10):
+            nm, cnt = C.c_char_p(), C.c_int64()
+            ms, fl, by = C.c_double(), C.c_double(), C.c_double()
+            _check(lib().gpipe_kernel_stats(self._h, cls, C.byref(nm), C.byref(cnt), C.byref(ms), C.byref(fl), C.byref(by)))
+            out[nm.value.decode()] = {"launches": cnt.value, "ms": ms.value, "flops": fl.value, "bytes": by.value}
+        return out
 
     def launch_count(self) -> int:
         return int(lib().gpipe_launch_count(self._h))

@@ -332,6 +332,27 @@ int gpipe_trace(gpipe_t *g, int enable, gpipe_trace_event *events_out, int64_t *
   return GPIPE_OK;
 }
 
+int gpipe_kernel_timing(gpipe_t *g, int enable) {
+  if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
+  g->e.ktiming_on = enable ? 1 : 0;
+  for (auto &st : g->e.kstats) st = KStat();
+  return GPIPE_OK;
+}
+
+int gpipe_kernel_stats(const gpipe_t *g, int cls, const char **name, int64_t *count, double *ms, double *flops, double *bytes) {
+  static const char *names[KC_NUM] = {"gemm_fwd", "gemm_dgrad", "gemm_wgrad", "attn_fwd", "attn_bwd",
+                                      "ln_fwd", "ln_bwd", "softmax_ce", "colsum", "embed"};
+  if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
+  if (cls < 0 || cls >= KC_NUM) return fail(GPIPE_EINVAL, "kernel class out of range");
+  const KStat &st = g->e.kstats[cls];
+  if (name) *name = names[cls];
+  if (count) *count = st.count;
+  if (ms) *ms = st.ms;
+  if (flops) *flops = st.flops;
+  if (bytes) *bytes = st.bytes;
+  return GPIPE_OK;
+}
+
 int64_t gpipe_launch_count(const gpipe_t *g) { return g ? g->e.launches : 0; }
 
 int gpipe_debug_read(gpipe_t *g, const char *what, int layer, float *host_out, int64_t max_elems, int64_t *n_elems) {

@@ -169,12 +169,27 @@ cudaEvent_t Engine::pool_event() {
 // ---------------------------------------------------------------------------------------------
 cudaError_t Engine::forward_cell(int k, int m, bool replay) {
   Ctx c = ctx(k);
+  const double lpb = (double)lp_size(dt);
+  const double Td = (double)T_mb;
+  // algorithmic bytes of a GEMM: operands once, output once (+ fused residual / accumulate reads)
+  auto tgemm = [&](int cls, const GemmArgs &g) -> cudaError_t {
+    double fl = 2.0 * g.M * g.N * (double)g.K;
+    double outb = (g.flags & (EPI_OUT_F32 | EPI_ACCUM)) ? 4.0 : lpb;
+    double by = ((double)g.M * g.K + (double)g.K * g.N) * lpb + (double)g.M * g.N * outb;
+    if (g.flags & EPI_RESID) by += (double)g.M * g.N * 4.0;
+    if (g.flags & EPI_ACCUM) by += (double)g.M * g.N * 4.0;
+    if (g.flags & EPI_MASK) by += (double)g.M * g.N * lpb;
+    return timed(k, cls, fl, by, [&] { return gemm(c, dt, g); });
+  };
+  auto tln = [&](const float *x_, const float *g_, const float *b_, void *y_, float *mu_, float *rs_) -> cudaError_t {
+    return timed(k, KC_LN_FWD, 0, Td * d * (4.0 + lpb), [&] { return ln_fwd(c, dt, x_, g_, b_, y_, mu_, rs_, T_mb, d, eps); });
+  };
   Workspace &w = wsp(k, m);
   const int32_t *tok = tok_dev + (int64_t)m * T_mb;
   const int32_t *lab = lab_dev + (int64_t)m * T_mb;
   float *x;
   if (k == 0) {
-    GP_TRY(embed_fwd(c, dt, tok, W(i_emb), pe, w.x_emb, T_mb, S, d));
+    GP_TRY(timed(k, KC_EMBED, 0, (double)T_mb * d * (lpb + 8), [&] { return embed_fwd(c, dt, tok, W(i_emb), pe, w.x_emb, T_mb, S, d); }));
     x = w.x_emb;
   } else {
     x = slot[k][m];
@@ -186,29 +201,30 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
     LayerBuf &b = w.layers[i];
     bool last = (i + 1 == nl);
     // a = LN1(x)                                                             (a5)
-    GP_TRY(ln_fwd(c, dt, x, P(q.ln1_g), P(q.ln1_b), b.a, b.mean1, b.rstd1, T_mb, d, eps));
+    GP_TRY(tln(x, P(q.ln1_g), P(q.ln1_b), b.a, b.mean1, b.rstd1));
     // [q|k|v] = a W_qkv + b_qkv                                              (a6)
     GemmArgs g{};
     g.M = (int)T_mb; g.N = 3 * da; g.K = d;
     g.A = b.a; g.lda = d; g.B = W(q.w_qkv); g.ldb = 3 * da; g.C = b.qkv; g.ldc = 3 * da;
     g.bias = P(q.b_qkv); g.flags = EPI_BIAS;
-    GP_TRY(gemm(c, dt, g));
+    GP_TRY(tgemm(KC_GEMM_FWD, g));
     // o = softmax(q k^T / sqrt(dh) + mask) v                                 (a7)
-    GP_TRY(attn_fwd(c, dt, b.qkv, b.o, b.lse, (int)nb, S, A, dh, causal[l]));
+    GP_TRY(timed(k, KC_ATTN_FWD, 4.0 * Td * S * da * (causal[l] ? (S + 1.0) / (2.0 * S) : 1.0), Td * 4.0 * da * lpb,
+                 [&] { return attn_fwd(c, dt, b.qkv, b.o, b.lse, (int)nb, S, A, dh, causal[l]); }));
     // x1 = x + o W_o + b_o                                                   (a8)
     g = GemmArgs{};
     g.M = (int)T_mb; g.N = d; g.K = da;
     g.A = b.o; g.lda = da; g.B = W(q.w_o); g.ldb = d; g.C = b.x1; g.ldc = d;
     g.bias = P(q.b_o); g.resid = x; g.flags = EPI_BIAS | EPI_RESID | EPI_OUT_F32;
-    GP_TRY(gemm(c, dt, g));
+    GP_TRY(tgemm(KC_GEMM_FWD, g));
     // c = LN2(x1)                                                            (a9)
-    GP_TRY(ln_fwd(c, dt, b.x1, P(q.ln2_g), P(q.ln2_b), b.c, b.mean2, b.rstd2, T_mb, d, eps));
+    GP_TRY(tln(b.x1, P(q.ln2_g), P(q.ln2_b), b.c, b.mean2, b.rstd2));
     // h = relu(c W_1 + b_1)                                                  (a10)
     g = GemmArgs{};
     g.M = (int)T_mb; g.N = H; g.K = d;
     g.A = b.c; g.lda = d; g.B = W(q.w_1); g.ldb = H; g.C = b.h; g.ldc = H;
     g.bias = P(q.b_1); g.flags = EPI_BIAS | EPI_RELU;
-    GP_TRY(gemm(c, dt, g));
+    GP_TRY(tgemm(KC_GEMM_FWD, g));
     // x2 = x1 + h W_2 + b_2                                                  (a11)
     float *x2;
     if (!last) x2 = b.x2;
@@ -221,20 +237,21 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
       g.M = (int)T_mb; g.N = d; g.K = H;
       g.A = b.h; g.lda = H; g.B = W(q.w_2); g.ldb = d; g.C = x2; g.ldc = d;
       g.bias = P(q.b_2); g.resid = b.x1; g.flags = EPI_BIAS | EPI_RESID | EPI_OUT_F32;
-      GP_TRY(gemm(c, dt, g));
+      GP_TRY(tgemm(KC_GEMM_FWD, g));
     }
     x = x2;
   }
   if (k == K - 1) {
     if (nl == 0 && K == 1) x = w.x_emb;
     // y = LN_f(x_L); logits = y W_out; fused softmax-CE -> loss partial, dlogits   (a13, a14)
-    GP_TRY(ln_fwd(c, dt, x, P(i_lnf_g), P(i_lnf_b), w.y, w.meanf, w.rstdf, T_mb, d, eps));
+    GP_TRY(tln(x, P(i_lnf_g), P(i_lnf_b), w.y, w.meanf, w.rstdf));
     GemmArgs g{};
     g.M = (int)T_mb; g.N = V; g.K = d;
     g.A = w.y; g.lda = d; g.B = W(i_w_out); g.ldb = V; g.C = w.logits; g.ldc = V;
     g.flags = 0;
-    GP_TRY(gemm(c, dt, g));
-    GP_TRY(softmax_ce(c, dt, w.logits, lab, w.rowloss, T_mb, V, 1.f / (float)T_total));
+    GP_TRY(tgemm(KC_GEMM_FWD, g));
+    GP_TRY(timed(k, KC_CE, 0, Td * V * 2.0 * lpb,
+                 [&] { return softmax_ce(c, dt, w.logits, lab, w.rowloss, T_mb, V, 1.f / (float)T_total); }));
     GP_TRY(loss_reduce(c, w.rowloss, replay ? loss_dummy : loss_parts + m, T_mb));
   }
   return cudaSuccess;
@@ -252,13 +269,26 @@ cudaError_t Engine::backward_cell(int k, int m) {
   const float *dx;            // gradient of the residual stream at the current position
   const void *dxo;            // its lp operand copy
   int cur = 0;                // which ping-pong buffer the NEXT producer writes
+  const double lpb = (double)lp_size(dt);
+  const double Td = (double)T_mb;
+  auto tlnb = [&](const void *dy_, const float *x_, const float *mu_, const float *rs_, const float *g_,
+                  const float *dres_, float *dxo_, void *dxlp_, float *dg_, float *db_) -> cudaError_t {
+    double by = Td * d * (lpb + 4.0 + (dres_ ? 4.0 : 0.0) + 4.0 + (dxlp_ ? lpb : 0.0));
+    return timed(k, KC_LN_BWD, 0, by, [&] {
+      return ln_bwd(c, dt, dy_, x_, mu_, rs_, g_, dres_, dxo_, dxlp_, s.ln_partials, dg_, db_, T_mb, d);
+    });
+  };
+  auto tcol = [&](const void *dy_, int64_t ld_, float *out_, int n_) -> cudaError_t {
+    return timed(k, KC_COLSUM, 0, Td * n_ * lpb, [&] { return colsum_accum(c, dt, dy_, ld_, out_, T_mb, n_); });
+  };
   auto wgrad = [&](const void *X, int64_t ldx, int Min, const void *dY, int64_t ldy, int Nout,
                    int iw) -> cudaError_t {
     GemmArgs g{};
     g.M = Min; g.N = Nout; g.K = (int)T_mb;
     g.A = X; g.lda = ldx; g.transA = 1; g.B = dY; g.ldb = ldy; g.transB = 0;
     g.C = G(iw); g.ldc = Nout; g.flags = EPI_ACCUM | EPI_OUT_F32;
-    return gemm(c, dt, g);
+    double by = ((double)g.M * g.K + (double)g.K * g.N) * lpb + (double)g.M * g.N * 8.0;
+    return timed(k, KC_GEMM_WGRAD, 2.0 * g.M * g.N * (double)g.K, by, [&] { return gemm(c, dt, g); });
   };
   auto dgrad = [&](const void *dY, int64_t ldy, int Kout, int iw, int Nin, void *dX,
                    const void *mask) -> cudaError_t {
@@ -266,16 +296,16 @@ cudaError_t Engine::backward_cell(int k, int m) {
     g.M = (int)T_mb; g.N = Nin; g.K = Kout;
     g.A = dY; g.lda = ldy; g.transA = 0; g.B = W(iw); g.ldb = Kout; g.transB = 1;
     g.C = dX; g.ldc = Nin; g.mask = mask; g.ldmask = Nin; g.flags = mask ? EPI_MASK : 0;
-    return gemm(c, dt, g);
+    double by = ((double)g.M * g.K + (double)g.K * g.N + (double)g.M * g.N * (mask ? 2.0 : 1.0)) * lpb;
+    return timed(k, KC_GEMM_DGRAD, 2.0 * g.M * g.N * (double)g.K, by, [&] { return gemm(c, dt, g); });
   };
 
   if (k == K - 1) {
     const float *xL = nl > 0 ? w.x_out : (K == 1 ? w.x_emb : slot[k][m]);
     GP_TRY(wgrad(w.y, d, d, w.logits, V, V, i_w_out));                 // dW_out += y^T dlogits
     GP_TRY(dgrad(w.logits, V, V, i_w_out, d, s.dc, nullptr));          // dy = dlogits W_out^T
-    GP_TRY(ln_bwd(c, dt, s.dc, xL, w.meanf, w.rstdf, P(i_lnf_g), nullptr, s.dx[cur],
-                  dt == GP_BF16 ? s.dx_lp[cur] : nullptr, s.ln_partials, G(i_lnf_g), G(i_lnf_b),
-                  T_mb, d));
+    GP_TRY(tlnb(s.dc, xL, w.meanf, w.rstdf, P(i_lnf_g), nullptr, s.dx[cur],
+                dt == GP_BF16 ? s.dx_lp[cur] : nullptr, G(i_lnf_g), G(i_lnf_b)));
     dx = s.dx[cur];
     dxo = s.dx_lp[cur];
     cur ^= 1;
@@ -291,27 +321,27 @@ cudaError_t Engine::backward_cell(int k, int m) {
     // FFN: dh = (dx W_2^T) * [h > 0]; dW_2 += h^T dx; db_2 += sum_t dx
     GP_TRY(dgrad(dxo, d, d, q.w_2, H, s.dh, b.h));
     GP_TRY(wgrad(b.h, H, H, dxo, d, d, q.w_2));
-    GP_TRY(colsum_accum(c, dt, dxo, d, G(q.b_2), T_mb, d));
+    GP_TRY(tcol(dxo, d, G(q.b_2), d));
     // dc = dh W_1^T; dW_1 += c^T dh; db_1 += sum_t dh
     GP_TRY(dgrad(s.dh, H, H, q.w_1, d, s.dc, nullptr));
     GP_TRY(wgrad(b.c, d, d, s.dh, H, H, q.w_1));
-    GP_TRY(colsum_accum(c, dt, s.dh, H, G(q.b_1), T_mb, H));
+    GP_TRY(tcol(s.dh, H, G(q.b_1), H));
     // LN2 backward; residual adds gradients: dx1 = dx + LN2'(dc)
-    GP_TRY(ln_bwd(c, dt, s.dc, b.x1, b.mean2, b.rstd2, P(q.ln2_g), dx, s.dx[cur],
-                  dt == GP_BF16 ? s.dx_lp[cur] : nullptr, s.ln_partials, G(q.ln2_g), G(q.ln2_b),
-                  T_mb, d));
+    GP_TRY(tlnb(s.dc, b.x1, b.mean2, b.rstd2, P(q.ln2_g), dx, s.dx[cur],
+                dt == GP_BF16 ? s.dx_lp[cur] : nullptr, G(q.ln2_g), G(q.ln2_b)));
     dx = s.dx[cur];
     dxo = s.dx_lp[cur];
     cur ^= 1;
     // attention block: do = dx1 W_o^T; dW_o += o^T dx1; db_o += sum_t dx1
     GP_TRY(dgrad(dxo, d, d, q.w_o, da, s.d_o, nullptr));
     GP_TRY(wgrad(b.o, da, da, dxo, d, d, q.w_o));
-    GP_TRY(colsum_accum(c, dt, dxo, d, G(q.b_o), T_mb, d));
-    GP_TRY(attn_bwd(c, dt, b.qkv, b.o, s.d_o, b.lse, s.dqkv, s.dvec, (int)nb, S, A, dh, causal[l]));
+    GP_TRY(tcol(dxo, d, G(q.b_o), d));
+    GP_TRY(timed(k, KC_ATTN_BWD, 10.0 * Td * S * da * (causal[l] ? (S + 1.0) / (2.0 * S) : 1.0), Td * 8.0 * da * lpb,
+                 [&] { return attn_bwd(c, dt, b.qkv, b.o, s.d_o, b.lse, s.dqkv, s.dvec, (int)nb, S, A, dh, causal[l]); }));
     // da = dqkv W_qkv^T; dW_qkv += a^T dqkv; db_qkv += sum_t dqkv
     GP_TRY(dgrad(s.dqkv, 3 * da, 3 * da, q.w_qkv, d, s.dc, nullptr));
     GP_TRY(wgrad(b.a, d, d, s.dqkv, 3 * da, 3 * da, q.w_qkv));
-    GP_TRY(colsum_accum(c, dt, s.dqkv, 3 * da, G(q.b_qkv), T_mb, 3 * da));
+    GP_TRY(tcol(s.dqkv, 3 * da, G(q.b_qkv), 3 * da));
     // LN1 backward: dx_in = dx1 + LN1'(da); the cell's first layer writes the boundary gradient
     float *out = s.dx[cur];
     void *out_lp = s.dx_lp[cur];
@@ -319,13 +349,14 @@ cudaError_t Engine::backward_cell(int k, int m) {
       out = dbound[m & 1][k];
       out_lp = dbound_lp[m & 1][k];
     }
-    GP_TRY(ln_bwd(c, dt, s.dc, x_in, b.mean1, b.rstd1, P(q.ln1_g), dx, out,
-                  dt == GP_BF16 ? out_lp : nullptr, s.ln_partials, G(q.ln1_g), G(q.ln1_b), T_mb, d));
+    GP_TRY(tlnb(s.dc, x_in, b.mean1, b.rstd1, P(q.ln1_g), dx, out, dt == GP_BF16 ? out_lp : nullptr,
+                G(q.ln1_g), G(q.ln1_b)));
     dx = out;
     dxo = out_lp;
     cur ^= 1;
   }
-  if (k == 0) GP_TRY(embed_bwd(c, tok, dx, G(i_emb), T_mb, d));       // dE[tok] += dx0
+  if (k == 0)                                                          // dE[tok] += dx0
+    GP_TRY(timed(k, KC_EMBED, 0, Td * d * 12.0, [&] { return embed_bwd(c, tok, dx, G(i_emb), T_mb, d); }));
   return cudaSuccess;
 }
 
@@ -335,9 +366,21 @@ cudaError_t Engine::backward_cell(int k, int m) {
 //   forward ticks   F(k,m), m = tau - k                      F(k,m) <- F(k-1,m)
 //   backward ticks  [R(k,m)] B(k,m), m = M-1 - (tau-(K-1-k))  B(k,m) <- B(k+1,m);  R(k,m) <- slot only
 // ---------------------------------------------------------------------------------------------
+cudaError_t Engine::resolve_kernel_timing() {
+  for (const KRec &r : krecs) {
+    float ms = 0.f;
+    GP_TRY(cudaEventElapsedTime(&ms, r.e0, r.e1));
+    KStat &st = kstats[r.cls];
+    st.count += 1; st.ms += ms; st.flops += r.flops; st.bytes += r.bytes;
+  }
+  krecs.clear();
+  return cudaSuccess;
+}
+
 cudaError_t Engine::run_step(float *loss_out) {
   ev_pool_used = 0;
   trace.clear();
+  krecs.clear();
   int idx = 0;
   auto task = [&](int kind, int k, int m) -> cudaError_t {
     TraceRec r{kind, k, m, idx++, nullptr, nullptr};
@@ -385,6 +428,7 @@ cudaError_t Engine::run_step(float *loss_out) {
   }
   GP_TRY(cudaMemcpyAsync(host_loss, loss_parts, sizeof(float) * M, cudaMemcpyDeviceToHost, streams[0]));
   GP_TRY(cudaStreamSynchronize(streams[0]));
+  if (ktiming_on) GP_TRY(resolve_kernel_timing());
   double s = 0.0;
   for (int m = 0; m < M; ++m) s += (double)host_loss[m];
   *loss_out = (float)s;

@@ -54,6 +54,12 @@ struct Arena {
   void *alloc(size_t bytes, int cat, int cell);
 };
 
+// kernel classes of the per-launch timing facility (gpipe_kernel_timing / gpipe_kernel_stats)
+enum KClass { KC_GEMM_FWD = 0, KC_GEMM_DGRAD, KC_GEMM_WGRAD, KC_ATTN_FWD, KC_ATTN_BWD, KC_LN_FWD, KC_LN_BWD,
+              KC_CE, KC_COLSUM, KC_EMBED, KC_NUM };
+struct KRec { int cls; double flops, bytes; cudaEvent_t e0, e1; };
+struct KStat { int64_t count = 0; double ms = 0, flops = 0, bytes = 0; };
+
 struct TraceRec {
   int kind, k, m, idx;
   cudaEvent_t e0, e1;
@@ -101,6 +107,22 @@ struct Engine {
   size_t ev_pool_used = 0;
   cudaEvent_t ev_t0 = nullptr;
   int64_t launches = 0;
+  int ktiming_on = 0;
+  std::vector<KRec> krecs;
+  KStat kstats[KC_NUM];
+  cudaError_t resolve_kernel_timing();
+  template <typename F>
+  cudaError_t timed(int k, int cls, double flops, double bytes, F &&fn) {
+    if (!ktiming_on) return fn();
+    KRec r{cls, flops, bytes, pool_event(), pool_event()};
+    cudaError_t e = cudaEventRecord(r.e0, streams[k]);
+    if (e != cudaSuccess) return e;
+    e = fn();
+    if (e != cudaSuccess) return e;
+    e = cudaEventRecord(r.e1, streams[k]);
+    krecs.push_back(r);
+    return e;
+  }
 
   // -- construction --
   int build_inventory(std::string &err);

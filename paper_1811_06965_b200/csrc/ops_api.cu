@@ -14,6 +14,12 @@ cudaError_t attn_bwd_simt(const Ctx &c, int dt, const void *qkv, const void *o, 
                           const float *lse, void *dqkv, float *dvec, int n_seq, int S, int A, int dh,
                           int causal);
 
+bool attn_mma_supported(int dt, int S, int A, int dh);
+cudaError_t attn_fwd_mma(const Ctx &c, const void *qkv, void *o, float *lse, int n_seq, int S, int A, int dh,
+                         int causal);
+cudaError_t attn_bwd_mma(const Ctx &c, const void *qkv, const void *o, const void *d_o, const float *lse,
+                         void *dqkv, float *dvec, int n_seq, int S, int A, int dh, int causal);
+
 cudaError_t gemm(const Ctx &c, int dt, const GemmArgs &a) {
   if (c.gemm_backend != 1 && gemm_tc_supported(dt, a)) return gemm_tc(c, a);
   if (c.gemm_backend == 2) return cudaErrorNotSupported;
@@ -21,11 +27,13 @@ cudaError_t gemm(const Ctx &c, int dt, const GemmArgs &a) {
 }
 cudaError_t attn_fwd(const Ctx &c, int dt, const void *qkv, void *o, float *lse, int n_seq, int S,
                      int A, int dh, int causal) {
+  if (attn_mma_supported(dt, S, A, dh)) return attn_fwd_mma(c, qkv, o, lse, n_seq, S, A, dh, causal);
   return attn_fwd_simt(c, dt, qkv, o, lse, n_seq, S, A, dh, causal);
 }
 cudaError_t attn_bwd(const Ctx &c, int dt, const void *qkv, const void *o, const void *d_o,
                      const float *lse, void *dqkv, float *dvec, int n_seq, int S, int A, int dh,
                      int causal) {
+  if (attn_mma_supported(dt, S, A, dh)) return attn_bwd_mma(c, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal);
   return attn_bwd_simt(c, dt, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal);
 }
 }  // namespace gp

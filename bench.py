@@ -224,7 +224,7 @@ def run_ours(args, w, rank, world, local_rank):
     clocks = sampler.stop() if sampler else None
     ms_e2e = timed(lambda: eng.step(tok_h, lab_h), args.steps)
     # one extra step with per-launch CUDA events for the roofline of the dominant kernel class
-    eng.kernel_timing(True)
+    eng.kernel_timing(True, serial=True)         # each launch alone on the GPU: standalone durations
     eng.step(tok_d, lab_d)
     stats = eng.kernel_stats()
     eng.kernel_timing(False)

@@ -158,7 +158,8 @@ int gpipe_trace(gpipe_t *g, int enable, gpipe_trace_event *events_out, int64_t *
  * steps is bracketed by CUDA events on its stream and accumulated per kernel class (enabling
  * resets the counters).  gpipe_kernel_stats returns, for class cls in [0, GPIPE_NUM_KCLASSES):
  * its name, launches, summed device milliseconds, and summed ALGORITHMIC flops and bytes
- * (2MNK per GEMM; operand + output bytes once). */
+ * (2MNK per GEMM; operand + output bytes once).  enable bit 1 (value 2 or 3)
+ * additionally serialises all cells onto stream 0, so that each launch is timed running alone. */
 #define GPIPE_NUM_KCLASSES 10
 int gpipe_kernel_timing(gpipe_t *g, int enable);
 int gpipe_kernel_stats(const gpipe_t *g, int cls, const char **name, int64_t *count, double *ms,

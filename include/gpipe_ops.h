@@ -29,24 +29,30 @@ extern "C" {
 #define GPIPE_EPI_RESID   8   /* + resid[m,n]         (fp32 [M, ldc], may alias C)                */
 #define GPIPE_EPI_ACCUM  16   /* C (fp32) += v        (wgrad accumulation across micro-batches)   */
 #define GPIPE_EPI_OUT_F32 32  /* C is fp32, else lp                                               */
+#define GPIPE_EPI_COLSUM 64   /* colsum_out[n] += sum_m C[m,n] of the stored values (bias gradient
+                                 of the layer below, fused into the dgrad GEMM); lp output only   */
 
 /* C[M,N] = epilogue(op(A)[M,K] op(B)[K,N]), fp32 accumulation.  transA = 0: A stored [M,K]
  * row-major, 1: stored [K,M]; transB = 0: B stored [K,N], 1: stored [N,K].  backend: 0 = auto
  * (tcgen05 tensor cores for bf16 when the shape is tile-aligned), 1 = fp32-FMA SIMT kernel,
- * 2 = tcgen05 or fail with GPIPE_EINVAL. */
+ * 2 = tcgen05 or fail with GPIPE_EINVAL.  colsum_out fp32 [N] / colsum_scratch fp32
+ * [gpipe_op_colsum_scratch_floats(M, N)] are only read with GPIPE_EPI_COLSUM. */
 int gpipe_op_gemm(void *stream, int dtype, int M, int N, int K, const void *A, int64_t lda, int transA,
                   const void *B, int64_t ldb, int transB, void *C, int64_t ldc, const float *bias,
-                  const float *resid, const void *mask, int64_t ldmask, int flags, int backend);
+                  const float *resid, const void *mask, int64_t ldmask, float *colsum_out,
+                  float *colsum_scratch, int flags, int backend);
 
 /* y = LayerNorm(x) * gamma + beta over the last axis (biased variance); y lp [n_tok,d]; x fp32. */
 int gpipe_op_ln_fwd(void *stream, int dtype, const float *x, const float *gamma, const float *beta,
                     void *y, float *mean, float *rstd, int64_t n_tok, int d, float eps);
-/* dx_out = (dres_in ? dres_in : 0) + LN'(dy); dx_out_lp optional lp copy; dgamma/dbeta += .
+/* dx_out = (dres_in ? dres_in : 0) + LN'(dy); dx_out_lp optional lp copy; dgamma/dbeta += ;
+ * colsum_out (optional, fp32 [d]) += sum_t dx_out[t,:] (the lp copy's values when there is one).
  * partials: fp32 scratch of gpipe_op_ln_bwd_scratch_floats(d) floats. */
 int64_t gpipe_op_ln_bwd_scratch_floats(int d);
 int gpipe_op_ln_bwd(void *stream, int dtype, const void *dy, const float *x, const float *mean,
                     const float *rstd, const float *gamma, const float *dres_in, float *dx_out,
-                    void *dx_out_lp, float *partials, float *dgamma, float *dbeta, int64_t n_tok, int d);
+                    void *dx_out_lp, float *partials, float *dgamma, float *dbeta, float *colsum_out,
+                    int64_t n_tok, int d);
 
 /* qkv lp [n_seq*S, 3*A*dh] (q|k|v blocks); o lp [n_seq*S, A*dh]; lse fp32 [n_seq, A, S].
  * backend: 0 = auto, 1 = SIMT. */
@@ -59,8 +65,10 @@ int gpipe_op_attn_bwd(void *stream, int dtype, const void *qkv, const void *o, c
 /* in place logits -> dlogits = (softmax - onehot) * inv_T; rowloss[t] = CE_t * inv_T */
 int gpipe_op_softmax_ce(void *stream, int dtype, void *logits, const int32_t *labels, float *rowloss,
                         int64_t n_tok, int V, float inv_T);
-/* out[n] += sum_t dy[t,n] */
-int gpipe_op_colsum(void *stream, int dtype, const void *dy, int64_t ld, float *out, int64_t n_tok, int n);
+/* out[n] += sum_t dy[t,n]; scratch: fp32 [gpipe_op_colsum_scratch_floats(n_tok, n)] */
+int64_t gpipe_op_colsum_scratch_floats(int64_t n_tok, int n);
+int gpipe_op_colsum(void *stream, int dtype, const void *dy, int64_t ld, float *out, float *scratch,
+                    int64_t n_tok, int n);
 /* x[t,:] = emb[tok[t],:] + pe[t mod S,:];  gemb[tok[t],:] += dx[t,:] */
 int gpipe_op_embed_fwd(void *stream, int dtype, const int32_t *tok, const void *emb, const float *pe,
                        float *x, int64_t n_tok, int S, int d);

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libgpipe_b200.so")
 
 DTYPE_FP32, DTYPE_BF16 = 0, 1
 CATEGORIES = ["weights", "masters", "grads", "boundary", "interior", "head", "misc", "bwd_scratch"]
-EPI_BIAS, EPI_RELU, EPI_MASK, EPI_RESID, EPI_ACCUM, EPI_OUT_F32 = 1, 2, 4, 8, 16, 32
+EPI_BIAS, EPI_RELU, EPI_MASK, EPI_RESID, EPI_ACCUM, EPI_OUT_F32, EPI_COLSUM = 1, 2, 4, 8, 16, 32, 64
 
 
 class GPipeError(RuntimeError):
@@ -79,14 +79,15 @@ def lib() -> C.CDLL:
         "gpipe_debug_read": (i32, [vp, C.c_char_p, i32, vp, i64, C.POINTER(i64)]),
         "gpipe_last_error": (C.c_char_p, []),
         "gpipe_version": (C.c_char_p, []),
-        "gpipe_op_gemm": (i32, [vp, i32, i32, i32, i32, vp, i64, i32, vp, i64, i32, vp, i64, vp, vp, vp, i64, i32, i32]),
+        "gpipe_op_gemm": (i32, [vp, i32, i32, i32, i32, vp, i64, i32, vp, i64, i32, vp, i64, vp, vp, vp, i64, vp, vp, i32, i32]),
         "gpipe_op_ln_fwd": (i32, [vp, i32, vp, vp, vp, vp, vp, vp, i64, i32, f32]),
         "gpipe_op_ln_bwd_scratch_floats": (i64, [i32]),
-        "gpipe_op_ln_bwd": (i32, [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, i32]),
+        "gpipe_op_ln_bwd": (i32, [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, i32]),
         "gpipe_op_attn_fwd": (i32, [vp, i32, vp, vp, vp, i32, i32, i32, i32, i32, i32]),
         "gpipe_op_attn_bwd": (i32, [vp, i32, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32]),
         "gpipe_op_softmax_ce": (i32, [vp, i32, vp, vp, vp, i64, i32, f32]),
-        "gpipe_op_colsum": (i32, [vp, i32, vp, i64, vp, i64, i32]),
+        "gpipe_op_colsum_scratch_floats": (i64, [i64, i32]),
+        "gpipe_op_colsum": (i32, [vp, i32, vp, i64, vp, vp, i64, i32]),
         "gpipe_op_embed_fwd": (i32, [vp, i32, vp, vp, vp, vp, i64, i32, i32]),
         "gpipe_op_embed_bwd": (i32, [vp, vp, vp, vp, i64, i32]),
         "gpipe_op_positional": (i32, [vp, vp, i32, i32]),
@@ -107,6 +108,7 @@ EXPORTED_SYMBOLS = [
     "gpipe_trace", "gpipe_launch_count", "gpipe_kernel_timing", "gpipe_kernel_stats", "gpipe_debug_read", "gpipe_last_error", "gpipe_version",
     "gpipe_op_gemm", "gpipe_op_ln_fwd", "gpipe_op_ln_bwd_scratch_floats", "gpipe_op_ln_bwd",
     "gpipe_op_attn_fwd", "gpipe_op_attn_bwd", "gpipe_op_softmax_ce", "gpipe_op_colsum",
+    "gpipe_op_colsum_scratch_floats",
     "gpipe_op_embed_fwd", "gpipe_op_embed_bwd", "gpipe_op_positional", "gpipe_op_sgd",
 ]
 
@@ -275,8 +277,9 @@ class GPipe:
         _check(lib().gpipe_trace(self._h, 1, buf, C.byref(n)))
         return [(chr(e.kind), e.k, e.m, e.enqueue_index, e.start_ms, e.end_ms) for e in buf[:n.value]]
 
-    def kernel_timing(self, enable: bool):
-        _check(lib().gpipe_kernel_timing(self._h, int(enable)))
+    def kernel_timing(self, enable: bool, serial: bool = False):
+        """Per-launch CUDA-event timing; serial=True also runs every cell on stream 0."""
+        _check(lib().gpipe_kernel_timing(self._h, (1 if enable else 0) | (2 if serial else 0)))
 
     def kernel_stats(self) -> Dict[str, Dict[str, float]]:
         out = {}

@@ -334,7 +334,8 @@ int gpipe_trace(gpipe_t *g, int enable, gpipe_trace_event *events_out, int64_t *
 
 int gpipe_kernel_timing(gpipe_t *g, int enable) {
   if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
-  g->e.ktiming_on = enable ? 1 : 0;
+  g->e.ktiming_on = (enable & 1) ? 1 : 0;
+  g->e.serial = (enable & 2) ? 1 : 0;
   for (auto &st : g->e.kstats) st = KStat();
   return GPIPE_OK;
 }

@@ -145,7 +145,14 @@ int Engine::build_plan(bool dry, std::string &err) {
     s.d_o = LP(Tm * da, cat, k);
     s.dqkv = LP(Tm * 3 * da, cat, k);
     s.dvec = F32(Tm * A, cat, k);
-    s.ln_partials = F32((size_t)ln_bwd_partial_rows(sm_count) * 2 * d, cat, k);
+    s.ln_partials = F32((size_t)ln_bwd_partial_rows(sm_count) * 3 * d, cat, k);
+    {
+      size_t rows = (Tm + 127) / 128;
+      if (rows < (size_t)colsum_scratch_rows(T_mb)) rows = colsum_scratch_rows(T_mb);
+      size_t cols = (size_t)(H > 3 * da ? H : 3 * da);
+      if (cols < (size_t)d) cols = d;
+      s.colsum_scratch = F32(rows * cols, cat, k);
+    }
   }
   if (!dry && arena.used > arena.cap) {
     err = "arena too small: need " + std::to_string(arena.used) + " bytes, have " +
@@ -272,14 +279,14 @@ cudaError_t Engine::backward_cell(int k, int m) {
   const double lpb = (double)lp_size(dt);
   const double Td = (double)T_mb;
   auto tlnb = [&](const void *dy_, const float *x_, const float *mu_, const float *rs_, const float *g_,
-                  const float *dres_, float *dxo_, void *dxlp_, float *dg_, float *db_) -> cudaError_t {
+                  const float *dres_, float *dxo_, void *dxlp_, float *dg_, float *db_, float *cs_) -> cudaError_t {
     double by = Td * d * (lpb + 4.0 + (dres_ ? 4.0 : 0.0) + 4.0 + (dxlp_ ? lpb : 0.0));
     return timed(k, KC_LN_BWD, 0, by, [&] {
-      return ln_bwd(c, dt, dy_, x_, mu_, rs_, g_, dres_, dxo_, dxlp_, s.ln_partials, dg_, db_, T_mb, d);
+      return ln_bwd(c, dt, dy_, x_, mu_, rs_, g_, dres_, dxo_, dxlp_, s.ln_partials, dg_, db_, cs_, T_mb, d);
     });
   };
   auto tcol = [&](const void *dy_, int64_t ld_, float *out_, int n_) -> cudaError_t {
-    return timed(k, KC_COLSUM, 0, Td * n_ * lpb, [&] { return colsum_accum(c, dt, dy_, ld_, out_, T_mb, n_); });
+    return timed(k, KC_COLSUM, 0, Td * n_ * lpb, [&] { return colsum_accum(c, dt, dy_, ld_, out_, s.colsum_scratch, T_mb, n_); });
   };
   auto wgrad = [&](const void *X, int64_t ldx, int Min, const void *dY, int64_t ldy, int Nout,
                    int iw) -> cudaError_t {
@@ -291,11 +298,12 @@ cudaError_t Engine::backward_cell(int k, int m) {
     return timed(k, KC_GEMM_WGRAD, 2.0 * g.M * g.N * (double)g.K, by, [&] { return gemm(c, dt, g); });
   };
   auto dgrad = [&](const void *dY, int64_t ldy, int Kout, int iw, int Nin, void *dX,
-                   const void *mask) -> cudaError_t {
+                   const void *mask, float *colsum_to = nullptr) -> cudaError_t {
     GemmArgs g{};
     g.M = (int)T_mb; g.N = Nin; g.K = Kout;
     g.A = dY; g.lda = ldy; g.transA = 0; g.B = W(iw); g.ldb = Kout; g.transB = 1;
     g.C = dX; g.ldc = Nin; g.mask = mask; g.ldmask = Nin; g.flags = mask ? EPI_MASK : 0;
+    if (colsum_to) { g.flags |= EPI_COLSUM; g.colsum_out = colsum_to; g.colsum_scratch = s.colsum_scratch; }
     double by = ((double)g.M * g.K + (double)g.K * g.N + (double)g.M * g.N * (mask ? 2.0 : 1.0)) * lpb;
     return timed(k, KC_GEMM_DGRAD, 2.0 * g.M * g.N * (double)g.K, by, [&] { return gemm(c, dt, g); });
   };
@@ -304,8 +312,10 @@ cudaError_t Engine::backward_cell(int k, int m) {
     const float *xL = nl > 0 ? w.x_out : (K == 1 ? w.x_emb : slot[k][m]);
     GP_TRY(wgrad(w.y, d, d, w.logits, V, V, i_w_out));                 // dW_out += y^T dlogits
     GP_TRY(dgrad(w.logits, V, V, i_w_out, d, s.dc, nullptr));          // dy = dlogits W_out^T
+    // the gradient of x_L is also the output gradient of the last layer's FFN2: db_2 += sum_t dx
     GP_TRY(tlnb(s.dc, xL, w.meanf, w.rstdf, P(i_lnf_g), nullptr, s.dx[cur],
-                dt == GP_BF16 ? s.dx_lp[cur] : nullptr, G(i_lnf_g), G(i_lnf_b)));
+                dt == GP_BF16 ? s.dx_lp[cur] : nullptr, G(i_lnf_g), G(i_lnf_b),
+                nl > 0 ? G(lp[cell_hi[k] - 1].b_2) : nullptr));
     dx = s.dx[cur];
     dxo = s.dx_lp[cur];
     cur ^= 1;
@@ -318,24 +328,23 @@ cudaError_t Engine::backward_cell(int k, int m) {
     const LayerParams &q = lp[l];
     LayerBuf &b = w.layers[i];
     const float *x_in = i > 0 ? w.layers[i - 1].x2 : (k == 0 ? w.x_emb : slot[k][m]);
-    // FFN: dh = (dx W_2^T) * [h > 0]; dW_2 += h^T dx; db_2 += sum_t dx
-    GP_TRY(dgrad(dxo, d, d, q.w_2, H, s.dh, b.h));
+    // FFN: dh = (dx W_2^T) * [h > 0] with db_1 += sum_t dh fused into the epilogue; dW_2 += h^T dx
+    // (db_2 += sum_t dx was fused into the LayerNorm-backward kernel that produced dx)
+    GP_TRY(dgrad(dxo, d, d, q.w_2, H, s.dh, b.h, G(q.b_1)));
     GP_TRY(wgrad(b.h, H, H, dxo, d, d, q.w_2));
-    GP_TRY(tcol(dxo, d, G(q.b_2), d));
-    // dc = dh W_1^T; dW_1 += c^T dh; db_1 += sum_t dh
+    // dc = dh W_1^T; dW_1 += c^T dh
     GP_TRY(dgrad(s.dh, H, H, q.w_1, d, s.dc, nullptr));
     GP_TRY(wgrad(b.c, d, d, s.dh, H, H, q.w_1));
-    GP_TRY(tcol(s.dh, H, G(q.b_1), H));
     // LN2 backward; residual adds gradients: dx1 = dx + LN2'(dc)
+    // (db_o += sum_t dx1 is fused here: dx1 is the output gradient of the out-projection)
     GP_TRY(tlnb(s.dc, b.x1, b.mean2, b.rstd2, P(q.ln2_g), dx, s.dx[cur],
-                dt == GP_BF16 ? s.dx_lp[cur] : nullptr, G(q.ln2_g), G(q.ln2_b)));
+                dt == GP_BF16 ? s.dx_lp[cur] : nullptr, G(q.ln2_g), G(q.ln2_b), G(q.b_o)));
     dx = s.dx[cur];
     dxo = s.dx_lp[cur];
     cur ^= 1;
-    // attention block: do = dx1 W_o^T; dW_o += o^T dx1; db_o += sum_t dx1
+    // attention block: do = dx1 W_o^T; dW_o += o^T dx1
     GP_TRY(dgrad(dxo, d, d, q.w_o, da, s.d_o, nullptr));
     GP_TRY(wgrad(b.o, da, da, dxo, d, d, q.w_o));
-    GP_TRY(tcol(dxo, d, G(q.b_o), d));
     GP_TRY(timed(k, KC_ATTN_BWD, 10.0 * Td * S * da * (causal[l] ? (S + 1.0) / (2.0 * S) : 1.0), Td * 8.0 * da * lpb,
                  [&] { return attn_bwd(c, dt, b.qkv, b.o, s.d_o, b.lse, s.dqkv, s.dvec, (int)nb, S, A, dh, causal[l]); }));
     // da = dqkv W_qkv^T; dW_qkv += a^T dqkv; db_qkv += sum_t dqkv
@@ -349,8 +358,10 @@ cudaError_t Engine::backward_cell(int k, int m) {
       out = dbound[m & 1][k];
       out_lp = dbound_lp[m & 1][k];
     }
+    // its output is the FFN2 output gradient of the layer below (possibly in the previous cell):
+    // db_2(l-1) += sum_t dx
     GP_TRY(tlnb(s.dc, x_in, b.mean1, b.rstd1, P(q.ln1_g), dx, out, dt == GP_BF16 ? out_lp : nullptr,
-                G(q.ln1_g), G(q.ln1_b)));
+                G(q.ln1_g), G(q.ln1_b), l > 0 ? G(lp[l - 1].b_2) : nullptr));
     dx = out;
     dxo = out_lp;
     cur ^= 1;
@@ -387,43 +398,43 @@ cudaError_t Engine::run_step(float *loss_out) {
     if (trace_on) {
       r.e0 = pool_event();
       r.e1 = pool_event();
-      GP_TRY(cudaEventRecord(r.e0, streams[k]));
+      GP_TRY(cudaEventRecord(r.e0, st(k)));
     }
     cudaError_t e = kind == 'B' ? backward_cell(k, m) : forward_cell(k, m, kind == 'R');
     if (e != cudaSuccess) return e;
     if (trace_on) {
-      GP_TRY(cudaEventRecord(r.e1, streams[k]));
+      GP_TRY(cudaEventRecord(r.e1, st(k)));
       trace.push_back(r);
     }
     return cudaSuccess;
   };
   // inputs are on stream 0; every other cell waits for them
   GP_TRY(cudaEventRecord(ev_in, streams[0]));
-  for (int k = 1; k < K; ++k) GP_TRY(cudaStreamWaitEvent(streams[k], ev_in, 0));
+  for (int k = 1; k < K; ++k) GP_TRY(cudaStreamWaitEvent(st(k), ev_in, 0));
   if (trace_on) GP_TRY(cudaEventRecord(ev_t0, streams[0]));
 
   for (int tau = 0; tau < M + K - 1; ++tau)
     for (int k = 0; k < K; ++k) {
       int m = tau - k;
       if (m < 0 || m >= M) continue;
-      if (k > 0) GP_TRY(cudaStreamWaitEvent(streams[k], ev_f[k - 1][m], 0));
+      if (k > 0) GP_TRY(cudaStreamWaitEvent(st(k), ev_f[k - 1][m], 0));
       GP_TRY(task('F', k, m));
-      if (k + 1 < K) GP_TRY(cudaEventRecord(ev_f[k][m], streams[k]));
+      if (k + 1 < K) GP_TRY(cudaEventRecord(ev_f[k][m], st(k)));
     }
   for (int tau = 0; tau < M + K - 1; ++tau)
     for (int k = K - 1; k >= 0; --k) {
       int m = M - 1 - (tau - (K - 1 - k));
       if (m < 0 || m >= M) continue;
       if (remat) GP_TRY(task('R', k, m));                       // early: no wait on B(k+1,m)
-      if (k + 1 < K) GP_TRY(cudaStreamWaitEvent(streams[k], ev_b[k + 1][m], 0));
+      if (k + 1 < K) GP_TRY(cudaStreamWaitEvent(st(k), ev_b[k + 1][m], 0));
       // the boundary-gradient ring has two entries: B(k,m) reuses the one B(k-1,m+2) read
-      if (k > 0 && m + 2 < M) GP_TRY(cudaStreamWaitEvent(streams[k], ev_b[k - 1][m + 2], 0));
+      if (k > 0 && m + 2 < M) GP_TRY(cudaStreamWaitEvent(st(k), ev_b[k - 1][m + 2], 0));
       GP_TRY(task('B', k, m));
-      GP_TRY(cudaEventRecord(ev_b[k][m], streams[k]));
+      GP_TRY(cudaEventRecord(ev_b[k][m], st(k)));
     }
   // join: stream 0 waits for every cell, then the loss partials come back
   for (int k = 1; k < K; ++k) {
-    GP_TRY(cudaEventRecord(ev_done[k], streams[k]));
+    GP_TRY(cudaEventRecord(ev_done[k], st(k)));
     GP_TRY(cudaStreamWaitEvent(streams[0], ev_done[k], 0));
   }
   GP_TRY(cudaMemcpyAsync(host_loss, loss_parts, sizeof(float) * M, cudaMemcpyDeviceToHost, streams[0]));

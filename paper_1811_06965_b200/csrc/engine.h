@@ -43,6 +43,7 @@ struct BwdScratch {                      // one per cell
   void *dh, *dc, *d_o, *dqkv;            // lp activation gradients
   float *dvec;                           // attention D = rowsum(dO*O)
   float *ln_partials;
+  float *colsum_scratch;                 // [max(T_mb/128, colsum rows), max(H, 3*da, d)]
 };
 
 struct Arena {
@@ -108,6 +109,8 @@ struct Engine {
   cudaEvent_t ev_t0 = nullptr;
   int64_t launches = 0;
   int ktiming_on = 0;
+  int serial = 0;                                      // debug/profiling: every cell on stream 0
+  cudaStream_t st(int k) const { return streams[serial ? 0 : k]; }
   std::vector<KRec> krecs;
   KStat kstats[KC_NUM];
   cudaError_t resolve_kernel_timing();
@@ -115,11 +118,11 @@ struct Engine {
   cudaError_t timed(int k, int cls, double flops, double bytes, F &&fn) {
     if (!ktiming_on) return fn();
     KRec r{cls, flops, bytes, pool_event(), pool_event()};
-    cudaError_t e = cudaEventRecord(r.e0, streams[k]);
+    cudaError_t e = cudaEventRecord(r.e0, st(k));
     if (e != cudaSuccess) return e;
     e = fn();
     if (e != cudaSuccess) return e;
-    e = cudaEventRecord(r.e1, streams[k]);
+    e = cudaEventRecord(r.e1, st(k));
     krecs.push_back(r);
     return e;
   }
@@ -128,7 +131,7 @@ struct Engine {
   int build_inventory(std::string &err);
   int build_plan(bool dry, std::string &err);
   // -- helpers --
-  Ctx ctx(int k) { return Ctx{streams[k], &launches, sm_count, gemm_backend}; }
+  Ctx ctx(int k) { return Ctx{st(k), &launches, sm_count, gemm_backend}; }
   float *P(int i) const { return master + tensors[i].off; }            // fp32 vector param
   const void *W(int i) const {                                         // matrix operand
     return dt == GP_BF16 ? (const void *)((const char *)w_lp + tensors[i].off * 2)

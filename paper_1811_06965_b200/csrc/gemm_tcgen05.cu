@@ -122,6 +122,7 @@ struct Params {
   int64_t ldmask;
   int flags;
   int tiles_m, tiles_n;
+  float *colpart;               // EPI_COLSUM: fp32 [tiles_m, N] per-tile-row column sums
 };
 
 // ------------------------------------------------------------------------------------------
@@ -137,6 +138,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_cons
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t bars[2 * STAGES + 4];
   __shared__ uint32_t tmem_base_smem;
+  __shared__ float colbuf[4][BN];                  // EPI_COLSUM: per-warp column sums of one tile
 
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;      // 1024-B aligned (swizzle atoms)
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -259,11 +261,12 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_cons
         tmem_ld32(t_row + c * 32, r);
         tmem_ld_wait();
         const int col0 = n0 + c * 32;
-        if (row_ok && col0 < p.N) {
-          float v[32];
+        const bool active = row_ok && col0 < p.N;
+        const bool full = col0 + 32 <= p.N;
+        float v[32];
 #pragma unroll
-          for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]);
-          const bool full = col0 + 32 <= p.N;
+        for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]);
+        if (active) {
           if (full) {
             if (p.flags & EPI_BIAS) {
 #pragma unroll
@@ -317,30 +320,70 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_cons
                 uint4 u;
                 __nv_bfloat162 *h = reinterpret_cast<__nv_bfloat162 *>(&u);
 #pragma unroll
-                for (int q = 0; q < 4; ++q) h[q] = __floats2bfloat162_rn(v[j + 2 * q], v[j + 2 * q + 1]);
+                for (int q = 0; q < 4; ++q) {
+                  h[q] = __floats2bfloat162_rn(v[j + 2 * q], v[j + 2 * q + 1]);
+                  float2 f = __bfloat1622float2(h[q]);          // the stored values (for EPI_COLSUM)
+                  v[j + 2 * q] = f.x;
+                  v[j + 2 * q + 1] = f.y;
+                }
                 *reinterpret_cast<uint4 *>(cp + j) = u;
               }
             }
           } else {
             // ragged right edge: element-wise, guarded
+#pragma unroll
             for (int j = 0; j < 32; ++j) {
               const int col = col0 + j;
-              if (col >= p.N) break;
               float x = v[j];
-              if (p.flags & EPI_BIAS) x += p.bias[col];
-              if (p.flags & EPI_RELU) x = fmaxf(x, 0.f);
-              if (p.flags & EPI_MASK) x = __bfloat162float(p.mask[(int64_t)row * p.ldmask + col]) > 0.f ? x : 0.f;
-              if (p.flags & EPI_RESID) x += p.resid[(int64_t)row * p.ldc + col];
-              if (out_f32) {
-                float *cp = (float *)p.C + (int64_t)row * p.ldc + col;
-                if (p.flags & EPI_ACCUM) x += *cp;
-                *cp = x;
+              if (col < p.N) {
+                if (p.flags & EPI_BIAS) x += p.bias[col];
+                if (p.flags & EPI_RELU) x = fmaxf(x, 0.f);
+                if (p.flags & EPI_MASK) x = __bfloat162float(p.mask[(int64_t)row * p.ldmask + col]) > 0.f ? x : 0.f;
+                if (p.flags & EPI_RESID) x += p.resid[(int64_t)row * p.ldc + col];
+                if (out_f32) {
+                  float *cp = (float *)p.C + (int64_t)row * p.ldc + col;
+                  if (p.flags & EPI_ACCUM) x += *cp;
+                  *cp = x;
+                } else {
+                  bf16 xb = __float2bfloat16_rn(x);
+                  ((bf16 *)p.C)[(int64_t)row * p.ldc + col] = xb;
+                  x = __bfloat162float(xb);
+                }
               } else {
-                ((bf16 *)p.C)[(int64_t)row * p.ldc + col] = __float2bfloat16_rn(x);
+                x = 0.f;
               }
+              v[j] = x;
             }
           }
         }
+        if (p.flags & EPI_COLSUM) {
+          // column sums over this warp's 32 rows: transpose-reduce across lanes (31 shuffles);
+          // afterwards lane j holds the sum of column col0 + j
+          if (!active) {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) v[j] = 0.f;
+          }
+#pragma unroll
+          for (int off = 16; off >= 1; off >>= 1) {
+            const bool hi = (lane & off) != 0;
+#pragma unroll
+            for (int i = 0; i < off; ++i) {
+              float send = hi ? v[i] : v[i + off];
+              float keep = hi ? v[i + off] : v[i];
+              v[i] = keep + __shfl_xor_sync(0xffffffffu, send, off);
+            }
+          }
+          colbuf[quad][c * 32 + lane] = v[0];
+        }
+      }
+      if (p.flags & EPI_COLSUM) {
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        const int e = threadIdx.x - EPI_WARP0 * 32;
+        for (int cc = e; cc < BN; cc += 128) {
+          float ssum = (colbuf[0][cc] + colbuf[1][cc]) + (colbuf[2][cc] + colbuf[3][cc]);
+          if (n0 + cc < p.N) p.colpart[(int64_t)(t % p.tiles_m) * p.N + n0 + cc] = ssum;
+        }
+        asm volatile("bar.sync 1, 128;" ::: "memory");
       }
       tcgen05_fence_before();
       __syncwarp();
@@ -432,6 +475,7 @@ static cudaError_t launch(const Ctx &c, const GemmArgs &a) {
   p.b_mn_major = a.transB ? 0 : 1;
   p.C = a.C; p.ldc = a.ldc; p.bias = a.bias; p.resid = a.resid; p.mask = (const bf16 *)a.mask; p.ldmask = a.ldmask;
   p.flags = a.flags;
+  p.colpart = a.colsum_scratch;
   p.tiles_m = (a.M + BM - 1) / BM;
   p.tiles_n = (a.N + BN - 1) / BN;
   CUtensorMap ma, mb;

@@ -145,27 +145,36 @@ cudaError_t ln_fwd(const Ctx &c, int dt, const float *x, const float *gamma, con
 // ---------------------------------------------------------------------------------------------
 // LayerNorm backward.  dxhat = dy*gamma; dx = (dxhat - mean(dxhat) - xhat*mean(dxhat*xhat))*rstd
 // dx_out = dres_in + dx (residual adds gradients); optional lp copy (the next GEMM's operand).
-// dgamma/dbeta: each warp accumulates its rows in registers; per-block partials are written to
-// `partials` [gridDim.x, 2, d] and summed by ln_bwd_reduce_kernel in a fixed order.
+// Fused reductions over the token axis, all in a fixed order (deterministic):
+//   dgamma += sum_t dy*xhat, dbeta += sum_t dy, and optionally colsum_out += sum_t dx_out (the bias
+//   gradient of the linear layer whose output gradient dx_out is: db_2 / db_o).
+// One block per SM, 8 warps, one warp per row; each warp accumulates in registers, the block
+// combines its warps through shared memory and writes one partial row [3][d]; a second small
+// kernel sums the partial rows.
 // ---------------------------------------------------------------------------------------------
+constexpr int LNB_WARPS = 8;
+
 template <typename T, int NV>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(LNB_WARPS * 32)
 ln_bwd_kernel(const T *__restrict__ dy, const float *__restrict__ x, const float *__restrict__ mean,
               const float *__restrict__ rstd, const float *__restrict__ gamma,
               const float *__restrict__ dres_in, float *__restrict__ dx_out,
-              T *__restrict__ dx_out_lp, float *__restrict__ partials, int64_t n_tok, int d) {
-  extern __shared__ float sm[];       // [4 warps][2][d]
+              T *__restrict__ dx_out_lp, float *__restrict__ partials, int64_t n_tok, int d, int want_colsum) {
+  extern __shared__ float sm[];       // [d] gamma, then [3][d] block partial
+  float *gsm = sm, *psm = sm + d;
   int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   int d4 = d >> 2;
-  float4 g[NV], ag[NV], ab[NV];
+  for (int i = threadIdx.x; i < d; i += blockDim.x) gsm[i] = gamma[i];
+  for (int i = threadIdx.x; i < 3 * d; i += blockDim.x) psm[i] = 0.f;
+  __syncthreads();
+  float4 ag[NV], ab[NV], ac[NV];
 #pragma unroll
   for (int i = 0; i < NV; ++i) {
-    int j = lane + 32 * i;
-    g[i] = j < d4 ? load4(gamma + 4 * j) : make_float4(0.f, 0.f, 0.f, 0.f);
     ag[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    ab[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    ab[i] = ag[i];
+    ac[i] = ag[i];
   }
-  for (int64_t row = (int64_t)blockIdx.x * 4 + w; row < n_tok; row += (int64_t)gridDim.x * 4) {
+  for (int64_t row = (int64_t)blockIdx.x * LNB_WARPS + w; row < n_tok; row += (int64_t)gridDim.x * LNB_WARPS) {
     float mu = mean[row], rs = rstd[row];
     float4 xh[NV], dh[NV];
     float s1 = 0.f, s2 = 0.f;
@@ -173,18 +182,22 @@ ln_bwd_kernel(const T *__restrict__ dy, const float *__restrict__ x, const float
     for (int i = 0; i < NV; ++i) {
       int j = lane + 32 * i;
       if (j < d4) {
-        float4 xv = load4(x + row * d + 4 * j);
-        float4 dv = load4(dy + row * d + 4 * j);
-        xh[i] = make_float4((xv.x - mu) * rs, (xv.y - mu) * rs, (xv.z - mu) * rs, (xv.w - mu) * rs);
-        ag[i].x += dv.x * xh[i].x; ag[i].y += dv.y * xh[i].y;
-        ag[i].z += dv.z * xh[i].z; ag[i].w += dv.w * xh[i].w;
-        ab[i].x += dv.x; ab[i].y += dv.y; ab[i].z += dv.z; ab[i].w += dv.w;
-        dh[i] = make_float4(dv.x * g[i].x, dv.y * g[i].y, dv.z * g[i].z, dv.w * g[i].w);
+        xh[i] = load4(x + row * d + 4 * j);
+        dh[i] = load4(dy + row * d + 4 * j);
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      int j = lane + 32 * i;
+      if (j < d4) {
+        float4 gv = *reinterpret_cast<const float4 *>(gsm + 4 * j);
+        xh[i] = make_float4((xh[i].x - mu) * rs, (xh[i].y - mu) * rs, (xh[i].z - mu) * rs, (xh[i].w - mu) * rs);
+        ag[i].x += dh[i].x * xh[i].x; ag[i].y += dh[i].y * xh[i].y;
+        ag[i].z += dh[i].z * xh[i].z; ag[i].w += dh[i].w * xh[i].w;
+        ab[i].x += dh[i].x; ab[i].y += dh[i].y; ab[i].z += dh[i].z; ab[i].w += dh[i].w;
+        dh[i] = make_float4(dh[i].x * gv.x, dh[i].y * gv.y, dh[i].z * gv.z, dh[i].w * gv.w);
         s1 += (dh[i].x + dh[i].y) + (dh[i].z + dh[i].w);
         s2 += (dh[i].x * xh[i].x + dh[i].y * xh[i].y) + (dh[i].z * xh[i].z + dh[i].w * xh[i].w);
-      } else {
-        xh[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-        dh[i] = xh[i];
       }
     }
     float m1 = warp_sum(s1) / (float)d, m2 = warp_sum(s2) / (float)d;
@@ -202,67 +215,86 @@ ln_bwd_kernel(const T *__restrict__ dy, const float *__restrict__ x, const float
           o.x += r.x; o.y += r.y; o.z += r.z; o.w += r.w;
         }
         store4(dx_out + row * d + 4 * j, o);
-        if (dx_out_lp) store4(dx_out_lp + row * d + 4 * j, o);
+        if (dx_out_lp) {
+          store4(dx_out_lp + row * d + 4 * j, o);
+          if (want_colsum)                                           // sum what the GEMMs will read
+            o = make_float4(to_f<T>(from_f<T>(o.x)), to_f<T>(from_f<T>(o.y)), to_f<T>(from_f<T>(o.z)),
+                            to_f<T>(from_f<T>(o.w)));
+        }
+        ac[i].x += o.x; ac[i].y += o.y; ac[i].z += o.z; ac[i].w += o.w;
       }
     }
   }
-  // cross-warp reduction of the dgamma/dbeta partials, fixed order w = 0..3
-  float *mine = sm + (size_t)w * 2 * d;
+  // combine the warps of the block in a fixed order (w = 0..7), then one partial row per block
+  for (int turn = 0; turn < LNB_WARPS; ++turn) {
+    if (w == turn) {
 #pragma unroll
-  for (int i = 0; i < NV; ++i) {
-    int j = lane + 32 * i;
-    if (j < d4) {
-      store4(mine + 4 * j, ag[i]);
-      store4(mine + d + 4 * j, ab[i]);
+      for (int i = 0; i < NV; ++i) {
+        int j = lane + 32 * i;
+        if (j < d4) {
+          float4 *p0 = reinterpret_cast<float4 *>(psm + 4 * j);
+          float4 *p1 = reinterpret_cast<float4 *>(psm + d + 4 * j);
+          float4 *p2 = reinterpret_cast<float4 *>(psm + 2 * d + 4 * j);
+          float4 a = *p0, b = *p1, c = *p2;
+          a.x += ag[i].x; a.y += ag[i].y; a.z += ag[i].z; a.w += ag[i].w;
+          b.x += ab[i].x; b.y += ab[i].y; b.z += ab[i].z; b.w += ab[i].w;
+          c.x += ac[i].x; c.y += ac[i].y; c.z += ac[i].z; c.w += ac[i].w;
+          *p0 = a; *p1 = b; *p2 = c;
+        }
+      }
     }
+    __syncthreads();
   }
-  __syncthreads();
-  float *out = partials + (size_t)blockIdx.x * 2 * d;
-  for (int i = threadIdx.x; i < 2 * d; i += blockDim.x)
-    out[i] = (sm[i] + sm[2 * d + i]) + (sm[4 * d + i] + sm[6 * d + i]);
+  float *out = partials + (size_t)blockIdx.x * 3 * d;
+  for (int i = threadIdx.x; i < 3 * d; i += blockDim.x) out[i] = psm[i];
 }
 
-__global__ void ln_bwd_reduce_kernel(const float *__restrict__ partials, int n_part, int d,
-                                     float *__restrict__ dgamma, float *__restrict__ dbeta) {
-  // one warp per 32 columns; each lane sums a strided subset of the partial rows, fixed order
+// dst[which][col] += sum_r partials[r][which][col]; block = 8 row-lanes x 32 columns
+__global__ void __launch_bounds__(256)
+ln_bwd_reduce_kernel(const float *__restrict__ partials, int n_part, int d, float *__restrict__ dgamma,
+                     float *__restrict__ dbeta, float *__restrict__ colsum_out) {
   __shared__ float red[8][33];
-  int col = blockIdx.x * 32 + (threadIdx.x & 31);
   int which = blockIdx.y;
-  int ry = threadIdx.x >> 5;                      // 8 row groups
-  float s = 0.f;
-  if (col < d)
-    for (int r = ry; r < n_part; r += 8) s += partials[((size_t)r * 2 + which) * d + col];
-  red[ry][threadIdx.x & 31] = s;
+  float *dst = which == 0 ? dgamma : (which == 1 ? dbeta : colsum_out);
+  if (!dst) return;
+  int col = blockIdx.x * 32 + (threadIdx.x & 31);
+  int ry = threadIdx.x >> 5;
+  float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+  if (col < d) {
+    int r = ry;
+    for (; r + 24 < n_part; r += 32) {
+      s0 += partials[((size_t)r * 3 + which) * d + col];
+      s1 += partials[((size_t)(r + 8) * 3 + which) * d + col];
+      s2 += partials[((size_t)(r + 16) * 3 + which) * d + col];
+      s3 += partials[((size_t)(r + 24) * 3 + which) * d + col];
+    }
+    for (; r < n_part; r += 8) s0 += partials[((size_t)r * 3 + which) * d + col];
+  }
+  red[ry][threadIdx.x & 31] = (s0 + s1) + (s2 + s3);
   __syncthreads();
   if (ry == 0 && col < d) {
     float t = 0.f;
 #pragma unroll
     for (int r = 0; r < 8; ++r) t += red[r][threadIdx.x & 31];
-    float *dst = which == 0 ? dgamma : dbeta;
     dst[col] += t;
   }
 }
 
-int ln_bwd_partial_rows(int sm_count) { return sm_count * 2; }
+int ln_bwd_partial_rows(int sm_count) { return sm_count; }
 
 template <typename T>
 static cudaError_t ln_bwd_t(const Ctx &c, const T *dy, const float *x, const float *mean,
                             const float *rstd, const float *gamma, const float *dres_in,
                             float *dx_out, T *dx_out_lp, float *partials, float *dgamma,
-                            float *dbeta, int64_t n_tok, int d) {
+                            float *dbeta, float *colsum_out, int64_t n_tok, int d) {
   if (n_tok == 0) return cudaSuccess;
-  int64_t want = (n_tok + 3) / 4;
+  int64_t want = (n_tok + LNB_WARPS - 1) / LNB_WARPS;
   int grid = (int)(want < ln_bwd_partial_rows(c.sm_count) ? want : ln_bwd_partial_rows(c.sm_count));
-  size_t smem = (size_t)4 * 2 * d * sizeof(float);
+  size_t smem = (size_t)4 * d * sizeof(float);
   int nv = (d / 4 + 31) / 32;
 #define GP_LNB(NV_)                                                                               \
-  do {                                                                                            \
-    if (smem > 48 * 1024)                                                                         \
-      cudaFuncSetAttribute(ln_bwd_kernel<T, NV_>, cudaFuncAttributeMaxDynamicSharedMemorySize,    \
-                           (int)smem);                                                            \
-    ln_bwd_kernel<T, NV_><<<grid, 128, smem, c.stream>>>(dy, x, mean, rstd, gamma, dres_in,       \
-                                                         dx_out, dx_out_lp, partials, n_tok, d);  \
-  } while (0)
+  ln_bwd_kernel<T, NV_><<<grid, LNB_WARPS * 32, smem, c.stream>>>(dy, x, mean, rstd, gamma, dres_in, \
+                                                                   dx_out, dx_out_lp, partials, n_tok, d, colsum_out != nullptr)
   if (nv <= 1) GP_LNB(1);
   else if (nv <= 8) GP_LNB(8);
   else if (nv <= 16) GP_LNB(16);
@@ -271,65 +303,104 @@ static cudaError_t ln_bwd_t(const Ctx &c, const T *dy, const float *x, const flo
   if (c.launches) ++*c.launches;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  dim3 rg((d + 31) / 32, 2);
-  ln_bwd_reduce_kernel<<<rg, 256, 0, c.stream>>>(partials, grid, d, dgamma, dbeta);
+  dim3 rg((d + 31) / 32, colsum_out ? 3 : 2);
+  ln_bwd_reduce_kernel<<<rg, 256, 0, c.stream>>>(partials, grid, d, dgamma, dbeta, colsum_out);
   GP_LAUNCH_CHECK(c);
 }
 
 cudaError_t ln_bwd(const Ctx &c, int dt, const void *dy, const float *x, const float *mean,
                    const float *rstd, const float *gamma, const float *dres_in, float *dx_out,
-                   void *dx_out_lp, float *partials, float *dgamma, float *dbeta, int64_t n_tok,
-                   int d) {
+                   void *dx_out_lp, float *partials, float *dgamma, float *dbeta, float *colsum_out,
+                   int64_t n_tok, int d) {
   return dt == GP_BF16
              ? ln_bwd_t<bf16>(c, (const bf16 *)dy, x, mean, rstd, gamma, dres_in, dx_out,
-                              (bf16 *)dx_out_lp, partials, dgamma, dbeta, n_tok, d)
+                              (bf16 *)dx_out_lp, partials, dgamma, dbeta, colsum_out, n_tok, d)
              : ln_bwd_t<float>(c, (const float *)dy, x, mean, rstd, gamma, dres_in, dx_out,
-                               (float *)dx_out_lp, partials, dgamma, dbeta, n_tok, d);
+                               (float *)dx_out_lp, partials, dgamma, dbeta, colsum_out, n_tok, d);
 }
 
 // ---------------------------------------------------------------------------------------------
-// bias gradient: out[n] += sum_t dy[t,n].  Block = 8 warps x 64 columns; warp w takes rows
-// w, w+8, ...; lanes take two adjacent columns.  Fixed summation order (deterministic).
+// bias gradient: out[n] += sum_t dy[t,n], two deterministic stages.  Stage 1: block = 16 row-lanes
+// x 16 column groups of 8 (16-byte loads), grid (n/128, R slabs) -> partial [R][n].  Stage 2 sums
+// the R partial rows.  Fixed summation order.
 // ---------------------------------------------------------------------------------------------
 template <typename T>
 __global__ void __launch_bounds__(256)
-colsum_kernel(const T *__restrict__ dy, int64_t ld, float *__restrict__ out, int64_t n_tok, int n) {
-  __shared__ float red[8][64];
-  int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  int col = blockIdx.x * 64 + lane * 2;
-  float a = 0.f, b = 0.f;
-  if (col + 1 < n) {
-    for (int64_t r = w; r < n_tok; r += 8) {
-      const T *p = dy + r * ld + col;
-      a += to_f<T>(p[0]);
-      b += to_f<T>(p[1]);
+colsum_stage1_kernel(const T *__restrict__ dy, int64_t ld, float *__restrict__ partial, int64_t n_tok, int n,
+                     int rows_per_slab) {
+  __shared__ float red[16][129];
+  int cg = threadIdx.x & 15, rl = threadIdx.x >> 4;
+  int col = blockIdx.x * 128 + cg * 8;
+  int64_t r0 = (int64_t)blockIdx.y * rows_per_slab;
+  int64_t r1 = r0 + rows_per_slab < n_tok ? r0 + rows_per_slab : n_tok;
+  float acc[8];
+#pragma unroll
+  for (int e = 0; e < 8; ++e) acc[e] = 0.f;
+  if (col + 8 <= n && (ld % 8) == 0 && sizeof(T) == 2) {
+    for (int64_t r = r0 + rl; r < r1; r += 16) {
+      uint4 u = *reinterpret_cast<const uint4 *>(dy + r * ld + col);
+      const __nv_bfloat162 *h = reinterpret_cast<const __nv_bfloat162 *>(&u);
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        float2 f = __bfloat1622float2(h[q]);
+        acc[2 * q] += f.x;
+        acc[2 * q + 1] += f.y;
+      }
     }
-  } else if (col < n) {
-    for (int64_t r = w; r < n_tok; r += 8) a += to_f<T>(dy[r * ld + col]);
+  } else {
+    for (int64_t r = r0 + rl; r < r1; r += 16)
+#pragma unroll
+      for (int e = 0; e < 8; ++e)
+        if (col + e < n) acc[e] += to_f<T>(dy[r * ld + col + e]);
   }
-  red[w][lane * 2] = a;
-  red[w][lane * 2 + 1] = b;
+#pragma unroll
+  for (int e = 0; e < 8; ++e) red[rl][cg * 8 + e] = acc[e];
   __syncthreads();
-  if (threadIdx.x < 64) {
-    int cidx = blockIdx.x * 64 + threadIdx.x;
+  if (threadIdx.x < 128) {
+    int cidx = blockIdx.x * 128 + threadIdx.x;
     if (cidx < n) {
       float t = 0.f;
 #pragma unroll
-      for (int r = 0; r < 8; ++r) t += red[r][threadIdx.x];
-      out[cidx] += t;
+      for (int r = 0; r < 16; ++r) t += red[r][threadIdx.x];
+      partial[(size_t)blockIdx.y * n + cidx] = t;
     }
   }
 }
 
-cudaError_t colsum_accum(const Ctx &c, int dt, const void *dy, int64_t ld, float *out,
-                         int64_t n_tok, int n) {
+__global__ void __launch_bounds__(256)
+colsum_stage2_kernel(const float *__restrict__ partial, int R, int n, float *__restrict__ out) {
+  int col = blockIdx.x * 256 + threadIdx.x;
+  if (col >= n) return;
+  float t = 0.f;
+  for (int r = 0; r < R; ++r) t += partial[(size_t)r * n + col];
+  out[col] += t;
+}
+
+int colsum_scratch_rows(int64_t n_tok) {
+  int64_t r = (n_tok + 127) / 128;
+  return (int)(r < 1 ? 1 : (r > 32 ? 32 : r));
+}
+
+cudaError_t colsum_reduce_partials(const Ctx &c, const float *partial, int R, int n, float *out) {
   if (n == 0) return cudaSuccess;
-  unsigned grid = (unsigned)((n + 63) / 64);
-  if (dt == GP_BF16)
-    colsum_kernel<bf16><<<grid, 256, 0, c.stream>>>((const bf16 *)dy, ld, out, n_tok, n);
-  else
-    colsum_kernel<float><<<grid, 256, 0, c.stream>>>((const float *)dy, ld, out, n_tok, n);
+  colsum_stage2_kernel<<<(n + 255) / 256, 256, 0, c.stream>>>(partial, R, n, out);
   GP_LAUNCH_CHECK(c);
+}
+
+cudaError_t colsum_accum(const Ctx &c, int dt, const void *dy, int64_t ld, float *out, float *scratch,
+                         int64_t n_tok, int n) {
+  if (n == 0 || n_tok == 0) return cudaSuccess;
+  int R = colsum_scratch_rows(n_tok);
+  int rows_per_slab = (int)((n_tok + R - 1) / R);
+  dim3 grid((n + 127) / 128, R);
+  if (dt == GP_BF16)
+    colsum_stage1_kernel<bf16><<<grid, 256, 0, c.stream>>>((const bf16 *)dy, ld, scratch, n_tok, n, rows_per_slab);
+  else
+    colsum_stage1_kernel<float><<<grid, 256, 0, c.stream>>>((const float *)dy, ld, scratch, n_tok, n, rows_per_slab);
+  if (c.launches) ++*c.launches;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  return colsum_reduce_partials(c, scratch, R, n, out);
 }
 
 template <typename T>

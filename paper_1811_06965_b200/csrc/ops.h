@@ -31,7 +31,8 @@ enum {
   EPI_MASK = 4,       // mask: lp [M, ldmask]; keeps v where mask > 0, else 0 (ReLU backward)
   EPI_RESID = 8,      // resid: fp32 [M, ldc]  (may alias C)
   EPI_ACCUM = 16,     // C is fp32 and is read-modify-written: C += v   (wgrad accumulation)
-  EPI_OUT_F32 = 32    // C is fp32 (else lp)
+  EPI_OUT_F32 = 32,   // C is fp32 (else lp)
+  EPI_COLSUM = 64     // colsum_out[n] += sum_m C[m,n] (of the stored, rounded values); needs colsum_scratch
 };
 struct GemmArgs {
   int M, N, K;
@@ -42,6 +43,8 @@ struct GemmArgs {
   const float *resid;
   const void *mask; int64_t ldmask;
   int flags;
+  float *colsum_out;       // EPI_COLSUM: fp32 [N], accumulated into
+  float *colsum_scratch;   // EPI_COLSUM: fp32 [ceil(M/128), N]
 };
 cudaError_t gemm(const Ctx &c, int dt, const GemmArgs &a);
 // true when the tcgen05 kernel handles this problem (bf16, aligned shapes)
@@ -59,17 +62,21 @@ cudaError_t positional_table(const Ctx &c, float *pe, int S, int d);
 cudaError_t ln_fwd(const Ctx &c, int dt, const float *x, const float *gamma, const float *beta,
                    void *y, float *mean, float *rstd, int64_t n_tok, int d, float eps);
 // dx_out = (dres_in ? dres_in : 0) + LN'(dy);  dx_out_lp (optional) = lp copy of dx_out.
-// partials: fp32 [ln_bwd_partial_rows(), 2, d] scratch; then dgamma += sum, dbeta += sum.
+// partials: fp32 [ln_bwd_partial_rows(), 3, d] scratch; then dgamma += sum, dbeta += sum and,
+// if colsum_out != NULL, colsum_out[n] += sum_t dx_out[t,n] (the lp copy's values when there is one).
 int ln_bwd_partial_rows(int sm_count);
 cudaError_t ln_bwd(const Ctx &c, int dt, const void *dy, const float *x, const float *mean,
                    const float *rstd, const float *gamma, const float *dres_in, float *dx_out,
-                   void *dx_out_lp, float *partials, float *dgamma, float *dbeta, int64_t n_tok,
-                   int d);
+                   void *dx_out_lp, float *partials, float *dgamma, float *dbeta, float *colsum_out,
+                   int64_t n_tok, int d);
 
 // ---- bias gradient ----------------------------------------------------------------------------
-// out[n] += sum_t dy[t, n]; dy is lp [n_tok, ld]
-cudaError_t colsum_accum(const Ctx &c, int dt, const void *dy, int64_t ld, float *out,
+// out[n] += sum_t dy[t, n]; dy is lp [n_tok, ld]; scratch: fp32 [colsum_scratch_rows(n_tok), n]
+int colsum_scratch_rows(int64_t n_tok);
+cudaError_t colsum_accum(const Ctx &c, int dt, const void *dy, int64_t ld, float *out, float *scratch,
                          int64_t n_tok, int n);
+// out[n] += sum_r partial[r][n]
+cudaError_t colsum_reduce_partials(const Ctx &c, const float *partial, int R, int n, float *out);
 // fp32 -> lp copy (the operand copy of a residual gradient)
 cudaError_t cast_to_lp(const Ctx &c, int dt, const float *src, void *dst, int64_t n);
 

@@ -21,9 +21,18 @@ cudaError_t attn_bwd_mma(const Ctx &c, const void *qkv, const void *o, const voi
                          void *dqkv, float *dvec, int n_seq, int S, int A, int dh, int causal);
 
 cudaError_t gemm(const Ctx &c, int dt, const GemmArgs &a) {
-  if (c.gemm_backend != 1 && gemm_tc_supported(dt, a)) return gemm_tc(c, a);
+  const bool colsum = (a.flags & EPI_COLSUM) != 0;
+  if (colsum && (!a.colsum_out || !a.colsum_scratch || (a.flags & (EPI_OUT_F32 | EPI_ACCUM))))
+    return cudaErrorInvalidValue;
+  if (c.gemm_backend != 1 && gemm_tc_supported(dt, a)) {
+    cudaError_t e = gemm_tc(c, a);             // EPI_COLSUM: per-tile-row partial sums -> scratch
+    if (e != cudaSuccess || !colsum) return e;
+    return colsum_reduce_partials(c, a.colsum_scratch, (a.M + 127) / 128, a.N, a.colsum_out);
+  }
   if (c.gemm_backend == 2) return cudaErrorNotSupported;
-  return gemm_simt(c, dt, a);
+  cudaError_t e = gemm_simt(c, dt, a);
+  if (e != cudaSuccess || !colsum) return e;
+  return colsum_accum(c, dt, a.C, a.ldc, a.colsum_out, a.colsum_scratch, a.M, a.N);
 }
 cudaError_t attn_fwd(const Ctx &c, int dt, const void *qkv, void *o, float *lse, int n_seq, int S,
                      int A, int dh, int causal) {
@@ -63,8 +72,10 @@ static int ret(cudaError_t e, const char *where) {
 extern "C" {
 int gpipe_op_gemm(void *stream, int dtype, int M, int N, int K, const void *A, int64_t lda, int transA,
                   const void *B, int64_t ldb, int transB, void *C, int64_t ldc, const float *bias,
-                  const float *resid, const void *mask, int64_t ldmask, int flags, int backend) {
+                  const float *resid, const void *mask, int64_t ldmask, float *colsum_out,
+                  float *colsum_scratch, int flags, int backend) {
   GemmArgs g{};
+  g.colsum_out = colsum_out; g.colsum_scratch = colsum_scratch;
   g.M = M; g.N = N; g.K = K;
   g.A = A; g.lda = lda; g.transA = transA;
   g.B = B; g.ldb = ldb; g.transB = transB;
@@ -77,13 +88,14 @@ int gpipe_op_ln_fwd(void *stream, int dtype, const float *x, const float *gamma,
   return ret(ln_fwd(mk(stream), dtype, x, gamma, beta, y, mean, rstd, n_tok, d, eps), "gpipe_op_ln_fwd");
 }
 int64_t gpipe_op_ln_bwd_scratch_floats(int d) {
-  return (int64_t)ln_bwd_partial_rows(sm_count_cached()) * 2 * d;
+  return (int64_t)ln_bwd_partial_rows(sm_count_cached()) * 3 * d;
 }
 int gpipe_op_ln_bwd(void *stream, int dtype, const void *dy, const float *x, const float *mean,
                     const float *rstd, const float *gamma, const float *dres_in, float *dx_out,
-                    void *dx_out_lp, float *partials, float *dgamma, float *dbeta, int64_t n_tok, int d) {
+                    void *dx_out_lp, float *partials, float *dgamma, float *dbeta, float *colsum_out,
+                    int64_t n_tok, int d) {
   return ret(ln_bwd(mk(stream), dtype, dy, x, mean, rstd, gamma, dres_in, dx_out, dx_out_lp, partials,
-                    dgamma, dbeta, n_tok, d), "gpipe_op_ln_bwd");
+                    dgamma, dbeta, colsum_out, n_tok, d), "gpipe_op_ln_bwd");
 }
 int gpipe_op_attn_fwd(void *stream, int dtype, const void *qkv, void *o, float *lse, int n_seq, int S,
                       int A, int dh, int causal, int backend) {
@@ -105,8 +117,13 @@ int gpipe_op_softmax_ce(void *stream, int dtype, void *logits, const int32_t *la
                         int64_t n_tok, int V, float inv_T) {
   return ret(softmax_ce(mk(stream), dtype, logits, labels, rowloss, n_tok, V, inv_T), "gpipe_op_softmax_ce");
 }
-int gpipe_op_colsum(void *stream, int dtype, const void *dy, int64_t ld, float *out, int64_t n_tok, int n) {
-  return ret(colsum_accum(mk(stream), dtype, dy, ld, out, n_tok, n), "gpipe_op_colsum");
+int64_t gpipe_op_colsum_scratch_floats(int64_t n_tok, int n) {
+  int64_t r = colsum_scratch_rows(n_tok), t = (n_tok + 127) / 128;
+  return (r > t ? r : t) * n;
+}
+int gpipe_op_colsum(void *stream, int dtype, const void *dy, int64_t ld, float *out, float *scratch,
+                    int64_t n_tok, int n) {
+  return ret(colsum_accum(mk(stream), dtype, dy, ld, out, scratch, n_tok, n), "gpipe_op_colsum");
 }
 int gpipe_op_embed_fwd(void *stream, int dtype, const int32_t *tok, const void *emb, const float *pe,
                        float *x, int64_t n_tok, int S, int d) {

@@ -30,7 +30,7 @@ def _stream():
 
 
 def gemm(A, B_, C, *, transA=False, transB=False, bias=None, resid=None, mask=None, relu=False,
-         accumulate=False, backend=0):
+         accumulate=False, colsum_out=None, backend=0):
     """C = epilogue(op(A) @ op(B)); shapes follow gpipe_op_gemm.  C is written in place."""
     torch = _torch()
     M, N = C.shape
@@ -42,9 +42,14 @@ def gemm(A, B_, C, *, transA=False, transB=False, bias=None, resid=None, mask=No
     if resid is not None: flags |= B.EPI_RESID
     if accumulate: flags |= B.EPI_ACCUM
     if C.dtype == torch.float32: flags |= B.EPI_OUT_F32
+    scratch = None
+    if colsum_out is not None:
+        flags |= B.EPI_COLSUM
+        scratch = torch.empty(B.lib().gpipe_op_colsum_scratch_floats(M, N), dtype=torch.float32, device=C.device)
     B._check(B.lib().gpipe_op_gemm(_stream(), _dt(A), M, N, K, _p(A), A.stride(0), int(transA), _p(B_),
                                    B_.stride(0), int(transB), _p(C), C.stride(0), _p(bias), _p(resid),
-                                   _p(mask), mask.stride(0) if mask is not None else 0, flags, backend))
+                                   _p(mask), mask.stride(0) if mask is not None else 0, _p(colsum_out),
+                                   _p(scratch), flags, backend))
     return C
 
 
@@ -53,12 +58,12 @@ def ln_fwd(x, gamma, beta, y, mean, rstd, eps=1e-5):
     B._check(B.lib().gpipe_op_ln_fwd(_stream(), _dt(y), _p(x), _p(gamma), _p(beta), _p(y), _p(mean), _p(rstd), n, d, eps))
 
 
-def ln_bwd(dy, x, mean, rstd, gamma, dres_in, dx_out, dx_out_lp, dgamma, dbeta):
+def ln_bwd(dy, x, mean, rstd, gamma, dres_in, dx_out, dx_out_lp, dgamma, dbeta, colsum_out=None):
     torch = _torch()
     n, d = x.shape
     scratch = torch.empty(B.lib().gpipe_op_ln_bwd_scratch_floats(d), dtype=torch.float32, device=x.device)
     B._check(B.lib().gpipe_op_ln_bwd(_stream(), _dt(dy), _p(dy), _p(x), _p(mean), _p(rstd), _p(gamma), _p(dres_in),
-                                     _p(dx_out), _p(dx_out_lp), _p(scratch), _p(dgamma), _p(dbeta), n, d))
+                                     _p(dx_out), _p(dx_out_lp), _p(scratch), _p(dgamma), _p(dbeta), _p(colsum_out), n, d))
     return scratch
 
 
@@ -77,8 +82,10 @@ def softmax_ce(logits, labels, rowloss, inv_T):
 
 
 def colsum(dy, out):
+    torch = _torch()
     n, c = dy.shape
-    B._check(B.lib().gpipe_op_colsum(_stream(), _dt(dy), _p(dy), dy.stride(0), _p(out), n, c))
+    scratch = torch.empty(B.lib().gpipe_op_colsum_scratch_floats(n, c), dtype=torch.float32, device=dy.device)
+    B._check(B.lib().gpipe_op_colsum(_stream(), _dt(dy), _p(dy), dy.stride(0), _p(out), _p(scratch), n, c))
 
 
 def embed_fwd(tok, emb, pe, x, S):

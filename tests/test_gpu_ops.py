@@ -86,6 +86,20 @@ def test_gemm_epilogues(dtype, backend):
     assert maxrel(_np(rt), ref + bias + resid) <= 2e-5
     ops.gemm(At, Bt, C, mask=maskt, backend=backend)
     assert maxrel(_np(C), ref * (maskq > 0)) <= tol
+    # ReLU-mask + fused column sums of the stored output (dh and db_1 of a16 in one kernel)
+    cs0 = r.standard_normal(N).astype(np.float32)
+    cst = torch.tensor(cs0, device=DEV)
+    ops.gemm(At, Bt, C, mask=maskt, colsum_out=cst, backend=backend)
+    assert maxrel(_np(C), ref * (maskq > 0)) <= tol
+    assert maxrel(_np(cst), cs0 + _np(C).sum(0)) <= 2e-5
+    Mr, Nr = 200, 328                                        # ragged tiles
+    Ar, Arq = _lp(r.standard_normal((Mr, K)), dtype)
+    Br, Brq = _lp(r.standard_normal((K, Nr)), dtype)
+    Cr = torch.empty((Mr, Nr), device=DEV, dtype=At.dtype)
+    csr = torch.zeros(Nr, device=DEV)
+    ops.gemm(Ar, Br, Cr, colsum_out=csr, backend=backend)
+    assert maxrel(_np(Cr), Arq @ Brq) <= tol
+    assert maxrel(_np(csr), _np(Cr).sum(0)) <= 2e-5
     acc0 = r.standard_normal((K, N)).astype(np.float32)
     acc = torch.tensor(acc0, device=DEV)
     Xt, Xq = _lp(r.standard_normal((M, K)), dtype)
@@ -129,6 +143,12 @@ def test_layernorm_fwd_bwd(dtype, n, d):
     assert maxrel(_np(dbt), db_ref[0]) <= 2e-5
     ops.ln_bwd(dyt, xt, mean, rs, gt, None, dx, None, dgt, dbt)   # no incoming residual gradient
     assert maxrel(_np(dx), dx_ref) <= 2e-5
+    # fused bias gradient: colsum_out += sum_t dx_out (of the lp copy's values when there is one)
+    cs0 = r.standard_normal(d).astype(np.float32)
+    cst = torch.tensor(cs0, device=DEV)
+    ops.ln_bwd(dyt, xt, mean, rs, gt, torch.tensor(dres, device=DEV), dx, dx_lp, dgt, dbt, colsum_out=cst)
+    summed = _np(dx_lp) if dx_lp is not None else _np(dx)
+    assert maxrel(_np(cst), cs0 + summed.sum(0)) <= 2e-5
 
 
 # -------------------------------------------------------------------------------------------------

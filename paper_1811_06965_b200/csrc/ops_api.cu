@@ -22,7 +22,9 @@ cudaError_t attn_bwd_mma(const Ctx &c, const void *qkv, const void *o, const voi
 
 cudaError_t gemm(const Ctx &c, int dt, const GemmArgs &a) {
   const bool colsum = (a.flags & EPI_COLSUM) != 0;
-  if (colsum && (!a.colsum_out || !a.colsum_scratch || (a.flags & (EPI_OUT_F32 | EPI_ACCUM))))
+  // column sums are taken of the stored lp output (in fp32 mode lp storage is fp32 itself)
+  if (colsum && (!a.colsum_out || !a.colsum_scratch || (a.flags & EPI_ACCUM) ||
+                 ((a.flags & EPI_OUT_F32) && dt != GP_F32)))
     return cudaErrorInvalidValue;
   if (c.gemm_backend != 1 && gemm_tc_supported(dt, a)) {
     cudaError_t e = gemm_tc(c, a);             // EPI_COLSUM: per-tile-row partial sums -> scratch

@@ -62,6 +62,41 @@ def test_gemm_simt_all_layouts(dtype, transA, transB):
         assert cosine(_np(C), ref) >= cos
 
 
+# tensor-core path: shapes spanning several 256 x 256 pair tiles, a ragged tail in M, N and K, more
+# k-blocks than pipeline stages, and small shapes that take the 1-CTA kernel
+TC_SHAPES = [(512, 768, 320), (304, 520, 200), (1024, 256, 1088), (128, 136, 72), (264, 1032, 64)]
+
+
+@pytest.mark.parametrize("transA,transB", [(0, 0), (0, 1), (1, 0), (1, 1)])
+def test_gemm_tcgen05_all_layouts(transA, transB):
+    for (M, N, K) in TC_SHAPES:
+        r = _rng(M * 1000 + N + K)
+        At, Aq = _lp(r.standard_normal((K, M) if transA else (M, K)), "bf16")
+        Bt, Bq = _lp(r.standard_normal((N, K) if transB else (K, N)), "bf16")
+        ref = (Aq.T if transA else Aq) @ (Bq.T if transB else Bq)
+        Cf = torch.empty((M, N), device=DEV, dtype=torch.float32)
+        ops.gemm(At, Bt, Cf, transA=bool(transA), transB=bool(transB), backend=2)
+        assert maxrel(_np(Cf), ref) <= 2e-5, (M, N, K)          # fp32 accumulation of exact bf16 products
+        C = torch.empty((M, N), device=DEV, dtype=torch.bfloat16)
+        ops.gemm(At, Bt, C, transA=bool(transA), transB=bool(transB), backend=2)
+        assert maxrel(_np(C), ref) <= 2 ** -7 and cosine(_np(C), ref) >= 0.99999, (M, N, K)
+
+
+def test_gemm_tcgen05_bench_shapes_sampled():
+    """The launch configurations bench.py times (T_mb = 2048 tokens, d = 1024): full-size GEMMs
+    checked on sampled rows the oracle's matmul can compute one by one."""
+    r = _rng(77)
+    for (M, N, K, tA, tB) in [(2048, 1024, 4096, 0, 0), (2048, 4096, 1024, 0, 1), (1024, 4096, 2048, 1, 0)]:
+        At, Aq = _lp(r.standard_normal((K, M) if tA else (M, K)) * 0.5, "bf16")
+        Bt, Bq = _lp(r.standard_normal((N, K) if tB else (K, N)) * 0.5, "bf16")
+        Cf = torch.empty((M, N), device=DEV, dtype=torch.float32)
+        ops.gemm(At, Bt, Cf, transA=bool(tA), transB=bool(tB), backend=2)
+        rows = r.choice(M, size=24, replace=False)
+        A_rows = (Aq.T if tA else Aq)[rows]
+        ref = A_rows @ (Bq.T if tB else Bq)
+        assert maxrel(_np(Cf)[rows], ref) <= 2e-5, (M, N, K)
+
+
 @pytest.mark.parametrize("dtype", ["fp32", "bf16"])
 @pytest.mark.parametrize("backend", [1, 0])
 def test_gemm_epilogues(dtype, backend):

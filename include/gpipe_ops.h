@@ -25,12 +25,16 @@ extern "C" {
 /* epilogue flags of gpipe_op_gemm */
 #define GPIPE_EPI_BIAS    1   /* + bias[n]            (fp32 [N])                                  */
 #define GPIPE_EPI_RELU    2   /* max(v, 0)                                                        */
-#define GPIPE_EPI_MASK    4   /* v * [mask[m,n] > 0]  (lp [M, ldmask]; ReLU backward)             */
+#define GPIPE_EPI_MASK    4   /* v * maskbit[m,n]: mask is a bit-packed uint32 [M, ldmask] array, bit
+                                 (n % 32) of word n / 32 (ReLU backward); ldmask >= ceil(N / 32)      */
 #define GPIPE_EPI_RESID   8   /* + resid[m,n]         (fp32 [M, ldc], may alias C)                */
 #define GPIPE_EPI_ACCUM  16   /* C (fp32) += v        (wgrad accumulation across micro-batches)   */
 #define GPIPE_EPI_OUT_F32 32  /* C is fp32, else lp                                               */
 #define GPIPE_EPI_COLSUM 64   /* colsum_out[n] += sum_m C[m,n] of the stored values (bias gradient
                                  of the layer below, fused into the dgrad GEMM); lp output only   */
+#define GPIPE_EPI_BITS_OUT 128 /* mask (layout of GPIPE_EPI_MASK) is an OUTPUT: bit = [stored C > 0]
+                                 (the FFN1 epilogue records the ReLU pattern in 1 bit per unit
+                                 instead of having backward re-read h)                             */
 
 /* C[M,N] = epilogue(op(A)[M,K] op(B)[K,N]), fp32 accumulation.  transA = 0: A stored [M,K]
  * row-major, 1: stored [K,M]; transB = 0: B stored [K,N], 1: stored [N,K].  backend: 0 = auto
@@ -39,7 +43,7 @@ extern "C" {
  * [gpipe_op_colsum_scratch_floats(M, N)] are only read with GPIPE_EPI_COLSUM. */
 int gpipe_op_gemm(void *stream, int dtype, int M, int N, int K, const void *A, int64_t lda, int transA,
                   const void *B, int64_t ldb, int transB, void *C, int64_t ldc, const float *bias,
-                  const float *resid, const void *mask, int64_t ldmask, float *colsum_out,
+                  const float *resid, void *mask, int64_t ldmask, float *colsum_out,
                   float *colsum_scratch, int flags, int backend);
 
 /* y = LayerNorm(x) * gamma + beta over the last axis (biased variance); y lp [n_tok,d]; x fp32. */

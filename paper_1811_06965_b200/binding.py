@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libgpipe_b200.so")
 
 DTYPE_FP32, DTYPE_BF16 = 0, 1
 CATEGORIES = ["weights", "masters", "grads", "boundary", "interior", "head", "misc", "bwd_scratch"]
-EPI_BIAS, EPI_RELU, EPI_MASK, EPI_RESID, EPI_ACCUM, EPI_OUT_F32, EPI_COLSUM = 1, 2, 4, 8, 16, 32, 64
+EPI_BIAS, EPI_RELU, EPI_MASK, EPI_RESID, EPI_ACCUM, EPI_OUT_F32, EPI_COLSUM, EPI_BITS_OUT = 1, 2, 4, 8, 16, 32, 64, 128
 
 
 class GPipeError(RuntimeError):

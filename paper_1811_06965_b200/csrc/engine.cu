@@ -118,6 +118,7 @@ int Engine::build_plan(bool dry, std::string &err) {
         b.o = LP(Tm * da, cat, k);
         b.c = LP(Tm * d, cat, k);
         b.h = LP(Tm * H, cat, k);
+        b.hbits = (uint32_t *)arena.alloc(Tm * (size_t)((H + 31) / 32) * 4, cat, k);
         b.x1 = F32(Tm * d, cat, k);
         b.x2 = i + 1 < nl ? F32(Tm * d, cat, k) : nullptr;
         b.lse = F32(Tm * A, cat, k);
@@ -185,7 +186,7 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
     double by = ((double)g.M * g.K + (double)g.K * g.N) * lpb + (double)g.M * g.N * outb;
     if (g.flags & EPI_RESID) by += (double)g.M * g.N * 4.0;
     if (g.flags & EPI_ACCUM) by += (double)g.M * g.N * 4.0;
-    if (g.flags & EPI_MASK) by += (double)g.M * g.N * lpb;
+    if (g.flags & (EPI_MASK | EPI_BITS_OUT)) by += (double)g.M * g.N / 8.0;
     return timed(k, cls, fl, by, [&] { return gemm(c, dt, g); });
   };
   auto tln = [&](const float *x_, const float *g_, const float *b_, void *y_, float *mu_, float *rs_) -> cudaError_t {
@@ -230,7 +231,8 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
     g = GemmArgs{};
     g.M = (int)T_mb; g.N = H; g.K = d;
     g.A = b.c; g.lda = d; g.B = W(q.w_1); g.ldb = H; g.C = b.h; g.ldc = H;
-    g.bias = P(q.b_1); g.flags = EPI_BIAS | EPI_RELU;
+    g.bias = P(q.b_1); g.flags = EPI_BIAS | EPI_RELU | EPI_BITS_OUT;
+    g.mask = b.hbits; g.ldmask = (H + 31) / 32;   // 1 bit per unit for the ReLU backward (a16)
     GP_TRY(tgemm(KC_GEMM_FWD, g));
     // x2 = x1 + h W_2 + b_2                                                  (a11)
     float *x2;
@@ -298,13 +300,13 @@ cudaError_t Engine::backward_cell(int k, int m) {
     return timed(k, KC_GEMM_WGRAD, 2.0 * g.M * g.N * (double)g.K, by, [&] { return gemm(c, dt, g); });
   };
   auto dgrad = [&](const void *dY, int64_t ldy, int Kout, int iw, int Nin, void *dX,
-                   const void *mask, float *colsum_to = nullptr) -> cudaError_t {
+                   uint32_t *mask, float *colsum_to = nullptr) -> cudaError_t {
     GemmArgs g{};
     g.M = (int)T_mb; g.N = Nin; g.K = Kout;
     g.A = dY; g.lda = ldy; g.transA = 0; g.B = W(iw); g.ldb = Kout; g.transB = 1;
-    g.C = dX; g.ldc = Nin; g.mask = mask; g.ldmask = Nin; g.flags = mask ? EPI_MASK : 0;
+    g.C = dX; g.ldc = Nin; g.mask = mask; g.ldmask = (Nin + 31) / 32; g.flags = mask ? EPI_MASK : 0;
     if (colsum_to) { g.flags |= EPI_COLSUM; g.colsum_out = colsum_to; g.colsum_scratch = s.colsum_scratch; }
-    double by = ((double)g.M * g.K + (double)g.K * g.N + (double)g.M * g.N * (mask ? 2.0 : 1.0)) * lpb;
+    double by = ((double)g.M * g.K + (double)g.K * g.N + (double)g.M * g.N) * lpb + (mask ? (double)g.M * g.N / 8.0 : 0.0);
     return timed(k, KC_GEMM_DGRAD, 2.0 * g.M * g.N * (double)g.K, by, [&] { return gemm(c, dt, g); });
   };
 
@@ -330,7 +332,7 @@ cudaError_t Engine::backward_cell(int k, int m) {
     const float *x_in = i > 0 ? w.layers[i - 1].x2 : (k == 0 ? w.x_emb : slot[k][m]);
     // FFN: dh = (dx W_2^T) * [h > 0] with db_1 += sum_t dh fused into the epilogue; dW_2 += h^T dx
     // (db_2 += sum_t dx was fused into the LayerNorm-backward kernel that produced dx)
-    GP_TRY(dgrad(dxo, d, d, q.w_2, H, s.dh, b.h, G(q.b_1)));
+    GP_TRY(dgrad(dxo, d, d, q.w_2, H, s.dh, b.hbits, G(q.b_1)));
     GP_TRY(wgrad(b.h, H, H, dxo, d, d, q.w_2));
     // dc = dh W_1^T; dW_1 += c^T dh
     GP_TRY(dgrad(s.dh, H, H, q.w_1, d, s.dc, nullptr));

@@ -25,6 +25,7 @@ struct LayerParams {  // indices into Engine::tensors
 // Interior activations of one layer that the backward pass needs.
 struct LayerBuf {
   void *a, *qkv, *o, *c, *h;             // lp
+  uint32_t *hbits;                       // [T_mb, H/32] bit-packed ReLU pattern [h > 0] (written by FFN1's epilogue)
   float *x1, *x2;                        // fp32 residual stream (x2 unused for the cell's last layer)
   float *lse, *mean1, *rstd1, *mean2, *rstd2;
 };

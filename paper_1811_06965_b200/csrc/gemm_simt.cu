@@ -1,8 +1,8 @@
 // gemm_simt.cu - fp32-FMA GEMM (no tensor cores, TF32 off) for the fp32 parity configuration and
 // for shapes the tcgen05 kernel does not take (ragged / unaligned).  64x64x16 tiles, 256 threads,
 // 4x4 outputs per thread, any transposition via index arithmetic, bounds-checked edges.
-// The same fused epilogue as the tensor-core kernel (ops.h): +bias, ReLU, ReLU-mask, +residual,
-// fp32 accumulate.  Bound: ALU (fp32 FMA); only correctness matters for this path.
+// The same fused epilogue as the tensor-core kernel (ops.h): +bias, ReLU, bit-packed ReLU mask
+// in / out, +residual, fp32 accumulate.  Bound: ALU (fp32 FMA); only correctness matters for this path.
 #include "common.cuh"
 
 namespace gp {
@@ -72,19 +72,19 @@ gemm_simt_kernel(GemmArgs g) {
     __syncthreads();
   }
 
-  const T *mask = (const T *)g.mask;
+  const uint32_t *maskbits = (const uint32_t *)g.mask;
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
     int m = m0 + ty * 4 + i;
-    if (m >= g.M) continue;
+    uint32_t nib = 0;                                 // [stored value > 0] of this thread's 4 columns
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
       int n = n0 + tx * 4 + j;
-      if (n >= g.N) continue;
+      if (m >= g.M || n >= g.N) continue;
       float v = acc[i][j];
       if (g.flags & EPI_BIAS) v += g.bias[n];
       if (g.flags & EPI_RELU) v = fmaxf(v, 0.f);
-      if (g.flags & EPI_MASK) v = to_f<T>(mask[(int64_t)m * g.ldmask + n]) > 0.f ? v : 0.f;
+      if (g.flags & EPI_MASK) v = ((maskbits[(int64_t)m * g.ldmask + (n >> 5)] >> (n & 31)) & 1u) ? v : 0.f;
       if (g.flags & EPI_RESID) v += g.resid[(int64_t)m * g.ldc + n];
       int64_t ci = (int64_t)m * g.ldc + n;
       if (g.flags & EPI_ACCUM) {
@@ -93,8 +93,20 @@ gemm_simt_kernel(GemmArgs g) {
       } else if (g.flags & EPI_OUT_F32) {
         ((float *)g.C)[ci] = v;
       } else {
-        ((T *)g.C)[ci] = from_f<T>(v);
+        T s = from_f<T>(v);
+        ((T *)g.C)[ci] = s;
+        v = to_f<T>(s);
       }
+      nib |= (v > 0.f ? 1u : 0u) << j;
+    }
+    if (g.flags & EPI_BITS_OUT) {
+      // the 8 threads tx & ~7 .. tx | 7 of a row hold one 32-bit word (consecutive lanes of a warp)
+      uint32_t w = nib << (4 * (tx & 7));
+      w |= __shfl_xor_sync(0xffffffffu, w, 1);
+      w |= __shfl_xor_sync(0xffffffffu, w, 2);
+      w |= __shfl_xor_sync(0xffffffffu, w, 4);
+      int n_word = n0 + (tx & ~7) * 4;
+      if ((tx & 7) == 0 && m < g.M && n_word < g.N) ((uint32_t *)g.mask)[(int64_t)m * g.ldmask + (n_word >> 5)] = w;
     }
   }
 }

@@ -24,15 +24,17 @@ inline size_t lp_size(int dt) { return dt == GP_BF16 ? 2 : 4; }
 // C[M,N] = epilogue( op(A)[M,K] * op(B)[K,N] ), fp32 accumulation.
 //   transA == 0: A stored [M,K] row-major (lda >= K);  transA == 1: A stored [K,M] (lda >= M)
 //   transB == 0: B stored [K,N] row-major (ldb >= N);  transB == 1: B stored [N,K] (ldb >= K)
-// Epilogue, in this order: +bias[n]; relu; *[mask[m,n] > 0]; +resid[m,n]; +C_old[m,n].
+// Epilogue, in this order: +bias[n]; relu; *maskbit[m,n]; +resid[m,n]; +C_old[m,n]; store; bits out.
 enum {
   EPI_BIAS = 1,       // bias: fp32 [N]
   EPI_RELU = 2,
-  EPI_MASK = 4,       // mask: lp [M, ldmask]; keeps v where mask > 0, else 0 (ReLU backward)
+  EPI_MASK = 4,       // mask: bit-packed uint32 [M, ldmask] (bit n%32 of word n/32); keeps v where the bit
+                      // is set, else 0 (ReLU backward); ldmask >= ceil(N/32)
   EPI_RESID = 8,      // resid: fp32 [M, ldc]  (may alias C)
   EPI_ACCUM = 16,     // C is fp32 and is read-modify-written: C += v   (wgrad accumulation)
   EPI_OUT_F32 = 32,   // C is fp32 (else lp)
-  EPI_COLSUM = 64     // colsum_out[n] += sum_m C[m,n] (of the stored, rounded values); needs colsum_scratch
+  EPI_COLSUM = 64,    // colsum_out[n] += sum_m C[m,n] (of the stored, rounded values); needs colsum_scratch
+  EPI_BITS_OUT = 128  // mask (same layout as EPI_MASK) is WRITTEN: bit = [stored value > 0]
 };
 struct GemmArgs {
   int M, N, K;
@@ -41,7 +43,7 @@ struct GemmArgs {
   void *C; int64_t ldc;
   const float *bias;
   const float *resid;
-  const void *mask; int64_t ldmask;
+  void *mask; int64_t ldmask;      // uint32 words, ldmask in words
   int flags;
   float *colsum_out;       // EPI_COLSUM: fp32 [N], accumulated into
   float *colsum_scratch;   // EPI_COLSUM: fp32 [ceil(M/128), N]

@@ -74,7 +74,7 @@ static int ret(cudaError_t e, const char *where) {
 extern "C" {
 int gpipe_op_gemm(void *stream, int dtype, int M, int N, int K, const void *A, int64_t lda, int transA,
                   const void *B, int64_t ldb, int transB, void *C, int64_t ldc, const float *bias,
-                  const float *resid, const void *mask, int64_t ldmask, float *colsum_out,
+                  const float *resid, void *mask, int64_t ldmask, float *colsum_out,
                   float *colsum_scratch, int flags, int backend) {
   GemmArgs g{};
   g.colsum_out = colsum_out; g.colsum_scratch = colsum_scratch;

@@ -30,8 +30,9 @@ def _stream():
 
 
 def gemm(A, B_, C, *, transA=False, transB=False, bias=None, resid=None, mask=None, relu=False,
-         accumulate=False, colsum_out=None, backend=0):
-    """C = epilogue(op(A) @ op(B)); shapes follow gpipe_op_gemm.  C is written in place."""
+         accumulate=False, colsum_out=None, bits_out=None, backend=0):
+    """C = epilogue(op(A) @ op(B)); shapes follow gpipe_op_gemm.  C is written in place.
+    mask / bits_out: int32 [M, N/32] bit-packed ReLU pattern (read / written)."""
     torch = _torch()
     M, N = C.shape
     K = A.shape[0] if transA else A.shape[1]
@@ -39,6 +40,10 @@ def gemm(A, B_, C, *, transA=False, transB=False, bias=None, resid=None, mask=No
     if bias is not None: flags |= B.EPI_BIAS
     if relu: flags |= B.EPI_RELU
     if mask is not None: flags |= B.EPI_MASK
+    if bits_out is not None:
+        assert mask is None
+        flags |= B.EPI_BITS_OUT
+        mask = bits_out
     if resid is not None: flags |= B.EPI_RESID
     if accumulate: flags |= B.EPI_ACCUM
     if C.dtype == torch.float32: flags |= B.EPI_OUT_F32

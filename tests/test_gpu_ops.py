@@ -107,25 +107,30 @@ def test_gemm_epilogues(dtype, backend):
     Bt, Bq = _lp(r.standard_normal((K, N)), dtype)
     bias = r.standard_normal(N).astype(np.float32)
     resid = r.standard_normal((M, N)).astype(np.float32)
-    maskt, maskq = _lp(np.maximum(r.standard_normal((M, N)), 0), dtype)
+    maskq = r.standard_normal((M, N)) > 0                   # bit-packed ReLU pattern, bit n%32 of word n/32
+    maskt = torch.tensor(np.packbits(maskq.reshape(M, N // 32, 32), axis=-1, bitorder="little")
+                         .view(np.uint32).reshape(M, N // 32).view(np.int32), device=DEV)
     bt, rt = torch.tensor(bias, device=DEV), torch.tensor(resid, device=DEV)
     tol, cos = _tol(dtype)
     ref = Aq @ Bq
     C = torch.empty((M, N), device=DEV, dtype=At.dtype)
-    ops.gemm(At, Bt, C, bias=bt, relu=True, backend=backend)
+    bits = torch.zeros((M, N // 32), device=DEV, dtype=torch.int32)
+    ops.gemm(At, Bt, C, bias=bt, relu=True, bits_out=bits, backend=backend)
     assert maxrel(_np(C), np.maximum(ref + bias, 0)) <= tol
+    got = np.unpackbits(bits.cpu().numpy().view(np.uint8).reshape(M, N // 8), axis=-1, bitorder="little").astype(bool)
+    assert np.array_equal(got, _np(C) > 0)                   # the recorded pattern is [stored h > 0]
     Cf = torch.empty((M, N), device=DEV, dtype=torch.float32)
     ops.gemm(At, Bt, Cf, bias=bt, resid=rt, backend=backend)
     assert maxrel(_np(Cf), ref + bias + resid) <= 2e-5
     ops.gemm(At, Bt, rt, bias=bt, resid=rt, backend=backend)            # residual aliasing the output
     assert maxrel(_np(rt), ref + bias + resid) <= 2e-5
     ops.gemm(At, Bt, C, mask=maskt, backend=backend)
-    assert maxrel(_np(C), ref * (maskq > 0)) <= tol
+    assert maxrel(_np(C), ref * maskq) <= tol
     # ReLU-mask + fused column sums of the stored output (dh and db_1 of a16 in one kernel)
     cs0 = r.standard_normal(N).astype(np.float32)
     cst = torch.tensor(cs0, device=DEV)
     ops.gemm(At, Bt, C, mask=maskt, colsum_out=cst, backend=backend)
-    assert maxrel(_np(C), ref * (maskq > 0)) <= tol
+    assert maxrel(_np(C), ref * maskq) <= tol
     assert maxrel(_np(cst), cs0 + _np(C).sum(0)) <= 2e-5
     Mr, Nr = 200, 328                                        # ragged tiles
     Ar, Arq = _lp(r.standard_normal((Mr, K)), dtype)

@@ -40,11 +40,16 @@ extern "C" {
  * row-major, 1: stored [K,M]; transB = 0: B stored [K,N], 1: stored [N,K].  backend: 0 = auto
  * (tcgen05 tensor cores for bf16 when the shape is tile-aligned), 1 = fp32-FMA SIMT kernel,
  * 2 = tcgen05 or fail with GPIPE_EINVAL.  colsum_out fp32 [N] / colsum_scratch fp32
- * [gpipe_op_colsum_scratch_floats(M, N)] are only read with GPIPE_EPI_COLSUM. */
+ * [gpipe_op_colsum_scratch_floats(M, N)] are only read with GPIPE_EPI_COLSUM.
+ * workspace (device, may be NULL): gpipe_op_gemm_workspace_bytes(M, N, K) bytes that were ZERO before
+ * their first use and are only ever used by launches on one stream at a time; with it, shapes
+ * with few output tiles and a long K are split along K over all SMs and reduced in a fixed order
+ * (deterministic); without it they are not split. */
+int64_t gpipe_op_gemm_workspace_bytes(int M, int N, int K);
 int gpipe_op_gemm(void *stream, int dtype, int M, int N, int K, const void *A, int64_t lda, int transA,
                   const void *B, int64_t ldb, int transB, void *C, int64_t ldc, const float *bias,
                   const float *resid, void *mask, int64_t ldmask, float *colsum_out,
-                  float *colsum_scratch, int flags, int backend);
+                  float *colsum_scratch, void *workspace, int64_t workspace_bytes, int flags, int backend);
 
 /* y = LayerNorm(x) * gamma + beta over the last axis (biased variance); y lp [n_tok,d]; x fp32. */
 int gpipe_op_ln_fwd(void *stream, int dtype, const float *x, const float *gamma, const float *beta,

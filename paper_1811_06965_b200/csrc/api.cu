@@ -139,6 +139,8 @@ int gpipe_create(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t 
   if (ce == cudaSuccess) ce = cudaMemsetAsync(e.grad, 0, (size_t)e.n_flat * 4, c.stream);
   if (ce == cudaSuccess && e.dt == GP_BF16) ce = cudaMemsetAsync(e.w_lp, 0, (size_t)e.n_flat * 2, c.stream);
   if (ce == cudaSuccess) ce = cudaMemsetAsync(e.flag_dev, 0, 4, c.stream);
+  for (int k = 0; k < K && ce == cudaSuccess; ++k)          // split-K counters start at zero and reset themselves
+    if (e.bwd[k].splitk_ws) ce = cudaMemsetAsync(e.bwd[k].splitk_ws, 0, e.splitk_ws_bytes, c.stream);
   if (ce == cudaSuccess) ce = positional_table(c, e.pe, e.S, e.d);
   if (ce == cudaSuccess) ce = cudaStreamSynchronize(c.stream);
   if (ce != cudaSuccess) { gpipe_destroy(g); return cuda_fail(ce, "gpipe_create"); }

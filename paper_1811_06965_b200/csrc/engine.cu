@@ -99,6 +99,18 @@ int Engine::build_plan(bool dry, std::string &err) {
     }
   }
 
+  // split-K workspace: the largest any GEMM shape of a cell needs (forward, dgrad, wgrad)
+  splitk_ws_bytes = 0;
+  if (dt == GP_BF16) {
+    const int T = (int)T_mb;
+    const int shapes[][3] = {{T, 3 * da, d}, {T, d, da}, {T, H, d}, {T, d, H}, {T, V, d},          // forward
+                             {T, da, d}, {T, d, 3 * da}, {T, d, V},                                 // dgrad (others as forward)
+                             {H, d, T}, {d, H, T}, {da, d, T}, {d, 3 * da, T}, {d, V, T}};            // wgrad
+    for (auto &sh : shapes) {
+      size_t b = gemm_splitk_ws_bytes(sh[0], sh[1], sh[2], sm_count);
+      if (b > splitk_ws_bytes) splitk_ws_bytes = b;
+    }
+  }
   ws.assign(K, std::vector<Workspace>());
   bwd.assign(K, BwdScratch());
   for (int k = 0; k < K; ++k) {
@@ -154,6 +166,7 @@ int Engine::build_plan(bool dry, std::string &err) {
       if (cols < (size_t)d) cols = d;
       s.colsum_scratch = F32(rows * cols, cat, k);
     }
+    s.splitk_ws = splitk_ws_bytes ? arena.alloc(splitk_ws_bytes, cat, k) : nullptr;
   }
   if (!dry && arena.used > arena.cap) {
     err = "arena too small: need " + std::to_string(arena.used) + " bytes, have " +
@@ -187,7 +200,9 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
     if (g.flags & EPI_RESID) by += (double)g.M * g.N * 4.0;
     if (g.flags & EPI_ACCUM) by += (double)g.M * g.N * 4.0;
     if (g.flags & (EPI_MASK | EPI_BITS_OUT)) by += (double)g.M * g.N / 8.0;
-    return timed(k, cls, fl, by, [&] { return gemm(c, dt, g); });
+    GemmArgs gw = g;
+    gw.ws = bwd[k].splitk_ws; gw.ws_bytes = splitk_ws_bytes;
+    return timed(k, cls, fl, by, [&] { return gemm(c, dt, gw); });
   };
   auto tln = [&](const float *x_, const float *g_, const float *b_, void *y_, float *mu_, float *rs_) -> cudaError_t {
     return timed(k, KC_LN_FWD, 0, Td * d * (4.0 + lpb), [&] { return ln_fwd(c, dt, x_, g_, b_, y_, mu_, rs_, T_mb, d, eps); });
@@ -296,6 +311,7 @@ cudaError_t Engine::backward_cell(int k, int m) {
     g.M = Min; g.N = Nout; g.K = (int)T_mb;
     g.A = X; g.lda = ldx; g.transA = 1; g.B = dY; g.ldb = ldy; g.transB = 0;
     g.C = G(iw); g.ldc = Nout; g.flags = EPI_ACCUM | EPI_OUT_F32;
+    g.ws = s.splitk_ws; g.ws_bytes = splitk_ws_bytes;
     double by = ((double)g.M * g.K + (double)g.K * g.N) * lpb + (double)g.M * g.N * 8.0;
     return timed(k, KC_GEMM_WGRAD, 2.0 * g.M * g.N * (double)g.K, by, [&] { return gemm(c, dt, g); });
   };
@@ -306,6 +322,7 @@ cudaError_t Engine::backward_cell(int k, int m) {
     g.A = dY; g.lda = ldy; g.transA = 0; g.B = W(iw); g.ldb = Kout; g.transB = 1;
     g.C = dX; g.ldc = Nin; g.mask = mask; g.ldmask = (Nin + 31) / 32; g.flags = mask ? EPI_MASK : 0;
     if (colsum_to) { g.flags |= EPI_COLSUM; g.colsum_out = colsum_to; g.colsum_scratch = s.colsum_scratch; }
+    g.ws = s.splitk_ws; g.ws_bytes = splitk_ws_bytes;
     double by = ((double)g.M * g.K + (double)g.K * g.N + (double)g.M * g.N) * lpb + (mask ? (double)g.M * g.N / 8.0 : 0.0);
     return timed(k, KC_GEMM_DGRAD, 2.0 * g.M * g.N * (double)g.K, by, [&] { return gemm(c, dt, g); });
   };

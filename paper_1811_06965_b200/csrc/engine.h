@@ -45,6 +45,7 @@ struct BwdScratch {                      // one per cell
   float *dvec;                           // attention D = rowsum(dO*O)
   float *ln_partials;
   float *colsum_scratch;                 // [max(T_mb/128, colsum rows), max(H, 3*da, d)]
+  void *splitk_ws;                       // split-K partials + counters of this cell's GEMMs (one stream -> one user at a time)
 };
 
 struct Arena {
@@ -77,6 +78,7 @@ struct Engine {
   int sm_count = 148;
   int gemm_backend = 0;
   int replay_full = 0;
+  size_t splitk_ws_bytes = 0;
 
   std::vector<TensorInfo> tensors;
   std::vector<LayerParams> lp;

@@ -54,6 +54,14 @@ struct Params {
   int flags;
   int tiles_m, tiles_n;
   float *colpart;               // EPI_COLSUM: fp32 [ceil(M/128), N] per-128-row column sums
+  // split-K (few output tiles, long K): `splits` work units per tile, each a contiguous range of
+  // kb_per_split K-blocks.  The first splits-1 CTAs to finish a (tile, rank) write their raw fp32
+  // accumulators to ws_part; the last one adds them to its own IN SPLIT ORDER (bitwise
+  // deterministic, whoever is last) and runs the epilogue.  Nobody waits on a CTA that is not
+  // already running.  ws_cnt: 2 self-resetting counters per (tile, rank).
+  int splits, kb_per_split;
+  float *ws_part;               // [tile][split][rank][128][BN] fp32
+  unsigned int *ws_cnt;         // [tile][rank][2]: arrivals, partials ready
 };
 
 template <int BN> struct PairCfg {
@@ -97,6 +105,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
   __shared__ uint32_t tmem_base_smem;
   __shared__ __align__(16) float bias_s[2][BN];
   __shared__ float colbuf[4][BN];
+  __shared__ int split_last_s;
 
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t staging_base = smem_base + NST * STAGE_BYTES;
@@ -135,7 +144,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
   tcgen05_fence_after();
   const uint32_t tmem_base = tmem_base_smem;
 
-  const int num_tiles = p.tiles_m * p.tiles_n;
+  const int num_units = p.tiles_m * p.tiles_n * p.splits;     // work units: (tile, split), splits adjacent
   const int num_kb = (p.K + BK - 1) / BK;
 
   if (warp == 0) {
@@ -143,9 +152,11 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
     if (lane == 0) {
       int stage = 0;
       uint32_t phase = 0;
-      for (int t = pair; t < num_tiles; t += num_pairs) {
+      for (int u = pair; u < num_units; u += num_pairs) {
+        const int t = u / p.splits, sp = u - t * p.splits;
         const int m0 = (t % p.tiles_m) * 256 + (int)rank * 128, n0 = (t / p.tiles_m) * BN + (int)rank * BNH;
-        for (int kb = 0; kb < num_kb; ++kb) {
+        const int kb0 = sp * p.kb_per_split, kb1 = min(num_kb, kb0 + p.kb_per_split);
+        for (int kb = kb0; kb < kb1; ++kb) {
           mbar_wait(empty_bar(stage), phase ^ 1);
           const uint32_t sa = smem_base + stage * STAGE_BYTES, sb = sa + A_BYTES;
           if (rank == 0) mbar_expect_tx(full_bar(stage), 2 * STAGE_BYTES);
@@ -184,11 +195,13 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
       uint32_t phase = 0;
       int as = 0;
       uint32_t aphase = 0;
-      for (int t = pair; t < num_tiles; t += num_pairs) {
+      for (int u = pair; u < num_units; u += num_pairs) {
+        const int sp = u % p.splits;
+        const int kb0 = sp * p.kb_per_split, kb1 = min(num_kb, kb0 + p.kb_per_split);
         mbar_wait(tempty_bar(as), aphase ^ 1);       // both CTAs' epilogues have drained this accumulator
         tcgen05_fence_after();
         const uint32_t d_tmem = tmem_base + (uint32_t)(as * BN);
-        for (int kb = 0; kb < num_kb; ++kb) {
+        for (int kb = kb0; kb < kb1; ++kb) {
           mbar_wait(full_bar(stage), phase);
           tcgen05_fence_after();
           const uint32_t sa = smem_base + stage * STAGE_BYTES, sb = sa + A_BYTES;
@@ -196,7 +209,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
           for (int k = 0; k < BK / 16; ++k) {
             const uint64_t ad = make_smem_desc(sa + k * a_kstep, a_lbo, a_sbo);
             const uint64_t bd = make_smem_desc(sb + k * b_kstep, b_lbo, b_sbo);
-            umma_bf16_pair(d_tmem, ad, bd, idesc, (kb | k) ? 1u : 0u);
+            umma_bf16_pair(d_tmem, ad, bd, idesc, (kb > kb0 || k) ? 1u : 0u);
           }
           tcgen05_commit_pair(empty_bar(stage), 3);  // frees this stage in both CTAs
           if (++stage == NST) { stage = 0; phase ^= 1; }
@@ -215,7 +228,8 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
     const uint32_t swz = (uint32_t)(lane & 7);
     int as = 0, it = 0, sbuf = 0;
     uint32_t aphase = 0;
-    for (int t = pair; t < num_tiles; t += num_pairs, ++it) {
+    for (int u = pair; u < num_units; u += num_pairs, ++it) {
+      const int t = u / p.splits, sp = u - t * p.splits;
       const int m0 = (t % p.tiles_m) * 256 + (int)rank * 128, n0 = (t / p.tiles_m) * BN;
       const int row0 = m0 + quad * 32, row = row0 + lane;
       const bool row_ok = row < p.M;
@@ -223,21 +237,51 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
       if (p.flags & EPI_BIAS) {
         for (int i = et; i < BN; i += 128) bs[i] = (n0 + i < p.N) ? __ldg(p.bias + n0 + i) : 0.f;
       }
-      uint32_t mb[NCH];
-      if (p.flags & EPI_MASK) {
+      // this row's ReLU-pattern words for the whole tile (one 32-byte sector), fetched before the wait
+      uint32_t mb[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+      if ((p.flags & EPI_MASK) && row_ok) {
+        const uint32_t *mp = p.maskbits + (int64_t)row * p.ldmask + (n0 >> 5);
+        if (NCH == 8 && n0 + BN <= p.N && (p.ldmask & 3) == 0) {
+          const uint4 lo = __ldg(reinterpret_cast<const uint4 *>(mp)), hi = __ldg(reinterpret_cast<const uint4 *>(mp + 4));
+          mb[0] = lo.x; mb[1] = lo.y; mb[2] = lo.z; mb[3] = lo.w;
+          mb[4] = hi.x; mb[5] = hi.y; mb[6] = hi.z; mb[7] = hi.w;
+        } else {
 #pragma unroll
-        for (int c = 0; c < NCH; ++c)
-          mb[c] = (row_ok && n0 + c * 32 < p.N) ? __ldg(p.maskbits + (int64_t)row * p.ldmask + (n0 >> 5) + c) : 0u;
+          for (int c = 0; c < NCH; ++c)
+            if (n0 + c * 32 < p.N) mb[c] = __ldg(mp + c);
+        }
       }
       asm volatile("bar.sync 1, 128;" ::: "memory");       // bias_s visible; colbuf of the previous tile consumed
       mbar_wait(tfull_bar(as), aphase);
       tcgen05_fence_after();
       const uint32_t t_row = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(as * BN);
-      uint32_t wbits[NCH];
-#pragma unroll
+      // ---- split-K: am I the last of this (tile, rank)'s splits to finish? ----
+      bool write_partial = false;
+      if (p.splits > 1) {
+        unsigned int *cnt = p.ws_cnt + ((size_t)t * 2 + rank) * 2;
+        if (et == 0) {
+          const unsigned int arrived = atomicAdd(cnt, 1u);
+          if (arrived == (unsigned int)p.splits - 1) {          // last: wait for the partials already being written
+            while (atomicAdd(cnt + 1, 0u) < (unsigned int)p.splits - 1) __nanosleep(64);
+            cnt[0] = 0u;                                        // self-reset for the next launch on this stream
+            cnt[1] = 0u;
+            __threadfence();
+            split_last_s = 1;
+          } else {
+            split_last_s = 0;
+          }
+        }
+        asm volatile("bar.sync 2, 128;" ::: "memory");
+        write_partial = split_last_s == 0;
+      }
+      float *part_row = p.ws_part + (((size_t)t * p.splits) * 2 + rank) * (size_t)(128 * BN) +
+                        (size_t)(quad * 32 + lane) * BN;          // split 0 of this (tile, rank), this lane's row
+      const size_t part_split_stride = (size_t)2 * 128 * BN;
+      // one 32-column chunk per iteration; NOT unrolled: the epilogue has to stay resident in the
+      // instruction cache next to the other warp roles
+#pragma unroll 1
       for (int c = 0; c < NCH; ++c) {
         const int col0 = n0 + c * 32;
-        wbits[c] = 0u;
         if (col0 < p.N) {                                    // uniform over the CTA
           uint32_t r[32];
           tmem_ld32(t_row + c * 32, r);
@@ -264,6 +308,36 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
           float v[32];
 #pragma unroll
           for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]);
+          if (p.splits > 1) {
+            if (write_partial) {                               // raw accumulators -> workspace; no epilogue
+              float4 *dst = reinterpret_cast<float4 *>(part_row + sp * part_split_stride + c * 32);
+#pragma unroll
+              for (int j = 0; j < 8; ++j) __stcg(dst + j, make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]));
+              continue;
+            }
+            float own[32];
+#pragma unroll
+            for (int j = 0; j < 32; ++j) own[j] = v[j];
+            for (int s2 = 0; s2 < p.splits; ++s2) {            // fixed summation order: split 0, 1, ...
+              if (s2 == sp) {
+                if (s2 == 0) continue;                         // v already holds the own (first) term
+#pragma unroll
+                for (int j = 0; j < 32; ++j) v[j] += own[j];
+              } else {
+                const float4 *src = reinterpret_cast<const float4 *>(part_row + s2 * part_split_stride + c * 32);
+                float4 q4[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) q4[j] = __ldcg(src + j);
+                if (s2 == 0) {
+#pragma unroll
+                  for (int j = 0; j < 8; ++j) { v[4 * j] = q4[j].x; v[4 * j + 1] = q4[j].y; v[4 * j + 2] = q4[j].z; v[4 * j + 3] = q4[j].w; }
+                } else {
+#pragma unroll
+                  for (int j = 0; j < 8; ++j) { v[4 * j] += q4[j].x; v[4 * j + 1] += q4[j].y; v[4 * j + 2] += q4[j].z; v[4 * j + 3] += q4[j].w; }
+                }
+              }
+            }
+          }
           if (p.flags & EPI_BIAS) {
 #pragma unroll
             for (int j = 0; j < 32; j += 4) {
@@ -277,7 +351,12 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
           }
           if (p.flags & EPI_MASK) {
 #pragma unroll
-            for (int j = 0; j < 32; ++j) v[j] = ((mb[c] >> j) & 1u) ? v[j] : 0.f;
+            const uint32_t w01 = (c & 1) ? mb[1] : mb[0], w23 = (c & 1) ? mb[3] : mb[2];
+            const uint32_t w45 = (c & 1) ? mb[5] : mb[4], w67 = (c & 1) ? mb[7] : mb[6];
+            const uint32_t w03 = (c & 2) ? w23 : w01, w47 = (c & 2) ? w67 : w45;
+            const uint32_t mw = (c & 4) ? w47 : w03;
+#pragma unroll
+            for (int j = 0; j < 32; ++j) v[j] = ((mw >> j) & 1u) ? v[j] : 0.f;
           }
           if (p.flags & EPI_RESID) {
 #pragma unroll
@@ -337,7 +416,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
             uint32_t w = 0;
 #pragma unroll
             for (int j = 0; j < 32; ++j) w |= (v[j] > 0.f ? 1u : 0u) << j;
-            wbits[c] = w;
+            if (row_ok) p.maskbits[(int64_t)row * p.ldmask + (col0 >> 5)] = w;
           }
           if (p.flags & EPI_COLSUM) {
             const bool ragged = col0 + 32 > p.N;
@@ -353,17 +432,11 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
       __syncwarp();
       if (lane == 0) mbar_arrive_cluster_relaxed(as ? tempty_leader1 : tempty_leader0);
       if (++as == 2) { as = 0; aphase ^= 1; }
-      if ((p.flags & EPI_BITS_OUT) && row_ok) {
-        uint32_t *bp = p.maskbits + (int64_t)row * p.ldmask + (n0 >> 5);
-        if (NCH == 8 && n0 + BN <= p.N && (p.ldmask & 3) == 0) {
-          *reinterpret_cast<uint4 *>(bp) = make_uint4(wbits[0], wbits[1], wbits[2], wbits[3]);
-          *reinterpret_cast<uint4 *>(bp + 4) =
-              make_uint4(wbits[4 % NCH], wbits[5 % NCH], wbits[6 % NCH], wbits[7 % NCH]);
-        } else {
-#pragma unroll
-          for (int c = 0; c < NCH; ++c)
-            if (n0 + c * 32 < p.N) bp[c] = wbits[c];
-        }
+      if (write_partial) {                                   // publish: all 4 warps' partial rows, then one ready tick
+        __threadfence();
+        asm volatile("bar.sync 2, 128;" ::: "memory");
+        if (et == 0) atomicAdd(p.ws_cnt + ((size_t)t * 2 + rank) * 2 + 1, 1u);
+        continue;
       }
       if (p.flags & EPI_COLSUM) {
         asm volatile("bar.sync 2, 128;" ::: "memory");
@@ -452,6 +525,18 @@ static bool get_map(const void *ptr, uint32_t esize, uint64_t inner, uint64_t ou
   return true;
 }
 
+// Split-K when the output has too few 256 x 256 tiles to occupy the CTA pairs and K is long enough
+// that each split still runs a real main loop (>= 8 K-blocks).  All units run in ONE wave.
+static int splitk_factor(int tiles, int num_kb, int pairs) {
+  static const int off = getenv("GPIPE_NO_SPLITK") ? atoi(getenv("GPIPE_NO_SPLITK")) : 0;
+  if (off || tiles * 2 > pairs) return 1;
+  int s = pairs / tiles;
+  if (s > 4) s = 4;
+  while (s > 1 && num_kb / s < 8) --s;
+  return s;
+}
+static size_t splitk_cnt_bytes(int tiles) { return (((size_t)tiles * 2 * 2 * sizeof(unsigned int)) + 1023) & ~(size_t)1023; }
+
 template <int BN>
 static cudaError_t launch_pair(const Ctx &c, const GemmArgs &a) {
   using Cfg = PairCfg<BN>;
@@ -464,6 +549,14 @@ static cudaError_t launch_pair(const Ctx &c, const GemmArgs &a) {
   p.colpart = a.colsum_scratch;
   p.tiles_m = (a.M + 255) / 256;
   p.tiles_n = (a.N + BN - 1) / BN;
+  const int pairs = c.sm_count / 2;
+  const int num_kb = (a.K + BK - 1) / BK;
+  p.splits = splitk_factor(p.tiles_m * p.tiles_n, num_kb, pairs);
+  if (p.splits > 1 && (!a.ws || a.ws_bytes < gemm_splitk_ws_bytes(a.M, a.N, a.K, c.sm_count))) p.splits = 1;
+  p.kb_per_split = (num_kb + p.splits - 1) / p.splits;
+  p.splits = (num_kb + p.kb_per_split - 1) / p.kb_per_split;             // no empty split
+  p.ws_cnt = (unsigned int *)a.ws;
+  p.ws_part = (float *)((char *)a.ws + splitk_cnt_bytes(p.tiles_m * p.tiles_n));
   const bool out_f32 = (a.flags & (EPI_OUT_F32 | EPI_ACCUM)) != 0;
   CUtensorMap ma, mb, mc;
   bool ok;
@@ -483,14 +576,23 @@ static cudaError_t launch_pair(const Ctx &c, const GemmArgs &a) {
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  int tiles = p.tiles_m * p.tiles_n;
-  int pairs = c.sm_count / 2;
-  int grid = 2 * (tiles < pairs ? tiles : pairs);
+  int units = p.tiles_m * p.tiles_n * p.splits;
+  int grid = 2 * (units < pairs ? units : pairs);
   gemm_tcgen05_pair_kernel<BN><<<grid, NUM_THREADS, Cfg::SMEM, c.stream>>>(ma, mb, mc, p);
   GP_LAUNCH_CHECK(c);
 }
 
 }  // namespace tc
+
+// Workspace a split-K launch of this shape needs (0 when the shape is not split); the first
+// splitk_cnt_bytes() bytes are the counters and must be ZERO before the first launch (they reset
+// themselves afterwards).
+size_t gemm_splitk_ws_bytes(int M, int N, int K, int sm_count) {
+  const int tiles = ((M + 255) / 256) * ((N + 255) / 256);
+  const int s = tc::splitk_factor(tiles, (K + tc::BK - 1) / tc::BK, sm_count / 2);
+  if (s <= 1) return 0;
+  return tc::splitk_cnt_bytes(tiles) + (size_t)tiles * s * 2 * 128 * 256 * sizeof(float);
+}
 
 bool gemm_tc_supported(int dt, const GemmArgs &a) {
   if (dt != GP_BF16) return false;

@@ -47,8 +47,10 @@ struct GemmArgs {
   int flags;
   float *colsum_out;       // EPI_COLSUM: fp32 [N], accumulated into
   float *colsum_scratch;   // EPI_COLSUM: fp32 [ceil(M/128), N]
+  void *ws; size_t ws_bytes;   // split-K workspace (gemm_splitk_ws_bytes), counters zeroed once; NULL: never split
 };
 cudaError_t gemm(const Ctx &c, int dt, const GemmArgs &a);
+size_t gemm_splitk_ws_bytes(int M, int N, int K, int sm_count);
 // true when the tcgen05 kernel handles this problem (bf16, aligned shapes)
 bool gemm_tc_supported(int dt, const GemmArgs &a);
 

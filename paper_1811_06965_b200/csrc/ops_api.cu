@@ -75,9 +75,10 @@ extern "C" {
 int gpipe_op_gemm(void *stream, int dtype, int M, int N, int K, const void *A, int64_t lda, int transA,
                   const void *B, int64_t ldb, int transB, void *C, int64_t ldc, const float *bias,
                   const float *resid, void *mask, int64_t ldmask, float *colsum_out,
-                  float *colsum_scratch, int flags, int backend) {
+                  float *colsum_scratch, void *workspace, int64_t workspace_bytes, int flags, int backend) {
   GemmArgs g{};
   g.colsum_out = colsum_out; g.colsum_scratch = colsum_scratch;
+  g.ws = workspace; g.ws_bytes = workspace_bytes > 0 ? (size_t)workspace_bytes : 0;
   g.M = M; g.N = N; g.K = K;
   g.A = A; g.lda = lda; g.transA = transA;
   g.B = B; g.ldb = ldb; g.transB = transB;
@@ -88,6 +89,9 @@ int gpipe_op_gemm(void *stream, int dtype, int M, int N, int K, const void *A, i
 int gpipe_op_ln_fwd(void *stream, int dtype, const float *x, const float *gamma, const float *beta,
                     void *y, float *mean, float *rstd, int64_t n_tok, int d, float eps) {
   return ret(ln_fwd(mk(stream), dtype, x, gamma, beta, y, mean, rstd, n_tok, d, eps), "gpipe_op_ln_fwd");
+}
+int64_t gpipe_op_gemm_workspace_bytes(int M, int N, int K) {
+  return (int64_t)gemm_splitk_ws_bytes(M, N, K, sm_count_cached());
 }
 int64_t gpipe_op_ln_bwd_scratch_floats(int d) {
   return (int64_t)ln_bwd_partial_rows(sm_count_cached()) * 3 * d;

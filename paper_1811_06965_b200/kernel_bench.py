@@ -125,14 +125,16 @@ def main():
             if ep.get("bias"): kw["bias"] = torch.randn(N, device=dev)
             if ep.get("relu"): kw["relu"] = True
             if ep.get("resid"): kw["resid"] = torch.randn((M, N), device=dev)
-            if ep.get("mask"): kw["mask"] = torch.randn((M, N), device=dev).to(bf)
+            if ep.get("mask"): kw["mask"] = torch.randint(-2 ** 31, 2 ** 31 - 1, (M, N // 32), device=dev, dtype=torch.int32)
             if ep.get("accum"): kw["accumulate"] = True
             if ep.get("colsum"): kw["colsum_out"] = torch.zeros(N, device=dev)
+            kw["workspace"] = ops.gemm_workspace(M, N, K, dev)
+            if kw["workspace"] is None: kw["workspace"] = False
             sets.append((A, Bm, Cm, kw))
         fns = [(lambda s=s: ops.gemm(s[0], s[1], s[2], transA=bool(tA), transB=bool(tB), **s[3])) for s in sets]
         ms = time_it(fns, args.reps)
         byts = per + (M * N * 4 if ep.get("resid") else 0) + (M * N * 4 if ep.get("accum") else 0) + \
-            (M * N * 2 if ep.get("mask") else 0)
+            (M * N // 8 if ep.get("mask") else 0)
         extra = {"M": M, "N": N, "K": K, "transA": tA, "transB": tB}
         if args.compare:
             cf = [(lambda s=s: torch.matmul(s[0].t() if tA else s[0], s[1].t() if tB else s[1])) for s in sets]

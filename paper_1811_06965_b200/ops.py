@@ -30,9 +30,11 @@ def _stream():
 
 
 def gemm(A, B_, C, *, transA=False, transB=False, bias=None, resid=None, mask=None, relu=False,
-         accumulate=False, colsum_out=None, bits_out=None, backend=0):
+         accumulate=False, colsum_out=None, bits_out=None, workspace=None, backend=0):
     """C = epilogue(op(A) @ op(B)); shapes follow gpipe_op_gemm.  C is written in place.
-    mask / bits_out: int32 [M, N/32] bit-packed ReLU pattern (read / written)."""
+    mask / bits_out: int32 [M, N/32] bit-packed ReLU pattern (read / written).
+    workspace: None -> a zeroed split-K workspace is allocated when the shape wants one; False -> never
+    split; or a uint8 tensor from gemm_workspace() that this stream reuses."""
     torch = _torch()
     M, N = C.shape
     K = A.shape[0] if transA else A.shape[1]
@@ -51,11 +53,22 @@ def gemm(A, B_, C, *, transA=False, transB=False, bias=None, resid=None, mask=No
     if colsum_out is not None:
         flags |= B.EPI_COLSUM
         scratch = torch.empty(B.lib().gpipe_op_colsum_scratch_floats(M, N), dtype=torch.float32, device=C.device)
+    if workspace is None:
+        workspace = gemm_workspace(M, N, K, C.device)
+    elif workspace is False:
+        workspace = None
     B._check(B.lib().gpipe_op_gemm(_stream(), _dt(A), M, N, K, _p(A), A.stride(0), int(transA), _p(B_),
                                    B_.stride(0), int(transB), _p(C), C.stride(0), _p(bias), _p(resid),
                                    _p(mask), mask.stride(0) if mask is not None else 0, _p(colsum_out),
-                                   _p(scratch), flags, backend))
+                                   _p(scratch), _p(workspace), workspace.numel() if workspace is not None else 0,
+                                   flags, backend))
     return C
+
+
+def gemm_workspace(M, N, K, device):
+    """Zeroed split-K workspace for a [M,N,K] GEMM (None when the shape is not split)."""
+    n = B.lib().gpipe_op_gemm_workspace_bytes(M, N, K)
+    return _torch().zeros(n, dtype=_torch().uint8, device=device) if n > 0 else None
 
 
 def ln_fwd(x, gamma, beta, y, mean, rstd, eps=1e-5):

@@ -51,6 +51,15 @@ int gpipe_op_gemm(void *stream, int dtype, int M, int N, int K, const void *A, i
                   const float *resid, void *mask, int64_t ldmask, float *colsum_out,
                   float *colsum_scratch, void *workspace, int64_t workspace_bytes, int flags, int backend);
 
+/* Profiling hook (not on the product path): while dev_buf != NULL every tcgen05 GEMM launch writes 8
+ * %globaltimer stamps (ns) per CTA to dev_buf[blockIdx * 32 + i] - kernel entry, prologue done, first
+ * operands landed, all MMAs issued, first accumulator complete, last output chunk handed to the TMA,
+ * stores complete, exit - followed by 24 SM-clock stamps of the first tile's epilogue chunks (4 per chunk:
+ * accumulator in registers, staged in shared memory, fenced, handed to the TMA).  dev_buf: device memory,
+ * 32 * SM-count uint64, owned by the caller; pass NULL
+ * to switch the probe off.  Process-global, not thread-safe.  Always returns GPIPE_OK. */
+int gpipe_op_gemm_timeline(void *dev_buf);
+
 /* y = LayerNorm(x) * gamma + beta over the last axis (biased variance); y lp [n_tok,d]; x fp32. */
 int gpipe_op_ln_fwd(void *stream, int dtype, const float *x, const float *gamma, const float *beta,
                     void *y, float *mean, float *rstd, int64_t n_tok, int d, float eps);

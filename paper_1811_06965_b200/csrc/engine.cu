@@ -100,8 +100,10 @@ int Engine::build_plan(bool dry, std::string &err) {
   }
 
   // split-K workspace: the largest any GEMM shape of a cell needs (forward, dgrad, wgrad)
+  // Split-K buys single-kernel latency at the price of SM-time; with >= 4 cells in flight the other
+  // streams fill the SMs a few-tile GEMM leaves idle, so only shallow pipelines split.
   splitk_ws_bytes = 0;
-  if (dt == GP_BF16) {
+  if (dt == GP_BF16 && K < 4) {
     const int T = (int)T_mb;
     const int shapes[][3] = {{T, 3 * da, d}, {T, d, da}, {T, H, d}, {T, d, H}, {T, V, d},          // forward
                              {T, da, d}, {T, d, 3 * da}, {T, d, V},                                 // dgrad (others as forward)

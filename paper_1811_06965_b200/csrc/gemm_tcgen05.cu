@@ -40,8 +40,9 @@ namespace gp {
 namespace tc {
 
 constexpr int BK = 64;
-constexpr int NUM_THREADS = 256;
+constexpr int NUM_THREADS = 384;
 constexpr int EPI_WARP0 = 4;
+constexpr int NUM_EPI_THREADS = 256;             // 8 epilogue warps
 
 struct Params {
   int M, N, K;
@@ -62,16 +63,32 @@ struct Params {
   int splits, kb_per_split;
   float *ws_part;               // [tile][split][rank][128][BN] fp32
   unsigned int *ws_cnt;         // [tile][rank][2]: arrivals, partials ready
+  unsigned long long *tl;       // optional timeline probe: 8 globaltimer stamps per CTA (gemm_tc_set_timeline)
 };
 
-template <int BN> struct PairCfg {
+__device__ __forceinline__ void tl_stamp(const Params &p, int slot) {
+  if (p.tl) {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    p.tl[(size_t)blockIdx.x * 32 + slot] = t;
+  }
+}
+// fine-grained: SM clock stamps of the first tile's first four chunks (epilogue warp 0, lane 0)
+__device__ __forceinline__ void tl_clock(const Params &p, bool on, int c, int which) {
+  if (p.tl && on && c < 6) p.tl[(size_t)blockIdx.x * 32 + 8 + c * 4 + which] = (unsigned long long)clock64();
+}
+
+// STG: staging buffers ([32 rows x 128 B]) per epilogue warp.  Dynamic shared memory: operand ring,
+// staging, bias (2 x BN floats), column-sum exchange (4 x BN floats), 1 KB alignment slack.
+template <int BN, int STG> struct PairCfg {
   static constexpr int BNH = BN / 2;
   static constexpr uint32_t A_BYTES = 128 * BK * 2, B_BYTES = BNH * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;
-  static constexpr uint32_t STAGING_BYTES = 4 * 2 * 4096;      // 4 epilogue warps x 2 buffers x [32 rows x 128 B]
-  static constexpr int STAGES_MAX = (int)((220 * 1024 - STAGING_BYTES) / STAGE_BYTES);
+  static constexpr uint32_t STAGING_BYTES = 8 * STG * 4096;
+  static constexpr uint32_t AUX_BYTES = 6 * BN * 4;
+  static constexpr int STAGES_MAX = (int)((225 * 1024 - STAGING_BYTES - AUX_BYTES) / STAGE_BYTES);
   static constexpr int STAGES = STAGES_MAX > 8 ? 8 : STAGES_MAX;
   static constexpr uint32_t TMEM_COLS = 2 * BN > 256 ? 512 : 256;
-  static constexpr size_t SMEM = (size_t)STAGES * STAGE_BYTES + STAGING_BYTES + 1024;
+  static constexpr size_t SMEM = (size_t)STAGES * STAGE_BYTES + STAGING_BYTES + AUX_BYTES + 1024;
 };
 
 // Column sums over a warp's 32 rows: transpose-reduce across lanes (31 shuffles); afterwards
@@ -92,23 +109,25 @@ __device__ __forceinline__ void warp_colsum32(float (&v)[32], const int lane) {
 // ------------------------------------------------------------------------------------------
 // the kernel
 // ------------------------------------------------------------------------------------------
-template <int BN>
+// F >= 0: the epilogue flags are this compile-time constant and the launch is never split along K
+// (compact straight-line epilogue: the generic one is instruction-fetch bound); F < 0: p.flags at run time.
+template <int BN, int STG, int F>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NUM_THREADS, 1)
 gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_b,
                          const __grid_constant__ CUtensorMap map_c, const Params p) {
-  using Cfg = PairCfg<BN>;
-  constexpr int NST = Cfg::STAGES, BNH = Cfg::BNH, NCH = BN / 32;
+  using Cfg = PairCfg<BN, STG>;
+  constexpr int NST = Cfg::STAGES, BNH = Cfg::BNH;
   constexpr uint32_t A_BYTES = Cfg::A_BYTES, STAGE_BYTES = Cfg::STAGE_BYTES;
-  static_assert(BN % 32 == 0 && BN <= 256 && BNH % 8 == 0, "tile N");
+  static_assert(BN == 256, "the epilogue splits the tile into two 128-column halves of four 32-column chunks");
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t bars[2 * NST + 4];
   __shared__ uint32_t tmem_base_smem;
-  __shared__ __align__(16) float bias_s[2][BN];
-  __shared__ float colbuf[4][BN];
   __shared__ int split_last_s;
 
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t staging_base = smem_base + NST * STAGE_BYTES;
+  float *bias_s = reinterpret_cast<float *>(smem_raw + (staging_base - smem_u32(smem_raw)) + Cfg::STAGING_BYTES);  // [2][BN]
+  float *colbuf = bias_s + 2 * BN;                                                                                // [4][BN]
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
   const int pair = blockIdx.x >> 1, num_pairs = gridDim.x >> 1;
@@ -118,6 +137,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
   auto tfull_bar = [&](int s) { return bar0 + 8u * (2 * NST + s); };
   auto tempty_bar = [&](int s) { return bar0 + 8u * (2 * NST + 2 + s); };
 
+  if (threadIdx.x == 0) tl_stamp(p, 0);                // kernel entry
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&map_a);
     tma_prefetch_desc(&map_b);
@@ -130,7 +150,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
     }
     for (int s = 0; s < 2; ++s) {
       mbar_init(tfull_bar(s), 1);
-      mbar_init(tempty_bar(s), 8);                 // leader's: 4 epilogue warps of each CTA
+      mbar_init(tempty_bar(s), 16);                // leader's: 8 epilogue warps of each CTA
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -143,8 +163,11 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
   cluster_sync_all();
   tcgen05_fence_after();
   const uint32_t tmem_base = tmem_base_smem;
+  if (threadIdx.x == 0) tl_stamp(p, 1);                // prologue done
 
-  const int num_units = p.tiles_m * p.tiles_n * p.splits;     // work units: (tile, split), splits adjacent
+  const int flags = F >= 0 ? F : p.flags;
+  const int splits = F >= 0 ? 1 : p.splits;
+  const int num_units = p.tiles_m * p.tiles_n * splits;       // work units: (tile, split), splits adjacent
   const int num_kb = (p.K + BK - 1) / BK;
 
   if (warp == 0) {
@@ -153,7 +176,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
       int stage = 0;
       uint32_t phase = 0;
       for (int u = pair; u < num_units; u += num_pairs) {
-        const int t = u / p.splits, sp = u - t * p.splits;
+        const int t = u / splits, sp = u - t * splits;
         const int m0 = (t % p.tiles_m) * 256 + (int)rank * 128, n0 = (t / p.tiles_m) * BN + (int)rank * BNH;
         const int kb0 = sp * p.kb_per_split, kb1 = min(num_kb, kb0 + p.kb_per_split);
         for (int kb = kb0; kb < kb1; ++kb) {
@@ -196,7 +219,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
       int as = 0;
       uint32_t aphase = 0;
       for (int u = pair; u < num_units; u += num_pairs) {
-        const int sp = u % p.splits;
+        const int sp = u % splits;
         const int kb0 = sp * p.kb_per_split, kb1 = min(num_kb, kb0 + p.kb_per_split);
         mbar_wait(tempty_bar(as), aphase ^ 1);       // both CTAs' epilogues have drained this accumulator
         tcgen05_fence_after();
@@ -204,6 +227,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
         for (int kb = kb0; kb < kb1; ++kb) {
           mbar_wait(full_bar(stage), phase);
           tcgen05_fence_after();
+          if (u == pair && kb == kb0) tl_stamp(p, 2);  // first operands landed
           const uint32_t sa = smem_base + stage * STAGE_BYTES, sb = sa + A_BYTES;
 #pragma unroll
           for (int k = 0; k < BK / 16; ++k) {
@@ -217,52 +241,60 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
         tcgen05_commit_pair(tfull_bar(as), 3);       // accumulator complete -> both epilogues
         if (++as == 2) { as = 0; aphase ^= 1; }
       }
+      tl_stamp(p, 3);                                  // every MMA issued
     }
   } else if (warp >= EPI_WARP0) {
     // ===================== epilogue (both CTAs): own 128 rows of the tile =====================
-    const int quad = warp & 3;                       // TMEM lane quadrant of this warp
-    const int et = threadIdx.x - EPI_WARP0 * 32;     // 0..127 within the epilogue warps
-    const bool out_f32 = (p.flags & (EPI_OUT_F32 | EPI_ACCUM)) != 0;
-    const uint32_t stg0 = staging_base + (uint32_t)quad * 8192u;
+    // 8 warps: warp ew reads TMEM lane quadrant ew & 3 (rows) and column half ew >> 2 (4 chunks of 32
+    // columns).  The tcgen05.ld of chunk c+1 is in flight while chunk c is converted and staged.
+    const int ew = warp - EPI_WARP0;
+    const int quad = ew & 3, chalf = ew >> 2;
+    const int et = threadIdx.x - EPI_WARP0 * 32;     // 0..255 within the epilogue warps
+    const bool out_f32 = (flags & (EPI_OUT_F32 | EPI_ACCUM)) != 0;
+    const uint32_t stg0 = staging_base + (uint32_t)ew * (uint32_t)(STG * 4096);
     const uint32_t tempty_leader0 = mapa_shared(tempty_bar(0), 0), tempty_leader1 = mapa_shared(tempty_bar(1), 0);
     const uint32_t swz = (uint32_t)(lane & 7);
     int as = 0, it = 0, sbuf = 0;
     uint32_t aphase = 0;
     for (int u = pair; u < num_units; u += num_pairs, ++it) {
-      const int t = u / p.splits, sp = u - t * p.splits;
+      const int t = u / splits, sp = u - t * splits;
       const int m0 = (t % p.tiles_m) * 256 + (int)rank * 128, n0 = (t / p.tiles_m) * BN;
       const int row0 = m0 + quad * 32, row = row0 + lane;
       const bool row_ok = row < p.M;
-      float *bs = bias_s[it & 1];
-      if (p.flags & EPI_BIAS) {
-        for (int i = et; i < BN; i += 128) bs[i] = (n0 + i < p.N) ? __ldg(p.bias + n0 + i) : 0.f;
+      float *bs = bias_s + (it & 1) * BN;
+      if (flags & EPI_BIAS) {
+        for (int i = et; i < BN; i += NUM_EPI_THREADS) bs[i] = (n0 + i < p.N) ? __ldg(p.bias + n0 + i) : 0.f;
       }
-      // this row's ReLU-pattern words for the whole tile (one 32-byte sector), fetched before the wait
-      uint32_t mb[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
-      if ((p.flags & EPI_MASK) && row_ok) {
-        const uint32_t *mp = p.maskbits + (int64_t)row * p.ldmask + (n0 >> 5);
-        if (NCH == 8 && n0 + BN <= p.N && (p.ldmask & 3) == 0) {
-          const uint4 lo = __ldg(reinterpret_cast<const uint4 *>(mp)), hi = __ldg(reinterpret_cast<const uint4 *>(mp + 4));
-          mb[0] = lo.x; mb[1] = lo.y; mb[2] = lo.z; mb[3] = lo.w;
-          mb[4] = hi.x; mb[5] = hi.y; mb[6] = hi.z; mb[7] = hi.w;
+      // this row's ReLU-pattern words for this warp's four chunks (16 bytes), fetched before the wait
+      uint32_t mb0 = 0u, mb1 = 0u, mb2 = 0u, mb3 = 0u;
+      if ((flags & EPI_MASK) && row_ok) {
+        const uint32_t *mp = p.maskbits + (int64_t)row * p.ldmask + (n0 >> 5) + chalf * 4;
+        if (n0 + BN <= p.N && (p.ldmask & 3) == 0) {
+          const uint4 q = __ldg(reinterpret_cast<const uint4 *>(mp));
+          mb0 = q.x; mb1 = q.y; mb2 = q.z; mb3 = q.w;
         } else {
-#pragma unroll
-          for (int c = 0; c < NCH; ++c)
-            if (n0 + c * 32 < p.N) mb[c] = __ldg(mp + c);
+          const int cb = n0 + chalf * 128;
+          if (cb < p.N) mb0 = __ldg(mp);
+          if (cb + 32 < p.N) mb1 = __ldg(mp + 1);
+          if (cb + 64 < p.N) mb2 = __ldg(mp + 2);
+          if (cb + 96 < p.N) mb3 = __ldg(mp + 3);
         }
       }
-      asm volatile("bar.sync 1, 128;" ::: "memory");       // bias_s visible; colbuf of the previous tile consumed
+      asm volatile("bar.sync 1, 256;" ::: "memory");       // bias_s visible; colbuf of the previous tile consumed
       mbar_wait(tfull_bar(as), aphase);
       tcgen05_fence_after();
-      const uint32_t t_row = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(as * BN);
+      if (it == 0 && et == 0) tl_stamp(p, 4);          // first accumulator complete
+      const uint32_t t_row = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(as * BN + chalf * 128);
+      uint32_t rn[32];
+      tmem_ld32(t_row, rn);                              // first chunk in flight during the split-K handshake
       // ---- split-K: am I the last of this (tile, rank)'s splits to finish? ----
       bool write_partial = false;
-      if (p.splits > 1) {
+      if (splits > 1) {
         unsigned int *cnt = p.ws_cnt + ((size_t)t * 2 + rank) * 2;
         if (et == 0) {
           const unsigned int arrived = atomicAdd(cnt, 1u);
-          if (arrived == (unsigned int)p.splits - 1) {          // last: wait for the partials already being written
-            while (atomicAdd(cnt + 1, 0u) < (unsigned int)p.splits - 1) __nanosleep(64);
+          if (arrived == (unsigned int)splits - 1) {          // last: wait for the partials already being written
+            while (atomicAdd(cnt + 1, 0u) < (unsigned int)splits - 1) __nanosleep(64);
             cnt[0] = 0u;                                        // self-reset for the next launch on this stream
             cnt[1] = 0u;
             __threadfence();
@@ -271,160 +303,169 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
             split_last_s = 0;
           }
         }
-        asm volatile("bar.sync 2, 128;" ::: "memory");
+        asm volatile("bar.sync 2, 256;" ::: "memory");
         write_partial = split_last_s == 0;
       }
-      float *part_row = p.ws_part + (((size_t)t * p.splits) * 2 + rank) * (size_t)(128 * BN) +
+      float *part_row = p.ws_part + (((size_t)t * splits) * 2 + rank) * (size_t)(128 * BN) +
                         (size_t)(quad * 32 + lane) * BN;          // split 0 of this (tile, rank), this lane's row
       const size_t part_split_stride = (size_t)2 * 128 * BN;
+      uint32_t wb0 = 0u, wb1 = 0u, wb2 = 0u, wb3 = 0u;     // EPI_BITS_OUT words of this row
       // one 32-column chunk per iteration; NOT unrolled: the epilogue has to stay resident in the
       // instruction cache next to the other warp roles
-#pragma unroll 1
-      for (int c = 0; c < NCH; ++c) {
+#pragma unroll (F >= 0 ? 4 : 1)
+      for (int cl = 0; cl < 4; ++cl) {
+        const int c = chalf * 4 + cl;
         const int col0 = n0 + c * 32;
-        if (col0 < p.N) {                                    // uniform over the CTA
-          uint32_t r[32];
-          tmem_ld32(t_row + c * 32, r);
-          float4 rr[8];
-          if ((p.flags & EPI_RESID) && row_ok) {
-            const float *rp = p.resid + (int64_t)row * p.ldr + col0;
-            if (col0 + 32 <= p.N) {
+        const bool col_ok = col0 < p.N;                      // uniform over the warp
+        float4 rr[8];
+        if ((flags & EPI_RESID) && row_ok && col_ok) {
+          const float *rp = p.resid + (int64_t)row * p.ldr + col0;
+          if (col0 + 32 <= p.N) {
 #pragma unroll
-              for (int j = 0; j < 8; ++j) rr[j] = *reinterpret_cast<const float4 *>(rp + 4 * j);
-            } else {
-#pragma unroll
-              for (int j = 0; j < 8; ++j) {
-                rr[j].x = col0 + 4 * j + 0 < p.N ? rp[4 * j + 0] : 0.f;
-                rr[j].y = col0 + 4 * j + 1 < p.N ? rp[4 * j + 1] : 0.f;
-                rr[j].z = col0 + 4 * j + 2 < p.N ? rp[4 * j + 2] : 0.f;
-                rr[j].w = col0 + 4 * j + 3 < p.N ? rp[4 * j + 3] : 0.f;
-              }
-            }
+            for (int j = 0; j < 8; ++j) rr[j] = *reinterpret_cast<const float4 *>(rp + 4 * j);
           } else {
-#pragma unroll
-            for (int j = 0; j < 8; ++j) rr[j] = make_float4(0.f, 0.f, 0.f, 0.f);
-          }
-          tmem_ld_wait();
-          float v[32];
-#pragma unroll
-          for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]);
-          if (p.splits > 1) {
-            if (write_partial) {                               // raw accumulators -> workspace; no epilogue
-              float4 *dst = reinterpret_cast<float4 *>(part_row + sp * part_split_stride + c * 32);
-#pragma unroll
-              for (int j = 0; j < 8; ++j) __stcg(dst + j, make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]));
-              continue;
-            }
-            float own[32];
-#pragma unroll
-            for (int j = 0; j < 32; ++j) own[j] = v[j];
-            for (int s2 = 0; s2 < p.splits; ++s2) {            // fixed summation order: split 0, 1, ...
-              if (s2 == sp) {
-                if (s2 == 0) continue;                         // v already holds the own (first) term
-#pragma unroll
-                for (int j = 0; j < 32; ++j) v[j] += own[j];
-              } else {
-                const float4 *src = reinterpret_cast<const float4 *>(part_row + s2 * part_split_stride + c * 32);
-                float4 q4[8];
-#pragma unroll
-                for (int j = 0; j < 8; ++j) q4[j] = __ldcg(src + j);
-                if (s2 == 0) {
-#pragma unroll
-                  for (int j = 0; j < 8; ++j) { v[4 * j] = q4[j].x; v[4 * j + 1] = q4[j].y; v[4 * j + 2] = q4[j].z; v[4 * j + 3] = q4[j].w; }
-                } else {
-#pragma unroll
-                  for (int j = 0; j < 8; ++j) { v[4 * j] += q4[j].x; v[4 * j + 1] += q4[j].y; v[4 * j + 2] += q4[j].z; v[4 * j + 3] += q4[j].w; }
-                }
-              }
-            }
-          }
-          if (p.flags & EPI_BIAS) {
-#pragma unroll
-            for (int j = 0; j < 32; j += 4) {
-              float4 b = *reinterpret_cast<const float4 *>(bs + c * 32 + j);
-              v[j] += b.x; v[j + 1] += b.y; v[j + 2] += b.z; v[j + 3] += b.w;
-            }
-          }
-          if (p.flags & EPI_RELU) {
-#pragma unroll
-            for (int j = 0; j < 32; ++j) v[j] = fmaxf(v[j], 0.f);
-          }
-          if (p.flags & EPI_MASK) {
-#pragma unroll
-            const uint32_t w01 = (c & 1) ? mb[1] : mb[0], w23 = (c & 1) ? mb[3] : mb[2];
-            const uint32_t w45 = (c & 1) ? mb[5] : mb[4], w67 = (c & 1) ? mb[7] : mb[6];
-            const uint32_t w03 = (c & 2) ? w23 : w01, w47 = (c & 2) ? w67 : w45;
-            const uint32_t mw = (c & 4) ? w47 : w03;
-#pragma unroll
-            for (int j = 0; j < 32; ++j) v[j] = ((mw >> j) & 1u) ? v[j] : 0.f;
-          }
-          if (p.flags & EPI_RESID) {
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-              v[4 * j] += rr[j].x; v[4 * j + 1] += rr[j].y; v[4 * j + 2] += rr[j].z; v[4 * j + 3] += rr[j].w;
+              rr[j].x = col0 + 4 * j + 0 < p.N ? rp[4 * j + 0] : 0.f;
+              rr[j].y = col0 + 4 * j + 1 < p.N ? rp[4 * j + 1] : 0.f;
+              rr[j].z = col0 + 4 * j + 2 < p.N ? rp[4 * j + 2] : 0.f;
+              rr[j].w = col0 + 4 * j + 3 < p.N ? rp[4 * j + 3] : 0.f;
             }
           }
-          // ---- registers -> swizzled staging -> TMA ----
-          if (out_f32) {
-            const uint32_t buf = stg0 + (uint32_t)sbuf * 4096u;
-            if (lane == 0) bulk_wait_read<1>();              // the store that last used this buffer has read it
-            __syncwarp();
+        } else {
 #pragma unroll
-            for (int q = 0; q < 8; ++q)
-              st_shared_v4(buf + (uint32_t)lane * 128u + (((uint32_t)q ^ swz) << 4), __float_as_uint(v[4 * q]),
-                           __float_as_uint(v[4 * q + 1]), __float_as_uint(v[4 * q + 2]), __float_as_uint(v[4 * q + 3]));
+          for (int j = 0; j < 8; ++j) rr[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        tmem_ld_wait();
+        float v[32];
+#pragma unroll
+        for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(rn[j]);
+        if (cl < 3) tmem_ld32(t_row + (cl + 1) * 32, rn);    // next chunk: overlaps this chunk's arithmetic and staging
+        const bool tlon = it == 0 && et == 0;
+        tl_clock(p, tlon, cl, 0);
+        if (!col_ok) continue;
+        if (splits > 1) {
+          if (write_partial) {                               // raw accumulators -> workspace; no epilogue
+            float4 *dst = reinterpret_cast<float4 *>(part_row + sp * part_split_stride + c * 32);
+#pragma unroll
+            for (int j = 0; j < 8; ++j) __stcg(dst + j, make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]));
+            continue;
+          }
+          // fixed summation order: split 0, 1, ... with the own accumulators at position sp
+          float acc[32];
+          bool first = true;
+          for (int s2 = 0; s2 < splits; ++s2) {
+            if (s2 == sp) {
+              if (first) {
+#pragma unroll
+                for (int j = 0; j < 32; ++j) acc[j] = v[j];
+              } else {
+#pragma unroll
+                for (int j = 0; j < 32; ++j) acc[j] += v[j];
+              }
+            } else {
+              const float4 *src = reinterpret_cast<const float4 *>(part_row + s2 * part_split_stride + c * 32);
+#pragma unroll
+              for (int j = 0; j < 8; ++j) {
+                const float4 q4 = __ldcg(src + j);
+                if (first) { acc[4 * j] = q4.x; acc[4 * j + 1] = q4.y; acc[4 * j + 2] = q4.z; acc[4 * j + 3] = q4.w; }
+                else { acc[4 * j] += q4.x; acc[4 * j + 1] += q4.y; acc[4 * j + 2] += q4.z; acc[4 * j + 3] += q4.w; }
+              }
+            }
+            first = false;
+          }
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[j] = acc[j];
+        }
+        if (flags & EPI_BIAS) {
+#pragma unroll
+          for (int j = 0; j < 32; j += 4) {
+            float4 b = *reinterpret_cast<const float4 *>(bs + c * 32 + j);
+            v[j] += b.x; v[j + 1] += b.y; v[j + 2] += b.z; v[j + 3] += b.w;
+          }
+        }
+        if (flags & EPI_RELU) {
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[j] = fmaxf(v[j], 0.f);
+        }
+        if (flags & EPI_MASK) {
+          const uint32_t w01 = (cl & 1) ? mb1 : mb0, w23 = (cl & 1) ? mb3 : mb2;
+          const uint32_t mw = (cl & 2) ? w23 : w01;
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[j] = ((mw >> j) & 1u) ? v[j] : 0.f;
+        }
+        if (flags & EPI_RESID) {
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            v[4 * j] += rr[j].x; v[4 * j + 1] += rr[j].y; v[4 * j + 2] += rr[j].z; v[4 * j + 3] += rr[j].w;
+          }
+        }
+        // ---- registers -> swizzled staging -> TMA ----
+        if (out_f32) {
+          const uint32_t buf = stg0 + (uint32_t)sbuf * 4096u;
+          if (lane == 0) bulk_wait_read<STG - 1>();          // the store that last used this buffer has read it
+          __syncwarp();
+#pragma unroll
+          for (int q = 0; q < 8; ++q)
+            st_shared_v4(buf + (uint32_t)lane * 128u + (((uint32_t)q ^ swz) << 4), __float_as_uint(v[4 * q]),
+                         __float_as_uint(v[4 * q + 1]), __float_as_uint(v[4 * q + 2]), __float_as_uint(v[4 * q + 3]));
+          tl_clock(p, tlon, cl, 1);
+          fence_proxy_async_smem();
+          __syncwarp();
+          tl_clock(p, tlon, cl, 2);
+          if (lane == 0) {
+            if (flags & EPI_ACCUM) tma_reduce_add_2d(&map_c, buf, col0, row0);
+            else tma_store_2d(&map_c, buf, col0, row0);
+            bulk_commit();
+          }
+          if (STG > 1) sbuf ^= 1;
+          tl_clock(p, tlon, cl, 3);
+        } else {
+          const uint32_t buf = stg0 + (uint32_t)sbuf * 4096u;
+          const int half = cl & 1;
+          if (!half) {
+            if (lane == 0) bulk_wait_read<STG - 1>();
+            __syncwarp();
+          }
+          uint32_t pk[16];
+#pragma unroll
+          for (int j = 0; j < 16; ++j) {
+            __nv_bfloat162 h = __floats2bfloat162_rn(v[2 * j], v[2 * j + 1]);
+            pk[j] = *reinterpret_cast<uint32_t *>(&h);
+            float2 f = __bfloat1622float2(h);               // the stored values (EPI_COLSUM, EPI_BITS_OUT)
+            v[2 * j] = f.x;
+            v[2 * j + 1] = f.y;
+          }
+#pragma unroll
+          for (int q = 0; q < 4; ++q)
+            st_shared_v4(buf + (uint32_t)lane * 128u + (((uint32_t)(half * 4 + q) ^ swz) << 4), pk[4 * q],
+                         pk[4 * q + 1], pk[4 * q + 2], pk[4 * q + 3]);
+          const bool flush = half || col0 + 32 >= p.N;
+          tl_clock(p, tlon, cl, 1);
+          if (flush) {
             fence_proxy_async_smem();
             __syncwarp();
+            tl_clock(p, tlon, cl, 2);
             if (lane == 0) {
-              if (p.flags & EPI_ACCUM) tma_reduce_add_2d(&map_c, buf, col0, row0);
-              else tma_store_2d(&map_c, buf, col0, row0);
+              tma_store_2d(&map_c, buf, col0 - half * 32, row0);      // columns past N are clipped
               bulk_commit();
             }
-            sbuf ^= 1;
-          } else {
-            const uint32_t buf = stg0 + (uint32_t)sbuf * 4096u;
-            const int half = c & 1;
-            if (!half) {
-              if (lane == 0) bulk_wait_read<1>();
-              __syncwarp();
-            }
-            uint32_t pk[16];
-#pragma unroll
-            for (int j = 0; j < 16; ++j) {
-              __nv_bfloat162 h = __floats2bfloat162_rn(v[2 * j], v[2 * j + 1]);
-              pk[j] = *reinterpret_cast<uint32_t *>(&h);
-              float2 f = __bfloat1622float2(h);               // the stored values (EPI_COLSUM, EPI_BITS_OUT)
-              v[2 * j] = f.x;
-              v[2 * j + 1] = f.y;
-            }
-#pragma unroll
-            for (int q = 0; q < 4; ++q)
-              st_shared_v4(buf + (uint32_t)lane * 128u + (((uint32_t)(half * 4 + q) ^ swz) << 4), pk[4 * q],
-                           pk[4 * q + 1], pk[4 * q + 2], pk[4 * q + 3]);
-            const bool flush = half || c == NCH - 1 || col0 + 32 >= p.N;
-            if (flush) {
-              fence_proxy_async_smem();
-              __syncwarp();
-              if (lane == 0) {
-                tma_store_2d(&map_c, buf, col0 - half * 32, row0);      // columns past N are clipped
-                bulk_commit();
-              }
-              sbuf ^= 1;
-            }
+            if (STG > 1) sbuf ^= 1;
           }
-          if (p.flags & EPI_BITS_OUT) {
-            uint32_t w = 0;
+          tl_clock(p, tlon, cl, 3);
+        }
+        if (flags & EPI_BITS_OUT) {
+          uint32_t w = 0;
 #pragma unroll
-            for (int j = 0; j < 32; ++j) w |= (v[j] > 0.f ? 1u : 0u) << j;
-            if (row_ok) p.maskbits[(int64_t)row * p.ldmask + (col0 >> 5)] = w;
-          }
-          if (p.flags & EPI_COLSUM) {
-            const bool ragged = col0 + 32 > p.N;
+          for (int j = 0; j < 32; ++j) w |= (v[j] > 0.f ? 1u : 0u) << j;
+          wb0 = cl == 0 ? w : wb0; wb1 = cl == 1 ? w : wb1; wb2 = cl == 2 ? w : wb2; wb3 = cl == 3 ? w : wb3;
+        }
+        if (flags & EPI_COLSUM) {
+          const bool ragged = col0 + 32 > p.N;
 #pragma unroll
-            for (int j = 0; j < 32; ++j) v[j] = (row_ok && !(ragged && col0 + j >= p.N)) ? v[j] : 0.f;
-            warp_colsum32(v, lane);
-            colbuf[quad][c * 32 + lane] = v[0];
-          }
+          for (int j = 0; j < 32; ++j) v[j] = (row_ok && !(ragged && col0 + j >= p.N)) ? v[j] : 0.f;
+          warp_colsum32(v, lane);
+          colbuf[quad * BN + c * 32 + lane] = v[0];
         }
       }
       // every TMEM read of this accumulator stage has completed (tcgen05.wait::ld): release it
@@ -432,25 +473,40 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
       __syncwarp();
       if (lane == 0) mbar_arrive_cluster_relaxed(as ? tempty_leader1 : tempty_leader0);
       if (++as == 2) { as = 0; aphase ^= 1; }
-      if (write_partial) {                                   // publish: all 4 warps' partial rows, then one ready tick
+      if (write_partial) {                                   // publish: all 8 warps' partial rows, then one ready tick
         __threadfence();
-        asm volatile("bar.sync 2, 128;" ::: "memory");
+        asm volatile("bar.sync 2, 256;" ::: "memory");
         if (et == 0) atomicAdd(p.ws_cnt + ((size_t)t * 2 + rank) * 2 + 1, 1u);
         continue;
       }
-      if (p.flags & EPI_COLSUM) {
-        asm volatile("bar.sync 2, 128;" ::: "memory");
-        for (int cc = et; cc < BN; cc += 128) {
-          float ssum = (colbuf[0][cc] + colbuf[1][cc]) + (colbuf[2][cc] + colbuf[3][cc]);
+      if ((flags & EPI_BITS_OUT) && row_ok) {              // this row's four pattern words: one 16-byte store
+        uint32_t *mp = p.maskbits + (int64_t)row * p.ldmask + (n0 >> 5) + chalf * 4;
+        const int cb = n0 + chalf * 128;
+        if (cb + 128 <= p.N && (p.ldmask & 3) == 0) {
+          *reinterpret_cast<uint4 *>(mp) = make_uint4(wb0, wb1, wb2, wb3);
+        } else {
+          if (cb < p.N) mp[0] = wb0;
+          if (cb + 32 < p.N) mp[1] = wb1;
+          if (cb + 64 < p.N) mp[2] = wb2;
+          if (cb + 96 < p.N) mp[3] = wb3;
+        }
+      }
+      if (flags & EPI_COLSUM) {
+        asm volatile("bar.sync 2, 256;" ::: "memory");
+        for (int cc = et; cc < BN; cc += NUM_EPI_THREADS) {
+          float ssum = (colbuf[cc] + colbuf[BN + cc]) + (colbuf[2 * BN + cc] + colbuf[3 * BN + cc]);
           if (n0 + cc < p.N && m0 < p.M) p.colpart[(int64_t)(m0 >> 7) * p.N + n0 + cc] = ssum;
         }
       }
     }
+    if (et == 0) tl_stamp(p, 5);                       // last chunk handed to the TMA
     if (lane == 0) bulk_wait_all();                    // staging must outlive the TMA reads; C complete at exit
+    if (et == 0) tl_stamp(p, 6);                       // stores complete
   }
 
   tcgen05_fence_before();
   cluster_sync_all();                                  // the peer's smem / TMEM / barriers stay valid until both are done
+  if (threadIdx.x == 0) tl_stamp(p, 7);                // both CTAs done
   if (warp == 2) {
     tcgen05_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(Cfg::TMEM_COLS));
@@ -537,9 +593,11 @@ static int splitk_factor(int tiles, int num_kb, int pairs) {
 }
 static size_t splitk_cnt_bytes(int tiles) { return (((size_t)tiles * 2 * 2 * sizeof(unsigned int)) + 1023) & ~(size_t)1023; }
 
-template <int BN>
+static unsigned long long *g_timeline = nullptr;
+
+template <int BN, int STG, int F>
 static cudaError_t launch_pair(const Ctx &c, const GemmArgs &a) {
-  using Cfg = PairCfg<BN>;
+  using Cfg = PairCfg<BN, STG>;
   Params p{};
   p.M = a.M; p.N = a.N; p.K = a.K;
   p.a_mn_major = a.transA ? 1 : 0;
@@ -551,10 +609,11 @@ static cudaError_t launch_pair(const Ctx &c, const GemmArgs &a) {
   p.tiles_n = (a.N + BN - 1) / BN;
   const int pairs = c.sm_count / 2;
   const int num_kb = (a.K + BK - 1) / BK;
-  p.splits = splitk_factor(p.tiles_m * p.tiles_n, num_kb, pairs);
+  p.splits = F >= 0 ? 1 : splitk_factor(p.tiles_m * p.tiles_n, num_kb, pairs);
   if (p.splits > 1 && (!a.ws || a.ws_bytes < gemm_splitk_ws_bytes(a.M, a.N, a.K, c.sm_count))) p.splits = 1;
   p.kb_per_split = (num_kb + p.splits - 1) / p.splits;
   p.splits = (num_kb + p.kb_per_split - 1) / p.kb_per_split;             // no empty split
+  p.tl = g_timeline;
   p.ws_cnt = (unsigned int *)a.ws;
   p.ws_part = (float *)((char *)a.ws + splitk_cnt_bytes(p.tiles_m * p.tiles_n));
   const bool out_f32 = (a.flags & (EPI_OUT_F32 | EPI_ACCUM)) != 0;
@@ -571,18 +630,24 @@ static cudaError_t launch_pair(const Ctx &c, const GemmArgs &a) {
   if (!ok) return cudaErrorInvalidValue;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(gemm_tcgen05_pair_kernel<BN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(gemm_tcgen05_pair_kernel<BN, STG, F>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)Cfg::SMEM);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
   int units = p.tiles_m * p.tiles_n * p.splits;
   int grid = 2 * (units < pairs ? units : pairs);
-  gemm_tcgen05_pair_kernel<BN><<<grid, NUM_THREADS, Cfg::SMEM, c.stream>>>(ma, mb, mc, p);
+  gemm_tcgen05_pair_kernel<BN, STG, F><<<grid, NUM_THREADS, Cfg::SMEM, c.stream>>>(ma, mb, mc, p);
   GP_LAUNCH_CHECK(c);
 }
 
 }  // namespace tc
+
+// Profiling hook: when set, every tcgen05 GEMM launch writes 8 %globaltimer stamps per CTA to buf
+// (entry, prologue done, first operands landed, all MMAs issued, first accumulator complete, last
+// chunk handed to the TMA, stores complete, exit) plus 24 SM-clock stamps of the first tile's epilogue
+// chunks.  buf must hold 32 * SM-count uint64.
+void gemm_tc_set_timeline(unsigned long long *buf) { tc::g_timeline = buf; }
 
 // Workspace a split-K launch of this shape needs (0 when the shape is not split); the first
 // splitk_cnt_bytes() bytes are the counters and must be ZERO before the first launch (they reset
@@ -608,6 +673,24 @@ bool gemm_tc_supported(int dt, const GemmArgs &a) {
   return true;
 }
 
-cudaError_t gemm_tc(const Ctx &c, const GemmArgs &a) { return tc::launch_pair<256>(c, a); }
+// The epilogue combinations the engine launches get their own instantiation; anything else (and every
+// split-K launch) takes the run-time-flag kernel.
+cudaError_t gemm_tc(const Ctx &c, const GemmArgs &a) {
+  static const int generic_only = getenv("GPIPE_GEMM_GENERIC") ? atoi(getenv("GPIPE_GEMM_GENERIC")) : 0;
+  const int tiles = ((a.M + 255) / 256) * ((a.N + 255) / 256);
+  const bool split = a.ws && tc::splitk_factor(tiles, (a.K + tc::BK - 1) / tc::BK, c.sm_count / 2) > 1;
+  if (!split && !generic_only) {
+    switch (a.flags) {
+      case 0: return tc::launch_pair<256, 1, 0>(c, a);
+      case EPI_BIAS: return tc::launch_pair<256, 1, EPI_BIAS>(c, a);
+      case EPI_BIAS | EPI_RESID | EPI_OUT_F32: return tc::launch_pair<256, 1, EPI_BIAS | EPI_RESID | EPI_OUT_F32>(c, a);
+      case EPI_BIAS | EPI_RELU | EPI_BITS_OUT: return tc::launch_pair<256, 1, EPI_BIAS | EPI_RELU | EPI_BITS_OUT>(c, a);
+      case EPI_MASK | EPI_COLSUM: return tc::launch_pair<256, 1, EPI_MASK | EPI_COLSUM>(c, a);
+      case EPI_ACCUM | EPI_OUT_F32: return tc::launch_pair<256, 1, EPI_ACCUM | EPI_OUT_F32>(c, a);
+      default: break;
+    }
+  }
+  return tc::launch_pair<256, 1, -1>(c, a);
+}
 
 }  // namespace gp

@@ -8,6 +8,7 @@
 namespace gp {
 cudaError_t gemm_simt(const Ctx &c, int dt, const GemmArgs &a);
 cudaError_t gemm_tc(const Ctx &c, const GemmArgs &a);
+void gemm_tc_set_timeline(unsigned long long *buf);
 cudaError_t attn_fwd_simt(const Ctx &c, int dt, const void *qkv, void *o, float *lse, int n_seq,
                           int S, int A, int dh, int causal);
 cudaError_t attn_bwd_simt(const Ctx &c, int dt, const void *qkv, const void *o, const void *d_o,
@@ -89,6 +90,10 @@ int gpipe_op_gemm(void *stream, int dtype, int M, int N, int K, const void *A, i
 int gpipe_op_ln_fwd(void *stream, int dtype, const float *x, const float *gamma, const float *beta,
                     void *y, float *mean, float *rstd, int64_t n_tok, int d, float eps) {
   return ret(ln_fwd(mk(stream), dtype, x, gamma, beta, y, mean, rstd, n_tok, d, eps), "gpipe_op_ln_fwd");
+}
+int gpipe_op_gemm_timeline(void *dev_buf) {
+  gemm_tc_set_timeline((unsigned long long *)dev_buf);
+  return GPIPE_OK;
 }
 int64_t gpipe_op_gemm_workspace_bytes(int M, int N, int K) {
   return (int64_t)gemm_splitk_ws_bytes(M, N, K, sm_count_cached());

@@ -60,9 +60,13 @@ int gpipe_op_gemm(void *stream, int dtype, int M, int N, int K, const void *A, i
  * to switch the probe off.  Process-global, not thread-safe.  Always returns GPIPE_OK. */
 int gpipe_op_gemm_timeline(void *dev_buf);
 
-/* y = LayerNorm(x) * gamma + beta over the last axis (biased variance); y lp [n_tok,d]; x fp32. */
+/* y = LayerNorm(x) * gamma + beta over the last axis (biased variance); y lp [n_tok,d]; x fp32.
+ * Fused residual: if resid_out != NULL (fp32 [n_tok,d], device, caller-owned)
+ * the kernel also writes resid_out = x + resid_bias (fp32 [d], required then) - the buffer the branch's
+ * output GEMM accumulates into with GPIPE_EPI_ACCUM, giving x' = x + branch(y) + bias. */
 int gpipe_op_ln_fwd(void *stream, int dtype, const float *x, const float *gamma, const float *beta,
-                    void *y, float *mean, float *rstd, int64_t n_tok, int d, float eps);
+                    void *y, float *mean, float *rstd, const float *resid_bias, float *resid_out,
+                    int64_t n_tok, int d, float eps);
 /* dx_out = (dres_in ? dres_in : 0) + LN'(dy); dx_out_lp optional lp copy; dgamma/dbeta += ;
  * colsum_out (optional, fp32 [d]) += sum_t dx_out[t,:] (the lp copy's values when there is one).
  * partials: fp32 scratch of gpipe_op_ln_bwd_scratch_floats(d) floats. */

@@ -206,8 +206,11 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
     gw.ws = bwd[k].splitk_ws; gw.ws_bytes = splitk_ws_bytes;
     return timed(k, cls, fl, by, [&] { return gemm(c, dt, gw); });
   };
-  auto tln = [&](const float *x_, const float *g_, const float *b_, void *y_, float *mu_, float *rs_) -> cudaError_t {
-    return timed(k, KC_LN_FWD, 0, Td * d * (4.0 + lpb), [&] { return ln_fwd(c, dt, x_, g_, b_, y_, mu_, rs_, T_mb, d, eps); });
+  // rb_/ro_: fused residual init ro_ = x_ + rb_ (the branch's output GEMM then accumulates into ro_)
+  auto tln = [&](const float *x_, const float *g_, const float *b_, void *y_, float *mu_, float *rs_,
+                 const float *rb_, float *ro_) -> cudaError_t {
+    return timed(k, KC_LN_FWD, 0, Td * d * (4.0 + lpb + (ro_ ? 4.0 : 0.0)),
+                 [&] { return ln_fwd(c, dt, x_, g_, b_, y_, mu_, rs_, rb_, ro_, T_mb, d, eps); });
   };
   Workspace &w = wsp(k, m);
   const int32_t *tok = tok_dev + (int64_t)m * T_mb;
@@ -225,8 +228,8 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
     const LayerParams &q = lp[l];
     LayerBuf &b = w.layers[i];
     bool last = (i + 1 == nl);
-    // a = LN1(x)                                                             (a5)
-    GP_TRY(tln(x, P(q.ln1_g), P(q.ln1_b), b.a, b.mean1, b.rstd1));
+    // a = LN1(x); x1 <- x + b_o                                              (a5)
+    GP_TRY(tln(x, P(q.ln1_g), P(q.ln1_b), b.a, b.mean1, b.rstd1, P(q.b_o), b.x1));
     // [q|k|v] = a W_qkv + b_qkv                                              (a6)
     GemmArgs g{};
     g.M = (int)T_mb; g.N = 3 * da; g.K = d;
@@ -236,14 +239,21 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
     // o = softmax(q k^T / sqrt(dh) + mask) v                                 (a7)
     GP_TRY(timed(k, KC_ATTN_FWD, 4.0 * Td * S * da * (causal[l] ? (S + 1.0) / (2.0 * S) : 1.0), Td * 4.0 * da * lpb,
                  [&] { return attn_fwd(c, dt, b.qkv, b.o, b.lse, (int)nb, S, A, dh, causal[l]); }));
-    // x1 = x + o W_o + b_o                                                   (a8)
+    // x1 += o W_o      (x1 = x + o W_o + b_o, the residual was staged by LN1)   (a8)
     g = GemmArgs{};
     g.M = (int)T_mb; g.N = d; g.K = da;
     g.A = b.o; g.lda = da; g.B = W(q.w_o); g.ldb = d; g.C = b.x1; g.ldc = d;
-    g.bias = P(q.b_o); g.resid = x; g.flags = EPI_BIAS | EPI_RESID | EPI_OUT_F32;
+    g.flags = EPI_ACCUM | EPI_OUT_F32;
     GP_TRY(tgemm(KC_GEMM_FWD, g));
-    // c = LN2(x1)                                                            (a9)
-    GP_TRY(tln(b.x1, P(q.ln2_g), P(q.ln2_b), b.c, b.mean2, b.rstd2));
+    // where x2 = x1 + h W_2 + b_2 goes                                        (a11, a12)
+    float *x2;
+    if (!last) x2 = b.x2;
+    else if (k == K - 1) x2 = w.x_out;
+    else if (!replay) x2 = slot[k + 1][m];            // boundary stash (a12)
+    else if (replay_full) x2 = w.x_out;               // replay output nobody reads
+    else x2 = nullptr;                                // skipped: B_k does not need F_k's output
+    // c = LN2(x1); x2 <- x1 + b_2                                            (a9)
+    GP_TRY(tln(b.x1, P(q.ln2_g), P(q.ln2_b), b.c, b.mean2, b.rstd2, x2 ? P(q.b_2) : nullptr, x2));
     // h = relu(c W_1 + b_1)                                                  (a10)
     g = GemmArgs{};
     g.M = (int)T_mb; g.N = H; g.K = d;
@@ -251,18 +261,12 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
     g.bias = P(q.b_1); g.flags = EPI_BIAS | EPI_RELU | EPI_BITS_OUT;
     g.mask = b.hbits; g.ldmask = (H + 31) / 32;   // 1 bit per unit for the ReLU backward (a16)
     GP_TRY(tgemm(KC_GEMM_FWD, g));
-    // x2 = x1 + h W_2 + b_2                                                  (a11)
-    float *x2;
-    if (!last) x2 = b.x2;
-    else if (k == K - 1) x2 = w.x_out;
-    else if (!replay) x2 = slot[k + 1][m];            // boundary stash (a12)
-    else if (replay_full) x2 = w.x_out;               // replay output nobody reads
-    else x2 = nullptr;                                // skipped: B_k does not need F_k's output
+    // x2 += h W_2                                                            (a11)
     if (x2) {
       g = GemmArgs{};
       g.M = (int)T_mb; g.N = d; g.K = H;
       g.A = b.h; g.lda = H; g.B = W(q.w_2); g.ldb = d; g.C = x2; g.ldc = d;
-      g.bias = P(q.b_2); g.resid = b.x1; g.flags = EPI_BIAS | EPI_RESID | EPI_OUT_F32;
+      g.flags = EPI_ACCUM | EPI_OUT_F32;
       GP_TRY(tgemm(KC_GEMM_FWD, g));
     }
     x = x2;
@@ -270,7 +274,7 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
   if (k == K - 1) {
     if (nl == 0 && K == 1) x = w.x_emb;
     // y = LN_f(x_L); logits = y W_out; fused softmax-CE -> loss partial, dlogits   (a13, a14)
-    GP_TRY(tln(x, P(i_lnf_g), P(i_lnf_b), w.y, w.meanf, w.rstdf));
+    GP_TRY(tln(x, P(i_lnf_g), P(i_lnf_b), w.y, w.meanf, w.rstdf, nullptr, nullptr));
     GemmArgs g{};
     g.M = (int)T_mb; g.N = V; g.K = d;
     g.A = w.y; g.lda = d; g.B = W(i_w_out); g.ldb = V; g.C = w.logits; g.ldc = V;

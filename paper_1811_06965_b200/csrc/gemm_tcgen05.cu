@@ -683,7 +683,6 @@ cudaError_t gemm_tc(const Ctx &c, const GemmArgs &a) {
     switch (a.flags) {
       case 0: return tc::launch_pair<256, 1, 0>(c, a);
       case EPI_BIAS: return tc::launch_pair<256, 1, EPI_BIAS>(c, a);
-      case EPI_BIAS | EPI_RESID | EPI_OUT_F32: return tc::launch_pair<256, 1, EPI_BIAS | EPI_RESID | EPI_OUT_F32>(c, a);
       case EPI_BIAS | EPI_RELU | EPI_BITS_OUT: return tc::launch_pair<256, 1, EPI_BIAS | EPI_RELU | EPI_BITS_OUT>(c, a);
       case EPI_MASK | EPI_COLSUM: return tc::launch_pair<256, 1, EPI_MASK | EPI_COLSUM>(c, a);
       case EPI_ACCUM | EPI_OUT_F32: return tc::launch_pair<256, 1, EPI_ACCUM | EPI_OUT_F32>(c, a);

@@ -68,13 +68,17 @@ cudaError_t positional_table(const Ctx &c, float *pe, int S, int d) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// LayerNorm forward: one warp per row, row in registers (NV float4 per lane), two-pass variance
+// LayerNorm forward: one warp per row, row in registers (NV float4 per lane), two-pass variance.
+// Fused residual: when resid_out != NULL the kernel also writes resid_out = x + resid_bias, the
+// value the branch's output GEMM then accumulates into (x' = x + branch(LN(x)) + b, SURVEY 8(a)
+// a5/a8, a9/a11): the GEMM epilogue becomes a TMA reduce-add and never reads x into the SM.
 // ---------------------------------------------------------------------------------------------
 template <typename T, int NV>
 __global__ void __launch_bounds__(128)
 ln_fwd_kernel(const float *__restrict__ x, const float *__restrict__ gamma,
               const float *__restrict__ beta, T *__restrict__ y, float *__restrict__ mean,
-              float *__restrict__ rstd, int64_t n_tok, int d, float eps) {
+              float *__restrict__ rstd, const float *__restrict__ resid_bias, float *__restrict__ resid_out,
+              int64_t n_tok, int d, float eps) {
   int lane = threadIdx.x & 31;
   int64_t row = (int64_t)blockIdx.x * 4 + (threadIdx.x >> 5);
   if (row >= n_tok) return;
@@ -115,31 +119,38 @@ ln_fwd_kernel(const float *__restrict__ x, const float *__restrict__ gamma,
       o.z = (v[i].z - mu) * rs * g.z + b.z;
       o.w = (v[i].w - mu) * rs * g.w + b.w;
       store4(yr + 4 * j, o);
+      if (resid_out) {
+        float4 rb = load4(resid_bias + 4 * j);
+        store4(resid_out + row * d + 4 * j, make_float4(v[i].x + rb.x, v[i].y + rb.y, v[i].z + rb.z, v[i].w + rb.w));
+      }
     }
   }
 }
 
 template <typename T>
 static cudaError_t ln_fwd_t(const Ctx &c, const float *x, const float *gamma, const float *beta,
-                            T *y, float *mean, float *rstd, int64_t n_tok, int d, float eps) {
+                            T *y, float *mean, float *rstd, const float *resid_bias, float *resid_out,
+                            int64_t n_tok, int d, float eps) {
   if (n_tok == 0) return cudaSuccess;
   unsigned grid = (unsigned)((n_tok + 3) / 4);
   int nv = (d / 4 + 31) / 32;
   if (nv <= 1)
-    ln_fwd_kernel<T, 1><<<grid, 128, 0, c.stream>>>(x, gamma, beta, y, mean, rstd, n_tok, d, eps);
+    ln_fwd_kernel<T, 1><<<grid, 128, 0, c.stream>>>(x, gamma, beta, y, mean, rstd, resid_bias, resid_out, n_tok, d, eps);
   else if (nv <= 8)
-    ln_fwd_kernel<T, 8><<<grid, 128, 0, c.stream>>>(x, gamma, beta, y, mean, rstd, n_tok, d, eps);
+    ln_fwd_kernel<T, 8><<<grid, 128, 0, c.stream>>>(x, gamma, beta, y, mean, rstd, resid_bias, resid_out, n_tok, d, eps);
   else if (nv <= 16)
-    ln_fwd_kernel<T, 16><<<grid, 128, 0, c.stream>>>(x, gamma, beta, y, mean, rstd, n_tok, d, eps);
+    ln_fwd_kernel<T, 16><<<grid, 128, 0, c.stream>>>(x, gamma, beta, y, mean, rstd, resid_bias, resid_out, n_tok, d, eps);
   else
     return cudaErrorInvalidValue;
   GP_LAUNCH_CHECK(c);
 }
 
 cudaError_t ln_fwd(const Ctx &c, int dt, const float *x, const float *gamma, const float *beta,
-                   void *y, float *mean, float *rstd, int64_t n_tok, int d, float eps) {
-  return dt == GP_BF16 ? ln_fwd_t<bf16>(c, x, gamma, beta, (bf16 *)y, mean, rstd, n_tok, d, eps)
-                       : ln_fwd_t<float>(c, x, gamma, beta, (float *)y, mean, rstd, n_tok, d, eps);
+                   void *y, float *mean, float *rstd, const float *resid_bias, float *resid_out,
+                   int64_t n_tok, int d, float eps) {
+  if (resid_out && !resid_bias) return cudaErrorInvalidValue;
+  return dt == GP_BF16 ? ln_fwd_t<bf16>(c, x, gamma, beta, (bf16 *)y, mean, rstd, resid_bias, resid_out, n_tok, d, eps)
+                       : ln_fwd_t<float>(c, x, gamma, beta, (float *)y, mean, rstd, resid_bias, resid_out, n_tok, d, eps);
 }
 
 // ---------------------------------------------------------------------------------------------

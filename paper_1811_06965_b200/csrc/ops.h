@@ -63,8 +63,11 @@ cudaError_t positional_table(const Ctx &c, float *pe, int S, int d);
 
 // ---- LayerNorm ------------------------------------------------------------------------------
 // y = (x - mean) * rstd * gamma + beta, biased variance; y is lp, stats fp32 [n_tok].
+// resid_out (optional, fp32 [n_tok, d]) = x + resid_bias[d]: the residual-initialised output the
+// branch's last GEMM accumulates into (EPI_ACCUM).
 cudaError_t ln_fwd(const Ctx &c, int dt, const float *x, const float *gamma, const float *beta,
-                   void *y, float *mean, float *rstd, int64_t n_tok, int d, float eps);
+                   void *y, float *mean, float *rstd, const float *resid_bias, float *resid_out,
+                   int64_t n_tok, int d, float eps);
 // dx_out = (dres_in ? dres_in : 0) + LN'(dy);  dx_out_lp (optional) = lp copy of dx_out.
 // partials: fp32 [ln_bwd_partial_rows(), 3, d] scratch; then dgamma += sum, dbeta += sum and,
 // if colsum_out != NULL, colsum_out[n] += sum_t dx_out[t,n] (the lp copy's values when there is one).

@@ -88,8 +88,10 @@ int gpipe_op_gemm(void *stream, int dtype, int M, int N, int K, const void *A, i
   return ret(gemm(mk(stream, backend), dtype, g), "gpipe_op_gemm");
 }
 int gpipe_op_ln_fwd(void *stream, int dtype, const float *x, const float *gamma, const float *beta,
-                    void *y, float *mean, float *rstd, int64_t n_tok, int d, float eps) {
-  return ret(ln_fwd(mk(stream), dtype, x, gamma, beta, y, mean, rstd, n_tok, d, eps), "gpipe_op_ln_fwd");
+                    void *y, float *mean, float *rstd, const float *resid_bias, float *resid_out,
+                    int64_t n_tok, int d, float eps) {
+  return ret(ln_fwd(mk(stream), dtype, x, gamma, beta, y, mean, rstd, resid_bias, resid_out, n_tok, d, eps),
+             "gpipe_op_ln_fwd");
 }
 int gpipe_op_gemm_timeline(void *dev_buf) {
   gemm_tc_set_timeline((unsigned long long *)dev_buf);

@@ -40,9 +40,9 @@ def gemm_cases(w, T):
     # name, M, N, K, transA, transB, epilogue kwargs (as the engine launches them)
     return [
         ("qkv_fwd", T, 3 * da, d, 0, 0, dict(bias=1)),
-        ("oproj_fwd", T, d, da, 0, 0, dict(bias=1, resid=1)),
+        ("oproj_fwd", T, d, da, 0, 0, dict(accum=1)),
         ("ffn1_fwd", T, H, d, 0, 0, dict(bias=1, relu=1)),
-        ("ffn2_fwd", T, d, H, 0, 0, dict(bias=1, resid=1)),
+        ("ffn2_fwd", T, d, H, 0, 0, dict(accum=1)),
         ("logits_fwd", T, V, d, 0, 0, dict()),
         ("ffn2_dgrad", T, H, d, 0, 1, dict(mask=1, colsum=1)),
         ("ffn1_dgrad", T, d, H, 0, 1, dict()),

@@ -76,9 +76,11 @@ def gemm_workspace(M, N, K, device):
     return _torch().zeros(n, dtype=_torch().uint8, device=device) if n > 0 else None
 
 
-def ln_fwd(x, gamma, beta, y, mean, rstd, eps=1e-5):
+def ln_fwd(x, gamma, beta, y, mean, rstd, eps=1e-5, resid_bias=None, resid_out=None):
+    """resid_out (optional fp32 [n,d]) = x + resid_bias: the buffer the branch's output GEMM accumulates into."""
     n, d = x.shape
-    B._check(B.lib().gpipe_op_ln_fwd(_stream(), _dt(y), _p(x), _p(gamma), _p(beta), _p(y), _p(mean), _p(rstd), n, d, eps))
+    B._check(B.lib().gpipe_op_ln_fwd(_stream(), _dt(y), _p(x), _p(gamma), _p(beta), _p(y), _p(mean), _p(rstd),
+                                     _p(resid_bias), _p(resid_out), n, d, eps))
 
 
 def ln_bwd(dy, x, mean, rstd, gamma, dres_in, dx_out, dx_out_lp, dgamma, dbeta, colsum_out=None):

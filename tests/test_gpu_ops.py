@@ -171,6 +171,12 @@ def test_layernorm_fwd_bwd(dtype, n, d):
     tol, cos = _tol(dtype)
     assert maxrel(_np(y), y_ref) <= tol
     assert maxrel(_np(rs), rstd[:, 0]) <= 1e-5 and maxrel(_np(mean), x.astype(np.float64).mean(1)) <= 1e-5
+    # fused residual init: resid_out = x + bias (what the branch's output GEMM accumulates into)
+    rb = r.standard_normal(d).astype(np.float32)
+    ro, y2 = torch.empty((n, d), device=DEV), torch.empty_like(y)
+    ops.ln_fwd(xt, gt, bt, y2, mean, rs, resid_bias=torch.tensor(rb, device=DEV), resid_out=ro)
+    assert torch.equal(y2, y)
+    assert np.array_equal(_np(ro), x + rb[None, :])
     dx = torch.empty((n, d), device=DEV)
     dx_lp = torch.empty((n, d), device=DEV, dtype=dyt.dtype) if dtype == "bf16" else None
     dg0 = r.standard_normal(d).astype(np.float32)

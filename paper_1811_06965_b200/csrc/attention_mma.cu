@@ -246,18 +246,30 @@ attn_bwd_dq_mma_kernel(const bf16 *__restrict__ qkv, const bf16 *__restrict__ o,
   load_tile<DH>(Vs, base + 2 * da, 3 * da, 0, nkb * BLK, nk);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   const int64_t sbase = ((int64_t)seq * A + h) * S;
-  // D_i = sum_c dO[i,c] * O[i,c], 16 rows per warp, straight from global memory
-  for (int rr = 0; rr < 16; ++rr) {
-    int row = q0 + warp * 16 + rr;
+  // D_i = sum_c dO[i,c] * O[i,c]: two lanes per row, every load of the warp's 16 rows in flight at once
+  {
+    const int rr = lane >> 1, hf = lane & 1;
+    const int row = q0 + warp * 16 + rr;
     float acc = 0.f;
-    if (row < S)
-      for (int c = lane * 2; c < DH; c += 64) {
-        float2 a = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162 *>(dobase + (int64_t)row * da + c));
-        float2 b = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162 *>(obase + (int64_t)row * da + c));
-        acc += a.x * b.x + a.y * b.y;
+    if (row < S) {
+      const uint4 *pa = reinterpret_cast<const uint4 *>(dobase + (int64_t)row * da + hf * (DH / 2));
+      const uint4 *pb = reinterpret_cast<const uint4 *>(obase + (int64_t)row * da + hf * (DH / 2));
+      uint4 ua[DH / 16], ub[DH / 16];
+#pragma unroll
+      for (int i = 0; i < DH / 16; ++i) { ua[i] = __ldg(pa + i); ub[i] = __ldg(pb + i); }
+#pragma unroll
+      for (int i = 0; i < DH / 16; ++i) {
+        const __nv_bfloat162 *ha = reinterpret_cast<const __nv_bfloat162 *>(&ua[i]);
+        const __nv_bfloat162 *hb = reinterpret_cast<const __nv_bfloat162 *>(&ub[i]);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          float2 a = __bfloat1622float2(ha[e]), b = __bfloat1622float2(hb[e]);
+          acc += a.x * b.x + a.y * b.y;
+        }
       }
-    acc = warp_sum(acc);
-    if (lane == 0) {
+    }
+    acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+    if (hf == 0) {
       Dsm[warp * 16 + rr] = acc;
       if (row < S) dvec[sbase + row] = acc;
     }

@@ -159,139 +159,142 @@ cudaError_t ln_fwd(const Ctx &c, int dt, const float *x, const float *gamma, con
 // Fused reductions over the token axis, all in a fixed order (deterministic):
 //   dgamma += sum_t dy*xhat, dbeta += sum_t dy, and optionally colsum_out += sum_t dx_out (the bias
 //   gradient of the linear layer whose output gradient dx_out is: db_2 / db_o).
-// One block per SM, 8 warps, one warp per row; each warp accumulates in registers, the block
-// combines its warps through shared memory and writes one partial row [3][d]; a second small
-// kernel sums the partial rows.
+// One warp per row, WARPS rows per block pass, every load of a row (x, dy, incoming residual
+// gradient) in flight at once: the kernel is one DRAM round trip deep.  Each warp leaves its row's
+// three contribution vectors in its own shared-memory slot; the block sums the slots column-wise
+// (thread t owns columns t, t + blockDim, ...), keeps the running sums in registers across passes
+// and writes one partial row [3][d] per block; a second small kernel sums the partial rows.
 // ---------------------------------------------------------------------------------------------
-constexpr int LNB_WARPS = 8;
-
-template <typename T, int NV>
-__global__ void __launch_bounds__(LNB_WARPS * 32)
+template <typename T, int NV, int WARPS>
+__global__ void __launch_bounds__(WARPS * 32, 1)
 ln_bwd_kernel(const T *__restrict__ dy, const float *__restrict__ x, const float *__restrict__ mean,
               const float *__restrict__ rstd, const float *__restrict__ gamma,
               const float *__restrict__ dres_in, float *__restrict__ dx_out,
               T *__restrict__ dx_out_lp, float *__restrict__ partials, int64_t n_tok, int d, int want_colsum) {
-  extern __shared__ float sm[];       // [d] gamma, then [3][d] block partial
-  float *gsm = sm, *psm = sm + d;
-  int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  int d4 = d >> 2;
-  for (int i = threadIdx.x; i < d; i += blockDim.x) gsm[i] = gamma[i];
-  for (int i = threadIdx.x; i < 3 * d; i += blockDim.x) psm[i] = 0.f;
-  __syncthreads();
-  float4 ag[NV], ab[NV], ac[NV];
+  extern __shared__ __align__(16) float red[];       // [WARPS][3][d]
+  constexpr int NT = WARPS * 32;
+  constexpr int NACC = (3 * 128 * NV + NT - 1) / NT; // columns of [3][d] per thread (d <= 128*NV)
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int d4 = d >> 2;
+  float *slot = red + (size_t)w * 3 * d;
+  float acc[NACC];
 #pragma unroll
-  for (int i = 0; i < NV; ++i) {
-    ag[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    ab[i] = ag[i];
-    ac[i] = ag[i];
-  }
-  for (int64_t row = (int64_t)blockIdx.x * LNB_WARPS + w; row < n_tok; row += (int64_t)gridDim.x * LNB_WARPS) {
-    float mu = mean[row], rs = rstd[row];
-    float4 xh[NV], dh[NV];
-    float s1 = 0.f, s2 = 0.f;
-#pragma unroll
-    for (int i = 0; i < NV; ++i) {
-      int j = lane + 32 * i;
-      if (j < d4) {
-        xh[i] = load4(x + row * d + 4 * j);
-        dh[i] = load4(dy + row * d + 4 * j);
-      }
-    }
-#pragma unroll
-    for (int i = 0; i < NV; ++i) {
-      int j = lane + 32 * i;
-      if (j < d4) {
-        float4 gv = *reinterpret_cast<const float4 *>(gsm + 4 * j);
-        xh[i] = make_float4((xh[i].x - mu) * rs, (xh[i].y - mu) * rs, (xh[i].z - mu) * rs, (xh[i].w - mu) * rs);
-        ag[i].x += dh[i].x * xh[i].x; ag[i].y += dh[i].y * xh[i].y;
-        ag[i].z += dh[i].z * xh[i].z; ag[i].w += dh[i].w * xh[i].w;
-        ab[i].x += dh[i].x; ab[i].y += dh[i].y; ab[i].z += dh[i].z; ab[i].w += dh[i].w;
-        dh[i] = make_float4(dh[i].x * gv.x, dh[i].y * gv.y, dh[i].z * gv.z, dh[i].w * gv.w);
-        s1 += (dh[i].x + dh[i].y) + (dh[i].z + dh[i].w);
-        s2 += (dh[i].x * xh[i].x + dh[i].y * xh[i].y) + (dh[i].z * xh[i].z + dh[i].w * xh[i].w);
-      }
-    }
-    float m1 = warp_sum(s1) / (float)d, m2 = warp_sum(s2) / (float)d;
-#pragma unroll
-    for (int i = 0; i < NV; ++i) {
-      int j = lane + 32 * i;
-      if (j < d4) {
-        float4 o;
-        o.x = (dh[i].x - m1 - xh[i].x * m2) * rs;
-        o.y = (dh[i].y - m1 - xh[i].y * m2) * rs;
-        o.z = (dh[i].z - m1 - xh[i].z * m2) * rs;
-        o.w = (dh[i].w - m1 - xh[i].w * m2) * rs;
-        if (dres_in) {
-          float4 r = load4(dres_in + row * d + 4 * j);
-          o.x += r.x; o.y += r.y; o.z += r.z; o.w += r.w;
-        }
-        store4(dx_out + row * d + 4 * j, o);
-        if (dx_out_lp) {
-          store4(dx_out_lp + row * d + 4 * j, o);
-          if (want_colsum)                                           // sum what the GEMMs will read
-            o = make_float4(to_f<T>(from_f<T>(o.x)), to_f<T>(from_f<T>(o.y)), to_f<T>(from_f<T>(o.z)),
-                            to_f<T>(from_f<T>(o.w)));
-        }
-        ac[i].x += o.x; ac[i].y += o.y; ac[i].z += o.z; ac[i].w += o.w;
-      }
-    }
-  }
-  // combine the warps of the block in a fixed order (w = 0..7), then one partial row per block
-  for (int turn = 0; turn < LNB_WARPS; ++turn) {
-    if (w == turn) {
+  for (int j = 0; j < NACC; ++j) acc[j] = 0.f;
+  for (int64_t base = (int64_t)blockIdx.x * WARPS; base < n_tok; base += (int64_t)gridDim.x * WARPS) {
+    const int64_t row = base + w;
+    if (row < n_tok) {
+      float4 xh[NV], dh[NV], dr[NV];
 #pragma unroll
       for (int i = 0; i < NV; ++i) {
-        int j = lane + 32 * i;
+        const int j = lane + 32 * i;
         if (j < d4) {
-          float4 *p0 = reinterpret_cast<float4 *>(psm + 4 * j);
-          float4 *p1 = reinterpret_cast<float4 *>(psm + d + 4 * j);
-          float4 *p2 = reinterpret_cast<float4 *>(psm + 2 * d + 4 * j);
-          float4 a = *p0, b = *p1, c = *p2;
-          a.x += ag[i].x; a.y += ag[i].y; a.z += ag[i].z; a.w += ag[i].w;
-          b.x += ab[i].x; b.y += ab[i].y; b.z += ab[i].z; b.w += ab[i].w;
-          c.x += ac[i].x; c.y += ac[i].y; c.z += ac[i].z; c.w += ac[i].w;
-          *p0 = a; *p1 = b; *p2 = c;
+          xh[i] = load4(x + row * d + 4 * j);
+          dh[i] = load4(dy + row * d + 4 * j);
+          dr[i] = dres_in ? load4(dres_in + row * d + 4 * j) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
+      }
+      const float mu = mean[row], rs = rstd[row];
+      float s1 = 0.f, s2 = 0.f;
+#pragma unroll
+      for (int i = 0; i < NV; ++i) {
+        const int j = lane + 32 * i;
+        if (j < d4) {
+          const float4 gv = load4(gamma + 4 * j);
+          xh[i] = make_float4((xh[i].x - mu) * rs, (xh[i].y - mu) * rs, (xh[i].z - mu) * rs, (xh[i].w - mu) * rs);
+          *reinterpret_cast<float4 *>(slot + 4 * j) =
+              make_float4(dh[i].x * xh[i].x, dh[i].y * xh[i].y, dh[i].z * xh[i].z, dh[i].w * xh[i].w);
+          *reinterpret_cast<float4 *>(slot + d + 4 * j) = dh[i];
+          dh[i] = make_float4(dh[i].x * gv.x, dh[i].y * gv.y, dh[i].z * gv.z, dh[i].w * gv.w);
+          s1 += (dh[i].x + dh[i].y) + (dh[i].z + dh[i].w);
+          s2 += (dh[i].x * xh[i].x + dh[i].y * xh[i].y) + (dh[i].z * xh[i].z + dh[i].w * xh[i].w);
+        }
+      }
+      const float m1 = warp_sum(s1) / (float)d, m2 = warp_sum(s2) / (float)d;
+#pragma unroll
+      for (int i = 0; i < NV; ++i) {
+        const int j = lane + 32 * i;
+        if (j < d4) {
+          float4 o;
+          o.x = (dh[i].x - m1 - xh[i].x * m2) * rs + dr[i].x;
+          o.y = (dh[i].y - m1 - xh[i].y * m2) * rs + dr[i].y;
+          o.z = (dh[i].z - m1 - xh[i].z * m2) * rs + dr[i].z;
+          o.w = (dh[i].w - m1 - xh[i].w * m2) * rs + dr[i].w;
+          store4(dx_out + row * d + 4 * j, o);
+          if (dx_out_lp) {
+            store4(dx_out_lp + row * d + 4 * j, o);
+            if (want_colsum)                                           // sum what the GEMMs will read
+              o = make_float4(to_f<T>(from_f<T>(o.x)), to_f<T>(from_f<T>(o.y)), to_f<T>(from_f<T>(o.z)),
+                              to_f<T>(from_f<T>(o.w)));
+          }
+          *reinterpret_cast<float4 *>(slot + 2 * d + 4 * j) = o;
+        }
+      }
+    } else {
+      for (int j = lane; j < 3 * d4; j += 32) *reinterpret_cast<float4 *>(slot + 4 * j) = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < NACC; ++j) {
+      const int idx = threadIdx.x + NT * j;
+      if (idx < 3 * d) {
+        float t = 0.f;
+#pragma unroll
+        for (int r = 0; r < WARPS; ++r) t += red[(size_t)r * 3 * d + idx];      // rows in order
+        acc[j] += t;
       }
     }
     __syncthreads();
   }
   float *out = partials + (size_t)blockIdx.x * 3 * d;
-  for (int i = threadIdx.x; i < 3 * d; i += blockDim.x) out[i] = psm[i];
+#pragma unroll
+  for (int j = 0; j < NACC; ++j) {
+    const int idx = threadIdx.x + NT * j;
+    if (idx < 3 * d) out[idx] = acc[j];
+  }
 }
 
-// dst[which][col] += sum_r partials[r][which][col]; block = 8 row-lanes x 32 columns
-__global__ void __launch_bounds__(256)
+// dst[which][col] += sum_r partials[r][which][col]; block = 32 row-lanes x 32 columns
+__global__ void __launch_bounds__(1024)
 ln_bwd_reduce_kernel(const float *__restrict__ partials, int n_part, int d, float *__restrict__ dgamma,
                      float *__restrict__ dbeta, float *__restrict__ colsum_out) {
-  __shared__ float red[8][33];
+  __shared__ float red[32][33];
   int which = blockIdx.y;
   float *dst = which == 0 ? dgamma : (which == 1 ? dbeta : colsum_out);
   if (!dst) return;
-  int col = blockIdx.x * 32 + (threadIdx.x & 31);
-  int ry = threadIdx.x >> 5;
-  float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
-  if (col < d) {
-    int r = ry;
-    for (; r + 24 < n_part; r += 32) {
-      s0 += partials[((size_t)r * 3 + which) * d + col];
-      s1 += partials[((size_t)(r + 8) * 3 + which) * d + col];
-      s2 += partials[((size_t)(r + 16) * 3 + which) * d + col];
-      s3 += partials[((size_t)(r + 24) * 3 + which) * d + col];
-    }
-    for (; r < n_part; r += 8) s0 += partials[((size_t)r * 3 + which) * d + col];
-  }
-  red[ry][threadIdx.x & 31] = (s0 + s1) + (s2 + s3);
+  const int cx = threadIdx.x & 31, ry = threadIdx.x >> 5;
+  const int col = blockIdx.x * 32 + cx;
+  float s = 0.f;
+  if (col < d)
+    for (int r = ry; r < n_part; r += 32) s += partials[((size_t)r * 3 + which) * d + col];
+  red[ry][cx] = s;
   __syncthreads();
   if (ry == 0 && col < d) {
     float t = 0.f;
 #pragma unroll
-    for (int r = 0; r < 8; ++r) t += red[r][threadIdx.x & 31];
+    for (int r = 0; r < 32; ++r) t += red[r][cx];
     dst[col] += t;
   }
 }
 
 int ln_bwd_partial_rows(int sm_count) { return sm_count; }
+
+template <typename T, int NV, int WARPS>
+static cudaError_t ln_bwd_launch(const Ctx &c, const T *dy, const float *x, const float *mean, const float *rstd,
+                                 const float *gamma, const float *dres_in, float *dx_out, T *dx_out_lp,
+                                 float *partials, int64_t n_tok, int d, int want_colsum, int *grid_out) {
+  int64_t want = (n_tok + WARPS - 1) / WARPS;
+  int grid = (int)(want < ln_bwd_partial_rows(c.sm_count) ? want : ln_bwd_partial_rows(c.sm_count));
+  size_t smem = (size_t)WARPS * 3 * d * sizeof(float);
+  auto kern = ln_bwd_kernel<T, NV, WARPS>;
+  if (smem > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+  }
+  kern<<<grid, WARPS * 32, smem, c.stream>>>(dy, x, mean, rstd, gamma, dres_in, dx_out, dx_out_lp, partials, n_tok, d,
+                                             want_colsum);
+  *grid_out = grid;
+  return cudaGetLastError();
+}
 
 template <typename T>
 static cudaError_t ln_bwd_t(const Ctx &c, const T *dy, const float *x, const float *mean,
@@ -299,23 +302,18 @@ static cudaError_t ln_bwd_t(const Ctx &c, const T *dy, const float *x, const flo
                             float *dx_out, T *dx_out_lp, float *partials, float *dgamma,
                             float *dbeta, float *colsum_out, int64_t n_tok, int d) {
   if (n_tok == 0) return cudaSuccess;
-  int64_t want = (n_tok + LNB_WARPS - 1) / LNB_WARPS;
-  int grid = (int)(want < ln_bwd_partial_rows(c.sm_count) ? want : ln_bwd_partial_rows(c.sm_count));
-  size_t smem = (size_t)4 * d * sizeof(float);
-  int nv = (d / 4 + 31) / 32;
-#define GP_LNB(NV_)                                                                               \
-  ln_bwd_kernel<T, NV_><<<grid, LNB_WARPS * 32, smem, c.stream>>>(dy, x, mean, rstd, gamma, dres_in, \
-                                                                   dx_out, dx_out_lp, partials, n_tok, d, colsum_out != nullptr)
-  if (nv <= 1) GP_LNB(1);
-  else if (nv <= 8) GP_LNB(8);
-  else if (nv <= 16) GP_LNB(16);
+  const int nv = (d / 4 + 31) / 32;
+  const int wc = colsum_out != nullptr;
+  int grid = 0;
+  cudaError_t e;
+  if (nv <= 1) e = ln_bwd_launch<T, 1, 16>(c, dy, x, mean, rstd, gamma, dres_in, dx_out, dx_out_lp, partials, n_tok, d, wc, &grid);
+  else if (nv <= 8) e = ln_bwd_launch<T, 8, 16>(c, dy, x, mean, rstd, gamma, dres_in, dx_out, dx_out_lp, partials, n_tok, d, wc, &grid);
+  else if (nv <= 16) e = ln_bwd_launch<T, 16, 8>(c, dy, x, mean, rstd, gamma, dres_in, dx_out, dx_out_lp, partials, n_tok, d, wc, &grid);
   else return cudaErrorInvalidValue;
-#undef GP_LNB
   if (c.launches) ++*c.launches;
-  cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   dim3 rg((d + 31) / 32, colsum_out ? 3 : 2);
-  ln_bwd_reduce_kernel<<<rg, 256, 0, c.stream>>>(partials, grid, d, dgamma, dbeta, colsum_out);
+  ln_bwd_reduce_kernel<<<rg, 1024, 0, c.stream>>>(partials, grid, d, dgamma, dbeta, colsum_out);
   GP_LAUNCH_CHECK(c);
 }
 

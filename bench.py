@@ -102,6 +102,15 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+_T0 = time.perf_counter()
+
+
+def progress(msg):
+    """Phase marker on stderr (stdout carries only the JSON line)."""
+    if int(os.environ.get("RANK", "0")) == 0:
+        print("[bench %7.1fs] %s" % (time.perf_counter() - _T0, msg), file=sys.stderr, flush=True)
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -193,8 +202,10 @@ def run_ours(args, w, rank, world, local_rank):
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     peaks = measured_peaks()
+    progress("library built and loaded; creating engine for %s" % w.name)
     eng = gp.from_workload(w, device=dev)
     eng.init_params(seed=1000 + rank, std=0.02, parity=False)
+    progress("engine ready (%.1f GB arena)" % (eng.peak_bytes()["total"] / 1e9))
     tok, lab = gi.make_tokens(w, 2000 + rank)
     tok_d, lab_d = torch.tensor(tok, device=dev), torch.tensor(lab, device=dev)
     tok_h = torch.tensor(tok).pin_memory().numpy()
@@ -214,18 +225,22 @@ def run_ours(args, w, rank, world, local_rank):
         return max_over_ranks(e0.elapsed_time(e1), world)
 
     loss = None
-    for _ in range(args.warmup):
+    for i in range(args.warmup):
         loss = eng.step(tok_d, lab_d)
         eng.zero_grads()
+        progress("warm-up step %d done, loss %.4f" % (i, loss))
     sampler = ClockSampler(local_rank) if rank == 0 else None
     l0 = eng.launch_count()
     ms = timed(lambda: eng.step(tok_d, lab_d), args.steps)
     launches = (eng.launch_count() - l0)
     clocks = sampler.stop() if sampler else None
+    progress("timed region done: %.1f ms/step" % (ms / args.steps))
     ms_e2e = timed(lambda: eng.step(tok_h, lab_h), args.steps)
     # one extra step with per-launch CUDA events for the roofline of the dominant kernel class
+    progress("e2e region done: %.1f ms/step; per-launch timing step" % (ms_e2e / args.steps))
     eng.kernel_timing(True, serial=True)         # each launch alone on the GPU: standalone durations
     eng.step(tok_d, lab_d)
+    progress("per-launch timing step done")
     stats = eng.kernel_stats()
     eng.kernel_timing(False)
     eng.zero_grads()
@@ -267,6 +282,7 @@ def run_ours(args, w, rank, world, local_rank):
                     "h2d_bytes_per_step": int(tok.nbytes + lab.nbytes), "d2h_bytes_per_step": 4 * w.M},
             "gpu_launches": int(launches)}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        progress("timing the CPU oracle sample")
         line["cpu_baseline"] = {k: v for k, v in oracle_sample(w).items() if k != "seconds"}
     eng.close()
     if rank == 0:

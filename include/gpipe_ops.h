@@ -77,7 +77,8 @@ int gpipe_op_ln_bwd(void *stream, int dtype, const void *dy, const float *x, con
                     int64_t n_tok, int d);
 
 /* qkv lp [n_seq*S, 3*A*dh] (q|k|v blocks); o lp [n_seq*S, A*dh]; lse fp32 [n_seq, A, S].
- * backend: 0 = auto, 1 = SIMT. */
+ * backend: 0 = auto (bf16: tcgen05 when d_head = 64 and S <= 256, else mma.sync; fp32: SIMT), 1 = SIMT,
+ * 2 = legacy mma.sync kernels (bf16, d_head 32 / 64; GPIPE_ENOTIMPL-style CUDA error otherwise). */
 int gpipe_op_attn_fwd(void *stream, int dtype, const void *qkv, void *o, float *lse, int n_seq, int S,
                       int A, int dh, int causal, int backend);
 int gpipe_op_attn_bwd(void *stream, int dtype, const void *qkv, const void *o, const void *d_o,

@@ -1,0 +1,589 @@
+// attention_tcgen05.cu - attention forward / backward on the 5th-generation tensor cores (sm_100a)
+// for sequences of at most 256 tokens and d_head = 64 (every bf16 workload of BASELINE.json;
+// SURVEY 8(a) a7, a16; K5/K6 of DESIGN.md).
+//
+// With S <= 256 a whole row of scores fits one TMEM accumulator (128 lanes x 256 fp32 columns), so
+// the forward softmax is a plain two-pass row softmax by the thread that owns the TMEM lane: no
+// online rescaling, no cross-thread reduction.  All five backward products of a head run on
+// tcgen05.mma from 128-byte-swizzled shared-memory tiles that TMA fetched where the tensors lie
+// (head h = 64 columns of the [tokens, 3*d_a] qkv matrix; 3-D tensor maps [seq][row][col] clip and
+// zero-fill at the end of a sequence).
+//
+// forward  (one CTA = 128 query rows of one (sequence, head), 4 warps, 2 CTAs / SM):
+//   TMA Q, K, V -> S = Q K^T (M 128, N <= 256, K 64) in TMEM -> per-lane row max, P = exp2(..) as bf16
+//   into swizzled K-major panels (overlaying Q / K, which are dead by then) -> O = P V
+//   (M 128, N 64, K <= 256; V is the MN-major B operand as it lies) -> O / l -> TMA store; LSE.
+// backward (one CTA = one (sequence, head), 8 compute warps + 1 control warp, 1 CTA / SM):
+//   for key block j, query block i (128 x 128 each):  S = Q_i K_j^T, dP = dO_i V_j^T  (TMEM)
+//   -> P = exp2(S - lse), dS = P (dP - D) as bf16 panels in shared memory
+//   -> dV_j += P^T dO_i, dK_j += dS^T Q_i (the panels read as MN-major A), dQ_i += dS K_j (K-major A);
+//   dV_j, dK_j, dQ_0, dQ_1 stay in TMEM (4 x 64 columns) next to S and dP (2 x 128): 512 columns.
+//   The control thread issues S/dP of the next block pair as soon as the compute warps have pulled
+//   the current pair into registers, so the tensor pipe works under the exponentials.
+//   Deterministic: no atomics, fixed accumulation order.
+// Roofline: bf16 tensor pipe / MUFU.EX2.
+#include <cuda.h>
+#include <math.h>
+
+#include <mutex>
+#include <unordered_map>
+
+#include "common.cuh"
+#include "tcgen05.cuh"
+
+namespace gp {
+namespace fat {
+
+using namespace tc;
+
+constexpr int DH = 64;
+constexpr uint32_t TILE = 128 * 128;          // bytes of a [128 rows x 64 bf16] swizzled tile
+constexpr float LOG2E = 1.4426950408889634f;
+
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1, int c2) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+      ::"r"(dst), "l"((uint64_t)map), "r"(bar), "r"(c0), "r"(c1), "r"(c2)
+      : "memory");
+}
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap *map, uint32_t src, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4}], [%1];"
+               ::"l"((uint64_t)map), "r"(src), "r"(c0), "r"(c1), "r"(c2)
+               : "memory");
+}
+__device__ __forceinline__ float ex2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ uint32_t pack2(float lo, float hi) {
+  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t *>(&v);
+}
+// instruction descriptor: D fp32, A / B bf16, majorness (1 = MN-major), N, M = 128
+__device__ __forceinline__ uint32_t idesc(int a_mn, int b_mn, int N) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)a_mn << 15) | ((uint32_t)b_mn << 16) |
+         ((uint32_t)(N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+}
+// K-major operand tile [rows x 64 k] (8-row atoms 1024 B apart): descriptor of k-step ks (16 k = 32 B)
+__device__ __forceinline__ uint64_t desc_k(uint32_t tile, int ks) { return make_smem_desc(tile + ks * 32, 16, 1024); }
+// MN-major operand: [k rows x 64 mn] panels (128 B rows), panels TILE bytes apart; k-step = 16 rows
+__device__ __forceinline__ uint64_t desc_mn(uint32_t tile, int ks) { return make_smem_desc(tile + ks * 2048, TILE, 1024); }
+
+// one row of a swizzled [128 x 128 B] panel: 16-byte chunk c of row r
+__device__ __forceinline__ uint32_t panel_addr(uint32_t panel, int r, int c) {
+  return panel + (uint32_t)r * 128u + (uint32_t)((c ^ (r & 7)) << 4);
+}
+
+// ---------------------------------------------------------------------------------------------
+// forward
+// ---------------------------------------------------------------------------------------------
+// shared memory (from a 1024-byte aligned base): Q [0,16K) | K [16K,48K) | pad [48K,64K) | V [64K,96K);
+// P (4 panels, 64 KB) overlays [0,64K); the O staging (4 warps x 4 KB) overlays [0,16K) afterwards.
+constexpr size_t FWD_SMEM = 96 * 1024 + 1024;
+
+__global__ void __launch_bounds__(128)
+attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_constant__ CUtensorMap map_o,
+                   float *__restrict__ lse, int S, int A, int causal, float scale) {
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ __align__(8) uint64_t bars[4];
+  __shared__ uint32_t tmem_base_smem;
+  const uint32_t sb = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sQ = sb, sK = sb + TILE, sV = sb + 4 * TILE, sP = sb;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int da = A * DH, seq = blockIdx.y / A, h = blockIdx.y - seq * A;
+  const int q0 = blockIdx.x * 128;
+  const int nk = causal ? min(S, q0 + 128) : S;          // keys this block can see
+  const int nkb = (nk + 127) >> 7;
+  const int N = (nk + 15) & ~15;                         // MMA N of the score product / K of P V
+  const uint32_t bar_qk = smem_u32(&bars[0]), bar_v = smem_u32(&bars[1]), bar_s = smem_u32(&bars[2]),
+                 bar_o = smem_u32(&bars[3]);
+  if (threadIdx.x == 0) {
+    tma_prefetch_desc(&map_qkv);
+    tma_prefetch_desc(&map_o);
+    for (int i = 0; i < 4; ++i) mbar_init(bar_qk + 8 * i, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_smem)), "n"(256));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  tcgen05_fence_before();
+  __syncthreads();
+  tcgen05_fence_after();
+  const uint32_t tmem = tmem_base_smem;
+
+  if (threadIdx.x == 0) {
+    mbar_expect_tx(bar_qk, (1 + nkb) * TILE);
+    tma_load_3d(sQ, &map_qkv, bar_qk, h * DH, q0, seq);
+    for (int b = 0; b < nkb; ++b) tma_load_3d(sK + b * TILE, &map_qkv, bar_qk, da + h * DH, b * 128, seq);
+    mbar_expect_tx(bar_v, nkb * TILE);
+    for (int b = 0; b < nkb; ++b) tma_load_3d(sV + b * TILE, &map_qkv, bar_v, 2 * da + h * DH, b * 128, seq);
+    mbar_wait(bar_qk, 0);
+    tcgen05_fence_after();
+    const uint32_t id = idesc(0, 0, N);
+#pragma unroll
+    for (int ks = 0; ks < DH / 16; ++ks) umma_bf16(tmem, desc_k(sQ, ks), desc_k(sK, ks), id, ks ? 1u : 0u);
+    tcgen05_commit(bar_s);
+  }
+  __syncwarp();
+
+  // ---- softmax of this thread's row ----
+  const int row = q0 + warp * 32 + lane;
+  const uint32_t t_row = tmem + ((uint32_t)(warp * 32) << 16);
+  const float sl2 = scale * LOG2E;
+  const int kmax_w = causal ? min(nk, q0 + warp * 32 + 32) : nk;     // keys any row of this warp can see
+  const int nch = (kmax_w + 31) >> 5, nch_all = (N + 31) >> 5;
+  mbar_wait(bar_s, 0);
+  tcgen05_fence_after();
+  float mx = -INFINITY;
+  uint32_t r[32];
+  for (int c = 0; c < nch; ++c) {
+    tmem_ld32(t_row + c * 32, r);
+    tmem_ld_wait();
+    const bool edge = c * 32 + 32 > nk || (causal && c * 32 + 31 > q0 + warp * 32);
+    if (edge) {
+#pragma unroll
+      for (int j = 0; j < 32; ++j) {
+        const int key = c * 32 + j;
+        if (key < nk && !(causal && key > row)) mx = fmaxf(mx, __uint_as_float(r[j]));
+      }
+    } else {
+#pragma unroll
+      for (int j = 0; j < 32; ++j) mx = fmaxf(mx, __uint_as_float(r[j]));
+    }
+  }
+  const float ms = mx * sl2;
+  float l = 0.f;
+  for (int c = 0; c < nch_all; ++c) {
+    uint32_t pk[16];
+    if (c < nch) {
+      tmem_ld32(t_row + c * 32, r);
+      tmem_ld_wait();
+      const bool edge = c * 32 + 32 > nk || (causal && c * 32 + 31 > q0 + warp * 32);
+      float p[32];
+#pragma unroll
+      for (int j = 0; j < 32; ++j) p[j] = ex2(fmaf(__uint_as_float(r[j]), sl2, -ms));
+      if (edge) {
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+          const int key = c * 32 + j;
+          if (!(key < nk && !(causal && key > row))) p[j] = 0.f;
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < 32; ++j) l += p[j];
+#pragma unroll
+      for (int j = 0; j < 16; ++j) pk[j] = pack2(p[2 * j], p[2 * j + 1]);
+    } else {
+#pragma unroll
+      for (int j = 0; j < 16; ++j) pk[j] = 0u;
+    }
+    const uint32_t panel = sP + (uint32_t)(c >> 1) * TILE;
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+      st_shared_v4(panel_addr(panel, warp * 32 + lane, (c & 1) * 4 + q), pk[4 * q], pk[4 * q + 1], pk[4 * q + 2], pk[4 * q + 3]);
+  }
+  fence_proxy_async_smem();
+  tcgen05_fence_before();
+  __syncthreads();
+
+  if (threadIdx.x == 0) {
+    tcgen05_fence_after();
+    mbar_wait(bar_v, 0);
+    const uint32_t id = idesc(0, 1, DH);
+    for (int kk = 0; kk < N / 16; ++kk)
+      umma_bf16(tmem, desc_k(sP + (uint32_t)(kk >> 2) * TILE, kk & 3), desc_mn(sV, kk), id, kk ? 1u : 0u);
+    tcgen05_commit(bar_o);
+  }
+  __syncwarp();
+  mbar_wait(bar_o, 0);
+  tcgen05_fence_after();
+  const float inv = 1.f / l;
+  const uint32_t stg = sb + (uint32_t)warp * 4096u;         // this warp's 32 rows x 128 B
+#pragma unroll
+  for (int c = 0; c < 2; ++c) {
+    tmem_ld32(t_row + c * 32, r);
+    tmem_ld_wait();
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+      st_shared_v4(panel_addr(stg, lane, c * 4 + q),
+                   pack2(__uint_as_float(r[8 * q]) * inv, __uint_as_float(r[8 * q + 1]) * inv),
+                   pack2(__uint_as_float(r[8 * q + 2]) * inv, __uint_as_float(r[8 * q + 3]) * inv),
+                   pack2(__uint_as_float(r[8 * q + 4]) * inv, __uint_as_float(r[8 * q + 5]) * inv),
+                   pack2(__uint_as_float(r[8 * q + 6]) * inv, __uint_as_float(r[8 * q + 7]) * inv));
+  }
+  fence_proxy_async_smem();
+  __syncwarp();
+  if (lane == 0) {
+    tma_store_3d(&map_o, stg, h * DH, q0 + warp * 32, seq);   // rows past S are clipped
+    bulk_commit();
+  }
+  if (row < S) lse[((int64_t)seq * A + h) * S + row] = mx * scale + logf(l);
+  if (lane == 0) bulk_wait_all();
+  tcgen05_fence_before();
+  __syncthreads();
+  if (warp == 0) {
+    tcgen05_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(256));
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// backward
+// ---------------------------------------------------------------------------------------------
+// shared memory: Q | K | V | dO (2 tiles each: 128 KB) | P (2 panels) | dS (2 panels).  A warp stages its
+// output rows in the 4 KB slab of the P panel that only it writes.
+constexpr size_t BWD_SMEM = 12 * TILE + 1024;
+constexpr int BWD_THREADS = 288;
+// TMEM columns
+constexpr uint32_t C_S = 0, C_DP = 128, C_DV = 256, C_DK = 320, C_DQ = 384;
+
+__global__ void __launch_bounds__(BWD_THREADS, 1)
+attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_constant__ CUtensorMap map_do,
+                   const __grid_constant__ CUtensorMap map_dqkv, const bf16 *__restrict__ o,
+                   const bf16 *__restrict__ d_o, const float *__restrict__ lse, int S, int A, int causal,
+                   float scale) {
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ __align__(8) uint64_t bars[5];
+  __shared__ uint32_t tmem_base_smem;
+  __shared__ float Lsm[256], Dsm[256];
+  const uint32_t sb = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sQ = sb, sK = sb + 2 * TILE, sV = sb + 4 * TILE, sdO = sb + 6 * TILE, sP = sb + 8 * TILE,
+                 sdS = sb + 10 * TILE;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int da = A * DH, seq = blockIdx.x / A, h = blockIdx.x - seq * A;
+  const int nblk = (S + 127) >> 7;                       // 1 or 2 blocks of 128 rows
+  const uint32_t bar_ld = smem_u32(&bars[0]), bar_sp = smem_u32(&bars[1]), bar_tfree = smem_u32(&bars[2]),
+                 bar_pds = smem_u32(&bars[3]), bar_acc = smem_u32(&bars[4]);
+  if (threadIdx.x == 0) {
+    tma_prefetch_desc(&map_qkv);
+    tma_prefetch_desc(&map_do);
+    tma_prefetch_desc(&map_dqkv);
+    mbar_init(bar_ld, 1);
+    mbar_init(bar_sp, 1);
+    mbar_init(bar_tfree, 256);
+    mbar_init(bar_pds, 256);
+    mbar_init(bar_acc, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 8) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_smem)), "n"(512));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  tcgen05_fence_before();
+  __syncthreads();
+  tcgen05_fence_after();
+  const uint32_t tmem = tmem_base_smem;
+
+  if (warp == 8) {
+    // ===================== control: TMA loads, every tcgen05.mma =====================
+    if (lane == 0) {
+      mbar_expect_tx(bar_ld, 4 * nblk * TILE);
+      for (int b = 0; b < nblk; ++b) {
+        tma_load_3d(sQ + b * TILE, &map_qkv, bar_ld, h * DH, b * 128, seq);
+        tma_load_3d(sK + b * TILE, &map_qkv, bar_ld, da + h * DH, b * 128, seq);
+        tma_load_3d(sV + b * TILE, &map_qkv, bar_ld, 2 * da + h * DH, b * 128, seq);
+        tma_load_3d(sdO + b * TILE, &map_do, bar_ld, h * DH, b * 128, seq);
+      }
+      mbar_wait(bar_ld, 0);
+      tcgen05_fence_after();
+      const uint32_t id_sp = idesc(0, 0, 128), id_g_mn = idesc(1, 1, DH), id_g_k = idesc(0, 1, DH);
+      auto issue_sp = [&](int i, int j) {
+#pragma unroll
+        for (int ks = 0; ks < 4; ++ks)
+          umma_bf16(tmem + C_S, desc_k(sQ + i * TILE, ks), desc_k(sK + j * TILE, ks), id_sp, ks ? 1u : 0u);
+#pragma unroll
+        for (int ks = 0; ks < 4; ++ks)
+          umma_bf16(tmem + C_DP, desc_k(sdO + i * TILE, ks), desc_k(sV + j * TILE, ks), id_sp, ks ? 1u : 0u);
+        tcgen05_commit(bar_sp);
+      };
+      // block pairs in order: j outer, i inner (i >= j when causal)
+      int n = 0;
+      uint32_t dq_started = 0;                            // bit i: dQ_i already holds a partial sum
+      issue_sp(0, 0);
+      for (int j = 0; j < nblk; ++j) {
+        const int i_first = causal ? j : 0;
+        for (int i = i_first; i < nblk; ++i, ++n) {
+          mbar_wait(bar_tfree, n & 1);                    // S / dP of this pair are in registers
+          tcgen05_fence_after();
+          int ni = i + 1, nj = j;                         // next pair
+          if (ni == nblk) { nj = j + 1; ni = causal ? nj : 0; }
+          if (nj < nblk) issue_sp(ni, nj);
+          mbar_wait(bar_pds, n & 1);                      // P / dS panels written
+          tcgen05_fence_after();
+#pragma unroll
+          for (int kk = 0; kk < 8; ++kk)                  // dV_j += P^T dO_i   (K = 128 queries)
+            umma_bf16(tmem + C_DV, desc_mn(sP, kk), desc_mn(sdO + i * TILE, kk), id_g_mn, (i > i_first || kk) ? 1u : 0u);
+#pragma unroll
+          for (int kk = 0; kk < 8; ++kk)                  // dK_j += dS^T Q_i
+            umma_bf16(tmem + C_DK, desc_mn(sdS, kk), desc_mn(sQ + i * TILE, kk), id_g_mn, (i > i_first || kk) ? 1u : 0u);
+#pragma unroll
+          for (int kk = 0; kk < 8; ++kk)                  // dQ_i += dS K_j     (K = 128 keys)
+            umma_bf16(tmem + C_DQ + 64 * i, desc_k(sdS + (uint32_t)(kk >> 2) * TILE, kk & 3), desc_mn(sK + j * TILE, kk),
+                      id_g_k, (((dq_started >> i) & 1u) || kk) ? 1u : 0u);
+          dq_started |= 1u << i;
+          tcgen05_commit(bar_acc);
+        }
+      }
+    }
+    __syncwarp();
+  } else {
+    // ===================== compute warps =====================
+    const int quad = warp & 3, chalf = warp >> 2;
+    const int64_t sbase = ((int64_t)seq * A + h) * S;
+    // D = rowsum(dO * O), L = lse * log2(e): 8 lanes per row, 4 rows per pass, 8 passes per warp
+    {
+      const int sub = lane >> 3, l8 = lane & 7;
+#pragma unroll
+      for (int it = 0; it < 8; ++it) {
+        const int rr = warp * 32 + it * 4 + sub;
+        float acc = 0.f;
+        if (rr < S) {
+          const int64_t off = ((int64_t)seq * S + rr) * da + h * DH + l8 * 8;
+          const uint4 ua = __ldg(reinterpret_cast<const uint4 *>(d_o + off));
+          const uint4 ub = __ldg(reinterpret_cast<const uint4 *>(o + off));
+          const __nv_bfloat162 *ha = reinterpret_cast<const __nv_bfloat162 *>(&ua);
+          const __nv_bfloat162 *hb = reinterpret_cast<const __nv_bfloat162 *>(&ub);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const float2 a = __bfloat1622float2(ha[e]), b = __bfloat1622float2(hb[e]);
+            acc += a.x * b.x + a.y * b.y;
+          }
+        }
+        acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+        acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+        acc += __shfl_xor_sync(0xffffffffu, acc, 4);
+        if (l8 == 0) {
+          Dsm[rr] = acc;
+          Lsm[rr] = rr < S ? lse[sbase + rr] * LOG2E : 0.f;
+        }
+      }
+    }
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+    const float sl2 = scale * LOG2E;
+    const uint32_t stg = sP + (uint32_t)chalf * TILE + (uint32_t)quad * 4096u;   // == this warp's rows of its P panel
+    const int r_loc = quad * 32 + lane;                   // row within the 128-row block
+    int n = 0;
+    for (int j = 0; j < nblk; ++j) {
+      const int i_first = causal ? j : 0;
+      for (int i = i_first; i < nblk; ++i, ++n) {
+        const int row = i * 128 + r_loc;
+        const int key0 = j * 128 + chalf * 64;
+        // whole strip masked (causal, above the diagonal) ?
+        const bool dead = causal && i == j && chalf * 64 > quad * 32 + 31;
+        uint32_t ppk[32], dpk[32];
+        mbar_wait(bar_sp, n & 1);
+        tcgen05_fence_after();
+        if (!dead) {
+          const float Lr = Lsm[row], Dr = Dsm[row];
+          const bool edge = (causal && i == j) || key0 + 64 > S || row >= S;
+          const uint32_t t_row = tmem + ((uint32_t)(quad * 32) << 16) + (uint32_t)(chalf * 64);
+#pragma unroll
+          for (int c = 0; c < 2; ++c) {
+            uint32_t rs[32], rd[32];
+            tmem_ld32(t_row + C_S + c * 32, rs);
+            tmem_ld32(t_row + C_DP + c * 32, rd);
+            tmem_ld_wait();
+#pragma unroll
+            for (int jj = 0; jj < 32; jj += 2) {
+              float p0 = ex2(fmaf(__uint_as_float(rs[jj]), sl2, -Lr));
+              float p1 = ex2(fmaf(__uint_as_float(rs[jj + 1]), sl2, -Lr));
+              if (edge) {
+                const int k0 = key0 + c * 32 + jj;
+                if (row >= S || k0 >= S || (causal && k0 > row)) p0 = 0.f;
+                if (row >= S || k0 + 1 >= S || (causal && k0 + 1 > row)) p1 = 0.f;
+              }
+              ppk[c * 16 + (jj >> 1)] = pack2(p0, p1);
+              dpk[c * 16 + (jj >> 1)] = pack2(p0 * (__uint_as_float(rd[jj]) - Dr), p1 * (__uint_as_float(rd[jj + 1]) - Dr));
+            }
+          }
+        } else {
+#pragma unroll
+          for (int q = 0; q < 32; ++q) { ppk[q] = 0u; dpk[q] = 0u; }
+        }
+        tcgen05_fence_before();
+        mbar_arrive(bar_tfree);                            // TMEM S / dP may be overwritten
+        if (n > 0) mbar_wait(bar_acc, (n - 1) & 1);        // the MMAs that read the previous panels are done
+        if (lane == 0) bulk_wait_read<0>();                // ... and so is the TMA store staged in this warp's slab
+        __syncwarp();
+        const uint32_t pp = sP + (uint32_t)chalf * TILE, dp = sdS + (uint32_t)chalf * TILE;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+          st_shared_v4(panel_addr(pp, r_loc, q), ppk[4 * q], ppk[4 * q + 1], ppk[4 * q + 2], ppk[4 * q + 3]);
+          st_shared_v4(panel_addr(dp, r_loc, q), dpk[4 * q], dpk[4 * q + 1], dpk[4 * q + 2], dpk[4 * q + 3]);
+        }
+        fence_proxy_async_smem();
+        mbar_arrive(bar_pds);
+        if (i == nblk - 1) {
+          // ---- dV_j (warps 0-3) / dK_j (warps 4-7) complete: TMEM -> bf16 -> staging -> TMA store ----
+          mbar_wait(bar_acc, n & 1);
+          tcgen05_fence_after();
+          const uint32_t t_acc = tmem + ((uint32_t)(quad * 32) << 16) + (chalf ? C_DK : C_DV);
+          const float mul = chalf ? scale : 1.f;
+          if (lane == 0) bulk_wait_read<0>();
+          __syncwarp();
+#pragma unroll
+          for (int c = 0; c < 2; ++c) {
+            uint32_t rr[32];
+            tmem_ld32(t_acc + c * 32, rr);
+            tmem_ld_wait();
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+              st_shared_v4(panel_addr(stg, lane, c * 4 + q),
+                           pack2(__uint_as_float(rr[8 * q]) * mul, __uint_as_float(rr[8 * q + 1]) * mul),
+                           pack2(__uint_as_float(rr[8 * q + 2]) * mul, __uint_as_float(rr[8 * q + 3]) * mul),
+                           pack2(__uint_as_float(rr[8 * q + 4]) * mul, __uint_as_float(rr[8 * q + 5]) * mul),
+                           pack2(__uint_as_float(rr[8 * q + 6]) * mul, __uint_as_float(rr[8 * q + 7]) * mul));
+          }
+          fence_proxy_async_smem();
+          __syncwarp();
+          if (lane == 0) {
+            tma_store_3d(&map_dqkv, stg, (chalf ? da : 2 * da) + h * DH, j * 128 + quad * 32, seq);
+            bulk_commit();
+          }
+        }
+      }
+    }
+    // ---- dQ: warps 0-3 -> block 0, warps 4-7 -> block 1 (every MMA has completed: last bar_acc) ----
+    if (chalf < nblk) {
+      const uint32_t t_acc = tmem + ((uint32_t)(quad * 32) << 16) + C_DQ + 64 * chalf;
+      if (lane == 0) bulk_wait_read<0>();
+      __syncwarp();
+#pragma unroll
+      for (int c = 0; c < 2; ++c) {
+        uint32_t rr[32];
+        tmem_ld32(t_acc + c * 32, rr);
+        tmem_ld_wait();
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+          st_shared_v4(panel_addr(stg, lane, c * 4 + q),
+                       pack2(__uint_as_float(rr[8 * q]) * scale, __uint_as_float(rr[8 * q + 1]) * scale),
+                       pack2(__uint_as_float(rr[8 * q + 2]) * scale, __uint_as_float(rr[8 * q + 3]) * scale),
+                       pack2(__uint_as_float(rr[8 * q + 4]) * scale, __uint_as_float(rr[8 * q + 5]) * scale),
+                       pack2(__uint_as_float(rr[8 * q + 6]) * scale, __uint_as_float(rr[8 * q + 7]) * scale));
+      }
+      fence_proxy_async_smem();
+      __syncwarp();
+      if (lane == 0) {
+        tma_store_3d(&map_dqkv, stg, h * DH, chalf * 128 + quad * 32, seq);
+        bulk_commit();
+      }
+    }
+    if (lane == 0) bulk_wait_all();
+  }
+  tcgen05_fence_before();
+  __syncthreads();
+  if (warp == 8) {
+    tcgen05_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  static std::once_flag once;
+  std::call_once(once, [] {
+    void *p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)p;
+  });
+  return fn;
+}
+
+struct Key {
+  const void *ptr;
+  int64_t width, S, n_seq;
+  int box_rows;
+  bool operator==(const Key &o) const {
+    return ptr == o.ptr && width == o.width && S == o.S && n_seq == o.n_seq && box_rows == o.box_rows;
+  }
+};
+struct KeyHash {
+  size_t operator()(const Key &k) const {
+    size_t h = (size_t)k.ptr;
+    auto mix = [&](uint64_t v) { h ^= v + 0x9e3779b97f4a7c15ull + (h << 6) + (h >> 2); };
+    mix((uint64_t)k.width); mix((uint64_t)k.S); mix((uint64_t)k.n_seq); mix((uint64_t)k.box_rows);
+    return h;
+  }
+};
+
+// bf16 [n_seq][S][width] (row pitch = width), box [1][box_rows][64], 128-byte swizzle, zero fill
+static bool get_map3(const void *ptr, int64_t width, int64_t S, int64_t n_seq, int box_rows, CUtensorMap *out) {
+  static std::unordered_map<Key, CUtensorMap, KeyHash> cache;
+  static std::mutex mu;
+  Key key{ptr, width, S, n_seq, box_rows};
+  std::lock_guard<std::mutex> lock(mu);
+  auto it = cache.find(key);
+  if (it != cache.end()) {
+    *out = it->second;
+    return true;
+  }
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[3] = {(cuuint64_t)width, (cuuint64_t)S, (cuuint64_t)n_seq};
+  cuuint64_t strides[2] = {(cuuint64_t)width * 2, (cuuint64_t)width * 2 * (cuuint64_t)S};
+  cuuint32_t box[3] = {64, (cuuint32_t)box_rows, 1};
+  cuuint32_t estr[3] = {1, 1, 1};
+  CUtensorMap m;
+  CUresult r = fn(&m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void *>(ptr), dims, strides, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return false;
+  if (cache.size() > 16384) cache.clear();
+  cache.emplace(key, m);
+  *out = m;
+  return true;
+}
+
+}  // namespace fat
+
+bool attn_tc_supported(int dt, int S, int A, int dh) {
+  (void)A;
+  return dt == GP_BF16 && dh == 64 && S >= 1 && S <= 256;
+}
+
+cudaError_t attn_fwd_tc(const Ctx &c, const void *qkv, void *o, float *lse, int n_seq, int S, int A, int causal) {
+  if (n_seq == 0) return cudaSuccess;
+  const int da = A * fat::DH;
+  CUtensorMap mq, mo;
+  if (!fat::get_map3(qkv, 3 * da, S, n_seq, 128, &mq) || !fat::get_map3(o, da, S, n_seq, 32, &mo)) return cudaErrorInvalidValue;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(fat::attn_fwd_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fat::FWD_SMEM);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  dim3 grid((S + 127) / 128, n_seq * A);
+  fat::attn_fwd_tc_kernel<<<grid, 128, fat::FWD_SMEM, c.stream>>>(mq, mo, lse, S, A, causal, 1.f / sqrtf((float)fat::DH));
+  GP_LAUNCH_CHECK(c);
+}
+
+cudaError_t attn_bwd_tc(const Ctx &c, const void *qkv, const void *o, const void *d_o, const float *lse, void *dqkv,
+                        int n_seq, int S, int A, int causal) {
+  if (n_seq == 0) return cudaSuccess;
+  const int da = A * fat::DH;
+  CUtensorMap mq, md, mg;
+  if (!fat::get_map3(qkv, 3 * da, S, n_seq, 128, &mq) || !fat::get_map3(d_o, da, S, n_seq, 128, &md) ||
+      !fat::get_map3(dqkv, 3 * da, S, n_seq, 32, &mg))
+    return cudaErrorInvalidValue;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(fat::attn_bwd_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fat::BWD_SMEM);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  fat::attn_bwd_tc_kernel<<<n_seq * A, fat::BWD_THREADS, fat::BWD_SMEM, c.stream>>>(
+      mq, md, mg, (const bf16 *)o, (const bf16 *)d_o, lse, S, A, causal, 1.f / sqrtf((float)fat::DH));
+  GP_LAUNCH_CHECK(c);
+}
+
+}  // namespace gp

@@ -1,4 +1,6 @@
 // ops_api.cu - extern "C" wrappers of include/gpipe_ops.h and the backend dispatch of ops.h.
+#include <stdlib.h>
+
 #include <string>
 
 #include "../../include/gpipe.h"
@@ -21,6 +23,16 @@ cudaError_t attn_fwd_mma(const Ctx &c, const void *qkv, void *o, float *lse, int
 cudaError_t attn_bwd_mma(const Ctx &c, const void *qkv, const void *o, const void *d_o, const float *lse,
                          void *dqkv, float *dvec, int n_seq, int S, int A, int dh, int causal);
 
+bool attn_tc_supported(int dt, int S, int A, int dh);
+cudaError_t attn_fwd_tc(const Ctx &c, const void *qkv, void *o, float *lse, int n_seq, int S, int A, int causal);
+cudaError_t attn_bwd_tc(const Ctx &c, const void *qkv, const void *o, const void *d_o, const float *lse, void *dqkv,
+                        int n_seq, int S, int A, int causal);
+// GPIPE_ATTN_BACKEND=mma keeps the legacy mma.sync kernels (A/B comparisons); default: tcgen05 where it applies
+static bool attn_use_tc() {
+  static const int v = [] { const char *e = getenv("GPIPE_ATTN_BACKEND"); return (e && std::string(e) == "mma") ? 0 : 1; }();
+  return v != 0;
+}
+
 cudaError_t gemm(const Ctx &c, int dt, const GemmArgs &a) {
   const bool colsum = (a.flags & EPI_COLSUM) != 0;
   // column sums are taken of the stored lp output (in fp32 mode lp storage is fp32 itself)
@@ -39,12 +51,14 @@ cudaError_t gemm(const Ctx &c, int dt, const GemmArgs &a) {
 }
 cudaError_t attn_fwd(const Ctx &c, int dt, const void *qkv, void *o, float *lse, int n_seq, int S,
                      int A, int dh, int causal) {
+  if (attn_use_tc() && attn_tc_supported(dt, S, A, dh)) return attn_fwd_tc(c, qkv, o, lse, n_seq, S, A, causal);
   if (attn_mma_supported(dt, S, A, dh)) return attn_fwd_mma(c, qkv, o, lse, n_seq, S, A, dh, causal);
   return attn_fwd_simt(c, dt, qkv, o, lse, n_seq, S, A, dh, causal);
 }
 cudaError_t attn_bwd(const Ctx &c, int dt, const void *qkv, const void *o, const void *d_o,
                      const float *lse, void *dqkv, float *dvec, int n_seq, int S, int A, int dh,
                      int causal) {
+  if (attn_use_tc() && attn_tc_supported(dt, S, A, dh)) return attn_bwd_tc(c, qkv, o, d_o, lse, dqkv, n_seq, S, A, causal);
   if (attn_mma_supported(dt, S, A, dh)) return attn_bwd_mma(c, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal);
   return attn_bwd_simt(c, dt, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal);
 }
@@ -113,17 +127,20 @@ int gpipe_op_ln_bwd(void *stream, int dtype, const void *dy, const float *x, con
 int gpipe_op_attn_fwd(void *stream, int dtype, const void *qkv, void *o, float *lse, int n_seq, int S,
                       int A, int dh, int causal, int backend) {
   Ctx c = mk(stream);
-  return ret(backend == 1 ? attn_fwd_simt(c, dtype, qkv, o, lse, n_seq, S, A, dh, causal)
-                          : attn_fwd(c, dtype, qkv, o, lse, n_seq, S, A, dh, causal),
+  if (backend == 2 && !attn_mma_supported(dtype, S, A, dh)) return ret(cudaErrorNotSupported, "gpipe_op_attn_fwd");
+  return ret(backend == 1   ? attn_fwd_simt(c, dtype, qkv, o, lse, n_seq, S, A, dh, causal)
+             : backend == 2 ? attn_fwd_mma(c, qkv, o, lse, n_seq, S, A, dh, causal)
+                            : attn_fwd(c, dtype, qkv, o, lse, n_seq, S, A, dh, causal),
              "gpipe_op_attn_fwd");
 }
 int gpipe_op_attn_bwd(void *stream, int dtype, const void *qkv, const void *o, const void *d_o,
                       const float *lse, void *dqkv, float *dvec, int n_seq, int S, int A, int dh,
                       int causal, int backend) {
   Ctx c = mk(stream);
-  return ret(backend == 1
-                 ? attn_bwd_simt(c, dtype, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal)
-                 : attn_bwd(c, dtype, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal),
+  if (backend == 2 && !attn_mma_supported(dtype, S, A, dh)) return ret(cudaErrorNotSupported, "gpipe_op_attn_bwd");
+  return ret(backend == 1   ? attn_bwd_simt(c, dtype, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal)
+             : backend == 2 ? attn_bwd_mma(c, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal)
+                            : attn_bwd(c, dtype, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal),
              "gpipe_op_attn_bwd");
 }
 int gpipe_op_softmax_ce(void *stream, int dtype, void *logits, const int32_t *labels, float *rowloss,

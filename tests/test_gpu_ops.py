@@ -201,19 +201,23 @@ def test_layernorm_fwd_bwd(dtype, n, d):
 # attention
 # -------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("dtype", ["fp32", "bf16"])
-@pytest.mark.parametrize("S,A,dh", [(16, 4, 16), (40, 3, 32), (256, 2, 64), (100, 2, 64)])
+@pytest.mark.parametrize("S,A,dh", [(16, 4, 16), (40, 3, 32), (256, 2, 64), (100, 2, 64), (129, 3, 64), (64, 1, 64),
+                                    (200, 2, 64), (3, 1, 64)])
 @pytest.mark.parametrize("causal", [0, 1])
-def test_attention_fwd_bwd(dtype, S, A, dh, causal):
+@pytest.mark.parametrize("backend", [0, 2])       # 0: auto (tcgen05 for bf16, d_head 64, S <= 256); 2: legacy mma.sync
+def test_attention_fwd_bwd(dtype, S, A, dh, causal, backend):
+    if backend == 2 and (dtype != "bf16" or dh not in (32, 64)):
+        pytest.skip("mma.sync attention: bf16, d_head 32 / 64 only")
     n_seq, da = 2, A * dh
     r = _rng(S * A + dh + causal)
     qkvt, qkvq = _lp(r.standard_normal((n_seq * S, 3 * da)), dtype)
     dot, doq = _lp(r.standard_normal((n_seq * S, da)), dtype)
     o = torch.empty((n_seq * S, da), device=DEV, dtype=qkvt.dtype)
     lse = torch.empty((n_seq, A, S), device=DEV)
-    ops.attn_fwd(qkvt, o, lse, n_seq, S, A, dh, causal)
+    ops.attn_fwd(qkvt, o, lse, n_seq, S, A, dh, causal, backend)
     dqkv = torch.empty_like(qkvt)
     dvec = torch.empty((n_seq, A, S), device=DEV)
-    ops.attn_bwd(qkvt, o, dot, lse, dqkv, dvec, n_seq, S, A, dh, causal)
+    ops.attn_bwd(qkvt, o, dot, lse, dqkv, dvec, n_seq, S, A, dh, causal, backend)
     tol, cos = _tol(dtype)
     if dtype == "bf16":
         tol = 2 ** -6                                   # P and dS are rounded to bf16 on tensor cores

@@ -23,7 +23,7 @@ static int fail(int code, const std::string &msg) {
   return code;
 }
 static int cuda_fail(cudaError_t e, const char *where) {
-  g_err = std::string(where) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")";
+  g_err = std::string(where) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")" + watchdog_describe();
   return GPIPE_ECUDA;
 }
 #define API_CUDA(x, where)                            \
@@ -107,6 +107,7 @@ int gpipe_create(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t 
   if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&e.sm_count, cudaDevAttrMultiProcessorCount, dev);
   int cc_major = 0;
   if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev);
+  if (ce == cudaSuccess) ce = watchdog_init();
   if (ce != cudaSuccess) { delete g; return cuda_fail(ce, "gpipe_create: no usable CUDA device"); }
   if (cc_major != 10) { delete g; return fail(GPIPE_ECUDA, "gpipe_create: this library is built for sm_100a (B200) only"); }
   std::string err;

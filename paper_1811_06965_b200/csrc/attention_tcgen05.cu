@@ -119,7 +119,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
     for (int b = 0; b < nkb; ++b) tma_load_3d(sK + b * TILE, &map_qkv, bar_qk, da + h * DH, b * 128, seq);
     mbar_expect_tx(bar_v, nkb * TILE);
     for (int b = 0; b < nkb; ++b) tma_load_3d(sV + b * TILE, &map_qkv, bar_v, 2 * da + h * DH, b * 128, seq);
-    mbar_wait(bar_qk, 0);
+    mbar_wait(bar_qk, 0, 0x21);
     tcgen05_fence_after();
     const uint32_t id = idesc(0, 0, N);
 #pragma unroll
@@ -134,7 +134,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
   const float sl2 = scale * LOG2E;
   const int kmax_w = causal ? min(nk, q0 + warp * 32 + 32) : nk;     // keys any row of this warp can see
   const int nch = (kmax_w + 31) >> 5, nch_all = (N + 31) >> 5;
-  mbar_wait(bar_s, 0);
+  mbar_wait(bar_s, 0, 0x22);
   tcgen05_fence_after();
   float mx = -INFINITY;
   uint32_t r[32];
@@ -190,14 +190,14 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
 
   if (threadIdx.x == 0) {
     tcgen05_fence_after();
-    mbar_wait(bar_v, 0);
+    mbar_wait(bar_v, 0, 0x23);
     const uint32_t id = idesc(0, 1, DH);
     for (int kk = 0; kk < N / 16; ++kk)
       umma_bf16(tmem, desc_k(sP + (uint32_t)(kk >> 2) * TILE, kk & 3), desc_mn(sV, kk), id, kk ? 1u : 0u);
     tcgen05_commit(bar_o);
   }
   __syncwarp();
-  mbar_wait(bar_o, 0);
+  mbar_wait(bar_o, 0, 0x24);
   tcgen05_fence_after();
   const float inv = 1.f / l;
   const uint32_t stg = sb + (uint32_t)warp * 4096u;         // this warp's 32 rows x 128 B
@@ -286,7 +286,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
         tma_load_3d(sV + b * TILE, &map_qkv, bar_ld, 2 * da + h * DH, b * 128, seq);
         tma_load_3d(sdO + b * TILE, &map_do, bar_ld, h * DH, b * 128, seq);
       }
-      mbar_wait(bar_ld, 0);
+      mbar_wait(bar_ld, 0, 0x31);
       tcgen05_fence_after();
       const uint32_t id_sp = idesc(0, 0, 128), id_g_mn = idesc(1, 1, DH), id_g_k = idesc(0, 1, DH);
       auto issue_sp = [&](int i, int j) {
@@ -305,12 +305,12 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
       for (int j = 0; j < nblk; ++j) {
         const int i_first = causal ? j : 0;
         for (int i = i_first; i < nblk; ++i, ++n) {
-          mbar_wait(bar_tfree, n & 1);                    // S / dP of this pair are in registers
+          mbar_wait(bar_tfree, n & 1, 0x32);                    // S / dP of this pair are in registers
           tcgen05_fence_after();
           int ni = i + 1, nj = j;                         // next pair
           if (ni == nblk) { nj = j + 1; ni = causal ? nj : 0; }
           if (nj < nblk) issue_sp(ni, nj);
-          mbar_wait(bar_pds, n & 1);                      // P / dS panels written
+          mbar_wait(bar_pds, n & 1, 0x33);                      // P / dS panels written
           tcgen05_fence_after();
 #pragma unroll
           for (int kk = 0; kk < 8; ++kk)                  // dV_j += P^T dO_i   (K = 128 queries)
@@ -373,7 +373,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
         // whole strip masked (causal, above the diagonal) ?
         const bool dead = causal && i == j && chalf * 64 > quad * 32 + 31;
         uint32_t ppk[32], dpk[32];
-        mbar_wait(bar_sp, n & 1);
+        mbar_wait(bar_sp, n & 1, 0x34);
         tcgen05_fence_after();
         if (!dead) {
           const float Lr = Lsm[row], Dr = Dsm[row];
@@ -404,7 +404,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
         }
         tcgen05_fence_before();
         mbar_arrive(bar_tfree);                            // TMEM S / dP may be overwritten
-        if (n > 0) mbar_wait(bar_acc, (n - 1) & 1);        // the MMAs that read the previous panels are done
+        if (n > 0) mbar_wait(bar_acc, (n - 1) & 1, 0x35);        // the MMAs that read the previous panels are done
         if (lane == 0) bulk_wait_read<0>();                // ... and so is the TMA store staged in this warp's slab
         __syncwarp();
         const uint32_t pp = sP + (uint32_t)chalf * TILE, dp = sdS + (uint32_t)chalf * TILE;
@@ -417,7 +417,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
         mbar_arrive(bar_pds);
         if (i == nblk - 1) {
           // ---- dV_j (warps 0-3) / dK_j (warps 4-7) complete: TMEM -> bf16 -> staging -> TMA store ----
-          mbar_wait(bar_acc, n & 1);
+          mbar_wait(bar_acc, n & 1, 0x36);
           tcgen05_fence_after();
           const uint32_t t_acc = tmem + ((uint32_t)(quad * 32) << 16) + (chalf ? C_DK : C_DV);
           const float mul = chalf ? scale : 1.f;
@@ -545,6 +545,10 @@ static bool get_map3(const void *ptr, int64_t width, int64_t S, int64_t n_seq, i
 }
 
 }  // namespace fat
+
+cudaError_t attn_tc_set_watchdog(unsigned long long *mapped) {
+  return cudaMemcpyToSymbol(tc::g_watchdog, &mapped, sizeof(mapped));
+}
 
 bool attn_tc_supported(int dt, int S, int A, int dh) {
   (void)A;

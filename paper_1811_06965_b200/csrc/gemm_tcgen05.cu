@@ -154,6 +154,14 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  // Both CTAs of the pair are running (and their barriers initialised) before the pair-wide TMEM
+  // allocation is attempted, and - see the teardown - neither SM is handed to another kernel before
+  // BOTH CTAs have returned their columns: a pair dealloc that lands after the peer's SM already hosts
+  // a CTA of another TMEM-using kernel wedges that SM's allocator (observed as a later kernel stuck
+  // in its prologue).
+#ifndef GP_GEMM_NO_PRESYNC
+  cluster_sync_all();
+#endif
   if (warp == 2) {
     asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_smem)),
                  "n"(Cfg::TMEM_COLS));
@@ -180,7 +188,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
         const int m0 = (t % p.tiles_m) * 256 + (int)rank * 128, n0 = (t / p.tiles_m) * BN + (int)rank * BNH;
         const int kb0 = sp * p.kb_per_split, kb1 = min(num_kb, kb0 + p.kb_per_split);
         for (int kb = kb0; kb < kb1; ++kb) {
-          mbar_wait(empty_bar(stage), phase ^ 1);
+          mbar_wait(empty_bar(stage), phase ^ 1, 0x11);
           const uint32_t sa = smem_base + stage * STAGE_BYTES, sb = sa + A_BYTES;
           if (rank == 0) mbar_expect_tx(full_bar(stage), 2 * STAGE_BYTES);
           const uint32_t fb = mapa_shared(full_bar(stage), 0);
@@ -221,11 +229,11 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
       for (int u = pair; u < num_units; u += num_pairs) {
         const int sp = u % splits;
         const int kb0 = sp * p.kb_per_split, kb1 = min(num_kb, kb0 + p.kb_per_split);
-        mbar_wait(tempty_bar(as), aphase ^ 1);       // both CTAs' epilogues have drained this accumulator
+        mbar_wait(tempty_bar(as), aphase ^ 1, 0x12);       // both CTAs' epilogues have drained this accumulator
         tcgen05_fence_after();
         const uint32_t d_tmem = tmem_base + (uint32_t)(as * BN);
         for (int kb = kb0; kb < kb1; ++kb) {
-          mbar_wait(full_bar(stage), phase);
+          mbar_wait(full_bar(stage), phase, 0x13);
           tcgen05_fence_after();
           if (u == pair && kb == kb0) tl_stamp(p, 2);  // first operands landed
           const uint32_t sa = smem_base + stage * STAGE_BYTES, sb = sa + A_BYTES;
@@ -281,7 +289,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
         }
       }
       asm volatile("bar.sync 1, 256;" ::: "memory");       // bias_s visible; colbuf of the previous tile consumed
-      mbar_wait(tfull_bar(as), aphase);
+      mbar_wait(tfull_bar(as), aphase, 0x14);
       tcgen05_fence_after();
       if (it == 0 && et == 0) tl_stamp(p, 4);          // first accumulator complete
       const uint32_t t_row = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(as * BN + chalf * 128);
@@ -511,6 +519,9 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
     tcgen05_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(Cfg::TMEM_COLS));
   }
+#ifndef GP_GEMM_NO_POSTSYNC
+  cluster_sync_all();                                  // no CTA of the pair exits before both deallocations
+#endif
 }
 
 // ------------------------------------------------------------------------------------------
@@ -648,6 +659,9 @@ static cudaError_t launch_pair(const Ctx &c, const GemmArgs &a) {
 // chunk handed to the TMA, stores complete, exit) plus 24 SM-clock stamps of the first tile's epilogue
 // chunks.  buf must hold 32 * SM-count uint64.
 void gemm_tc_set_timeline(unsigned long long *buf) { tc::g_timeline = buf; }
+cudaError_t gemm_tc_set_watchdog(unsigned long long *mapped) {
+  return cudaMemcpyToSymbol(tc::g_watchdog, &mapped, sizeof(mapped));
+}
 
 // Workspace a split-K launch of this shape needs (0 when the shape is not split); the first
 // splitk_cnt_bytes() bytes are the counters and must be ZERO before the first launch (they reset

@@ -97,6 +97,13 @@ cudaError_t attn_bwd(const Ctx &c, int dt, const void *qkv, const void *o, const
                      const float *lse, void *dqkv, float *dvec, int n_seq, int S, int A, int dh,
                      int causal);
 
+// ---- watchdog -------------------------------------------------------------------------------------
+// The tcgen05 kernels bound every mbarrier wait (tcgen05.cuh); a wait that times out records where it
+// was in a block of mapped host memory and traps.  watchdog_init() allocates that block once per
+// process and hands it to the kernels; watchdog_describe() returns "" or a one-line diagnosis.
+cudaError_t watchdog_init();
+const char *watchdog_describe();
+
 // ---- softmax cross-entropy ----------------------------------------------------------------------
 // In place: logits lp [n_tok, V] -> dlogits = (softmax - onehot) * inv_T; rowloss[t] =
 // (logsumexp - logit[label]) * inv_T.  Then loss_reduce sums rowloss into *loss (fp32, overwritten).

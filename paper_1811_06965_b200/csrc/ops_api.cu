@@ -1,4 +1,5 @@
 // ops_api.cu - extern "C" wrappers of include/gpipe_ops.h and the backend dispatch of ops.h.
+#include <stdio.h>
 #include <stdlib.h>
 
 #include <string>
@@ -27,6 +28,36 @@ bool attn_tc_supported(int dt, int S, int A, int dh);
 cudaError_t attn_fwd_tc(const Ctx &c, const void *qkv, void *o, float *lse, int n_seq, int S, int A, int causal);
 cudaError_t attn_bwd_tc(const Ctx &c, const void *qkv, const void *o, const void *d_o, const float *lse, void *dqkv,
                         int n_seq, int S, int A, int causal);
+cudaError_t gemm_tc_set_watchdog(unsigned long long *mapped);
+cudaError_t attn_tc_set_watchdog(unsigned long long *mapped);
+
+static unsigned long long *g_wd_host = nullptr;
+cudaError_t watchdog_init() {
+  static cudaError_t status = [] {
+    unsigned long long *h = nullptr, *d = nullptr;
+    cudaError_t e = cudaHostAlloc((void **)&h, 64, cudaHostAllocMapped);
+    if (e != cudaSuccess) return e;
+    for (int i = 0; i < 8; ++i) h[i] = 0;
+    e = cudaHostGetDevicePointer((void **)&d, h, 0);
+    if (e == cudaSuccess) e = gemm_tc_set_watchdog(d);
+    if (e == cudaSuccess) e = attn_tc_set_watchdog(d);
+    if (e == cudaSuccess) g_wd_host = h;
+    return e;
+  }();
+  return status;
+}
+const char *watchdog_describe() {
+  static thread_local char buf[256];
+  buf[0] = 0;
+  volatile unsigned long long *h = g_wd_host;
+  if (!h || (h[0] >> 16) != 0x5744ull) return buf;
+  static const char *kern[] = {"?", "gemm_tcgen05_pair_kernel", "attn_fwd_tc_kernel", "attn_bwd_tc_kernel"};
+  const unsigned tag = (unsigned)(h[0] & 0xFFFF), k = tag >> 4;
+  snprintf(buf, sizeof(buf), " [watchdog: %s wait #%u timed out: block (%llu,%llu) thread %llu, barrier smem 0x%llx parity %llu]",
+           kern[k < 4 ? k : 0], tag & 15, h[1] & 0xFFFFFFFFull, h[1] >> 32, h[2], h[3] & 0xFFFFFFFFull, h[3] >> 32);
+  return buf;
+}
+
 // GPIPE_ATTN_BACKEND=mma keeps the legacy mma.sync kernels (A/B comparisons); default: tcgen05 where it applies
 static bool attn_use_tc() {
   static const int v = [] { const char *e = getenv("GPIPE_ATTN_BACKEND"); return (e && std::string(e) == "mma") ? 0 : 1; }();
@@ -78,11 +109,12 @@ static int sm_count_cached() {
   return n;
 }
 static Ctx mk(void *stream, int backend = 0) {
+  watchdog_init();
   return Ctx{(cudaStream_t)stream, nullptr, sm_count_cached(), backend};
 }
 static int ret(cudaError_t e, const char *where) {
   if (e == cudaSuccess) return GPIPE_OK;
-  gpipe_set_error_(std::string(where) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")");
+  gpipe_set_error_(std::string(where) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")" + watchdog_describe());
   return e == cudaErrorInvalidValue || e == cudaErrorNotSupported ? GPIPE_EINVAL : GPIPE_ECUDA;
 }
 

@@ -36,9 +36,54 @@ __device__ __forceinline__ uint32_t mbar_try_wait(uint32_t bar, uint32_t parity)
       : "memory");
   return ok;
 }
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+// Watchdog (compile with -DGP_WATCHDOG=1; off by default: the GEMM main loop is sensitive to the
+// extra code at its wait sites).  Every translation unit that includes this header owns a pointer to
+// a few words of MAPPED HOST memory (set through its *_set_watchdog()).  A wait that has spun for
+// more than WAIT_TIMEOUT_NS writes {tag, block, thread, barrier, parity} there and traps: a protocol
+// bug then surfaces as a CUDA error carrying a diagnosis (watchdog_describe()) instead of a hung GPU.
+static __device__ unsigned long long *g_watchdog = nullptr;
+#ifndef GP_WATCHDOG
+#define GP_WATCHDOG 0
+#endif
+#if GP_WATCHDOG
+constexpr unsigned long long WAIT_TIMEOUT_NS = 20ull * 1000 * 1000 * 1000;
+static __device__ __noinline__ void mbar_wait_watchdog(uint32_t bar, uint32_t parity, uint32_t tag) {
+  unsigned long long t0, t1;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+  uint32_t spins = 0;
+  while (!mbar_try_wait(bar, parity)) {
+    if ((++spins & 0x3FFu) == 0) {
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+      if (t1 - t0 > WAIT_TIMEOUT_NS) {
+        volatile unsigned long long *w = g_watchdog;
+        if (w) {
+          w[1] = ((unsigned long long)blockIdx.y << 32) | blockIdx.x;
+          w[2] = threadIdx.x;
+          w[3] = ((unsigned long long)parity << 32) | bar;
+          w[0] = 0x57440000ull | tag;                      // written last
+          __threadfence_system();
+        }
+        __trap();
+      }
+    }
+  }
+}
+#endif
+// tag: which wait this is (kernel * 16 + role), reported by the watchdog
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, uint32_t tag = 0) {
+#if GP_WATCHDOG
+  uint32_t spins = 0;
+  while (!mbar_try_wait(bar, parity)) {
+    if (++spins == (1u << 16)) {
+      mbar_wait_watchdog(bar, parity, tag);
+      return;
+    }
+  }
+#else
+  (void)tag;
   while (!mbar_try_wait(bar, parity)) {
   }
+#endif
 }
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1) {
   asm volatile(

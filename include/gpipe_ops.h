@@ -59,6 +59,8 @@ int gpipe_op_gemm(void *stream, int dtype, int M, int N, int K, const void *A, i
  * 32 * SM-count uint64, owned by the caller; pass NULL
  * to switch the probe off.  Process-global, not thread-safe.  Always returns GPIPE_OK. */
 int gpipe_op_gemm_timeline(void *dev_buf);
+/* Same for the tcgen05 attention backward kernel: 32 %globaltimer stamps per (sequence, head) CTA; NULL disables. */
+int gpipe_op_attn_timeline(void *dev_buf);
 
 /* y = LayerNorm(x) * gamma + beta over the last axis (biased variance); y lp [n_tok,d]; x fp32.
  * Fused residual: if resid_out != NULL (fp32 [n_tok,d], device, caller-owned)

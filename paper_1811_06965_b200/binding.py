@@ -82,6 +82,7 @@ def lib() -> C.CDLL:
         "gpipe_op_gemm": (i32, [vp, i32, i32, i32, i32, vp, i64, i32, vp, i64, i32, vp, i64, vp, vp, vp, i64, vp, vp, vp, i64, i32, i32]),
         "gpipe_op_gemm_workspace_bytes": (i64, [i32, i32, i32]),
         "gpipe_op_gemm_timeline": (i32, [vp]),
+        "gpipe_op_attn_timeline": (i32, [vp]),
         "gpipe_op_ln_fwd": (i32, [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, i64, i32, f32]),
         "gpipe_op_ln_bwd_scratch_floats": (i64, [i32]),
         "gpipe_op_ln_bwd": (i32, [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, i32]),
@@ -108,7 +109,7 @@ EXPORTED_SYMBOLS = [
     "gpipe_step_device", "gpipe_apply_sgd", "gpipe_zero_grads", "gpipe_num_tensors",
     "gpipe_tensor_info", "gpipe_get_param", "gpipe_set_param", "gpipe_get_grad", "gpipe_peak_bytes",
     "gpipe_trace", "gpipe_launch_count", "gpipe_kernel_timing", "gpipe_kernel_stats", "gpipe_debug_read", "gpipe_last_error", "gpipe_version",
-    "gpipe_op_gemm", "gpipe_op_gemm_workspace_bytes", "gpipe_op_gemm_timeline", "gpipe_op_ln_fwd", "gpipe_op_ln_bwd_scratch_floats", "gpipe_op_ln_bwd",
+    "gpipe_op_gemm", "gpipe_op_gemm_workspace_bytes", "gpipe_op_gemm_timeline", "gpipe_op_attn_timeline", "gpipe_op_ln_fwd", "gpipe_op_ln_bwd_scratch_floats", "gpipe_op_ln_bwd",
     "gpipe_op_attn_fwd", "gpipe_op_attn_bwd", "gpipe_op_softmax_ce", "gpipe_op_colsum",
     "gpipe_op_colsum_scratch_floats",
     "gpipe_op_embed_fwd", "gpipe_op_embed_bwd", "gpipe_op_positional", "gpipe_op_sgd",

@@ -79,18 +79,25 @@ __device__ __forceinline__ uint32_t panel_addr(uint32_t panel, int r, int c) {
 // forward
 // ---------------------------------------------------------------------------------------------
 // shared memory (from a 1024-byte aligned base): Q [0,16K) | K [16K,48K) | pad [48K,64K) | V [64K,96K);
-// P (4 panels, 64 KB) overlays [0,64K); the O staging (4 warps x 4 KB) overlays [0,16K) afterwards.
+// P (4 panels, 64 KB) overlays [0,64K) once the score product has retired.
+// 8 warps: warps w and w + 4 own TMEM lane quadrant w & 3 (32 query rows) and split the row's key
+// chunks (32 columns each) in two halves; the halves exchange row max and row sum through shared
+// memory.  TMEM read bandwidth (S is read twice: max, then exp) bounds the softmax, so each thread
+// keeps the next chunk's tcgen05.ld in flight while it works on the current one.
 constexpr size_t FWD_SMEM = 96 * 1024 + 1024;
+constexpr int FWD_THREADS = 256;
 
-__global__ void __launch_bounds__(128)
-attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_constant__ CUtensorMap map_o,
-                   float *__restrict__ lse, int S, int A, int causal, float scale) {
+__global__ void __launch_bounds__(FWD_THREADS, 2)
+attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict__ o, float *__restrict__ lse, int S,
+                   int A, int causal, float scale) {
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t bars[4];
   __shared__ uint32_t tmem_base_smem;
+  __shared__ float xm[2][128], xl[2][128];
   const uint32_t sb = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = sb, sK = sb + TILE, sV = sb + 4 * TILE, sP = sb;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int quad = warp & 3, chalf = warp >> 2;
   const int da = A * DH, seq = blockIdx.y / A, h = blockIdx.y - seq * A;
   const int q0 = blockIdx.x * 128;
   const int nk = causal ? min(S, q0 + 128) : S;          // keys this block can see
@@ -100,11 +107,10 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
                  bar_o = smem_u32(&bars[3]);
   if (threadIdx.x == 0) {
     tma_prefetch_desc(&map_qkv);
-    tma_prefetch_desc(&map_o);
     for (int i = 0; i < 4; ++i) mbar_init(bar_qk + 8 * i, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == 0) {
+  if (warp == 1) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_smem)), "n"(256));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
@@ -128,62 +134,79 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
   }
   __syncwarp();
 
-  // ---- softmax of this thread's row ----
-  const int row = q0 + warp * 32 + lane;
-  const uint32_t t_row = tmem + ((uint32_t)(warp * 32) << 16);
+  // ---- softmax: this thread's row, this half's chunks ----
+  const int r_loc = quad * 32 + lane, row = q0 + r_loc;
+  const uint32_t t_row = tmem + ((uint32_t)(quad * 32) << 16);
   const float sl2 = scale * LOG2E;
-  const int kmax_w = causal ? min(nk, q0 + warp * 32 + 32) : nk;     // keys any row of this warp can see
-  const int nch = (kmax_w + 31) >> 5, nch_all = (N + 31) >> 5;
+  const int kmax = min(nk - 1, causal ? row : nk - 1);              // last key this row sees
+  const int kvis_w = causal ? min(nk, q0 + quad * 32 + 32) : nk;    // keys any row of this warp sees
+  const int nch_all = (N + 31) >> 5, split = (nch_all + 1) >> 1;
+  const int c0 = chalf ? split : 0, c1 = chalf ? nch_all : split;
+  const int cv = min(c1, (kvis_w + 31) >> 5);                        // chunks [c0, cv) hold visible keys
+  // chunk c needs per-element masking when it reaches past the first row's diagonal or past nk
+  auto edge = [&](int c) { return c * 32 + 32 > nk || (causal && c * 32 + 31 > q0 + quad * 32); };
   mbar_wait(bar_s, 0, 0x22);
   tcgen05_fence_after();
+  uint32_t ra[32], rb[32];
   float mx = -INFINITY;
-  uint32_t r[32];
-  for (int c = 0; c < nch; ++c) {
-    tmem_ld32(t_row + c * 32, r);
-    tmem_ld_wait();
-    const bool edge = c * 32 + 32 > nk || (causal && c * 32 + 31 > q0 + warp * 32);
-    if (edge) {
+  auto max_chunk = [&](const uint32_t *r, int c) {
+    if (edge(c)) {
 #pragma unroll
-      for (int j = 0; j < 32; ++j) {
-        const int key = c * 32 + j;
-        if (key < nk && !(causal && key > row)) mx = fmaxf(mx, __uint_as_float(r[j]));
-      }
+      for (int j = 0; j < 32; ++j) mx = fmaxf(mx, c * 32 + j <= kmax ? __uint_as_float(r[j]) : -INFINITY);
     } else {
 #pragma unroll
       for (int j = 0; j < 32; ++j) mx = fmaxf(mx, __uint_as_float(r[j]));
     }
+  };
+  if (c0 < cv) tmem_ld32(t_row + c0 * 32, ra);
+  for (int c = c0; c < cv; c += 2) {
+    tmem_ld_wait();
+    if (c + 1 < cv) tmem_ld32(t_row + (c + 1) * 32, rb);
+    max_chunk(ra, c);
+    if (c + 1 < cv) {
+      tmem_ld_wait();
+      if (c + 2 < cv) tmem_ld32(t_row + (c + 2) * 32, ra);
+      max_chunk(rb, c + 1);
+    }
   }
+  xm[chalf][r_loc] = mx;
+  if (c0 < cv) tmem_ld32(t_row + c0 * 32, ra);           // first chunk of the second pass: in flight over the barrier
+  __syncthreads();
+  mx = fmaxf(xm[0][r_loc], xm[1][r_loc]);                // finite: key 0 is visible to every row
   const float ms = mx * sl2;
   float l = 0.f;
-  for (int c = 0; c < nch_all; ++c) {
-    uint32_t pk[16];
-    if (c < nch) {
-      tmem_ld32(t_row + c * 32, r);
-      tmem_ld_wait();
-      const bool edge = c * 32 + 32 > nk || (causal && c * 32 + 31 > q0 + warp * 32);
-      float p[32];
+  auto exp_chunk = [&](const uint32_t *r, int c) {
+    float p[32];
 #pragma unroll
-      for (int j = 0; j < 32; ++j) p[j] = ex2(fmaf(__uint_as_float(r[j]), sl2, -ms));
-      if (edge) {
+    for (int j = 0; j < 32; ++j) p[j] = ex2(fmaf(__uint_as_float(r[j]), sl2, -ms));
+    if (edge(c)) {
 #pragma unroll
-        for (int j = 0; j < 32; ++j) {
-          const int key = c * 32 + j;
-          if (!(key < nk && !(causal && key > row))) p[j] = 0.f;
-        }
-      }
-#pragma unroll
-      for (int j = 0; j < 32; ++j) l += p[j];
-#pragma unroll
-      for (int j = 0; j < 16; ++j) pk[j] = pack2(p[2 * j], p[2 * j + 1]);
-    } else {
-#pragma unroll
-      for (int j = 0; j < 16; ++j) pk[j] = 0u;
+      for (int j = 0; j < 32; ++j) p[j] = c * 32 + j <= kmax ? p[j] : 0.f;
     }
+#pragma unroll
+    for (int j = 0; j < 32; ++j) l += p[j];
     const uint32_t panel = sP + (uint32_t)(c >> 1) * TILE;
 #pragma unroll
     for (int q = 0; q < 4; ++q)
-      st_shared_v4(panel_addr(panel, warp * 32 + lane, (c & 1) * 4 + q), pk[4 * q], pk[4 * q + 1], pk[4 * q + 2], pk[4 * q + 3]);
+      st_shared_v4(panel_addr(panel, r_loc, (c & 1) * 4 + q), pack2(p[8 * q], p[8 * q + 1]), pack2(p[8 * q + 2], p[8 * q + 3]),
+                   pack2(p[8 * q + 4], p[8 * q + 5]), pack2(p[8 * q + 6], p[8 * q + 7]));
+  };
+  for (int c = c0; c < cv; c += 2) {
+    tmem_ld_wait();
+    if (c + 1 < cv) tmem_ld32(t_row + (c + 1) * 32, rb);
+    exp_chunk(ra, c);
+    if (c + 1 < cv) {
+      tmem_ld_wait();
+      if (c + 2 < cv) tmem_ld32(t_row + (c + 2) * 32, ra);
+      exp_chunk(rb, c + 1);
+    }
   }
+  for (int c = max(cv, c0); c < c1; ++c) {                // chunks no row of this warp sees: P = 0
+    const uint32_t panel = sP + (uint32_t)(c >> 1) * TILE;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) st_shared_v4(panel_addr(panel, r_loc, (c & 1) * 4 + q), 0u, 0u, 0u, 0u);
+  }
+  xl[chalf][r_loc] = l;
   fence_proxy_async_smem();
   tcgen05_fence_before();
   __syncthreads();
@@ -197,33 +220,25 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
     tcgen05_commit(bar_o);
   }
   __syncwarp();
+  l = xl[0][r_loc] + xl[1][r_loc];
   mbar_wait(bar_o, 0, 0x24);
   tcgen05_fence_after();
-  const float inv = 1.f / l;
-  const uint32_t stg = sb + (uint32_t)warp * 4096u;         // this warp's 32 rows x 128 B
-#pragma unroll
-  for (int c = 0; c < 2; ++c) {
-    tmem_ld32(t_row + c * 32, r);
-    tmem_ld_wait();
+  tmem_ld32(t_row + chalf * 32, ra);                      // this thread's 32 of the row's 64 output columns
+  tmem_ld_wait();
+  if (row < S) {
+    const float inv = 1.f / l;
+    uint4 *dst = reinterpret_cast<uint4 *>(o + ((int64_t)seq * S + row) * da + h * DH + chalf * 32);
 #pragma unroll
     for (int q = 0; q < 4; ++q)
-      st_shared_v4(panel_addr(stg, lane, c * 4 + q),
-                   pack2(__uint_as_float(r[8 * q]) * inv, __uint_as_float(r[8 * q + 1]) * inv),
-                   pack2(__uint_as_float(r[8 * q + 2]) * inv, __uint_as_float(r[8 * q + 3]) * inv),
-                   pack2(__uint_as_float(r[8 * q + 4]) * inv, __uint_as_float(r[8 * q + 5]) * inv),
-                   pack2(__uint_as_float(r[8 * q + 6]) * inv, __uint_as_float(r[8 * q + 7]) * inv));
+      dst[q] = make_uint4(pack2(__uint_as_float(ra[8 * q]) * inv, __uint_as_float(ra[8 * q + 1]) * inv),
+                          pack2(__uint_as_float(ra[8 * q + 2]) * inv, __uint_as_float(ra[8 * q + 3]) * inv),
+                          pack2(__uint_as_float(ra[8 * q + 4]) * inv, __uint_as_float(ra[8 * q + 5]) * inv),
+                          pack2(__uint_as_float(ra[8 * q + 6]) * inv, __uint_as_float(ra[8 * q + 7]) * inv));
+    if (chalf == 0) lse[((int64_t)seq * A + h) * S + row] = mx * scale + logf(l);
   }
-  fence_proxy_async_smem();
-  __syncwarp();
-  if (lane == 0) {
-    tma_store_3d(&map_o, stg, h * DH, q0 + warp * 32, seq);   // rows past S are clipped
-    bulk_commit();
-  }
-  if (row < S) lse[((int64_t)seq * A + h) * S + row] = mx * scale + logf(l);
-  if (lane == 0) bulk_wait_all();
   tcgen05_fence_before();
   __syncthreads();
-  if (warp == 0) {
+  if (warp == 1) {
     tcgen05_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(256));
   }
@@ -232,8 +247,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
 // ---------------------------------------------------------------------------------------------
 // backward
 // ---------------------------------------------------------------------------------------------
-// shared memory: Q | K | V | dO (2 tiles each: 128 KB) | P (2 panels) | dS (2 panels).  A warp stages its
-// output rows in the 4 KB slab of the P panel that only it writes.
+// shared memory: Q | K | V | dO (2 tiles each: 128 KB) | P (2 panels) | dS (2 panels)
 constexpr size_t BWD_SMEM = 12 * TILE + 1024;
 constexpr int BWD_THREADS = 288;
 // TMEM columns
@@ -241,11 +255,18 @@ constexpr uint32_t C_S = 0, C_DP = 128, C_DV = 256, C_DK = 320, C_DQ = 384;
 
 __global__ void __launch_bounds__(BWD_THREADS, 1)
 attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_constant__ CUtensorMap map_do,
-                   const __grid_constant__ CUtensorMap map_dqkv, const bf16 *__restrict__ o,
-                   const bf16 *__restrict__ d_o, const float *__restrict__ lse, int S, int A, int causal,
-                   float scale) {
+                   const bf16 *__restrict__ o, const bf16 *__restrict__ d_o, const float *__restrict__ lse,
+                   bf16 *__restrict__ dqkv, int S, int A, int causal, float scale, unsigned long long *tl) {
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t bars[5];
+  // optional timeline probe (attn_tc_set_timeline): 32 %globaltimer stamps per CTA
+  auto stamp = [&](int slot) {
+    if (tl) {
+      unsigned long long t;
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+      tl[(size_t)blockIdx.x * 32 + slot] = t;
+    }
+  };
   __shared__ uint32_t tmem_base_smem;
   __shared__ float Lsm[256], Dsm[256];
   const uint32_t sb = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -259,7 +280,6 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
   if (threadIdx.x == 0) {
     tma_prefetch_desc(&map_qkv);
     tma_prefetch_desc(&map_do);
-    tma_prefetch_desc(&map_dqkv);
     mbar_init(bar_ld, 1);
     mbar_init(bar_sp, 1);
     mbar_init(bar_tfree, 256);
@@ -279,6 +299,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
   if (warp == 8) {
     // ===================== control: TMA loads, every tcgen05.mma =====================
     if (lane == 0) {
+      stamp(0);
       mbar_expect_tx(bar_ld, 4 * nblk * TILE);
       for (int b = 0; b < nblk; ++b) {
         tma_load_3d(sQ + b * TILE, &map_qkv, bar_ld, h * DH, b * 128, seq);
@@ -288,6 +309,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
       }
       mbar_wait(bar_ld, 0, 0x31);
       tcgen05_fence_after();
+      stamp(1);
       const uint32_t id_sp = idesc(0, 0, 128), id_g_mn = idesc(1, 1, DH), id_g_k = idesc(0, 1, DH);
       auto issue_sp = [&](int i, int j) {
 #pragma unroll
@@ -305,13 +327,15 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
       for (int j = 0; j < nblk; ++j) {
         const int i_first = causal ? j : 0;
         for (int i = i_first; i < nblk; ++i, ++n) {
-          mbar_wait(bar_tfree, n & 1, 0x32);                    // S / dP of this pair are in registers
+          mbar_wait(bar_tfree, n & 1, 0x32);              // S / dP of this pair are in registers
           tcgen05_fence_after();
+          if (n < 4) stamp(2 + 3 * n);
           int ni = i + 1, nj = j;                         // next pair
           if (ni == nblk) { nj = j + 1; ni = causal ? nj : 0; }
           if (nj < nblk) issue_sp(ni, nj);
-          mbar_wait(bar_pds, n & 1, 0x33);                      // P / dS panels written
+          mbar_wait(bar_pds, n & 1, 0x33);                // P / dS panels written (and dV_{j-1}, dK_{j-1} read out)
           tcgen05_fence_after();
+          if (n < 4) stamp(3 + 3 * n);
 #pragma unroll
           for (int kk = 0; kk < 8; ++kk)                  // dV_j += P^T dO_i   (K = 128 queries)
             umma_bf16(tmem + C_DV, desc_mn(sP, kk), desc_mn(sdO + i * TILE, kk), id_g_mn, (i > i_first || kk) ? 1u : 0u);
@@ -324,6 +348,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
                       id_g_k, (((dq_started >> i) & 1u) || kk) ? 1u : 0u);
           dq_started |= 1u << i;
           tcgen05_commit(bar_acc);
+          if (n < 4) stamp(4 + 3 * n);
         }
       }
     }
@@ -332,81 +357,113 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
     // ===================== compute warps =====================
     const int quad = warp & 3, chalf = warp >> 2;
     const int64_t sbase = ((int64_t)seq * A + h) * S;
-    // D = rowsum(dO * O), L = lse * log2(e): 8 lanes per row, 4 rows per pass, 8 passes per warp
+    // D = rowsum(dO * O), L = lse * log2(e): 8 lanes per row, 4 rows per pass; all 16 loads of a thread
+    // are issued before the first is used
     {
       const int sub = lane >> 3, l8 = lane & 7;
+      uint4 ua[8], ub[8];
+#pragma unroll
+      for (int it = 0; it < 8; ++it) {
+        const int rr = min(warp * 32 + it * 4 + sub, S - 1);
+        const int64_t off = ((int64_t)seq * S + rr) * da + h * DH + l8 * 8;
+        ua[it] = __ldg(reinterpret_cast<const uint4 *>(d_o + off));
+        ub[it] = __ldg(reinterpret_cast<const uint4 *>(o + off));
+      }
+      const float lv = lane < 32 && warp * 32 + lane < S ? lse[sbase + warp * 32 + lane] * LOG2E : 0.f;
 #pragma unroll
       for (int it = 0; it < 8; ++it) {
         const int rr = warp * 32 + it * 4 + sub;
+        const __nv_bfloat162 *ha = reinterpret_cast<const __nv_bfloat162 *>(&ua[it]);
+        const __nv_bfloat162 *hb = reinterpret_cast<const __nv_bfloat162 *>(&ub[it]);
         float acc = 0.f;
-        if (rr < S) {
-          const int64_t off = ((int64_t)seq * S + rr) * da + h * DH + l8 * 8;
-          const uint4 ua = __ldg(reinterpret_cast<const uint4 *>(d_o + off));
-          const uint4 ub = __ldg(reinterpret_cast<const uint4 *>(o + off));
-          const __nv_bfloat162 *ha = reinterpret_cast<const __nv_bfloat162 *>(&ua);
-          const __nv_bfloat162 *hb = reinterpret_cast<const __nv_bfloat162 *>(&ub);
 #pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const float2 a = __bfloat1622float2(ha[e]), b = __bfloat1622float2(hb[e]);
-            acc += a.x * b.x + a.y * b.y;
-          }
+        for (int e = 0; e < 4; ++e) {
+          const float2 a = __bfloat1622float2(ha[e]), b = __bfloat1622float2(hb[e]);
+          acc += a.x * b.x + a.y * b.y;
         }
         acc += __shfl_xor_sync(0xffffffffu, acc, 1);
         acc += __shfl_xor_sync(0xffffffffu, acc, 2);
         acc += __shfl_xor_sync(0xffffffffu, acc, 4);
-        if (l8 == 0) {
-          Dsm[rr] = acc;
-          Lsm[rr] = rr < S ? lse[sbase + rr] * LOG2E : 0.f;
-        }
+        if (l8 == 0) Dsm[rr] = rr < S ? acc : 0.f;
       }
+      Lsm[warp * 32 + lane] = lv;
     }
     asm volatile("bar.sync 1, 256;" ::: "memory");
+    if (threadIdx.x == 0) stamp(16);
     const float sl2 = scale * LOG2E;
-    const uint32_t stg = sP + (uint32_t)chalf * TILE + (uint32_t)quad * 4096u;   // == this warp's rows of its P panel
     const int r_loc = quad * 32 + lane;                   // row within the 128-row block
+    const uint32_t t_lane = tmem + ((uint32_t)(quad * 32) << 16);
+    // 32 rows x 32 columns of a finished accumulator (this warp's lane quadrant) -> bf16 -> global
+    auto store_acc = [&](uint32_t col, float mul, bf16 *dst_row, bool ok) {
+      uint32_t rr[32];
+      tmem_ld32(t_lane + col, rr);
+      tmem_ld_wait();
+      if (ok) {
+        uint4 *dst = reinterpret_cast<uint4 *>(dst_row);
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+          dst[q] = make_uint4(pack2(__uint_as_float(rr[8 * q]) * mul, __uint_as_float(rr[8 * q + 1]) * mul),
+                              pack2(__uint_as_float(rr[8 * q + 2]) * mul, __uint_as_float(rr[8 * q + 3]) * mul),
+                              pack2(__uint_as_float(rr[8 * q + 4]) * mul, __uint_as_float(rr[8 * q + 5]) * mul),
+                              pack2(__uint_as_float(rr[8 * q + 6]) * mul, __uint_as_float(rr[8 * q + 7]) * mul));
+      }
+    };
+    // dV_j (warps 0-3) / dK_j (warps 4-7): this thread's key row, 64 columns
+    auto store_dvdk = [&](int j) {
+      const int key = j * 128 + r_loc;
+      bf16 *dst = dqkv + ((int64_t)seq * S + key) * (3 * da) + (chalf ? da : 2 * da) + h * DH;
+      store_acc((chalf ? C_DK : C_DV), chalf ? scale : 1.f, dst, key < S);
+      store_acc((chalf ? C_DK : C_DV) + 32, chalf ? scale : 1.f, dst + 32, key < S);
+    };
     int n = 0;
     for (int j = 0; j < nblk; ++j) {
       const int i_first = causal ? j : 0;
       for (int i = i_first; i < nblk; ++i, ++n) {
         const int row = i * 128 + r_loc;
-        const int key0 = j * 128 + chalf * 64;
-        // whole strip masked (causal, above the diagonal) ?
-        const bool dead = causal && i == j && chalf * 64 > quad * 32 + 31;
+        const int key0 = j * 128 + chalf * 64;             // first key of this thread's 64-column strip
+        // last key this row sees (-1: none)
+        const int kmax = row < S ? min(S - 1, causal ? row : S - 1) : -1;
+        // keys any row of this warp sees end before ...
+        const int kvis_w = causal ? min(S, i * 128 + quad * 32 + 32) : S;
         uint32_t ppk[32], dpk[32];
         mbar_wait(bar_sp, n & 1, 0x34);
         tcgen05_fence_after();
-        if (!dead) {
-          const float Lr = Lsm[row], Dr = Dsm[row];
-          const bool edge = (causal && i == j) || key0 + 64 > S || row >= S;
-          const uint32_t t_row = tmem + ((uint32_t)(quad * 32) << 16) + (uint32_t)(chalf * 64);
+        if (threadIdx.x == 0 && n < 4) stamp(17 + 3 * n);
+        const float Lr = Lsm[row], Dr = Dsm[row];
 #pragma unroll
-          for (int c = 0; c < 2; ++c) {
+        for (int c = 0; c < 2; ++c) {
+          const int kc = key0 + c * 32;
+          if (kc < kvis_w) {                               // warp-uniform
             uint32_t rs[32], rd[32];
-            tmem_ld32(t_row + C_S + c * 32, rs);
-            tmem_ld32(t_row + C_DP + c * 32, rd);
+            tmem_ld32(t_lane + C_S + chalf * 64 + c * 32, rs);
+            tmem_ld32(t_lane + C_DP + chalf * 64 + c * 32, rd);
             tmem_ld_wait();
+            const bool edge = kc + 31 > min(S - 1, causal ? i * 128 + quad * 32 : S - 1) || i * 128 + quad * 32 + 31 >= S;
 #pragma unroll
             for (int jj = 0; jj < 32; jj += 2) {
               float p0 = ex2(fmaf(__uint_as_float(rs[jj]), sl2, -Lr));
               float p1 = ex2(fmaf(__uint_as_float(rs[jj + 1]), sl2, -Lr));
               if (edge) {
-                const int k0 = key0 + c * 32 + jj;
-                if (row >= S || k0 >= S || (causal && k0 > row)) p0 = 0.f;
-                if (row >= S || k0 + 1 >= S || (causal && k0 + 1 > row)) p1 = 0.f;
+                p0 = kc + jj <= kmax ? p0 : 0.f;
+                p1 = kc + jj + 1 <= kmax ? p1 : 0.f;
               }
               ppk[c * 16 + (jj >> 1)] = pack2(p0, p1);
               dpk[c * 16 + (jj >> 1)] = pack2(p0 * (__uint_as_float(rd[jj]) - Dr), p1 * (__uint_as_float(rd[jj + 1]) - Dr));
             }
-          }
-        } else {
+          } else {
 #pragma unroll
-          for (int q = 0; q < 32; ++q) { ppk[q] = 0u; dpk[q] = 0u; }
+            for (int q = 0; q < 16; ++q) { ppk[c * 16 + q] = 0u; dpk[c * 16 + q] = 0u; }
+          }
         }
         tcgen05_fence_before();
         mbar_arrive(bar_tfree);                            // TMEM S / dP may be overwritten
-        if (n > 0) mbar_wait(bar_acc, (n - 1) & 1, 0x35);        // the MMAs that read the previous panels are done
-        if (lane == 0) bulk_wait_read<0>();                // ... and so is the TMA store staged in this warp's slab
-        __syncwarp();
+        if (threadIdx.x == 0 && n < 4) stamp(18 + 3 * n);
+        if (n > 0) {
+          mbar_wait(bar_acc, (n - 1) & 1, 0x35);           // the products that read the previous panels are done
+          tcgen05_fence_after();
+          // ... and with them, at the first pair of a new key block, dV / dK of the previous one
+          if (i == i_first) store_dvdk(j - 1);
+        }
         const uint32_t pp = sP + (uint32_t)chalf * TILE, dp = sdS + (uint32_t)chalf * TILE;
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
@@ -414,63 +471,22 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
           st_shared_v4(panel_addr(dp, r_loc, q), dpk[4 * q], dpk[4 * q + 1], dpk[4 * q + 2], dpk[4 * q + 3]);
         }
         fence_proxy_async_smem();
+        tcgen05_fence_before();                            // the dV / dK read-out precedes the next products
         mbar_arrive(bar_pds);
-        if (i == nblk - 1) {
-          // ---- dV_j (warps 0-3) / dK_j (warps 4-7) complete: TMEM -> bf16 -> staging -> TMA store ----
-          mbar_wait(bar_acc, n & 1, 0x36);
-          tcgen05_fence_after();
-          const uint32_t t_acc = tmem + ((uint32_t)(quad * 32) << 16) + (chalf ? C_DK : C_DV);
-          const float mul = chalf ? scale : 1.f;
-          if (lane == 0) bulk_wait_read<0>();
-          __syncwarp();
-#pragma unroll
-          for (int c = 0; c < 2; ++c) {
-            uint32_t rr[32];
-            tmem_ld32(t_acc + c * 32, rr);
-            tmem_ld_wait();
-#pragma unroll
-            for (int q = 0; q < 4; ++q)
-              st_shared_v4(panel_addr(stg, lane, c * 4 + q),
-                           pack2(__uint_as_float(rr[8 * q]) * mul, __uint_as_float(rr[8 * q + 1]) * mul),
-                           pack2(__uint_as_float(rr[8 * q + 2]) * mul, __uint_as_float(rr[8 * q + 3]) * mul),
-                           pack2(__uint_as_float(rr[8 * q + 4]) * mul, __uint_as_float(rr[8 * q + 5]) * mul),
-                           pack2(__uint_as_float(rr[8 * q + 6]) * mul, __uint_as_float(rr[8 * q + 7]) * mul));
-          }
-          fence_proxy_async_smem();
-          __syncwarp();
-          if (lane == 0) {
-            tma_store_3d(&map_dqkv, stg, (chalf ? da : 2 * da) + h * DH, j * 128 + quad * 32, seq);
-            bulk_commit();
-          }
-        }
+        if (threadIdx.x == 0 && n < 4) stamp(19 + 3 * n);
       }
     }
-    // ---- dQ: warps 0-3 -> block 0, warps 4-7 -> block 1 (every MMA has completed: last bar_acc) ----
+    // ---- tail: dV / dK of the last key block, then dQ (warps 0-3: block 0, warps 4-7: block 1) ----
+    mbar_wait(bar_acc, (n - 1) & 1, 0x36);
+    tcgen05_fence_after();
+    store_dvdk(nblk - 1);
     if (chalf < nblk) {
-      const uint32_t t_acc = tmem + ((uint32_t)(quad * 32) << 16) + C_DQ + 64 * chalf;
-      if (lane == 0) bulk_wait_read<0>();
-      __syncwarp();
-#pragma unroll
-      for (int c = 0; c < 2; ++c) {
-        uint32_t rr[32];
-        tmem_ld32(t_acc + c * 32, rr);
-        tmem_ld_wait();
-#pragma unroll
-        for (int q = 0; q < 4; ++q)
-          st_shared_v4(panel_addr(stg, lane, c * 4 + q),
-                       pack2(__uint_as_float(rr[8 * q]) * scale, __uint_as_float(rr[8 * q + 1]) * scale),
-                       pack2(__uint_as_float(rr[8 * q + 2]) * scale, __uint_as_float(rr[8 * q + 3]) * scale),
-                       pack2(__uint_as_float(rr[8 * q + 4]) * scale, __uint_as_float(rr[8 * q + 5]) * scale),
-                       pack2(__uint_as_float(rr[8 * q + 6]) * scale, __uint_as_float(rr[8 * q + 7]) * scale));
-      }
-      fence_proxy_async_smem();
-      __syncwarp();
-      if (lane == 0) {
-        tma_store_3d(&map_dqkv, stg, h * DH, chalf * 128 + quad * 32, seq);
-        bulk_commit();
-      }
+      const int qrow = chalf * 128 + r_loc;
+      bf16 *dst = dqkv + ((int64_t)seq * S + qrow) * (3 * da) + h * DH;
+      store_acc(C_DQ + 64 * chalf, scale, dst, qrow < S);
+      store_acc(C_DQ + 64 * chalf + 32, scale, dst + 32, qrow < S);
     }
-    if (lane == 0) bulk_wait_all();
+    if (threadIdx.x == 0) stamp(31);
   }
   tcgen05_fence_before();
   __syncthreads();
@@ -546,6 +562,13 @@ static bool get_map3(const void *ptr, int64_t width, int64_t S, int64_t n_seq, i
 
 }  // namespace fat
 
+static unsigned long long *g_attn_tl = nullptr;
+// Profiling hook: when set, every backward CTA writes 32 %globaltimer stamps to buf (control thread:
+// 0 start, 1 operands landed, 2+3n / 3+3n / 4+3n: pair n registers pulled / panels written / products
+// issued; compute thread 0: 16 D done, 17+3n / 18+3n / 19+3n: pair n S,dP ready / pulled / panels
+// written, 30 last store issued, 31 stores complete).  buf: 32 * n_seq * A uint64.
+void attn_tc_set_timeline(unsigned long long *buf) { g_attn_tl = buf; }
+
 cudaError_t attn_tc_set_watchdog(unsigned long long *mapped) {
   return cudaMemcpyToSymbol(tc::g_watchdog, &mapped, sizeof(mapped));
 }
@@ -558,8 +581,8 @@ bool attn_tc_supported(int dt, int S, int A, int dh) {
 cudaError_t attn_fwd_tc(const Ctx &c, const void *qkv, void *o, float *lse, int n_seq, int S, int A, int causal) {
   if (n_seq == 0) return cudaSuccess;
   const int da = A * fat::DH;
-  CUtensorMap mq, mo;
-  if (!fat::get_map3(qkv, 3 * da, S, n_seq, 128, &mq) || !fat::get_map3(o, da, S, n_seq, 32, &mo)) return cudaErrorInvalidValue;
+  CUtensorMap mq;
+  if (!fat::get_map3(qkv, 3 * da, S, n_seq, 128, &mq)) return cudaErrorInvalidValue;
   static bool attr_set = false;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(fat::attn_fwd_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fat::FWD_SMEM);
@@ -567,7 +590,8 @@ cudaError_t attn_fwd_tc(const Ctx &c, const void *qkv, void *o, float *lse, int 
     attr_set = true;
   }
   dim3 grid((S + 127) / 128, n_seq * A);
-  fat::attn_fwd_tc_kernel<<<grid, 128, fat::FWD_SMEM, c.stream>>>(mq, mo, lse, S, A, causal, 1.f / sqrtf((float)fat::DH));
+  fat::attn_fwd_tc_kernel<<<grid, fat::FWD_THREADS, fat::FWD_SMEM, c.stream>>>(mq, (bf16 *)o, lse, S, A, causal,
+                                                                              1.f / sqrtf((float)fat::DH));
   GP_LAUNCH_CHECK(c);
 }
 
@@ -575,10 +599,8 @@ cudaError_t attn_bwd_tc(const Ctx &c, const void *qkv, const void *o, const void
                         int n_seq, int S, int A, int causal) {
   if (n_seq == 0) return cudaSuccess;
   const int da = A * fat::DH;
-  CUtensorMap mq, md, mg;
-  if (!fat::get_map3(qkv, 3 * da, S, n_seq, 128, &mq) || !fat::get_map3(d_o, da, S, n_seq, 128, &md) ||
-      !fat::get_map3(dqkv, 3 * da, S, n_seq, 32, &mg))
-    return cudaErrorInvalidValue;
+  CUtensorMap mq, md;
+  if (!fat::get_map3(qkv, 3 * da, S, n_seq, 128, &mq) || !fat::get_map3(d_o, da, S, n_seq, 128, &md)) return cudaErrorInvalidValue;
   static bool attr_set = false;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(fat::attn_bwd_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fat::BWD_SMEM);
@@ -586,7 +608,7 @@ cudaError_t attn_bwd_tc(const Ctx &c, const void *qkv, const void *o, const void
     attr_set = true;
   }
   fat::attn_bwd_tc_kernel<<<n_seq * A, fat::BWD_THREADS, fat::BWD_SMEM, c.stream>>>(
-      mq, md, mg, (const bf16 *)o, (const bf16 *)d_o, lse, S, A, causal, 1.f / sqrtf((float)fat::DH));
+      mq, md, (const bf16 *)o, (const bf16 *)d_o, lse, (bf16 *)dqkv, S, A, causal, 1.f / sqrtf((float)fat::DH), g_attn_tl);
   GP_LAUNCH_CHECK(c);
 }
 

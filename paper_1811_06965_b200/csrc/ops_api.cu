@@ -12,6 +12,7 @@ namespace gp {
 cudaError_t gemm_simt(const Ctx &c, int dt, const GemmArgs &a);
 cudaError_t gemm_tc(const Ctx &c, const GemmArgs &a);
 void gemm_tc_set_timeline(unsigned long long *buf);
+void attn_tc_set_timeline(unsigned long long *buf);
 cudaError_t attn_fwd_simt(const Ctx &c, int dt, const void *qkv, void *o, float *lse, int n_seq,
                           int S, int A, int dh, int causal);
 cudaError_t attn_bwd_simt(const Ctx &c, int dt, const void *qkv, const void *o, const void *d_o,
@@ -138,6 +139,10 @@ int gpipe_op_ln_fwd(void *stream, int dtype, const float *x, const float *gamma,
                     int64_t n_tok, int d, float eps) {
   return ret(ln_fwd(mk(stream), dtype, x, gamma, beta, y, mean, rstd, resid_bias, resid_out, n_tok, d, eps),
              "gpipe_op_ln_fwd");
+}
+int gpipe_op_attn_timeline(void *dev_buf) {
+  attn_tc_set_timeline((unsigned long long *)dev_buf);
+  return GPIPE_OK;
 }
 int gpipe_op_gemm_timeline(void *dev_buf) {
   gemm_tc_set_timeline((unsigned long long *)dev_buf);

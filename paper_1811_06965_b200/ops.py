@@ -70,6 +70,11 @@ def gemm_timeline(buf):
     B._check(B.lib().gpipe_op_gemm_timeline(_p(buf)))
 
 
+def attn_timeline(buf):
+    """Profiling hook of the tcgen05 attention backward: buf = int64 CUDA tensor of 32 * n_seq * A elements (or None)."""
+    B._check(B.lib().gpipe_op_attn_timeline(_p(buf)))
+
+
 def gemm_workspace(M, N, K, device):
     """Zeroed split-K workspace for a [M,N,K] GEMM (None when the shape is not split)."""
     n = B.lib().gpipe_op_gemm_workspace_bytes(M, N, K)

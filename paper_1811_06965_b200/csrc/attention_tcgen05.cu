@@ -39,6 +39,7 @@ using namespace tc;
 constexpr int DH = 64;
 constexpr uint32_t TILE = 128 * 128;          // bytes of a [128 rows x 64 bf16] swizzled tile
 constexpr float LOG2E = 1.4426950408889634f;
+static unsigned long long *g_attn_tl = nullptr;     // host: timeline buffer handed to the next launches
 
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1, int c2) {
   asm volatile(
@@ -89,8 +90,17 @@ constexpr int FWD_THREADS = 256;
 
 __global__ void __launch_bounds__(FWD_THREADS, 2)
 attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict__ o, float *__restrict__ lse, int S,
-                   int A, int causal, float scale) {
+                   int A, int causal, float scale, unsigned long long *tl) {
   extern __shared__ uint8_t smem_raw[];
+  // optional timeline probe (attn_tc_set_timeline): 8 %globaltimer stamps per CTA, written by thread 0
+  auto stamp = [&](int slot) {
+    if (tl && threadIdx.x == 0) {
+      unsigned long long t;
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+      tl[((size_t)blockIdx.y * gridDim.x + blockIdx.x) * 8 + slot] = t;
+    }
+  };
+  stamp(0);
   __shared__ __align__(8) uint64_t bars[4];
   __shared__ uint32_t tmem_base_smem;
   __shared__ float xm[2][128], xl[2][128];
@@ -127,6 +137,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
     for (int b = 0; b < nkb; ++b) tma_load_3d(sV + b * TILE, &map_qkv, bar_v, 2 * da + h * DH, b * 128, seq);
     mbar_wait(bar_qk, 0, 0x21);
     tcgen05_fence_after();
+    stamp(1);
     const uint32_t id = idesc(0, 0, N);
 #pragma unroll
     for (int ks = 0; ks < DH / 16; ++ks) umma_bf16(tmem, desc_k(sQ, ks), desc_k(sK, ks), id, ks ? 1u : 0u);
@@ -147,6 +158,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
   auto edge = [&](int c) { return c * 32 + 32 > nk || (causal && c * 32 + 31 > q0 + quad * 32); };
   mbar_wait(bar_s, 0, 0x22);
   tcgen05_fence_after();
+  stamp(2);
   uint32_t ra[32], rb[32];
   float mx = -INFINITY;
   auto max_chunk = [&](const uint32_t *r, int c) {
@@ -172,6 +184,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
   xm[chalf][r_loc] = mx;
   if (c0 < cv) tmem_ld32(t_row + c0 * 32, ra);           // first chunk of the second pass: in flight over the barrier
   __syncthreads();
+  stamp(3);
   mx = fmaxf(xm[0][r_loc], xm[1][r_loc]);                // finite: key 0 is visible to every row
   const float ms = mx * sl2;
   float l = 0.f;
@@ -211,6 +224,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
   tcgen05_fence_before();
   __syncthreads();
 
+  stamp(4);
   if (threadIdx.x == 0) {
     tcgen05_fence_after();
     mbar_wait(bar_v, 0, 0x23);
@@ -223,6 +237,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
   l = xl[0][r_loc] + xl[1][r_loc];
   mbar_wait(bar_o, 0, 0x24);
   tcgen05_fence_after();
+  stamp(5);
   tmem_ld32(t_row + chalf * 32, ra);                      // this thread's 32 of the row's 64 output columns
   tmem_ld_wait();
   if (row < S) {
@@ -236,6 +251,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
                           pack2(__uint_as_float(ra[8 * q + 6]) * inv, __uint_as_float(ra[8 * q + 7]) * inv));
     if (chalf == 0) lse[((int64_t)seq * A + h) * S + row] = mx * scale + logf(l);
   }
+  stamp(6);
   tcgen05_fence_before();
   __syncthreads();
   if (warp == 1) {
@@ -562,12 +578,11 @@ static bool get_map3(const void *ptr, int64_t width, int64_t S, int64_t n_seq, i
 
 }  // namespace fat
 
-static unsigned long long *g_attn_tl = nullptr;
 // Profiling hook: when set, every backward CTA writes 32 %globaltimer stamps to buf (control thread:
 // 0 start, 1 operands landed, 2+3n / 3+3n / 4+3n: pair n registers pulled / panels written / products
 // issued; compute thread 0: 16 D done, 17+3n / 18+3n / 19+3n: pair n S,dP ready / pulled / panels
 // written, 30 last store issued, 31 stores complete).  buf: 32 * n_seq * A uint64.
-void attn_tc_set_timeline(unsigned long long *buf) { g_attn_tl = buf; }
+void attn_tc_set_timeline(unsigned long long *buf) { fat::g_attn_tl = buf; }
 
 cudaError_t attn_tc_set_watchdog(unsigned long long *mapped) {
   return cudaMemcpyToSymbol(tc::g_watchdog, &mapped, sizeof(mapped));
@@ -591,7 +606,7 @@ cudaError_t attn_fwd_tc(const Ctx &c, const void *qkv, void *o, float *lse, int 
   }
   dim3 grid((S + 127) / 128, n_seq * A);
   fat::attn_fwd_tc_kernel<<<grid, fat::FWD_THREADS, fat::FWD_SMEM, c.stream>>>(mq, (bf16 *)o, lse, S, A, causal,
-                                                                              1.f / sqrtf((float)fat::DH));
+                                                                              1.f / sqrtf((float)fat::DH), fat::g_attn_tl);
   GP_LAUNCH_CHECK(c);
 }
 
@@ -608,7 +623,7 @@ cudaError_t attn_bwd_tc(const Ctx &c, const void *qkv, const void *o, const void
     attr_set = true;
   }
   fat::attn_bwd_tc_kernel<<<n_seq * A, fat::BWD_THREADS, fat::BWD_SMEM, c.stream>>>(
-      mq, md, (const bf16 *)o, (const bf16 *)d_o, lse, (bf16 *)dqkv, S, A, causal, 1.f / sqrtf((float)fat::DH), g_attn_tl);
+      mq, md, (const bf16 *)o, (const bf16 *)d_o, lse, (bf16 *)dqkv, S, A, causal, 1.f / sqrtf((float)fat::DH), fat::g_attn_tl);
   GP_LAUNCH_CHECK(c);
 }
 

@@ -593,13 +593,16 @@ static bool get_map(const void *ptr, uint32_t esize, uint64_t inner, uint64_t ou
 }
 
 // Split-K when the output has too few 256 x 256 tiles to occupy the CTA pairs and K is long enough
-// that each split still runs a real main loop (>= 8 K-blocks).  All units run in ONE wave.
+// that each split still runs a long main loop (>= 192 K-blocks = 12288 deep): the split launch takes
+// the run-time-flag kernel and pays a workspace round trip, which only the very deep products
+// (dlogits W_out^T, K = V) win back - measured: K = 2048 20.5 us unsplit vs 43.6 us split, K = 6144
+// 37.1 vs 54.5, K = 16384 86.4 vs 84.7, K = 64000 296.6 vs 207.1.  All units run in ONE wave.
 static int splitk_factor(int tiles, int num_kb, int pairs) {
   static const int off = getenv("GPIPE_NO_SPLITK") ? atoi(getenv("GPIPE_NO_SPLITK")) : 0;
   if (off || tiles * 2 > pairs) return 1;
   int s = pairs / tiles;
   if (s > 4) s = 4;
-  while (s > 1 && num_kb / s < 8) --s;
+  while (s > 1 && num_kb / s < 192) --s;
   return s;
 }
 static size_t splitk_cnt_bytes(int tiles) { return (((size_t)tiles * 2 * 2 * sizeof(unsigned int)) + 1023) & ~(size_t)1023; }

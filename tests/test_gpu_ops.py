@@ -82,6 +82,29 @@ def test_gemm_tcgen05_all_layouts(transA, transB):
         assert maxrel(_np(C), ref) <= 2 ** -7 and cosine(_np(C), ref) >= 0.99999, (M, N, K)
 
 
+def test_gemm_tcgen05_split_k_deep():
+    """Few output tiles and a very deep K (the dlogits W_out^T shape class): the launch is split along K,
+    partials are reduced in split order, so two runs are bitwise equal and match the unsplit result."""
+    r = _rng(123)
+    M, N, K = 300, 256, 2 * 192 * 64 + 40                # 2 tiles, 385 K-blocks -> 2 splits, ragged tail
+    ws = ops.gemm_workspace(M, N, K, DEV)
+    assert ws is not None and ws.numel() > 0, "shape no longer split: pick a deeper K"
+    At, Aq = _lp(r.standard_normal((M, K)), "bf16")
+    Bt, Bq = _lp(r.standard_normal((N, K)), "bf16")
+    ref = Aq @ Bq.T
+    bias = torch.tensor(r.standard_normal(N).astype(np.float32), device=DEV)
+    C1 = torch.empty((M, N), device=DEV)
+    C2 = torch.empty((M, N), device=DEV)
+    C0 = torch.empty((M, N), device=DEV)
+    ops.gemm(At, Bt, C1, transB=True, bias=bias, workspace=ws, backend=2)
+    ops.gemm(At, Bt, C2, transB=True, bias=bias, workspace=ws, backend=2)      # counters reset themselves
+    ops.gemm(At, Bt, C0, transB=True, bias=bias, workspace=False, backend=2)   # never split
+    assert torch.equal(C1, C2)
+    assert maxrel(_np(C1), ref + _np(bias)[None, :]) <= 2e-5
+    assert maxrel(_np(C0), ref + _np(bias)[None, :]) <= 1e-4       # one 24 616-deep fp32 accumulation chain
+    assert maxrel(_np(C1), _np(C0)) <= 1e-4
+
+
 def test_gemm_tcgen05_bench_shapes_sampled():
     """The launch configurations bench.py times (T_mb = 2048 tokens, d = 1024): full-size GEMMs
     checked on sampled rows the oracle's matmul can compute one by one."""

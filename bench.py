@@ -258,7 +258,10 @@ def run_ours(args, w, rank, world, local_rank):
     roofline = {"bound": "tensor", "kernel": "gemm_tcgen05_kernel (fwd + dgrad + wgrad launches)",
                 "achieved": achieved, "peak": peaks["sustained"], "unit": "TFLOP/s",
                 "frac": achieved / peaks["sustained"], "peak_src": peaks["src"] + " sustained bf16 (kernel timed inside a long step)",
-                "traffic": None, "launches": int(sum(v["launches"] for v in gem.values())),
+                # DRAM read + write bytes of one FFN1-forward launch (the most frequent large shape), from the
+                # committed `ncu --set full` capture profiles/gemm_ffn1_fwd_r01.md; algorithmic bytes 109 MB
+                "traffic": 58.3e6, "traffic_src": "profiles/gemm_ffn1_fwd_r01.md (ffn1_fwd launch, dram read+write)",
+                "launches": int(sum(v["launches"] for v in gem.values())),
                 "share_of_kernel_time": gem_ms / tot_ms if tot_ms else None,
                 "per_class": {k: {"launches": int(v["launches"]), "ms": round(v["ms"], 3),
                                   "tflops": (v["flops"] / v["ms"] / 1e9) if v["ms"] > 0 and v["flops"] > 0 else None,

@@ -263,6 +263,34 @@ def test_attention_fwd_bwd(dtype, S, A, dh, causal, backend):
             assert cosine(got[:, blk * da:(blk + 1) * da], ref) >= (cos if dtype == "fp32" else 0.9999), name
 
 
+@pytest.mark.parametrize("causal", [0, 1])
+def test_attention_bench_shape_sampled(causal):
+    """The launch configuration bench.py times at config 5 (8 sequences x 32 heads, S 256, d_head 64: 512 forward
+    CTAs, 256 backward CTAs, more than one wave), checked on sampled (sequence, head) pairs the oracle
+    computes one by one."""
+    n_seq, S, A, dh = 8, 256, 32, 64
+    da = A * dh
+    r = _rng(4242 + causal)
+    qkvt, qkvq = _lp(r.standard_normal((n_seq * S, 3 * da)), "bf16")
+    dot, doq = _lp(r.standard_normal((n_seq * S, da)), "bf16")
+    o = torch.empty((n_seq * S, da), device=DEV, dtype=torch.bfloat16)
+    lse = torch.empty((n_seq, A, S), device=DEV)
+    dqkv = torch.empty_like(qkvt)
+    dvec = torch.empty((n_seq, A, S), device=DEV)
+    ops.attn_fwd(qkvt, o, lse, n_seq, S, A, dh, causal)
+    ops.attn_bwd(qkvt, o, dot, lse, dqkv, dvec, n_seq, S, A, dh, causal)
+    got_o, got_d = _np(o), _np(dqkv)
+    for (b, h) in [(0, 0), (0, 31), (3, 7), (4, 16), (7, 0), (7, 31)]:
+        rows, c = slice(b * S, (b + 1) * S), slice(h * dh, (h + 1) * dh)
+        q, k, v = qkvq[rows, :da][:, c], qkvq[rows, da:2 * da][:, c], qkvq[rows, 2 * da:][:, c]
+        o_ref, ps = go.attention_fwd(q, k, v, 1, dh, causal)
+        assert maxrel(got_o[rows, c], o_ref) <= 2 ** -6, (b, h)
+        dq, dk, dv = go.attention_bwd(doq[rows, c], q, k, v, ps, 1, dh)
+        for name, ref, blk in (("dq", dq, 0), ("dk", dk, 1), ("dv", dv, 2)):
+            g = got_d[rows, blk * da + h * dh: blk * da + (h + 1) * dh]
+            assert maxrel(g, ref) <= 2 ** -4 and cosine(g, ref) >= 0.9999, (name, b, h)
+
+
 # -------------------------------------------------------------------------------------------------
 # softmax cross-entropy, column sums, embedding, SGD
 # -------------------------------------------------------------------------------------------------

@@ -278,3 +278,54 @@ def test_bf16_invariance_over_M_and_remat():
         assert abs(loss - ref[0]) <= 1e-5 * abs(ref[0])
         for n in g:
             assert maxrel(g[n], ref[1][n]) <= 2e-3, (K, M, remat, n, maxrel(g[n], ref[1][n]))
+
+
+# -------------------------------------------------------------------------------------------------
+# full-size workloads, in the launch configuration bench.py times: properties that hold at any size
+# (the oracle cannot run 6 B parameters; its per-kernel and reduced-shape parity is above)
+# -------------------------------------------------------------------------------------------------
+def test_full_size_config5_properties():
+    """T(64,16384,32), K 16, M 16, remat on - the bench workload.  (i) loss at initialisation equals the closed
+    form P7 (ln V + sigma^2 d / 2: the logits of an untied N(0, sigma^2) head over a LayerNorm output are
+    N(0, sigma^2 d)); (ii) the step is deterministic and gpipe_step ACCUMULATES: a second step on the same
+    batch reproduces the loss bitwise and doubles every sampled gradient (to fp32 running-sum rounding); (iii) rows of dW_out sum to
+    ~0 over the vocabulary (softmax - onehot sums to zero per token: P8); (iv) peak HBM within 180 GB."""
+    w = gi.CONFIGS["T(64,16384,32)"]
+    tok, lab = gi.make_tokens(w, 2004)
+    sample = ["l0.w_qkv", "l63.b_1", "l64.w_o", "l127.ln2_g", "l127.b_2", "lnf_g"]
+    with _engine(w) as e:
+        e.init_params(seed=1004, std=0.02, parity=False)
+        assert e.peak_bytes()["total"] <= 180e9
+        loss1 = e.step(tok, lab)
+        assert abs(loss1 - (np.log(w.vocab) + 0.5 * 0.02 ** 2 * w.d_model)) < 0.05
+        g1 = {n: e.get_grad(n).copy() for n in sample}
+        gw = e.get_grad("w_out")
+        assert np.isfinite(gw).all() and np.abs(gw).max() > 0
+        # dlogits is stored in bf16 (2^-9 relative per entry), so the row sums cancel to that level
+        assert np.abs(gw.sum(axis=1)).max() <= 2 ** -7 * np.abs(gw).sum(axis=1).max()
+        loss2 = e.step(tok, lab)
+        assert loss2 == loss1
+        for n in sample:
+            g2 = e.get_grad(n)
+            assert np.isfinite(g2).all() and np.abs(g2).max() > 0, n
+            assert maxrel(g2, 2.0 * g1[n]) <= 1e-5, n          # same 16 addends again, fp32 running sum
+
+
+def test_full_size_config4_invariant_to_M():
+    """T(24,16384,32), K 8: M = 32 (T_mb 2048, the nominal split) against M = 16 (T_mb 4096) on the same batch
+    and device-drawn parameters - PAPER.md:67: the accumulated gradient is the mini-batch gradient whatever M
+    is.  Per-token forward values are bitwise independent of the split, so only the fp32 summation order of
+    the gradient sums differs."""
+    w = gi.CONFIGS["T(24,16384,32)"]
+    tok, lab = gi.make_tokens(w, 2003)
+    sample = ["l0.w_1", "l0.b_qkv", "l11.w_o", "l23.w_2", "l23.ln1_b", "lnf_b"]
+    res = []
+    for M in (32, 16):
+        with _engine(w, M=M) as e:
+            e.init_params(seed=1003, std=0.02, parity=True)
+            loss = e.step(tok, lab)
+            res.append((loss, {n: e.get_grad(n).copy() for n in sample}))
+    assert abs(res[0][0] - res[1][0]) <= 1e-5 * abs(res[0][0])
+    for n in sample:
+        assert maxrel(res[0][1][n], res[1][1][n]) <= 2e-3, (n, maxrel(res[0][1][n], res[1][1][n]))
+        assert cosine(res[0][1][n], res[1][1][n]) >= 0.99999, n

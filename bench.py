@@ -203,7 +203,7 @@ def run_ours(args, w, rank, world, local_rank):
     dev = torch.device("cuda", local_rank)
     peaks = measured_peaks()
     progress("library built and loaded; creating engine for %s" % w.name)
-    eng = gp.from_workload(w, device=dev)
+    eng = gp.from_workload(w, device=dev, partition=None if args.partition == "equal" else args.partition)
     eng.init_params(seed=1000 + rank, std=0.02, parity=False)
     progress("engine ready (%.1f GB arena)" % (eng.peak_bytes()["total"] / 1e9))
     tok, lab = gi.make_tokens(w, 2000 + rank)
@@ -272,7 +272,9 @@ def run_ours(args, w, rank, world, local_rank):
             "vs_baseline": None, "dtype": "bf16" if w.dtype == "bf16" else "f32", "data": "synthetic",
             "config": {"workload": w.name, "L": w.n_layers, "d_model": w.d_model, "d_ffn": w.d_ffn,
                        "n_heads": w.n_heads, "d_head": w.d_head, "vocab": w.vocab, "seq_len": w.seq_len,
-                       "n_seqs": w.n_seqs, "K": w.K, "M": w.M, "remat": w.remat, "parallelism": "replicas" if world > 1 else "1 GPU, K streams",
+                       "n_seqs": w.n_seqs, "K": w.K, "M": w.M, "remat": w.remat, "partition": args.partition,
+                       "layers_per_cell": [hi - lo for lo, hi in eng.cells],
+                       "parallelism": "replicas" if world > 1 else "1 GPU, K streams",
                        "l2": "inputs larger than L2 (activations+weights per step >> 126 MB)"},
             "loss": loss,
             "tflops_executed": fl["executed"] / step_s / 1e12, "tflops_model": fl["model"] / step_s / 1e12,
@@ -302,6 +304,8 @@ def main():
     ap.add_argument("--M", type=int, default=None)
     ap.add_argument("--K", type=int, default=None)
     ap.add_argument("--no-remat", action="store_true")
+    ap.add_argument("--partition", default="equal", choices=["equal", "cost"],
+                    help="equal: L/K consecutive layers per cell; cost: minimum variance of the estimated cell costs (PAPER.md:65)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))

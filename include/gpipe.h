@@ -113,6 +113,30 @@ int gpipe_create(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t 
                  const gpipe_env *env, gpipe_t **out);
 void gpipe_destroy(gpipe_t *g);
 
+/* ---- cell partitioning ("consecutive layers between layers i and j"; "the
+ * partitioning algorithm minimizes the variance in the estimated cost of all cells") ----
+ *
+ * gpipe_layer_costs: the per-token FLOP estimate c_i of every layer of `spec` (forward + backward, plus the replayed
+ * forward when remat != 0; SURVEY.md 8(d) formulas: causal layers count the unmasked half of the attention
+ * products), the cost the embedding adds to cell 0 (0: a gather) and the cost the head (final LayerNorm, logits,
+ * loss) adds to cell K-1.  Host only.  layer_cost_out: host [n_layers]; any out pointer may be NULL.
+ *
+ * gpipe_partition_min_variance: boundaries cell_lo_out[K+1] (host; cell k = layers [lo[k], lo[k+1]), lo[0] = 0,
+ * lo[K] = L, every cell non-empty) that minimise the variance of C_k = sum of layer_cost over the cell
+ * (+ first_extra for k = 0, + last_extra for k = K-1) over ALL consecutive partitions - exact (dynamic
+ * program); among equal minima the one with the earliest boundaries.  Needs 1 <= K <= L, costs >= 0. Host only.
+ *
+ * gpipe_create_partitioned: gpipe_create with explicit boundaries cell_lo[K+1] (host, read during the call).
+ * The arena need is the same as gpipe_plan_bytes reports (it does not depend on the boundaries).
+ * gpipe_cell_range: the layers [*lo, *hi) cell k of a handle runs. */
+int gpipe_layer_costs(const gpipe_layer_spec *spec, int remat, double *layer_cost_out, double *embed_cost,
+                      double *head_cost);
+int gpipe_partition_min_variance(const double *layer_cost, int L, double first_extra, double last_extra, int K,
+                                 int32_t *cell_lo_out);
+int gpipe_create_partitioned(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs,
+                             const gpipe_env *env, const int32_t *cell_lo, gpipe_t **out);
+int gpipe_cell_range(const gpipe_t *g, int k, int32_t *lo, int32_t *hi);
+
 /* N(0, std) for matrices and emb, from a counter-based generator on the device (Philox-4x32-10
  * + Box-Muller); parity != 0 also draws biases / beta ~ N(0,std) and gamma = 1 + N(0,std)
  * (reading A10), parity == 0 sets gamma = 1, beta = bias = 0.  bf16 mode: the master is the

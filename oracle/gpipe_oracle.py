@@ -203,10 +203,18 @@ class GPipeOracle:
     """gpipe_create / gpipe_step / gpipe_apply_sgd on the host (BASELINE.json north_star)."""
 
     def __init__(self, spec: Spec, K: int, M: int, remat: bool, dtype=np.float64,
-                 round_operands: bool = False):
+                 round_operands: bool = False, cell_lo=None):
         if K < 1 or K > max(spec.n_layers, 1) or M < 1:
             raise ValueError("need 1 <= K <= L and M >= 1")
         self.s, self.K, self.M, self.remat = spec, int(K), int(M), bool(remat)
+        # cells are ANY consecutive partition of the layers (PAPER.md:59); default: the equal split
+        if cell_lo is None:
+            self.cells = [cell_layers(spec.n_layers, self.K, k) for k in range(self.K)]
+        else:
+            if (len(cell_lo) != self.K + 1 or cell_lo[0] != 0 or cell_lo[-1] != spec.n_layers
+                    or any(cell_lo[k] >= cell_lo[k + 1] for k in range(self.K))):
+                raise ValueError("cell_lo must be K+1 strictly increasing boundaries from 0 to L")
+            self.cells = [range(cell_lo[k], cell_lo[k + 1]) for k in range(self.K)]
         self.dt = np.dtype(dtype).type
         self.rnd = bf16_rne if round_operands else (lambda a: a)
         self.names = [n for n, _ in tensor_list(spec)]
@@ -271,7 +279,7 @@ class GPipeOracle:
             x = p["emb"][tokens_mb.reshape(-1)] + np.tile(self.pe, (nb, 1))
         else:
             x = x_in
-        for l in cell_layers(s.n_layers, self.K, k):
+        for l in self.cells[k]:
             q_ = "l%d." % l
             a, xhat1, rstd1 = layernorm_fwd(x, p[q_ + "ln1_g"], p[q_ + "ln1_b"], s.ln_eps)
             a = r(a)

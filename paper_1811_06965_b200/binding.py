@@ -60,6 +60,13 @@ def lib() -> C.CDLL:
         "gpipe_plan_bytes": (i32, [C.POINTER(LayerSpec), i32, i32, i32, i64, C.POINTER(C.c_size_t)]),
         "gpipe_create": (i32, [C.POINTER(LayerSpec), i32, i32, i32, i64, C.POINTER(Env), C.POINTER(vp)]),
         "gpipe_destroy": (None, [vp]),
+        "gpipe_layer_costs": (i32, [C.POINTER(LayerSpec), i32, C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                    C.POINTER(C.c_double)]),
+        "gpipe_partition_min_variance": (i32, [C.POINTER(C.c_double), i32, C.c_double, C.c_double, i32,
+                                               C.POINTER(C.c_int32)]),
+        "gpipe_create_partitioned": (i32, [C.POINTER(LayerSpec), i32, i32, i32, i64, C.POINTER(Env),
+                                           C.POINTER(C.c_int32), C.POINTER(vp)]),
+        "gpipe_cell_range": (i32, [vp, i32, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]),
         "gpipe_init_params": (i32, [vp, C.c_uint64, f32, i32]),
         "gpipe_step": (i32, [vp, vp, vp, C.POINTER(f32)]),
         "gpipe_step_device": (i32, [vp, vp, vp, C.POINTER(f32)]),
@@ -105,7 +112,8 @@ def lib() -> C.CDLL:
 
 
 EXPORTED_SYMBOLS = [
-    "gpipe_plan_bytes", "gpipe_create", "gpipe_destroy", "gpipe_init_params", "gpipe_step",
+    "gpipe_plan_bytes", "gpipe_create", "gpipe_destroy", "gpipe_layer_costs", "gpipe_partition_min_variance",
+    "gpipe_create_partitioned", "gpipe_cell_range", "gpipe_init_params", "gpipe_step",
     "gpipe_step_device", "gpipe_apply_sgd", "gpipe_zero_grads", "gpipe_num_tensors",
     "gpipe_tensor_info", "gpipe_get_param", "gpipe_set_param", "gpipe_get_grad", "gpipe_peak_bytes",
     "gpipe_trace", "gpipe_launch_count", "gpipe_kernel_timing", "gpipe_kernel_stats", "gpipe_debug_read", "gpipe_last_error", "gpipe_version",
@@ -142,11 +150,31 @@ def plan_bytes(spec: LayerSpec, K: int, M: int, remat: bool, n_seqs: int) -> int
     return int(out.value)
 
 
+def layer_costs(spec: LayerSpec, remat: bool) -> Tuple[List[float], float, float]:
+    """gpipe_layer_costs: (per-layer costs, embedding cost, head cost); host-only."""
+    L = spec.n_layers
+    arr = (C.c_double * max(L, 1))()
+    emb, head = C.c_double(0), C.c_double(0)
+    _check(lib().gpipe_layer_costs(C.byref(spec), int(bool(remat)), arr, C.byref(emb), C.byref(head)))
+    return [arr[i] for i in range(L)], emb.value, head.value
+
+
+def partition_min_variance(costs, first_extra: float, last_extra: float, K: int) -> List[int]:
+    """gpipe_partition_min_variance: the K+1 cell boundaries; host-only."""
+    L = len(costs)
+    arr = (C.c_double * max(L, 1))(*[float(c) for c in costs])
+    out = (C.c_int32 * (K + 1))()
+    _check(lib().gpipe_partition_min_variance(arr, L, float(first_extra), float(last_extra), K, out))
+    return [out[i] for i in range(K + 1)]
+
+
 class GPipe:
-    """gpipe_create / gpipe_step / gpipe_apply_sgd (BASELINE.json north_star) on one B200."""
+    """gpipe_create / gpipe_step / gpipe_apply_sgd (BASELINE.json north_star) on one B200.
+    partition: None (equal consecutive split), "cost" (gpipe_layer_costs + gpipe_partition_min_variance,
+    PAPER.md:65) or an explicit list of K+1 boundaries."""
 
     def __init__(self, *, n_layers, d_model, d_ffn, n_heads, d_head, vocab, seq_len, dtype, K, M,
-                 remat=True, n_seqs, causal=None, ln_eps=1e-5, device="cuda:0"):
+                 remat=True, n_seqs, causal=None, ln_eps=1e-5, device="cuda:0", partition=None):
         import torch
         if not torch.cuda.is_available():
             raise GPipeError(-2, "no CUDA device: the GPipe path has no CPU fallback")
@@ -164,8 +192,23 @@ class GPipe:
             self._stream_arr = (C.c_void_p * K)(*[s.cuda_stream for s in self.streams])
             env = Env(base, nbytes, C.cast(self._stream_arr, C.POINTER(C.c_void_p)), K)
             torch.cuda.synchronize(self.device)
-            _check(lib().gpipe_create(C.byref(self.spec), K, M, int(self.remat), n_seqs, C.byref(env),
-                                      C.byref(self._h)))
+            if partition is None:
+                _check(lib().gpipe_create(C.byref(self.spec), K, M, int(self.remat), n_seqs, C.byref(env),
+                                          C.byref(self._h)))
+            else:
+                if isinstance(partition, str):
+                    if partition != "cost":
+                        raise ValueError("partition must be None, 'cost' or a list of K+1 boundaries")
+                    costs, c_emb, c_head = layer_costs(self.spec, self.remat)
+                    partition = partition_min_variance(costs, c_emb, c_head, K)
+                lo = (C.c_int32 * (K + 1))(*[int(v) for v in partition])
+                _check(lib().gpipe_create_partitioned(C.byref(self.spec), K, M, int(self.remat), n_seqs,
+                                                      C.byref(env), lo, C.byref(self._h)))
+        self.cells = []
+        for k in range(K):
+            lo_k, hi_k = C.c_int32(0), C.c_int32(0)
+            _check(lib().gpipe_cell_range(self._h, k, C.byref(lo_k), C.byref(hi_k)))
+            self.cells.append((lo_k.value, hi_k.value))
         self.names: List[str] = []
         self.shapes: Dict[str, Tuple[int, int]] = {}
         for i in range(lib().gpipe_num_tensors(self._h)):

@@ -5,6 +5,7 @@
 
 #include <new>
 #include <string>
+#include <vector>
 
 #include "engine.h"
 
@@ -38,7 +39,8 @@ static int env_int(const char *name, int dflt) {
 }
 
 // fills the shape fields of an Engine from the spec; no CUDA calls
-static int configure(Engine &e, const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs) {
+static int configure(Engine &e, const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs,
+                     const int32_t *cell_lo = nullptr) {
   if (!spec) return fail(GPIPE_EINVAL, "spec is NULL");
   e.spec = *spec;
   e.dt = spec->dtype;
@@ -67,6 +69,14 @@ static int configure(Engine &e, const gpipe_layer_spec *spec, int K, int M, int 
     e.cell_lo[k] = k * base + (k < extra ? k : extra);
     e.cell_hi[k] = e.cell_lo[k] + base + (k < extra ? 1 : 0);
   }
+  if (cell_lo) {                            // explicit consecutive partition: lo[0] = 0 < ... < lo[K] = L
+    if (cell_lo[0] != 0 || cell_lo[K] != L) return fail(GPIPE_EINVAL, "cell_lo[0] must be 0 and cell_lo[K] must be L");
+    for (int k = 0; k < K; ++k) {
+      if (L > 0 && cell_lo[k + 1] <= cell_lo[k]) return fail(GPIPE_EINVAL, "cell_lo must be strictly increasing (no empty cell)");
+      e.cell_lo[k] = cell_lo[k];
+      e.cell_hi[k] = cell_lo[k + 1];
+    }
+  }
   e.gemm_backend = env_int("GPIPE_GEMM_SIMT", 0);
   e.replay_full = env_int("GPIPE_REPLAY_FULL", 0);
   std::string err;
@@ -91,14 +101,85 @@ int gpipe_plan_bytes(const gpipe_layer_spec *spec, int K, int M, int remat, int6
   return GPIPE_OK;
 }
 
+static int create_impl(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs, const gpipe_env *env,
+                       const int32_t *cell_lo, gpipe_t **out);
 int gpipe_create(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs, const gpipe_env *env, gpipe_t **out) {
+  return create_impl(spec, K, M, remat, n_seqs, env, nullptr, out);
+}
+int gpipe_create_partitioned(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs, const gpipe_env *env,
+                             const int32_t *cell_lo, gpipe_t **out) {
+  if (!cell_lo) return fail(GPIPE_EINVAL, "cell_lo is NULL");
+  return create_impl(spec, K, M, remat, n_seqs, env, cell_lo, out);
+}
+int gpipe_cell_range(const gpipe_t *g, int k, int32_t *lo, int32_t *hi) {
+  if (!g || k < 0 || k >= g->e.K) return fail(GPIPE_EINVAL, "handle is NULL or cell index out of range");
+  if (lo) *lo = g->e.cell_lo[k];
+  if (hi) *hi = g->e.cell_hi[k];
+  return GPIPE_OK;
+}
+
+// Cost model per token: F_g = 2 (4 d d_a + 2 d H), F_a = 4 S d_a (x (S+1)/2S when causal),
+// F_v = 2 d V; a layer costs forward + backward (2 F_g + 2.5 F_a) + replay (forward again) when remat is on.
+int gpipe_layer_costs(const gpipe_layer_spec *spec, int remat, double *layer_cost_out, double *embed_cost, double *head_cost) {
+  Engine e;
+  int rc = configure(e, spec, 1, 1, remat, 1);
+  if (rc) return rc;
+  const double d = e.d, da = e.da, H = e.H, S = e.S, V = e.V;
+  const double Fg = 2.0 * (4.0 * d * da + 2.0 * d * H), Fv = 2.0 * d * V;
+  const double passes_g = 3.0 + (remat ? 1.0 : 0.0), passes_a = 3.5 + (remat ? 1.0 : 0.0);
+  for (int l = 0; l < spec->n_layers; ++l) {
+    const double Fa = 4.0 * S * da * (e.causal[l] ? (S + 1.0) / (2.0 * S) : 1.0);
+    if (layer_cost_out) layer_cost_out[l] = passes_g * Fg + passes_a * Fa;
+  }
+  if (embed_cost) *embed_cost = 0.0;                       // a gather: no FLOPs
+  if (head_cost) *head_cost = passes_g * Fv;
+  return GPIPE_OK;
+}
+
+// "the partitioning algorithm minimizes the variance in the estimated cost of all cells".
+// The mean of the K cell costs is fixed by the total, so minimum variance = minimum sum of squares; consecutive
+// cells make that an exact dynamic program: best[k][j] = min over i of best[k-1][i] + C(i, j)^2.  O(K L^2).
+int gpipe_partition_min_variance(const double *layer_cost, int L, double first_extra, double last_extra, int K,
+                                 int32_t *cell_lo_out) {
+  if (!layer_cost || !cell_lo_out) return fail(GPIPE_EINVAL, "layer_cost and cell_lo_out are required");
+  if (L < 1 || K < 1 || K > L) return fail(GPIPE_EINVAL, "need 1 <= K <= L");
+  for (int l = 0; l < L; ++l)
+    if (!(layer_cost[l] >= 0.0)) return fail(GPIPE_EINVAL, "layer costs must be >= 0");
+  if (!(first_extra >= 0.0) || !(last_extra >= 0.0)) return fail(GPIPE_EINVAL, "extra costs must be >= 0");
+  std::vector<double> pre(L + 1, 0.0);
+  for (int l = 0; l < L; ++l) pre[l + 1] = pre[l] + layer_cost[l];
+  auto cost = [&](int k, int i, int j) {                   // cell k = layers [i, j)
+    double c = pre[j] - pre[i];
+    if (k == 0) c += first_extra;
+    if (k == K - 1) c += last_extra;
+    return c * c;
+  };
+  const double INF = 1e300;
+  std::vector<std::vector<double>> best(K, std::vector<double>(L + 1, INF));
+  std::vector<std::vector<int>> arg(K, std::vector<int>(L + 1, -1));
+  for (int j = 1; j <= L - (K - 1); ++j) { best[0][j] = cost(0, 0, j); arg[0][j] = 0; }
+  for (int k = 1; k < K; ++k)
+    for (int j = k + 1; j <= L - (K - 1 - k); ++j)
+      for (int i = k; i < j; ++i) {                        // ascending i, strict <: ties keep the earliest boundary
+        if (best[k - 1][i] >= INF) continue;
+        double v = best[k - 1][i] + cost(k, i, j);
+        if (v < best[k][j]) { best[k][j] = v; arg[k][j] = i; }
+      }
+  int j = L;
+  cell_lo_out[K] = L;
+  for (int k = K - 1; k >= 0; --k) { j = arg[k][j]; cell_lo_out[k] = j; }
+  return GPIPE_OK;
+}
+
+static int create_impl(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs, const gpipe_env *env,
+                       const int32_t *cell_lo, gpipe_t **out) {
   if (!out) return fail(GPIPE_EINVAL, "out is NULL");
   *out = nullptr;
   if (!env || !env->arena || !env->streams) return fail(GPIPE_EINVAL, "env, env->arena and env->streams are required");
   gpipe *g = new (std::nothrow) gpipe();
   if (!g) return fail(GPIPE_ENOMEM, "host allocation failed");
   Engine &e = g->e;
-  int rc = configure(e, spec, K, M, remat, n_seqs);
+  int rc = configure(e, spec, K, M, remat, n_seqs, cell_lo);
   if (rc) { delete g; return rc; }
   if (env->n_streams < K) { delete g; return fail(GPIPE_EINVAL, "need one stream per cell (n_streams >= K)"); }
   if ((uintptr_t)env->arena % 1024) { delete g; return fail(GPIPE_EINVAL, "arena must be 1024-byte aligned"); }

@@ -329,3 +329,53 @@ def test_full_size_config4_invariant_to_M():
     for n in sample:
         assert maxrel(res[0][1][n], res[1][1][n]) <= 2e-3, (n, maxrel(res[0][1][n], res[1][1][n]))
         assert cosine(res[0][1][n], res[1][1][n]) >= 0.99999, n
+
+
+# -------------------------------------------------------------------------------------------------
+# cell partitioning
+# -------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cell_lo", [[0, 1, 4, 5], [0, 3, 4, 5], [0, 2, 3, 5]])
+def test_fp32_parity_explicit_partition(cell_lo):
+    w = _tiny().replace(n_layers=5, causal=(1, 0, 1, 0, 1), K=3)
+    params = gi.make_params(w, 1001, round_bf16=False)
+    tok, lab = gi.make_tokens(w, 2001)
+    o, loss_ref = run_oracle(w, params, tok, lab, cell_lo=cell_lo)
+    with _engine(w, partition=cell_lo) as e:
+        assert e.cells == [(cell_lo[k], cell_lo[k + 1]) for k in range(3)]
+        e.set_params(params)
+        loss = e.step(tok, lab)
+        assert abs(loss - loss_ref) <= FP32_TOL * abs(loss_ref)
+        for n in e.names:
+            assert maxrel(e.get_grad(n), o.g[n]) <= FP32_TOL, n
+        e.trace(True)
+        e.zero_grads()
+        e.step(tok, lab)
+        ev = e.trace_events()
+    assert sorted({k for (_, k, _, _, _, _) in ev}) == [0, 1, 2]
+
+
+def test_bf16_cost_partition_changes_nothing_but_the_cut():
+    """partition="cost": the head's cost shortens the last cell; per-token values do not depend on where the
+    cuts are, so loss and every gradient are bitwise those of the equal split."""
+    w = gi.CONFIGS["T(6,4096,16)"].replace(name="bf16-part", n_layers=6, d_model=256, d_ffn=512, n_heads=4, d_head=64,
+                                           vocab=4096, seq_len=64, n_seqs=8, M=4, K=2, causal=(0, 1, 0, 1, 0, 1))
+    params = gi.make_params(w, 1005)
+    tok, lab = gi.make_tokens(w, 2005)
+    out = []
+    for part in (None, "cost", [0, 1, 6]):
+        with _engine(w, partition=part) as e:
+            e.set_params(params)
+            out.append((e.cells, e.step(tok, lab), e.grads(), e.peak_bytes()["total"]))
+    assert out[0][0] == [(0, 3), (3, 6)]
+    assert out[1][0][1][1] - out[1][0][1][0] < 3                      # the head costs more than a layer here
+    for cells, loss, g, peak in out[1:]:
+        assert loss == out[0][1] and peak == out[0][3]
+        for n in g:
+            assert np.array_equal(g[n], out[0][2][n]), (cells, n)
+
+
+def test_partition_error_paths():
+    w = _tiny().replace(n_layers=4, causal=(1, 1, 1, 1), K=2)
+    for bad in ([0, 0, 4], [0, 4, 4], [1, 2, 4], [0, 2, 5], [0, 3, 2]):
+        with pytest.raises(gp.GPipeError):
+            _engine(w, partition=bad)

@@ -207,6 +207,29 @@ def test_p4_gradients_independent_of_K_and_M_fp32():
                 assert _maxrel(o.g[n].astype(np.float64), ref.g[n].astype(np.float64)) <= 1e-5, (K, M, n)
 
 
+def test_p4_gradients_independent_of_the_partition():
+    """a cell is ANY run of consecutive layers; the gradient is that of the whole sequence of layers
+    whatever the cut points are (explicit boundaries vs the equal split vs one cell)."""
+    w = _tiny().replace(n_layers=5, causal=(1, 0, 1, 0, 1))
+    params = gi.make_params(w, 1001, round_bf16=False)
+    tok, lab = gi.make_tokens(w, 2001)
+    spec = go.Spec(w.n_layers, w.d_model, w.d_ffn, w.n_heads, w.d_head, w.vocab, w.seq_len, w.causal, w.ln_eps)
+    res = []
+    for K, cell_lo in [(1, None), (3, None), (3, [0, 1, 4, 5]), (3, [0, 3, 4, 5]), (5, [0, 1, 2, 3, 4, 5])]:
+        o = go.GPipeOracle(spec, K, 4, True, cell_lo=cell_lo)
+        o.set_params(params)
+        res.append((o.step(tok, lab), o))
+        assert [len(c) for c in o.cells] == ([b - a for a, b in zip(cell_lo, cell_lo[1:])] if cell_lo else
+                                             [len(go.cell_layers(5, K, k)) for k in range(K)])
+    for l, o in res[1:]:
+        assert abs(l - res[0][0]) <= 1e-12 * abs(res[0][0])
+        for n in o.names:
+            assert _maxrel(o.g[n], res[0][1].g[n]) <= 1e-10, n
+    for bad in ([0, 2, 5], [0, 0, 3, 5], [1, 2, 3, 5], [0, 2, 4, 6], [0, 4, 3, 5]):
+        with pytest.raises(ValueError):
+            go.GPipeOracle(spec, 3, 4, True, cell_lo=bad)
+
+
 def test_p5_remat_equals_stored_bitwise():
     """recomputing F_k from the boundary activation gives the same gradients."""
     w = _tiny((0, 1))

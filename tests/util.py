@@ -20,9 +20,10 @@ def oracle_spec(w):
     return go.Spec(w.n_layers, w.d_model, w.d_ffn, w.n_heads, w.d_head, w.vocab, w.seq_len, w.causal, w.ln_eps)
 
 
-def run_oracle(w, params, tok, lab, K=None, M=None, remat=None, dtype=np.float64, round_operands=False):
+def run_oracle(w, params, tok, lab, K=None, M=None, remat=None, dtype=np.float64, round_operands=False, cell_lo=None):
     o = go.GPipeOracle(oracle_spec(w), w.K if K is None else K, w.M if M is None else M,
-                       w.remat if remat is None else remat, dtype=dtype, round_operands=round_operands)
+                       w.remat if remat is None else remat, dtype=dtype, round_operands=round_operands,
+                       cell_lo=cell_lo)
     o.set_params(params)
     loss = o.step(tok, lab)
     return o, loss

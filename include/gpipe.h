@@ -158,6 +158,17 @@ int gpipe_step_device(gpipe_t *g, const int32_t *tokens_dev, const int32_t *labe
 int gpipe_apply_sgd(gpipe_t *g, float lr);
 int gpipe_zero_grads(gpipe_t *g);
 
+/* RMSProp, the optimizer the paper's memory table assumes ("Each model parameter needs 12 bytes since we applied
+ * RMSProp": weight + gradient + one slot).  The slot is caller-owned DEVICE memory
+ * (the library never allocates): gpipe_optimizer_slot_bytes() bytes, 16-byte aligned, handed over once with
+ * gpipe_attach_optimizer_slots (zeroed there; must outlive the handle).  gpipe_apply_rmsprop, once per mini-batch:
+ *   ms <- rho * ms + (1 - rho) * g^2;   w <- w - lr * g / (sqrt(ms) + eps);   g <- 0        (reading A20)
+ * bf16 mode updates the fp32 master and re-rounds the bf16 working copy.  0 <= rho < 1, eps > 0 (a parameter
+ * whose gradient is exactly zero then stays put: 0 / (0 + eps)). */
+int gpipe_optimizer_slot_bytes(const gpipe_t *g, size_t *bytes_out);
+int gpipe_attach_optimizer_slots(gpipe_t *g, void *slots_dev, size_t bytes);
+int gpipe_apply_rmsprop(gpipe_t *g, float lr, float rho, float eps);
+
 int gpipe_num_tensors(const gpipe_t *g);
 /* *name points into library-owned storage valid until gpipe_destroy. */
 int gpipe_tensor_info(const gpipe_t *g, int i, const char **name, int64_t *rows, int64_t *cols);

@@ -100,6 +100,9 @@ int gpipe_op_embed_fwd(void *stream, int dtype, const int32_t *tok, const void *
 int gpipe_op_embed_bwd(void *stream, const int32_t *tok, const float *dx, float *gemb, int64_t n_tok, int d);
 int gpipe_op_positional(void *stream, float *pe, int S, int d);
 /* master -= lr*grad; w_lp = RNE(master) (bf16 mode, may be NULL); grad = 0.  n multiple of 4. */
+/* ms = rho*ms + (1-rho)*grad^2; master -= lr*grad/(sqrt(ms)+eps); w_lp = RNE(master) (may be NULL); grad = 0. */
+int gpipe_op_rmsprop(void *stream, int dtype, float *master, float *grad, float *ms, void *w_lp, int64_t n, float lr,
+                     float rho, float eps);
 int gpipe_op_sgd(void *stream, int dtype, float *master, float *grad, void *w_lp, int64_t n, float lr);
 
 #if defined(__GNUC__)

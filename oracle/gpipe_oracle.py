@@ -245,6 +245,18 @@ class GPipeOracle:
             self.p[n] = self.p[n] - lr * self.g[n]
         self.zero_grads()
 
+    def apply_rmsprop(self, lr: float, rho: float = 0.9, eps: float = 1e-8):
+        """RMSProp, the optimizer of the paper's memory table (12 bytes per parameter = weight +
+        gradient + one slot).  The paper does not spell the update out; reading A20: the slot starts
+        at 0, ms <- rho ms + (1 - rho) g^2, w <- w - lr g / (sqrt(ms) + eps), then g <- 0."""
+        if not hasattr(self, "ms"):
+            self.ms = {n: np.zeros(sh, self.dt) for n, sh in self.shapes.items()}
+        lr, rho, eps = self.dt(lr), self.dt(rho), self.dt(eps)
+        for n in self.names:
+            self.ms[n] = rho * self.ms[n] + (self.dt(1) - rho) * self.g[n] * self.g[n]
+            self.p[n] = self.p[n] - lr * self.g[n] / (np.sqrt(self.ms[n]) + eps)
+        self.zero_grads()
+
     # -- activation-memory accounting (PAPER.md:87) -------------------------------------
     def _hold(self, n_elems):
         self._live_act += n_elems

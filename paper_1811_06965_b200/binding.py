@@ -71,6 +71,9 @@ def lib() -> C.CDLL:
         "gpipe_step": (i32, [vp, vp, vp, C.POINTER(f32)]),
         "gpipe_step_device": (i32, [vp, vp, vp, C.POINTER(f32)]),
         "gpipe_apply_sgd": (i32, [vp, f32]),
+        "gpipe_optimizer_slot_bytes": (i32, [vp, C.POINTER(C.c_size_t)]),
+        "gpipe_attach_optimizer_slots": (i32, [vp, vp, C.c_size_t]),
+        "gpipe_apply_rmsprop": (i32, [vp, f32, f32, f32]),
         "gpipe_zero_grads": (i32, [vp]),
         "gpipe_num_tensors": (i32, [vp]),
         "gpipe_tensor_info": (i32, [vp, i32, C.POINTER(C.c_char_p), C.POINTER(i64), C.POINTER(i64)]),
@@ -102,6 +105,7 @@ def lib() -> C.CDLL:
         "gpipe_op_embed_bwd": (i32, [vp, vp, vp, vp, i64, i32]),
         "gpipe_op_positional": (i32, [vp, vp, i32, i32]),
         "gpipe_op_sgd": (i32, [vp, i32, vp, vp, vp, i64, f32]),
+        "gpipe_op_rmsprop": (i32, [vp, i32, vp, vp, vp, vp, i64, f32, f32, f32]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -114,7 +118,8 @@ def lib() -> C.CDLL:
 EXPORTED_SYMBOLS = [
     "gpipe_plan_bytes", "gpipe_create", "gpipe_destroy", "gpipe_layer_costs", "gpipe_partition_min_variance",
     "gpipe_create_partitioned", "gpipe_cell_range", "gpipe_init_params", "gpipe_step",
-    "gpipe_step_device", "gpipe_apply_sgd", "gpipe_zero_grads", "gpipe_num_tensors",
+    "gpipe_step_device", "gpipe_apply_sgd", "gpipe_optimizer_slot_bytes", "gpipe_attach_optimizer_slots",
+    "gpipe_apply_rmsprop", "gpipe_op_rmsprop", "gpipe_zero_grads", "gpipe_num_tensors",
     "gpipe_tensor_info", "gpipe_get_param", "gpipe_set_param", "gpipe_get_grad", "gpipe_peak_bytes",
     "gpipe_trace", "gpipe_launch_count", "gpipe_kernel_timing", "gpipe_kernel_stats", "gpipe_debug_read", "gpipe_last_error", "gpipe_version",
     "gpipe_op_gemm", "gpipe_op_gemm_workspace_bytes", "gpipe_op_gemm_timeline", "gpipe_op_attn_timeline", "gpipe_op_ln_fwd", "gpipe_op_ln_bwd_scratch_floats", "gpipe_op_ln_bwd",
@@ -224,6 +229,7 @@ class GPipe:
             lib().gpipe_destroy(self._h)
             self._h = C.c_void_p(None)
         self.arena = None
+        self._slots = None
 
     def __del__(self):
         try:
@@ -263,6 +269,16 @@ class GPipe:
                     raise ValueError("tokens/labels must be [n_seqs, seq_len]")
                 _check(lib().gpipe_step(self._h, t.ctypes.data, l.ctypes.data, C.byref(loss)))
         return float(loss.value)
+
+    def apply_rmsprop(self, lr: float, rho: float = 0.9, eps: float = 1e-8):
+        """RMSProp; the fp32 slot (4 B / parameter) is allocated on first use."""
+        with self._torch.cuda.device(self.device):
+            if getattr(self, "_slots", None) is None:
+                n = C.c_size_t(0)
+                _check(lib().gpipe_optimizer_slot_bytes(self._h, C.byref(n)))
+                self._slots = self._torch.empty(n.value, dtype=self._torch.uint8, device=self.device)
+                _check(lib().gpipe_attach_optimizer_slots(self._h, self._slots.data_ptr(), n.value))
+            _check(lib().gpipe_apply_rmsprop(self._h, lr, rho, eps))
 
     def apply_sgd(self, lr: float):
         with self._torch.cuda.device(self.device):

@@ -314,6 +314,35 @@ int gpipe_apply_sgd(gpipe_t *g, float lr) {
   return GPIPE_OK;
 }
 
+int gpipe_optimizer_slot_bytes(const gpipe_t *g, size_t *bytes_out) {
+  if (!g || !bytes_out) return fail(GPIPE_EINVAL, "handle and bytes_out are required");
+  *bytes_out = (size_t)g->e.n_flat * sizeof(float);
+  return GPIPE_OK;
+}
+
+int gpipe_attach_optimizer_slots(gpipe_t *g, void *slots_dev, size_t bytes) {
+  if (!g || !slots_dev) return fail(GPIPE_EINVAL, "handle and slots_dev are required");
+  Engine &e = g->e;
+  if (bytes < (size_t)e.n_flat * sizeof(float)) return fail(GPIPE_ENOMEM, "optimizer slots too small: need " + std::to_string((size_t)e.n_flat * 4) + " bytes");
+  if ((uintptr_t)slots_dev % 16) return fail(GPIPE_EINVAL, "optimizer slots must be 16-byte aligned");
+  API_CUDA(cudaMemsetAsync(slots_dev, 0, (size_t)e.n_flat * sizeof(float), e.streams[0]), "gpipe_attach_optimizer_slots");
+  API_CUDA(cudaStreamSynchronize(e.streams[0]), "gpipe_attach_optimizer_slots");
+  e.opt_ms = (float *)slots_dev;
+  return GPIPE_OK;
+}
+
+int gpipe_apply_rmsprop(gpipe_t *g, float lr, float rho, float eps) {
+  if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
+  Engine &e = g->e;
+  if (!e.opt_ms) return fail(GPIPE_EINVAL, "call gpipe_attach_optimizer_slots first");
+  if (!(rho >= 0.f && rho < 1.f) || !(eps > 0.f)) return fail(GPIPE_EINVAL, "need 0 <= rho < 1 and eps > 0");
+  Ctx c = e.ctx(0);
+  API_CUDA(rmsprop_apply(c, e.dt, e.master, e.grad, e.opt_ms, e.dt == GP_BF16 ? e.w_lp : nullptr, e.n_flat, lr, rho, eps),
+           "gpipe_apply_rmsprop");
+  API_CUDA(cudaStreamSynchronize(c.stream), "gpipe_apply_rmsprop");
+  return GPIPE_OK;
+}
+
 int gpipe_zero_grads(gpipe_t *g) {
   if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
   Engine &e = g->e;

@@ -115,6 +115,7 @@ struct Engine {
   int serial = 0;                                      // debug/profiling: every cell on stream 0
   cudaStream_t st(int k) const { return streams[serial ? 0 : k]; }
   std::vector<KRec> krecs;
+  float *opt_ms = nullptr;           // RMSProp second-moment slot (caller-supplied device memory, n_flat floats)
   KStat kstats[KC_NUM];
   cudaError_t resolve_kernel_timing();
   template <typename F>

@@ -193,6 +193,41 @@ cudaError_t sgd_apply(const Ctx &c, int dt, float *master, float *grad, void *w_
 }
 
 // ---------------------------------------------------------------------------------------------
+// RMSProp apply ("12 bytes [per parameter] since we applied RMSProp": weight +
+// gradient + one fp32 slot).  ms = rho*ms + (1-rho)*g^2; master -= lr * g / (sqrt(ms) + eps); working copy =
+// RNE(master); g = 0 (reading A20).  One pass: 26 B / parameter in bf16 mode (g r+w, ms r+w, master r+w, lp w).
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256)
+rmsprop_kernel(float *__restrict__ master, float *__restrict__ grad, float *__restrict__ ms, T *__restrict__ w_lp,
+               int64_t n4, float lr, float rho, float eps) {
+  const float om = 1.f - rho;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    float4 m = load4(master + 4 * i), g = load4(grad + 4 * i), v = load4(ms + 4 * i);
+    v.x = rho * v.x + om * g.x * g.x; v.y = rho * v.y + om * g.y * g.y;
+    v.z = rho * v.z + om * g.z * g.z; v.w = rho * v.w + om * g.w * g.w;
+    m.x -= lr * g.x / (sqrtf(v.x) + eps); m.y -= lr * g.y / (sqrtf(v.y) + eps);
+    m.z -= lr * g.z / (sqrtf(v.z) + eps); m.w -= lr * g.w / (sqrtf(v.w) + eps);
+    store4(ms + 4 * i, v);
+    store4(master + 4 * i, m);
+    if (w_lp) store4(w_lp + 4 * i, m);
+    store4(grad + 4 * i, make_float4(0.f, 0.f, 0.f, 0.f));
+  }
+}
+
+cudaError_t rmsprop_apply(const Ctx &c, int dt, float *master, float *grad, float *ms, void *w_lp, int64_t n,
+                          float lr, float rho, float eps) {
+  if (n == 0) return cudaSuccess;
+  int64_t n4 = n / 4;
+  int64_t want = (n4 + 255) / 256;
+  unsigned grid = (unsigned)(want < (int64_t)c.sm_count * 16 ? want : (int64_t)c.sm_count * 16);
+  if (dt == GP_BF16) rmsprop_kernel<bf16><<<grid, 256, 0, c.stream>>>(master, grad, ms, (bf16 *)w_lp, n4, lr, rho, eps);
+  else rmsprop_kernel<float><<<grid, 256, 0, c.stream>>>(master, grad, ms, (float *)nullptr, n4, lr, rho, eps);
+  GP_LAUNCH_CHECK(c);
+}
+
+// ---------------------------------------------------------------------------------------------
 // Philox-4x32-10 counter RNG + Box-Muller; element i uses counter (i/4, stream_id), lane i%4
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ void philox_round(uint32_t &c0, uint32_t &c1, uint32_t &c2, uint32_t &c3,

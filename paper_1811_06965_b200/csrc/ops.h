@@ -114,6 +114,8 @@ cudaError_t loss_reduce(const Ctx &c, const float *rowloss, float *loss, int64_t
 // ---- parameters ---------------------------------------------------------------------------------
 cudaError_t sgd_apply(const Ctx &c, int dt, float *master, float *grad, void *w_lp, int64_t n,
                       float lr);
+cudaError_t rmsprop_apply(const Ctx &c, int dt, float *master, float *grad, float *ms, void *w_lp, int64_t n,
+                          float lr, float rho, float eps);
 cudaError_t init_normal(const Ctx &c, int dt, float *master, void *w_lp, int64_t n, uint64_t seed,
                         uint64_t stream_id, float mean, float std);
 cudaError_t fill_f32(const Ctx &c, float *p, int64_t n, float v);

@@ -202,6 +202,10 @@ int gpipe_op_embed_bwd(void *stream, const int32_t *tok, const float *dx, float 
 int gpipe_op_positional(void *stream, float *pe, int S, int d) {
   return ret(positional_table(mk(stream), pe, S, d), "gpipe_op_positional");
 }
+int gpipe_op_rmsprop(void *stream, int dtype, float *master, float *grad, float *ms, void *w_lp, int64_t n, float lr,
+                     float rho, float eps) {
+  return ret(rmsprop_apply(mk(stream), dtype, master, grad, ms, w_lp, n, lr, rho, eps), "gpipe_op_rmsprop");
+}
 int gpipe_op_sgd(void *stream, int dtype, float *master, float *grad, void *w_lp, int64_t n, float lr) {
   return ret(sgd_apply(mk(stream), dtype, master, grad, w_lp, n, lr), "gpipe_op_sgd");
 }

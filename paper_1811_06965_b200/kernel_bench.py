@@ -201,6 +201,9 @@ def main():
                 for _ in range(2)]
         ms = time_it([(lambda s=s: ops.sgd(s[0], s[1], s[2], 1e-3)) for s in sets], max(2, args.reps // 2))
         report("sgd", "sgd_apply", ms, 0, n * 18.0)
+        sets = [s + (torch.rand(n, device=dev),) for s in sets]
+        ms = time_it([(lambda s=s: ops.rmsprop(s[0], s[1], s[3], s[2], 1e-3, 0.9, 1e-6)) for s in sets], max(2, args.reps // 2))
+        report("sgd", "rmsprop_apply", ms, 0, n * 26.0)          # g r+w, ms r+w, master r+w, bf16 copy w
 
     if args.json:
         os.makedirs(os.path.dirname(os.path.abspath(args.json)), exist_ok=True)

@@ -136,3 +136,8 @@ def positional(pe):
 def sgd(master, grad, w_lp, lr):
     B._check(B.lib().gpipe_op_sgd(_stream(), B.DTYPE_BF16 if w_lp is not None else B.DTYPE_FP32, _p(master), _p(grad),
                                   _p(w_lp), master.numel(), lr))
+
+
+def rmsprop(master, grad, ms, w_lp, lr, rho, eps):
+    B._check(B.lib().gpipe_op_rmsprop(_stream(), B.DTYPE_BF16 if w_lp is not None else B.DTYPE_FP32, _p(master), _p(grad),
+                                      _p(ms), _p(w_lp), master.numel(), lr, rho, eps))

@@ -379,3 +379,31 @@ def test_partition_error_paths():
     for bad in ([0, 0, 4], [0, 4, 4], [1, 2, 4], [0, 2, 5], [0, 3, 2]):
         with pytest.raises(gp.GPipeError):
             _engine(w, partition=bad)
+
+
+def test_rmsprop_training_steps_match_oracle():
+    """SURVEY.md 8(f) f3 / PAPER.md:71: three mini-batches of step + gpipe_apply_rmsprop against the oracle."""
+    w = _tiny((0, 1))
+    params = gi.make_params(w, 1001, round_bf16=False)
+    o = None
+    with _engine(w) as e:
+        e.set_params(params)
+        with pytest.raises(gp.GPipeError):
+            gp.binding._check(gp.lib().gpipe_apply_rmsprop(e._h, 0.01, 0.9, 1e-6))      # no slots attached yet
+        for it in range(3):
+            tok, lab = gi.make_tokens(w, 2001 + it)
+            if o is None:
+                o, _ = run_oracle(w, params, tok, lab)      # builds the oracle (and runs one step we discard)
+                o.zero_grads()
+            loss_ref = o.step(tok, lab)
+            loss = e.step(tok, lab)
+            assert abs(loss - loss_ref) <= 2e-4 * abs(loss_ref), it
+            o.apply_rmsprop(0.002, 0.9, 1e-6)
+            e.apply_rmsprop(0.002, 0.9, 1e-6)
+            for n in e.names:
+                assert maxrel(e.get_param(n), o.p[n]) <= 2e-4, (it, n)
+                assert not e.get_grad(n).any()
+        with pytest.raises(gp.GPipeError):
+            e.apply_rmsprop(0.01, 1.0, 1e-6)
+        with pytest.raises(gp.GPipeError):
+            e.apply_rmsprop(0.01, 0.9, 0.0)

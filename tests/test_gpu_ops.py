@@ -345,3 +345,29 @@ def test_colsum_embedding_sgd(dtype):
     assert not g.any()
     if wl is not None:
         assert torch.equal(wl, m.to(torch.bfloat16))
+
+
+@pytest.mark.parametrize("dtype", ["fp32", "bf16"])
+def test_rmsprop_kernel_matches_library_routine(dtype):
+    """gpipe_op_rmsprop against torch.optim.RMSprop on the CPU (alpha = rho, no momentum, not centered) over three
+    applications; the bf16 working copy is the RNE rounding of the fp32 master; the gradient is cleared."""
+    r = _rng(31)
+    n = 4096 + 64
+    lr, rho, eps = 0.05, 0.9, 1e-6
+    w0 = r.standard_normal(n).astype(np.float32)
+    m = torch.tensor(w0, device=DEV)
+    ms = torch.zeros(n, device=DEV)
+    wl = torch.empty(n, device=DEV, dtype=torch.bfloat16) if dtype == "bf16" else None
+    tp = torch.tensor(w0.astype(np.float64), requires_grad=True)
+    opt = torch.optim.RMSprop([tp], lr=lr, alpha=rho, eps=eps)
+    for step in range(3):
+        g0 = (r.standard_normal(n) * 10.0 ** r.integers(-4, 3, size=n)).astype(np.float32)
+        g0[::7] = 0.0
+        g = torch.tensor(g0, device=DEV)
+        ops.rmsprop(m, g, ms, wl, lr, rho, eps)
+        tp.grad = torch.tensor(g0.astype(np.float64))
+        opt.step()
+        assert not _np(g).any()
+        assert maxrel(_np(m), tp.detach().numpy()) <= 2e-6, step
+        if wl is not None:
+            assert torch.equal(wl, m.to(torch.bfloat16))

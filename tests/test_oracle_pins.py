@@ -406,6 +406,53 @@ def test_p10_sgd_update_identity_and_descent():
     assert l1 < l0
 
 
+def test_p10_rmsprop_closed_forms_and_library():
+    """Reading A20 (PAPER.md:71 names RMSProp, not its formula).  (i) a constant gradient g applied n times gives
+    ms_n = (1 - rho^n) g^2 and w_n = w_0 - lr sum_k g / (sqrt(1 - rho^k) |g| + eps); (ii) with eps -> 0 the first
+    update is lr sign(g) / sqrt(1 - rho) whatever the scale of g; (iii) a zero gradient moves nothing;
+    (iv) torch.optim.RMSprop (alpha = rho, no momentum, not centered) walks the same trajectory."""
+    w = _tiny()
+    spec = go.Spec(w.n_layers, w.d_model, w.d_ffn, w.n_heads, w.d_head, w.vocab, w.seq_len, w.causal, w.ln_eps)
+    r = np.random.default_rng(5)
+    lr, rho, eps = 0.01, 0.9, 1e-3
+    o = go.GPipeOracle(spec, 1, 1, False)
+    p0 = {n: r.standard_normal(sh) for n, sh in o.shapes.items()}
+    g = {n: r.standard_normal(sh) * 10.0 ** r.integers(-3, 2) for n, sh in o.shapes.items()}
+    o.set_params(p0)
+    for n_steps in range(1, 5):
+        for n in o.names:
+            o.g[n] = g[n].copy()
+        o.apply_rmsprop(lr, rho, eps)
+        for n in ("emb", "l0.w_1", "l1.b_o", "lnf_g"):
+            assert np.allclose(o.ms[n], (1 - rho ** n_steps) * g[n] ** 2, rtol=1e-12, atol=0)
+            want = p0[n] - lr * sum(g[n] / (math.sqrt(1 - rho ** k) * np.abs(g[n]) + eps) for k in range(1, n_steps + 1))
+            assert np.allclose(o.p[n], want, rtol=1e-11, atol=1e-13)
+            assert not o.g[n].any()                                        # applied once, then cleared (PAPER.md:67)
+    o2 = go.GPipeOracle(spec, 1, 1, False)
+    o2.set_params(p0)
+    for scale in (1e-4, 1.0, 1e4):
+        o2.set_params(p0)
+        if hasattr(o2, "ms"):
+            del o2.ms
+        o2.g["l0.w_2"] = g["l0.w_2"] * scale
+        o2.apply_rmsprop(lr, rho, 1e-30)
+        assert np.allclose(o2.p["l0.w_2"], p0["l0.w_2"] - lr * np.sign(g["l0.w_2"]) / math.sqrt(1 - rho), rtol=1e-12)
+        assert np.array_equal(o2.p["l0.w_1"], p0["l0.w_1"])                # zero gradient: untouched
+    # torch's implementation as the independent routine
+    o3 = go.GPipeOracle(spec, 1, 1, False)
+    o3.set_params(p0)
+    name = "l1.w_qkv"
+    tp = torch.tensor(p0[name], dtype=torch.float64, requires_grad=True)
+    opt = torch.optim.RMSprop([tp], lr=lr, alpha=rho, eps=eps, momentum=0.0, centered=False)
+    for step in range(4):
+        gs = r.standard_normal(p0[name].shape)
+        o3.g[name] = gs.copy()
+        o3.apply_rmsprop(lr, rho, eps)
+        tp.grad = torch.tensor(gs)
+        opt.step()
+        assert np.allclose(o3.p[name], tp.detach().numpy(), rtol=1e-12, atol=1e-14), step
+
+
 def test_step_accumulates_until_apply():
     """gpipe_step ADDS into the gradient buffers (SURVEY.md 8(b) accumulation semantics)."""
     w = _tiny()

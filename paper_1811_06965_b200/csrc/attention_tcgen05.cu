@@ -229,8 +229,14 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
     tcgen05_fence_after();
     mbar_wait(bar_v, 0, 0x23);
     const uint32_t id = idesc(0, 1, DH);
-    for (int kk = 0; kk < N / 16; ++kk)
-      umma_bf16(tmem, desc_k(sP + (uint32_t)(kk >> 2) * TILE, kk & 3), desc_mn(sV, kk), id, kk ? 1u : 0u);
+    // descriptors differ only in their (address >> 4) field: one base each, a constant added per k-step - the
+    // N = 64 products retire in ~40 cycles, so the issuing thread must not spend longer than that per MMA
+    const uint64_t aP = desc_k(sP, 0), bV = desc_mn(sV, 0);
+    const int nkk = N / 16;
+#pragma unroll
+    for (int kk = 0; kk < 16; ++kk)
+      if (kk < nkk)
+        umma_bf16(tmem, aP + (uint64_t)((kk >> 2) * (TILE >> 4) + (kk & 3) * 2), bV + (uint64_t)(kk * 128), id, kk ? 1u : 0u);
     tcgen05_commit(bar_o);
   }
   __syncwarp();
@@ -328,13 +334,18 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
       tcgen05_fence_after();
       stamp(1);
       const uint32_t id_sp = idesc(0, 0, 128), id_g_mn = idesc(1, 1, DH), id_g_k = idesc(0, 1, DH);
+      // Descriptors differ only in their (address >> 4) field: bases are built once and a constant is added
+      // per tile / k-step, so that the issuing thread spends a few instructions per MMA (an N = 64 product
+      // retires in ~40 cycles; rebuilding two descriptors per MMA took ~90 and made the issue the bottleneck).
+      constexpr uint64_t T16 = TILE >> 4;                 // one tile further
+      const uint64_t kQ = desc_k(sQ, 0), kK = desc_k(sK, 0), kV = desc_k(sV, 0), kdO = desc_k(sdO, 0), kdS = desc_k(sdS, 0);
+      const uint64_t mP = desc_mn(sP, 0), mdS = desc_mn(sdS, 0), mQ = desc_mn(sQ, 0), mK = desc_mn(sK, 0), mdO = desc_mn(sdO, 0);
       auto issue_sp = [&](int i, int j) {
+        const uint64_t a0 = kQ + i * T16, b0 = kK + j * T16, a1 = kdO + i * T16, b1 = kV + j * T16;
 #pragma unroll
-        for (int ks = 0; ks < 4; ++ks)
-          umma_bf16(tmem + C_S, desc_k(sQ + i * TILE, ks), desc_k(sK + j * TILE, ks), id_sp, ks ? 1u : 0u);
+        for (int ks = 0; ks < 4; ++ks) umma_bf16(tmem + C_S, a0 + ks * 2, b0 + ks * 2, id_sp, ks ? 1u : 0u);
 #pragma unroll
-        for (int ks = 0; ks < 4; ++ks)
-          umma_bf16(tmem + C_DP, desc_k(sdO + i * TILE, ks), desc_k(sV + j * TILE, ks), id_sp, ks ? 1u : 0u);
+        for (int ks = 0; ks < 4; ++ks) umma_bf16(tmem + C_DP, a1 + ks * 2, b1 + ks * 2, id_sp, ks ? 1u : 0u);
         tcgen05_commit(bar_sp);
       };
       // block pairs in order: j outer, i inner (i >= j when causal)
@@ -353,16 +364,19 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
           mbar_wait(bar_pds, n & 1, 0x33);                // P / dS panels written (and dV_{j-1}, dK_{j-1} read out)
           tcgen05_fence_after();
           if (n < 4) stamp(3 + 3 * n);
+          {
+            const uint64_t bdO = mdO + i * T16, bQ = mQ + i * T16, bK = mK + j * T16;
+            const uint32_t acc_kv = i > i_first ? 1u : 0u, acc_q = (dq_started >> i) & 1u;
 #pragma unroll
-          for (int kk = 0; kk < 8; ++kk)                  // dV_j += P^T dO_i   (K = 128 queries)
-            umma_bf16(tmem + C_DV, desc_mn(sP, kk), desc_mn(sdO + i * TILE, kk), id_g_mn, (i > i_first || kk) ? 1u : 0u);
+            for (int kk = 0; kk < 8; ++kk)                // dV_j += P^T dO_i   (K = 128 queries)
+              umma_bf16(tmem + C_DV, mP + kk * 128, bdO + kk * 128, id_g_mn, kk ? 1u : acc_kv);
 #pragma unroll
-          for (int kk = 0; kk < 8; ++kk)                  // dK_j += dS^T Q_i
-            umma_bf16(tmem + C_DK, desc_mn(sdS, kk), desc_mn(sQ + i * TILE, kk), id_g_mn, (i > i_first || kk) ? 1u : 0u);
+            for (int kk = 0; kk < 8; ++kk)                // dK_j += dS^T Q_i
+              umma_bf16(tmem + C_DK, mdS + kk * 128, bQ + kk * 128, id_g_mn, kk ? 1u : acc_kv);
 #pragma unroll
-          for (int kk = 0; kk < 8; ++kk)                  // dQ_i += dS K_j     (K = 128 keys)
-            umma_bf16(tmem + C_DQ + 64 * i, desc_k(sdS + (uint32_t)(kk >> 2) * TILE, kk & 3), desc_mn(sK + j * TILE, kk),
-                      id_g_k, (((dq_started >> i) & 1u) || kk) ? 1u : 0u);
+            for (int kk = 0; kk < 8; ++kk)                // dQ_i += dS K_j     (K = 128 keys)
+              umma_bf16(tmem + C_DQ + 64 * i, kdS + (kk >> 2) * T16 + (kk & 3) * 2, bK + kk * 128, id_g_k, kk ? 1u : acc_q);
+          }
           dq_started |= 1u << i;
           tcgen05_commit(bar_acc);
           if (n < 4) stamp(4 + 3 * n);

@@ -3,25 +3,27 @@
 // SURVEY 8(a) a7, a16; K5/K6 of DESIGN.md).
 //
 // With S <= 256 a whole row of scores fits one TMEM accumulator (128 lanes x 256 fp32 columns), so
-// the forward softmax is a plain two-pass row softmax by the thread that owns the TMEM lane: no
-// online rescaling, no cross-thread reduction.  All five backward products of a head run on
-// tcgen05.mma from 128-byte-swizzled shared-memory tiles that TMA fetched where the tensors lie
-// (head h = 64 columns of the [tokens, 3*d_a] qkv matrix; 3-D tensor maps [seq][row][col] clip and
-// zero-fill at the end of a sequence).
+// the forward softmax is a plain two-pass row softmax over TMEM: no online rescaling.  All five
+// backward products of a head run on tcgen05.mma from 128-byte-swizzled shared-memory tiles that TMA
+// fetched where the tensors lie (head h = 64 columns of the [tokens, 3*d_a] qkv matrix; 3-D tensor
+// maps [seq][row][col] zero-fill past the end of a sequence).
 //
-// forward  (one CTA = 128 query rows of one (sequence, head), 4 warps, 2 CTAs / SM):
-//   TMA Q, K, V -> S = Q K^T (M 128, N <= 256, K 64) in TMEM -> per-lane row max, P = exp2(..) as bf16
-//   into swizzled K-major panels (overlaying Q / K, which are dead by then) -> O = P V
-//   (M 128, N 64, K <= 256; V is the MN-major B operand as it lies) -> O / l -> TMA store; LSE.
+// forward  (one CTA = 128 query rows of one (sequence, head), 8 warps, 2 CTAs / SM):
+//   TMA Q, K, V -> S = Q K^T (M 128, N <= 256, K 64) in TMEM -> row max, P = exp2(..) as bf16 into
+//   swizzled K-major panels (overlaying Q / K, which are dead by then) -> O = P V (M 128, N 64,
+//   K <= 256; V is the MN-major B operand as it lies) -> O / l and the LSE stored directly.
 // backward (one CTA = one (sequence, head), 8 compute warps + 1 control warp, 1 CTA / SM):
 //   for key block j, query block i (128 x 128 each):  S = Q_i K_j^T, dP = dO_i V_j^T  (TMEM)
 //   -> P = exp2(S - lse), dS = P (dP - D) as bf16 panels in shared memory
 //   -> dV_j += P^T dO_i, dK_j += dS^T Q_i (the panels read as MN-major A), dQ_i += dS K_j (K-major A);
 //   dV_j, dK_j, dQ_0, dQ_1 stay in TMEM (4 x 64 columns) next to S and dP (2 x 128): 512 columns.
 //   The control thread issues S/dP of the next block pair as soon as the compute warps have pulled
-//   the current pair into registers, so the tensor pipe works under the exponentials.
+//   the current pair into registers, so the tensor pipe works under the exponentials; dV_j / dK_j are
+//   read out inside the first pair of the next key block.  Gradients leave through a per-warp
+//   shared-memory transposer (coalesced 64-byte row segments).
 //   Deterministic: no atomics, fixed accumulation order.
-// Roofline: bf16 tensor pipe / MUFU.EX2.
+// What bounds them (profiles/attn_r01.md): forward - MUFU.EX2 and the serial load / S / softmax / P V
+// chain of a CTA; backward - the panel hand-over between the compute warps and the N = 64 products.
 #include <cuda.h>
 #include <math.h>
 
@@ -46,11 +48,6 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *map
       "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
       ::"r"(dst), "l"((uint64_t)map), "r"(bar), "r"(c0), "r"(c1), "r"(c2)
       : "memory");
-}
-__device__ __forceinline__ void tma_store_3d(const CUtensorMap *map, uint32_t src, int c0, int c1, int c2) {
-  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4}], [%1];"
-               ::"l"((uint64_t)map), "r"(src), "r"(c0), "r"(c1), "r"(c2)
-               : "memory");
 }
 __device__ __forceinline__ float ex2(float x) {
   float y;

@@ -23,13 +23,32 @@ __global__ void embed_fwd_kernel(const int32_t *__restrict__ tok, const T *__res
   store4(x + t * d + c, make_float4(e.x + p.x, e.y + p.y, e.z + p.z, e.w + p.w));
 }
 
-__global__ void embed_bwd_kernel(const int32_t *__restrict__ tok, const float *__restrict__ dx,
-                                 float *__restrict__ gemb, int64_t n_tok, int d) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n_tok * d) return;
-  int64_t t = i / d;
-  int c = (int)(i - t * d);
-  atomicAdd(gemb + (int64_t)tok[t] * d + c, dx[i]);      // dE[tok] += dx0 (order-free, A13)
+// dE[tok[t]] += dx0[t], without atomics and in a fixed order: warp w of the grid owns the vocabulary rows v
+// with v mod W == w (W = warps in the grid), scans all token ids 32 at a time and adds the rows of the
+// tokens it owns in ascending t.  One owner per row + program order within a lane = a deterministic
+// sum whatever the multiplicity of an id (the atomicAdd version was the last order-dependent kernel).
+__global__ void __launch_bounds__(256)
+embed_bwd_kernel(const int32_t *__restrict__ tok, const float *__restrict__ dx, float *__restrict__ gemb,
+                 int64_t n_tok, int d) {
+  const int lane = threadIdx.x & 31;
+  const unsigned W = gridDim.x * (blockDim.x >> 5), w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  const int d4 = d >> 2;
+  for (int64_t base = 0; base < n_tok; base += 32) {
+    const int64_t t = base + lane;
+    const int id = t < n_tok ? tok[t] : -1;
+    unsigned mine = __ballot_sync(0xffffffffu, id >= 0 && (unsigned)id % W == w);
+    while (mine) {
+      const int src = __ffs(mine) - 1;
+      mine &= mine - 1;
+      const int v = __shfl_sync(0xffffffffu, id, src);
+      const float *row = dx + (base + src) * d;
+      float *dst = gemb + (int64_t)v * d;
+      for (int j = lane; j < d4; j += 32) {
+        float4 a = load4(dst + 4 * j), b = load4(row + 4 * j);
+        store4(dst + 4 * j, make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w));
+      }
+    }
+  }
 }
 
 // PE[t,2i] = sin(t / 10000^(2i/d)), PE[t,2i+1] = cos(...), evaluated in double, stored fp32
@@ -56,9 +75,12 @@ cudaError_t embed_fwd(const Ctx &c, int dt, const int32_t *tok, const void *emb,
 
 cudaError_t embed_bwd(const Ctx &c, const int32_t *tok, const float *dx, float *gemb,
                       int64_t n_tok, int d) {
-  int64_t n = n_tok * d;
-  if (n == 0) return cudaSuccess;
-  embed_bwd_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(tok, dx, gemb, n_tok, d);
+  if (n_tok == 0 || d == 0) return cudaSuccess;
+  if (d % 4) return cudaErrorInvalidValue;
+  // ~one owned token per warp at T_mb = 2048; never more warps than tokens
+  int64_t blocks = (n_tok + 7) / 8;
+  if (blocks > 2 * (int64_t)c.sm_count) blocks = 2 * (int64_t)c.sm_count;
+  embed_bwd_kernel<<<(unsigned)blocks, 256, 0, c.stream>>>(tok, dx, gemb, n_tok, d);
   GP_LAUNCH_CHECK(c);
 }
 

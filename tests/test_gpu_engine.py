@@ -87,7 +87,7 @@ def test_gradients_independent_of_K_M_remat_on_gpu():
 
 def test_remat_equals_stored_bitwise_on_gpu():
     """replayed activations are bit-identical, so every gradient that is summed in
-    a fixed order is bit-identical (everything except the atomically accumulated embedding)."""
+    a fixed order is bit-identical - which is every gradient (the embedding scatter-add has a fixed order too)."""
     w = _tiny((0, 1))
     params = gi.make_params(w, 1001, round_bf16=False)
     tok, lab = gi.make_tokens(w, 2001)
@@ -98,8 +98,7 @@ def test_remat_equals_stored_bitwise_on_gpu():
             out.append((e.step(tok, lab), e.grads()))
     assert out[0][0] == out[1][0]
     for n in out[0][1]:
-        if n != "emb":
-            assert np.array_equal(out[0][1][n], out[1][1][n]), n
+        assert np.array_equal(out[0][1][n], out[1][1][n]), n
 
 
 def test_step_accumulates_and_sgd_applies():
@@ -356,8 +355,8 @@ def test_fp32_parity_explicit_partition(cell_lo):
 
 def test_bf16_cost_partition_changes_nothing_but_the_cut():
     """partition="cost": the head's cost shortens the last cell; per-token values do not depend on where the
-    cuts are, so loss and every gradient are bitwise those of the equal split (the embedding gradient, a float
-    atomic scatter-add, to summation order)."""
+    cuts are, so loss and every gradient (the embedding's too: its scatter-add has a fixed order) are bitwise
+    those of the equal split."""
     w = gi.CONFIGS["T(6,4096,16)"].replace(name="bf16-part", n_layers=6, d_model=256, d_ffn=512, n_heads=4, d_head=64,
                                            vocab=4096, seq_len=64, n_seqs=8, M=4, K=2, causal=(0, 1, 0, 1, 0, 1))
     params = gi.make_params(w, 1005)
@@ -372,10 +371,7 @@ def test_bf16_cost_partition_changes_nothing_but_the_cut():
     for cells, loss, g, peak in out[1:]:
         assert loss == out[0][1] and peak == out[0][3]
         for n in g:
-            if n == "emb":      # the one float-atomic kernel (scatter-add of dx0 over repeated token ids, reading A13)
-                assert maxrel(g[n], out[0][2][n]) <= 1e-6, cells
-            else:
-                assert np.array_equal(g[n], out[0][2][n]), (cells, n)
+            assert np.array_equal(g[n], out[0][2][n]), (cells, n)
 
 
 def test_partition_error_paths():

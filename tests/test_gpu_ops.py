@@ -402,3 +402,25 @@ def test_rmsprop_kernel_matches_library_routine(dtype):
         assert maxrel(_np(m), tp.detach().numpy()) <= 2e-6, step
         if wl is not None:
             assert torch.equal(wl, m.to(torch.bfloat16))
+
+
+@pytest.mark.parametrize("n_tok,V,d", [(2048, 64000, 1024), (2048, 7, 1024), (77, 50, 64), (1, 3, 8), (5000, 300, 256)])
+def test_embedding_backward_is_exact_and_deterministic(n_tok, V, d):
+    """dE[tok[t]] += dx0[t] (a17): every vocabulary row has one owner that adds its tokens in ascending t, so the
+    result is the fp32 running sum in token order - reproduced here with a sequential fp32 loop - bitwise, on every
+    launch, whatever the multiplicity of an id (V = 7: ~300 tokens per row)."""
+    r = _rng(n_tok + V)
+    tok = r.integers(0, V, size=n_tok).astype(np.int32)
+    dx = r.standard_normal((n_tok, d)).astype(np.float32)
+    g0 = r.standard_normal((V, d)).astype(np.float32)
+    ref = g0.copy()
+    for t in range(n_tok):                                   # the definition, in the kernel's order and precision
+        ref[tok[t]] += dx[t]
+    tt, dxt = torch.tensor(tok, device=DEV), torch.tensor(dx, device=DEV)
+    outs = []
+    for _ in range(3):
+        gemb = torch.tensor(g0, device=DEV)
+        ops.embed_bwd(tt, dxt, gemb)
+        outs.append(_np(gemb).astype(np.float32))
+    assert np.array_equal(outs[0], ref)
+    assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])

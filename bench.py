@@ -12,7 +12,8 @@ the ids and D2H of the loss partials inside the timed region).  The default work
 BASELINE.json's T(64,16384,32) configuration - the one its target is quoted on; it fits one GPU.
 Prints ONE JSON line on rank 0.  `--impl reference` times the CPU oracle on a bounded sample
 (see DESIGN.md "Measurement").  N > 1: independent replicas, no collective (the
-north star fixes "no sharding across GPUs and no collectives").
+north star fixes "no sharding across GPUs and no collectives"); launched under torchrun, or by plain
+`python bench.py --gpus N`, which starts the N ranks itself.
 """
 from __future__ import annotations
 
@@ -111,6 +112,22 @@ def progress(msg):
         print("[bench %7.1fs] %s" % (time.perf_counter() - _T0, msg), file=sys.stderr, flush=True)
 
 
+def ncu_traffic(kernel_key):
+    """DRAM read+write bytes per launch of the dominant kernel from the committed ncu --set full capture
+    (profiles/ncu_traffic.json, written by `python -m paper_1811_06965_b200.ncu_summary`); None when absent."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if not os.path.exists(p):
+        return None, "absent: no profiles/ncu_traffic.json"
+    try:
+        j = json.load(open(p))
+    except Exception as ex:                                   # a damaged file must not take the bench down
+        return None, "absent: %s" % ex
+    rec = j.get(kernel_key)
+    if not rec:
+        return None, "absent: no entry %r in profiles/ncu_traffic.json" % kernel_key
+    return float(rec["dram_bytes_per_launch"]), "profiles/ncu_traffic.json[%s] (%s)" % (kernel_key, rec.get("source", "?"))
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -165,15 +182,44 @@ def oracle_sample(w, repeats=2):
             "seconds": t_head + t_some}
 
 
+def oracle_full(w):
+    """One WHOLE oracle step of the full workload (all N sequences, all L layers, the K/M schedule with replay),
+    fp32, timed once after a one-sequence warm-up of the BLAS pool.  Minutes for config 2; do not use on 4/5."""
+    from oracle import gpipe_oracle as go
+    try:
+        from threadpoolctl import threadpool_info
+        cores = max([i.get("num_threads", 1) for i in threadpool_info()] + [1])
+    except Exception:
+        cores = os.cpu_count() or 1
+    params = gi.make_params(w, 1, parity=False, round_bf16=False)
+    tok, lab = gi.make_tokens(w, 2)
+    spec = go.Spec(w.n_layers, w.d_model, w.d_ffn, w.n_heads, w.d_head, w.vocab, w.seq_len, w.causal, w.ln_eps)
+    warm = go.GPipeOracle(spec, w.K, 1, w.remat, dtype=np.float32)
+    warm.set_params(params)
+    warm.step(tok[:1], lab[:1])
+    o = go.GPipeOracle(spec, w.K, w.M, w.remat, dtype=np.float32)
+    o.set_params(params)
+    t0 = time.perf_counter()
+    loss = o.step(tok, lab)
+    dt = time.perf_counter() - t0
+    return {"value": w.tokens_per_step / dt, "unit": UNIT, "cores": int(cores), "kind": "oracle",
+            "sample": "one full fp32 numpy oracle step of %s (%d sequences x %d tokens, K %d, M %d, remat %s): %.1f s, "
+                      "loss %.4f" % (w.name, w.n_seqs, w.seq_len, w.K, w.M, w.remat, dt, loss),
+            "seconds": dt}
+
+
 def run_reference(args, w, rank, world):
     if rank != 0:
         return
     times = []
     res = None
     for i in range(args.warmup + args.steps):
-        res = oracle_sample(w)
+        res = oracle_full(w) if args.oracle_full else oracle_sample(w)
         if i >= args.warmup:
             times.append(res["value"])
+        if args.oracle_full:
+            times = [res["value"]]                          # one full step is the measurement
+            break
     value = float(np.mean(times))
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * w.tokens_per_step / value,
@@ -196,13 +242,16 @@ def run_ours(args, w, rank, world, local_rank):
     from paper_1811_06965_b200 import build
     from paper_1811_06965_b200.dist_util import max_over_ranks, barrier
 
+    torch.cuda.set_device(local_rank)                    # before the first (NCCL) barrier
+    dev = torch.device("cuda", local_rank)
     if rank == 0:
         build.build()
     barrier(world)
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
     peaks = measured_peaks()
     progress("library built and loaded; creating engine for %s" % w.name)
+    torch.cuda.synchronize(dev)
+    free_before, _ = torch.cuda.mem_get_info(dev)
+    torch.cuda.reset_peak_memory_stats(dev)
     eng = gp.from_workload(w, device=dev, partition=None if args.partition == "equal" else args.partition)
     eng.init_params(seed=1000 + rank, std=0.02, parity=False)
     progress("engine ready (%.1f GB arena)" % (eng.peak_bytes()["total"] / 1e9))
@@ -236,15 +285,28 @@ def run_ours(args, w, rank, world, local_rank):
     clocks = sampler.stop() if sampler else None
     progress("timed region done: %.1f ms/step" % (ms / args.steps))
     ms_e2e = timed(lambda: eng.step(tok_h, lab_h), args.steps)
-    # one extra step with per-launch CUDA events for the roofline of the dominant kernel class
-    progress("e2e region done: %.1f ms/step; per-launch timing step" % (ms_e2e / args.steps))
-    eng.kernel_timing(True, serial=True)         # each launch alone on the GPU: standalone durations
+    # two extra steps with per-launch CUDA events for the roofline of the dominant kernel class:
+    # (1) "isolated": every cell on stream 0, each launch alone on the GPU (standalone durations);
+    # (2) "in-step": the K-stream schedule as timed above, each launch bracketed on its own stream (durations
+    #     then include the SMs it shares with the other cells' kernels)
+    progress("e2e region done: %.1f ms/step; per-launch timing steps" % (ms_e2e / args.steps))
+    eng.kernel_timing(True, serial=True)
     eng.step(tok_d, lab_d)
-    progress("per-launch timing step done")
     stats = eng.kernel_stats()
+    eng.kernel_timing(True, serial=False)
+    eng.step(tok_d, lab_d)
+    stats_conc = eng.kernel_stats()
+    progress("per-launch timing steps done")
     eng.kernel_timing(False)
     eng.zero_grads()
     peak_hbm = eng.peak_bytes()
+    torch.cuda.synchronize(dev)
+    free_after, _ = torch.cuda.mem_get_info(dev)
+    hbm_check = {"gpipe_peak_bytes": peak_hbm["total"],
+                 "torch_max_memory_allocated": int(torch.cuda.max_memory_allocated(dev)),
+                 "cudaMemGetInfo_delta": int(free_before - free_after),
+                 "note": "the arena is one torch allocation of gpipe_plan_bytes; the deltas also hold the id tensors "
+                         "and the caching allocator's rounding"}
 
     tokens = w.tokens_per_step * world
     value = tokens * args.steps / (ms / 1e3)
@@ -255,18 +317,40 @@ def run_ours(args, w, rank, world, local_rank):
     gem_fl = sum(v["flops"] for v in gem.values())
     tot_ms = sum(v["ms"] for v in stats.values())
     achieved = gem_fl / (gem_ms / 1e3) / 1e12 if gem_ms > 0 else 0.0
-    roofline = {"bound": "tensor", "kernel": "gemm_tcgen05_kernel (fwd + dgrad + wgrad launches)",
+    traffic, traffic_src = ncu_traffic("gemm_tcgen05:ffn1_fwd")
+
+    def per_class(st):
+        return {k: {"launches": int(v["launches"]), "ms": round(v["ms"], 3),
+                    "tflops": (v["flops"] / v["ms"] / 1e9) if v["ms"] > 0 and v["flops"] > 0 else None,
+                    "gbs": (v["bytes"] / v["ms"] / 1e6) if v["ms"] > 0 else None}
+                for k, v in st.items()}
+
+    n_gemm = int(sum(v["launches"] for v in gem.values()))
+    # in-step regime: what the timed step achieves on the tensor cores - all GEMM + attention FLOPs it executes,
+    # over the step's device time (K streams co-running; HBM-bound kernels share the same clock)
+    tens_fl = sum(v["flops"] for v in stats.values())
+    gem_c_ms = sum(stats_conc[k]["ms"] for k in gem)
+    roofline = {"bound": "tensor", "kernel": "gemm_tcgen05_pair_kernel (fwd + dgrad + wgrad launches)",
+                "regime": "isolated",
+                "regime_note": "each launch timed alone on the GPU (all cells serialised on one stream, one extra step); "
+                               "achieved = sum of 2MNK / sum of launch durations",
                 "achieved": achieved, "peak": peaks["sustained"], "unit": "TFLOP/s",
                 "frac": achieved / peaks["sustained"], "peak_src": peaks["src"] + " sustained bf16 (kernel timed inside a long step)",
-                # DRAM read + write bytes of one FFN1-forward launch (the most frequent large shape), from the
-                # committed `ncu --set full` capture profiles/gemm_ffn1_fwd_r01.md; algorithmic bytes 109 MB
-                "traffic": 58.3e6, "traffic_src": "profiles/gemm_ffn1_fwd_r01.md (ffn1_fwd launch, dram read+write)",
-                "launches": int(sum(v["launches"] for v in gem.values())),
+                "frac_of_burst": achieved / peaks["burst"],
+                "traffic": traffic, "traffic_src": traffic_src,
+                "launches": n_gemm,
+                "avg_launch_us": 1e3 * gem_ms / n_gemm if n_gemm else None,
                 "share_of_kernel_time": gem_ms / tot_ms if tot_ms else None,
-                "per_class": {k: {"launches": int(v["launches"]), "ms": round(v["ms"], 3),
-                                  "tflops": (v["flops"] / v["ms"] / 1e9) if v["ms"] > 0 and v["flops"] > 0 else None,
-                                  "gbs": (v["bytes"] / v["ms"] / 1e6) if v["ms"] > 0 else None}
-                              for k, v in stats.items()}}
+                "per_class": per_class(stats),
+                "in_step": {"regime": "in-step",
+                            "regime_note": "the timed K-stream schedule: executed tensor FLOPs (GEMM + attention) / step "
+                                           "device time; per_class durations are per-launch events on the launch's own "
+                                           "stream while the other cells' kernels share the SMs",
+                            "achieved": tens_fl / step_s / 1e12, "peak": peaks["sustained"], "unit": "TFLOP/s",
+                            "frac": tens_fl / step_s / 1e12 / peaks["sustained"],
+                            "gemm_share_of_stream_time": gem_c_ms / sum(v["ms"] for v in stats_conc.values())
+                            if stats_conc else None,
+                            "per_class": per_class(stats_conc)}}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "bf16" if w.dtype == "bf16" else "f32", "data": "synthetic",
@@ -282,13 +366,15 @@ def run_ours(args, w, rank, world, local_rank):
             "mfu_model_flops": fl["model"] / step_s / 1e12 / peaks["burst"],
             "peak_tflops_burst": peaks["burst"], "peak_tflops_sustained": peaks["sustained"],
             "peak_hbm_bytes": peak_hbm["total"], "peak_hbm_by_category": peak_hbm["by_category"],
+            "peak_hbm_cross_check": hbm_check,
             "clocks": clocks, "roofline": roofline,
             "e2e": {"value": tokens * args.steps / (ms_e2e / 1e3), "unit": UNIT,
                     "h2d_bytes_per_step": int(tok.nbytes + lab.nbytes), "d2h_bytes_per_step": 4 * w.M},
             "gpu_launches": int(launches)}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         progress("timing the CPU oracle sample")
-        line["cpu_baseline"] = {k: v for k, v in oracle_sample(w).items() if k != "seconds"}
+        line["cpu_baseline"] = {k: v for k, v in (oracle_full(w) if args.oracle_full else oracle_sample(w)).items()
+                                if k != "seconds"}
     eng.close()
     if rank == 0:
         print(json.dumps(line), flush=True)
@@ -304,9 +390,14 @@ def main():
     ap.add_argument("--M", type=int, default=None)
     ap.add_argument("--K", type=int, default=None)
     ap.add_argument("--no-remat", action="store_true")
+    ap.add_argument("--d-head", type=int, default=None,
+                    help="variant row of reading A3: d_head = d_model / n_heads = 32 for the 32-head configs (d_attn 1024)")
     ap.add_argument("--partition", default="equal", choices=["equal", "cost"],
                     help="equal: L/K consecutive layers per cell; cost: minimum variance of the estimated cell costs (PAPER.md:65)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--oracle-full", action="store_true",
+                    help="cpu_baseline / --impl reference: one WHOLE oracle step of the workload instead of the bounded "
+                         "sample (config 2: minutes; BASELINE.md section 3)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -318,9 +409,22 @@ def main():
         w = w.replace(K=args.K)
     if args.no_remat:
         w = w.replace(remat=False)
+    if args.d_head:
+        w = w.replace(d_head=args.d_head, name="%s d_head=%d" % (w.name, args.d_head))
     if args.impl == "reference":
         run_reference(args, w, rank, world)
         return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # plain `python bench.py --gpus N`: start the N replica ranks ourselves, one per GPU, over NCCL
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        sys.exit(subprocess.call(cmd))
+    if world != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE is %d" % (args.gpus, world))
     if world > 1:
         import torch.distributed as dist
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")

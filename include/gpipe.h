@@ -75,7 +75,7 @@ typedef struct gpipe gpipe_t;   /* opaque handle, owned by the library */
 typedef struct {
   int32_t n_layers;     /* L >= 0                                                              */
   int32_t d_model;      /* d, multiple of 4 (bf16 mode: multiple of 64)                        */
-  int32_t d_ffn;        /* H                                                                   */
+  int32_t d_ffn;        /* H, multiple of 4 (bf16 mode: multiple of 32)                        */
   int32_t n_heads;      /* A                                                                   */
   int32_t d_head;       /* 0 -> d_model / n_heads.  Supported: 16, 32, 64, 128                 */
   int32_t vocab;        /* V                                                                   */
@@ -179,6 +179,17 @@ int gpipe_get_param(gpipe_t *g, int i, float *host_out);
 int gpipe_set_param(gpipe_t *g, int i, const float *host_in);
 int gpipe_get_grad(gpipe_t *g, int i, float *host_out);
 
+/* Exact training state, for checkpoint / resume (a step is deterministic, so save -> restore -> step reproduces an
+ * uninterrupted run bit for bit).  gpipe_get_master / gpipe_set_master move the fp32 MASTER copy of tensor i with
+ * no rounding (bf16 mode: set_master re-derives the bf16 working copy as RNE(master); fp32 mode: same as
+ * get/set_param).  gpipe_get_optimizer_slot / gpipe_set_optimizer_slot move the RMSProp second-moment slot of
+ * tensor i (GPIPE_EINVAL until gpipe_attach_optimizer_slots was called).  host_out / host_in: HOST fp32
+ * [rows*cols]. */
+int gpipe_get_master(gpipe_t *g, int i, float *host_out);
+int gpipe_set_master(gpipe_t *g, int i, const float *host_in);
+int gpipe_get_optimizer_slot(gpipe_t *g, int i, float *host_out);
+int gpipe_set_optimizer_slot(gpipe_t *g, int i, const float *host_in);
+
 /* Peak-HBM tracker: bytes the engine holds at its high-water mark, total, by category
  * (by_category[GPIPE_NUM_CATS], may be NULL) and by cell (by_cell[K], activations and scratch
  * owned by that cell; may be NULL). */
@@ -204,7 +215,9 @@ int gpipe_kernel_stats(const gpipe_t *g, int cls, const char **name, int64_t *co
 int64_t gpipe_launch_count(const gpipe_t *g);
 
 /* Debug/verification taps for the per-kernel parity tests: copies a named device buffer of the
- * LAST executed (cell k, micro-batch m) task to host as fp32.  Names: see DESIGN.md. */
+ * LAST executed (cell k, micro-batch m) task to host as fp32.  layer >= 0: "a", "qkv", "o", "c", "h", "x1",
+ * "lse", and "hbits" - the bit-packed ReLU pattern [h > 0] (bit n%32 of word n/32, [T_mb, ceil(H/32)] uint32
+ * words copied bit-exact into the 4-byte slots of host_out; reading A14 (iii)).  layer < 0: "y", "dlogits", "x_out". */
 int gpipe_debug_read(gpipe_t *g, const char *what, int layer, float *host_out, int64_t max_elems,
                      int64_t *n_elems);
 

@@ -38,7 +38,9 @@ extern "C" {
 
 /* C[M,N] = epilogue(op(A)[M,K] op(B)[K,N]), fp32 accumulation.  transA = 0: A stored [M,K]
  * row-major, 1: stored [K,M]; transB = 0: B stored [K,N], 1: stored [N,K].  backend: 0 = auto
- * (tcgen05 tensor cores for bf16 when the shape is tile-aligned), 1 = fp32-FMA SIMT kernel,
+ * (tcgen05 tensor cores for bf16 - a bf16 problem the tensor-core kernel cannot take, i.e. an
+ * unaligned base / row pitch or N % 32 != 0 with a ReLU pattern, fails with GPIPE_EINVAL; the SIMT
+ * kernel for fp32), 1 = fp32-FMA SIMT kernel,
  * 2 = tcgen05 or fail with GPIPE_EINVAL.  colsum_out fp32 [N] / colsum_scratch fp32
  * [gpipe_op_colsum_scratch_floats(M, N)] are only read with GPIPE_EPI_COLSUM.
  * workspace (device, may be NULL): gpipe_op_gemm_workspace_bytes(M, N, K) bytes that were ZERO before
@@ -50,17 +52,6 @@ int gpipe_op_gemm(void *stream, int dtype, int M, int N, int K, const void *A, i
                   const void *B, int64_t ldb, int transB, void *C, int64_t ldc, const float *bias,
                   const float *resid, void *mask, int64_t ldmask, float *colsum_out,
                   float *colsum_scratch, void *workspace, int64_t workspace_bytes, int flags, int backend);
-
-/* Profiling hook (not on the product path): while dev_buf != NULL every tcgen05 GEMM launch writes 8
- * %globaltimer stamps (ns) per CTA to dev_buf[blockIdx * 32 + i] - kernel entry, prologue done, first
- * operands landed, all MMAs issued, first accumulator complete, last output chunk handed to the TMA,
- * stores complete, exit - followed by 24 SM-clock stamps of the first tile's epilogue chunks (4 per chunk:
- * accumulator in registers, staged in shared memory, fenced, handed to the TMA).  dev_buf: device memory,
- * 32 * SM-count uint64, owned by the caller; pass NULL
- * to switch the probe off.  Process-global, not thread-safe.  Always returns GPIPE_OK. */
-int gpipe_op_gemm_timeline(void *dev_buf);
-/* Same for the tcgen05 attention backward kernel: 32 %globaltimer stamps per (sequence, head) CTA; NULL disables. */
-int gpipe_op_attn_timeline(void *dev_buf);
 
 /* y = LayerNorm(x) * gamma + beta over the last axis (biased variance); y lp [n_tok,d]; x fp32.
  * Fused residual: if resid_out != NULL (fp32 [n_tok,d], device, caller-owned)

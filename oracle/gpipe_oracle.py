@@ -24,7 +24,10 @@ A matmul is numpy's `@`; there is no blocking, fusion or reordering beyond that.
 
 `round_operands=True` additionally applies bf16 round-to-nearest-even at the points where the
 bf16 CUDA path *stores* a tensor in bf16; it is the same
-code plus one rounding function and is only used to report the bf16 noise floor (reading A14).
+code plus one rounding function and is only used to report the bf16 noise floor (reading A14:
+tests/golden/make_bf16_floor.py -> tests/golden/bf16_floor.json).  Pinned by
+test_round_operands_mode_matches_independent_straight_through_model: an independent torch-autograd
+model with torch's own bf16 conversion applied straight-through to the listed tensors.
 
 Pins: see tests/test_oracle_pins.py - Table 1 parameter counts, section 5
 model sizes, fp64 finite differences, M/K invariance, remat == stored,

@@ -80,6 +80,10 @@ def lib() -> C.CDLL:
         "gpipe_get_param": (i32, [vp, i32, vp]),
         "gpipe_set_param": (i32, [vp, i32, vp]),
         "gpipe_get_grad": (i32, [vp, i32, vp]),
+        "gpipe_get_master": (i32, [vp, i32, vp]),
+        "gpipe_set_master": (i32, [vp, i32, vp]),
+        "gpipe_get_optimizer_slot": (i32, [vp, i32, vp]),
+        "gpipe_set_optimizer_slot": (i32, [vp, i32, vp]),
         "gpipe_peak_bytes": (i32, [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]),
         "gpipe_trace": (i32, [vp, i32, C.POINTER(TraceEvent), C.POINTER(i64)]),
         "gpipe_launch_count": (i64, [vp]),
@@ -91,8 +95,6 @@ def lib() -> C.CDLL:
         "gpipe_version": (C.c_char_p, []),
         "gpipe_op_gemm": (i32, [vp, i32, i32, i32, i32, vp, i64, i32, vp, i64, i32, vp, i64, vp, vp, vp, i64, vp, vp, vp, i64, i32, i32]),
         "gpipe_op_gemm_workspace_bytes": (i64, [i32, i32, i32]),
-        "gpipe_op_gemm_timeline": (i32, [vp]),
-        "gpipe_op_attn_timeline": (i32, [vp]),
         "gpipe_op_ln_fwd": (i32, [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, i64, i32, f32]),
         "gpipe_op_ln_bwd_scratch_floats": (i64, [i32]),
         "gpipe_op_ln_bwd": (i32, [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, i32]),
@@ -120,9 +122,10 @@ EXPORTED_SYMBOLS = [
     "gpipe_create_partitioned", "gpipe_cell_range", "gpipe_init_params", "gpipe_step",
     "gpipe_step_device", "gpipe_apply_sgd", "gpipe_optimizer_slot_bytes", "gpipe_attach_optimizer_slots",
     "gpipe_apply_rmsprop", "gpipe_op_rmsprop", "gpipe_zero_grads", "gpipe_num_tensors",
-    "gpipe_tensor_info", "gpipe_get_param", "gpipe_set_param", "gpipe_get_grad", "gpipe_peak_bytes",
+    "gpipe_tensor_info", "gpipe_get_param", "gpipe_set_param", "gpipe_get_grad", "gpipe_get_master", "gpipe_set_master",
+    "gpipe_get_optimizer_slot", "gpipe_set_optimizer_slot", "gpipe_peak_bytes",
     "gpipe_trace", "gpipe_launch_count", "gpipe_kernel_timing", "gpipe_kernel_stats", "gpipe_debug_read", "gpipe_last_error", "gpipe_version",
-    "gpipe_op_gemm", "gpipe_op_gemm_workspace_bytes", "gpipe_op_gemm_timeline", "gpipe_op_attn_timeline", "gpipe_op_ln_fwd", "gpipe_op_ln_bwd_scratch_floats", "gpipe_op_ln_bwd",
+    "gpipe_op_gemm", "gpipe_op_gemm_workspace_bytes", "gpipe_op_ln_fwd", "gpipe_op_ln_bwd_scratch_floats", "gpipe_op_ln_bwd",
     "gpipe_op_attn_fwd", "gpipe_op_attn_bwd", "gpipe_op_softmax_ce", "gpipe_op_colsum",
     "gpipe_op_colsum_scratch_floats",
     "gpipe_op_embed_fwd", "gpipe_op_embed_bwd", "gpipe_op_positional", "gpipe_op_sgd",
@@ -273,12 +276,16 @@ class GPipe:
     def apply_rmsprop(self, lr: float, rho: float = 0.9, eps: float = 1e-8):
         """RMSProp; the fp32 slot (4 B / parameter) is allocated on first use."""
         with self._torch.cuda.device(self.device):
+            self._ensure_slots()
+            _check(lib().gpipe_apply_rmsprop(self._h, lr, rho, eps))
+
+    def _ensure_slots(self):
+        with self._torch.cuda.device(self.device):
             if getattr(self, "_slots", None) is None:
                 n = C.c_size_t(0)
                 _check(lib().gpipe_optimizer_slot_bytes(self._h, C.byref(n)))
                 self._slots = self._torch.empty(n.value, dtype=self._torch.uint8, device=self.device)
                 _check(lib().gpipe_attach_optimizer_slots(self._h, self._slots.data_ptr(), n.value))
-            _check(lib().gpipe_apply_rmsprop(self._h, lr, rho, eps))
 
     def apply_sgd(self, lr: float):
         with self._torch.cuda.device(self.device):
@@ -304,6 +311,42 @@ class GPipe:
 
     def get_grad(self, key) -> np.ndarray:
         return self._get(lib().gpipe_get_grad, key)
+
+    def get_master(self, key) -> np.ndarray:
+        """fp32 master copy, every bit (checkpointing)."""
+        return self._get(lib().gpipe_get_master, key)
+
+    def get_optimizer_slot(self, key) -> np.ndarray:
+        return self._get(lib().gpipe_get_optimizer_slot, key)
+
+    def _set(self, fn, key, value):
+        i = self._idx(key)
+        a = np.ascontiguousarray(value, dtype=np.float32)
+        if a.size != self.shapes[self.names[i]][0] * self.shapes[self.names[i]][1]:
+            raise ValueError("wrong size for %s" % self.names[i])
+        with self._torch.cuda.device(self.device):
+            _check(fn(self._h, i, a.ctypes.data))
+
+    def set_master(self, key, value):
+        self._set(lib().gpipe_set_master, key, value)
+
+    def set_optimizer_slot(self, key, value):
+        self._ensure_slots()
+        self._set(lib().gpipe_set_optimizer_slot, key, value)
+
+    def state_dict(self) -> Dict[str, Dict[str, np.ndarray]]:
+        """Exact training state: fp32 masters (+ RMSProp slots once they exist)."""
+        out = {"master": {n: self.get_master(n) for n in self.names}}
+        if getattr(self, "_slots", None) is not None:
+            out["slot"] = {n: self.get_optimizer_slot(n) for n in self.names}
+        return out
+
+    def load_state_dict(self, state):
+        for n in self.names:
+            self.set_master(n, state["master"][n])
+        if "slot" in state:
+            for n in self.names:
+                self.set_optimizer_slot(n, state["slot"][n])
 
     def set_param(self, key, value):
         i = self._idx(key)

@@ -33,10 +33,12 @@ static int cuda_fail(cudaError_t e, const char *where) {
     if (e__ != cudaSuccess) return cuda_fail(e__, where); \
   } while (0)
 
+#if GP_PROBES
 static int env_int(const char *name, int dflt) {
   const char *v = getenv(name);
   return v && *v ? atoi(v) : dflt;
 }
+#endif
 
 // fills the shape fields of an Engine from the spec; no CUDA calls
 static int configure(Engine &e, const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs,
@@ -52,7 +54,8 @@ static int configure(Engine &e, const gpipe_layer_spec *spec, int K, int M, int 
   if (e.dh != 16 && e.dh != 32 && e.dh != 64 && e.dh != 128) return fail(GPIPE_EINVAL, "d_head must be 16, 32, 64 or 128");
   e.da = e.A * e.dh;
   if (e.d % 4 || e.H % 4 || e.V % 4 || e.d > 2048) return fail(GPIPE_EINVAL, "d_model, d_ffn, vocab must be multiples of 4 and d_model <= 2048");
-  if (e.dt == GPIPE_DTYPE_BF16 && (e.d % 8 || e.H % 8 || e.V % 8)) return fail(GPIPE_EINVAL, "bf16 mode needs d_model, d_ffn, vocab multiples of 8");
+  if (e.dt == GPIPE_DTYPE_BF16 && (e.d % 8 || e.H % 32 || e.V % 8))
+    return fail(GPIPE_EINVAL, "bf16 mode needs d_model and vocab multiples of 8 and d_ffn a multiple of 32 (TMA row pitches; bit-packed ReLU pattern)");
   e.eps = spec->ln_eps > 0.f ? spec->ln_eps : 1e-5f;
   int L = spec->n_layers;
   if (K < 1 || K > (L > 1 ? L : 1)) return fail(GPIPE_EINVAL, "need 1 <= K <= max(L, 1)");
@@ -77,8 +80,10 @@ static int configure(Engine &e, const gpipe_layer_spec *spec, int K, int M, int 
       e.cell_hi[k] = cell_lo[k + 1];
     }
   }
+#if GP_PROBES                                 // A/B switches of the debug build only
   e.gemm_backend = env_int("GPIPE_GEMM_SIMT", 0);
   e.replay_full = env_int("GPIPE_REPLAY_FULL", 0);
+#endif
   std::string err;
   e.build_inventory(err);
   return GPIPE_OK;
@@ -185,6 +190,7 @@ static int create_impl(const gpipe_layer_spec *spec, int K, int M, int remat, in
   if ((uintptr_t)env->arena % 1024) { delete g; return fail(GPIPE_EINVAL, "arena must be 1024-byte aligned"); }
   int dev = 0;
   cudaError_t ce = cudaGetDevice(&dev);
+  e.device = dev;
   if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&e.sm_count, cudaDevAttrMultiProcessorCount, dev);
   int cc_major = 0;
   if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev);
@@ -408,6 +414,53 @@ int gpipe_set_param(gpipe_t *g, int i, const float *host_in) {
   return GPIPE_OK;
 }
 
+// ---- exact state access for checkpoint / resume: no rounding anywhere -------------------------------------------
+int gpipe_get_master(gpipe_t *g, int i, float *host_out) {
+  int rc = tensor_check(g, i, host_out);
+  if (rc) return rc;
+  Engine &e = g->e;
+  const TensorInfo &t = e.tensors[i];
+  API_CUDA(cudaMemcpyAsync(host_out, e.master + t.off, (size_t)(t.rows * t.cols) * 4, cudaMemcpyDeviceToHost, e.streams[0]), "gpipe_get_master");
+  API_CUDA(cudaStreamSynchronize(e.streams[0]), "gpipe_get_master");
+  return GPIPE_OK;
+}
+
+int gpipe_set_master(gpipe_t *g, int i, const float *host_in) {
+  int rc = tensor_check(g, i, host_in);
+  if (rc) return rc;
+  Engine &e = g->e;
+  const TensorInfo &t = e.tensors[i];
+  int64_t n = t.rows * t.cols;
+  Ctx c = e.ctx(0);
+  API_CUDA(cudaMemcpyAsync(e.master + t.off, host_in, (size_t)n * 4, cudaMemcpyHostToDevice, c.stream), "gpipe_set_master");
+  if (e.dt == GP_BF16)   // working copy = RNE(master); the master keeps every bit
+    API_CUDA(master_to_lp(c, e.dt, e.master + t.off, (char *)e.w_lp + t.off * 2, n, 0), "gpipe_set_master");
+  API_CUDA(cudaStreamSynchronize(c.stream), "gpipe_set_master");
+  return GPIPE_OK;
+}
+
+int gpipe_get_optimizer_slot(gpipe_t *g, int i, float *host_out) {
+  int rc = tensor_check(g, i, host_out);
+  if (rc) return rc;
+  Engine &e = g->e;
+  if (!e.opt_ms) return fail(GPIPE_EINVAL, "no optimizer slots attached");
+  const TensorInfo &t = e.tensors[i];
+  API_CUDA(cudaMemcpyAsync(host_out, e.opt_ms + t.off, (size_t)(t.rows * t.cols) * 4, cudaMemcpyDeviceToHost, e.streams[0]), "gpipe_get_optimizer_slot");
+  API_CUDA(cudaStreamSynchronize(e.streams[0]), "gpipe_get_optimizer_slot");
+  return GPIPE_OK;
+}
+
+int gpipe_set_optimizer_slot(gpipe_t *g, int i, const float *host_in) {
+  int rc = tensor_check(g, i, host_in);
+  if (rc) return rc;
+  Engine &e = g->e;
+  if (!e.opt_ms) return fail(GPIPE_EINVAL, "no optimizer slots attached");
+  const TensorInfo &t = e.tensors[i];
+  API_CUDA(cudaMemcpyAsync(e.opt_ms + t.off, host_in, (size_t)(t.rows * t.cols) * 4, cudaMemcpyHostToDevice, e.streams[0]), "gpipe_set_optimizer_slot");
+  API_CUDA(cudaStreamSynchronize(e.streams[0]), "gpipe_set_optimizer_slot");
+  return GPIPE_OK;
+}
+
 int gpipe_get_grad(gpipe_t *g, int i, float *host_out) {
   int rc = tensor_check(g, i, host_out);
   if (rc) return rc;
@@ -493,6 +546,8 @@ int gpipe_debug_read(gpipe_t *g, const char *what, int layer, float *host_out, i
     else if (w == "h") { src = b.h; n = T * e.H; }
     else if (w == "x1") { src = b.x1; n = T * e.d; is_lp = false; }
     else if (w == "lse") { src = b.lse; n = T * e.A; is_lp = false; }
+    // the bit-packed ReLU pattern [h > 0] FFN1's epilogue wrote: uint32 words, returned bit-exact in the fp32 slots
+    else if (w == "hbits") { src = b.hbits; n = T * (int64_t)((e.H + 31) / 32); is_lp = false; }
   } else {
     if (w == "y") { src = ws.y; n = T * e.d; }
     else if (w == "dlogits") { src = ws.logits; n = T * e.V; }

@@ -41,7 +41,11 @@ using namespace tc;
 constexpr int DH = 64;
 constexpr uint32_t TILE = 128 * 128;          // bytes of a [128 rows x 64 bf16] swizzled tile
 constexpr float LOG2E = 1.4426950408889634f;
+#if GP_PROBES
 static unsigned long long *g_attn_tl = nullptr;     // host: timeline buffer handed to the next launches
+#else
+constexpr unsigned long long *g_attn_tl = nullptr;
+#endif
 
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1, int c2) {
   asm volatile(
@@ -91,11 +95,15 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
   extern __shared__ uint8_t smem_raw[];
   // optional timeline probe (attn_tc_set_timeline): 8 %globaltimer stamps per CTA, written by thread 0
   auto stamp = [&](int slot) {
+#if GP_PROBES
     if (tl && threadIdx.x == 0) {
       unsigned long long t;
       asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
       tl[((size_t)blockIdx.y * gridDim.x + blockIdx.x) * 8 + slot] = t;
     }
+#else
+    (void)slot; (void)tl;
+#endif
   };
   stamp(0);
   __shared__ __align__(8) uint64_t bars[4];
@@ -280,11 +288,15 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
   __shared__ __align__(8) uint64_t bars[5];
   // optional timeline probe (attn_tc_set_timeline): 32 %globaltimer stamps per CTA
   auto stamp = [&](int slot) {
+#if GP_PROBES
     if (tl) {
       unsigned long long t;
       asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
       tl[(size_t)blockIdx.x * 32 + slot] = t;
     }
+#else
+    (void)slot; (void)tl;
+#endif
   };
   __shared__ uint32_t tmem_base_smem;
   __shared__ float Lsm[256], Dsm[256];
@@ -605,7 +617,9 @@ static bool get_map3(const void *ptr, int64_t width, int64_t S, int64_t n_seq, i
 // 0 start, 1 operands landed, 2+3n / 3+3n / 4+3n: pair n registers pulled / panels written / products
 // issued; compute thread 0: 16 D done, 17+3n / 18+3n / 19+3n: pair n S,dP ready / pulled / panels
 // written, 30 last store issued, 31 stores complete).  buf: 32 * n_seq * A uint64.
+#if GP_PROBES
 void attn_tc_set_timeline(unsigned long long *buf) { fat::g_attn_tl = buf; }
+#endif
 
 cudaError_t attn_tc_set_watchdog(unsigned long long *mapped) {
   return cudaMemcpyToSymbol(tc::g_watchdog, &mapped, sizeof(mapped));
@@ -621,11 +635,10 @@ cudaError_t attn_fwd_tc(const Ctx &c, const void *qkv, void *o, float *lse, int 
   const int da = A * fat::DH;
   CUtensorMap mq;
   if (!fat::get_map3(qkv, 3 * da, S, n_seq, 128, &mq)) return cudaErrorInvalidValue;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(fat::attn_fwd_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fat::FWD_SMEM);
+  if ((int64_t)n_seq * A > 65535) return cudaErrorInvalidValue;       // grid.y
+  {
+    cudaError_t e = ensure_dyn_smem<fat::attn_fwd_tc_kernel>(fat::FWD_SMEM, c.device);
     if (e != cudaSuccess) return e;
-    attr_set = true;
   }
   dim3 grid((S + 127) / 128, n_seq * A);
   fat::attn_fwd_tc_kernel<<<grid, fat::FWD_THREADS, fat::FWD_SMEM, c.stream>>>(mq, (bf16 *)o, lse, S, A, causal,
@@ -639,11 +652,9 @@ cudaError_t attn_bwd_tc(const Ctx &c, const void *qkv, const void *o, const void
   const int da = A * fat::DH;
   CUtensorMap mq, md;
   if (!fat::get_map3(qkv, 3 * da, S, n_seq, 128, &mq) || !fat::get_map3(d_o, da, S, n_seq, 128, &md)) return cudaErrorInvalidValue;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(fat::attn_bwd_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fat::BWD_SMEM);
+  {
+    cudaError_t e = ensure_dyn_smem<fat::attn_bwd_tc_kernel>(fat::BWD_SMEM, c.device);
     if (e != cudaSuccess) return e;
-    attr_set = true;
   }
   fat::attn_bwd_tc_kernel<<<n_seq * A, fat::BWD_THREADS, fat::BWD_SMEM, c.stream>>>(
       mq, md, (const bf16 *)o, (const bf16 *)d_o, lse, (bf16 *)dqkv, S, A, causal, 1.f / sqrtf((float)fat::DH), fat::g_attn_tl);

@@ -4,17 +4,38 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+
 #include "ops.h"
 
 namespace gp {
 
 typedef __nv_bfloat16 bf16;
 
+// Debug instrumentation (timeline probes inside the tcgen05 kernels, getenv A/B switches, the
+// gpipe_op_*_timeline entry points) is compiled only with -DGP_PROBES=1
+// (GPIPE_NVCC_EXTRA="-DGP_PROBES=1" python -m paper_1811_06965_b200.build --force); off by default.
+#ifndef GP_PROBES
+#define GP_PROBES 0
+#endif
+
 #define GP_LAUNCH_CHECK(c)                      \
   do {                                          \
     if ((c).launches) ++*(c).launches;          \
     return cudaGetLastError();                  \
   } while (0)
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute: set it once per (kernel, device), off the
+// launch path afterwards.  One bit per device ordinal; a lost race only repeats an idempotent call.
+template <auto Kern>
+inline cudaError_t ensure_dyn_smem(size_t bytes, int device) {
+  static std::atomic<uint64_t> done{0};
+  const uint64_t bit = 1ull << (device & 63);
+  if (done.load(std::memory_order_acquire) & bit) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(Kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+  if (e == cudaSuccess) done.fetch_or(bit, std::memory_order_release);
+  return e;
+}
 
 template <typename T> __device__ __forceinline__ float to_f(T v);
 template <> __device__ __forceinline__ float to_f<float>(float v) { return v; }

@@ -109,7 +109,7 @@ int Engine::build_plan(bool dry, std::string &err) {
                              {T, da, d}, {T, d, 3 * da}, {T, d, V},                                 // dgrad (others as forward)
                              {H, d, T}, {d, H, T}, {da, d, T}, {d, 3 * da, T}, {d, V, T}};            // wgrad
     for (auto &sh : shapes) {
-      size_t b = gemm_splitk_ws_bytes(sh[0], sh[1], sh[2], sm_count);
+      size_t b = gemm_splitk_ws_bytes(sh[0], sh[1], sh[2], kPlanSmCount);
       if (b > splitk_ws_bytes) splitk_ws_bytes = b;
     }
   }
@@ -160,7 +160,7 @@ int Engine::build_plan(bool dry, std::string &err) {
     s.d_o = LP(Tm * da, cat, k);
     s.dqkv = LP(Tm * 3 * da, cat, k);
     s.dvec = F32(Tm * A, cat, k);
-    s.ln_partials = F32((size_t)ln_bwd_partial_rows(sm_count) * 3 * d, cat, k);
+    s.ln_partials = F32((size_t)ln_bwd_partial_rows(kPlanSmCount) * 3 * d, cat, k);
     {
       size_t rows = (Tm + 127) / 128;
       if (rows < (size_t)colsum_scratch_rows(T_mb)) rows = colsum_scratch_rows(T_mb);
@@ -180,8 +180,12 @@ int Engine::build_plan(bool dry, std::string &err) {
 
 cudaEvent_t Engine::pool_event() {
   if (ev_pool_used == ev_pool.size()) {
-    cudaEvent_t e;
-    cudaEventCreate(&e);
+    cudaEvent_t e = nullptr;
+    cudaError_t err = cudaEventCreate(&e);
+    if (err != cudaSuccess) {
+      pool_err = err;
+      return nullptr;
+    }
     ev_pool.push_back(e);
   }
   return ev_pool[ev_pool_used++];
@@ -423,6 +427,7 @@ cudaError_t Engine::run_step(float *loss_out) {
     if (trace_on) {
       r.e0 = pool_event();
       r.e1 = pool_event();
+      if (!r.e0 || !r.e1) return pool_err;
       GP_TRY(cudaEventRecord(r.e0, st(k)));
     }
     cudaError_t e = kind == 'B' ? backward_cell(k, m) : forward_cell(k, m, kind == 'R');

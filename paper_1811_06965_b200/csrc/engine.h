@@ -75,7 +75,11 @@ struct Engine {
   int64_t n_seqs = 0, nb = 0, T_mb = 0, T_total = 0;   // nb = sequences per micro-batch
   int d = 0, H = 0, A = 0, dh = 0, da = 0, V = 0, S = 0;
   float eps = 1e-5f;
-  int sm_count = 148;
+  int sm_count = 148;                                  // of the device the handle lives on (launch geometry)
+  // The memory plan must not depend on the device (gpipe_plan_bytes is host-only): scratch whose size follows the
+  // launch geometry is planned for this fixed SM-count bound and the launchers clamp to what was planned.
+  static constexpr int kPlanSmCount = 148;
+  int device = 0;
   int gemm_backend = 0;
   int replay_full = 0;
   size_t splitk_ws_bytes = 0;
@@ -122,6 +126,7 @@ struct Engine {
   cudaError_t timed(int k, int cls, double flops, double bytes, F &&fn) {
     if (!ktiming_on) return fn();
     KRec r{cls, flops, bytes, pool_event(), pool_event()};
+    if (!r.e0 || !r.e1) return pool_err;
     cudaError_t e = cudaEventRecord(r.e0, st(k));
     if (e != cudaSuccess) return e;
     e = fn();
@@ -135,7 +140,7 @@ struct Engine {
   int build_inventory(std::string &err);
   int build_plan(bool dry, std::string &err);
   // -- helpers --
-  Ctx ctx(int k) { return Ctx{st(k), &launches, sm_count, gemm_backend}; }
+  Ctx ctx(int k) { return Ctx{st(k), &launches, sm_count, gemm_backend, device}; }
   float *P(int i) const { return master + tensors[i].off; }            // fp32 vector param
   const void *W(int i) const {                                         // matrix operand
     return dt == GP_BF16 ? (const void *)((const char *)w_lp + tensors[i].off * 2)
@@ -147,7 +152,8 @@ struct Engine {
   cudaError_t forward_cell(int k, int m, bool replay);
   cudaError_t backward_cell(int k, int m);
   cudaError_t run_step(float *loss_out);
-  cudaEvent_t pool_event();
+  cudaEvent_t pool_event();                            // nullptr (and pool_err set) when cudaEventCreate fails
+  cudaError_t pool_err = cudaSuccess;
 };
 
 }  // namespace gp

@@ -63,9 +63,12 @@ struct Params {
   int splits, kb_per_split;
   float *ws_part;               // [tile][split][rank][128][BN] fp32
   unsigned int *ws_cnt;         // [tile][rank][2]: arrivals, partials ready
+#if GP_PROBES
   unsigned long long *tl;       // optional timeline probe: 8 globaltimer stamps per CTA (gemm_tc_set_timeline)
+#endif
 };
 
+#if GP_PROBES
 __device__ __forceinline__ void tl_stamp(const Params &p, int slot) {
   if (p.tl) {
     unsigned long long t;
@@ -77,6 +80,10 @@ __device__ __forceinline__ void tl_stamp(const Params &p, int slot) {
 __device__ __forceinline__ void tl_clock(const Params &p, bool on, int c, int which) {
   if (p.tl && on && c < 6) p.tl[(size_t)blockIdx.x * 32 + 8 + c * 4 + which] = (unsigned long long)clock64();
 }
+#else
+__device__ __forceinline__ void tl_stamp(const Params &, int) {}
+__device__ __forceinline__ void tl_clock(const Params &, bool, int, int) {}
+#endif
 
 // STG: staging buffers ([32 rows x 128 B]) per epilogue warp.  Dynamic shared memory: operand ring,
 // staging, bias (2 x BN floats), column-sum exchange (4 x BN floats), 1 KB alignment slack.
@@ -159,9 +166,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
   // BOTH CTAs have returned their columns: a pair dealloc that lands after the peer's SM already hosts
   // a CTA of another TMEM-using kernel wedges that SM's allocator (observed as a later kernel stuck
   // in its prologue).
-#ifndef GP_GEMM_NO_PRESYNC
   cluster_sync_all();
-#endif
   if (warp == 2) {
     asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_smem)),
                  "n"(Cfg::TMEM_COLS));
@@ -519,9 +524,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
     tcgen05_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(Cfg::TMEM_COLS));
   }
-#ifndef GP_GEMM_NO_POSTSYNC
   cluster_sync_all();                                  // no CTA of the pair exits before both deallocations
-#endif
 }
 
 // ------------------------------------------------------------------------------------------
@@ -598,8 +601,11 @@ static bool get_map(const void *ptr, uint32_t esize, uint64_t inner, uint64_t ou
 // (dlogits W_out^T, K = V) win back - measured: K = 2048 20.5 us unsplit vs 43.6 us split, K = 6144
 // 37.1 vs 54.5, K = 16384 86.4 vs 84.7, K = 64000 296.6 vs 207.1.  All units run in ONE wave.
 static int splitk_factor(int tiles, int num_kb, int pairs) {
+#if GP_PROBES
   static const int off = getenv("GPIPE_NO_SPLITK") ? atoi(getenv("GPIPE_NO_SPLITK")) : 0;
-  if (off || tiles * 2 > pairs) return 1;
+  if (off) return 1;
+#endif
+  if (tiles * 2 > pairs) return 1;
   int s = pairs / tiles;
   if (s > 4) s = 4;
   while (s > 1 && num_kb / s < 192) --s;
@@ -607,7 +613,9 @@ static int splitk_factor(int tiles, int num_kb, int pairs) {
 }
 static size_t splitk_cnt_bytes(int tiles) { return (((size_t)tiles * 2 * 2 * sizeof(unsigned int)) + 1023) & ~(size_t)1023; }
 
+#if GP_PROBES
 static unsigned long long *g_timeline = nullptr;
+#endif
 
 template <int BN, int STG, int F>
 static cudaError_t launch_pair(const Ctx &c, const GemmArgs &a) {
@@ -621,13 +629,21 @@ static cudaError_t launch_pair(const Ctx &c, const GemmArgs &a) {
   p.colpart = a.colsum_scratch;
   p.tiles_m = (a.M + 255) / 256;
   p.tiles_n = (a.N + BN - 1) / BN;
-  const int pairs = c.sm_count / 2;
+  int pairs = c.sm_count / 2;
+#if GP_PROBES
+  {                                                  // experiment knob: run on fewer CTA pairs
+    static const int lim = getenv("GPIPE_GEMM_PAIRS") ? atoi(getenv("GPIPE_GEMM_PAIRS")) : 0;
+    if (lim > 0 && lim < pairs) pairs = lim;
+  }
+#endif
   const int num_kb = (a.K + BK - 1) / BK;
   p.splits = F >= 0 ? 1 : splitk_factor(p.tiles_m * p.tiles_n, num_kb, pairs);
   if (p.splits > 1 && (!a.ws || a.ws_bytes < gemm_splitk_ws_bytes(a.M, a.N, a.K, c.sm_count))) p.splits = 1;
   p.kb_per_split = (num_kb + p.splits - 1) / p.splits;
   p.splits = (num_kb + p.kb_per_split - 1) / p.kb_per_split;             // no empty split
+#if GP_PROBES
   p.tl = g_timeline;
+#endif
   p.ws_cnt = (unsigned int *)a.ws;
   p.ws_part = (float *)((char *)a.ws + splitk_cnt_bytes(p.tiles_m * p.tiles_n));
   const bool out_f32 = (a.flags & (EPI_OUT_F32 | EPI_ACCUM)) != 0;
@@ -642,12 +658,9 @@ static cudaError_t launch_pair(const Ctx &c, const GemmArgs &a) {
   // C: boxes of 32 rows x 128 bytes (32 fp32 / 64 bf16 columns), written from swizzled staging
   ok = get_map(a.C, out_f32 ? 4 : 2, (uint64_t)a.N, (uint64_t)a.M, (uint64_t)a.ldc, out_f32 ? 32 : 64, 32, &mc);
   if (!ok) return cudaErrorInvalidValue;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(gemm_tcgen05_pair_kernel<BN, STG, F>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)Cfg::SMEM);
+  {
+    cudaError_t e = ensure_dyn_smem<gemm_tcgen05_pair_kernel<BN, STG, F>>(Cfg::SMEM, c.device);
     if (e != cudaSuccess) return e;
-    attr_set = true;
   }
   int units = p.tiles_m * p.tiles_n * p.splits;
   int grid = 2 * (units < pairs ? units : pairs);
@@ -661,7 +674,9 @@ static cudaError_t launch_pair(const Ctx &c, const GemmArgs &a) {
 // (entry, prologue done, first operands landed, all MMAs issued, first accumulator complete, last
 // chunk handed to the TMA, stores complete, exit) plus 24 SM-clock stamps of the first tile's epilogue
 // chunks.  buf must hold 32 * SM-count uint64.
+#if GP_PROBES
 void gemm_tc_set_timeline(unsigned long long *buf) { tc::g_timeline = buf; }
+#endif
 cudaError_t gemm_tc_set_watchdog(unsigned long long *mapped) {
   return cudaMemcpyToSymbol(tc::g_watchdog, &mapped, sizeof(mapped));
 }
@@ -693,7 +708,11 @@ bool gemm_tc_supported(int dt, const GemmArgs &a) {
 // The epilogue combinations the engine launches get their own instantiation; anything else (and every
 // split-K launch) takes the run-time-flag kernel.
 cudaError_t gemm_tc(const Ctx &c, const GemmArgs &a) {
+#if GP_PROBES
   static const int generic_only = getenv("GPIPE_GEMM_GENERIC") ? atoi(getenv("GPIPE_GEMM_GENERIC")) : 0;
+#else
+  constexpr int generic_only = 0;
+#endif
   const int tiles = ((a.M + 255) / 256) * ((a.N + 255) / 256);
   const bool split = a.ws && tc::splitk_factor(tiles, (a.K + tc::BK - 1) / tc::BK, c.sm_count / 2) > 1;
   if (!split && !generic_only) {

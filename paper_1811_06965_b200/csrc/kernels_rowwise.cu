@@ -298,7 +298,8 @@ ln_bwd_reduce_kernel(const float *__restrict__ partials, int n_part, int d, floa
   }
 }
 
-int ln_bwd_partial_rows(int sm_count) { return sm_count; }
+// one partial row per block, at most one block per SM and never more than the memory plan provides for (148)
+int ln_bwd_partial_rows(int sm_count) { return sm_count < 148 ? sm_count : 148; }
 
 template <typename T, int NV, int WARPS>
 static cudaError_t ln_bwd_launch(const Ctx &c, const T *dy, const float *x, const float *mean, const float *rstd,
@@ -308,8 +309,8 @@ static cudaError_t ln_bwd_launch(const Ctx &c, const T *dy, const float *x, cons
   int grid = (int)(want < ln_bwd_partial_rows(c.sm_count) ? want : ln_bwd_partial_rows(c.sm_count));
   size_t smem = (size_t)WARPS * 3 * d * sizeof(float);
   auto kern = ln_bwd_kernel<T, NV, WARPS>;
-  if (smem > 48 * 1024) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (smem > 48 * 1024) {                                  // once per device, for the widest row this instantiation takes
+    cudaError_t e = ensure_dyn_smem<ln_bwd_kernel<T, NV, WARPS>>((size_t)WARPS * 3 * 128 * NV * sizeof(float), c.device);
     if (e != cudaSuccess) return e;
   }
   kern<<<grid, WARPS * 32, smem, c.stream>>>(dy, x, mean, rstd, gamma, dres_in, dx_out, dx_out_lp, partials, n_tok, d,

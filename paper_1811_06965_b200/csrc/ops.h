@@ -15,7 +15,8 @@ struct Ctx {
   cudaStream_t stream;
   int64_t *launches;   // host counter, incremented once per kernel launch
   int sm_count;
-  int gemm_backend;    // 0 = auto (tcgen05 for bf16 when shape allows), 1 = force SIMT
+  int gemm_backend;    // 0 = auto (tcgen05 for bf16, SIMT for fp32), 1 = force SIMT, 2 = tcgen05 or fail
+  int device;          // CUDA device ordinal the stream belongs to (per-device function attributes)
 };
 
 inline size_t lp_size(int dt) { return dt == GP_BF16 ? 2 : 4; }

@@ -11,8 +11,10 @@
 namespace gp {
 cudaError_t gemm_simt(const Ctx &c, int dt, const GemmArgs &a);
 cudaError_t gemm_tc(const Ctx &c, const GemmArgs &a);
+#if GP_PROBES
 void gemm_tc_set_timeline(unsigned long long *buf);
 void attn_tc_set_timeline(unsigned long long *buf);
+#endif
 cudaError_t attn_fwd_simt(const Ctx &c, int dt, const void *qkv, void *o, float *lse, int n_seq,
                           int S, int A, int dh, int causal);
 cudaError_t attn_bwd_simt(const Ctx &c, int dt, const void *qkv, const void *o, const void *d_o,
@@ -59,10 +61,15 @@ const char *watchdog_describe() {
   return buf;
 }
 
-// GPIPE_ATTN_BACKEND=mma keeps the legacy mma.sync kernels (A/B comparisons); default: tcgen05 where it applies
+// tcgen05 attention where it applies (bf16, d_head 64, S <= 256); with -DGP_PROBES=1, GPIPE_ATTN_BACKEND=mma keeps
+// the mma.sync kernels for A/B comparisons
 static bool attn_use_tc() {
+#if GP_PROBES
   static const int v = [] { const char *e = getenv("GPIPE_ATTN_BACKEND"); return (e && std::string(e) == "mma") ? 0 : 1; }();
   return v != 0;
+#else
+  return true;
+#endif
 }
 
 cudaError_t gemm(const Ctx &c, int dt, const GemmArgs &a) {
@@ -76,7 +83,10 @@ cudaError_t gemm(const Ctx &c, int dt, const GemmArgs &a) {
     if (e != cudaSuccess || !colsum) return e;
     return colsum_reduce_partials(c, a.colsum_scratch, (a.M + 127) / 128, a.N, a.colsum_out);
   }
-  if (c.gemm_backend == 2) return cudaErrorNotSupported;
+  // bf16 operands belong on the tensor cores: a bf16 problem the tcgen05 kernel cannot take (unaligned base or
+  // pitch, N % 32 != 0 with a ReLU pattern) is an error, never a silent ~50x slower SIMT launch.  The SIMT kernel
+  // is the fp32 (TF32 off) path, or an explicit request (backend 1: the per-kernel tests).
+  if (c.gemm_backend == 2 || (dt == GP_BF16 && c.gemm_backend != 1)) return cudaErrorNotSupported;
   cudaError_t e = gemm_simt(c, dt, a);
   if (e != cudaSuccess || !colsum) return e;
   return colsum_accum(c, dt, a.C, a.ldc, a.colsum_out, a.colsum_scratch, a.M, a.N);
@@ -111,7 +121,9 @@ static int sm_count_cached() {
 }
 static Ctx mk(void *stream, int backend = 0) {
   watchdog_init();
-  return Ctx{(cudaStream_t)stream, nullptr, sm_count_cached(), backend};
+  int dev = 0;
+  cudaGetDevice(&dev);
+  return Ctx{(cudaStream_t)stream, nullptr, sm_count_cached(), backend, dev};
 }
 static int ret(cudaError_t e, const char *where) {
   if (e == cudaSuccess) return GPIPE_OK;
@@ -140,14 +152,16 @@ int gpipe_op_ln_fwd(void *stream, int dtype, const float *x, const float *gamma,
   return ret(ln_fwd(mk(stream), dtype, x, gamma, beta, y, mean, rstd, resid_bias, resid_out, n_tok, d, eps),
              "gpipe_op_ln_fwd");
 }
-int gpipe_op_attn_timeline(void *dev_buf) {
+#if GP_PROBES
+__attribute__((visibility("default"))) int gpipe_op_attn_timeline(void *dev_buf) {
   attn_tc_set_timeline((unsigned long long *)dev_buf);
   return GPIPE_OK;
 }
-int gpipe_op_gemm_timeline(void *dev_buf) {
+__attribute__((visibility("default"))) int gpipe_op_gemm_timeline(void *dev_buf) {
   gemm_tc_set_timeline((unsigned long long *)dev_buf);
   return GPIPE_OK;
 }
+#endif
 int64_t gpipe_op_gemm_workspace_bytes(int M, int N, int K) {
   return (int64_t)gemm_splitk_ws_bytes(M, N, K, sm_count_cached());
 }

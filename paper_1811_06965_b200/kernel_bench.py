@@ -41,7 +41,7 @@ def gemm_cases(w, T):
     return [
         ("qkv_fwd", T, 3 * da, d, 0, 0, dict(bias=1)),
         ("oproj_fwd", T, d, da, 0, 0, dict(accum=1)),
-        ("ffn1_fwd", T, H, d, 0, 0, dict(bias=1, relu=1)),
+        ("ffn1_fwd", T, H, d, 0, 0, dict(bias=1, relu=1, bits=1)),
         ("ffn2_fwd", T, d, H, 0, 0, dict(accum=1)),
         ("logits_fwd", T, V, d, 0, 0, dict()),
         ("ffn2_dgrad", T, H, d, 0, 1, dict(mask=1, colsum=1)),
@@ -124,6 +124,7 @@ def main():
             kw = {}
             if ep.get("bias"): kw["bias"] = torch.randn(N, device=dev)
             if ep.get("relu"): kw["relu"] = True
+            if ep.get("bits"): kw["bits_out"] = torch.zeros((M, N // 32), device=dev, dtype=torch.int32)
             if ep.get("resid"): kw["resid"] = torch.randn((M, N), device=dev)
             if ep.get("mask"): kw["mask"] = torch.randint(-2 ** 31, 2 ** 31 - 1, (M, N // 32), device=dev, dtype=torch.int32)
             if ep.get("accum"): kw["accumulate"] = True
@@ -134,7 +135,7 @@ def main():
         fns = [(lambda s=s: ops.gemm(s[0], s[1], s[2], transA=bool(tA), transB=bool(tB), **s[3])) for s in sets]
         ms = time_it(fns, args.reps)
         byts = per + (M * N * 4 if ep.get("resid") else 0) + (M * N * 4 if ep.get("accum") else 0) + \
-            (M * N // 8 if ep.get("mask") else 0)
+            (M * N // 8 if ep.get("mask") or ep.get("bits") else 0)
         extra = {"M": M, "N": N, "K": K, "transA": tA, "transB": tB}
         if args.compare:
             cf = [(lambda s=s: torch.matmul(s[0].t() if tA else s[0], s[1].t() if tB else s[1])) for s in sets]

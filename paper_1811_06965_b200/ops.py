@@ -65,16 +65,6 @@ def gemm(A, B_, C, *, transA=False, transB=False, bias=None, resid=None, mask=No
     return C
 
 
-def gemm_timeline(buf):
-    """Profiling hook: buf = int64 CUDA tensor of 32 * SM-count elements (or None to switch it off)."""
-    B._check(B.lib().gpipe_op_gemm_timeline(_p(buf)))
-
-
-def attn_timeline(buf):
-    """Profiling hook of the tcgen05 attention backward: buf = int64 CUDA tensor of 32 * n_seq * A elements (or None)."""
-    B._check(B.lib().gpipe_op_attn_timeline(_p(buf)))
-
-
 def gemm_workspace(M, N, K, device):
     """Zeroed split-K workspace for a [M,N,K] GEMM (None when the shape is not split)."""
     n = B.lib().gpipe_op_gemm_workspace_bytes(M, N, K)

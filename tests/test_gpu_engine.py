@@ -67,7 +67,8 @@ def test_zero_layer_model():
 
 
 def test_gradients_independent_of_K_M_remat_on_gpu():
-    """PAPER.md:45/:67/:209 on the GPU itself; dE uses float atomics so not bitwise."""
+    """PAPER.md:45/:67/:209 on the GPU itself: the accumulated gradient does not depend on K, M or remat (only the
+    fp32 summation order of the per-micro-batch terms differs between M values, hence 1e-5 and not bitwise)."""
     w = _tiny((0, 1))
     params = gi.make_params(w, 1001, round_bf16=False)
     tok, lab = gi.make_tokens(w, 2001)
@@ -214,6 +215,62 @@ def test_peak_bytes_tracker():
     assert peaks[1] > peaks[2] > peaks[4] > peaks[8]
     with _engine(w, M=8, remat=False) as e:
         assert e.peak_bytes()["by_category"]["interior"] > 4 * peaks[8]
+
+
+def test_host_plan_equals_device_plan_and_allocator_view():
+    """gpipe_plan_bytes (host only, no device query) is exactly what gpipe_create carves on the device
+    (gpipe_peak_bytes total), for fp32 and bf16 plans with and without a split-K workspace; and the arena torch
+    allocated for it shows up in torch.cuda.memory_allocated / cudaMemGetInfo (SURVEY.md 8(d) cross-check)."""
+    import torch
+    for w in (_tiny(), _bf16_small(), _bf16_small().replace(K=1, M=2), gi.reduced(gi.CONFIGS["T(12,8192,16)"])):
+        spec, keep = gp.make_spec(w.n_layers, w.d_model, w.d_ffn, w.n_heads, w.d_head, w.vocab, w.seq_len, w.dtype,
+                                  list(w.causal))
+        plan = gp.plan_bytes(spec, w.K, w.M, w.remat, w.n_seqs)
+        torch.cuda.synchronize()
+        free0, _ = torch.cuda.mem_get_info()
+        alloc0 = torch.cuda.memory_allocated()
+        with _engine(w) as e:
+            assert e.peak_bytes()["total"] == plan
+            assert torch.cuda.memory_allocated() - alloc0 >= plan
+            assert torch.cuda.max_memory_allocated() >= plan
+            free1, _ = torch.cuda.mem_get_info()
+            # the caching allocator may serve the arena from memory it already holds: the device-level
+            # free memory never drops by more than the arena (+ allocator rounding)
+            assert free0 - free1 <= plan + (64 << 20)
+
+
+def test_checkpoint_restore_is_bitwise():
+    """gpipe_get_master / gpipe_set_master / optimizer-slot access (no rounding): three RMSProp mini-batches
+    uninterrupted == one mini-batch, save, restore into a NEW handle, two more - bit for bit, in bf16 mode where
+    get_param / set_param alone would lose the fp32 master bits and the optimizer state."""
+    w = _bf16_small()
+    params = gi.make_params(w, 1002)
+    batches = [gi.make_tokens(w, 2100 + i) for i in range(3)]
+
+    def run(e, its):
+        losses = []
+        for it in its:
+            losses.append(e.step(*batches[it]))
+            e.apply_rmsprop(0.002, 0.9, 1e-6)
+        return losses
+
+    with _engine(w) as e:
+        e.set_params(params)
+        ref_losses = run(e, range(3))
+        ref_state = e.state_dict()
+    with _engine(w) as e:
+        e.set_params(params)
+        l0 = run(e, [0])
+        saved = e.state_dict()
+        assert any((saved["master"][n] != e.get_param(n)).any() for n in e.names)    # masters carry more than bf16
+    with _engine(w) as e2:
+        e2.load_state_dict(saved)
+        l12 = run(e2, [1, 2])
+        got = e2.state_dict()
+    assert l0 + l12 == ref_losses
+    for kind in ("master", "slot"):
+        for n in ref_state[kind]:
+            assert np.array_equal(got[kind][n], ref_state[kind][n]), (kind, n)
 
 
 def test_device_init_params_statistics():

@@ -82,6 +82,27 @@ def test_gemm_tcgen05_all_layouts(transA, transB):
         assert maxrel(_np(C), ref) <= 2 ** -7 and cosine(_np(C), ref) >= 0.99999, (M, N, K)
 
 
+def test_gemm_bf16_never_falls_back_silently():
+    """A bf16 problem the tcgen05 kernel cannot take (row pitch not a multiple of 16 bytes; a ReLU pattern with
+    N % 32 != 0) is GPIPE_EINVAL on the default backend, not a ~50x slower SIMT launch; backend 1 still runs it."""
+    from paper_1811_06965_b200 import GPipeError
+    r = _rng(9)
+    At, Aq = _lp(r.standard_normal((64, 36)), "bf16")        # lda = 36: 72-byte row pitch
+    Bt, Bq = _lp(r.standard_normal((36, 64)), "bf16")
+    C = torch.empty((64, 64), device=DEV, dtype=torch.bfloat16)
+    with pytest.raises(GPipeError) as err:
+        ops.gemm(At, Bt, C)
+    assert err.value.code == -1
+    ops.gemm(At, Bt, C, backend=1)
+    assert maxrel(_np(C), Aq @ Bq) <= 2 ** -7
+    A2, _ = _lp(r.standard_normal((64, 64)), "bf16")
+    B2, _ = _lp(r.standard_normal((64, 48)), "bf16")
+    C2 = torch.empty((64, 48), device=DEV, dtype=torch.bfloat16)
+    bits = torch.zeros((64, 2), device=DEV, dtype=torch.int32)
+    with pytest.raises(GPipeError):
+        ops.gemm(A2, B2, C2, relu=True, bits_out=bits)
+
+
 def test_gemm_tcgen05_split_k_deep():
     """Few output tiles and a very deep K (the dlogits W_out^T shape class): the launch is split along K,
     partials are reduced in split order, so two runs are bitwise equal and match the unsplit result."""
@@ -105,19 +126,109 @@ def test_gemm_tcgen05_split_k_deep():
     assert maxrel(_np(C1), _np(C0)) <= 1e-4
 
 
-def test_gemm_tcgen05_bench_shapes_sampled():
-    """The launch configurations bench.py times (T_mb = 2048 tokens, d = 1024): full-size GEMMs
-    checked on sampled rows the oracle's matmul can compute one by one."""
-    r = _rng(77)
-    for (M, N, K, tA, tB) in [(2048, 1024, 4096, 0, 0), (2048, 4096, 1024, 0, 1), (1024, 4096, 2048, 1, 0)]:
-        At, Aq = _lp(r.standard_normal((K, M) if tA else (M, K)) * 0.5, "bf16")
-        Bt, Bq = _lp(r.standard_normal((N, K) if tB else (K, N)) * 0.5, "bf16")
-        Cf = torch.empty((M, N), device=DEV, dtype=torch.float32)
-        ops.gemm(At, Bt, Cf, transA=bool(tA), transB=bool(tB), backend=2)
-        rows = r.choice(M, size=24, replace=False)
-        A_rows = (Aq.T if tA else Aq)[rows]
-        ref = A_rows @ (Bq.T if tB else Bq)
-        assert maxrel(_np(Cf)[rows], ref) <= 2e-5, (M, N, K)
+def _pack_mask(maskq):
+    M, N = maskq.shape
+    return torch.tensor(np.packbits(maskq.reshape(M, N // 32, 32), axis=-1, bitorder="little")
+                        .view(np.uint32).reshape(M, N // 32).view(np.int32), device=DEV)
+
+
+def _unpack_mask(bits, M, N):
+    return np.unpackbits(bits.cpu().numpy().view(np.uint8).reshape(M, N // 8), axis=-1, bitorder="little").astype(bool)
+
+
+# Every GEMM launch of one layer + head of the bench workload T(64,16384,32) (T_mb = 2048, d = 1024, d_a = 2048,
+# H = 16384, V = 64000), in the compile-time epilogue instantiation engine.cu launches it with:
+#   name, M, N, K, transA, transB, epilogue
+BENCH_GEMMS = [
+    ("qkv_fwd", 2048, 6144, 1024, 0, 0, "bias"),
+    ("oproj_fwd", 2048, 1024, 2048, 0, 0, "accum"),
+    ("ffn1_fwd", 2048, 16384, 1024, 0, 0, "bias_relu_bits"),
+    ("ffn2_fwd", 2048, 1024, 16384, 0, 0, "accum"),
+    ("logits_fwd", 2048, 64000, 1024, 0, 0, "plain"),
+    ("ffn2_dgrad", 2048, 16384, 1024, 0, 1, "mask_colsum"),
+    ("ffn1_dgrad", 2048, 1024, 16384, 0, 1, "plain"),
+    ("oproj_dgrad", 2048, 2048, 1024, 0, 1, "plain"),
+    ("qkv_dgrad", 2048, 1024, 6144, 0, 1, "plain"),
+    ("logits_dgrad", 2048, 1024, 64000, 0, 1, "plain"),
+    ("logits_dgrad_splitk", 2048, 1024, 64000, 0, 1, "plain_ws"),
+    ("ffn2_wgrad", 16384, 1024, 2048, 1, 0, "accum2"),
+    ("ffn1_wgrad", 1024, 16384, 2048, 1, 0, "accum2"),
+    ("oproj_wgrad", 2048, 1024, 2048, 1, 0, "accum2"),
+    ("qkv_wgrad", 1024, 6144, 2048, 1, 0, "accum2"),
+    ("logits_wgrad", 1024, 64000, 2048, 1, 0, "accum2"),
+]
+
+
+@pytest.mark.parametrize("case", BENCH_GEMMS, ids=[c[0] for c in BENCH_GEMMS])
+def test_gemm_tcgen05_bench_shapes_sampled(case):
+    """The launch configurations bench.py times: full-size GEMMs of the
+    config-5 micro-batch, each with the epilogue the engine fuses into it (>= 7 waves of 256 x 256 tiles on the
+    big outputs, 16 to 1000 K-blocks), compared on 24 sampled output rows with the oracle's definition - a plain
+    fp64 matmul of the same bf16-representable operands plus the epilogue written out.  fp32 outputs: 2e-5
+    (fp32 accumulation of exact products; 1e-4 for the 64000-deep chain); bf16 outputs: one rounding, 2^-7."""
+    name, M, N, K, tA, tB, epi = case
+    r = _rng(sum(map(ord, name)))
+    At, Aq = _lp(r.standard_normal((K, M) if tA else (M, K), dtype=np.float32) * 0.5, "bf16")
+    Bt, Bq = _lp(r.standard_normal((N, K) if tB else (K, N), dtype=np.float32) * 0.5, "bf16")
+    rows = np.sort(r.choice(M, size=24, replace=False))
+    ref = (Aq.T[rows] if tA else Aq[rows]) @ (Bq.T if tB else Bq)          # [24, N] fp64
+    f32_tol = 1e-4 if K > 20000 else 2e-5
+    if epi == "plain" or epi == "plain_ws":
+        C = torch.empty((M, N), device=DEV, dtype=torch.bfloat16)
+        ws = None
+        if epi == "plain_ws":
+            # config 2's engine (K = 2 cells < 4) hands its GEMMs a split-K workspace; the deep dlogits product
+            # is the launch that takes it
+            ws = ops.gemm_workspace(M, N, K, DEV)
+            assert ws is not None and ws.numel() > 0, "dlogits W_out^T is no longer split along K"
+        ops.gemm(At, Bt, C, transA=bool(tA), transB=bool(tB), workspace=ws if ws is not None else False, backend=2)
+        assert maxrel(_np(C[rows]), ref) <= 2 ** -7 and cosine(_np(C[rows]), ref) >= 0.99999
+        if ws is not None:
+            C2 = torch.empty_like(C)
+            ops.gemm(At, Bt, C2, transA=bool(tA), transB=bool(tB), workspace=ws, backend=2)
+            assert torch.equal(C, C2)                                       # deterministic, counters self-reset
+    elif epi == "bias":
+        bias = r.standard_normal(N).astype(np.float32)
+        C = torch.empty((M, N), device=DEV, dtype=torch.bfloat16)
+        ops.gemm(At, Bt, C, bias=torch.tensor(bias, device=DEV), workspace=False, backend=2)
+        assert maxrel(_np(C[rows]), ref + bias) <= 2 ** -7 and cosine(_np(C[rows]), ref + bias) >= 0.99999
+    elif epi == "bias_relu_bits":
+        bias = r.standard_normal(N).astype(np.float32)
+        C = torch.empty((M, N), device=DEV, dtype=torch.bfloat16)
+        bits = torch.zeros((M, N // 32), device=DEV, dtype=torch.int32)
+        ops.gemm(At, Bt, C, bias=torch.tensor(bias, device=DEV), relu=True, bits_out=bits, workspace=False, backend=2)
+        want = np.maximum(ref + bias, 0)
+        assert maxrel(_np(C[rows]), want) <= 2 ** -7 and cosine(_np(C[rows]), want) >= 0.99999
+        got_bits = _unpack_mask(bits, M, N)
+        assert np.array_equal(got_bits, _np(C) > 0)                        # every row: pattern == [stored h > 0]
+        # and the pattern is the oracle's [z > 0] except where |z| is within bf16 rounding of 0
+        z = ref + bias
+        clear = np.abs(z) > 2 ** -7 * np.abs(z).max()
+        assert np.array_equal(got_bits[rows][clear], (z > 0)[clear])
+    elif epi == "accum":
+        c0 = r.standard_normal((M, N)).astype(np.float32)
+        C = torch.tensor(c0, device=DEV)
+        ops.gemm(At, Bt, C, accumulate=True, workspace=False, backend=2)    # x += branch (a8, a11)
+        assert maxrel(_np(C[rows]), c0[rows] + ref) <= f32_tol
+    elif epi == "accum2":
+        c0 = r.standard_normal((M, N)).astype(np.float32)
+        C = torch.tensor(c0, device=DEV)
+        ops.gemm(At, Bt, C, transA=True, accumulate=True, workspace=False, backend=2)   # dW += X^T dY, two
+        ops.gemm(At, Bt, C, transA=True, accumulate=True, workspace=False, backend=2)   # micro-batches (a18)
+        assert maxrel(_np(C[rows]), c0[rows] + 2 * ref) <= f32_tol
+    elif epi == "mask_colsum":
+        maskq = r.standard_normal((M, N)) > 0
+        cs0 = r.standard_normal(N).astype(np.float32)
+        cst = torch.tensor(cs0, device=DEV)
+        C = torch.empty((M, N), device=DEV, dtype=torch.bfloat16)
+        ops.gemm(At, Bt, C, transB=True, mask=_pack_mask(maskq), colsum_out=cst, workspace=False, backend=2)
+        want = ref * maskq[rows]
+        assert maxrel(_np(C[rows]), want) <= 2 ** -7 and cosine(_np(C[rows]), want) >= 0.99999
+        full = _np(C)
+        assert not full[~maskq].any()                                      # masked units are exactly zero
+        assert maxrel(_np(cst), cs0 + full.sum(0)) <= 2e-5                  # db_1 += column sums of the stored dh
+    else:
+        raise AssertionError(epi)
 
 
 @pytest.mark.parametrize("dtype", ["fp32", "bf16"])

@@ -150,9 +150,27 @@ def test_p3_oracle_trace_respects_dependencies():
 # ---------------------------------------------------------------------------------------------
 # Whole-model pin: an independent torch-autograd model of the same definition
 # ---------------------------------------------------------------------------------------------
-def _torch_model_grads(w, params, tok, lab):
+class _RoundThrough(torch.autograd.Function):
+    """Identity whose forward value and/or incoming gradient is stored in bf16 (torch's own RNE conversion) -
+    the straight-through model of "this tensor lives in HBM as bf16"."""
+
+    @staticmethod
+    def forward(ctx, x, fwd, bwd):
+        ctx.bwd = bwd
+        return x.to(torch.bfloat16).to(x.dtype) if fwd else x
+
+    @staticmethod
+    def backward(ctx, g):
+        return (g.to(torch.bfloat16).to(g.dtype) if ctx.bwd else g), None, None
+
+
+def _torch_model_grads(w, params, tok, lab, rounded=False):
     """Textbook definition with library routines (F.layer_norm, torch.softmax, F.cross_entropy)
-    and autograd for every derivative; no cells, no micro-batches."""
+    and autograd for every derivative; no cells, no micro-batches.  rounded=True stores the tensors
+    DESIGN.md section 6 lists as bf16 (forward value and/or gradient) - the independent statement of
+    the oracle's round_operands mode."""
+    def rt(x, fwd, bwd):
+        return _RoundThrough.apply(x, fwd, bwd) if rounded else x
     P = {n: torch.tensor(np.asarray(a, np.float64), requires_grad=True) for n, a in params.items()}
     d, A, dh, S = w.d_model, w.n_heads, w.d_head, w.seq_len
     pos = torch.arange(S, dtype=torch.float64)[:, None]
@@ -164,18 +182,20 @@ def _torch_model_grads(w, params, tok, lab):
     N = x.shape[0]
     for l in range(w.n_layers):
         g = lambda n: P[f"l{l}.{n}"]
-        a = F.layer_norm(x, (d,), g("ln1_g")[0], g("ln1_b")[0], w.ln_eps)
-        qkv = a @ g("w_qkv") + g("b_qkv")[0]
+        a = rt(F.layer_norm(x, (d,), g("ln1_g")[0], g("ln1_b")[0], w.ln_eps), True, True)
+        qkv = rt(a @ g("w_qkv") + g("b_qkv")[0], True, True)
         q, k, v = [t.reshape(N, S, A, dh).transpose(1, 2) for t in qkv.split(A * dh, dim=-1)]
-        s = q @ k.transpose(-1, -2) / math.sqrt(dh)
+        s = rt(q @ k.transpose(-1, -2) * (1.0 / math.sqrt(dh)), False, True)          # dS is an MMA operand
         if w.causal[l]:
             s = s.masked_fill(torch.triu(torch.ones(S, S, dtype=torch.bool), 1), float("-inf"))
-        o = (torch.softmax(s, -1) @ v).transpose(1, 2).reshape(N, S, A * dh)
-        x = x + o @ g("w_o") + g("b_o")[0]
-        c = F.layer_norm(x, (d,), g("ln2_g")[0], g("ln2_b")[0], w.ln_eps)
-        x = x + torch.relu(c @ g("w_1") + g("b_1")[0]) @ g("w_2") + g("b_2")[0]
-    y = F.layer_norm(x, (d,), P["lnf_g"][0], P["lnf_b"][0], w.ln_eps)
-    logits = y @ P["w_out"]
+        o = (rt(torch.softmax(s, -1), True, False) @ v).transpose(1, 2).reshape(N, S, A * dh)   # P is an MMA operand
+        o = rt(o, True, True)
+        x = x + rt(o @ g("w_o") + g("b_o")[0], False, True)       # fp32 residual stream; bf16 operand copy of its gradient
+        c = rt(F.layer_norm(x, (d,), g("ln2_g")[0], g("ln2_b")[0], w.ln_eps), True, True)
+        z = rt(c @ g("w_1") + g("b_1")[0], False, True)
+        x = x + rt(rt(torch.relu(z), True, False) @ g("w_2") + g("b_2")[0], False, True)
+    y = rt(F.layer_norm(x, (d,), P["lnf_g"][0], P["lnf_b"][0], w.ln_eps), True, True)
+    logits = rt(y @ P["w_out"], True, True)
     loss = F.cross_entropy(logits.reshape(-1, w.vocab), torch.tensor(lab, dtype=torch.long).reshape(-1))
     loss.backward()
     return float(loss.detach()), {n: P[n].grad.numpy() for n in P}
@@ -190,6 +210,27 @@ def test_whole_model_matches_torch_autograd(causal):
     assert abs(loss - tl) <= 1e-12 * abs(tl)
     for n in o.names:
         assert _maxrel(o.g[n], tg[n].reshape(o.g[n].shape)) <= 1e-10, n
+
+
+def test_round_operands_mode_matches_independent_straight_through_model():
+    """The oracle's round_operands mode (used only to report the bf16 noise floor, reading A14) against an
+    independent statement of the same thing: the torch-autograd model with torch's own bf16 conversion applied,
+    straight-through, to the forward value and / or the gradient of exactly the tensors DESIGN.md section 6 lists as
+    stored in bf16.  A rounding point that is missing, misplaced or applied to the wrong side moves the result
+    by ~1e-3 relative; the two agree to fp64 rounding."""
+    w = _tiny((0, 1), d_model=128, n_heads=2, d_head=64, d_ffn=512, seq_len=32, n_seqs=4, M=2)
+    params = gi.make_params(w, 1001, round_bf16=True)
+    tok, lab = gi.make_tokens(w, 2001)
+    o = go.GPipeOracle(_spec(w), 2, 2, True, round_operands=True)
+    o.set_params(params)
+    loss = o.step(tok, lab)
+    tl, tg = _torch_model_grads(w, params, tok, lab, rounded=True)
+    assert abs(loss - tl) <= 1e-12 * abs(tl)
+    for n in o.names:
+        assert _maxrel(o.g[n], tg[n].reshape(o.g[n].shape)) <= 1e-9, n
+    # and the rounding is not a no-op: the plain oracle differs at the bf16 level
+    pl, pg = _torch_model_grads(w, params, tok, lab, rounded=False)
+    assert max(_maxrel(o.g[n], pg[n].reshape(o.g[n].shape)) for n in o.names) > 1e-4
 
 
 # ---------------------------------------------------------------------------------------------

@@ -27,3 +27,28 @@ def run_oracle(w, params, tok, lab, K=None, M=None, remat=None, dtype=np.float64
     o.set_params(params)
     loss = o.step(tok, lab)
     return o, loss
+
+
+# ---------------------------------------------------------------------------------------------
+# Shape-preserving reductions of BASELINE.json configs 2-5 (SURVEY.md 8(c) "Big-config parity"):
+# same d, H, A, d_head, V, S, K and M as the full config, one layer per cell (L = K) and one
+# sequence per micro-batch (N = M).  The oracle runs them in full.  Oracle precision: fp64 for
+# configs 2 and 3; fp32 ("plain, slow fp32 CPU implementation", BASELINE.json north_star) for
+# configs 4 and 5, whose 24 TFLOP per step would not fit the GPU test tier's time limit in fp64 -
+# the fp32 oracle's own error (~1e-6, pin P6) is three orders below the bf16 effects compared.
+# ---------------------------------------------------------------------------------------------
+REDUCED_CASES = {
+    "T(6,4096,16)": dict(seed_p=1012, seed_t=2012, oracle_dtype="float64"),
+    "T(12,8192,16)": dict(seed_p=1013, seed_t=2013, oracle_dtype="float64"),
+    "T(24,16384,32)": dict(seed_p=1014, seed_t=2014, oracle_dtype="float32"),
+    "T(64,16384,32)": dict(seed_p=1015, seed_t=2015, oracle_dtype="float32"),
+}
+
+
+def reduced_case(name):
+    """(workload, params, tokens, labels, oracle dtype) of the reduced parity case of config `name`."""
+    c = REDUCED_CASES[name]
+    w = gi.reduced(gi.CONFIGS[name])
+    params = gi.make_params(w, c["seed_p"])                 # bf16-representable, parity init (A10, A12)
+    tok, lab = gi.make_tokens(w, c["seed_t"])
+    return w, params, tok, lab, np.dtype(c["oracle_dtype"]).type

@@ -214,6 +214,17 @@ int gpipe_kernel_stats(const gpipe_t *g, int cls, const char **name, int64_t *co
 /* Number of kernels the library launched since gpipe_create (for bench.py's gpu_launches). */
 int64_t gpipe_launch_count(const gpipe_t *g);
 
+/* CUDA graph of the step (on by default): the first gpipe_step of a handle enqueues its ~(M K) tasks eagerly on the
+ * K streams, the second captures the same fork / join DAG into a CUDA graph (the memory plan is static: every
+ * pointer and TMA descriptor of a step is the same each time) and every later step is one cudaGraphLaunch - the
+ * host then spends microseconds per step instead of enqueueing tens of thousands of launches.  Results are
+ * bit-identical to eager enqueue (same kernels, same dependencies).  Steps with gpipe_trace or gpipe_kernel_timing
+ * enabled enqueue eagerly.  gpipe_cuda_graph(g, 0) switches the graph off (and frees it), 1 on again.
+ * gpipe_cuda_graph_state: 0 = eager so far, 1 = next step captures, 2 = replaying a graph, -1 = capture failed and
+ * the handle stays eager (not an error). */
+int gpipe_cuda_graph(gpipe_t *g, int enable);
+int gpipe_cuda_graph_state(const gpipe_t *g);
+
 /* Debug/verification taps for the per-kernel parity tests: copies a named device buffer of the
  * LAST executed (cell k, micro-batch m) task to host as fp32.  layer >= 0: "a", "qkv", "o", "c", "h", "x1",
  * "lse", and "hbits" - the bit-packed ReLU pattern [h > 0] (bit n%32 of word n/32, [T_mb, ceil(H/32)] uint32

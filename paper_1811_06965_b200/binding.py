@@ -87,6 +87,8 @@ def lib() -> C.CDLL:
         "gpipe_peak_bytes": (i32, [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]),
         "gpipe_trace": (i32, [vp, i32, C.POINTER(TraceEvent), C.POINTER(i64)]),
         "gpipe_launch_count": (i64, [vp]),
+        "gpipe_cuda_graph": (i32, [vp, i32]),
+        "gpipe_cuda_graph_state": (i32, [vp]),
         "gpipe_kernel_timing": (i32, [vp, i32]),
         "gpipe_kernel_stats": (i32, [vp, i32, C.POINTER(C.c_char_p), C.POINTER(i64), C.POINTER(C.c_double),
                                      C.POINTER(C.c_double), C.POINTER(C.c_double)]),
@@ -124,7 +126,7 @@ EXPORTED_SYMBOLS = [
     "gpipe_apply_rmsprop", "gpipe_op_rmsprop", "gpipe_zero_grads", "gpipe_num_tensors",
     "gpipe_tensor_info", "gpipe_get_param", "gpipe_set_param", "gpipe_get_grad", "gpipe_get_master", "gpipe_set_master",
     "gpipe_get_optimizer_slot", "gpipe_set_optimizer_slot", "gpipe_peak_bytes",
-    "gpipe_trace", "gpipe_launch_count", "gpipe_kernel_timing", "gpipe_kernel_stats", "gpipe_debug_read", "gpipe_last_error", "gpipe_version",
+    "gpipe_trace", "gpipe_launch_count", "gpipe_cuda_graph", "gpipe_cuda_graph_state", "gpipe_kernel_timing", "gpipe_kernel_stats", "gpipe_debug_read", "gpipe_last_error", "gpipe_version",
     "gpipe_op_gemm", "gpipe_op_gemm_workspace_bytes", "gpipe_op_ln_fwd", "gpipe_op_ln_bwd_scratch_floats", "gpipe_op_ln_bwd",
     "gpipe_op_attn_fwd", "gpipe_op_attn_bwd", "gpipe_op_softmax_ce", "gpipe_op_colsum",
     "gpipe_op_colsum_scratch_floats",
@@ -394,6 +396,13 @@ class GPipe:
             _check(lib().gpipe_kernel_stats(self._h, cls, C.byref(nm), C.byref(cnt), C.byref(ms), C.byref(fl), C.byref(by)))
             out[nm.value.decode()] = {"launches": cnt.value, "ms": ms.value, "flops": fl.value, "bytes": by.value}
         return out
+
+    def cuda_graph(self, enable: bool):
+        """Replay the step as one CUDA graph (default on) or enqueue it eagerly."""
+        _check(lib().gpipe_cuda_graph(self._h, int(enable)))
+
+    def cuda_graph_state(self) -> int:
+        return int(lib().gpipe_cuda_graph_state(self._h))
 
     def launch_count(self) -> int:
         return int(lib().gpipe_launch_count(self._h))

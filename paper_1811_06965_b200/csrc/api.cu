@@ -240,6 +240,7 @@ void gpipe_destroy(gpipe_t *g) {
   if (!g) return;
   Engine &e = g->e;
   for (auto s : e.streams) cudaStreamSynchronize(s);
+  e.drop_graph();
   for (auto &v : e.ev_f) for (auto ev : v) if (ev) cudaEventDestroy(ev);
   for (auto &v : e.ev_b) for (auto ev : v) if (ev) cudaEventDestroy(ev);
   for (auto ev : e.ev_done) if (ev) cudaEventDestroy(ev);
@@ -521,6 +522,18 @@ int gpipe_kernel_stats(const gpipe_t *g, int cls, const char **name, int64_t *co
 }
 
 int64_t gpipe_launch_count(const gpipe_t *g) { return g ? g->e.launches : 0; }
+
+int gpipe_cuda_graph(gpipe_t *g, int enable) {
+  if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
+  Engine &e = g->e;
+  for (auto s : e.streams) cudaStreamSynchronize(s);
+  e.use_graph = enable ? 1 : 0;
+  if (!enable) { e.drop_graph(); e.graph_state = 0; }
+  else if (e.graph_state < 0) e.graph_state = 0;
+  return GPIPE_OK;
+}
+
+int gpipe_cuda_graph_state(const gpipe_t *g) { return g ? (g->e.use_graph ? g->e.graph_state : 0) : fail(GPIPE_EINVAL, "handle is NULL"); }
 
 int gpipe_debug_read(gpipe_t *g, const char *what, int layer, float *host_out, int64_t max_elems, int64_t *n_elems) {
   if (!g || !what || !host_out || !n_elems) return fail(GPIPE_EINVAL, "arguments are required");

@@ -417,10 +417,7 @@ cudaError_t Engine::resolve_kernel_timing() {
   return cudaSuccess;
 }
 
-cudaError_t Engine::run_step(float *loss_out) {
-  ev_pool_used = 0;
-  trace.clear();
-  krecs.clear();
+cudaError_t Engine::enqueue_step() {
   int idx = 0;
   auto task = [&](int kind, int k, int m) -> cudaError_t {
     TraceRec r{kind, k, m, idx++, nullptr, nullptr};
@@ -468,6 +465,54 @@ cudaError_t Engine::run_step(float *loss_out) {
     GP_TRY(cudaStreamWaitEvent(streams[0], ev_done[k], 0));
   }
   GP_TRY(cudaMemcpyAsync(host_loss, loss_parts, sizeof(float) * M, cudaMemcpyDeviceToHost, streams[0]));
+  return cudaSuccess;
+}
+
+void Engine::drop_graph() {
+  if (graph_exec) cudaGraphExecDestroy(graph_exec);
+  if (graph) cudaGraphDestroy(graph);
+  graph_exec = nullptr;
+  graph = nullptr;
+}
+
+cudaError_t Engine::run_step(float *loss_out) {
+  ev_pool_used = 0;
+  trace.clear();
+  krecs.clear();
+  const bool eager = !use_graph || trace_on || ktiming_on || serial || graph_state < 0;
+  if (eager || graph_state == 0) {
+    GP_TRY(enqueue_step());
+    if (!eager) graph_state = 1;
+  } else {
+    if (graph_state == 1) {
+      // Relaxed mode: other host threads (the caller's allocator, another handle) may call CUDA while this thread
+      // captures; nothing enqueue_step does is capture-unsafe (kernel launches, event record / wait, one async copy).
+      const int64_t l0 = launches;
+      cudaError_t e = cudaStreamBeginCapture(streams[0], cudaStreamCaptureModeRelaxed);
+      if (e == cudaSuccess) {
+        e = enqueue_step();
+        cudaGraph_t gcap = nullptr;
+        cudaError_t e2 = cudaStreamEndCapture(streams[0], &gcap);     // always end the capture, even after an error
+        if (e == cudaSuccess) e = e2;
+        graph = gcap;
+      }
+      if (e == cudaSuccess) e = cudaGraphInstantiate(&graph_exec, graph, 0);
+      graph_launches = launches - l0;
+      launches = l0;
+      if (e != cudaSuccess) {                                         // not fatal: this handle stays on eager enqueue
+        cudaGetLastError();
+        drop_graph();
+        graph_state = -1;
+        GP_TRY(enqueue_step());
+      } else {
+        graph_state = 2;
+      }
+    }
+    if (graph_state == 2) {
+      GP_TRY(cudaGraphLaunch(graph_exec, streams[0]));
+      launches += graph_launches;
+    }
+  }
   GP_TRY(cudaStreamSynchronize(streams[0]));
   if (ktiming_on) GP_TRY(resolve_kernel_timing());
   double s = 0.0;

@@ -109,6 +109,19 @@ struct Engine {
   cudaEvent_t ev_in = nullptr;
   std::vector<cudaEvent_t> ev_done;                    // per stream
 
+  // CUDA graph of one step: the K-stream fork / join DAG of run_step is captured once - the plan is
+  // static, so every kernel argument and every TMA descriptor of a step is the same each time - and replayed with one
+  // cudaGraphLaunch; tracing and per-launch timing enqueue eagerly.  graph_state: 0 = first step runs eagerly (sets
+  // function attributes, fills the descriptor cache), 1 = capture on this step, 2 = replay, -1 = capture failed:
+  // stay eager.
+  int use_graph = 1;
+  int graph_state = 0;
+  cudaGraph_t graph = nullptr;
+  cudaGraphExec_t graph_exec = nullptr;
+  int64_t graph_launches = 0;                          // kernels inside the graph (gpipe_launch_count)
+  cudaError_t enqueue_step();                          // every task of a mini-batch + the loss copy, on the K streams
+  void drop_graph();
+
   int trace_on = 0;
   std::vector<TraceRec> trace;
   std::vector<cudaEvent_t> ev_pool;

@@ -65,8 +65,14 @@ struct Params {
   unsigned int *ws_cnt;         // [tile][rank][2]: arrivals, partials ready
 #if GP_PROBES
   unsigned long long *tl;       // optional timeline probe: 8 globaltimer stamps per CTA (gemm_tc_set_timeline)
+  int dbg;                      // GPIPE_GEMM_DBG: 1 = epilogue only drains TMEM, 2 = no TMA loads (results are garbage)
 #endif
 };
+#if GP_PROBES
+#define GP_DBG(p, bit) (((p).dbg & (bit)) != 0)
+#else
+#define GP_DBG(p, bit) false
+#endif
 
 #if GP_PROBES
 __device__ __forceinline__ void tl_stamp(const Params &p, int slot) {
@@ -195,6 +201,11 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
         for (int kb = kb0; kb < kb1; ++kb) {
           mbar_wait(empty_bar(stage), phase ^ 1, 0x11);
           const uint32_t sa = smem_base + stage * STAGE_BYTES, sb = sa + A_BYTES;
+          if (GP_DBG(p, 2)) {
+            if (rank == 0) mbar_arrive(full_bar(stage));
+            if (++stage == NST) { stage = 0; phase ^= 1; }
+            continue;
+          }
           if (rank == 0) mbar_expect_tx(full_bar(stage), 2 * STAGE_BYTES);
           const uint32_t fb = mapa_shared(full_bar(stage), 0);
           const int k0 = kb * BK;
@@ -357,6 +368,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
         const bool tlon = it == 0 && et == 0;
         tl_clock(p, tlon, cl, 0);
         if (!col_ok) continue;
+        if (GP_DBG(p, 1)) continue;
         if (splits > 1) {
           if (write_partial) {                               // raw accumulators -> workspace; no epilogue
             float4 *dst = reinterpret_cast<float4 *>(part_row + sp * part_split_stride + c * 32);
@@ -643,6 +655,10 @@ static cudaError_t launch_pair(const Ctx &c, const GemmArgs &a) {
   p.splits = (num_kb + p.kb_per_split - 1) / p.kb_per_split;             // no empty split
 #if GP_PROBES
   p.tl = g_timeline;
+  {
+    static const int dbg = getenv("GPIPE_GEMM_DBG") ? atoi(getenv("GPIPE_GEMM_DBG")) : 0;
+    p.dbg = dbg;
+  }
 #endif
   p.ws_cnt = (unsigned int *)a.ws;
   p.ws_part = (float *)((char *)a.ws + splitk_cnt_bytes(p.tiles_m * p.tiles_n));

@@ -61,9 +61,10 @@ def _gpu_run(w, params, tok, lab, remat):
     return loss, grads, bits, peak
 
 
-@pytest.mark.parametrize("name", list(REDUCED_CASES))
+@pytest.mark.parametrize("name", list(REDUCED_CASES), ids=["config2", "config3", "config4", "config5"])
 def test_reduced_config_matches_oracle(name):
     w, params, tok, lab, dt = reduced_case(name)
+    assert name in FLOOR, "run tests/golden/make_bf16_floor.py for %s" % name
     fl = FLOOR[name]
     assert fl["workload"]["n_layers"] == w.n_layers and fl["workload"]["d_ffn"] == w.d_ffn
     assert fl["workload"]["causal"] == list(w.causal) and fl["oracle_dtype"] == REDUCED_CASES[name]["oracle_dtype"]
@@ -115,6 +116,9 @@ def test_reduced_config_matches_oracle(name):
     assert rel_loss <= 1e-2
     for n, c in cos.items():
         assert c >= min(COS_BOUND, floor[n] - FLOOR_SLACK), (n, c, floor[n])
-    # a flipped unit removes or adds its whole row of dW_1: the deficit is of the order of the flip fraction
+    # a flipped unit removes or adds its whole column of dW_1, so for the LAST layer (no flips downstream of it)
+    # 1 - cos(dW_1) equals the flip fraction (measured: 7.7e-4 vs 7.5e-4 at config 2's shape, 9.7e-4 vs 9.9e-4 at
+    # config 3's); the GPU's flip fraction is the one the oracle's own bf16-rounding run shows
     assert mism <= 3e-3
-    assert 0.25 * mism - 1e-4 <= deficit <= 4.0 * mism + 1e-4, (mism, deficit)
+    assert 0.7 * mism <= deficit <= 1.4 * mism, (mism, deficit)
+    assert 0.7 * fl["relu_mismatch_m0"][str(l)] <= mism <= 1.4 * fl["relu_mismatch_m0"][str(l)]

@@ -131,6 +131,30 @@ def test_step_accumulates_and_sgd_applies():
             assert maxrel(e.get_param(n), o.p[n]) <= 1e-5, n
 
 
+@pytest.mark.parametrize("which", ["tiny-fp32", "small-bf16"])
+def test_cuda_graph_replay_is_bitwise_eager(which):
+    """The step as one CUDA graph (capture on the second step, replay afterwards) against eager enqueue of the same
+    K-stream DAG: same kernels, same dependencies, so loss and every accumulated gradient are bit-identical, on
+    different batches (the ids are copied outside the graph), and the launch count is the same."""
+    w = _tiny((0, 1)) if which == "tiny-fp32" else _bf16_small()
+    params = gi.make_params(w, 1001)
+    batches = [gi.make_tokens(w, 2200 + i) for i in range(4)]
+    out = {}
+    for graph in (True, False):
+        with _engine(w) as e:
+            e.cuda_graph(graph)
+            e.set_params(params)
+            losses = [e.step(*b) for b in batches]
+            out[graph] = (losses, e.grads(), e.launch_count(), e.cuda_graph_state())
+            e.apply_sgd(0.1)                                     # the graph survives parameter updates (same pointers)
+            out[graph] += (e.step(*batches[0]),)
+    assert out[True][3] == 2 and out[False][3] == 0
+    assert out[True][0] == out[False][0] and out[True][4] == out[False][4]
+    assert out[True][2] == out[False][2] > 0
+    for n in out[True][1]:
+        assert np.array_equal(out[True][1][n], out[False][1][n]), n
+
+
 def test_device_resident_inputs_match_host_inputs():
     import torch
     w = _tiny()

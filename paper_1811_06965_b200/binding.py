@@ -13,7 +13,8 @@ from typing import Dict, List, Optional, Sequence, Tuple
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libgpipe_b200.so")
+# GPIPE_LIB_PATH selects another build of the same ABI (A/B comparisons of two kernel versions inside one gpurun call)
+LIB_PATH = os.environ.get("GPIPE_LIB_PATH") or os.path.join(_HERE, "libgpipe_b200.so")
 
 DTYPE_FP32, DTYPE_BF16 = 0, 1
 CATEGORIES = ["weights", "masters", "grads", "boundary", "interior", "head", "misc", "bwd_scratch"]

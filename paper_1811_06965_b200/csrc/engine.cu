@@ -99,9 +99,12 @@ int Engine::build_plan(bool dry, std::string &err) {
     }
   }
 
-  // split-K workspace: the largest any GEMM shape of a cell needs (forward, dgrad, wgrad)
-  // Split-K buys single-kernel latency at the price of SM-time; with >= 4 cells in flight the other
-  // streams fill the SMs a few-tile GEMM leaves idle, so only shallow pipelines split.
+  // split-K workspace: the largest any GEMM shape of a cell needs (forward, dgrad, wgrad); one per cell - a cell's
+  // launches are ordered on its stream, so one user at a time.  Split-K buys single-kernel latency at the price of
+  // SM-time (FFN2 forward at T_mb 2048: 85.8 us on 64 SMs unsplit, 68.0 us on 128 SMs split in two), so only shallow
+  // pipelines split: with >= 4 cells in flight the other streams fill the SMs a few-tile GEMM leaves idle, and the
+  // config-5 step measured 5 % SLOWER with every [T_mb x 1024] output split (round 2).  It also keeps the K-loop
+  // order, hence every per-token forward value, independent of the micro-batch size for the deep pipelines.
   splitk_ws_bytes = 0;
   if (dt == GP_BF16 && K < 4) {
     const int T = (int)T_mb;

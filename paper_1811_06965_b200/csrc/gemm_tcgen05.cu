@@ -91,17 +91,25 @@ __device__ __forceinline__ void tl_stamp(const Params &, int) {}
 __device__ __forceinline__ void tl_clock(const Params &, bool, int, int) {}
 #endif
 
-// STG: staging buffers ([32 rows x 128 B]) per epilogue warp.  Dynamic shared memory: operand ring,
-// staging, bias (2 x BN floats), column-sum exchange (4 x BN floats), 1 KB alignment slack.
-template <int BN, int STG> struct PairCfg {
+// Dynamic shared memory: operand ring (5 stages of 32 KB), epilogue staging (one [32 rows x 128 B] buffer per
+// epilogue warp), bias (2 x BN floats, only with EPI_BIAS), column-sum exchange (4 x BN floats, only with
+// EPI_COLSUM), 1 KB alignment slack.  An instantiation whose flags are compile-time constants carries only the
+// auxiliary buffers it uses.  STG = 2 (a second staging buffer per warp, which fits for the flag sets without
+// column sums) was measured in the config-5 step against STG = 1 on one box: 1500-1504 ms vs 1492 ms - the extra
+// shared-memory footprint buys nothing, the epilogue is not waiting on its staging buffer.
+template <int BN, int F> struct PairCfg {
   static constexpr int BNH = BN / 2;
   static constexpr uint32_t A_BYTES = 128 * BK * 2, B_BYTES = BNH * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;
+  static constexpr int STAGES = 5;
+  static constexpr int STG = 1;
+  static constexpr uint32_t BIAS_BYTES = (F < 0 || (F & EPI_BIAS)) ? 2 * BN * 4 : 0;
+  static constexpr uint32_t COLBUF_BYTES = (F < 0 || (F & EPI_COLSUM)) ? 4 * BN * 4 : 0;
+  static constexpr uint32_t AUX_BYTES = BIAS_BYTES + COLBUF_BYTES;
+  static constexpr uint32_t LIMIT = 227 * 1024 - 512;                // opt-in maximum minus the static barriers etc.
   static constexpr uint32_t STAGING_BYTES = 8 * STG * 4096;
-  static constexpr uint32_t AUX_BYTES = 6 * BN * 4;
-  static constexpr int STAGES_MAX = (int)((225 * 1024 - STAGING_BYTES - AUX_BYTES) / STAGE_BYTES);
-  static constexpr int STAGES = STAGES_MAX > 8 ? 8 : STAGES_MAX;
   static constexpr uint32_t TMEM_COLS = 2 * BN > 256 ? 512 : 256;
   static constexpr size_t SMEM = (size_t)STAGES * STAGE_BYTES + STAGING_BYTES + AUX_BYTES + 1024;
+  static_assert(SMEM <= LIMIT, "shared-memory budget");
 };
 
 // Column sums over a warp's 32 rows: transpose-reduce across lanes (31 shuffles); afterwards
@@ -122,14 +130,14 @@ __device__ __forceinline__ void warp_colsum32(float (&v)[32], const int lane) {
 // ------------------------------------------------------------------------------------------
 // the kernel
 // ------------------------------------------------------------------------------------------
-// F >= 0: the epilogue flags are this compile-time constant and the launch is never split along K
-// (compact straight-line epilogue: the generic one is instruction-fetch bound); F < 0: p.flags at run time.
-template <int BN, int STG, int F>
+// F >= 0: the epilogue flags are this compile-time constant (compact straight-line epilogue: the generic one is
+// instruction-fetch bound); F < 0: p.flags at run time.  SPLITK: the launch may be split along K (p.splits).
+template <int BN, int F, bool SPLITK>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NUM_THREADS, 1)
 gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_b,
                          const __grid_constant__ CUtensorMap map_c, const Params p) {
-  using Cfg = PairCfg<BN, STG>;
-  constexpr int NST = Cfg::STAGES, BNH = Cfg::BNH;
+  using Cfg = PairCfg<BN, F>;
+  constexpr int NST = Cfg::STAGES, BNH = Cfg::BNH, STG = Cfg::STG;
   constexpr uint32_t A_BYTES = Cfg::A_BYTES, STAGE_BYTES = Cfg::STAGE_BYTES;
   static_assert(BN == 256, "the epilogue splits the tile into two 128-column halves of four 32-column chunks");
   extern __shared__ uint8_t smem_raw[];
@@ -140,7 +148,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t staging_base = smem_base + NST * STAGE_BYTES;
   float *bias_s = reinterpret_cast<float *>(smem_raw + (staging_base - smem_u32(smem_raw)) + Cfg::STAGING_BYTES);  // [2][BN]
-  float *colbuf = bias_s + 2 * BN;                                                                                // [4][BN]
+  float *colbuf = bias_s + Cfg::BIAS_BYTES / 4;                                                                   // [4][BN]
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
   const int pair = blockIdx.x >> 1, num_pairs = gridDim.x >> 1;
@@ -185,7 +193,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
   if (threadIdx.x == 0) tl_stamp(p, 1);                // prologue done
 
   const int flags = F >= 0 ? F : p.flags;
-  const int splits = F >= 0 ? 1 : p.splits;
+  const int splits = SPLITK ? p.splits : 1;
   const int num_units = p.tiles_m * p.tiles_n * splits;       // work units: (tile, split), splits adjacent
   const int num_kb = (p.K + BK - 1) / BK;
 
@@ -313,7 +321,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
       tmem_ld32(t_row, rn);                              // first chunk in flight during the split-K handshake
       // ---- split-K: am I the last of this (tile, rank)'s splits to finish? ----
       bool write_partial = false;
-      if (splits > 1) {
+      if constexpr (SPLITK) if (splits > 1) {
         unsigned int *cnt = p.ws_cnt + ((size_t)t * 2 + rank) * 2;
         if (et == 0) {
           const unsigned int arrived = atomicAdd(cnt, 1u);
@@ -330,8 +338,9 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
         asm volatile("bar.sync 2, 256;" ::: "memory");
         write_partial = split_last_s == 0;
       }
+      // partials: [tile][split][rank][chunk][row 128][32 floats] - the 32 x 128 B a warp writes per chunk are contiguous
       float *part_row = p.ws_part + (((size_t)t * splits) * 2 + rank) * (size_t)(128 * BN) +
-                        (size_t)(quad * 32 + lane) * BN;          // split 0 of this (tile, rank), this lane's row
+                        (size_t)(quad * 32 + lane) * 32;          // split 0 of this (tile, rank), chunk 0, this lane's row
       const size_t part_split_stride = (size_t)2 * 128 * BN;
       uint32_t wb0 = 0u, wb1 = 0u, wb2 = 0u, wb3 = 0u;     // EPI_BITS_OUT words of this row
       // one 32-column chunk per iteration; NOT unrolled: the epilogue has to stay resident in the
@@ -371,7 +380,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
         if (GP_DBG(p, 1)) continue;
         if (splits > 1) {
           if (write_partial) {                               // raw accumulators -> workspace; no epilogue
-            float4 *dst = reinterpret_cast<float4 *>(part_row + sp * part_split_stride + c * 32);
+            float4 *dst = reinterpret_cast<float4 *>(part_row + sp * part_split_stride + (size_t)c * (128 * 32));
 #pragma unroll
             for (int j = 0; j < 8; ++j) __stcg(dst + j, make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]));
             continue;
@@ -389,7 +398,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
                 for (int j = 0; j < 32; ++j) acc[j] += v[j];
               }
             } else {
-              const float4 *src = reinterpret_cast<const float4 *>(part_row + s2 * part_split_stride + c * 32);
+              const float4 *src = reinterpret_cast<const float4 *>(part_row + s2 * part_split_stride + (size_t)c * (128 * 32));
 #pragma unroll
               for (int j = 0; j < 8; ++j) {
                 const float4 q4 = __ldcg(src + j);
@@ -411,7 +420,16 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
         }
         if (flags & EPI_RELU) {
 #pragma unroll
-          for (int j = 0; j < 32; ++j) v[j] = fmaxf(v[j], 0.f);
+          for (int j = 0; j < 32; ++j) v[j] = fmaxf(v[j], 0.f);          // max(-0, +0) = +0
+        }
+        if ((flags & EPI_BITS_OUT) && (flags & EPI_RELU) && !out_f32) {
+          // bit j = [v_j > 0]: after the ReLU v_j >= +0, so v_j > 0 <=> its bit pattern is a positive integer <=> the
+          // top bit of (0 - pattern) is set; one subtract + one funnel shift per unit.  RNE to bf16 maps a positive
+          // fp32 normal to a positive bf16, so this is also [stored h > 0].
+          uint32_t w = 0;
+#pragma unroll
+          for (int j = 31; j >= 0; --j) w = __funnelshift_l(0u - __float_as_uint(v[j]), w, 1);
+          wb0 = cl == 0 ? w : wb0; wb1 = cl == 1 ? w : wb1; wb2 = cl == 2 ? w : wb2; wb3 = cl == 3 ? w : wb3;
         }
         if (flags & EPI_MASK) {
           const uint32_t w01 = (cl & 1) ? mb1 : mb0, w23 = (cl & 1) ? mb3 : mb2;
@@ -479,7 +497,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
           }
           tl_clock(p, tlon, cl, 3);
         }
-        if (flags & EPI_BITS_OUT) {
+        if ((flags & EPI_BITS_OUT) && !((flags & EPI_RELU) && !out_f32)) {
           uint32_t w = 0;
 #pragma unroll
           for (int j = 0; j < 32; ++j) w |= (v[j] > 0.f ? 1u : 0u) << j;
@@ -607,20 +625,27 @@ static bool get_map(const void *ptr, uint32_t esize, uint64_t inner, uint64_t ou
   return true;
 }
 
-// Split-K when the output has too few 256 x 256 tiles to occupy the CTA pairs and K is long enough
-// that each split still runs a long main loop (>= 192 K-blocks = 12288 deep): the split launch takes
-// the run-time-flag kernel and pays a workspace round trip, which only the very deep products
-// (dlogits W_out^T, K = V) win back - measured: K = 2048 20.5 us unsplit vs 43.6 us split, K = 6144
-// 37.1 vs 54.5, K = 16384 86.4 vs 84.7, K = 64000 296.6 vs 207.1.  All units run in ONE wave.
+// Split-K when the output has too few 256 x 256 tiles to occupy the CTA pairs (tiles <= pairs / 2) and K is so long
+// that each split still runs a main loop of >= 192 K-blocks (12288 deep): only the dlogits W_out^T product (K = V)
+// qualifies.  Measured, isolated (us, unsplit vs split): K = 2048 20.5 / 43.6 (run-time-flag kernel, round 1),
+// K = 16384 85.8 / 68.0, K = 64000 296.6 / 207.1 - and in the step: with every [T_mb x 1024] output split (>= 32
+// K-blocks per split, specialised kernels) config 2 ran 6 % slower (20.8 vs 19.6 ms) and config 5 5 % slower: a split
+// launch takes twice the SMs for 0.8x the time, and the step is bound by SM-time, not by single-kernel latency.
+// All units run in ONE wave; the first splits-1 CTAs of a (tile, rank) to finish leave raw fp32 accumulators in the
+// workspace, the last one sums them in split order (bitwise deterministic, whoever is last).
+constexpr int kSplitMinKb = 192;
 static int splitk_factor(int tiles, int num_kb, int pairs) {
+  int min_kb = kSplitMinKb;
 #if GP_PROBES
   static const int off = getenv("GPIPE_NO_SPLITK") ? atoi(getenv("GPIPE_NO_SPLITK")) : 0;
   if (off) return 1;
+  static const int mk = getenv("GPIPE_SPLITK_MINKB") ? atoi(getenv("GPIPE_SPLITK_MINKB")) : 0;
+  if (mk > 0) min_kb = mk;
 #endif
   if (tiles * 2 > pairs) return 1;
   int s = pairs / tiles;
   if (s > 4) s = 4;
-  while (s > 1 && num_kb / s < 192) --s;
+  while (s > 1 && num_kb / s < min_kb) --s;
   return s;
 }
 static size_t splitk_cnt_bytes(int tiles) { return (((size_t)tiles * 2 * 2 * sizeof(unsigned int)) + 1023) & ~(size_t)1023; }
@@ -629,9 +654,9 @@ static size_t splitk_cnt_bytes(int tiles) { return (((size_t)tiles * 2 * 2 * siz
 static unsigned long long *g_timeline = nullptr;
 #endif
 
-template <int BN, int STG, int F>
+template <int BN, int F, bool SPLITK>
 static cudaError_t launch_pair(const Ctx &c, const GemmArgs &a) {
-  using Cfg = PairCfg<BN, STG>;
+  using Cfg = PairCfg<BN, F>;
   Params p{};
   p.M = a.M; p.N = a.N; p.K = a.K;
   p.a_mn_major = a.transA ? 1 : 0;
@@ -649,7 +674,7 @@ static cudaError_t launch_pair(const Ctx &c, const GemmArgs &a) {
   }
 #endif
   const int num_kb = (a.K + BK - 1) / BK;
-  p.splits = F >= 0 ? 1 : splitk_factor(p.tiles_m * p.tiles_n, num_kb, pairs);
+  p.splits = SPLITK ? splitk_factor(p.tiles_m * p.tiles_n, num_kb, pairs) : 1;
   if (p.splits > 1 && (!a.ws || a.ws_bytes < gemm_splitk_ws_bytes(a.M, a.N, a.K, c.sm_count))) p.splits = 1;
   p.kb_per_split = (num_kb + p.splits - 1) / p.splits;
   p.splits = (num_kb + p.kb_per_split - 1) / p.kb_per_split;             // no empty split
@@ -675,12 +700,12 @@ static cudaError_t launch_pair(const Ctx &c, const GemmArgs &a) {
   ok = get_map(a.C, out_f32 ? 4 : 2, (uint64_t)a.N, (uint64_t)a.M, (uint64_t)a.ldc, out_f32 ? 32 : 64, 32, &mc);
   if (!ok) return cudaErrorInvalidValue;
   {
-    cudaError_t e = ensure_dyn_smem<gemm_tcgen05_pair_kernel<BN, STG, F>>(Cfg::SMEM, c.device);
+    cudaError_t e = ensure_dyn_smem<gemm_tcgen05_pair_kernel<BN, F, SPLITK>>(Cfg::SMEM, c.device);
     if (e != cudaSuccess) return e;
   }
   int units = p.tiles_m * p.tiles_n * p.splits;
   int grid = 2 * (units < pairs ? units : pairs);
-  gemm_tcgen05_pair_kernel<BN, STG, F><<<grid, NUM_THREADS, Cfg::SMEM, c.stream>>>(ma, mb, mc, p);
+  gemm_tcgen05_pair_kernel<BN, F, SPLITK><<<grid, NUM_THREADS, Cfg::SMEM, c.stream>>>(ma, mb, mc, p);
   GP_LAUNCH_CHECK(c);
 }
 
@@ -721,8 +746,9 @@ bool gemm_tc_supported(int dt, const GemmArgs &a) {
   return true;
 }
 
-// The epilogue combinations the engine launches get their own instantiation; anything else (and every
-// split-K launch) takes the run-time-flag kernel.
+// The epilogue combinations the engine launches get their own instantiation - the two that occur on few-tile,
+// deep-K shapes (plain bf16 output: dgrads; fp32 accumulate: FFN2 / out-projection forward, wgrads) also as a
+// split-K variant; anything else takes the run-time-flag kernel.
 cudaError_t gemm_tc(const Ctx &c, const GemmArgs &a) {
 #if GP_PROBES
   static const int generic_only = getenv("GPIPE_GEMM_GENERIC") ? atoi(getenv("GPIPE_GEMM_GENERIC")) : 0;
@@ -730,18 +756,23 @@ cudaError_t gemm_tc(const Ctx &c, const GemmArgs &a) {
   constexpr int generic_only = 0;
 #endif
   const int tiles = ((a.M + 255) / 256) * ((a.N + 255) / 256);
-  const bool split = a.ws && tc::splitk_factor(tiles, (a.K + tc::BK - 1) / tc::BK, c.sm_count / 2) > 1;
-  if (!split && !generic_only) {
+  const bool split = a.ws && tc::splitk_factor(tiles, (a.K + tc::BK - 1) / tc::BK, c.sm_count / 2) > 1 &&
+                     a.ws_bytes >= gemm_splitk_ws_bytes(a.M, a.N, a.K, c.sm_count);
+  if (!generic_only) {
     switch (a.flags) {
-      case 0: return tc::launch_pair<256, 1, 0>(c, a);
-      case EPI_BIAS: return tc::launch_pair<256, 1, EPI_BIAS>(c, a);
-      case EPI_BIAS | EPI_RELU | EPI_BITS_OUT: return tc::launch_pair<256, 1, EPI_BIAS | EPI_RELU | EPI_BITS_OUT>(c, a);
-      case EPI_MASK | EPI_COLSUM: return tc::launch_pair<256, 1, EPI_MASK | EPI_COLSUM>(c, a);
-      case EPI_ACCUM | EPI_OUT_F32: return tc::launch_pair<256, 1, EPI_ACCUM | EPI_OUT_F32>(c, a);
+      case 0: return split ? tc::launch_pair<256, 0, true>(c, a) : tc::launch_pair<256, 0, false>(c, a);
+      case EPI_ACCUM | EPI_OUT_F32:
+        return split ? tc::launch_pair<256, EPI_ACCUM | EPI_OUT_F32, true>(c, a)
+                     : tc::launch_pair<256, EPI_ACCUM | EPI_OUT_F32, false>(c, a);
+      case EPI_BIAS: if (!split) return tc::launch_pair<256, EPI_BIAS, false>(c, a); break;
+      case EPI_BIAS | EPI_RELU | EPI_BITS_OUT:
+        if (!split) return tc::launch_pair<256, EPI_BIAS | EPI_RELU | EPI_BITS_OUT, false>(c, a);
+        break;
+      case EPI_MASK | EPI_COLSUM: if (!split) return tc::launch_pair<256, EPI_MASK | EPI_COLSUM, false>(c, a); break;
       default: break;
     }
   }
-  return tc::launch_pair<256, 1, -1>(c, a);
+  return tc::launch_pair<256, -1, true>(c, a);
 }
 
 }  // namespace gp

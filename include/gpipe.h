@@ -169,6 +169,35 @@ int gpipe_optimizer_slot_bytes(const gpipe_t *g, size_t *bytes_out);
 int gpipe_attach_optimizer_slots(gpipe_t *g, void *slots_dev, size_t bytes);
 int gpipe_apply_rmsprop(gpipe_t *g, float lr, float rho, float eps);
 
+/* ---- data-parallel replicas with the gradient reduction fused into the apply (PAPER.md:45:
+ * GPipe "can be complemented with data parallelism to further scale training") ----
+ * R replicas - one handle per GPU, created with the same spec, K, M, remat and n_seqs, started from the same
+ * parameters - each run gpipe_step on their own mini-batch.  gpipe_dp_apply_* then replaces gpipe_apply_*: replica
+ * `rank` owns the shard gpipe_dp_shard(n_flat, rank, world) of the flat parameter range and, in ONE kernel, sums
+ * that shard's gradients over all replicas (loads through peer_arenas[p], rank order, times grad_scale - 1/R for
+ * the mean over replicas, which with equal mini-batch sizes is the mean loss of the union), zeroes them in every
+ * replica, applies the update to its master shard (SGD, or RMSProp with its own slot shard) and stores the new
+ * master and working-copy values into every replica: reduce-scatter + optimizer + all-gather over NVLink peer
+ * memory with no staging buffer and no collective call.  All replicas end with bit-identical parameters.
+ *   peer_arenas: HOST array of `world` DEVICE pointers, peer_arenas[p] = the address under which THIS process
+ *   reaches replica p's arena (its own arena for p == rank; a CUDA-IPC mapping - gpipe_ipc_export / gpipe_ipc_open -
+ *   or, several handles in one process, the other handle's arena).  Offsets inside the arena are the same for every
+ *   replica (gpipe_dp_layout reports them).
+ *   Ordering: the kernel waits on no other replica.  The CALLER separates the phases: every replica's gpipe_step has
+ *   returned before any replica calls gpipe_dp_apply_*, and every replica's gpipe_dp_apply_* has returned before
+ *   the next gpipe_step (torch.distributed barriers in the Python binding).  Synchronous on return. */
+int gpipe_dp_shard(int64_t n_flat, int rank, int world, int64_t *lo, int64_t *hi);      /* host only */
+int gpipe_dp_layout(const gpipe_t *g, int64_t *n_flat, size_t *master_off, size_t *grad_off, size_t *wlp_off);
+int gpipe_dp_apply_sgd(gpipe_t *g, int rank, int world, void *const *peer_arenas, float lr, float grad_scale);
+int gpipe_dp_apply_rmsprop(gpipe_t *g, int rank, int world, void *const *peer_arenas, float lr, float rho, float eps,
+                           float grad_scale);
+/* CUDA IPC for the peer arenas: handle (64 bytes, host) of the device ALLOCATION containing dev_ptr plus dev_ptr's
+ * byte offset in it; gpipe_ipc_open maps a peer's allocation into this process (returns its base; add the offset);
+ * gpipe_ipc_close unmaps it. */
+int gpipe_ipc_export(const void *dev_ptr, unsigned char *handle_out, size_t *offset_out);
+int gpipe_ipc_open(const unsigned char *handle, void **base_out);
+int gpipe_ipc_close(void *base);
+
 int gpipe_num_tensors(const gpipe_t *g);
 /* *name points into library-owned storage valid until gpipe_destroy. */
 int gpipe_tensor_info(const gpipe_t *g, int i, const char **name, int64_t *rows, int64_t *cols);

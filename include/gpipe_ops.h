@@ -91,6 +91,12 @@ int gpipe_op_embed_fwd(void *stream, int dtype, const int32_t *tok, const void *
 int gpipe_op_embed_bwd(void *stream, const int32_t *tok, const float *dx, float *gemb, int64_t n_tok, int d);
 int gpipe_op_positional(void *stream, float *pe, int S, int d);
 /* master -= lr*grad; w_lp = RNE(master) (bf16 mode, may be NULL); grad = 0.  n multiple of 4. */
+/* The fused data-parallel apply of gpipe_dp_apply_sgd on raw arrays: replica `rank` of `world`
+ * sums grad[0..world)[i] over its shard gpipe_dp_shard(n, rank, world) in rank order, times grad_scale, clears them,
+ * updates master[rank][i] and stores the result (and its RNE-bf16 copy when w_lp != NULL) into every replica.
+ * master / grad / w_lp: HOST arrays of `world` DEVICE pointers (n fp32 / n fp32 / n bf16 elements each). */
+int gpipe_op_dp_apply_sgd(void *stream, int dtype, int world, int rank, float *const *master, float *const *grad,
+                          void *const *w_lp, int64_t n, float lr, float grad_scale);
 /* ms = rho*ms + (1-rho)*grad^2; master -= lr*grad/(sqrt(ms)+eps); w_lp = RNE(master) (may be NULL); grad = 0. */
 int gpipe_op_rmsprop(void *stream, int dtype, float *master, float *grad, float *ms, void *w_lp, int64_t n, float lr,
                      float rho, float eps);

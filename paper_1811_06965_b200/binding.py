@@ -76,6 +76,13 @@ def lib() -> C.CDLL:
         "gpipe_attach_optimizer_slots": (i32, [vp, vp, C.c_size_t]),
         "gpipe_apply_rmsprop": (i32, [vp, f32, f32, f32]),
         "gpipe_zero_grads": (i32, [vp]),
+        "gpipe_dp_shard": (i32, [i64, i32, i32, C.POINTER(i64), C.POINTER(i64)]),
+        "gpipe_dp_layout": (i32, [vp, C.POINTER(i64), C.POINTER(C.c_size_t), C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]),
+        "gpipe_dp_apply_sgd": (i32, [vp, i32, i32, C.POINTER(vp), f32, f32]),
+        "gpipe_dp_apply_rmsprop": (i32, [vp, i32, i32, C.POINTER(vp), f32, f32, f32, f32]),
+        "gpipe_ipc_export": (i32, [vp, C.c_char_p, C.POINTER(C.c_size_t)]),
+        "gpipe_ipc_open": (i32, [C.c_char_p, C.POINTER(vp)]),
+        "gpipe_ipc_close": (i32, [vp]),
         "gpipe_num_tensors": (i32, [vp]),
         "gpipe_tensor_info": (i32, [vp, i32, C.POINTER(C.c_char_p), C.POINTER(i64), C.POINTER(i64)]),
         "gpipe_get_param": (i32, [vp, i32, vp]),
@@ -110,6 +117,7 @@ def lib() -> C.CDLL:
         "gpipe_op_embed_bwd": (i32, [vp, vp, vp, vp, i64, i32]),
         "gpipe_op_positional": (i32, [vp, vp, i32, i32]),
         "gpipe_op_sgd": (i32, [vp, i32, vp, vp, vp, i64, f32]),
+        "gpipe_op_dp_apply_sgd": (i32, [vp, i32, i32, i32, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), i64, f32, f32]),
         "gpipe_op_rmsprop": (i32, [vp, i32, vp, vp, vp, vp, i64, f32, f32, f32]),
     }
     for name, (res, args) in sig.items():
@@ -124,14 +132,15 @@ EXPORTED_SYMBOLS = [
     "gpipe_plan_bytes", "gpipe_create", "gpipe_destroy", "gpipe_layer_costs", "gpipe_partition_min_variance",
     "gpipe_create_partitioned", "gpipe_cell_range", "gpipe_init_params", "gpipe_step",
     "gpipe_step_device", "gpipe_apply_sgd", "gpipe_optimizer_slot_bytes", "gpipe_attach_optimizer_slots",
-    "gpipe_apply_rmsprop", "gpipe_op_rmsprop", "gpipe_zero_grads", "gpipe_num_tensors",
+    "gpipe_apply_rmsprop", "gpipe_op_rmsprop", "gpipe_zero_grads", "gpipe_dp_shard", "gpipe_dp_layout",
+    "gpipe_dp_apply_sgd", "gpipe_dp_apply_rmsprop", "gpipe_ipc_export", "gpipe_ipc_open", "gpipe_ipc_close", "gpipe_num_tensors",
     "gpipe_tensor_info", "gpipe_get_param", "gpipe_set_param", "gpipe_get_grad", "gpipe_get_master", "gpipe_set_master",
     "gpipe_get_optimizer_slot", "gpipe_set_optimizer_slot", "gpipe_peak_bytes",
     "gpipe_trace", "gpipe_launch_count", "gpipe_cuda_graph", "gpipe_cuda_graph_state", "gpipe_kernel_timing", "gpipe_kernel_stats", "gpipe_debug_read", "gpipe_last_error", "gpipe_version",
     "gpipe_op_gemm", "gpipe_op_gemm_workspace_bytes", "gpipe_op_ln_fwd", "gpipe_op_ln_bwd_scratch_floats", "gpipe_op_ln_bwd",
     "gpipe_op_attn_fwd", "gpipe_op_attn_bwd", "gpipe_op_softmax_ce", "gpipe_op_colsum",
     "gpipe_op_colsum_scratch_floats",
-    "gpipe_op_embed_fwd", "gpipe_op_embed_bwd", "gpipe_op_positional", "gpipe_op_sgd",
+    "gpipe_op_embed_fwd", "gpipe_op_embed_bwd", "gpipe_op_positional", "gpipe_op_sgd", "gpipe_op_dp_apply_sgd",
 ]
 
 
@@ -152,6 +161,13 @@ def make_spec(n_layers, d_model, d_ffn, n_heads, d_head, vocab, seq_len, dtype, 
         keep = (C.c_uint8 * max(n_layers, 1))(*[1 if c else 0 for c in causal])
         ptr = C.cast(keep, C.POINTER(C.c_uint8))
     return LayerSpec(n_layers, d_model, d_ffn, n_heads, d_head, vocab, seq_len, dt, ptr, ln_eps), keep
+
+
+def dp_shard(n_flat: int, rank: int, world: int) -> Tuple[int, int]:
+    """gpipe_dp_shard: the [lo, hi) element range of the flat parameter array replica `rank` owns; host-only."""
+    lo, hi = C.c_int64(), C.c_int64()
+    _check(lib().gpipe_dp_shard(n_flat, rank, world, C.byref(lo), C.byref(hi)))
+    return lo.value, hi.value
 
 
 def plan_bytes(spec: LayerSpec, K: int, M: int, remat: bool, n_seqs: int) -> int:
@@ -297,6 +313,34 @@ class GPipe:
     def zero_grads(self):
         with self._torch.cuda.device(self.device):
             _check(lib().gpipe_zero_grads(self._h))
+
+    # -- data-parallel replicas ---------------------------------------------------
+    @property
+    def arena_base(self) -> int:
+        """Device address of the (1024-byte aligned) arena this handle carved its memory from."""
+        return (self.arena.data_ptr() + 1023) // 1024 * 1024
+
+    def dp_layout(self) -> Dict[str, int]:
+        n, mo, go, wo = C.c_int64(), C.c_size_t(), C.c_size_t(), C.c_size_t()
+        _check(lib().gpipe_dp_layout(self._h, C.byref(n), C.byref(mo), C.byref(go), C.byref(wo)))
+        return {"n_flat": n.value, "master_off": mo.value, "grad_off": go.value, "wlp_off": wo.value}
+
+    def dp_apply_sgd(self, rank: int, peer_arenas: Sequence[int], lr: float, grad_scale: Optional[float] = None):
+        """Fused cross-replica gradient sum + SGD + all-gather of the update for this replica's shard.
+        peer_arenas[p]: device address of replica p's arena as seen from this process."""
+        world = len(peer_arenas)
+        arr = (C.c_void_p * world)(*[int(a) for a in peer_arenas])
+        with self._torch.cuda.device(self.device):
+            _check(lib().gpipe_dp_apply_sgd(self._h, rank, world, arr, lr, 1.0 / world if grad_scale is None else grad_scale))
+
+    def dp_apply_rmsprop(self, rank: int, peer_arenas: Sequence[int], lr: float, rho: float = 0.9, eps: float = 1e-8,
+                         grad_scale: Optional[float] = None):
+        world = len(peer_arenas)
+        arr = (C.c_void_p * world)(*[int(a) for a in peer_arenas])
+        with self._torch.cuda.device(self.device):
+            self._ensure_slots()
+            _check(lib().gpipe_dp_apply_rmsprop(self._h, rank, world, arr, lr, rho, eps,
+                                                1.0 / world if grad_scale is None else grad_scale))
 
     # -- parameters -----------------------------------------------------------------------------
     def _idx(self, key) -> int:

@@ -350,6 +350,93 @@ int gpipe_apply_rmsprop(gpipe_t *g, float lr, float rho, float eps) {
   return GPIPE_OK;
 }
 
+// ---- data-parallel replicas -------------------------------------------------------------------
+int gpipe_dp_shard(int64_t n_flat, int rank, int world, int64_t *lo, int64_t *hi) {
+  if (n_flat < 0 || world < 1 || rank < 0 || rank >= world || !lo || !hi) return fail(GPIPE_EINVAL, "need n_flat >= 0, 0 <= rank < world");
+  dp_shard(n_flat, rank, world, lo, hi);
+  return GPIPE_OK;
+}
+
+int gpipe_dp_layout(const gpipe_t *g, int64_t *n_flat, size_t *master_off, size_t *grad_off, size_t *wlp_off) {
+  if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
+  const Engine &e = g->e;
+  if (n_flat) *n_flat = e.n_flat;
+  if (master_off) *master_off = (size_t)((const char *)e.master - e.arena.base);
+  if (grad_off) *grad_off = (size_t)((const char *)e.grad - e.arena.base);
+  if (wlp_off) *wlp_off = e.dt == GP_BF16 ? (size_t)((const char *)e.w_lp - e.arena.base) : (size_t)0;
+  return GPIPE_OK;
+}
+
+static int dp_apply_impl(gpipe_t *g, int rank, int world, void *const *peer_arenas, float lr, float grad_scale, int rms,
+                         float rho, float eps, const char *where) {
+  if (!g || !peer_arenas) return fail(GPIPE_EINVAL, "handle and peer_arenas are required");
+  Engine &e = g->e;
+  if (world < 1 || world > DpPeers::kMax || rank < 0 || rank >= world)
+    return fail(GPIPE_EINVAL, "need 1 <= world <= " + std::to_string(DpPeers::kMax) + " and 0 <= rank < world");
+  if (peer_arenas[rank] != (void *)e.arena.base) return fail(GPIPE_EINVAL, "peer_arenas[rank] must be this handle's own arena");
+  if (rms && !e.opt_ms) return fail(GPIPE_EINVAL, "call gpipe_attach_optimizer_slots first");
+  if (rms && (!(rho >= 0.f && rho < 1.f) || !(eps > 0.f))) return fail(GPIPE_EINVAL, "need 0 <= rho < 1 and eps > 0");
+  DpPeers P{};
+  const size_t mo = (size_t)((char *)e.master - e.arena.base), go = (size_t)((char *)e.grad - e.arena.base);
+  const size_t wo = e.dt == GP_BF16 ? (size_t)((char *)e.w_lp - e.arena.base) : 0;
+  for (int p = 0; p < world; ++p) {
+    if (!peer_arenas[p]) return fail(GPIPE_EINVAL, "peer_arenas[" + std::to_string(p) + "] is NULL");
+    char *b = (char *)peer_arenas[p];                       // same spec, K, M, n_seqs -> same plan -> same offsets
+    P.master[p] = (float *)(b + mo);
+    P.grad[p] = (float *)(b + go);
+    P.wlp[p] = e.dt == GP_BF16 ? (void *)(b + wo) : nullptr;
+  }
+  P.slot = rms ? e.opt_ms : nullptr;
+  Ctx c = e.ctx(0);
+  API_CUDA(dp_apply(c, e.dt, P, world, rank, e.n_flat, lr, grad_scale, rms, rho, eps), where);
+  API_CUDA(cudaStreamSynchronize(c.stream), where);
+  return GPIPE_OK;
+}
+
+int gpipe_dp_apply_sgd(gpipe_t *g, int rank, int world, void *const *peer_arenas, float lr, float grad_scale) {
+  return dp_apply_impl(g, rank, world, peer_arenas, lr, grad_scale, 0, 0.f, 1.f, "gpipe_dp_apply_sgd");
+}
+
+int gpipe_dp_apply_rmsprop(gpipe_t *g, int rank, int world, void *const *peer_arenas, float lr, float rho, float eps,
+                           float grad_scale) {
+  return dp_apply_impl(g, rank, world, peer_arenas, lr, grad_scale, 1, rho, eps, "gpipe_dp_apply_rmsprop");
+}
+
+// CUDA IPC plumbing for the peer arenas (one process per GPU): the handle of the ALLOCATION that contains dev_ptr and
+// the offset of dev_ptr inside it; the peer opens the allocation and adds the offset.
+int gpipe_ipc_export(const void *dev_ptr, unsigned char *handle_out, size_t *offset_out) {
+  if (!dev_ptr || !handle_out || !offset_out) return fail(GPIPE_EINVAL, "arguments are required");
+  typedef int (*GetRangeFn)(unsigned long long *, size_t *, unsigned long long);
+  void *fp = nullptr;
+  cudaDriverEntryPointQueryResult q;
+  API_CUDA(cudaGetDriverEntryPoint("cuMemGetAddressRange", &fp, cudaEnableDefault, &q), "gpipe_ipc_export");
+  if (!fp || q != cudaDriverEntryPointSuccess) return fail(GPIPE_ECUDA, "gpipe_ipc_export: cuMemGetAddressRange unavailable");
+  unsigned long long base = 0;
+  size_t size = 0;
+  if (((GetRangeFn)fp)(&base, &size, (unsigned long long)(uintptr_t)dev_ptr) != 0)
+    return fail(GPIPE_ECUDA, "gpipe_ipc_export: cuMemGetAddressRange failed (not a device allocation?)");
+  cudaIpcMemHandle_t h;
+  API_CUDA(cudaIpcGetMemHandle(&h, (void *)(uintptr_t)base), "gpipe_ipc_export");
+  static_assert(sizeof(h) == 64, "cudaIpcMemHandle_t is 64 bytes");
+  memcpy(handle_out, &h, 64);
+  *offset_out = (size_t)((uintptr_t)dev_ptr - (uintptr_t)base);
+  return GPIPE_OK;
+}
+
+int gpipe_ipc_open(const unsigned char *handle, void **base_out) {
+  if (!handle || !base_out) return fail(GPIPE_EINVAL, "arguments are required");
+  cudaIpcMemHandle_t h;
+  memcpy(&h, handle, 64);
+  API_CUDA(cudaIpcOpenMemHandle(base_out, h, cudaIpcMemLazyEnablePeerAccess), "gpipe_ipc_open");
+  return GPIPE_OK;
+}
+
+int gpipe_ipc_close(void *base) {
+  if (!base) return GPIPE_OK;
+  API_CUDA(cudaIpcCloseMemHandle(base), "gpipe_ipc_close");
+  return GPIPE_OK;
+}
+
 int gpipe_zero_grads(gpipe_t *g) {
   if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
   Engine &e = g->e;

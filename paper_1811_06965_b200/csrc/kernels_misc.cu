@@ -228,6 +228,80 @@ cudaError_t rmsprop_apply(const Ctx &c, int dt, float *master, float *grad, floa
 }
 
 // ---------------------------------------------------------------------------------------------
+// Data-parallel replicas: gradient reduction fused with the apply ("scale ... using
+// data parallelism": R replicas of the pipeline hold identical parameters and take different mini-batches).
+// Replica r owns the contiguous shard [lo, hi) of the flat parameter range.  One kernel per replica, launched after
+// every replica's gpipe_step has finished:
+//   g   = scale * (grad_0[i] + grad_1[i] + ... + grad_{R-1}[i])       peer loads over NVLink, summed in rank order
+//   grad_p[i] = 0 for every p                                         (nobody but the owner reads shard elements)
+//   SGD:      m = master_r[i] - lr g
+//   RMSProp:  ms_r[i] = rho ms_r[i] + (1 - rho) g^2 ;  m = master_r[i] - lr g / (sqrt(ms_r[i]) + eps)
+//   master_p[i] = m, working copy_p[i] = RNE(m) for every p           peer stores: the all-gather of the update
+// i.e. reduce-scatter + optimizer + all-gather in one pass over the shard, no staging buffers, no collective
+// library call; every replica ends with bit-identical parameters (one owner computes each element, in a fixed
+// order).  The kernel waits on no other replica: ordering between replicas is the host's (a barrier before - all
+// gradients final - and after - all parameters updated), so R launches may also run back to back on ONE device
+// (how the single-GPU tests emulate R ranks).  Roofline: NVLink for R > 1 ((R-1)/R of 4 B read + 10 B written per
+// parameter cross the links), HBM for R = 1.
+// ---------------------------------------------------------------------------------------------
+template <typename T, bool RMS>
+__global__ void __launch_bounds__(256)
+dp_apply_kernel(DpPeers P, int world, int self, int64_t lo4, int64_t hi4, float lr, float gscale, float rho, float eps) {
+  const float om = 1.f - rho;
+  for (int64_t i = lo4 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < hi4; i += (int64_t)gridDim.x * blockDim.x) {
+    float4 g = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int p = 0; p < world; ++p) {                       // rank order: the sum is the same whoever computes it
+      const float4 q = load4(P.grad[p] + 4 * i);
+      g.x += q.x; g.y += q.y; g.z += q.z; g.w += q.w;
+    }
+    g.x *= gscale; g.y *= gscale; g.z *= gscale; g.w *= gscale;
+    float4 m = load4(P.master[self] + 4 * i);
+    if (RMS) {
+      float4 v = load4(P.slot + 4 * i);
+      v.x = rho * v.x + om * g.x * g.x; v.y = rho * v.y + om * g.y * g.y;
+      v.z = rho * v.z + om * g.z * g.z; v.w = rho * v.w + om * g.w * g.w;
+      m.x -= lr * g.x / (sqrtf(v.x) + eps); m.y -= lr * g.y / (sqrtf(v.y) + eps);
+      m.z -= lr * g.z / (sqrtf(v.z) + eps); m.w -= lr * g.w / (sqrtf(v.w) + eps);
+      store4(P.slot + 4 * i, v);
+    } else {
+      m.x -= lr * g.x; m.y -= lr * g.y; m.z -= lr * g.z; m.w -= lr * g.w;
+    }
+    for (int p = 0; p < world; ++p) {
+      store4(P.grad[p] + 4 * i, make_float4(0.f, 0.f, 0.f, 0.f));
+      store4(P.master[p] + 4 * i, m);
+      if (P.wlp[p]) store4(reinterpret_cast<T *>(P.wlp[p]) + 4 * i, m);
+    }
+  }
+}
+
+// the shard of replica `rank`: 64-element aligned cuts of [0, n) (every tensor starts on a 64-element boundary)
+void dp_shard(int64_t n, int rank, int world, int64_t *lo, int64_t *hi) {
+  const int64_t blocks = (n + 63) / 64, per = (blocks + world - 1) / world;
+  int64_t a = (int64_t)rank * per * 64, b = (int64_t)(rank + 1) * per * 64;
+  *lo = a < n ? a : n;
+  *hi = b < n ? b : n;
+}
+
+cudaError_t dp_apply(const Ctx &c, int dt, const DpPeers &P, int world, int self, int64_t n, float lr, float gscale,
+                     int rms, float rho, float eps) {
+  if (world < 1 || world > DpPeers::kMax || self < 0 || self >= world) return cudaErrorInvalidValue;
+  int64_t lo, hi;
+  dp_shard(n, self, world, &lo, &hi);
+  if (hi <= lo) return cudaSuccess;
+  const int64_t lo4 = lo / 4, hi4 = hi / 4, n4 = hi4 - lo4;
+  int64_t want = (n4 + 255) / 256;
+  unsigned grid = (unsigned)(want < (int64_t)c.sm_count * 16 ? want : (int64_t)c.sm_count * 16);
+  if (dt == GP_BF16) {
+    if (rms) dp_apply_kernel<bf16, true><<<grid, 256, 0, c.stream>>>(P, world, self, lo4, hi4, lr, gscale, rho, eps);
+    else dp_apply_kernel<bf16, false><<<grid, 256, 0, c.stream>>>(P, world, self, lo4, hi4, lr, gscale, rho, eps);
+  } else {
+    if (rms) dp_apply_kernel<float, true><<<grid, 256, 0, c.stream>>>(P, world, self, lo4, hi4, lr, gscale, rho, eps);
+    else dp_apply_kernel<float, false><<<grid, 256, 0, c.stream>>>(P, world, self, lo4, hi4, lr, gscale, rho, eps);
+  }
+  GP_LAUNCH_CHECK(c);
+}
+
+// ---------------------------------------------------------------------------------------------
 // Philox-4x32-10 counter RNG + Box-Muller; element i uses counter (i/4, stream_id), lane i%4
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ void philox_round(uint32_t &c0, uint32_t &c1, uint32_t &c2, uint32_t &c3,

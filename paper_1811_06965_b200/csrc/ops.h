@@ -117,6 +117,17 @@ cudaError_t sgd_apply(const Ctx &c, int dt, float *master, float *grad, void *w_
                       float lr);
 cudaError_t rmsprop_apply(const Ctx &c, int dt, float *master, float *grad, float *ms, void *w_lp, int64_t n,
                           float lr, float rho, float eps);
+// data-parallel replicas: fused gradient reduce + apply + all-gather of the update over peer-mapped pointers
+struct DpPeers {
+  static constexpr int kMax = 16;
+  float *master[kMax];       // replica p's fp32 master array (addressable from this device)
+  float *grad[kMax];         // replica p's fp32 gradient array
+  void *wlp[kMax];           // replica p's bf16 working copy (NULL in fp32 mode)
+  float *slot;               // this replica's RMSProp slot (NULL for SGD)
+};
+void dp_shard(int64_t n, int rank, int world, int64_t *lo, int64_t *hi);
+cudaError_t dp_apply(const Ctx &c, int dt, const DpPeers &P, int world, int self, int64_t n, float lr, float gscale,
+                     int rms, float rho, float eps);
 cudaError_t init_normal(const Ctx &c, int dt, float *master, void *w_lp, int64_t n, uint64_t seed,
                         uint64_t stream_id, float mean, float std);
 cudaError_t fill_f32(const Ctx &c, float *p, int64_t n, float v);

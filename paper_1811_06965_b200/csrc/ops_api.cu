@@ -220,6 +220,17 @@ int gpipe_op_rmsprop(void *stream, int dtype, float *master, float *grad, float 
                      float rho, float eps) {
   return ret(rmsprop_apply(mk(stream), dtype, master, grad, ms, w_lp, n, lr, rho, eps), "gpipe_op_rmsprop");
 }
+int gpipe_op_dp_apply_sgd(void *stream, int dtype, int world, int rank, float *const *master, float *const *grad,
+                          void *const *w_lp, int64_t n, float lr, float grad_scale) {
+  if (world < 1 || world > DpPeers::kMax || !master || !grad) return ret(cudaErrorInvalidValue, "gpipe_op_dp_apply_sgd");
+  DpPeers P{};
+  for (int p = 0; p < world; ++p) {
+    P.master[p] = master[p];
+    P.grad[p] = grad[p];
+    P.wlp[p] = w_lp ? w_lp[p] : nullptr;
+  }
+  return ret(dp_apply(mk(stream), dtype, P, world, rank, n, lr, grad_scale, 0, 0.f, 1.f), "gpipe_op_dp_apply_sgd");
+}
 int gpipe_op_sgd(void *stream, int dtype, float *master, float *grad, void *w_lp, int64_t n, float lr) {
   return ret(sgd_apply(mk(stream), dtype, master, grad, w_lp, n, lr), "gpipe_op_sgd");
 }

@@ -206,6 +206,20 @@ def main():
         ms = time_it([(lambda s=s: ops.rmsprop(s[0], s[1], s[3], s[2], 1e-3, 0.9, 1e-6)) for s in sets], max(2, args.reps // 2))
         report("sgd", "rmsprop_apply", ms, 0, n * 26.0)          # g r+w, ms r+w, master r+w, bf16 copy w
 
+    # ------------------------------------------------------------------ fused data-parallel apply (f3), R replicas
+    # emulated on this one device: the NVLink hop is absent, so this is the HBM roofline of the kernel -
+    # per parameter of the shard: R x 4 B gradient reads, 4 B master read, R x (4 + 4 + 2) B stores
+    if want("sgd", "dp_apply"):
+        n = 32 * 1024 * 1024
+        for R in (1, 2, 4):
+            ms_ = [torch.randn(n, device=dev) for _ in range(R)]
+            gs_ = [torch.randn(n, device=dev) for _ in range(R)]
+            ws_ = [torch.empty(n, device=dev, dtype=bf) for _ in range(R)]
+            fns = [(lambda r=r: ops.dp_apply_sgd(ms_, gs_, ws_, r, 1e-3)) for r in range(R)]
+            ms = time_it(fns, max(2, args.reps // 2)) * R          # all R shards = one whole update of n parameters
+            report("sgd", "dp_apply_R%d" % R, ms, 0, n * (4.0 * R + 4.0 + 10.0 * R))
+            del ms_, gs_, ws_
+
     if args.json:
         os.makedirs(os.path.dirname(os.path.abspath(args.json)), exist_ok=True)
         with open(args.json, "w") as f:

@@ -131,3 +131,13 @@ def sgd(master, grad, w_lp, lr):
 def rmsprop(master, grad, ms, w_lp, lr, rho, eps):
     B._check(B.lib().gpipe_op_rmsprop(_stream(), B.DTYPE_BF16 if w_lp is not None else B.DTYPE_FP32, _p(master), _p(grad),
                                       _p(ms), _p(w_lp), master.numel(), lr, rho, eps))
+
+
+def dp_apply_sgd(masters, grads, w_lps, rank, lr, grad_scale=None):
+    """Fused data-parallel apply on raw arrays: masters / grads / w_lps are lists (one entry per replica)."""
+    import ctypes as C
+    world = len(masters)
+    arr = lambda ts: (C.c_void_p * world)(*[t.data_ptr() for t in ts])
+    B._check(B.lib().gpipe_op_dp_apply_sgd(_stream(), B.DTYPE_BF16 if w_lps is not None else B.DTYPE_FP32, world, rank,
+                                           arr(masters), arr(grads), arr(w_lps) if w_lps is not None else None,
+                                           masters[0].numel(), lr, 1.0 / world if grad_scale is None else grad_scale))

@@ -102,7 +102,9 @@ def test_fused_dp_apply_bf16_replicas_stay_identical_and_equal_one_big_step():
                 assert np.array_equal(engines[1].get_master(n), m0), n
                 assert np.array_equal(engines[0].get_param(n), engines[1].get_param(n)), n
                 upd, ref = m0 - params[n], one.get_master(n) - params[n]
-                assert maxrel(upd, ref) <= 1e-5 and cosine(upd, ref) >= 0.9999999, n
+                # the update is read back as (new master - old parameter): a difference of fp32 numbers ~1e3 x larger
+                # than itself, so the comparison carries their rounding (2^-24 x |w| / |update| ~ 1e-5 .. 1e-4)
+                assert maxrel(upd, ref) <= 2e-4 and cosine(upd, ref) >= 0.999999, n
         import torch
         for e in engines:                                        # working copy = RNE(master) for matrices
             wq = e.get_param("l0.w_qkv")

@@ -252,7 +252,9 @@ def run_ours(args, w, rank, world, local_rank):
     torch.cuda.synchronize(dev)
     free_before, _ = torch.cuda.mem_get_info(dev)
     torch.cuda.reset_peak_memory_stats(dev)
-    eng = gp.from_workload(w, device=dev, partition=None if args.partition == "equal" else args.partition)
+    pipe_devices = [int(x) for x in args.pipeline_devices.split(",")] if args.pipeline_devices else None
+    eng = gp.from_workload(w, device=dev, partition=None if args.partition == "equal" else args.partition,
+                           devices=pipe_devices, staged=bool(pipe_devices) and args.pipeline_staged)
     eng.init_params(seed=1000 + rank, std=0.02, parity=False)
     progress("engine ready (%.1f GB arena)" % (eng.peak_bytes()["total"] / 1e9))
     tok, lab = gi.make_tokens(w, 2000 + rank)
@@ -358,7 +360,8 @@ def run_ours(args, w, rank, world, local_rank):
                        "n_heads": w.n_heads, "d_head": w.d_head, "vocab": w.vocab, "seq_len": w.seq_len,
                        "n_seqs": w.n_seqs, "K": w.K, "M": w.M, "remat": w.remat, "partition": args.partition,
                        "layers_per_cell": [hi - lo for lo, hi in eng.cells],
-                       "parallelism": "replicas" if world > 1 else "1 GPU, K streams",
+                       "parallelism": ("pipeline over devices %s%s" % (pipe_devices, " (staged boundary copies)" if args.pipeline_staged else ""))
+                       if pipe_devices else ("replicas" if world > 1 else "1 GPU, K streams"),
                        "l2": "inputs larger than L2 (activations+weights per step >> 126 MB)"},
             "loss": loss,
             "tflops_executed": fl["executed"] / step_s / 1e12, "tflops_model": fl["model"] / step_s / 1e12,
@@ -394,6 +397,10 @@ def main():
                     help="variant row of reading A3: d_head = d_model / n_heads = 32 for the 32-head configs (d_attn 1024)")
     ap.add_argument("--partition", default="equal", choices=["equal", "cost"],
                     help="equal: L/K consecutive layers per cell; cost: minimum variance of the estimated cell costs (PAPER.md:65)")
+    ap.add_argument("--pipeline-devices", default=None,
+                    help="comma-separated CUDA device ordinals, one per cell: run the step on the pipeline handle "
+                         "(gpipe_create_pipeline; PAPER.md:65) from THIS process; ordinals may repeat")
+    ap.add_argument("--pipeline-staged", action="store_true", help="force staged boundary copies when cells share a device")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--oracle-full", action="store_true",
                     help="cpu_baseline / --impl reference: one WHOLE oracle step of the workload instead of the bounded "

@@ -137,6 +137,37 @@ int gpipe_create_partitioned(const gpipe_layer_spec *spec, int K, int M, int rem
                              const gpipe_env *env, const int32_t *cell_lo, gpipe_t **out);
 int gpipe_cell_range(const gpipe_t *g, int k, int32_t *lo, int32_t *hi);
 
+/* ---- the pipeline across accelerators ("GPipe places the k-th cell on the k-th
+ * accelerator", "only needs to pass activation tensors at the partition boundaries") ----
+ * gpipe_create_pipeline builds the same engine with ONE arena, ONE stream and ONE device PER CELL: cell k's
+ * parameters, gradient accumulators, optimizer slots, boundary slots, interior workspaces and scratch live in
+ * cells[k].arena on device cells[k].device, and its tasks F(k,m), R(k,m), B(k,m) run on cells[k].stream.  The only
+ * tensors that move between arenas are the boundary activation ([T_mb, d] fp32, forward) and its gradient (fp32 +
+ * the bf16 operand copy, backward): cudaMemcpyPeerAsync on the producing cell's stream, ordered with the consumer
+ * by the same events as the single-device schedule (cudaStreamWaitEvent works across devices of one process).
+ * Token ids go to cell 0's device, labels to cell K-1's.  The schedule, the kernels and therefore every result
+ * are those of gpipe_create (bitwise, except the FFN2 bias gradient of each cell's last layer, which the owning
+ * cell now sums itself).  All devices must be visible to THIS process; the call enables peer access between
+ * neighbouring cells' devices.  Cells may share a device (cells[k].device all equal): the same code path on one
+ * GPU - how the single-GPU tests cover it; flags & GPIPE_PIPE_STAGED then forces the staged boundary copies that
+ * different devices always use.  One handle = one host thread driving K devices; the step is enqueued eagerly
+ * (no CUDA graph) when the devices differ.  gpipe_plan_bytes_pipeline: bytes each cell's arena needs (host only;
+ * cell_lo may be NULL for the equal split).  Optimizer slots: gpipe_attach_optimizer_slots_cell per cell
+ * (gpipe_cell_param_count(k) * 4 bytes on that cell's device). */
+typedef struct {
+  int32_t device;       /* CUDA device ordinal of this cell                                    */
+  void   *arena;        /* device memory ON THAT DEVICE, >= gpipe_plan_bytes_pipeline()[k], 1024-byte aligned */
+  size_t  arena_bytes;
+  void   *stream;       /* cudaStream_t created on that device                                 */
+} gpipe_cell_env;
+#define GPIPE_PIPE_STAGED 1
+int gpipe_plan_bytes_pipeline(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs,
+                              const int32_t *cell_lo, size_t *bytes_out /* [K] */);
+int gpipe_create_pipeline(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs,
+                          const gpipe_cell_env *cells /* [K] */, const int32_t *cell_lo, int flags, gpipe_t **out);
+int gpipe_attach_optimizer_slots_cell(gpipe_t *g, int k, void *slots_dev, size_t bytes);
+int gpipe_cell_param_count(const gpipe_t *g, int k, int64_t *n_out);
+
 /* N(0, std) for matrices and emb, from a counter-based generator on the device (Philox-4x32-10
  * + Box-Muller); parity != 0 also draws biases / beta ~ N(0,std) and gamma = 1 + N(0,std)
  * (reading A10), parity == 0 sets gamma = 1, beta = bias = 0.  bf16 mode: the master is the

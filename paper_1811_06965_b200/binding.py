@@ -39,6 +39,13 @@ class Env(C.Structure):
                 ("streams", C.POINTER(C.c_void_p)), ("n_streams", C.c_int32)]
 
 
+class CellEnv(C.Structure):
+    _fields_ = [("device", C.c_int32), ("arena", C.c_void_p), ("arena_bytes", C.c_size_t), ("stream", C.c_void_p)]
+
+
+PIPE_STAGED = 1
+
+
 class TraceEvent(C.Structure):
     _fields_ = [("kind", C.c_int32), ("k", C.c_int32), ("m", C.c_int32), ("enqueue_index", C.c_int32),
                 ("start_ms", C.c_float), ("end_ms", C.c_float)]
@@ -68,6 +75,12 @@ def lib() -> C.CDLL:
         "gpipe_create_partitioned": (i32, [C.POINTER(LayerSpec), i32, i32, i32, i64, C.POINTER(Env),
                                            C.POINTER(C.c_int32), C.POINTER(vp)]),
         "gpipe_cell_range": (i32, [vp, i32, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]),
+        "gpipe_plan_bytes_pipeline": (i32, [C.POINTER(LayerSpec), i32, i32, i32, i64, C.POINTER(C.c_int32),
+                                            C.POINTER(C.c_size_t)]),
+        "gpipe_create_pipeline": (i32, [C.POINTER(LayerSpec), i32, i32, i32, i64, C.POINTER(CellEnv),
+                                        C.POINTER(C.c_int32), i32, C.POINTER(vp)]),
+        "gpipe_attach_optimizer_slots_cell": (i32, [vp, i32, vp, C.c_size_t]),
+        "gpipe_cell_param_count": (i32, [vp, i32, C.POINTER(i64)]),
         "gpipe_init_params": (i32, [vp, C.c_uint64, f32, i32]),
         "gpipe_step": (i32, [vp, vp, vp, C.POINTER(f32)]),
         "gpipe_step_device": (i32, [vp, vp, vp, C.POINTER(f32)]),
@@ -130,7 +143,8 @@ def lib() -> C.CDLL:
 
 EXPORTED_SYMBOLS = [
     "gpipe_plan_bytes", "gpipe_create", "gpipe_destroy", "gpipe_layer_costs", "gpipe_partition_min_variance",
-    "gpipe_create_partitioned", "gpipe_cell_range", "gpipe_init_params", "gpipe_step",
+    "gpipe_create_partitioned", "gpipe_cell_range", "gpipe_plan_bytes_pipeline", "gpipe_create_pipeline",
+    "gpipe_attach_optimizer_slots_cell", "gpipe_cell_param_count", "gpipe_init_params", "gpipe_step",
     "gpipe_step_device", "gpipe_apply_sgd", "gpipe_optimizer_slot_bytes", "gpipe_attach_optimizer_slots",
     "gpipe_apply_rmsprop", "gpipe_op_rmsprop", "gpipe_zero_grads", "gpipe_dp_shard", "gpipe_dp_layout",
     "gpipe_dp_apply_sgd", "gpipe_dp_apply_rmsprop", "gpipe_ipc_export", "gpipe_ipc_open", "gpipe_ipc_close", "gpipe_num_tensors",
@@ -177,6 +191,14 @@ def plan_bytes(spec: LayerSpec, K: int, M: int, remat: bool, n_seqs: int) -> int
     return int(out.value)
 
 
+def plan_bytes_pipeline(spec: LayerSpec, K: int, M: int, remat: bool, n_seqs: int, cell_lo=None) -> List[int]:
+    """gpipe_plan_bytes_pipeline: bytes each cell's arena needs when every cell has its own; host-only."""
+    out = (C.c_size_t * K)()
+    lo = (C.c_int32 * (K + 1))(*[int(v) for v in cell_lo]) if cell_lo is not None else None
+    _check(lib().gpipe_plan_bytes_pipeline(C.byref(spec), K, M, int(bool(remat)), n_seqs, lo, out))
+    return [int(out[k]) for k in range(K)]
+
+
 def layer_costs(spec: LayerSpec, remat: bool) -> Tuple[List[float], float, float]:
     """gpipe_layer_costs: (per-layer costs, embedding cost, head cost); host-only."""
     L = spec.n_layers
@@ -198,10 +220,15 @@ def partition_min_variance(costs, first_extra: float, last_extra: float, K: int)
 class GPipe:
     """gpipe_create / gpipe_step / gpipe_apply_sgd (BASELINE.json north_star) on one B200.
     partition: None (equal consecutive split), "cost" (gpipe_layer_costs + gpipe_partition_min_variance,
-    PAPER.md:65) or an explicit list of K+1 boundaries."""
+    PAPER.md:65) or an explicit list of K+1 boundaries.
+    devices: None - all K cells on `device`, one arena, K streams; or a list of K CUDA device ordinals - the
+    pipeline across accelerators (gpipe_create_pipeline): cell k's arena and stream live on
+    devices[k] (the ordinals may repeat: several cells, or all of them, on one GPU); staged=True forces the
+    boundary copies that different devices always use."""
 
     def __init__(self, *, n_layers, d_model, d_ffn, n_heads, d_head, vocab, seq_len, dtype, K, M,
-                 remat=True, n_seqs, causal=None, ln_eps=1e-5, device="cuda:0", partition=None):
+                 remat=True, n_seqs, causal=None, ln_eps=1e-5, device="cuda:0", partition=None, devices=None,
+                 staged=False):
         import torch
         if not torch.cuda.is_available():
             raise GPipeError(-2, "no CUDA device: the GPipe path has no CPU fallback")
@@ -211,6 +238,43 @@ class GPipe:
                                           dtype, causal, ln_eps)
         self.K, self.M, self.remat, self.n_seqs, self.seq_len = K, M, bool(remat), n_seqs, seq_len
         self._h = C.c_void_p(None)
+        self.devices = None if devices is None else [int(d) for d in devices]
+        if self.devices is not None:
+            self._create_pipeline(torch, K, M, n_seqs, partition, staged)
+        else:
+            self._create_single(torch, K, M, remat, n_seqs, partition)
+        self._finish_init(K)
+
+    def _create_pipeline(self, torch, K, M, n_seqs, partition, staged):
+        if len(self.devices) != K:
+            raise ValueError("devices must list one CUDA device per cell")
+        if any(d < 0 or d >= torch.cuda.device_count() for d in self.devices):
+            raise ValueError("devices %r: this process sees %d CUDA device(s)" % (self.devices, torch.cuda.device_count()))
+        self.device = torch.device("cuda", self.devices[0])
+        if isinstance(partition, str):
+            if partition != "cost":
+                raise ValueError("partition must be None, 'cost' or a list of K+1 boundaries")
+            costs, c_emb, c_head = layer_costs(self.spec, self.remat)
+            partition = partition_min_variance(costs, c_emb, c_head, K)
+        need = plan_bytes_pipeline(self.spec, K, M, self.remat, n_seqs, partition)
+        self.arena = None
+        self.arenas, self.streams = [], []
+        cells = (CellEnv * K)()
+        for k, dev in enumerate(self.devices):
+            d = torch.device("cuda", dev)
+            with torch.cuda.device(d):
+                a = torch.empty(need[k] + 1024, dtype=torch.uint8, device=d)
+                st = torch.cuda.Stream(device=d)
+                torch.cuda.synchronize(d)
+            self.arenas.append(a)
+            self.streams.append(st)
+            cells[k] = CellEnv(dev, (a.data_ptr() + 1023) // 1024 * 1024, need[k], st.cuda_stream)
+        lo = (C.c_int32 * (K + 1))(*[int(v) for v in partition]) if partition is not None else None
+        with torch.cuda.device(self.device):
+            _check(lib().gpipe_create_pipeline(C.byref(self.spec), K, M, int(self.remat), n_seqs, cells, lo,
+                                               PIPE_STAGED if staged else 0, C.byref(self._h)))
+
+    def _create_single(self, torch, K, M, remat, n_seqs, partition):
         with torch.cuda.device(self.device):
             nbytes = plan_bytes(self.spec, K, M, remat, n_seqs)
             self.arena = torch.empty(nbytes + 1024, dtype=torch.uint8, device=self.device)
@@ -231,6 +295,8 @@ class GPipe:
                 lo = (C.c_int32 * (K + 1))(*[int(v) for v in partition])
                 _check(lib().gpipe_create_partitioned(C.byref(self.spec), K, M, int(self.remat), n_seqs,
                                                       C.byref(env), lo, C.byref(self._h)))
+
+    def _finish_init(self, K):
         self.cells = []
         for k in range(K):
             lo_k, hi_k = C.c_int32(0), C.c_int32(0)
@@ -251,6 +317,7 @@ class GPipe:
             lib().gpipe_destroy(self._h)
             self._h = C.c_void_p(None)
         self.arena = None
+        self.arenas = None
         self._slots = None
 
     def __del__(self):
@@ -299,6 +366,17 @@ class GPipe:
             _check(lib().gpipe_apply_rmsprop(self._h, lr, rho, eps))
 
     def _ensure_slots(self):
+        if getattr(self, "_slots", None) is None and self.devices is not None:
+            self._slots = []                                     # pipeline: each cell's slot shard on that cell's device
+            for k, dev in enumerate(self.devices):
+                n = C.c_int64(0)
+                _check(lib().gpipe_cell_param_count(self._h, k, C.byref(n)))
+                d = self._torch.device("cuda", dev)
+                t = self._torch.empty(max(n.value, 1) * 4, dtype=self._torch.uint8, device=d)
+                self._slots.append(t)
+                with self._torch.cuda.device(self.device):
+                    _check(lib().gpipe_attach_optimizer_slots_cell(self._h, k, t.data_ptr(), n.value * 4))
+            return
         with self._torch.cuda.device(self.device):
             if getattr(self, "_slots", None) is None:
                 n = C.c_size_t(0)

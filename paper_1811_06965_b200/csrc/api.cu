@@ -89,6 +89,29 @@ static int configure(Engine &e, const gpipe_layer_spec *spec, int K, int M, int 
   return GPIPE_OK;
 }
 
+// the optimizer kernels run per parameter home: one launch over the whole flat range, or one per cell (pipeline)
+template <typename F>
+static int for_each_home(Engine &e, const char *where, F &&fn) {
+  if (!e.multi()) {
+    Ctx c = e.ctx(0);
+    API_CUDA(fn(c, e.master, e.grad, e.dt == GP_BF16 ? e.w_lp : nullptr, e.opt_ms, e.n_flat), where);
+    API_CUDA(cudaStreamSynchronize(c.stream), where);
+    return GPIPE_OK;
+  }
+  for (int k = 0; k < e.K; ++k) {
+    API_CUDA(e.use(k), where);
+    Ctx c = e.ctx(k);
+    API_CUDA(fn(c, e.cmaster[k], e.cgrad[k], e.dt == GP_BF16 ? e.cwlp[k] : nullptr, e.copt.empty() ? nullptr : e.copt[k],
+                e.cell_off[k + 1] - e.cell_off[k]), where);
+  }
+  for (int k = 0; k < e.K; ++k) {
+    API_CUDA(e.use(k), where);
+    API_CUDA(cudaStreamSynchronize(e.st(k)), where);
+  }
+  API_CUDA(e.use(0), where);
+  return GPIPE_OK;
+}
+
 extern "C" {
 
 const char *gpipe_last_error(void) { return g_err.c_str(); }
@@ -106,8 +129,29 @@ int gpipe_plan_bytes(const gpipe_layer_spec *spec, int K, int M, int remat, int6
   return GPIPE_OK;
 }
 
+int gpipe_plan_bytes_pipeline(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs,
+                              const int32_t *cell_lo, size_t *bytes_out) {
+  if (!bytes_out) return fail(GPIPE_EINVAL, "bytes_out is NULL");
+  Engine e;
+  int rc = configure(e, spec, K, M, remat, n_seqs, cell_lo);
+  if (rc) return rc;
+  e.n_arenas = K;
+  e.parena.assign(K, Arena());
+  if (K > 1) e.boundary_staged = 1;
+  std::string err;
+  rc = e.build_plan(true, err);
+  if (rc) return fail(rc, err);
+  for (int k = 0; k < K; ++k) bytes_out[k] = e.parena[k].used;
+  return GPIPE_OK;
+}
+
 static int create_impl(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs, const gpipe_env *env,
-                       const int32_t *cell_lo, gpipe_t **out);
+                       const int32_t *cell_lo, gpipe_t **out, const gpipe_cell_env *cells = nullptr, int flags = 0);
+int gpipe_create_pipeline(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs,
+                          const gpipe_cell_env *cells, const int32_t *cell_lo, int flags, gpipe_t **out) {
+  if (!cells) return fail(GPIPE_EINVAL, "cells is NULL");
+  return create_impl(spec, K, M, remat, n_seqs, nullptr, cell_lo, out, cells, flags);
+}
 int gpipe_create(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs, const gpipe_env *env, gpipe_t **out) {
   return create_impl(spec, K, M, remat, n_seqs, env, nullptr, out);
 }
@@ -177,19 +221,41 @@ int gpipe_partition_min_variance(const double *layer_cost, int L, double first_e
 }
 
 static int create_impl(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs, const gpipe_env *env,
-                       const int32_t *cell_lo, gpipe_t **out) {
+                       const int32_t *cell_lo, gpipe_t **out, const gpipe_cell_env *cells, int flags) {
   if (!out) return fail(GPIPE_EINVAL, "out is NULL");
   *out = nullptr;
-  if (!env || !env->arena || !env->streams) return fail(GPIPE_EINVAL, "env, env->arena and env->streams are required");
+  const bool pipe = cells != nullptr;
+  if (!pipe && (!env || !env->arena || !env->streams)) return fail(GPIPE_EINVAL, "env, env->arena and env->streams are required");
   gpipe *g = new (std::nothrow) gpipe();
   if (!g) return fail(GPIPE_ENOMEM, "host allocation failed");
   Engine &e = g->e;
   int rc = configure(e, spec, K, M, remat, n_seqs, cell_lo);
   if (rc) { delete g; return rc; }
-  if (env->n_streams < K) { delete g; return fail(GPIPE_EINVAL, "need one stream per cell (n_streams >= K)"); }
-  if ((uintptr_t)env->arena % 1024) { delete g; return fail(GPIPE_EINVAL, "arena must be 1024-byte aligned"); }
   int dev = 0;
   cudaError_t ce = cudaGetDevice(&dev);
+  if (ce != cudaSuccess) { delete g; return cuda_fail(ce, "gpipe_create: no usable CUDA device"); }
+  const int dev_entry = dev;
+  if (pipe) {
+    e.n_arenas = K;
+    e.parena.assign(K, Arena());
+    e.cell_device.assign(K, dev);
+    for (int k = 0; k < K; ++k) {
+      if (!cells[k].arena || !cells[k].stream) { delete g; return fail(GPIPE_EINVAL, "cells[k].arena and cells[k].stream are required"); }
+      if ((uintptr_t)cells[k].arena % 1024) { delete g; return fail(GPIPE_EINVAL, "arenas must be 1024-byte aligned"); }
+      e.cell_device[k] = cells[k].device;
+      if (cells[k].device != cells[0].device) e.multi_device = true;
+      e.parena[k].base = (char *)cells[k].arena;
+      e.parena[k].cap = cells[k].arena_bytes;
+    }
+    e.boundary_staged = (K > 1 && (e.multi_device || (flags & GPIPE_PIPE_STAGED))) ? 1 : 0;
+    if (K > 1 && !e.multi_device && !(flags & GPIPE_PIPE_STAGED)) e.boundary_staged = 0;
+    dev = e.cell_device[0];
+  } else {
+    if (env->n_streams < K) { delete g; return fail(GPIPE_EINVAL, "need one stream per cell (n_streams >= K)"); }
+    if ((uintptr_t)env->arena % 1024) { delete g; return fail(GPIPE_EINVAL, "arena must be 1024-byte aligned"); }
+    e.arena.base = (char *)env->arena;
+    e.arena.cap = env->arena_bytes;
+  }
   e.device = dev;
   if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&e.sm_count, cudaDevAttrMultiProcessorCount, dev);
   int cc_major = 0;
@@ -197,40 +263,67 @@ static int create_impl(const gpipe_layer_spec *spec, int K, int M, int remat, in
   if (ce == cudaSuccess) ce = watchdog_init();
   if (ce != cudaSuccess) { delete g; return cuda_fail(ce, "gpipe_create: no usable CUDA device"); }
   if (cc_major != 10) { delete g; return fail(GPIPE_ECUDA, "gpipe_create: this library is built for sm_100a (B200) only"); }
+  if (e.multi_device) {
+    // neighbouring cells exchange the boundary tensors with peer copies; direct access makes them NVLink transfers
+    for (int k = 0; k + 1 < K && ce == cudaSuccess; ++k) {
+      const int a = e.cell_device[k], b = e.cell_device[k + 1];
+      if (a == b) continue;
+      for (int dir = 0; dir < 2 && ce == cudaSuccess; ++dir) {
+        int can = 0;
+        ce = cudaDeviceCanAccessPeer(&can, dir ? b : a, dir ? a : b);
+        if (ce == cudaSuccess && can) {
+          ce = cudaSetDevice(dir ? b : a);
+          if (ce == cudaSuccess) ce = cudaDeviceEnablePeerAccess(dir ? a : b, 0);
+          if (ce == cudaErrorPeerAccessAlreadyEnabled) { ce = cudaSuccess; cudaGetLastError(); }
+        }
+      }
+    }
+    if (ce != cudaSuccess) { cudaSetDevice(dev_entry); delete g; return cuda_fail(ce, "gpipe_create_pipeline: peer access"); }
+  }
   std::string err;
-  e.arena.base = (char *)env->arena;
-  e.arena.cap = env->arena_bytes;
   rc = e.build_plan(true, err);
-  if (rc == GPIPE_OK && e.arena.used > e.arena.cap)
-    rc = fail(GPIPE_ENOMEM, "arena too small: need " + std::to_string(e.arena.used) + " bytes, have " + std::to_string(e.arena.cap));
+  for (int k = 0; rc == GPIPE_OK && k < (pipe ? K : 1); ++k)
+    if (e.ar(k).used > e.ar(k).cap)
+      rc = fail(GPIPE_ENOMEM, "arena " + std::to_string(k) + " too small: need " + std::to_string(e.ar(k).used) +
+                                  " bytes, have " + std::to_string(e.ar(k).cap));
   if (rc == GPIPE_OK) { rc = e.build_plan(false, err); if (rc) fail(rc, err); }
-  if (rc) { delete g; return rc; }
+  if (rc) { cudaSetDevice(dev_entry); delete g; return rc; }
   e.streams.resize(K);
-  for (int k = 0; k < K; ++k) e.streams[k] = (cudaStream_t)env->streams[k];
+  for (int k = 0; k < K; ++k) e.streams[k] = (cudaStream_t)(pipe ? cells[k].stream : env->streams[k]);
   e.ev_f.assign(K, std::vector<cudaEvent_t>(e.M, nullptr));
   e.ev_b.assign(K, std::vector<cudaEvent_t>(e.M, nullptr));
   e.ev_done.assign(K, nullptr);
   for (int k = 0; k < K && ce == cudaSuccess; ++k) {
+    ce = e.use(k);                                             // an event lives on the device it is recorded on
     for (int m = 0; m < e.M && ce == cudaSuccess; ++m) {
       ce = cudaEventCreateWithFlags(&e.ev_f[k][m], cudaEventDisableTiming);
       if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&e.ev_b[k][m], cudaEventDisableTiming);
     }
     if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&e.ev_done[k], cudaEventDisableTiming);
   }
+  if (ce == cudaSuccess) ce = e.use(0);
   if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&e.ev_in, cudaEventDisableTiming);
   if (ce == cudaSuccess) ce = cudaEventCreate(&e.ev_t0);
   if (ce == cudaSuccess) ce = cudaMallocHost((void **)&e.host_loss, sizeof(float) * (e.M + 1));
-  if (ce == cudaSuccess) ce = cudaMallocHost((void **)&e.host_flag, sizeof(int));
-  Ctx c = e.ctx(0);
+  if (ce == cudaSuccess) ce = cudaMallocHost((void **)&e.host_flag, sizeof(int) * 2);
   // parameters, gradients start at zero; positional table is built once
-  if (ce == cudaSuccess) ce = cudaMemsetAsync(e.master, 0, (size_t)e.n_flat * 4, c.stream);
-  if (ce == cudaSuccess) ce = cudaMemsetAsync(e.grad, 0, (size_t)e.n_flat * 4, c.stream);
-  if (ce == cudaSuccess && e.dt == GP_BF16) ce = cudaMemsetAsync(e.w_lp, 0, (size_t)e.n_flat * 2, c.stream);
-  if (ce == cudaSuccess) ce = cudaMemsetAsync(e.flag_dev, 0, 4, c.stream);
-  for (int k = 0; k < K && ce == cudaSuccess; ++k)          // split-K counters start at zero and reset themselves
-    if (e.bwd[k].splitk_ws) ce = cudaMemsetAsync(e.bwd[k].splitk_ws, 0, e.splitk_ws_bytes, c.stream);
-  if (ce == cudaSuccess) ce = positional_table(c, e.pe, e.S, e.d);
-  if (ce == cudaSuccess) ce = cudaStreamSynchronize(c.stream);
+  for (int k = 0; k < K && ce == cudaSuccess; ++k) {
+    ce = e.use(k);
+    Ctx c = e.ctx(k);
+    const size_t n = (size_t)(e.cell_off[k + 1] - e.cell_off[k]);
+    if (ce == cudaSuccess) ce = cudaMemsetAsync(e.cmaster[k], 0, n * 4, c.stream);
+    if (ce == cudaSuccess) ce = cudaMemsetAsync(e.cgrad[k], 0, n * 4, c.stream);
+    if (ce == cudaSuccess && e.dt == GP_BF16) ce = cudaMemsetAsync(e.cwlp[k], 0, n * 2, c.stream);
+    if (ce == cudaSuccess && e.bwd[k].splitk_ws)                // split-K counters start at zero and reset themselves
+      ce = cudaMemsetAsync(e.bwd[k].splitk_ws, 0, e.splitk_ws_bytes, c.stream);
+    if (ce == cudaSuccess && k == K - 1) ce = cudaMemsetAsync(e.flag_dev_last, 0, 4, c.stream);
+    if (ce == cudaSuccess && k == 0) {
+      ce = cudaMemsetAsync(e.flag_dev, 0, 4, c.stream);
+      if (ce == cudaSuccess) ce = positional_table(c, e.pe, e.S, e.d);
+    }
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(c.stream);
+  }
+  if (e.multi_device) cudaSetDevice(dev_entry);
   if (ce != cudaSuccess) { gpipe_destroy(g); return cuda_fail(ce, "gpipe_create"); }
   *out = g;
   return GPIPE_OK;
@@ -239,7 +332,13 @@ static int create_impl(const gpipe_layer_spec *spec, int K, int M, int remat, in
 void gpipe_destroy(gpipe_t *g) {
   if (!g) return;
   Engine &e = g->e;
-  for (auto s : e.streams) cudaStreamSynchronize(s);
+  int dev_entry = 0;
+  cudaGetDevice(&dev_entry);
+  for (size_t k = 0; k < e.streams.size(); ++k) {
+    e.use((int)k);
+    cudaStreamSynchronize(e.streams[k]);
+  }
+  if (e.multi_device) cudaSetDevice(dev_entry);
   e.drop_graph();
   for (auto &v : e.ev_f) for (auto ev : v) if (ev) cudaEventDestroy(ev);
   for (auto &v : e.ev_b) for (auto ev : v) if (ev) cudaEventDestroy(ev);
@@ -255,12 +354,13 @@ void gpipe_destroy(gpipe_t *g) {
 int gpipe_init_params(gpipe_t *g, uint64_t seed, float std, int parity) {
   if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
   Engine &e = g->e;
-  Ctx c = e.ctx(0);
   for (size_t i = 0; i < e.tensors.size(); ++i) {
     const TensorInfo &t = e.tensors[i];
     int64_t n = ((t.rows * t.cols + 63) / 64) * 64;
-    float *m = e.master + t.off;
-    void *w = e.dt == GP_BF16 ? (void *)((char *)e.w_lp + t.off * 2) : nullptr;
+    float *m = e.P((int)i);
+    void *w = e.dt == GP_BF16 ? e.Wl((int)i) : nullptr;
+    API_CUDA(e.use(t.cell), "gpipe_init_params");
+    Ctx c = e.ctx(t.cell);
     bool gamma = !t.matrix && t.name.size() >= 2 && t.name.compare(t.name.size() - 2, 2, "_g") == 0;
     cudaError_t ce;
     if (t.matrix || parity) {
@@ -272,7 +372,11 @@ int gpipe_init_params(gpipe_t *g, uint64_t seed, float std, int parity) {
     if (ce != cudaSuccess) return cuda_fail(ce, "gpipe_init_params");
     // padding elements beyond rows*cols stay harmless: nothing reads them
   }
-  API_CUDA(cudaStreamSynchronize(c.stream), "gpipe_init_params");
+  for (int k = 0; k < e.K; ++k) {
+    API_CUDA(e.use(k), "gpipe_init_params");
+    API_CUDA(cudaStreamSynchronize(e.st(k)), "gpipe_init_params");
+  }
+  API_CUDA(e.use(0), "gpipe_init_params");
   return GPIPE_OK;
 }
 
@@ -292,33 +396,46 @@ int gpipe_step(gpipe_t *g, const int32_t *tokens, const int32_t *labels, float *
   for (int64_t i = 0; i < e.T_total; ++i)
     if (tokens[i] < 0 || tokens[i] >= e.V || labels[i] < 0 || labels[i] >= e.V)
       return fail(GPIPE_EINVAL, "token/label outside [0, V) at flat index " + std::to_string(i));
+  // tokens go where the embedding is (cell 0), labels where the loss is (cell K-1)
+  API_CUDA(e.use(0), "gpipe_step");
   API_CUDA(cudaMemcpyAsync(e.tok_dev, tokens, (size_t)e.T_total * 4, cudaMemcpyHostToDevice, e.streams[0]), "gpipe_step H2D");
-  API_CUDA(cudaMemcpyAsync(e.lab_dev, labels, (size_t)e.T_total * 4, cudaMemcpyHostToDevice, e.streams[0]), "gpipe_step H2D");
+  const int kl = e.multi() ? e.K - 1 : 0;
+  API_CUDA(e.use(kl), "gpipe_step");
+  API_CUDA(cudaMemcpyAsync(e.lab_dev, labels, (size_t)e.T_total * 4, cudaMemcpyHostToDevice, e.streams[kl]), "gpipe_step H2D");
+  API_CUDA(e.use(0), "gpipe_step");
   return step_common(e, loss_out);
 }
 
 int gpipe_step_device(gpipe_t *g, const int32_t *tokens_dev, const int32_t *labels_dev, float *loss_out) {
   if (!g || !tokens_dev || !labels_dev) return fail(GPIPE_EINVAL, "handle, tokens and labels are required");
   Engine &e = g->e;
-  Ctx c = e.ctx(0);
-  API_CUDA(cudaMemsetAsync(e.flag_dev, 0, 4, c.stream), "gpipe_step_device");
-  API_CUDA(check_ids(c, tokens_dev, e.T_total, e.V, e.flag_dev), "gpipe_step_device");
-  API_CUDA(check_ids(c, labels_dev, e.T_total, e.V, e.flag_dev), "gpipe_step_device");
-  API_CUDA(cudaMemcpyAsync(e.host_flag, e.flag_dev, 4, cudaMemcpyDeviceToHost, c.stream), "gpipe_step_device");
-  API_CUDA(cudaMemcpyAsync(e.tok_dev, tokens_dev, (size_t)e.T_total * 4, cudaMemcpyDeviceToDevice, c.stream), "gpipe_step_device");
-  API_CUDA(cudaMemcpyAsync(e.lab_dev, labels_dev, (size_t)e.T_total * 4, cudaMemcpyDeviceToDevice, c.stream), "gpipe_step_device");
-  API_CUDA(cudaStreamSynchronize(c.stream), "gpipe_step_device");
-  if (*e.host_flag) return fail(GPIPE_EINVAL, "token/label outside [0, V)");
+  const int kl = e.multi() ? e.K - 1 : 0;
+  // ids move to the cells that use them (cell 0: embedding, cell K-1: loss), are range-checked there, then the step runs
+  API_CUDA(e.use(0), "gpipe_step_device");
+  Ctx c0 = e.ctx(0);
+  API_CUDA(cudaMemsetAsync(e.flag_dev, 0, 4, c0.stream), "gpipe_step_device");
+  API_CUDA(cudaMemcpyAsync(e.tok_dev, tokens_dev, (size_t)e.T_total * 4, cudaMemcpyDefault, c0.stream), "gpipe_step_device");
+  API_CUDA(check_ids(c0, e.tok_dev, e.T_total, e.V, e.flag_dev), "gpipe_step_device");
+  API_CUDA(cudaMemcpyAsync(e.host_flag, e.flag_dev, 4, cudaMemcpyDeviceToHost, c0.stream), "gpipe_step_device");
+  API_CUDA(e.use(kl), "gpipe_step_device");
+  Ctx cl = e.ctx(kl);
+  if (e.multi()) API_CUDA(cudaMemsetAsync(e.flag_dev_last, 0, 4, cl.stream), "gpipe_step_device");
+  API_CUDA(cudaMemcpyAsync(e.lab_dev, labels_dev, (size_t)e.T_total * 4, cudaMemcpyDefault, cl.stream), "gpipe_step_device");
+  API_CUDA(check_ids(cl, e.lab_dev, e.T_total, e.V, e.flag_dev_last), "gpipe_step_device");
+  API_CUDA(cudaMemcpyAsync(e.host_flag + 1, e.flag_dev_last, 4, cudaMemcpyDeviceToHost, cl.stream), "gpipe_step_device");
+  API_CUDA(cudaStreamSynchronize(cl.stream), "gpipe_step_device");
+  API_CUDA(e.use(0), "gpipe_step_device");
+  API_CUDA(cudaStreamSynchronize(c0.stream), "gpipe_step_device");
+  if (e.host_flag[0] || e.host_flag[1]) return fail(GPIPE_EINVAL, "token/label outside [0, V)");
   return step_common(e, loss_out);
 }
 
 int gpipe_apply_sgd(gpipe_t *g, float lr) {
   if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
   Engine &e = g->e;
-  Ctx c = e.ctx(0);
-  API_CUDA(sgd_apply(c, e.dt, e.master, e.grad, e.dt == GP_BF16 ? e.w_lp : nullptr, e.n_flat, lr), "gpipe_apply_sgd");
-  API_CUDA(cudaStreamSynchronize(c.stream), "gpipe_apply_sgd");
-  return GPIPE_OK;
+  return for_each_home(e, "gpipe_apply_sgd", [&](const Ctx &c, float *m, float *gr, void *w, float *, int64_t n) {
+    return sgd_apply(c, e.dt, m, gr, w, n, lr);
+  });
 }
 
 int gpipe_optimizer_slot_bytes(const gpipe_t *g, size_t *bytes_out) {
@@ -330,11 +447,39 @@ int gpipe_optimizer_slot_bytes(const gpipe_t *g, size_t *bytes_out) {
 int gpipe_attach_optimizer_slots(gpipe_t *g, void *slots_dev, size_t bytes) {
   if (!g || !slots_dev) return fail(GPIPE_EINVAL, "handle and slots_dev are required");
   Engine &e = g->e;
+  if (e.multi()) return fail(GPIPE_ENOTIMPL, "pipeline handles take one slot buffer per cell: gpipe_attach_optimizer_slots_cell");
   if (bytes < (size_t)e.n_flat * sizeof(float)) return fail(GPIPE_ENOMEM, "optimizer slots too small: need " + std::to_string((size_t)e.n_flat * 4) + " bytes");
   if ((uintptr_t)slots_dev % 16) return fail(GPIPE_EINVAL, "optimizer slots must be 16-byte aligned");
   API_CUDA(cudaMemsetAsync(slots_dev, 0, (size_t)e.n_flat * sizeof(float), e.streams[0]), "gpipe_attach_optimizer_slots");
   API_CUDA(cudaStreamSynchronize(e.streams[0]), "gpipe_attach_optimizer_slots");
   e.opt_ms = (float *)slots_dev;
+  e.copt.assign(e.K, nullptr);
+  for (int k = 0; k < e.K; ++k) e.copt[k] = e.opt_ms + e.cell_off[k];
+  return GPIPE_OK;
+}
+
+int gpipe_attach_optimizer_slots_cell(gpipe_t *g, int k, void *slots_dev, size_t bytes) {
+  if (!g || !slots_dev) return fail(GPIPE_EINVAL, "handle and slots_dev are required");
+  Engine &e = g->e;
+  if (k < 0 || k >= e.K) return fail(GPIPE_EINVAL, "cell index out of range");
+  const size_t need = (size_t)(e.cell_off[k + 1] - e.cell_off[k]) * sizeof(float);
+  if (bytes < need) return fail(GPIPE_ENOMEM, "optimizer slots too small: need " + std::to_string(need) + " bytes");
+  if ((uintptr_t)slots_dev % 16) return fail(GPIPE_EINVAL, "optimizer slots must be 16-byte aligned");
+  API_CUDA(e.use(k), "gpipe_attach_optimizer_slots_cell");
+  API_CUDA(cudaMemsetAsync(slots_dev, 0, need, e.st(k)), "gpipe_attach_optimizer_slots_cell");
+  API_CUDA(cudaStreamSynchronize(e.st(k)), "gpipe_attach_optimizer_slots_cell");
+  API_CUDA(e.use(0), "gpipe_attach_optimizer_slots_cell");
+  if (e.copt.empty()) e.copt.assign(e.K, nullptr);
+  e.copt[k] = (float *)slots_dev;
+  bool all = true;
+  for (float *p : e.copt) all = all && p != nullptr;
+  if (all && e.multi()) e.opt_ms = e.copt[0];             // "slots attached" marker
+  return GPIPE_OK;
+}
+
+int gpipe_cell_param_count(const gpipe_t *g, int k, int64_t *n_out) {
+  if (!g || !n_out || k < 0 || k >= g->e.K) return fail(GPIPE_EINVAL, "handle, n_out and a valid cell index are required");
+  *n_out = g->e.cell_off[k + 1] - g->e.cell_off[k];
   return GPIPE_OK;
 }
 
@@ -343,11 +488,9 @@ int gpipe_apply_rmsprop(gpipe_t *g, float lr, float rho, float eps) {
   Engine &e = g->e;
   if (!e.opt_ms) return fail(GPIPE_EINVAL, "call gpipe_attach_optimizer_slots first");
   if (!(rho >= 0.f && rho < 1.f) || !(eps > 0.f)) return fail(GPIPE_EINVAL, "need 0 <= rho < 1 and eps > 0");
-  Ctx c = e.ctx(0);
-  API_CUDA(rmsprop_apply(c, e.dt, e.master, e.grad, e.opt_ms, e.dt == GP_BF16 ? e.w_lp : nullptr, e.n_flat, lr, rho, eps),
-           "gpipe_apply_rmsprop");
-  API_CUDA(cudaStreamSynchronize(c.stream), "gpipe_apply_rmsprop");
-  return GPIPE_OK;
+  return for_each_home(e, "gpipe_apply_rmsprop", [&](const Ctx &c, float *m, float *gr, void *w, float *ms, int64_t n) {
+    return rmsprop_apply(c, e.dt, m, gr, ms, w, n, lr, rho, eps);
+  });
 }
 
 // ---- data-parallel replicas -------------------------------------------------------------------
@@ -360,6 +503,7 @@ int gpipe_dp_shard(int64_t n_flat, int rank, int world, int64_t *lo, int64_t *hi
 int gpipe_dp_layout(const gpipe_t *g, int64_t *n_flat, size_t *master_off, size_t *grad_off, size_t *wlp_off) {
   if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
   const Engine &e = g->e;
+  if (e.multi()) return fail(GPIPE_ENOTIMPL, "data-parallel replicas of a pipeline handle are not built");
   if (n_flat) *n_flat = e.n_flat;
   if (master_off) *master_off = (size_t)((const char *)e.master - e.arena.base);
   if (grad_off) *grad_off = (size_t)((const char *)e.grad - e.arena.base);
@@ -371,6 +515,7 @@ static int dp_apply_impl(gpipe_t *g, int rank, int world, void *const *peer_aren
                          float rho, float eps, const char *where) {
   if (!g || !peer_arenas) return fail(GPIPE_EINVAL, "handle and peer_arenas are required");
   Engine &e = g->e;
+  if (e.multi()) return fail(GPIPE_ENOTIMPL, "data-parallel replicas of a pipeline handle are not built");
   if (world < 1 || world > DpPeers::kMax || rank < 0 || rank >= world)
     return fail(GPIPE_EINVAL, "need 1 <= world <= " + std::to_string(DpPeers::kMax) + " and 0 <= rank < world");
   if (peer_arenas[rank] != (void *)e.arena.base) return fail(GPIPE_EINVAL, "peer_arenas[rank] must be this handle's own arena");
@@ -440,9 +585,9 @@ int gpipe_ipc_close(void *base) {
 int gpipe_zero_grads(gpipe_t *g) {
   if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
   Engine &e = g->e;
-  API_CUDA(cudaMemsetAsync(e.grad, 0, (size_t)e.n_flat * 4, e.streams[0]), "gpipe_zero_grads");
-  API_CUDA(cudaStreamSynchronize(e.streams[0]), "gpipe_zero_grads");
-  return GPIPE_OK;
+  return for_each_home(e, "gpipe_zero_grads", [&](const Ctx &c, float *, float *gr, void *, float *, int64_t n) {
+    return cudaMemsetAsync(gr, 0, (size_t)n * 4, c.stream);
+  });
 }
 
 int gpipe_num_tensors(const gpipe_t *g) { return g ? (int)g->e.tensors.size() : fail(GPIPE_EINVAL, "handle is NULL"); }
@@ -469,13 +614,14 @@ int gpipe_get_param(gpipe_t *g, int i, float *host_out) {
   Engine &e = g->e;
   const TensorInfo &t = e.tensors[i];
   int64_t n = t.rows * t.cols;
-  Ctx c = e.ctx(0);
+  API_CUDA(e.use(t.cell), "gpipe_get_param");
+  Ctx c = e.ctx(t.cell);
   if (e.dt == GP_BF16 && t.matrix) {
-    // widen the bf16 working copy through the gradient-free scratch of cell 0 (dh is the largest)
-    // -> simpler and always big enough: convert in chunks through ln_partials? use a temp on host:
+    // widen the bf16 working copy on the host
     std::string tmp((size_t)n * 2, '\0');
-    API_CUDA(cudaMemcpyAsync(&tmp[0], (const char *)e.w_lp + t.off * 2, (size_t)n * 2, cudaMemcpyDeviceToHost, c.stream), "gpipe_get_param");
+    API_CUDA(cudaMemcpyAsync(&tmp[0], e.Wl(i), (size_t)n * 2, cudaMemcpyDeviceToHost, c.stream), "gpipe_get_param");
     API_CUDA(cudaStreamSynchronize(c.stream), "gpipe_get_param");
+    API_CUDA(e.use(0), "gpipe_get_param");
     const uint16_t *u = (const uint16_t *)tmp.data();
     for (int64_t j = 0; j < n; ++j) {
       uint32_t w = (uint32_t)u[j] << 16;
@@ -483,8 +629,9 @@ int gpipe_get_param(gpipe_t *g, int i, float *host_out) {
     }
     return GPIPE_OK;
   }
-  API_CUDA(cudaMemcpyAsync(host_out, e.master + t.off, (size_t)n * 4, cudaMemcpyDeviceToHost, c.stream), "gpipe_get_param");
+  API_CUDA(cudaMemcpyAsync(host_out, e.P(i), (size_t)n * 4, cudaMemcpyDeviceToHost, c.stream), "gpipe_get_param");
   API_CUDA(cudaStreamSynchronize(c.stream), "gpipe_get_param");
+  API_CUDA(e.use(0), "gpipe_get_param");
   return GPIPE_OK;
 }
 
@@ -494,11 +641,13 @@ int gpipe_set_param(gpipe_t *g, int i, const float *host_in) {
   Engine &e = g->e;
   const TensorInfo &t = e.tensors[i];
   int64_t n = t.rows * t.cols;
-  Ctx c = e.ctx(0);
-  API_CUDA(cudaMemcpyAsync(e.master + t.off, host_in, (size_t)n * 4, cudaMemcpyHostToDevice, c.stream), "gpipe_set_param");
+  API_CUDA(e.use(t.cell), "gpipe_set_param");
+  Ctx c = e.ctx(t.cell);
+  API_CUDA(cudaMemcpyAsync(e.P(i), host_in, (size_t)n * 4, cudaMemcpyHostToDevice, c.stream), "gpipe_set_param");
   if (e.dt == GP_BF16)   // RNE-round into the working copy; matrices also round the master (A12)
-    API_CUDA(master_to_lp(c, e.dt, e.master + t.off, (char *)e.w_lp + t.off * 2, n, t.matrix ? 1 : 0), "gpipe_set_param");
+    API_CUDA(master_to_lp(c, e.dt, e.P(i), e.Wl(i), n, t.matrix ? 1 : 0), "gpipe_set_param");
   API_CUDA(cudaStreamSynchronize(c.stream), "gpipe_set_param");
+  API_CUDA(e.use(0), "gpipe_set_param");
   return GPIPE_OK;
 }
 
@@ -508,8 +657,10 @@ int gpipe_get_master(gpipe_t *g, int i, float *host_out) {
   if (rc) return rc;
   Engine &e = g->e;
   const TensorInfo &t = e.tensors[i];
-  API_CUDA(cudaMemcpyAsync(host_out, e.master + t.off, (size_t)(t.rows * t.cols) * 4, cudaMemcpyDeviceToHost, e.streams[0]), "gpipe_get_master");
-  API_CUDA(cudaStreamSynchronize(e.streams[0]), "gpipe_get_master");
+  API_CUDA(e.use(t.cell), "gpipe_get_master");
+  API_CUDA(cudaMemcpyAsync(host_out, e.P(i), (size_t)(t.rows * t.cols) * 4, cudaMemcpyDeviceToHost, e.st(t.cell)), "gpipe_get_master");
+  API_CUDA(cudaStreamSynchronize(e.st(t.cell)), "gpipe_get_master");
+  API_CUDA(e.use(0), "gpipe_get_master");
   return GPIPE_OK;
 }
 
@@ -519,11 +670,13 @@ int gpipe_set_master(gpipe_t *g, int i, const float *host_in) {
   Engine &e = g->e;
   const TensorInfo &t = e.tensors[i];
   int64_t n = t.rows * t.cols;
-  Ctx c = e.ctx(0);
-  API_CUDA(cudaMemcpyAsync(e.master + t.off, host_in, (size_t)n * 4, cudaMemcpyHostToDevice, c.stream), "gpipe_set_master");
+  API_CUDA(e.use(t.cell), "gpipe_set_master");
+  Ctx c = e.ctx(t.cell);
+  API_CUDA(cudaMemcpyAsync(e.P(i), host_in, (size_t)n * 4, cudaMemcpyHostToDevice, c.stream), "gpipe_set_master");
   if (e.dt == GP_BF16)   // working copy = RNE(master); the master keeps every bit
-    API_CUDA(master_to_lp(c, e.dt, e.master + t.off, (char *)e.w_lp + t.off * 2, n, 0), "gpipe_set_master");
+    API_CUDA(master_to_lp(c, e.dt, e.P(i), e.Wl(i), n, 0), "gpipe_set_master");
   API_CUDA(cudaStreamSynchronize(c.stream), "gpipe_set_master");
+  API_CUDA(e.use(0), "gpipe_set_master");
   return GPIPE_OK;
 }
 
@@ -533,8 +686,10 @@ int gpipe_get_optimizer_slot(gpipe_t *g, int i, float *host_out) {
   Engine &e = g->e;
   if (!e.opt_ms) return fail(GPIPE_EINVAL, "no optimizer slots attached");
   const TensorInfo &t = e.tensors[i];
-  API_CUDA(cudaMemcpyAsync(host_out, e.opt_ms + t.off, (size_t)(t.rows * t.cols) * 4, cudaMemcpyDeviceToHost, e.streams[0]), "gpipe_get_optimizer_slot");
-  API_CUDA(cudaStreamSynchronize(e.streams[0]), "gpipe_get_optimizer_slot");
+  API_CUDA(e.use(t.cell), "gpipe_get_optimizer_slot");
+  API_CUDA(cudaMemcpyAsync(host_out, e.Opt(i), (size_t)(t.rows * t.cols) * 4, cudaMemcpyDeviceToHost, e.st(t.cell)), "gpipe_get_optimizer_slot");
+  API_CUDA(cudaStreamSynchronize(e.st(t.cell)), "gpipe_get_optimizer_slot");
+  API_CUDA(e.use(0), "gpipe_get_optimizer_slot");
   return GPIPE_OK;
 }
 
@@ -544,8 +699,10 @@ int gpipe_set_optimizer_slot(gpipe_t *g, int i, const float *host_in) {
   Engine &e = g->e;
   if (!e.opt_ms) return fail(GPIPE_EINVAL, "no optimizer slots attached");
   const TensorInfo &t = e.tensors[i];
-  API_CUDA(cudaMemcpyAsync(e.opt_ms + t.off, host_in, (size_t)(t.rows * t.cols) * 4, cudaMemcpyHostToDevice, e.streams[0]), "gpipe_set_optimizer_slot");
-  API_CUDA(cudaStreamSynchronize(e.streams[0]), "gpipe_set_optimizer_slot");
+  API_CUDA(e.use(t.cell), "gpipe_set_optimizer_slot");
+  API_CUDA(cudaMemcpyAsync(e.Opt(i), host_in, (size_t)(t.rows * t.cols) * 4, cudaMemcpyHostToDevice, e.st(t.cell)), "gpipe_set_optimizer_slot");
+  API_CUDA(cudaStreamSynchronize(e.st(t.cell)), "gpipe_set_optimizer_slot");
+  API_CUDA(e.use(0), "gpipe_set_optimizer_slot");
   return GPIPE_OK;
 }
 
@@ -554,17 +711,26 @@ int gpipe_get_grad(gpipe_t *g, int i, float *host_out) {
   if (rc) return rc;
   Engine &e = g->e;
   const TensorInfo &t = e.tensors[i];
-  API_CUDA(cudaMemcpyAsync(host_out, e.grad + t.off, (size_t)(t.rows * t.cols) * 4, cudaMemcpyDeviceToHost, e.streams[0]), "gpipe_get_grad");
-  API_CUDA(cudaStreamSynchronize(e.streams[0]), "gpipe_get_grad");
+  API_CUDA(e.use(t.cell), "gpipe_get_grad");
+  API_CUDA(cudaMemcpyAsync(host_out, e.G(i), (size_t)(t.rows * t.cols) * 4, cudaMemcpyDeviceToHost, e.st(t.cell)), "gpipe_get_grad");
+  API_CUDA(cudaStreamSynchronize(e.st(t.cell)), "gpipe_get_grad");
+  API_CUDA(e.use(0), "gpipe_get_grad");
   return GPIPE_OK;
 }
 
 int gpipe_peak_bytes(const gpipe_t *g, size_t *total, size_t *by_category, size_t *by_cell) {
   if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
   const Engine &e = g->e;
-  if (total) *total = e.arena.used;
-  if (by_category) for (int i = 0; i < GPIPE_NUM_CATS; ++i) by_category[i] = e.arena.by_cat[i];
-  if (by_cell) for (int k = 0; k < e.K; ++k) by_cell[k] = e.arena.by_cell[k];
+  // pipeline handle: totals over the K arenas; by_cell[k] is then everything cell k's device holds (PAPER.md:87 is
+  // stated per accelerator)
+  size_t tot = 0, cat[GPIPE_NUM_CATS] = {0};
+  for (int k = 0; k < (e.multi() ? e.K : 1); ++k) {
+    tot += e.ar(k).used;
+    for (int i = 0; i < GPIPE_NUM_CATS; ++i) cat[i] += e.ar(k).by_cat[i];
+  }
+  if (total) *total = tot;
+  if (by_category) for (int i = 0; i < GPIPE_NUM_CATS; ++i) by_category[i] = cat[i];
+  if (by_cell) for (int k = 0; k < e.K; ++k) by_cell[k] = e.multi() ? e.ar(k).used : e.arena.by_cell[k];
   return GPIPE_OK;
 }
 

@@ -60,6 +60,19 @@ int Engine::build_inventory(std::string &err) {
   i_lnf_b = add("lnf_b", 1, d, false);
   i_w_out = add("w_out", d, V, true);
   n_flat = off;
+  // owners: the canonical order is emb | layers in order | final LN, w_out and cells are consecutive layer ranges,
+  // so every cell owns one contiguous range of the flat order
+  tensors[i_emb].cell = 0;
+  for (int k = 0; k < K; ++k)
+    for (int l = cell_lo[k]; l < cell_hi[k]; ++l) {
+      const LayerParams &q = lp[l];
+      for (int i : {q.ln1_g, q.ln1_b, q.w_qkv, q.b_qkv, q.w_o, q.b_o, q.ln2_g, q.ln2_b, q.w_1, q.b_1, q.w_2, q.b_2})
+        tensors[i].cell = k;
+    }
+  tensors[i_lnf_g].cell = tensors[i_lnf_b].cell = tensors[i_w_out].cell = K - 1;
+  cell_off.assign(K + 1, n_flat);
+  cell_off[0] = 0;
+  for (int k = 1; k < K; ++k) cell_off[k] = cell_lo[k] < spec.n_layers ? tensors[lp[cell_lo[k]].ln1_g].off : tensors[i_lnf_g].off;
   return GPIPE_OK;
 }
 
@@ -67,25 +80,50 @@ int Engine::build_inventory(std::string &err) {
 // mark IS the peak (with remat, K*M boundary activations ~ N plus one cell interior
 // ~ (L/K)(N/M) per cell; without remat M interiors per cell ~ N*L).
 int Engine::build_plan(bool dry, std::string &err) {
-  arena.dry = dry;
-  arena.used = 0;
-  memset(arena.by_cat, 0, sizeof(arena.by_cat));
-  arena.by_cell.assign(K, 0);
+  auto reset = [&](Arena &a) {
+    a.dry = dry;
+    a.used = 0;
+    memset(a.by_cat, 0, sizeof(a.by_cat));
+    a.by_cell.assign(K, 0);
+  };
+  reset(arena);
+  for (auto &a : parena) reset(a);
   size_t lpb = lp_size(dt);
   size_t Tm = (size_t)T_mb;
-  auto F32 = [&](size_t n, int cat, int cell) { return (float *)arena.alloc(n * 4, cat, cell); };
-  auto LP = [&](size_t n, int cat, int cell) { return arena.alloc(n * lpb, cat, cell); };
+  // home(k): the arena of cell k; data that belongs to no cell goes to the cell that uses it
+  auto RAW = [&](size_t bytes, int cat, int cell, int home) { return ar(home).alloc(bytes, cat, cell); };
+  auto F32 = [&](size_t n, int cat, int cell) { return (float *)RAW(n * 4, cat, cell, cell < 0 ? 0 : cell); };
+  auto LP = [&](size_t n, int cat, int cell) { return RAW(n * lpb, cat, cell, cell < 0 ? 0 : cell); };
 
-  master = F32((size_t)n_flat, dt == GP_BF16 ? GPIPE_CAT_MASTERS : GPIPE_CAT_WEIGHTS, -1);
-  grad = F32((size_t)n_flat, GPIPE_CAT_GRADS, -1);
-  w_lp = dt == GP_BF16 ? arena.alloc((size_t)n_flat * 2, GPIPE_CAT_WEIGHTS, -1) : (void *)master;
+  cmaster.assign(K, nullptr); cgrad.assign(K, nullptr); cwlp.assign(K, nullptr);
+  const int cat_m = dt == GP_BF16 ? GPIPE_CAT_MASTERS : GPIPE_CAT_WEIGHTS;
+  if (!multi()) {
+    master = F32((size_t)n_flat, cat_m, -1);
+    grad = F32((size_t)n_flat, GPIPE_CAT_GRADS, -1);
+    w_lp = dt == GP_BF16 ? RAW((size_t)n_flat * 2, GPIPE_CAT_WEIGHTS, -1, 0) : (void *)master;
+    for (int k = 0; k < K; ++k) {
+      cmaster[k] = master ? master + cell_off[k] : nullptr;
+      cgrad[k] = grad ? grad + cell_off[k] : nullptr;
+      cwlp[k] = w_lp ? (void *)((char *)w_lp + cell_off[k] * (dt == GP_BF16 ? 2 : 4)) : nullptr;
+    }
+  } else {
+    master = grad = nullptr;
+    w_lp = nullptr;
+    for (int k = 0; k < K; ++k) {                        // cell k's parameters live on cell k's device
+      const size_t n = (size_t)(cell_off[k + 1] - cell_off[k]);
+      cmaster[k] = (float *)RAW(n * 4, cat_m, -1, k);
+      cgrad[k] = (float *)RAW(n * 4, GPIPE_CAT_GRADS, -1, k);
+      cwlp[k] = dt == GP_BF16 ? RAW(n * 2, GPIPE_CAT_WEIGHTS, -1, k) : (void *)cmaster[k];
+    }
+  }
 
-  tok_dev = (int32_t *)arena.alloc((size_t)T_total * 4, GPIPE_CAT_MISC, -1);
-  lab_dev = (int32_t *)arena.alloc((size_t)T_total * 4, GPIPE_CAT_MISC, -1);
-  pe = F32((size_t)S * d, GPIPE_CAT_MISC, -1);
-  loss_parts = F32((size_t)M + 1, GPIPE_CAT_HEAD, -1);
+  tok_dev = (int32_t *)RAW((size_t)T_total * 4, GPIPE_CAT_MISC, -1, 0);            // the embedding is in cell 0
+  lab_dev = (int32_t *)RAW((size_t)T_total * 4, GPIPE_CAT_MISC, -1, K - 1);        // the loss in cell K-1
+  pe = (float *)RAW((size_t)S * d * 4, GPIPE_CAT_MISC, -1, 0);
+  loss_parts = (float *)RAW((size_t)(M + 1) * 4, GPIPE_CAT_HEAD, -1, K - 1);
   loss_dummy = loss_parts ? loss_parts + M : nullptr;
-  flag_dev = (int *)arena.alloc(4, GPIPE_CAT_MISC, -1);
+  flag_dev = (int *)RAW(4, GPIPE_CAT_MISC, -1, 0);
+  flag_dev_last = multi() ? (int *)RAW(4, GPIPE_CAT_MISC, -1, K - 1) : flag_dev;
 
   slot.assign(K, std::vector<float *>(M, nullptr));
   for (int k = 1; k < K; ++k)
@@ -93,9 +131,22 @@ int Engine::build_plan(bool dry, std::string &err) {
   for (int i = 0; i < 2; ++i) {
     dbound[i].assign(K, nullptr);
     dbound_lp[i].assign(K, nullptr);
+    dout[i].assign(K, nullptr);
+    dout_lp[i].assign(K, nullptr);
     for (int k = 1; k < K; ++k) {
       dbound[i][k] = F32(Tm * d, GPIPE_CAT_BOUNDARY, k);
       dbound_lp[i][k] = dt == GP_BF16 ? LP(Tm * d, GPIPE_CAT_BOUNDARY, k) : (void *)dbound[i][k];
+    }
+    // the gradient wrt cell k's output is produced by cell k+1: in a pipeline handle it is copied into cell k's own
+    // arena (the backward boundary transfer), otherwise cell k reads it where cell k+1 left it
+    for (int k = 0; k + 1 < K; ++k) {
+      if (multi()) {
+        dout[i][k] = F32(Tm * d, GPIPE_CAT_BOUNDARY, k);
+        dout_lp[i][k] = dt == GP_BF16 ? LP(Tm * d, GPIPE_CAT_BOUNDARY, k) : (void *)dout[i][k];
+      } else {
+        dout[i][k] = dbound[i][k + 1];
+        dout_lp[i][k] = dbound_lp[i][k + 1];
+      }
     }
   }
 
@@ -125,7 +176,7 @@ int Engine::build_plan(bool dry, std::string &err) {
       Workspace &W_ = ws[k][w];
       const int cat = GPIPE_CAT_INTERIOR;
       if (k == 0) W_.x_emb = F32(Tm * d, cat, k);
-      if (k == K - 1 || remat) W_.x_out = F32(Tm * d, cat, k);
+      if (k == K - 1 || remat || multi()) W_.x_out = F32(Tm * d, cat, k);   // pipeline: also the outgoing boundary staging
       int nl = cell_hi[k] - cell_lo[k];
       W_.layers.resize(nl);
       for (int i = 0; i < nl; ++i) {
@@ -135,7 +186,7 @@ int Engine::build_plan(bool dry, std::string &err) {
         b.o = LP(Tm * da, cat, k);
         b.c = LP(Tm * d, cat, k);
         b.h = LP(Tm * H, cat, k);
-        b.hbits = (uint32_t *)arena.alloc(Tm * (size_t)((H + 31) / 32) * 4, cat, k);
+        b.hbits = (uint32_t *)RAW(Tm * (size_t)((H + 31) / 32) * 4, cat, k, k);
         b.x1 = F32(Tm * d, cat, k);
         b.x2 = i + 1 < nl ? F32(Tm * d, cat, k) : nullptr;
         b.lse = F32(Tm * A, cat, k);
@@ -171,13 +222,14 @@ int Engine::build_plan(bool dry, std::string &err) {
       if (cols < (size_t)d) cols = d;
       s.colsum_scratch = F32(rows * cols, cat, k);
     }
-    s.splitk_ws = splitk_ws_bytes ? arena.alloc(splitk_ws_bytes, cat, k) : nullptr;
+    s.splitk_ws = splitk_ws_bytes ? RAW(splitk_ws_bytes, cat, k, k) : nullptr;
   }
-  if (!dry && arena.used > arena.cap) {
-    err = "arena too small: need " + std::to_string(arena.used) + " bytes, have " +
-          std::to_string(arena.cap);
-    return GPIPE_ENOMEM;
-  }
+  for (int k = 0; k < (multi() ? K : 1); ++k)
+    if (!dry && ar(k).used > ar(k).cap) {
+      err = "arena " + std::to_string(k) + " too small: need " + std::to_string(ar(k).used) + " bytes, have " +
+            std::to_string(ar(k).cap);
+      return GPIPE_ENOMEM;
+    }
   return GPIPE_OK;
 }
 
@@ -256,7 +308,7 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
     float *x2;
     if (!last) x2 = b.x2;
     else if (k == K - 1) x2 = w.x_out;
-    else if (!replay) x2 = slot[k + 1][m];            // boundary stash (a12)
+    else if (!replay) x2 = boundary_staged ? w.x_out : slot[k + 1][m];   // boundary stash (a12)
     else if (replay_full) x2 = w.x_out;               // replay output nobody reads
     else x2 = nullptr;                                // skipped: B_k does not need F_k's output
     // c = LN2(x1); x2 <- x1 + b_2                                            (a9)
@@ -278,6 +330,10 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
     }
     x = x2;
   }
+  // pipeline handle: the boundary activation is the one tensor that leaves the device - one copy of
+  // [T_mb, d] fp32 into the next cell's slot, on this cell's stream, ahead of the event F(k+1,m) waits for
+  if (boundary_staged && k + 1 < K && !replay && nl > 0)
+    GP_TRY(peer_copy(k + 1, slot[k + 1][m], k, w.x_out, (size_t)T_mb * d * sizeof(float), c.stream));
   if (k == K - 1) {
     if (nl == 0 && K == 1) x = w.x_emb;
     // y = LN_f(x_L); logits = y W_out; fused softmax-CE -> loss partial, dlogits   (a13, a14)
@@ -352,8 +408,12 @@ cudaError_t Engine::backward_cell(int k, int m) {
     dxo = s.dx_lp[cur];
     cur ^= 1;
   } else {
-    dx = dbound[m & 1][k + 1];
-    dxo = dbound_lp[m & 1][k + 1];
+    dx = dout[m & 1][k];
+    dxo = dout_lp[m & 1][k];
+    // pipeline handle: the FFN2 bias gradient of this cell's last layer is the column sum of the incoming boundary
+    // gradient; with all cells in one arena the next cell's LayerNorm backward adds it (fused), across devices
+    // this cell does it itself
+    if (multi() && nl > 0) GP_TRY(tcol(dxo, d, G(lp[cell_hi[k] - 1].b_2), d));
   }
   for (int i = nl - 1; i >= 0; --i) {
     int l = cell_lo[k] + i;
@@ -393,14 +453,26 @@ cudaError_t Engine::backward_cell(int k, int m) {
     // its output is the FFN2 output gradient of the layer below (possibly in the previous cell):
     // db_2(l-1) += sum_t dx
     GP_TRY(tlnb(s.dc, x_in, b.mean1, b.rstd1, P(q.ln1_g), dx, out, dt == GP_BF16 ? out_lp : nullptr,
-                G(q.ln1_g), G(q.ln1_b), l > 0 ? G(lp[l - 1].b_2) : nullptr));
+                G(q.ln1_g), G(q.ln1_b), l > 0 && !(multi() && i == 0) ? G(lp[l - 1].b_2) : nullptr));
     dx = out;
     dxo = out_lp;
     cur ^= 1;
   }
   if (k == 0)                                                          // dE[tok] += dx0
     GP_TRY(timed(k, KC_EMBED, 0, Td * d * 12.0, [&] { return embed_bwd(c, tok, dx, G(i_emb), T_mb, d); }));
+  if (multi() && k > 0) {
+    // backward boundary transfer: the gradient wrt this cell's input becomes the previous cell's output gradient
+    GP_TRY(peer_copy(k - 1, dout[m & 1][k - 1], k, dbound[m & 1][k], (size_t)T_mb * d * sizeof(float), c.stream));
+    if (dt == GP_BF16)
+      GP_TRY(peer_copy(k - 1, dout_lp[m & 1][k - 1], k, dbound_lp[m & 1][k], (size_t)T_mb * d * 2, c.stream));
+  }
   return cudaSuccess;
+}
+
+cudaError_t Engine::peer_copy(int k_dst, void *dst, int k_src, const void *src, size_t bytes, cudaStream_t s) {
+  if (multi_device && cell_device[k_dst] != cell_device[k_src])
+    return cudaMemcpyPeerAsync(dst, cell_device[k_dst], src, cell_device[k_src], bytes, s);
+  return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, s);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -430,6 +502,7 @@ cudaError_t Engine::enqueue_step() {
       if (!r.e0 || !r.e1) return pool_err;
       GP_TRY(cudaEventRecord(r.e0, st(k)));
     }
+    GP_TRY(use(k));
     cudaError_t e = kind == 'B' ? backward_cell(k, m) : forward_cell(k, m, kind == 'R');
     if (e != cudaSuccess) return e;
     if (trace_on) {
@@ -462,12 +535,14 @@ cudaError_t Engine::enqueue_step() {
       GP_TRY(task('B', k, m));
       GP_TRY(cudaEventRecord(ev_b[k][m], st(k)));
     }
-  // join: stream 0 waits for every cell, then the loss partials come back
+  // join: the loss partials come back on the last cell's stream, and stream 0 waits for every cell
+  GP_TRY(use(K - 1));
+  GP_TRY(cudaMemcpyAsync(host_loss, loss_parts, sizeof(float) * M, cudaMemcpyDeviceToHost, st(K - 1)));
   for (int k = 1; k < K; ++k) {
     GP_TRY(cudaEventRecord(ev_done[k], st(k)));
     GP_TRY(cudaStreamWaitEvent(streams[0], ev_done[k], 0));
   }
-  GP_TRY(cudaMemcpyAsync(host_loss, loss_parts, sizeof(float) * M, cudaMemcpyDeviceToHost, streams[0]));
+  GP_TRY(use(0));
   return cudaSuccess;
 }
 
@@ -482,7 +557,7 @@ cudaError_t Engine::run_step(float *loss_out) {
   ev_pool_used = 0;
   trace.clear();
   krecs.clear();
-  const bool eager = !use_graph || trace_on || ktiming_on || serial || graph_state < 0;
+  const bool eager = !use_graph || trace_on || ktiming_on || serial || graph_state < 0 || multi_device;
   if (eager || graph_state == 0) {
     GP_TRY(enqueue_step());
     if (!eager) graph_state = 1;

@@ -14,8 +14,9 @@ namespace gp {
 struct TensorInfo {
   std::string name;
   int64_t rows, cols;
-  int64_t off;        // element offset into the flat master / grad / lp arrays
+  int64_t off;        // element offset into the flat master / grad / lp arrays (canonical order)
   bool matrix;        // matrices are tensor-core operands (lp working copy); vectors stay fp32
+  int cell = 0;       // the cell that owns the tensor (emb: 0, final LN / w_out: K-1, layer l: its cell)
 };
 
 struct LayerParams {  // indices into Engine::tensors
@@ -88,11 +89,28 @@ struct Engine {
   std::vector<LayerParams> lp;
   int i_emb = 0, i_lnf_g = 0, i_lnf_b = 0, i_w_out = 0;
   int64_t n_flat = 0;
-  float *master = nullptr, *grad = nullptr;
+  float *master = nullptr, *grad = nullptr;            // single-arena mode: the whole flat range
   void *w_lp = nullptr;                                // bf16 working copy (bf16 mode), else = master
 
   std::vector<int> cell_lo, cell_hi;                   // layers [lo, hi) of cell k
-  Arena arena;
+  // Memory homes.  n_arenas == 1: one arena, one device (K streams share it).  n_arenas == K ("pipeline" handle,
+  // SURVEY 8(f) f1 / PAPER.md:65 "places the k-th cell on the k-th accelerator"): cell k's parameters, gradients,
+  // activations and scratch live in arena k on device cell_device[k] and run on stream k of that device; the
+  // boundary activation and its gradient are the only data that cross.
+  int n_arenas = 1;
+  Arena arena;                                         // single-arena mode
+  std::vector<Arena> parena;                           // pipeline mode: [K]
+  std::vector<int> cell_device;                        // [K]
+  bool multi() const { return n_arenas > 1; }
+  bool multi_device = false;                           // cells on different devices (peer copies, no CUDA graph)
+  int boundary_staged = 0;                             // pipeline: F_k writes its output locally, then a peer copy moves it
+  Arena &ar(int k) { return multi() ? parena[k] : arena; }
+  const Arena &ar(int k) const { return multi() ? parena[k] : arena; }
+  std::vector<int64_t> cell_off;                       // [K+1]: cell k owns elements [cell_off[k], cell_off[k+1]) of the flat order
+  std::vector<float *> cmaster, cgrad, copt;           // per-cell bases (single mode: master + cell_off[k], ...)
+  std::vector<void *> cwlp;
+  std::vector<float *> dout[2];                        // pipeline: local copy of the gradient wrt cell k's OUTPUT
+  std::vector<void *> dout_lp[2];
   std::vector<cudaStream_t> streams;
   std::vector<std::vector<float *>> slot;              // slot[k][m], k = 1..K-1: input of cell k
   std::vector<float *> dbound[2];                      // dbound[i][k]: gradient wrt input of cell k
@@ -101,7 +119,7 @@ struct Engine {
   std::vector<BwdScratch> bwd;
   int32_t *tok_dev = nullptr, *lab_dev = nullptr;
   float *pe = nullptr, *loss_parts = nullptr, *loss_dummy = nullptr;
-  int *flag_dev = nullptr;
+  int *flag_dev = nullptr, *flag_dev_last = nullptr;   // id-check flags: with the tokens (cell 0) / the labels (cell K-1)
   float *host_loss = nullptr;                          // pinned
   int *host_flag = nullptr;                            // pinned
 
@@ -153,15 +171,23 @@ struct Engine {
   int build_inventory(std::string &err);
   int build_plan(bool dry, std::string &err);
   // -- helpers --
-  Ctx ctx(int k) { return Ctx{st(k), &launches, sm_count, gemm_backend, device}; }
-  float *P(int i) const { return master + tensors[i].off; }            // fp32 vector param
-  const void *W(int i) const {                                         // matrix operand
-    return dt == GP_BF16 ? (const void *)((const char *)w_lp + tensors[i].off * 2)
-                         : (const void *)(master + tensors[i].off);
+  Ctx ctx(int k) { return Ctx{st(k), &launches, sm_count, gemm_backend, multi() ? cell_device[k] : device}; }
+  int64_t rel(int i) const { return tensors[i].off - cell_off[tensors[i].cell]; }
+  float *P(int i) const { return cmaster[tensors[i].cell] + rel(i); }  // fp32 master / vector param
+  void *Wl(int i) const {                                              // bf16 working copy (bf16 mode)
+    return (void *)((char *)cwlp[tensors[i].cell] + rel(i) * 2);
   }
-  float *G(int i) const { return grad + tensors[i].off; }
+  const void *W(int i) const {                                         // matrix operand
+    return dt == GP_BF16 ? (const void *)Wl(i) : (const void *)P(i);
+  }
+  float *G(int i) const { return cgrad[tensors[i].cell] + rel(i); }
+  float *Opt(int i) const { return copt[tensors[i].cell] + rel(i); }
+  cudaError_t use(int k) const {                                       // make cell k's device current
+    return multi_device ? cudaSetDevice(cell_device[k]) : cudaSuccess;
+  }
   Workspace &wsp(int k, int m) { return ws[k][remat ? 0 : m]; }
   // -- schedule --
+  cudaError_t peer_copy(int k_dst, void *dst, int k_src, const void *src, size_t bytes, cudaStream_t s);
   cudaError_t forward_cell(int k, int m, bool replay);
   cudaError_t backward_cell(int k, int m);
   cudaError_t run_step(float *loss_out);

@@ -56,6 +56,26 @@ def test_plan_bytes_follows_paper_memory_law():
     assert s[32] > 5 * r[32]
 
 
+def test_per_accelerator_plan_follows_table1():
+    """PAPER.md:65 / :103 (Table 1): with cell k on accelerator k the parameters, gradients and activations are
+    spread over the K devices - the per-device need falls roughly as 1/K, which is what lets a larger model fit.
+    Host-only planner of the pipeline handle (gpipe_plan_bytes_pipeline)."""
+    from paper_1811_06965_b200.binding import plan_bytes_pipeline
+    w = gi.CONFIGS["T(64,16384,32)"]
+    spec, keep = _spec(w)
+    one = gp.plan_bytes(spec, 16, w.M, True, w.n_seqs)
+    per = {K: plan_bytes_pipeline(spec, K, w.M, True, w.n_seqs) for K in (2, 4, 8, 16)}
+    for K, need in per.items():
+        assert len(need) == K
+        # the split adds only the staging copies of the boundary tensors
+        assert abs(sum(need) - gp.plan_bytes(spec, K, w.M, True, w.n_seqs)) <= 0.02 * one
+        assert max(need[1:-1] or need) <= 1.15 * min(need[1:-1] or need)   # interior cells are balanced
+    assert max(per[16]) < 0.09 * one and max(per[16]) < 16e9               # the 6 B model on 16 small accelerators
+    assert max(per[2]) > 6 * max(per[16])
+    uneven = plan_bytes_pipeline(spec, 4, w.M, True, w.n_seqs, cell_lo=[0, 10, 40, 100, 128])
+    assert uneven[2] > 1.8 * uneven[1] > 3 * uneven[0]
+
+
 def test_config5_fits_180GB_with_remat():
     w = gi.CONFIGS["T(64,16384,32)"]
     spec, keep = _spec(w)

@@ -43,6 +43,12 @@ class Workload:
     causal: Tuple[int, ...]
     remat: bool = True
     ln_eps: float = 1e-5
+    n_dec: int = 0            # > 0: encoder-decoder T(L,H,A): the LAST n_dec layers are decoder layers
+    logit_clip: float = 0.0   # > 0: clamp the logits to [-c, c] before the softmax
+
+    @property
+    def n_enc(self) -> int:
+        return self.n_layers - self.n_dec
 
     @property
     def d_attn(self) -> int:
@@ -81,21 +87,32 @@ def reduced(w: Workload, layers_per_cell: int = 1, seqs_per_microbatch: int = 1)
     L = w.K * layers_per_cell
     n_causal = round(L * sum(w.causal) / len(w.causal))
     causal = (0,) * (L - n_causal) + (1,) * n_causal
+    n_dec = round(L * w.n_dec / w.n_layers)          # encoder-decoder: keep the encoder / decoder proportion
     return w.replace(name=w.name + "-reduced", n_layers=L, n_seqs=w.M * seqs_per_microbatch,
-                     causal=causal)
+                     causal=causal, n_dec=n_dec)
 
 
 def tensor_shapes(w: Workload) -> List[Tuple[str, Tuple[int, int]]]:
     """Canonical tensor list: names and [rows, cols]; vectors are [1, n].
-    A naming/shape convention only - each side builds its own list and the tests compare."""
+    A naming/shape convention only - each side builds its own list and the tests compare.
+    Encoder-decoder workloads (n_dec > 0): `lne_*` (encoder output LayerNorm) sits in front of the first
+    decoder layer and every decoder layer carries the cross-attention block after its self-attention."""
     d, H, da, V = w.d_model, w.d_ffn, w.d_attn, w.vocab
     out = [("emb", (V, d))]
     for l in range(w.n_layers):
         p = f"l{l}."
+        dec = w.n_dec > 0 and l >= w.n_enc
+        if dec and l == w.n_enc:
+            out += [("lne_g", (1, d)), ("lne_b", (1, d))]
         out += [(p + "ln1_g", (1, d)), (p + "ln1_b", (1, d)),
                 (p + "w_qkv", (d, 3 * da)), (p + "b_qkv", (1, 3 * da)),
-                (p + "w_o", (da, d)), (p + "b_o", (1, d)),
-                (p + "ln2_g", (1, d)), (p + "ln2_b", (1, d)),
+                (p + "w_o", (da, d)), (p + "b_o", (1, d))]
+        if dec:
+            out += [(p + "lnx_g", (1, d)), (p + "lnx_b", (1, d)),
+                    (p + "w_q", (d, da)), (p + "b_q", (1, da)),
+                    (p + "w_kv", (d, 2 * da)), (p + "b_kv", (1, 2 * da)),
+                    (p + "w_o2", (da, d)), (p + "b_o2", (1, d))]
+        out += [(p + "ln2_g", (1, d)), (p + "ln2_b", (1, d)),
                 (p + "w_1", (d, H)), (p + "b_1", (1, H)),
                 (p + "w_2", (H, d)), (p + "b_2", (1, d))]
     out += [("lnf_g", (1, d)), ("lnf_b", (1, d)), ("w_out", (d, V))]
@@ -121,10 +138,30 @@ def make_tokens(w: Workload, seed: int) -> Tuple[np.ndarray, np.ndarray]:
     return tokens, labels
 
 
+def make_tokens_encdec(w: Workload, seed: int) -> Tuple[np.ndarray, np.ndarray, np.ndarray]:
+    """Encoder-decoder inputs: source ids uniform on [0, V), [N, S]; target ids [N, S+1], target tokens =
+    ids[:, :S], labels = ids[:, 1:] (the decoder predicts the next target id)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    src = rng.integers(0, w.vocab, size=(w.n_seqs, w.seq_len), dtype=np.int64).astype(np.int32)
+    ids = rng.integers(0, w.vocab, size=(w.n_seqs, w.seq_len + 1), dtype=np.int64)
+    return (np.ascontiguousarray(src), np.ascontiguousarray(ids[:, :-1]).astype(np.int32),
+            np.ascontiguousarray(ids[:, 1:]).astype(np.int32))
+
+
+def encdec(name: str, L: int, H: int, A: int, vocab: int = 64000, n_seqs: int = 128, M: int = 16, K: int = 16,
+           d_model: int = 1024, d_head: int = 64, seq_len: int = 256, dtype: str = "bf16", logit_clip: float = 0.0,
+           remat: bool = True) -> Workload:
+    """T(L,H,A) of PAPER.md:160: L encoder layers followed by L decoder layers, d_model 1024."""
+    return Workload(name, 2 * L, d_model, H, A, d_head, vocab, seq_len, n_seqs, M, K, dtype,
+                    (0,) * L + (1,) * L, remat, 1e-5, L, logit_clip)
+
+
 def make_params(w: Workload, seed: int, std: float = 0.02, parity: bool = True,
-                round_bf16: Optional[bool] = None) -> Dict[str, np.ndarray]:
+                round_bf16: Optional[bool] = None, ffn_depth_scale: bool = False) -> Dict[str, np.ndarray]:
     """N(0, std) matrices; parity=True also randomises biases / beta and gamma = 1 + N(0,std);
-    parity=False gives gamma = 1, beta = b = 0 (benchmark init). fp32 arrays, [rows, cols]."""
+    parity=False gives gamma = 1, beta = b = 0 (benchmark init). fp32 arrays, [rows, cols].
+    ffn_depth_scale: w_1 and w_2 are drawn with std / n_layers (PAPER.md:174 (i): "we scale down the
+    initialization of all transformer feed-forward layers by the number of layers")."""
     if round_bf16 is None:
         round_bf16 = (w.dtype == "bf16")
     rng = np.random.Generator(np.random.PCG64(seed))
@@ -136,7 +173,8 @@ def make_params(w: Workload, seed: int, std: float = 0.02, parity: bool = True,
         if is_vec and not parity:
             a = np.ones(shape, np.float32) if is_gamma else np.zeros(shape, np.float32)
         else:
-            a = (rng.standard_normal(shape, dtype=np.float32) * np.float32(std)).astype(np.float32)
+            sd = std / w.n_layers if ffn_depth_scale and base in ("w_1", "w_2") else std
+            a = (rng.standard_normal(shape, dtype=np.float32) * np.float32(sd)).astype(np.float32)
             if is_gamma:
                 a = (a + np.float32(1.0)).astype(np.float32)
         out[name] = bf16_round(a) if round_bf16 else a

@@ -168,11 +168,50 @@ int gpipe_create_pipeline(const gpipe_layer_spec *spec, int K, int M, int remat,
 int gpipe_attach_optimizer_slots_cell(gpipe_t *g, int k, void *slots_dev, size_t bytes);
 int gpipe_cell_param_count(const gpipe_t *g, int k, int64_t *n_out);
 
+/* ---- the encoder-decoder Transformer T(L,H,A) on the same schedule ----
+ * PAPER.md:160 (footnote 1): "T(L,H,A) is a Transformer model with L encoder layers and L decoder layers, a
+ * feed-forward hidden dimension of H and A attention heads.  The model dimension is fixed to 1024"; PAPER.md:174:
+ * "we clip the logit predictions (softmax pre-activations) whenever their magnitude exceeds a certain value" and "we
+ * scale down the initialization of all transformer feed-forward layers by the number of layers".
+ * The model is still ONE sequence of layers enc_0 .. enc_{n_enc-1}, dec_0 .. dec_{n_dec-1} cut into K cells of
+ * consecutive layers; M micro-batches, boundary-only storage and replay are unchanged.  What crosses a
+ * cell boundary is a PAIR (x, aux): in the encoder x is the source stream and aux the target embedding; the cell
+ * holding dec_0 forms the memory LN_e(x_src), and from there x is the target stream and aux the memory.
+ * Readings (B1-B6): an encoder layer is the layer of gpipe_layer_spec without mask; a decoder layer
+ * is causal self-attention, then cross-attention (pre-LN on the target stream; queries from it, keys / values from
+ * the memory, no mask), then the ReLU FFN; one embedding table for source and target ids, untied w_out; source
+ * and target both have seq_len tokens.
+ * Canonical tensor order: emb; per layer l = 0 .. n_enc+n_dec-1: [lne_g, lne_b in front of layer n_enc;] ln1_g,
+ * ln1_b, w_qkv, b_qkv, w_o, b_o, [decoder layers: lnx_g, lnx_b, w_q [d,da], b_q, w_kv [d,2*da] (k|v), b_kv,
+ * w_o2 [da,d], b_o2,] ln2_g, ln2_b, w_1, b_1, w_2, b_2; lnf_g, lnf_b, w_out.
+ * gpipe_create_encdec: as gpipe_create; cell_lo (host, K+1 boundaries over the n_enc+n_dec layers) may be NULL for
+ * the equal split; 1 <= K <= n_enc + n_dec.  gpipe_step_encdec: src, tgt, labels are HOST int32 [n_seqs, seq_len]
+ * (labels[t] = the target id the decoder must predict at position t); gpipe_step_encdec_device: the same ids already
+ * in HBM.  gpipe_step / gpipe_step_device on such a handle (and these on a plain handle) return GPIPE_EINVAL.
+ * Every other call (apply, parameters, tracker, trace, graph, data-parallel apply) works unchanged; pipeline handles
+ * (gpipe_create_pipeline) are not built for this model. */
+typedef struct {
+  int32_t n_enc, n_dec; /* >= 1 each                                                           */
+  int32_t d_model, d_ffn, n_heads, d_head, vocab, seq_len, dtype;   /* as gpipe_layer_spec    */
+  float   ln_eps;       /* 0 -> 1e-5                                                           */
+  float   logit_clip;   /* c >= 0; 0 = no clipping                                             */
+} gpipe_encdec_spec;
+int gpipe_plan_bytes_encdec(const gpipe_encdec_spec *spec, int K, int M, int remat, int64_t n_seqs,
+                            const int32_t *cell_lo, size_t *bytes_out);
+int gpipe_create_encdec(const gpipe_encdec_spec *spec, int K, int M, int remat, int64_t n_seqs,
+                        const gpipe_env *env, const int32_t *cell_lo, gpipe_t **out);
+int gpipe_step_encdec(gpipe_t *g, const int32_t *src, const int32_t *tgt, const int32_t *labels, float *loss_out);
+int gpipe_step_encdec_device(gpipe_t *g, const int32_t *src_dev, const int32_t *tgt_dev, const int32_t *labels_dev,
+                             float *loss_out);
+
 /* N(0, std) for matrices and emb, from a counter-based generator on the device (Philox-4x32-10
  * + Box-Muller); parity != 0 also draws biases / beta ~ N(0,std) and gamma = 1 + N(0,std)
  * (reading A10), parity == 0 sets gamma = 1, beta = bias = 0.  bf16 mode: the master is the
  * RNE-bf16-rounded draw (reading A12). */
 int gpipe_init_params(gpipe_t *g, uint64_t seed, float std, int parity);
+/* The same draw with the FFN matrices w_1, w_2 of every layer drawn at std * ffn_scale ("we scale down
+ * the initialization of all transformer feed-forward layers by the number of layers": ffn_scale = 1 / n_layers). */
+int gpipe_init_params_scaled(gpipe_t *g, uint64_t seed, float std, int parity, float ffn_scale);
 
 /* gpipe_step(tokens, labels) -> loss.  tokens, labels: HOST, int32 [n_seqs, seq_len] row-major,
  * values in [0, V), read during the call only.  Runs the whole GPipe schedule (forward ticks,

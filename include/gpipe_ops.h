@@ -78,9 +78,12 @@ int gpipe_op_attn_bwd(void *stream, int dtype, const void *qkv, const void *o, c
                       const float *lse, void *dqkv, float *dvec, int n_seq, int S, int A, int dh,
                       int causal, int backend);
 
-/* in place logits -> dlogits = (softmax - onehot) * inv_T; rowloss[t] = CE_t * inv_T */
+/* in place logits -> dlogits = (softmax - onehot) * inv_T; rowloss[t] = CE_t * inv_T.
+ * clip > 0 ("we clip the logit predictions (softmax pre-activations) whenever their magnitude exceeds a
+ * certain value"; reading B5): the softmax and the loss see clamp(logit, -clip, clip) and dlogits is 0
+ * wherever |logit| > clip; clip == 0: no clipping. */
 int gpipe_op_softmax_ce(void *stream, int dtype, void *logits, const int32_t *labels, float *rowloss,
-                        int64_t n_tok, int V, float inv_T);
+                        int64_t n_tok, int V, float inv_T, float clip);
 /* out[n] += sum_t dy[t,n]; scratch: fp32 [gpipe_op_colsum_scratch_floats(n_tok, n)] */
 int64_t gpipe_op_colsum_scratch_floats(int64_t n_tok, int n);
 int gpipe_op_colsum(void *stream, int dtype, const void *dy, int64_t ld, float *out, float *scratch,

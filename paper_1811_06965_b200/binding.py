@@ -34,6 +34,12 @@ class LayerSpec(C.Structure):
                 ("ln_eps", C.c_float)]
 
 
+class EncDecSpec(C.Structure):
+    _fields_ = [("n_enc", C.c_int32), ("n_dec", C.c_int32), ("d_model", C.c_int32), ("d_ffn", C.c_int32),
+                ("n_heads", C.c_int32), ("d_head", C.c_int32), ("vocab", C.c_int32), ("seq_len", C.c_int32),
+                ("dtype", C.c_int32), ("ln_eps", C.c_float), ("logit_clip", C.c_float)]
+
+
 class Env(C.Structure):
     _fields_ = [("arena", C.c_void_p), ("arena_bytes", C.c_size_t),
                 ("streams", C.POINTER(C.c_void_p)), ("n_streams", C.c_int32)]
@@ -81,7 +87,14 @@ def lib() -> C.CDLL:
                                         C.POINTER(C.c_int32), i32, C.POINTER(vp)]),
         "gpipe_attach_optimizer_slots_cell": (i32, [vp, i32, vp, C.c_size_t]),
         "gpipe_cell_param_count": (i32, [vp, i32, C.POINTER(i64)]),
+        "gpipe_plan_bytes_encdec": (i32, [C.POINTER(EncDecSpec), i32, i32, i32, i64, C.POINTER(C.c_int32),
+                                          C.POINTER(C.c_size_t)]),
+        "gpipe_create_encdec": (i32, [C.POINTER(EncDecSpec), i32, i32, i32, i64, C.POINTER(Env), C.POINTER(C.c_int32),
+                                      C.POINTER(vp)]),
+        "gpipe_step_encdec": (i32, [vp, vp, vp, vp, C.POINTER(f32)]),
+        "gpipe_step_encdec_device": (i32, [vp, vp, vp, vp, C.POINTER(f32)]),
         "gpipe_init_params": (i32, [vp, C.c_uint64, f32, i32]),
+        "gpipe_init_params_scaled": (i32, [vp, C.c_uint64, f32, i32, f32]),
         "gpipe_step": (i32, [vp, vp, vp, C.POINTER(f32)]),
         "gpipe_step_device": (i32, [vp, vp, vp, C.POINTER(f32)]),
         "gpipe_apply_sgd": (i32, [vp, f32]),
@@ -123,7 +136,7 @@ def lib() -> C.CDLL:
         "gpipe_op_ln_bwd": (i32, [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, i32]),
         "gpipe_op_attn_fwd": (i32, [vp, i32, vp, vp, vp, i32, i32, i32, i32, i32, i32]),
         "gpipe_op_attn_bwd": (i32, [vp, i32, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32]),
-        "gpipe_op_softmax_ce": (i32, [vp, i32, vp, vp, vp, i64, i32, f32]),
+        "gpipe_op_softmax_ce": (i32, [vp, i32, vp, vp, vp, i64, i32, f32, f32]),
         "gpipe_op_colsum_scratch_floats": (i64, [i64, i32]),
         "gpipe_op_colsum": (i32, [vp, i32, vp, i64, vp, vp, i64, i32]),
         "gpipe_op_embed_fwd": (i32, [vp, i32, vp, vp, vp, vp, i64, i32, i32]),
@@ -144,7 +157,8 @@ def lib() -> C.CDLL:
 EXPORTED_SYMBOLS = [
     "gpipe_plan_bytes", "gpipe_create", "gpipe_destroy", "gpipe_layer_costs", "gpipe_partition_min_variance",
     "gpipe_create_partitioned", "gpipe_cell_range", "gpipe_plan_bytes_pipeline", "gpipe_create_pipeline",
-    "gpipe_attach_optimizer_slots_cell", "gpipe_cell_param_count", "gpipe_init_params", "gpipe_step",
+    "gpipe_attach_optimizer_slots_cell", "gpipe_cell_param_count", "gpipe_init_params", "gpipe_init_params_scaled",
+    "gpipe_plan_bytes_encdec", "gpipe_create_encdec", "gpipe_step_encdec", "gpipe_step_encdec_device", "gpipe_step",
     "gpipe_step_device", "gpipe_apply_sgd", "gpipe_optimizer_slot_bytes", "gpipe_attach_optimizer_slots",
     "gpipe_apply_rmsprop", "gpipe_op_rmsprop", "gpipe_zero_grads", "gpipe_dp_shard", "gpipe_dp_layout",
     "gpipe_dp_apply_sgd", "gpipe_dp_apply_rmsprop", "gpipe_ipc_export", "gpipe_ipc_open", "gpipe_ipc_close", "gpipe_num_tensors",
@@ -188,6 +202,14 @@ def plan_bytes(spec: LayerSpec, K: int, M: int, remat: bool, n_seqs: int) -> int
     """gpipe_plan_bytes: host-only, works without a GPU."""
     out = C.c_size_t(0)
     _check(lib().gpipe_plan_bytes(C.byref(spec), K, M, int(bool(remat)), n_seqs, C.byref(out)))
+    return int(out.value)
+
+
+def plan_bytes_encdec(spec: "EncDecSpec", K: int, M: int, remat: bool, n_seqs: int, cell_lo=None) -> int:
+    """gpipe_plan_bytes_encdec: host-only."""
+    out = C.c_size_t(0)
+    lo = (C.c_int32 * (K + 1))(*[int(v) for v in cell_lo]) if cell_lo is not None else None
+    _check(lib().gpipe_plan_bytes_encdec(C.byref(spec), K, M, int(bool(remat)), n_seqs, lo, C.byref(out)))
     return int(out.value)
 
 
@@ -333,9 +355,10 @@ class GPipe:
         self.close()
 
     # -- the three calls ------------------------------------------------------------------------
-    def init_params(self, seed: int, std: float = 0.02, parity: bool = False):
+    def init_params(self, seed: int, std: float = 0.02, parity: bool = False, ffn_scale: float = 1.0):
+        """ffn_scale: std multiplier of w_1 / w_2 (1 / n_layers for the depth-scaled initialisation)."""
         with self._torch.cuda.device(self.device):
-            _check(lib().gpipe_init_params(self._h, seed, std, int(parity)))
+            _check(lib().gpipe_init_params_scaled(self._h, seed, std, int(parity), ffn_scale))
 
     def step(self, tokens, labels) -> float:
         """tokens/labels: numpy int32 [N,S] or CPU torch tensors (host path, gpipe_step), or CUDA
@@ -542,3 +565,61 @@ class GPipe:
             self._torch.cuda.synchronize(self.device)
             _check(lib().gpipe_debug_read(self._h, what.encode(), layer, out.ctypes.data, max_elems, C.byref(n)))
         return out[:n.value].copy()
+
+
+class GPipeEncDec(GPipe):
+    """The encoder-decoder Transformer T(L,H,A) of PAPER.md:160 on the same schedule (gpipe_create_encdec /
+    gpipe_step_encdec): n_enc encoder layers, then n_dec decoder layers with cross-attention over the
+    encoder memory, cut into K cells of consecutive layers.  partition: None or K+1 boundaries over the n_enc + n_dec
+    layers.  logit_clip: PAPER.md:174 (0 = off)."""
+
+    def __init__(self, *, n_enc, n_dec, d_model, d_ffn, n_heads, d_head, vocab, seq_len, dtype, K, M, remat=True,
+                 n_seqs, ln_eps=1e-5, logit_clip=0.0, device="cuda:0", partition=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise GPipeError(-2, "no CUDA device: the GPipe path has no CPU fallback")
+        self._torch = torch
+        self.device = torch.device(device)
+        dt = {"fp32": DTYPE_FP32, "bf16": DTYPE_BF16, 0: 0, 1: 1}[dtype]
+        self.spec = EncDecSpec(n_enc, n_dec, d_model, d_ffn, n_heads, d_head, vocab, seq_len, dt, ln_eps, logit_clip)
+        self.K, self.M, self.remat, self.n_seqs, self.seq_len = K, M, bool(remat), n_seqs, seq_len
+        self._h = C.c_void_p(None)
+        self.devices = None
+        lo = (C.c_int32 * (K + 1))(*[int(v) for v in partition]) if partition is not None else None
+        with torch.cuda.device(self.device):
+            nbytes = plan_bytes_encdec(self.spec, K, M, remat, n_seqs, partition)
+            self.arena = torch.empty(nbytes + 1024, dtype=torch.uint8, device=self.device)
+            base = (self.arena.data_ptr() + 1023) // 1024 * 1024
+            self.streams = [torch.cuda.Stream(device=self.device) for _ in range(K)]
+            self._stream_arr = (C.c_void_p * K)(*[s.cuda_stream for s in self.streams])
+            env = Env(base, nbytes, C.cast(self._stream_arr, C.POINTER(C.c_void_p)), K)
+            torch.cuda.synchronize(self.device)
+            _check(lib().gpipe_create_encdec(C.byref(self.spec), K, M, int(self.remat), n_seqs, C.byref(env), lo,
+                                             C.byref(self._h)))
+        self._finish_init(K)
+
+    def step(self, src, tgt, labels) -> float:
+        """src / tgt / labels: numpy int32 [N,S] or CPU tensors (gpipe_step_encdec), or CUDA int32 tensors
+        (gpipe_step_encdec_device).  Returns the mean loss."""
+        torch = self._torch
+        loss = C.c_float(0)
+        n = self.n_seqs * self.seq_len
+        with torch.cuda.device(self.device):
+            if isinstance(src, torch.Tensor) and src.is_cuda:
+                ts = [t.contiguous() for t in (src, tgt, labels)]
+                if any(t.dtype != torch.int32 or t.numel() != n for t in ts):
+                    raise ValueError("device ids must be int32 [n_seqs, seq_len]")
+                torch.cuda.current_stream(self.device).synchronize()
+                _check(lib().gpipe_step_encdec_device(self._h, ts[0].data_ptr(), ts[1].data_ptr(), ts[2].data_ptr(),
+                                                      C.byref(loss)))
+            else:
+                hs = [np.ascontiguousarray(t.numpy() if isinstance(t, torch.Tensor) else t, dtype=np.int32)
+                      for t in (src, tgt, labels)]
+                if any(h.size != n for h in hs):
+                    raise ValueError("src/tgt/labels must be [n_seqs, seq_len]")
+                _check(lib().gpipe_step_encdec(self._h, hs[0].ctypes.data, hs[1].ctypes.data, hs[2].ctypes.data,
+                                               C.byref(loss)))
+        return float(loss.value)
+
+    def debug_read(self, *a, **kw):
+        raise GPipeError(-4, "debug taps are not built for the encoder-decoder handle")

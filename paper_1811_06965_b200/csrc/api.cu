@@ -42,9 +42,12 @@ static int env_int(const char *name, int dflt) {
 
 // fills the shape fields of an Engine from the spec; no CUDA calls
 static int configure(Engine &e, const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs,
-                     const int32_t *cell_lo = nullptr) {
+                     const int32_t *cell_lo = nullptr, int n_dec = 0, float logit_clip = 0.f) {
   if (!spec) return fail(GPIPE_EINVAL, "spec is NULL");
   e.spec = *spec;
+  e.n_dec = n_dec;
+  e.n_enc = spec->n_layers - n_dec;
+  e.logit_clip = logit_clip;
   e.dt = spec->dtype;
   if (e.dt != GPIPE_DTYPE_FP32 && e.dt != GPIPE_DTYPE_BF16) return fail(GPIPE_EINVAL, "dtype must be 0 (fp32) or 1 (bf16)");
   e.d = spec->d_model; e.H = spec->d_ffn; e.A = spec->n_heads; e.V = spec->vocab; e.S = spec->seq_len;
@@ -66,6 +69,8 @@ static int configure(Engine &e, const gpipe_layer_spec *spec, int K, int M, int 
   if (e.T_mb * (int64_t)(e.V > 3 * e.da ? e.V : 3 * e.da) >= ((int64_t)1 << 40)) return fail(GPIPE_EINVAL, "micro-batch too large");
   e.causal.assign(L, 1);
   if (spec->causal) for (int l = 0; l < L; ++l) e.causal[l] = spec->causal[l] ? 1 : 0;
+  e.spec.causal = nullptr;                  // the caller's array is read here only
+  if (e.encdec()) for (int l = 0; l < L; ++l) e.causal[l] = e.is_dec(l) ? 1 : 0;   // reading B1
   e.cell_lo.resize(K); e.cell_hi.resize(K);
   int base = L / K, extra = L % K;          // first L mod K cells get one more layer
   for (int k = 0; k < K; ++k) {
@@ -146,7 +151,8 @@ int gpipe_plan_bytes_pipeline(const gpipe_layer_spec *spec, int K, int M, int re
 }
 
 static int create_impl(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs, const gpipe_env *env,
-                       const int32_t *cell_lo, gpipe_t **out, const gpipe_cell_env *cells = nullptr, int flags = 0);
+                       const int32_t *cell_lo, gpipe_t **out, const gpipe_cell_env *cells = nullptr, int flags = 0,
+                       int n_dec = 0, float logit_clip = 0.f);
 int gpipe_create_pipeline(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs,
                           const gpipe_cell_env *cells, const int32_t *cell_lo, int flags, gpipe_t **out) {
   if (!cells) return fail(GPIPE_EINVAL, "cells is NULL");
@@ -160,6 +166,42 @@ int gpipe_create_partitioned(const gpipe_layer_spec *spec, int K, int M, int rem
   if (!cell_lo) return fail(GPIPE_EINVAL, "cell_lo is NULL");
   return create_impl(spec, K, M, remat, n_seqs, env, cell_lo, out);
 }
+// ---- encoder-decoder T(L,H,A) ------------------------------------------------------------------
+static int encdec_to_layer_spec(const gpipe_encdec_spec *s, gpipe_layer_spec *ls) {
+  if (!s) return fail(GPIPE_EINVAL, "spec is NULL");
+  if (s->n_enc < 1 || s->n_dec < 1) return fail(GPIPE_EINVAL, "an encoder-decoder model needs n_enc >= 1 and n_dec >= 1 (PAPER.md:160)");
+  if (!(s->logit_clip >= 0.f)) return fail(GPIPE_EINVAL, "logit_clip must be >= 0 (0 = off)");
+  memset(ls, 0, sizeof(*ls));
+  ls->n_layers = s->n_enc + s->n_dec;
+  ls->d_model = s->d_model; ls->d_ffn = s->d_ffn; ls->n_heads = s->n_heads; ls->d_head = s->d_head;
+  ls->vocab = s->vocab; ls->seq_len = s->seq_len; ls->dtype = s->dtype; ls->causal = nullptr; ls->ln_eps = s->ln_eps;
+  return GPIPE_OK;
+}
+
+int gpipe_plan_bytes_encdec(const gpipe_encdec_spec *spec, int K, int M, int remat, int64_t n_seqs, const int32_t *cell_lo,
+                            size_t *bytes_out) {
+  if (!bytes_out) return fail(GPIPE_EINVAL, "bytes_out is NULL");
+  gpipe_layer_spec ls;
+  int rc = encdec_to_layer_spec(spec, &ls);
+  if (rc) return rc;
+  Engine e;
+  rc = configure(e, &ls, K, M, remat, n_seqs, cell_lo, spec->n_dec, spec->logit_clip);
+  if (rc) return rc;
+  std::string err;
+  rc = e.build_plan(true, err);
+  if (rc) return fail(rc, err);
+  *bytes_out = e.arena.used;
+  return GPIPE_OK;
+}
+
+int gpipe_create_encdec(const gpipe_encdec_spec *spec, int K, int M, int remat, int64_t n_seqs, const gpipe_env *env,
+                        const int32_t *cell_lo, gpipe_t **out) {
+  gpipe_layer_spec ls;
+  int rc = encdec_to_layer_spec(spec, &ls);
+  if (rc) return rc;
+  return create_impl(&ls, K, M, remat, n_seqs, env, cell_lo, out, nullptr, 0, spec->n_dec, spec->logit_clip);
+}
+
 int gpipe_cell_range(const gpipe_t *g, int k, int32_t *lo, int32_t *hi) {
   if (!g || k < 0 || k >= g->e.K) return fail(GPIPE_EINVAL, "handle is NULL or cell index out of range");
   if (lo) *lo = g->e.cell_lo[k];
@@ -221,7 +263,8 @@ int gpipe_partition_min_variance(const double *layer_cost, int L, double first_e
 }
 
 static int create_impl(const gpipe_layer_spec *spec, int K, int M, int remat, int64_t n_seqs, const gpipe_env *env,
-                       const int32_t *cell_lo, gpipe_t **out, const gpipe_cell_env *cells, int flags) {
+                       const int32_t *cell_lo, gpipe_t **out, const gpipe_cell_env *cells, int flags, int n_dec,
+                       float logit_clip) {
   if (!out) return fail(GPIPE_EINVAL, "out is NULL");
   *out = nullptr;
   const bool pipe = cells != nullptr;
@@ -229,8 +272,9 @@ static int create_impl(const gpipe_layer_spec *spec, int K, int M, int remat, in
   gpipe *g = new (std::nothrow) gpipe();
   if (!g) return fail(GPIPE_ENOMEM, "host allocation failed");
   Engine &e = g->e;
-  int rc = configure(e, spec, K, M, remat, n_seqs, cell_lo);
+  int rc = configure(e, spec, K, M, remat, n_seqs, cell_lo, n_dec, logit_clip);
   if (rc) { delete g; return rc; }
+  if (pipe && e.encdec()) { delete g; return fail(GPIPE_ENOTIMPL, "pipeline handles are not built for the encoder-decoder model"); }
   int dev = 0;
   cudaError_t ce = cudaGetDevice(&dev);
   if (ce != cudaSuccess) { delete g; return cuda_fail(ce, "gpipe_create: no usable CUDA device"); }
@@ -352,7 +396,12 @@ void gpipe_destroy(gpipe_t *g) {
 }
 
 int gpipe_init_params(gpipe_t *g, uint64_t seed, float std, int parity) {
+  return gpipe_init_params_scaled(g, seed, std, parity, 1.f);
+}
+
+int gpipe_init_params_scaled(gpipe_t *g, uint64_t seed, float std, int parity, float ffn_scale) {
   if (!g) return fail(GPIPE_EINVAL, "handle is NULL");
+  if (!(ffn_scale > 0.f)) return fail(GPIPE_EINVAL, "ffn_scale must be > 0");
   Engine &e = g->e;
   for (size_t i = 0; i < e.tensors.size(); ++i) {
     const TensorInfo &t = e.tensors[i];
@@ -364,7 +413,9 @@ int gpipe_init_params(gpipe_t *g, uint64_t seed, float std, int parity) {
     bool gamma = !t.matrix && t.name.size() >= 2 && t.name.compare(t.name.size() - 2, 2, "_g") == 0;
     cudaError_t ce;
     if (t.matrix || parity) {
-      ce = init_normal(c, e.dt, m, w, n, seed, (uint64_t)i, gamma ? 1.f : 0.f, std);
+      const bool ffn = t.matrix && t.name.size() >= 3 && (t.name.compare(t.name.size() - 3, 3, "w_1") == 0 ||
+                                                          t.name.compare(t.name.size() - 3, 3, "w_2") == 0);
+      ce = init_normal(c, e.dt, m, w, n, seed, (uint64_t)i, gamma ? 1.f : 0.f, ffn ? std * ffn_scale : std);
     } else {
       ce = fill_f32(c, m, n, gamma ? 1.f : 0.f);
       if (ce == cudaSuccess) ce = master_to_lp(c, e.dt, m, w, n, 0);
@@ -390,9 +441,44 @@ static int step_common(Engine &e, float *loss_out) {
   return GPIPE_OK;
 }
 
+int gpipe_step_encdec(gpipe_t *g, const int32_t *src, const int32_t *tgt, const int32_t *labels, float *loss_out) {
+  if (!g || !src || !tgt || !labels) return fail(GPIPE_EINVAL, "handle, src, tgt and labels are required");
+  Engine &e = g->e;
+  if (!e.encdec()) return fail(GPIPE_EINVAL, "not an encoder-decoder handle: use gpipe_step");
+  for (int64_t i = 0; i < e.T_total; ++i)
+    if (src[i] < 0 || src[i] >= e.V || tgt[i] < 0 || tgt[i] >= e.V || labels[i] < 0 || labels[i] >= e.V)
+      return fail(GPIPE_EINVAL, "source/target/label id outside [0, V) at flat index " + std::to_string(i));
+  const size_t nb = (size_t)e.T_total * 4;
+  API_CUDA(cudaMemcpyAsync(e.tok_dev, src, nb, cudaMemcpyHostToDevice, e.streams[0]), "gpipe_step_encdec H2D");
+  API_CUDA(cudaMemcpyAsync(e.tgt_dev, tgt, nb, cudaMemcpyHostToDevice, e.streams[0]), "gpipe_step_encdec H2D");
+  API_CUDA(cudaMemcpyAsync(e.lab_dev, labels, nb, cudaMemcpyHostToDevice, e.streams[0]), "gpipe_step_encdec H2D");
+  return step_common(e, loss_out);
+}
+
+int gpipe_step_encdec_device(gpipe_t *g, const int32_t *src_dev, const int32_t *tgt_dev, const int32_t *labels_dev,
+                             float *loss_out) {
+  if (!g || !src_dev || !tgt_dev || !labels_dev) return fail(GPIPE_EINVAL, "handle, src, tgt and labels are required");
+  Engine &e = g->e;
+  if (!e.encdec()) return fail(GPIPE_EINVAL, "not an encoder-decoder handle: use gpipe_step_device");
+  Ctx c0 = e.ctx(0);
+  const size_t nb = (size_t)e.T_total * 4;
+  API_CUDA(cudaMemsetAsync(e.flag_dev, 0, 4, c0.stream), "gpipe_step_encdec_device");
+  API_CUDA(cudaMemcpyAsync(e.tok_dev, src_dev, nb, cudaMemcpyDefault, c0.stream), "gpipe_step_encdec_device");
+  API_CUDA(cudaMemcpyAsync(e.tgt_dev, tgt_dev, nb, cudaMemcpyDefault, c0.stream), "gpipe_step_encdec_device");
+  API_CUDA(cudaMemcpyAsync(e.lab_dev, labels_dev, nb, cudaMemcpyDefault, c0.stream), "gpipe_step_encdec_device");
+  API_CUDA(check_ids(c0, e.tok_dev, e.T_total, e.V, e.flag_dev), "gpipe_step_encdec_device");
+  API_CUDA(check_ids(c0, e.tgt_dev, e.T_total, e.V, e.flag_dev), "gpipe_step_encdec_device");
+  API_CUDA(check_ids(c0, e.lab_dev, e.T_total, e.V, e.flag_dev), "gpipe_step_encdec_device");
+  API_CUDA(cudaMemcpyAsync(e.host_flag, e.flag_dev, 4, cudaMemcpyDeviceToHost, c0.stream), "gpipe_step_encdec_device");
+  API_CUDA(cudaStreamSynchronize(c0.stream), "gpipe_step_encdec_device");
+  if (e.host_flag[0]) return fail(GPIPE_EINVAL, "source/target/label id outside [0, V)");
+  return step_common(e, loss_out);
+}
+
 int gpipe_step(gpipe_t *g, const int32_t *tokens, const int32_t *labels, float *loss_out) {
   if (!g || !tokens || !labels) return fail(GPIPE_EINVAL, "handle, tokens and labels are required");
   Engine &e = g->e;
+  if (e.encdec()) return fail(GPIPE_EINVAL, "encoder-decoder handle: use gpipe_step_encdec");
   for (int64_t i = 0; i < e.T_total; ++i)
     if (tokens[i] < 0 || tokens[i] >= e.V || labels[i] < 0 || labels[i] >= e.V)
       return fail(GPIPE_EINVAL, "token/label outside [0, V) at flat index " + std::to_string(i));
@@ -409,6 +495,7 @@ int gpipe_step(gpipe_t *g, const int32_t *tokens, const int32_t *labels, float *
 int gpipe_step_device(gpipe_t *g, const int32_t *tokens_dev, const int32_t *labels_dev, float *loss_out) {
   if (!g || !tokens_dev || !labels_dev) return fail(GPIPE_EINVAL, "handle, tokens and labels are required");
   Engine &e = g->e;
+  if (e.encdec()) return fail(GPIPE_EINVAL, "encoder-decoder handle: use gpipe_step_encdec_device");
   const int kl = e.multi() ? e.K - 1 : 0;
   // ids move to the cells that use them (cell 0: embedding, cell K-1: loss), are range-checked there, then the step runs
   API_CUDA(e.use(0), "gpipe_step_device");

@@ -42,12 +42,26 @@ int Engine::build_inventory(std::string &err) {
   for (int l = 0; l < spec.n_layers; ++l) {
     std::string p = "l" + std::to_string(l) + ".";
     LayerParams q;
+    if (encdec() && l == n_enc) {          // encoder output LayerNorm: in front of the first decoder layer
+      i_lne_g = add("lne_g", 1, d, false);
+      i_lne_b = add("lne_b", 1, d, false);
+    }
     q.ln1_g = add(p + "ln1_g", 1, d, false);
     q.ln1_b = add(p + "ln1_b", 1, d, false);
     q.w_qkv = add(p + "w_qkv", d, 3 * da, true);
     q.b_qkv = add(p + "b_qkv", 1, 3 * da, false);
     q.w_o = add(p + "w_o", da, d, true);
     q.b_o = add(p + "b_o", 1, d, false);
+    if (is_dec(l)) {                       // cross-attention block (canonical order of gpipe.h)
+      q.lnx_g = add(p + "lnx_g", 1, d, false);
+      q.lnx_b = add(p + "lnx_b", 1, d, false);
+      q.w_q = add(p + "w_q", d, da, true);
+      q.b_q = add(p + "b_q", 1, da, false);
+      q.w_kv = add(p + "w_kv", d, 2 * da, true);
+      q.b_kv = add(p + "b_kv", 1, 2 * da, false);
+      q.w_o2 = add(p + "w_o2", da, d, true);
+      q.b_o2 = add(p + "b_o2", 1, d, false);
+    }
     q.ln2_g = add(p + "ln2_g", 1, d, false);
     q.ln2_b = add(p + "ln2_b", 1, d, false);
     q.w_1 = add(p + "w_1", d, H, true);
@@ -63,16 +77,23 @@ int Engine::build_inventory(std::string &err) {
   // owners: the canonical order is emb | layers in order | final LN, w_out and cells are consecutive layer ranges,
   // so every cell owns one contiguous range of the flat order
   tensors[i_emb].cell = 0;
+  kt = 0;
   for (int k = 0; k < K; ++k)
     for (int l = cell_lo[k]; l < cell_hi[k]; ++l) {
       const LayerParams &q = lp[l];
-      for (int i : {q.ln1_g, q.ln1_b, q.w_qkv, q.b_qkv, q.w_o, q.b_o, q.ln2_g, q.ln2_b, q.w_1, q.b_1, q.w_2, q.b_2})
-        tensors[i].cell = k;
+      for (int i : {q.ln1_g, q.ln1_b, q.w_qkv, q.b_qkv, q.w_o, q.b_o, q.ln2_g, q.ln2_b, q.w_1, q.b_1, q.w_2, q.b_2,
+                    q.lnx_g, q.lnx_b, q.w_q, q.b_q, q.w_kv, q.b_kv, q.w_o2, q.b_o2})
+        if (i >= 0) tensors[i].cell = k;
+      if (encdec() && l == n_enc) { kt = k; tensors[i_lne_g].cell = tensors[i_lne_b].cell = k; }
     }
   tensors[i_lnf_g].cell = tensors[i_lnf_b].cell = tensors[i_w_out].cell = K - 1;
   cell_off.assign(K + 1, n_flat);
   cell_off[0] = 0;
-  for (int k = 1; k < K; ++k) cell_off[k] = cell_lo[k] < spec.n_layers ? tensors[lp[cell_lo[k]].ln1_g].off : tensors[i_lnf_g].off;
+  for (int k = 1; k < K; ++k) {
+    if (cell_lo[k] >= spec.n_layers) cell_off[k] = tensors[i_lnf_g].off;
+    else if (encdec() && cell_lo[k] == n_enc) cell_off[k] = tensors[i_lne_g].off;
+    else cell_off[k] = tensors[lp[cell_lo[k]].ln1_g].off;
+  }
   return GPIPE_OK;
 }
 
@@ -124,10 +145,24 @@ int Engine::build_plan(bool dry, std::string &err) {
   loss_dummy = loss_parts ? loss_parts + M : nullptr;
   flag_dev = (int *)RAW(4, GPIPE_CAT_MISC, -1, 0);
   flag_dev_last = multi() ? (int *)RAW(4, GPIPE_CAT_MISC, -1, K - 1) : flag_dev;
+  tgt_dev = encdec() ? (int32_t *)RAW((size_t)T_total * 4, GPIPE_CAT_MISC, -1, 0) : nullptr;
 
   slot.assign(K, std::vector<float *>(M, nullptr));
   for (int k = 1; k < K; ++k)
     for (int m = 0; m < M; ++m) slot[k][m] = F32(Tm * d, GPIPE_CAT_BOUNDARY, k);
+  // encoder-decoder: the second member of the boundary pair.  One buffer per micro-batch serves every cell that
+  // reads it (the hand-off is a pointer, as for x): the target embedding up to the transition cell, the memory
+  // after it; its gradient travels through a two-entry ring like the gradient of x.
+  aux_tgt.assign(M, nullptr);
+  aux_mem.assign(M, nullptr);
+  if (encdec()) {
+    for (int m = 0; m < M && kt > 0; ++m) aux_tgt[m] = F32(Tm * d, GPIPE_CAT_BOUNDARY, kt);
+    for (int m = 0; m < M && kt < K - 1; ++m) aux_mem[m] = LP(Tm * d, GPIPE_CAT_BOUNDARY, kt);
+  }
+  for (int i = 0; i < 2; ++i) {
+    dbound_aux[i].assign(K, nullptr);
+    for (int k = 1; k < K && encdec(); ++k) dbound_aux[i][k] = F32(Tm * d, GPIPE_CAT_BOUNDARY, k);
+  }
   for (int i = 0; i < 2; ++i) {
     dbound[i].assign(K, nullptr);
     dbound_lp[i].assign(K, nullptr);
@@ -161,7 +196,8 @@ int Engine::build_plan(bool dry, std::string &err) {
     const int T = (int)T_mb;
     const int shapes[][3] = {{T, 3 * da, d}, {T, d, da}, {T, H, d}, {T, d, H}, {T, V, d},          // forward
                              {T, da, d}, {T, d, 3 * da}, {T, d, V},                                 // dgrad (others as forward)
-                             {H, d, T}, {d, H, T}, {da, d, T}, {d, 3 * da, T}, {d, V, T}};            // wgrad
+                             {H, d, T}, {d, H, T}, {da, d, T}, {d, 3 * da, T}, {d, V, T},             // wgrad
+                             {T, da, d}, {T, 2 * da, d}, {T, d, 2 * da}, {d, da, T}, {d, 2 * da, T}};   // cross-attention
     for (auto &sh : shapes) {
       size_t b = gemm_splitk_ws_bytes(sh[0], sh[1], sh[2], kPlanSmCount);
       if (b > splitk_ws_bytes) splitk_ws_bytes = b;
@@ -176,6 +212,12 @@ int Engine::build_plan(bool dry, std::string &err) {
       Workspace &W_ = ws[k][w];
       const int cat = GPIPE_CAT_INTERIOR;
       if (k == 0) W_.x_emb = F32(Tm * d, cat, k);
+      if (encdec() && k == kt) {
+        if (k == 0) W_.aux_emb = F32(Tm * d, cat, k);
+        W_.mem = LP(Tm * d, cat, k);
+        W_.mean_e = F32(Tm, cat, k);
+        W_.rstd_e = F32(Tm, cat, k);
+      }
       if (k == K - 1 || remat || multi()) W_.x_out = F32(Tm * d, cat, k);   // pipeline: also the outgoing boundary staging
       int nl = cell_hi[k] - cell_lo[k];
       W_.layers.resize(nl);
@@ -194,6 +236,15 @@ int Engine::build_plan(bool dry, std::string &err) {
         b.rstd1 = F32(Tm, cat, k);
         b.mean2 = F32(Tm, cat, k);
         b.rstd2 = F32(Tm, cat, k);
+        if (is_dec(cell_lo[k] + i)) {
+          b.cx = LP(Tm * d, cat, k);
+          b.qkv2 = LP(Tm * 3 * da, cat, k);
+          b.o2 = LP(Tm * da, cat, k);
+          b.x1c = F32(Tm * d, cat, k);
+          b.lse2 = F32(Tm * A, cat, k);
+          b.meanx = F32(Tm, cat, k);
+          b.rstdx = F32(Tm, cat, k);
+        }
       }
       if (k == K - 1) {
         W_.meanf = F32(Tm, GPIPE_CAT_HEAD, k);
@@ -223,6 +274,10 @@ int Engine::build_plan(bool dry, std::string &err) {
       s.colsum_scratch = F32(rows * cols, cat, k);
     }
     s.splitk_ws = splitk_ws_bytes ? RAW(splitk_ws_bytes, cat, k, k) : nullptr;
+    if (encdec() && k == kt) {
+      s.daux = F32(Tm * d, cat, k);
+      if (k == 0) s.dtgt = F32(Tm * d, cat, k);
+    }
   }
   for (int k = 0; k < (multi() ? K : 1); ++k)
     if (!dry && ar(k).used > ar(k).cap) {
@@ -275,11 +330,28 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
   const int32_t *tok = tok_dev + (int64_t)m * T_mb;
   const int32_t *lab = lab_dev + (int64_t)m * T_mb;
   float *x;
+  // encoder-decoder: second member of the pair this cell works on - the target embedding (fp32) while the cell is
+  // still in the encoder, the memory (lp) once it is in the decoder
+  float *aux_x = nullptr;
+  const void *mem = nullptr;
   if (k == 0) {
     GP_TRY(timed(k, KC_EMBED, 0, (double)T_mb * d * (lpb + 8), [&] { return embed_fwd(c, dt, tok, W(i_emb), pe, w.x_emb, T_mb, S, d); }));
     x = w.x_emb;
+    if (encdec()) {
+      // cell 0 embeds both id sequences (one table, reading B3).  The target embedding is cell 0's second OUTPUT:
+      // written once, in the forward pass, into the buffer cells 1..kt read; a replay of cell 0 needs it only when
+      // cell 0 itself holds the transition (then it is interior and recomputed)
+      const int32_t *tgt = tgt_dev + (int64_t)m * T_mb;
+      aux_x = kt == 0 ? w.aux_emb : aux_tgt[m];
+      if (kt == 0 || !replay)
+        GP_TRY(timed(k, KC_EMBED, 0, (double)T_mb * d * (lpb + 8), [&] { return embed_fwd(c, dt, tgt, W(i_emb), pe, aux_x, T_mb, S, d); }));
+    }
   } else {
     x = slot[k][m];
+    if (encdec()) {
+      if (k <= kt) aux_x = aux_tgt[m];
+      else mem = aux_mem[m];
+    }
   }
   int nl = cell_hi[k] - cell_lo[k];
   for (int i = 0; i < nl; ++i) {
@@ -287,6 +359,14 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
     const LayerParams &q = lp[l];
     LayerBuf &b = w.layers[i];
     bool last = (i + 1 == nl);
+    if (encdec() && l == n_enc) {
+      // encoder -> decoder: memory = LN_e(x_src) (reading B2); the stream switches to the target embedding.  The
+      // forward pass writes the memory where the later cells read it; a replay (and a last cell) keeps it interior.
+      void *mdst = (!replay && kt < K - 1) ? aux_mem[m] : w.mem;
+      GP_TRY(tln(x, P(i_lne_g), P(i_lne_b), mdst, w.mean_e, w.rstd_e, nullptr, nullptr));
+      mem = mdst;
+      x = aux_x;
+    }
     // a = LN1(x); x1 <- x + b_o                                              (a5)
     GP_TRY(tln(x, P(q.ln1_g), P(q.ln1_b), b.a, b.mean1, b.rstd1, P(q.b_o), b.x1));
     // [q|k|v] = a W_qkv + b_qkv                                              (a6)
@@ -304,15 +384,39 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
     g.A = b.o; g.lda = da; g.B = W(q.w_o); g.ldb = d; g.C = b.x1; g.ldc = d;
     g.flags = EPI_ACCUM | EPI_OUT_F32;
     GP_TRY(tgemm(KC_GEMM_FWD, g));
-    // where x2 = x1 + h W_2 + b_2 goes                                        (a11, a12)
+    float *xa = b.x1;                                // the stream after the attention block(s)
+    if (is_dec(l)) {
+      // cross-attention (reading B1): cx = LN_x(x1); x1c <- x1 + b_o2; queries from cx, keys / values from the
+      // memory, written side by side as [q2 | k2 | v2] so that the self-attention kernels run it unchanged
+      GP_TRY(tln(b.x1, P(q.lnx_g), P(q.lnx_b), b.cx, b.meanx, b.rstdx, P(q.b_o2), b.x1c));
+      g = GemmArgs{};
+      g.M = (int)T_mb; g.N = da; g.K = d;
+      g.A = b.cx; g.lda = d; g.B = W(q.w_q); g.ldb = da; g.C = b.qkv2; g.ldc = 3 * da;
+      g.bias = P(q.b_q); g.flags = EPI_BIAS;
+      GP_TRY(tgemm(KC_GEMM_FWD, g));
+      g = GemmArgs{};
+      g.M = (int)T_mb; g.N = 2 * da; g.K = d;
+      g.A = mem; g.lda = d; g.B = W(q.w_kv); g.ldb = 2 * da; g.C = (char *)b.qkv2 + (size_t)da * lp_size(dt); g.ldc = 3 * da;
+      g.bias = P(q.b_kv); g.flags = EPI_BIAS;
+      GP_TRY(tgemm(KC_GEMM_FWD, g));
+      GP_TRY(timed(k, KC_ATTN_FWD, 4.0 * Td * S * da, Td * 4.0 * da * lpb,
+                   [&] { return attn_fwd(c, dt, b.qkv2, b.o2, b.lse2, (int)nb, S, A, dh, 0); }));
+      g = GemmArgs{};
+      g.M = (int)T_mb; g.N = d; g.K = da;
+      g.A = b.o2; g.lda = da; g.B = W(q.w_o2); g.ldb = d; g.C = b.x1c; g.ldc = d;
+      g.flags = EPI_ACCUM | EPI_OUT_F32;
+      GP_TRY(tgemm(KC_GEMM_FWD, g));
+      xa = b.x1c;
+    }
+    // where x2 = xa + h W_2 + b_2 goes                                        (a11, a12)
     float *x2;
     if (!last) x2 = b.x2;
     else if (k == K - 1) x2 = w.x_out;
     else if (!replay) x2 = boundary_staged ? w.x_out : slot[k + 1][m];   // boundary stash (a12)
     else if (replay_full) x2 = w.x_out;               // replay output nobody reads
     else x2 = nullptr;                                // skipped: B_k does not need F_k's output
-    // c = LN2(x1); x2 <- x1 + b_2                                            (a9)
-    GP_TRY(tln(b.x1, P(q.ln2_g), P(q.ln2_b), b.c, b.mean2, b.rstd2, x2 ? P(q.b_2) : nullptr, x2));
+    // c = LN2(xa); x2 <- xa + b_2                                            (a9)
+    GP_TRY(tln(xa, P(q.ln2_g), P(q.ln2_b), b.c, b.mean2, b.rstd2, x2 ? P(q.b_2) : nullptr, x2));
     // h = relu(c W_1 + b_1)                                                  (a10)
     g = GemmArgs{};
     g.M = (int)T_mb; g.N = H; g.K = d;
@@ -344,7 +448,7 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
     g.flags = 0;
     GP_TRY(tgemm(KC_GEMM_FWD, g));
     GP_TRY(timed(k, KC_CE, 0, Td * V * 2.0 * lpb,
-                 [&] { return softmax_ce(c, dt, w.logits, lab, w.rowloss, T_mb, V, 1.f / (float)T_total); }));
+                 [&] { return softmax_ce(c, dt, w.logits, lab, w.rowloss, T_mb, V, 1.f / (float)T_total, logit_clip); }));
     GP_TRY(loss_reduce(c, w.rowloss, replay ? loss_dummy : loss_parts + m, T_mb));
   }
   return cudaSuccess;
@@ -415,11 +519,25 @@ cudaError_t Engine::backward_cell(int k, int m) {
     // this cell does it itself
     if (multi() && nl > 0) GP_TRY(tcol(dxo, d, G(lp[cell_hi[k] - 1].b_2), d));
   }
+  // encoder-decoder: gradient of the second member of the pair.  In the decoder it is the gradient of the memory:
+  // every decoder layer's cross-attention adds dkv W_kv^T to it (fp32) - the first one of the cell on top of what the
+  // next cell handed down (nothing, in the last cell), the others in place.  In the encoder it is the gradient of the
+  // target embedding and only travels down to cell 0.
+  const float *daux_in = (encdec() && k + 1 < K) ? dbound_aux[m & 1][k + 1] : nullptr;
+  float *daux = nullptr;
+  bool daux_started = false;
+  if (encdec() && k >= kt) daux = k == kt ? s.daux : dbound_aux[m & 1][k];
+  const void *mem = nullptr;
+  if (encdec() && k >= kt) mem = k > kt ? (const void *)aux_mem[m] : (const void *)((remat || kt == K - 1) ? w.mem : aux_mem[m]);
   for (int i = nl - 1; i >= 0; --i) {
     int l = cell_lo[k] + i;
     const LayerParams &q = lp[l];
     LayerBuf &b = w.layers[i];
+    const bool dec = is_dec(l), trans = encdec() && l == n_enc;
+    // input of the layer: the previous layer's output, the cell's input - or, for the first decoder layer, the
+    // target embedding
     const float *x_in = i > 0 ? w.layers[i - 1].x2 : (k == 0 ? w.x_emb : slot[k][m]);
+    if (trans) x_in = kt == 0 ? w.aux_emb : aux_tgt[m];
     // FFN: dh = (dx W_2^T) * [h > 0] with db_1 += sum_t dh fused into the epilogue; dW_2 += h^T dx
     // (db_2 += sum_t dx was fused into the LayerNorm-backward kernel that produced dx)
     GP_TRY(dgrad(dxo, d, d, q.w_2, H, s.dh, b.hbits, G(q.b_1)));
@@ -427,13 +545,46 @@ cudaError_t Engine::backward_cell(int k, int m) {
     // dc = dh W_1^T; dW_1 += c^T dh
     GP_TRY(dgrad(s.dh, H, H, q.w_1, d, s.dc, nullptr));
     GP_TRY(wgrad(b.c, d, d, s.dh, H, H, q.w_1));
-    // LN2 backward; residual adds gradients: dx1 = dx + LN2'(dc)
-    // (db_o += sum_t dx1 is fused here: dx1 is the output gradient of the out-projection)
-    GP_TRY(tlnb(s.dc, b.x1, b.mean2, b.rstd2, P(q.ln2_g), dx, s.dx[cur],
-                dt == GP_BF16 ? s.dx_lp[cur] : nullptr, G(q.ln2_g), G(q.ln2_b), G(q.b_o)));
+    // LN2 backward; residual adds gradients: dxa = dx + LN2'(dc)
+    // (the bias gradient of the GEMM that produced xa is fused here: db_o, or db_o2 in a decoder layer)
+    GP_TRY(tlnb(s.dc, dec ? b.x1c : b.x1, b.mean2, b.rstd2, P(q.ln2_g), dx, s.dx[cur],
+                dt == GP_BF16 ? s.dx_lp[cur] : nullptr, G(q.ln2_g), G(q.ln2_b), G(dec ? q.b_o2 : q.b_o)));
     dx = s.dx[cur];
     dxo = s.dx_lp[cur];
     cur ^= 1;
+    if (dec) {
+      // cross-attention block: do2 = dx1c W_o2^T; dW_o2 += o2^T dx1c; attention backward over [q2 | k2 | v2]
+      const size_t kv_off = (size_t)da * lp_size(dt);
+      GP_TRY(dgrad(dxo, d, d, q.w_o2, da, s.d_o, nullptr));
+      GP_TRY(wgrad(b.o2, da, da, dxo, d, d, q.w_o2));
+      GP_TRY(timed(k, KC_ATTN_BWD, 10.0 * Td * S * da, Td * 8.0 * da * lpb,
+                   [&] { return attn_bwd(c, dt, b.qkv2, b.o2, s.d_o, b.lse2, s.dqkv, s.dvec, (int)nb, S, A, dh, 0); }));
+      // queries: dcx = dq2 W_q^T; dW_q += cx^T dq2; db_q += sum_t dq2
+      GP_TRY(dgrad(s.dqkv, 3 * da, da, q.w_q, d, s.dc, nullptr));
+      GP_TRY(wgrad(b.cx, d, d, s.dqkv, 3 * da, da, q.w_q));
+      GP_TRY(tcol(s.dqkv, 3 * da, G(q.b_q), da));
+      // keys / values: dmem += dkv W_kv^T (fp32); dW_kv += mem^T dkv; db_kv += sum_t dkv
+      {
+        GemmArgs g{};
+        g.M = (int)T_mb; g.N = d; g.K = 2 * da;
+        g.A = (const char *)s.dqkv + kv_off; g.lda = 3 * da; g.transA = 0; g.B = W(q.w_kv); g.ldb = 2 * da; g.transB = 1;
+        g.C = daux; g.ldc = d; g.flags = EPI_OUT_F32;
+        if (daux_started) g.flags |= EPI_ACCUM;
+        else if (daux_in) { g.flags |= EPI_RESID; g.resid = daux_in; }
+        g.ws = s.splitk_ws; g.ws_bytes = splitk_ws_bytes;
+        double by = ((double)g.M * g.K + (double)g.K * g.N) * lpb + (double)g.M * g.N * ((daux_started || daux_in) ? 8.0 : 4.0);
+        GP_TRY(timed(k, KC_GEMM_DGRAD, 2.0 * g.M * g.N * (double)g.K, by, [&] { return gemm(c, dt, g); }));
+        daux_started = true;
+      }
+      GP_TRY(wgrad(mem, d, d, (const char *)s.dqkv + kv_off, 3 * da, 2 * da, q.w_kv));
+      GP_TRY(tcol((const char *)s.dqkv + kv_off, 3 * da, G(q.b_kv), 2 * da));
+      // LN_x backward: dx1 = dx1c + LN_x'(dcx); db_o += sum_t dx1
+      GP_TRY(tlnb(s.dc, b.x1, b.meanx, b.rstdx, P(q.lnx_g), dx, s.dx[cur],
+                  dt == GP_BF16 ? s.dx_lp[cur] : nullptr, G(q.lnx_g), G(q.lnx_b), G(q.b_o)));
+      dx = s.dx[cur];
+      dxo = s.dx_lp[cur];
+      cur ^= 1;
+    }
     // attention block: do = dx1 W_o^T; dW_o += o^T dx1
     GP_TRY(dgrad(dxo, d, d, q.w_o, da, s.d_o, nullptr));
     GP_TRY(wgrad(b.o, da, da, dxo, d, d, q.w_o));
@@ -450,16 +601,36 @@ cudaError_t Engine::backward_cell(int k, int m) {
       out = dbound[m & 1][k];
       out_lp = dbound_lp[m & 1][k];
     }
-    // its output is the FFN2 output gradient of the layer below (possibly in the previous cell):
-    // db_2(l-1) += sum_t dx
-    GP_TRY(tlnb(s.dc, x_in, b.mean1, b.rstd1, P(q.ln1_g), dx, out, dt == GP_BF16 ? out_lp : nullptr,
-                G(q.ln1_g), G(q.ln1_b), l > 0 && !(multi() && i == 0) ? G(lp[l - 1].b_2) : nullptr));
+    if (trans) {
+      // the input of the first decoder layer is the target embedding: its gradient is the aux gradient this cell
+      // hands down (cell 0: kept for the embedding backward), and nobody's FFN2 output
+      float *dt_out = kt == 0 ? s.dtgt : dbound_aux[m & 1][kt];
+      GP_TRY(tlnb(s.dc, x_in, b.mean1, b.rstd1, P(q.ln1_g), dx, dt_out, nullptr, G(q.ln1_g), G(q.ln1_b), nullptr));
+      // back through memory = LN_e(x_src): dx_src = LN_e'(dmem) - the encoder's last FFN2 output gradient
+      const float *x_src = i > 0 ? w.layers[i - 1].x2 : slot[k][m];
+      GP_TRY(cast_to_lp(c, dt, daux, s.dc, T_mb * (int64_t)d));
+      GP_TRY(tlnb(s.dc, x_src, w.mean_e, w.rstd_e, P(i_lne_g), nullptr, out, dt == GP_BF16 ? out_lp : nullptr,
+                  G(i_lne_g), G(i_lne_b), G(lp[l - 1].b_2)));
+    } else {
+      // its output is the FFN2 output gradient of the layer below (possibly in the previous cell):
+      // db_2(l-1) += sum_t dx
+      GP_TRY(tlnb(s.dc, x_in, b.mean1, b.rstd1, P(q.ln1_g), dx, out, dt == GP_BF16 ? out_lp : nullptr,
+                  G(q.ln1_g), G(q.ln1_b), l > 0 && !(multi() && i == 0) ? G(lp[l - 1].b_2) : nullptr));
+    }
     dx = out;
     dxo = out_lp;
     cur ^= 1;
   }
   if (k == 0)                                                          // dE[tok] += dx0
     GP_TRY(timed(k, KC_EMBED, 0, Td * d * 12.0, [&] { return embed_bwd(c, tok, dx, G(i_emb), T_mb, d); }));
+  if (encdec() && k < kt) {
+    // an encoder cell passes the gradient of the target embedding on (cell 0: into the shared table, after the
+    // source tokens' rows: a fixed order, so the step stays bitwise reproducible)
+    if (k > 0) GP_TRY(cudaMemcpyAsync(dbound_aux[m & 1][k], daux_in, (size_t)T_mb * d * sizeof(float), cudaMemcpyDeviceToDevice, c.stream));
+    else GP_TRY(timed(k, KC_EMBED, 0, Td * d * 12.0, [&] { return embed_bwd(c, tgt_dev + (int64_t)m * T_mb, daux_in, G(i_emb), T_mb, d); }));
+  } else if (encdec() && k == 0) {                                     // cell 0 holds the transition
+    GP_TRY(timed(k, KC_EMBED, 0, Td * d * 12.0, [&] { return embed_bwd(c, tgt_dev + (int64_t)m * T_mb, s.dtgt, G(i_emb), T_mb, d); }));
+  }
   if (multi() && k > 0) {
     // backward boundary transfer: the gradient wrt this cell's input becomes the previous cell's output gradient
     GP_TRY(peer_copy(k - 1, dout[m & 1][k - 1], k, dbound[m & 1][k], (size_t)T_mb * d * sizeof(float), c.stream));

@@ -21,6 +21,8 @@ struct TensorInfo {
 
 struct LayerParams {  // indices into Engine::tensors
   int ln1_g, ln1_b, w_qkv, b_qkv, w_o, b_o, ln2_g, ln2_b, w_1, b_1, w_2, b_2;
+  // decoder layers of an encoder-decoder handle: the cross-attention block; -1 otherwise
+  int lnx_g = -1, lnx_b = -1, w_q = -1, b_q = -1, w_kv = -1, b_kv = -1, w_o2 = -1, b_o2 = -1;
 };
 
 // Interior activations of one layer that the backward pass needs.
@@ -29,6 +31,10 @@ struct LayerBuf {
   uint32_t *hbits;                       // [T_mb, H/32] bit-packed ReLU pattern [h > 0] (written by FFN1's epilogue)
   float *x1, *x2;                        // fp32 residual stream (x2 unused for the cell's last layer)
   float *lse, *mean1, *rstd1, *mean2, *rstd2;
+  // decoder layer: cx = LN_x(x1); qkv2 = [cx W_q + b_q | mem W_kv + b_kv] in the [q|k|v] layout of qkv, so the same
+  // attention kernels serve the cross-attention; o2 its output; x1c = x1 + o2 W_o2 + b_o2
+  void *cx = nullptr, *qkv2 = nullptr, *o2 = nullptr;
+  float *x1c = nullptr, *lse2 = nullptr, *meanx = nullptr, *rstdx = nullptr;
 };
 
 struct Workspace {                       // one per cell (remat) or per (cell, micro-batch)
@@ -37,6 +43,10 @@ struct Workspace {                       // one per cell (remat) or per (cell, m
   std::vector<LayerBuf> layers;
   float *meanf = nullptr, *rstdf = nullptr, *rowloss = nullptr;   // head (last cell)
   void *y = nullptr, *logits = nullptr;
+  // encoder-decoder: the cell that holds the first decoder layer turns the source stream into the memory
+  float *aux_emb = nullptr;              // cell 0 when it also holds the transition: the target embedding
+  void *mem = nullptr;                   // transition cell: LN_e(x_src) (lp), as replayed / when no later cell reads it
+  float *mean_e = nullptr, *rstd_e = nullptr;
 };
 
 struct BwdScratch {                      // one per cell
@@ -47,6 +57,8 @@ struct BwdScratch {                      // one per cell
   float *ln_partials;
   float *colsum_scratch;                 // [max(T_mb/128, colsum rows), max(H, 3*da, d)]
   void *splitk_ws;                       // split-K partials + counters of this cell's GEMMs (one stream -> one user at a time)
+  float *daux = nullptr;                 // encoder-decoder, transition cell: gradient of the memory (fp32, summed over the decoder layers)
+  float *dtgt = nullptr;                 // ... when that cell is cell 0: gradient of the target embedding
 };
 
 struct Arena {
@@ -76,6 +88,19 @@ struct Engine {
   int64_t n_seqs = 0, nb = 0, T_mb = 0, T_total = 0;   // nb = sequences per micro-batch
   int d = 0, H = 0, A = 0, dh = 0, da = 0, V = 0, S = 0;
   float eps = 1e-5f;
+  // encoder-decoder T(L,H,A): layers [0, n_enc) are encoder layers, [n_enc, L) decoder
+  // layers (causal self-attention + cross-attention over the encoder memory).  What crosses a cell boundary is the
+  // pair (x, aux): aux = target embedding up to the transition, the memory after it.  n_dec == 0: the plain stack.
+  int n_enc = 0, n_dec = 0;
+  float logit_clip = 0.f;                              // > 0: logits clamped to [-c, c] before the softmax
+  bool encdec() const { return n_dec > 0; }
+  bool is_dec(int l) const { return n_dec > 0 && l >= n_enc; }
+  int kt = 0;                                          // the cell that holds layer n_enc (the transition)
+  int i_lne_g = -1, i_lne_b = -1;
+  int32_t *tgt_dev = nullptr;                          // target ids (cell 0 embeds both id sequences)
+  std::vector<float *> aux_tgt;                        // [M]: target embedding, read by cells 1..kt   (kt > 0)
+  std::vector<void *> aux_mem;                         // [M]: memory (lp), read by cells kt+1..K-1    (kt < K-1)
+  std::vector<float *> dbound_aux[2];                  // [k]: gradient wrt the aux input of cell k (two-entry ring like dbound)
   int sm_count = 148;                                  // of the device the handle lives on (launch geometry)
   // The memory plan must not depend on the device (gpipe_plan_bytes is host-only): scratch whose size follows the
   // launch geometry is planned for this fixed SM-count bound and the launchers clamp to what was planned.

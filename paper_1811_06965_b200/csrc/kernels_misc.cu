@@ -8,6 +8,9 @@ namespace gp {
 // Fused softmax cross-entropy (reading A8): one block per token row.
 //   rowloss[t] = (log sum_v exp(z_v - max) + max - z_label) * inv_T
 //   z_v <- (exp(z_v - max)/sum - [v == label]) * inv_T            (in place: logits -> dlogits)
+// Logit clipping ("we clip the logit predictions (softmax pre-activations) whenever their magnitude
+// exceeds a certain value"; reading B5): with clip > 0 the softmax sees z = min(max(logit, -clip), clip) and the
+// gradient is zero wherever the clamp is active (|logit| > clip); clip == 0 turns it off.
 // The row is read once from HBM into registers (VPT vectors of 8 (bf16) / 4 (fp32) elements per
 // thread) when it fits, so HBM traffic is one read + one write of the row; longer rows fall
 // back to three passes over global memory (L2-resident row).
@@ -47,7 +50,8 @@ template <> struct VecIO<bf16> {
 template <typename T, int VPT>
 __global__ void __launch_bounds__(1024)
 softmax_ce_reg_kernel(T *__restrict__ logits, const int32_t *__restrict__ labels,
-                      float *__restrict__ rowloss, int V, float inv_T) {
+                      float *__restrict__ rowloss, int V, float inv_T, float clip) {
+  const float hi = clip > 0.f ? clip : INFINITY, lo = -hi;
   constexpr int W = VecIO<T>::W;
   __shared__ float red[33];
   int64_t row = blockIdx.x;
@@ -66,7 +70,8 @@ softmax_ce_reg_kernel(T *__restrict__ logits, const int32_t *__restrict__ labels
       for (int e = 0; e < W; ++e) mx = fmaxf(mx, v[e]);
     }
   }
-  mx = block_max(mx, red);
+  mx = fminf(block_max(mx, red), hi);    // max of the clamped row (the clamp is monotone; V >= 1 so mx >= lo after fmaxf below)
+  mx = fmaxf(mx, lo);
   float s = 0.f;
 #pragma unroll
   for (int i = 0; i < VPT; ++i) {
@@ -75,13 +80,14 @@ softmax_ce_reg_kernel(T *__restrict__ logits, const int32_t *__restrict__ labels
       float v[W];
       VecIO<T>::unpack(raw[i], v);
 #pragma unroll
-      for (int e = 0; e < W; ++e) s += expf(v[e] - mx);
+      for (int e = 0; e < W; ++e) s += expf(fminf(fmaxf(v[e], lo), hi) - mx);
     }
   }
   s = block_sum(s, red);
   int lab = labels[row];
   float inv = 1.f / s;
-  if (threadIdx.x == 0) rowloss[row] = (logf(s) + mx - to_f<T>(logits[row * (int64_t)V + lab])) * inv_T;
+  if (threadIdx.x == 0)
+    rowloss[row] = (logf(s) + mx - fminf(fmaxf(to_f<T>(logits[row * (int64_t)V + lab]), lo), hi)) * inv_T;
   __syncthreads();                       // z[lab] read before anyone overwrites it
 #pragma unroll
   for (int i = 0; i < VPT; ++i) {
@@ -91,9 +97,9 @@ softmax_ce_reg_kernel(T *__restrict__ logits, const int32_t *__restrict__ labels
       VecIO<T>::unpack(raw[i], v);
 #pragma unroll
       for (int e = 0; e < W; ++e) {
-        float p = expf(v[e] - mx) * inv;
+        float p = expf(fminf(fmaxf(v[e], lo), hi) - mx) * inv;
         if (j * W + e == lab) p -= 1.f;
-        v[e] = p * inv_T;
+        v[e] = (v[e] >= lo && v[e] <= hi) ? p * inv_T : 0.f;
       }
       z[j] = VecIO<T>::pack(v);
     }
@@ -103,50 +109,52 @@ softmax_ce_reg_kernel(T *__restrict__ logits, const int32_t *__restrict__ labels
 template <typename T>
 __global__ void __launch_bounds__(1024)
 softmax_ce_3pass_kernel(T *__restrict__ logits, const int32_t *__restrict__ labels,
-                        float *__restrict__ rowloss, int V, float inv_T) {
+                        float *__restrict__ rowloss, int V, float inv_T, float clip) {
+  const float hi = clip > 0.f ? clip : INFINITY, lo = -hi;
   __shared__ float red[33];
   int64_t row = blockIdx.x;
   T *z = logits + row * (int64_t)V;
   float mx = -INFINITY;
   for (int j = threadIdx.x; j < V; j += blockDim.x) mx = fmaxf(mx, to_f<T>(z[j]));
-  mx = block_max(mx, red);
+  mx = fmaxf(fminf(block_max(mx, red), hi), lo);
   float s = 0.f;
-  for (int j = threadIdx.x; j < V; j += blockDim.x) s += expf(to_f<T>(z[j]) - mx);
+  for (int j = threadIdx.x; j < V; j += blockDim.x) s += expf(fminf(fmaxf(to_f<T>(z[j]), lo), hi) - mx);
   s = block_sum(s, red);
   int lab = labels[row];
   float inv = 1.f / s;
-  if (threadIdx.x == 0) rowloss[row] = (logf(s) + mx - to_f<T>(z[lab])) * inv_T;
+  if (threadIdx.x == 0) rowloss[row] = (logf(s) + mx - fminf(fmaxf(to_f<T>(z[lab]), lo), hi)) * inv_T;
   __syncthreads();
   for (int j = threadIdx.x; j < V; j += blockDim.x) {
-    float p = expf(to_f<T>(z[j]) - mx) * inv;
+    const float zj = to_f<T>(z[j]);
+    float p = expf(fminf(fmaxf(zj, lo), hi) - mx) * inv;
     if (j == lab) p -= 1.f;
-    z[j] = from_f<T>(p * inv_T);
+    z[j] = from_f<T>((zj >= lo && zj <= hi) ? p * inv_T : 0.f);
   }
 }
 
 template <typename T>
 static cudaError_t softmax_ce_t(const Ctx &c, T *logits, const int32_t *labels, float *rowloss,
-                                int64_t n_tok, int V, float inv_T) {
+                                int64_t n_tok, int V, float inv_T, float clip) {
   if (n_tok == 0) return cudaSuccess;
   constexpr int W = VecIO<T>::W;
   unsigned grid = (unsigned)n_tok;
   int nvec = V / W;
   bool vec_ok = (V % W == 0);
   if (vec_ok && nvec <= 256)
-    softmax_ce_reg_kernel<T, 1><<<grid, 256, 0, c.stream>>>(logits, labels, rowloss, V, inv_T);
+    softmax_ce_reg_kernel<T, 1><<<grid, 256, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
   else if (vec_ok && nvec <= 1024 * 4)
-    softmax_ce_reg_kernel<T, 4><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T);
+    softmax_ce_reg_kernel<T, 4><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
   else if (vec_ok && nvec <= 1024 * 8)
-    softmax_ce_reg_kernel<T, 8><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T);
+    softmax_ce_reg_kernel<T, 8><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
   else
-    softmax_ce_3pass_kernel<T><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T);
+    softmax_ce_3pass_kernel<T><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
   GP_LAUNCH_CHECK(c);
 }
 
 cudaError_t softmax_ce(const Ctx &c, int dt, void *logits, const int32_t *labels, float *rowloss,
-                       int64_t n_tok, int V, float inv_T) {
-  return dt == GP_BF16 ? softmax_ce_t<bf16>(c, (bf16 *)logits, labels, rowloss, n_tok, V, inv_T)
-                       : softmax_ce_t<float>(c, (float *)logits, labels, rowloss, n_tok, V, inv_T);
+                       int64_t n_tok, int V, float inv_T, float clip) {
+  return dt == GP_BF16 ? softmax_ce_t<bf16>(c, (bf16 *)logits, labels, rowloss, n_tok, V, inv_T, clip)
+                       : softmax_ce_t<float>(c, (float *)logits, labels, rowloss, n_tok, V, inv_T, clip);
 }
 
 // single block, fixed order: loss = sum_t rowloss[t]

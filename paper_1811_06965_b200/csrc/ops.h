@@ -108,8 +108,10 @@ const char *watchdog_describe();
 // ---- softmax cross-entropy ----------------------------------------------------------------------
 // In place: logits lp [n_tok, V] -> dlogits = (softmax - onehot) * inv_T; rowloss[t] =
 // (logsumexp - logit[label]) * inv_T.  Then loss_reduce sums rowloss into *loss (fp32, overwritten).
+// clip > 0: the softmax sees the logits clamped to [-clip, clip] and dlogits is 0 where the clamp is active
+// (reading B5); clip == 0: off.
 cudaError_t softmax_ce(const Ctx &c, int dt, void *logits, const int32_t *labels, float *rowloss,
-                       int64_t n_tok, int V, float inv_T);
+                       int64_t n_tok, int V, float inv_T, float clip = 0.f);
 cudaError_t loss_reduce(const Ctx &c, const float *rowloss, float *loss, int64_t n_tok);
 
 // ---- parameters ---------------------------------------------------------------------------------

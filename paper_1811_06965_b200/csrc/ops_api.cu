@@ -195,8 +195,9 @@ int gpipe_op_attn_bwd(void *stream, int dtype, const void *qkv, const void *o, c
              "gpipe_op_attn_bwd");
 }
 int gpipe_op_softmax_ce(void *stream, int dtype, void *logits, const int32_t *labels, float *rowloss,
-                        int64_t n_tok, int V, float inv_T) {
-  return ret(softmax_ce(mk(stream), dtype, logits, labels, rowloss, n_tok, V, inv_T), "gpipe_op_softmax_ce");
+                        int64_t n_tok, int V, float inv_T, float clip) {
+  if (!(clip >= 0.f)) return ret(cudaErrorInvalidValue, "gpipe_op_softmax_ce: clip must be >= 0");
+  return ret(softmax_ce(mk(stream), dtype, logits, labels, rowloss, n_tok, V, inv_T, clip), "gpipe_op_softmax_ce");
 }
 int64_t gpipe_op_colsum_scratch_floats(int64_t n_tok, int n) {
   int64_t r = colsum_scratch_rows(n_tok), t = (n_tok + 127) / 128;

@@ -96,9 +96,9 @@ def attn_bwd(qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal, backend=0):
                                        n_seq, S, A, dh, int(causal), backend))
 
 
-def softmax_ce(logits, labels, rowloss, inv_T):
+def softmax_ce(logits, labels, rowloss, inv_T, clip=0.0):
     n, V = logits.shape
-    B._check(B.lib().gpipe_op_softmax_ce(_stream(), _dt(logits), _p(logits), _p(labels), _p(rowloss), n, V, inv_T))
+    B._check(B.lib().gpipe_op_softmax_ce(_stream(), _dt(logits), _p(logits), _p(labels), _p(rowloss), n, V, inv_T, clip))
 
 
 def colsum(dy, out):

@@ -109,3 +109,29 @@ def test_product_does_not_import_oracle():
         if fn.endswith(".py"):
             assert "paper_1811_06965_b200" not in open(os.path.join(ROOT, "oracle", fn)).read().replace(
                 "CUDA path (paper_1811_06965_b200/)", "")
+
+
+def test_encdec_planner_and_argument_checks():
+    """gpipe_plan_bytes_encdec (host only): the 6.04 B T(64,16384,32) of PAPER.md:158 fits one 180 GB B200 with
+    remat, K = M = 16; the activation law of PAPER.md:87 holds for the pair boundary too; bad arguments are refused."""
+    from paper_1811_06965_b200.binding import EncDecSpec, plan_bytes_encdec
+    s6 = EncDecSpec(64, 64, 1024, 16384, 32, 64, 64000, 256, 1, 1e-5, 0.0)
+    need = plan_bytes_encdec(s6, 16, 16, True, 128)
+    n_param = 6.04e9
+    assert 10 * n_param < need < 180e9                      # 10 B / parameter (bf16 copy + fp32 master + fp32 grad) + activations
+    r = {M: plan_bytes_encdec(s6, 16, M, True, 128) for M in (1, 4, 16)}
+    assert r[1] > r[4] > r[16]
+    assert plan_bytes_encdec(s6, 16, 16, False, 128) > 1.5 * need
+    # explicit boundaries over the 128 layers: same parameters, so nearly the same bytes
+    lo = [0] + [8 * k + 4 for k in range(1, 16)] + [128]
+    assert abs(plan_bytes_encdec(s6, 16, 16, True, 128, lo) - need) < 0.05 * need
+    tiny = EncDecSpec(2, 2, 64, 256, 4, 16, 512, 16, 0, 1e-5, 0.0)
+    assert plan_bytes_encdec(tiny, 4, 4, True, 8) > 0
+    for bad in (dict(K=5), dict(M=3), dict(lo=[0, 2, 2, 4], K=3)):
+        with pytest.raises(gp.GPipeError):
+            plan_bytes_encdec(tiny, bad.get("K", 2), bad.get("M", 4), True, 8, bad.get("lo"))
+    for spec in (EncDecSpec(0, 2, 64, 256, 4, 16, 512, 16, 0, 1e-5, 0.0),
+                 EncDecSpec(2, 0, 64, 256, 4, 16, 512, 16, 0, 1e-5, 0.0),
+                 EncDecSpec(2, 2, 64, 256, 4, 16, 512, 16, 0, 1e-5, -0.5)):
+        with pytest.raises(gp.GPipeError):
+            plan_bytes_encdec(spec, 2, 4, True, 8)

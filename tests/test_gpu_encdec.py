@@ -1,0 +1,189 @@
+"""GPU parity of the encoder-decoder Transformer T(L,H,A) on the GPipe schedule (PAPER.md:160,
+:174) against oracle/encdec_oracle.py, through the C ABI (gpipe_create_encdec / gpipe_step_encdec).
+
+  * fp32 (TF32 off): loss and every per-tensor max-relative gradient error <= 1e-4 against the fp64 oracle, for
+    partitions that put the encoder -> decoder transition at the start of a cell, in the middle of one, in cell 0
+    and in the last cell; remat on and off; with and without logit clipping (clip chosen so that the clamp is active
+    on a measurable share of the logits);
+  * bf16: loss within 1e-2 relative and per-tensor cosine >= 0.999, or >= floor - 5e-4 where the oracle's own
+    bf16-rounded run (round_operands=True) is below 0.999 (reading A14), on a small model and on a reduction of
+    T(L,16384,32) at the paper's widths (d 1024, H 16384, 32 heads of 64, V 64000, S 256);
+  * GPU-side invariants the paper fixes: replayed == stored bitwise, gradients independent of the
+    partition, one step bitwise reproducible, the CUDA graph replays the eager step bit for bit.
+"""
+import numpy as np
+import pytest
+
+import gpipe_inputs as gi
+import paper_1811_06965_b200 as gp
+from oracle import encdec_oracle as eo
+from tests.util import cosine, maxrel
+
+pytestmark = pytest.mark.gpu
+
+
+def _spec(w):
+    return eo.EncDecSpec(w.n_enc, w.n_dec, w.d_model, w.d_ffn, w.n_heads, w.d_head, w.vocab, w.seq_len, w.ln_eps,
+                         w.logit_clip)
+
+
+def _tiny(n_enc=2, n_dec=2, **kw):
+    w = gi.encdec("tiny-encdec", 1, 256, 4, vocab=512, n_seqs=8, M=4, K=2, d_model=64, d_head=16, seq_len=16,
+                  dtype="fp32")
+    L = n_enc + n_dec
+    return w.replace(n_layers=L, n_dec=n_dec, causal=(0,) * n_enc + (1,) * n_dec, **kw)
+
+
+def _oracle(w, params, ids, K=None, M=None, remat=None, cell_lo=None, dtype=np.float64, round_operands=False):
+    o = eo.GPipeEncDecOracle(_spec(w), w.K if K is None else K, w.M if M is None else M,
+                             w.remat if remat is None else remat, dtype=dtype, round_operands=round_operands,
+                             cell_lo=cell_lo)
+    o.set_params(params)
+    return o, o.step(*ids)
+
+
+def _gpu(w, params, ids, K=None, M=None, remat=None, partition=None, steps=1, graph=True):
+    kw = {}
+    if K is not None:
+        kw["K"] = K
+    if M is not None:
+        kw["M"] = M
+    if remat is not None:
+        kw["remat"] = remat
+    with gp.from_workload(w, partition=partition, **kw) as e:
+        assert e.names == [n for n, _ in gi.tensor_shapes(w)]
+        e.cuda_graph(graph)
+        e.set_params(params)
+        losses = []
+        for s in range(steps):
+            if s:
+                e.zero_grads()
+            losses.append(e.step(*ids))
+        return losses, e.grads(), e.launch_count(), e.peak_bytes()
+
+
+# K, boundaries over the 4 layers (enc0 enc1 | dec0 dec1 -> transition at layer 2), remat
+PARTITIONS = [
+    (1, None, True),               # everything in one cell: transition in cell 0 == last cell
+    (2, None, True),               # [0,2) [2,4): transition at the start of cell 1
+    (2, None, False),
+    (2, [0, 1, 4], True),          # transition in the middle of the last cell
+    (2, [0, 3, 4], True),          # transition in the middle of cell 0
+    (3, [0, 1, 3, 4], True),       # transition in the middle of cell 1, decoder cell after it
+    (4, None, True),               # one layer per cell
+    (4, None, False),
+]
+
+
+@pytest.mark.parametrize("K,cell_lo,remat", PARTITIONS)
+@pytest.mark.parametrize("clip", [0.0, 0.2])
+def test_tiny_fp32_matches_oracle(K, cell_lo, remat, clip):
+    w = _tiny(logit_clip=clip)
+    params = gi.make_params(w, 1101, round_bf16=False)
+    ids = gi.make_tokens_encdec(w, 2101)
+    o, loss_ref = _oracle(w, params, ids, K=K, remat=remat, cell_lo=cell_lo)
+    (loss,), grads, launches, _ = _gpu(w, params, ids, K=K, remat=remat, partition=cell_lo)
+    assert launches > 0
+    assert abs(loss - loss_ref) <= 1e-4 * abs(loss_ref), (loss, loss_ref)
+    worst = max((maxrel(grads[n], o.g[n]), n) for n in grads)
+    assert worst[0] <= 1e-4, worst
+    if clip:
+        # the clamp has to be doing something in this case, or the test proves nothing about it
+        o2, loss2 = _oracle(w.replace(logit_clip=0.0), params, ids, K=K, remat=remat, cell_lo=cell_lo)
+        assert abs(loss2 - loss_ref) > 1e-5 * abs(loss_ref)
+        assert maxrel(o2.g["w_out"], o.g["w_out"]) > 1e-3
+
+
+def test_uneven_depths_and_micro_batches():
+    """1 encoder + 3 decoder layers, and 3 + 1, K = 3 and M = 2 / 8 (one sequence per micro-batch)."""
+    for n_enc, n_dec, M in ((1, 3, 2), (3, 1, 8)):
+        w = _tiny(n_enc, n_dec, K=3, M=M)
+        params = gi.make_params(w, 1102, round_bf16=False)
+        ids = gi.make_tokens_encdec(w, 2102)
+        o, loss_ref = _oracle(w, params, ids)
+        (loss,), grads, _, _ = _gpu(w, params, ids)
+        assert abs(loss - loss_ref) <= 1e-4 * abs(loss_ref)
+        worst = max((maxrel(grads[n], o.g[n]), n) for n in grads)
+        assert worst[0] <= 1e-4, worst
+
+
+def test_gpu_invariants_remat_partition_determinism_graph():
+    w = _tiny(logit_clip=0.2)
+    params = gi.make_params(w, 1103, round_bf16=False)
+    ids = gi.make_tokens_encdec(w, 2103)
+    (l_r, l_r2), g_r, n_r, peak_r = _gpu(w, params, ids, K=2, remat=True, steps=2)      # step 2 replays the graph
+    (l_s,), g_s, n_s, peak_s = _gpu(w, params, ids, K=2, remat=False)
+    (l_e, l_e2), g_e, _, _ = _gpu(w, params, ids, K=2, remat=True, steps=2, graph=False)
+    assert l_r == l_s == l_e == l_r2 == l_e2
+    assert n_r > n_s and peak_s["by_category"]["interior"] > peak_r["by_category"]["interior"]
+    for n in g_r:
+        assert np.array_equal(g_r[n], g_s[n]), n          # replayed == stored, bitwise
+        assert np.array_equal(g_r[n], g_e[n]), n          # graph replay == eager enqueue, bitwise
+    # another partition: same gradients up to fp32 summation order of nothing (the kernels' K loops do not depend
+    # on the cut), except the embedding / bias column sums, whose order is fixed too -> bitwise
+    (l_p,), g_p, _, _ = _gpu(w, params, ids, K=3, partition=[0, 1, 3, 4])
+    assert l_p == l_r
+    for n in g_r:
+        assert np.array_equal(g_r[n], g_p[n]), n
+
+
+def test_wrong_entry_points_are_rejected():
+    w = _tiny()
+    ids = gi.make_tokens_encdec(w, 2104)
+    with gp.from_workload(w) as e:
+        with pytest.raises(gp.GPipeError):
+            gp.GPipe.step(e, ids[0], ids[2])              # gpipe_step on an encoder-decoder handle
+    with gp.from_workload(gi.CONFIGS["tiny"]) as e:
+        rc = gp.lib().gpipe_step_encdec(e._h, ids[0].ctypes.data, ids[1].ctypes.data, ids[2].ctypes.data, None)
+        assert rc == -1
+    with pytest.raises(gp.GPipeError):
+        gp.from_workload(_tiny(), K=5)                    # K > n_enc + n_dec
+    with pytest.raises(gp.GPipeError):
+        gp.from_workload(_tiny(logit_clip=-1.0))
+
+
+def _bf16_case(w, seed_p, seed_t, oracle_dtype, tag, clip_precondition=False):
+    params = gi.make_params(w, seed_p)                    # bf16-representable (A12)
+    ids = gi.make_tokens_encdec(w, seed_t)
+    o, loss_ref = _oracle(w, params, ids, dtype=oracle_dtype)
+    of, _ = _oracle(w, params, ids, dtype=oracle_dtype, round_operands=True)     # the bf16 floor (A14)
+    (loss, loss2), grads, _, peak = _gpu(w, params, ids, steps=2)
+    assert loss == loss2
+    rel = abs(loss - loss_ref) / abs(loss_ref)
+    cos = {n: cosine(grads[n], o.g[n]) for n in grads}
+    floor = {n: cosine(of.g[n], o.g[n]) for n in grads}
+    classes = {}
+    for n in cos:
+        classes.setdefault(n.split(".")[-1], []).append(n)
+    print()
+    print("PARITY|%s|n_enc %d n_dec %d K %d M %d N %d|loss gpu %.6f oracle %.6f rel %.2e|peak %.2f GB"
+          % (tag, w.n_enc, w.n_dec, w.K, w.M, w.n_seqs, loss, loss_ref, rel, peak["total"] / 1e9))
+    for cls, names in classes.items():
+        print("PARITY|%s|%-6s|n %3d|cos min %.6f|floor min %.6f|max-rel max %.2e"
+              % (tag, cls, len(names), min(cos[n] for n in names), min(floor[n] for n in names),
+                 max(maxrel(grads[n], o.g[n]) for n in names)))
+    if clip_precondition:
+        # The clamp is a discontinuity: a LABEL logit within one bf16 rounding of +-c would flip its whole (p - 1)/T
+        # term on or off and swamp the comparison (seen with other seeds: floor(w_out) 0.9984).  These seeds have
+        # none - the oracle's own rounded run says so - which is what makes the cosine bound meaningful here; the
+        # clamp pattern itself is compared exactly, on identical stored logits, in
+        # tests/test_gpu_ops.py::test_softmax_ce_with_logit_clipping.
+        assert floor["w_out"] >= 0.9999, floor["w_out"]
+    assert rel <= 1e-2
+    for n, c in cos.items():
+        assert c >= min(0.999, floor[n] - 5e-4), (n, c, floor[n])
+
+
+def test_small_bf16_matches_oracle():
+    w = gi.encdec("small-encdec", 2, 1024, 4, vocab=2048, n_seqs=8, M=4, K=2, d_model=256, d_head=64, seq_len=64,
+                  logit_clip=0.3)
+    _bf16_case(w, 1105, 2105, np.float64, "encdec-small-bf16", clip_precondition=True)
+    _bf16_case(w.replace(K=4, logit_clip=0.0), 1106, 2106, np.float64, "encdec-small-bf16-K4")
+
+
+def test_reduced_T_L_16384_32_matches_oracle():
+    """The paper's widths (d 1024, H 16384, A 32; 64k vocabulary, S 256) with 2 + 2 layers, K = 4
+    cells, M = 4 micro-batches of one sequence: cross-attention at S = 256 (two query blocks, 256 keys), the
+    [T, 3 d_a] side-by-side q2 | k2 | v2 layout at d_a = 2048, the fp32 memory-gradient accumulation across cells."""
+    w = gi.encdec("T(2,16384,32)-reduced", 2, 16384, 32, vocab=64000, n_seqs=4, M=4, K=4, logit_clip=0.0)
+    _bf16_case(w, 1107, 2107, np.float32, "encdec-T(L,16384,32)-reduced")

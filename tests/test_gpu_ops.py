@@ -459,6 +459,36 @@ def test_softmax_ce(dtype, n, V):
 
 
 @pytest.mark.parametrize("dtype", ["fp32", "bf16"])
+@pytest.mark.parametrize("n,V", [(9, 512), (5, 32000), (4, 64000), (3, 1000)])
+def test_softmax_ce_with_logit_clipping(dtype, n, V):
+    """PAPER.md:174 / reading B5: the softmax sees clamp(z, -c, c); dlogits is 0 where the clamp is active.  Both
+    sides clamp the SAME stored logits (bf16-representable inputs), so the clamp pattern must agree exactly; a
+    label whose logit is clipped makes the case bite (its -1/T would otherwise dominate the row)."""
+    from oracle import encdec_oracle as eo
+    r = _rng(3 * V + n)
+    zt, zq = _lp(r.standard_normal((n, V)) * 3, dtype)
+    labels = r.integers(0, V, size=n).astype(np.int32)
+    clip = 2.5
+    labels[0] = int(np.argmax(zq[0]))                       # a clipped label logit (max of ~N(0,3) draws > 2.5)
+    assert zq[0, labels[0]] > clip and (np.abs(zq) > clip).mean() > 0.2
+    rowloss = torch.empty(n, device=DEV)
+    loss_ref, dl_ref, per_tok = eo.softmax_ce_clipped(zq.astype(np.float64), labels, 77, clip)
+    ops.softmax_ce(zt, torch.tensor(labels, device=DEV), rowloss, 1.0 / 77, clip)
+    got = _np(zt)
+    assert np.array_equal(got == 0, dl_ref == 0)            # the clamp pattern, bit for bit
+    assert np.allclose(_np(rowloss), per_tok / 77, rtol=2e-5, atol=0)
+    tol, cos = _tol(dtype)
+    assert maxrel(got, dl_ref) <= tol
+    assert cosine(got, dl_ref) >= cos
+    # clip = 0 is "off": identical to the unclipped kernel
+    z0, _ = _lp(zq, dtype)
+    z1, _ = _lp(zq, dtype)
+    ops.softmax_ce(z0, torch.tensor(labels, device=DEV), rowloss, 1.0 / 77)
+    ops.softmax_ce(z1, torch.tensor(labels, device=DEV), rowloss, 1.0 / 77, 0.0)
+    assert torch.equal(z0, z1)
+
+
+@pytest.mark.parametrize("dtype", ["fp32", "bf16"])
 def test_colsum_embedding_sgd(dtype):
     r = _rng(11)
     dyt, dyq = _lp(r.standard_normal((300, 200)), dtype)

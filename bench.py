@@ -44,15 +44,22 @@ def flops_per_step(w, replay_skips_last_ffn2=True):
     d, H, da, V, S = w.d_model, w.d_ffn, w.d_attn, w.vocab, w.seq_len
     T = w.tokens_per_step
     f_qkv, f_o, f_1, f_2 = 2 * d * 3 * da, 2 * da * d, 2 * d * H, 2 * H * d
-    f_g = f_qkv + f_o + f_1 + f_2
     f_v = 2 * d * V
-    fa = [4 * S * da * ((S + 1) / (2 * S) if c else 1.0) for c in w.causal]
-    fwd = sum(f_g + a for a in fa) + f_v
-    bwd = sum(2 * f_g + 2.5 * a for a in fa) + 2 * f_v
+    n_dec = getattr(w, "n_dec", 0)
+    # per layer and token: GEMM FLOPs f_g[l], attention FLOPs f_a[l] (causal: the unmasked half).  A decoder layer of
+    # the encoder-decoder model adds the cross-attention block: q (d x da), k|v (d x 2 da) and
+    # output (da x d) projections and one unmasked attention over the S memory positions.
+    f_g, f_a = [], []
+    for l, c in enumerate(w.causal):
+        dec = n_dec > 0 and l >= w.n_layers - n_dec
+        f_g.append(f_qkv + f_o + f_1 + f_2 + (2 * d * da + 2 * d * 2 * da + 2 * da * d if dec else 0))
+        f_a.append(4 * S * da * ((S + 1) / (2 * S) if c else 1.0) + (4 * S * da if dec else 0))
+    fwd = sum(f_g) + sum(f_a) + f_v
+    bwd = 2 * sum(f_g) + 2.5 * sum(f_a) + 2 * f_v
     model = (fwd + bwd) * T
     replay = 0.0
     if w.remat:
-        replay = sum(f_g + a for a in fa) + f_v          # the head is replayed with its cell
+        replay = fwd                                      # the head is replayed with its cell
         if replay_skips_last_ffn2:
             replay -= (w.K - 1) * f_2                     # cells 0..K-2 skip their last FFN2 in replay
         replay *= T
@@ -182,6 +189,43 @@ def oracle_sample(w, repeats=2):
             "seconds": t_head + t_some}
 
 
+def oracle_sample_encdec(w, repeats=2):
+    """The bounded oracle sample for the encoder-decoder model (oracle/encdec_oracle.py as it stands): ONE source /
+    target sequence pair through the (1 + 1)-layer and the (2 + 2)-layer model of the same widths; the cost of one
+    encoder + decoder layer pair and the cost of embedding + head are separated and extrapolated linearly."""
+    from oracle import encdec_oracle as eo
+    try:
+        from threadpoolctl import threadpool_info
+        cores = max([i.get("num_threads", 1) for i in threadpool_info()] + [1])
+    except Exception:
+        cores = os.cpu_count() or 1
+
+    def run(L):
+        ww = w.replace(n_layers=2 * L, n_dec=L, causal=(0,) * L + (1,) * L, n_seqs=1, M=1, K=2)
+        params = gi.make_params(ww, 1, parity=False, round_bf16=False)
+        ids = gi.make_tokens_encdec(ww, 2)
+        o = eo.GPipeEncDecOracle(eo.EncDecSpec(L, L, ww.d_model, ww.d_ffn, ww.n_heads, ww.d_head, ww.vocab, ww.seq_len,
+                                               ww.ln_eps, ww.logit_clip), 2, 1, ww.remat, dtype=np.float32)
+        o.set_params(params)
+        o.step(*ids)
+        best = 1e30
+        for _ in range(repeats):
+            t0 = time.perf_counter()
+            o.step(*ids)
+            best = min(best, time.perf_counter() - t0)
+        return best
+
+    t1, t2 = run(1), run(2)
+    t_pair = max(t2 - t1, 0.0)
+    t_head = max(t1 - t_pair, 0.0)
+    t_seq = t_head + (w.n_dec) * t_pair
+    return {"value": w.seq_len / t_seq, "unit": UNIT, "cores": int(cores), "kind": "oracle",
+            "sample": "fp32 numpy encoder-decoder oracle step on 1 sequence pair of %d tokens: (1+1)-layer model %.3fs, "
+                      "(2+2)-layer model %.3fs; per-pair cost extrapolated linearly to %d+%d layers"
+                      % (w.seq_len, t1, t2, w.n_enc, w.n_dec),
+            "seconds": t1 + t2}
+
+
 def oracle_full(w):
     """One WHOLE oracle step of the full workload (all N sequences, all L layers, the K/M schedule with replay),
     fp32, timed once after a one-sequence warm-up of the BLAS pool.  Minutes for config 2; do not use on 4/5."""
@@ -214,7 +258,7 @@ def run_reference(args, w, rank, world):
     times = []
     res = None
     for i in range(args.warmup + args.steps):
-        res = oracle_full(w) if args.oracle_full else oracle_sample(w)
+        res = oracle_sample_encdec(w) if w.n_dec else (oracle_full(w) if args.oracle_full else oracle_sample(w))
         if i >= args.warmup:
             times.append(res["value"])
         if args.oracle_full:
@@ -253,14 +297,18 @@ def run_ours(args, w, rank, world, local_rank):
     free_before, _ = torch.cuda.mem_get_info(dev)
     torch.cuda.reset_peak_memory_stats(dev)
     pipe_devices = [int(x) for x in args.pipeline_devices.split(",")] if args.pipeline_devices else None
-    eng = gp.from_workload(w, device=dev, partition=None if args.partition == "equal" else args.partition,
-                           devices=pipe_devices, staged=bool(pipe_devices) and args.pipeline_staged)
-    eng.init_params(seed=1000 + rank, std=0.02, parity=False)
+    if w.n_dec:          # the encoder-decoder T(L,H,A): equal split, depth-scaled FFN init
+        eng = gp.from_workload(w, device=dev)
+        eng.init_params(seed=1000 + rank, std=0.02, parity=False, ffn_scale=1.0 / w.n_layers)
+        ids = gi.make_tokens_encdec(w, 2000 + rank)
+    else:
+        eng = gp.from_workload(w, device=dev, partition=None if args.partition == "equal" else args.partition,
+                               devices=pipe_devices, staged=bool(pipe_devices) and args.pipeline_staged)
+        eng.init_params(seed=1000 + rank, std=0.02, parity=False)
+        ids = gi.make_tokens(w, 2000 + rank)
     progress("engine ready (%.1f GB arena)" % (eng.peak_bytes()["total"] / 1e9))
-    tok, lab = gi.make_tokens(w, 2000 + rank)
-    tok_d, lab_d = torch.tensor(tok, device=dev), torch.tensor(lab, device=dev)
-    tok_h = torch.tensor(tok).pin_memory().numpy()
-    lab_h = torch.tensor(lab).pin_memory().numpy()
+    ids_d = [torch.tensor(a, device=dev) for a in ids]
+    ids_h = [torch.tensor(a).pin_memory().numpy() for a in ids]
     s0 = eng.streams[0]
 
     def timed(fn, steps):
@@ -277,26 +325,26 @@ def run_ours(args, w, rank, world, local_rank):
 
     loss = None
     for i in range(args.warmup):
-        loss = eng.step(tok_d, lab_d)
+        loss = eng.step(*ids_d)
         eng.zero_grads()
         progress("warm-up step %d done, loss %.4f" % (i, loss))
     sampler = ClockSampler(local_rank) if rank == 0 else None
     l0 = eng.launch_count()
-    ms = timed(lambda: eng.step(tok_d, lab_d), args.steps)
+    ms = timed(lambda: eng.step(*ids_d), args.steps)
     launches = (eng.launch_count() - l0)
     clocks = sampler.stop() if sampler else None
     progress("timed region done: %.1f ms/step" % (ms / args.steps))
-    ms_e2e = timed(lambda: eng.step(tok_h, lab_h), args.steps)
+    ms_e2e = timed(lambda: eng.step(*ids_h), args.steps)
     # two extra steps with per-launch CUDA events for the roofline of the dominant kernel class:
     # (1) "isolated": every cell on stream 0, each launch alone on the GPU (standalone durations);
     # (2) "in-step": the K-stream schedule as timed above, each launch bracketed on its own stream (durations
     #     then include the SMs it shares with the other cells' kernels)
     progress("e2e region done: %.1f ms/step; per-launch timing steps" % (ms_e2e / args.steps))
     eng.kernel_timing(True, serial=True)
-    eng.step(tok_d, lab_d)
+    eng.step(*ids_d)
     stats = eng.kernel_stats()
     eng.kernel_timing(True, serial=False)
-    eng.step(tok_d, lab_d)
+    eng.step(*ids_d)
     stats_conc = eng.kernel_stats()
     progress("per-launch timing steps done")
     eng.kernel_timing(False)
@@ -356,7 +404,8 @@ def run_ours(args, w, rank, world, local_rank):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "bf16" if w.dtype == "bf16" else "f32", "data": "synthetic",
-            "config": {"workload": w.name, "L": w.n_layers, "d_model": w.d_model, "d_ffn": w.d_ffn,
+            "config": {"workload": w.name, "L": w.n_layers, "n_enc": w.n_enc if w.n_dec else None, "n_dec": w.n_dec or None,
+                       "d_model": w.d_model, "d_ffn": w.d_ffn,
                        "n_heads": w.n_heads, "d_head": w.d_head, "vocab": w.vocab, "seq_len": w.seq_len,
                        "n_seqs": w.n_seqs, "K": w.K, "M": w.M, "remat": w.remat, "partition": args.partition,
                        "layers_per_cell": [hi - lo for lo, hi in eng.cells],
@@ -372,12 +421,12 @@ def run_ours(args, w, rank, world, local_rank):
             "peak_hbm_cross_check": hbm_check,
             "clocks": clocks, "roofline": roofline,
             "e2e": {"value": tokens * args.steps / (ms_e2e / 1e3), "unit": UNIT,
-                    "h2d_bytes_per_step": int(tok.nbytes + lab.nbytes), "d2h_bytes_per_step": 4 * w.M},
+                    "h2d_bytes_per_step": int(sum(a.nbytes for a in ids)), "d2h_bytes_per_step": 4 * w.M},
             "gpu_launches": int(launches)}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         progress("timing the CPU oracle sample")
-        line["cpu_baseline"] = {k: v for k, v in (oracle_full(w) if args.oracle_full else oracle_sample(w)).items()
-                                if k != "seconds"}
+        res = oracle_sample_encdec(w) if w.n_dec else (oracle_full(w) if args.oracle_full else oracle_sample(w))
+        line["cpu_baseline"] = {k: v for k, v in res.items() if k != "seconds"}
     eng.close()
     if rank == 0:
         print(json.dumps(line), flush=True)
@@ -389,7 +438,8 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=gi.CONFIG_ORDER)
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=gi.CONFIG_ORDER + list(gi.ENCDEC_CONFIGS),
+                    help="a BASELINE.json config, or the paper's own encoder-decoder T(64,16384,32) (PAPER.md:158-160)")
     ap.add_argument("--M", type=int, default=None)
     ap.add_argument("--K", type=int, default=None)
     ap.add_argument("--no-remat", action="store_true")
@@ -409,7 +459,7 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    w = gi.CONFIGS[args.workload]
+    w = gi.CONFIGS[args.workload] if args.workload in gi.CONFIGS else gi.ENCDEC_CONFIGS[args.workload]
     if args.M:
         w = w.replace(M=args.M)
     if args.K:

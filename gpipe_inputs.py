@@ -156,6 +156,13 @@ def encdec(name: str, L: int, H: int, A: int, vocab: int = 64000, n_seqs: int = 
                     (0,) * L + (1,) * L, remat, 1e-5, L, logit_clip)
 
 
+# The paper's own 6.04 B model: 64 encoder + 64 decoder layers, on the K = M = 16 schedule of
+# BASELINE.json configs[4].  Not one of BASELINE.json's configs: bench.py --workload selects it.
+ENCDEC_CONFIGS: Dict[str, Workload] = {
+    "T(64,16384,32)-encdec": encdec("T(64,16384,32)-encdec", 64, 16384, 32),
+}
+
+
 def make_params(w: Workload, seed: int, std: float = 0.02, parity: bool = True,
                 round_bf16: Optional[bool] = None, ffn_depth_scale: bool = False) -> Dict[str, np.ndarray]:
     """N(0, std) matrices; parity=True also randomises biases / beta and gamma = 1 + N(0,std);

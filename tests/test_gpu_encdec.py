@@ -187,3 +187,34 @@ def test_reduced_T_L_16384_32_matches_oracle():
     [T, 3 d_a] side-by-side q2 | k2 | v2 layout at d_a = 2048, the fp32 memory-gradient accumulation across cells."""
     w = gi.encdec("T(2,16384,32)-reduced", 2, 16384, 32, vocab=64000, n_seqs=4, M=4, K=4, logit_clip=0.0)
     _bf16_case(w, 1107, 2107, np.float32, "encdec-T(L,16384,32)-reduced")
+
+
+def test_full_size_T_64_16384_32_properties():
+    """The paper's 6.04 B model, K = M = 16, remat on, as bench.py --workload
+    'T(64,16384,32)-encdec' times it (device-side init with the depth-scaled FFN draw).  Properties that
+    hold at any size: (i) the tensor inventory counts 6.04 B parameters (pin P2) and the plan fits 180 GB; (ii) loss
+    at initialisation = ln V + sigma^2 d / 2 (pin P7: an untied N(0, sigma^2) head over a LayerNorm output); (iii) the
+    step is bitwise reproducible and ACCUMULATES (a second step doubles every sampled gradient); (iv) rows of dW_out
+    sum to ~0 over the vocabulary; (v) gradients of every block kind - encoder, decoder self-attention,
+    cross-attention, lne, both ends of the stack - are finite and non-zero."""
+    w = gi.ENCDEC_CONFIGS["T(64,16384,32)-encdec"]
+    ids = gi.make_tokens_encdec(w, 2108)
+    sample = ["l0.w_qkv", "l63.b_1", "lne_g", "l64.w_q", "l64.b_kv", "l100.w_kv", "l127.w_o2", "l127.lnx_b", "l127.b_2",
+              "lnf_g"]
+    with gp.from_workload(w) as e:
+        n_param = sum(r * c for r, c in e.shapes.values())
+        assert abs(n_param / 1e9 - 6.04) < 0.01
+        assert e.peak_bytes()["total"] <= 180e9
+        e.init_params(seed=1108, std=0.02, parity=False, ffn_scale=1.0 / w.n_layers)
+        loss1 = e.step(*ids)
+        assert abs(loss1 - (np.log(w.vocab) + 0.5 * 0.02 ** 2 * w.d_model)) < 0.05, loss1
+        g1 = {n: e.get_grad(n).copy() for n in sample}
+        gw = e.get_grad("w_out")
+        assert np.isfinite(gw).all() and np.abs(gw).max() > 0
+        assert np.abs(gw.sum(axis=1)).max() <= 2 ** -7 * np.abs(gw).sum(axis=1).max()
+        loss2 = e.step(*ids)
+        assert loss2 == loss1
+        for n in sample:
+            g2 = e.get_grad(n)
+            assert np.isfinite(g2).all() and np.abs(g2).max() > 0, n
+            assert maxrel(g2, 2.0 * g1[n]) <= 1e-5, n

@@ -463,7 +463,10 @@ def test_partition_error_paths():
 
 
 def test_rmsprop_training_steps_match_oracle():
-    """SURVEY.md 8(f) f3 / PAPER.md:71: three mini-batches of step + gpipe_apply_rmsprop against the oracle."""
+    """SURVEY.md 8(f) f3 / PAPER.md:71: three mini-batches of step + gpipe_apply_rmsprop against the oracle.
+    Tolerance 2e-4, twice the single-step fp32 bound (reading A20): from the second mini-batch on the two
+    sides start from parameters that already differ by their fp32 rounding, and the RMSProp quotient g / (sqrt(ms) + eps)
+    with ms ~ (1 - rho) g^2 turns a relative gradient error delta into ~ 3 delta of the update."""
     w = _tiny((0, 1))
     params = gi.make_params(w, 1001, round_bf16=False)
     o = None

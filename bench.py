@@ -63,6 +63,8 @@ def flops_per_step(w, replay_skips_last_ffn2=True):
         if replay_skips_last_ffn2:
             replay -= (w.K - 1) * f_2                     # cells 0..K-2 skip their last FFN2 in replay
         replay *= T
+        if replay_skips_last_ffn2:
+            replay *= (w.M - 1) / w.M                     # R(k, M-1) is elided: F(k, M-1)'s interior is still resident (A15b)
     return {"model": model, "executed": model + replay}
 
 

@@ -528,7 +528,10 @@ cudaError_t Engine::backward_cell(int k, int m) {
   bool daux_started = false;
   if (encdec() && k >= kt) daux = k == kt ? s.daux : dbound_aux[m & 1][k];
   const void *mem = nullptr;
-  if (encdec() && k >= kt) mem = k > kt ? (const void *)aux_mem[m] : (const void *)((remat || kt == K - 1) ? w.mem : aux_mem[m]);
+  // the transition cell's own memory: interior when it was replayed (or no later cell reads it), else what F(kt, m)
+  // wrote for the later cells (stored-activation mode, and the elided replay of the last micro-batch)
+  const bool replayed = remat && (m != M - 1 || replay_full);
+  if (encdec() && k >= kt) mem = k > kt ? (const void *)aux_mem[m] : (const void *)((replayed || kt == K - 1) ? w.mem : aux_mem[m]);
   for (int i = nl - 1; i >= 0; --i) {
     int l = cell_lo[k] + i;
     const LayerParams &q = lp[l];
@@ -699,7 +702,11 @@ cudaError_t Engine::enqueue_step() {
     for (int k = K - 1; k >= 0; --k) {
       int m = M - 1 - (tau - (K - 1 - k));
       if (m < 0 || m >= M) continue;
-      if (remat) GP_TRY(task('R', k, m));                       // early: no wait on B(k+1,m)
+      // early: no wait on B(k+1,m).  R(k, M-1) is elided (reading A15b): nothing of cell k runs between its last
+      // forward task F(k, M-1) and its first backward task B(k, M-1), so the cell's one workspace still holds, bit
+      // for bit, the interior that replay would recompute - re-materialization is there to bound memory, and that
+      // interior is resident anyway.  (GPIPE_REPLAY_FULL in a probes build replays it too.)
+      if (remat && (m != M - 1 || replay_full)) GP_TRY(task('R', k, m));
       if (k + 1 < K) GP_TRY(cudaStreamWaitEvent(st(k), ev_b[k + 1][m], 0));
       // the boundary-gradient ring has two entries: B(k,m) reuses the one B(k-1,m+2) read
       if (k > 0 && m + 2 < M) GP_TRY(cudaStreamWaitEvent(st(k), ev_b[k - 1][m + 2], 0));

@@ -294,7 +294,7 @@ def test_encdec_trace_is_the_gpipe_schedule_and_timing_modes_agree():
     tasks = {(kind, k, m): (s, t, idx) for kind, k, m, idx, s, t in ev}
     want = set()
     for k in range(K):
-        want |= set(sch.cell_program(k, K, M, True))
+        want |= set(sch.cell_program(k, K, M, True)) - {("R", k, M - 1)}      # elided replay (reading A15b)
     assert set(tasks) == want and len(ev) == len(want)
     for (kind, k, m), (s, t, idx) in tasks.items():
         for dep in sch.dependencies((kind, k, m), K, True, early=True):

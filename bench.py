@@ -40,7 +40,9 @@ DEFAULT_WORKLOAD = "T(64,16384,32)"
 # ---------------------------------------------------------------------------------------------
 # FLOP model
 # ---------------------------------------------------------------------------------------------
-def flops_per_step(w, replay_skips_last_ffn2=True):
+def flops_per_step(w, every_task=False):
+    """model: forward + backward of the whole model; executed: what the engine runs - with re-materialization the
+    replays too, minus the work it elides (readings A15, A15b, A15c; every_task=True: none elided)."""
     d, H, da, V, S = w.d_model, w.d_ffn, w.d_attn, w.vocab, w.seq_len
     T = w.tokens_per_step
     f_qkv, f_o, f_1, f_2 = 2 * d * 3 * da, 2 * da * d, 2 * d * H, 2 * H * d
@@ -54,18 +56,25 @@ def flops_per_step(w, replay_skips_last_ffn2=True):
         dec = n_dec > 0 and l >= w.n_layers - n_dec
         f_g.append(f_qkv + f_o + f_1 + f_2 + (2 * d * da + 2 * d * 2 * da + 2 * da * d if dec else 0))
         f_a.append(4 * S * da * ((S + 1) / (2 * S) if c else 1.0) + (4 * S * da if dec else 0))
-    fwd = sum(f_g) + sum(f_a) + f_v
-    bwd = 2 * sum(f_g) + 2.5 * sum(f_a) + 2 * f_v
-    model = (fwd + bwd) * T
-    replay = 0.0
-    if w.remat:
-        replay = fwd                                      # the head is replayed with its cell
-        if replay_skips_last_ffn2:
-            replay -= (w.K - 1) * f_2                     # cells 0..K-2 skip their last FFN2 in replay
-        replay *= T
-        if replay_skips_last_ffn2:
-            replay *= (w.M - 1) / w.M                     # R(k, M-1) is elided: F(k, M-1)'s interior is still resident (A15b)
-    return {"model": model, "executed": model + replay}
+    fwd_l = [g + a for g, a in zip(f_g, f_a)]
+    model = (sum(fwd_l) + f_v + 2 * sum(f_g) + 2.5 * sum(f_a) + 2 * f_v) * T
+    if not w.remat:
+        return {"model": model, "executed": model}
+    # cells of the equal split (the first L mod K cells get one more layer)
+    L, K, M = w.n_layers, w.K, w.M
+    base, extra = L // K, L % K
+    lo = [k * base + min(k, extra) for k in range(K + 1)]
+    executed = (2 * sum(f_g) + 2.5 * sum(f_a) + 2 * f_v) * T            # every backward task
+    for k in range(K):
+        cell = sum(fwd_l[lo[k]:lo[k + 1]]) + (f_v if k == K - 1 else 0.0)
+        if every_task:
+            executed += 2 * cell * T                                    # F(k, m) and R(k, m) for every m
+        elif k == K - 1:
+            executed += cell * T                                        # A15c: F(K-1, m) elided, R(K-1, m) runs (head included)
+        else:
+            # F(k, m) for every m; R(k, m) without the cell's last FFN2 (A15), and not for m = M-1 (A15b)
+            executed += cell * T + (cell - (f_2 if lo[k + 1] > lo[k] else 0.0)) * T * (M - 1) / M
+    return {"model": model, "executed": executed}
 
 
 # ---------------------------------------------------------------------------------------------
@@ -362,7 +371,7 @@ def run_ours(args, w, rank, world, local_rank):
 
     tokens = w.tokens_per_step * world
     value = tokens * args.steps / (ms / 1e3)
-    fl = flops_per_step(w, replay_skips_last_ffn2=not int(os.environ.get("GPIPE_REPLAY_FULL", "0")))
+    fl = flops_per_step(w, every_task=bool(int(os.environ.get("GPIPE_REPLAY_FULL", "0"))))
     step_s = ms / 1e3 / args.steps
     gem = {k: stats[k] for k in ("gemm_fwd", "gemm_dgrad", "gemm_wgrad")}
     gem_ms = sum(v["ms"] for v in gem.values())
@@ -416,6 +425,9 @@ def run_ours(args, w, rank, world, local_rank):
                        "l2": "inputs larger than L2 (activations+weights per step >> 126 MB)"},
             "loss": loss,
             "tflops_executed": fl["executed"] / step_s / 1e12, "tflops_model": fl["model"] / step_s / 1e12,
+            "executed_flops_per_step": {"formula": fl["executed"], "engine_count": tens_fl,
+                                        "note": "formula: flops_per_step (DESIGN.md section 9); engine_count: sum of 2MNK / attention "
+                                                "FLOPs over every launch of one step, counted by the library (gpipe_kernel_stats)"},
             "frac_of_bf16_peak_executed": fl["executed"] / step_s / 1e12 / peaks["burst"],
             "mfu_model_flops": fl["model"] / step_s / 1e12 / peaks["burst"],
             "peak_tflops_burst": peaks["burst"], "peak_tflops_sustained": peaks["sustained"],

@@ -376,15 +376,14 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
           {
             const uint64_t bdO = mdO + i * T16, bQ = mQ + i * T16, bK = mK + j * T16;
             const uint32_t acc_kv = i > i_first ? 1u : 0u, acc_q = (dq_started >> i) & 1u;
+            // the three products are independent accumulation chains of eight N = 64 k-steps each: issued round-robin,
+            // consecutive tcgen05.mma never wait on the accumulator of the one before
 #pragma unroll
-            for (int kk = 0; kk < 8; ++kk)                // dV_j += P^T dO_i   (K = 128 queries)
-              umma_bf16(tmem + C_DV, mP + kk * 128, bdO + kk * 128, id_g_mn, kk ? 1u : acc_kv);
-#pragma unroll
-            for (int kk = 0; kk < 8; ++kk)                // dK_j += dS^T Q_i
-              umma_bf16(tmem + C_DK, mdS + kk * 128, bQ + kk * 128, id_g_mn, kk ? 1u : acc_kv);
-#pragma unroll
-            for (int kk = 0; kk < 8; ++kk)                // dQ_i += dS K_j     (K = 128 keys)
-              umma_bf16(tmem + C_DQ + 64 * i, kdS + (kk >> 2) * T16 + (kk & 3) * 2, bK + kk * 128, id_g_k, kk ? 1u : acc_q);
+            for (int kk = 0; kk < 8; ++kk) {
+              umma_bf16(tmem + C_DV, mP + kk * 128, bdO + kk * 128, id_g_mn, kk ? 1u : acc_kv);      // dV_j += P^T dO_i   (K = 128 queries)
+              umma_bf16(tmem + C_DK, mdS + kk * 128, bQ + kk * 128, id_g_mn, kk ? 1u : acc_kv);      // dK_j += dS^T Q_i
+              umma_bf16(tmem + C_DQ + 64 * i, kdS + (kk >> 2) * T16 + (kk & 3) * 2, bK + kk * 128, id_g_k, kk ? 1u : acc_q);   // dQ_i += dS K_j (K = 128 keys)
+            }
           }
           dq_started |= 1u << i;
           tcgen05_commit(bar_acc);

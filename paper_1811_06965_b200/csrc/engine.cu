@@ -449,7 +449,9 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
     GP_TRY(tgemm(KC_GEMM_FWD, g));
     GP_TRY(timed(k, KC_CE, 0, Td * V * 2.0 * lpb,
                  [&] { return softmax_ce(c, dt, w.logits, lab, w.rowloss, T_mb, V, 1.f / (float)T_total, logit_clip); }));
-    GP_TRY(loss_reduce(c, w.rowloss, replay ? loss_dummy : loss_parts + m, T_mb));
+    // the micro-batch's loss partial comes from the pass that is not repeated: the forward task, or - when that is
+    // elided - the replay
+    GP_TRY(loss_reduce(c, w.rowloss, (replay && forward_runs(k)) ? loss_dummy : loss_parts + m, T_mb));
   }
   return cudaSuccess;
 }
@@ -530,7 +532,7 @@ cudaError_t Engine::backward_cell(int k, int m) {
   const void *mem = nullptr;
   // the transition cell's own memory: interior when it was replayed (or no later cell reads it), else what F(kt, m)
   // wrote for the later cells (stored-activation mode, and the elided replay of the last micro-batch)
-  const bool replayed = remat && (m != M - 1 || replay_full);
+  const bool replayed = replay_runs(k, m);
   if (encdec() && k >= kt) mem = k > kt ? (const void *)aux_mem[m] : (const void *)((replayed || kt == K - 1) ? w.mem : aux_mem[m]);
   for (int i = nl - 1; i >= 0; --i) {
     int l = cell_lo[k] + i;
@@ -694,6 +696,10 @@ cudaError_t Engine::enqueue_step() {
     for (int k = 0; k < K; ++k) {
       int m = tau - k;
       if (m < 0 || m >= M) continue;
+      // F(K-1, m) is elided under re-materialization (reading A15c): the last cell's forward has no consumer but the
+      // loss, and R(K-1, m) produces everything again, the loss included - R(K-1, m) is then the micro-batch's one
+      // pass through the last cell
+      if (!forward_runs(k)) continue;
       if (k > 0) GP_TRY(cudaStreamWaitEvent(st(k), ev_f[k - 1][m], 0));
       GP_TRY(task('F', k, m));
       if (k + 1 < K) GP_TRY(cudaEventRecord(ev_f[k][m], st(k)));
@@ -705,8 +711,11 @@ cudaError_t Engine::enqueue_step() {
       // early: no wait on B(k+1,m).  R(k, M-1) is elided (reading A15b): nothing of cell k runs between its last
       // forward task F(k, M-1) and its first backward task B(k, M-1), so the cell's one workspace still holds, bit
       // for bit, the interior that replay would recompute - re-materialization is there to bound memory, and that
-      // interior is resident anyway.  (GPIPE_REPLAY_FULL in a probes build replays it too.)
-      if (remat && (m != M - 1 || replay_full)) GP_TRY(task('R', k, m));
+      // interior is resident anyway.  (GPIPE_REPLAY_FULL in a probes build runs every task of Fig. 2c.)
+      if (replay_runs(k, m)) {
+        if (!forward_runs(k) && k > 0) GP_TRY(cudaStreamWaitEvent(st(k), ev_f[k - 1][m], 0));   // the cell's input slot
+        GP_TRY(task('R', k, m));
+      }
       if (k + 1 < K) GP_TRY(cudaStreamWaitEvent(st(k), ev_b[k + 1][m], 0));
       // the boundary-gradient ring has two entries: B(k,m) reuses the one B(k-1,m+2) read
       if (k > 0 && m + 2 < M) GP_TRY(cudaStreamWaitEvent(st(k), ev_b[k - 1][m + 2], 0));

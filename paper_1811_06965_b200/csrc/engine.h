@@ -211,6 +211,11 @@ struct Engine {
     return multi_device ? cudaSetDevice(cell_device[k]) : cudaSuccess;
   }
   Workspace &wsp(int k, int m) { return ws[k][remat ? 0 : m]; }
+  // Which of the schedule's tasks run (readings A15b / A15c).  With re-materialization the last cell's
+  // forward tasks are elided (their only product, the loss, comes out of the replay again), and for every other cell
+  // R(k, M-1) is: the workspace still holds F(k, M-1)'s interior when B(k, M-1) starts.
+  bool forward_runs(int k) const { return !(remat && k == K - 1) || replay_full; }
+  bool replay_runs(int k, int m) const { return remat && (!forward_runs(k) || m != M - 1 || replay_full); }
   // -- schedule --
   cudaError_t peer_copy(int k_dst, void *dst, int k_src, const void *src, size_t bytes, cudaStream_t s);
   cudaError_t forward_cell(int k, int m, bool replay);

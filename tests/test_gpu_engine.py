@@ -10,7 +10,7 @@ import pytest
 import gpipe_inputs as gi
 import paper_1811_06965_b200 as gp
 from oracle import schedule as sch
-from tests.util import cosine, maxrel, run_oracle
+from tests.util import cosine, engine_program, maxrel, run_oracle
 
 pytestmark = pytest.mark.gpu
 
@@ -206,19 +206,19 @@ def test_trace_is_a_valid_gpipe_schedule():
             e.step(tok, lab)
             ev = e.trace_events()
         tasks = {(kind, k, m): (s, t, idx) for kind, k, m, idx, s, t in ev}
-        # the engine elides R(k, M-1): F(k, M-1)'s interior is still in the cell's workspace (reading A15b)
-        elided = {("R", k, M - 1) for k in range(K)}
         want = set()
         for k in range(K):
-            want |= set(sch.cell_program(k, K, M, remat)) - elided
+            want |= set(engine_program(k, K, M, remat))     # Fig. 2c minus the elided tasks (readings A15b, A15c)
         assert set(tasks) == want and len(ev) == len(want)
         for (kind, k, m), (s, t, idx) in tasks.items():
             assert t >= s
             for dep in sch.dependencies((kind, k, m), K, remat, early=True):
                 assert tasks[dep][1] <= s + 1e-3, ((kind, k, m), dep)
+            if kind == "R" and k == K - 1 and k > 0:        # the replay that stands in for the elided F(K-1, m)
+                assert tasks[("F", k - 1, m)][1] <= s + 1e-3
         for k in range(K):
             prog = sorted([(v[2], key) for key, v in tasks.items() if key[1] == k])
-            assert [key for _, key in prog] == [t for t in sch.cell_program(k, K, M, remat) if t not in elided]
+            assert [key for _, key in prog] == engine_program(k, K, M, remat)
             times = [tasks[key] for _, key in prog]
             for a, b in zip(times, times[1:]):
                 assert a[1] <= b[0] + 1e-3                  # a stream is an in-order queue

@@ -52,3 +52,18 @@ def reduced_case(name):
     params = gi.make_params(w, c["seed_p"])                 # bf16-representable, parity init (A10, A12)
     tok, lab = gi.make_tokens(w, c["seed_t"])
     return w, params, tok, lab, np.dtype(c["oracle_dtype"]).type
+
+
+def engine_program(k, K, M, remat):
+    """The tasks of cell k's program (oracle/schedule.cell_program: Fig. 2c of the paper) that the CUDA engine
+    actually runs.  With re-materialization it elides work whose result is already resident or never read
+    (readings A15b, A15c; results bitwise unchanged): R(k, M-1) for k < K-1 - the cell's workspace still
+    holds the interior of F(k, M-1) when B(k, M-1) starts - and every forward task of the last cell, whose only
+    product, the loss, R(K-1, m) produces again."""
+    from oracle import schedule as sch
+    prog = sch.cell_program(k, K, M, remat)
+    if not remat:
+        return prog
+    if k == K - 1:
+        return [t for t in prog if t[0] != "F"]
+    return [t for t in prog if t != ("R", k, M - 1)]

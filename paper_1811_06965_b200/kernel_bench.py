@@ -152,7 +152,15 @@ def main():
                  torch.empty(T, device=dev), torch.empty(T, device=dev)) for _ in range(ns)]
         g, b = torch.ones(d, device=dev), torch.zeros(d, device=dev)
         ms = time_it([(lambda s=s: ops.ln_fwd(s[0], g, b, s[1], s[2], s[3])) for s in sets], args.reps)
-        report("ln", "ln_fwd", ms, 0, T * d * 6.0)
+        extra = None
+        if args.compare:
+            # comparators (never on the product path): the vendor LayerNorm on the same rows, and a plain fp32 -> bf16
+            # copy with exactly this kernel's traffic - what a launch of this size can reach at all
+            extra = {"cmp_us": time_it([(lambda s=s: torch.nn.functional.layer_norm(s[0], (d,), g, b)) for s in sets], args.reps) * 1e3}
+            cp = time_it([(lambda s=s: s[1].copy_(s[0])) for s in sets], args.reps)
+        report("ln", "ln_fwd", ms, 0, T * d * 6.0, extra)
+        if args.compare:
+            report("ln", "copy_floor", cp, 0, T * d * 6.0)
     if want("ln", "ln_bwd"):
         ns = nsets(T * d * 18)
         g = torch.ones(d, device=dev)

@@ -294,7 +294,14 @@ int gpipe_set_optimizer_slot(gpipe_t *g, int i, const float *host_in);
  * owned by that cell; may be NULL). */
 int gpipe_peak_bytes(const gpipe_t *g, size_t *total, size_t *by_category, size_t *by_cell);
 
-/* enable != 0: subsequent steps record one gpipe_trace_event per task.  With events_out != NULL
+/* Tasks that run.  A step runs the tasks of Fig. 2c - F(k,m), then per cell for m = M-1..0 the replay
+ * R(k,m) (remat only) and B(k,m) - except work whose result is already resident or never read (readings A15,
+ * A15b, A15c; results are bitwise those of running everything): with remat, R(k, M-1) for k < K-1 is elided (the cell's
+ * workspace still holds the interior of F(k, M-1) when B(k, M-1) starts), every F(K-1, m) is elided (the last cell's
+ * forward has no consumer but the loss, which R(K-1, m) produces again; the loss partial is taken from the replay),
+ * and a replay of cells 0..K-2 skips the cell's last FFN2.  The trace shows exactly the tasks that ran.
+ *
+ * enable != 0: subsequent steps record one gpipe_trace_event per task.  With events_out != NULL
  * copies up to *n_events events of the last step and sets *n_events to the number written;
  * with events_out == NULL sets *n_events to the number available. */
 int gpipe_trace(gpipe_t *g, int enable, gpipe_trace_event *events_out, int64_t *n_events);

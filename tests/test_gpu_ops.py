@@ -103,6 +103,58 @@ def test_gemm_bf16_never_falls_back_silently():
         ops.gemm(A2, B2, C2, relu=True, bits_out=bits)
 
 
+@pytest.mark.parametrize("dtype", ["fp32", "bf16"])
+def test_gemm_on_column_views_of_a_packed_buffer(dtype):
+    """The cross-attention block of a decoder layer packs q2 | k2 | v2 side by side in ONE [T, 3 da]
+    buffer so that the self-attention kernels serve it: GEMMs write column blocks of it (ldc = 3 da), read column
+    blocks of its gradient as A (lda = 3 da, dgrad) and as B (ldb = 3 da, wgrad), the memory gradient accumulates in
+    fp32 on top of another buffer (EPI_RESID, then EPI_ACCUM), column sums run over a block.  Every launch must touch
+    exactly its block: the rest of the buffer is filled with a sentinel and checked bit for bit."""
+    r = _rng(77)
+    T, d, da = 300, 192, 128                                  # ragged T: two 256-row tiles, the second one partial
+    lp = torch.bfloat16 if dtype == "bf16" else torch.float32
+    tol, cos = _tol(dtype)
+    cxt, cxq = _lp(r.standard_normal((T, d)) * 0.5, dtype)
+    memt, memq = _lp(r.standard_normal((T, d)) * 0.5, dtype)
+    wqt, wqq = _lp(r.standard_normal((d, da)) * 0.1, dtype)
+    wkvt, wkvq = _lp(r.standard_normal((d, 2 * da)) * 0.1, dtype)
+    bq = torch.tensor(r.standard_normal(da).astype(np.float32), device=DEV)
+    bkv = torch.tensor(r.standard_normal(2 * da).astype(np.float32), device=DEV)
+    SENT = 7.0
+    qkv2 = torch.full((T, 3 * da), SENT, device=DEV, dtype=lp)
+    ops.gemm(cxt, wqt, qkv2[:, :da], bias=bq)                 # q2 = cx W_q + b_q -> columns [0, da)
+    assert torch.equal(qkv2[:, da:], torch.full((T, 2 * da), SENT, device=DEV, dtype=lp))
+    assert maxrel(_np(qkv2[:, :da]), cxq @ wqq + _np(bq)) <= tol
+    ops.gemm(memt, wkvt, qkv2[:, da:], bias=bkv)              # k2 | v2 = mem W_kv + b_kv -> columns [da, 3 da)
+    assert maxrel(_np(qkv2[:, :da]), cxq @ wqq + _np(bq)) <= tol          # the first block is still there
+    assert maxrel(_np(qkv2[:, da:]), memq @ wkvq + _np(bkv)) <= tol
+    # backward: the gradient buffer in the same layout
+    dqt, dqq = _lp(r.standard_normal((T, 3 * da)) * 0.3, dtype)
+    dcx = torch.full((T, d), SENT, device=DEV, dtype=lp)
+    ops.gemm(dqt[:, :da], wqt, dcx, transB=True)              # dcx = dq2 W_q^T            (A view, lda = 3 da)
+    assert maxrel(_np(dcx), dqq[:, :da] @ wqq.T) <= tol
+    gq = torch.tensor(r.standard_normal((d, da)).astype(np.float32), device=DEV)
+    gq0 = _np(gq)
+    ops.gemm(cxt, dqt[:, :da], gq, transA=True, accumulate=True)          # dW_q += cx^T dq2   (B view, ldb = 3 da)
+    assert maxrel(_np(gq), gq0 + cxq.T @ dqq[:, :da]) <= 2e-5 * (1 if dtype == "bf16" else 5)
+    gkv = torch.zeros((d, 2 * da), device=DEV)
+    ops.gemm(memt, dqt[:, da:], gkv, transA=True, accumulate=True)        # dW_kv += mem^T dkv
+    assert maxrel(_np(gkv), memq.T @ dqq[:, da:]) <= 2e-5 * (1 if dtype == "bf16" else 5)
+    # memory gradient: first decoder layer of a cell adds to what the next cell handed down, later layers accumulate
+    handed = torch.tensor(r.standard_normal((T, d)).astype(np.float32), device=DEV)
+    dmem = torch.full((T, d), SENT, device=DEV)
+    ops.gemm(dqt[:, da:], wkvt, dmem, transB=True, resid=handed)
+    ref = _np(handed) + dqq[:, da:] @ wkvq.T
+    assert maxrel(_np(dmem), ref) <= 2e-5 * (1 if dtype == "bf16" else 5)
+    ops.gemm(dqt[:, da:], wkvt, dmem, transB=True, accumulate=True)
+    assert maxrel(_np(dmem), ref + dqq[:, da:] @ wkvq.T) <= 2e-5 * (1 if dtype == "bf16" else 5)
+    # bias gradients over the two blocks
+    dbq, dbkv = torch.zeros(da, device=DEV), torch.zeros(2 * da, device=DEV)
+    ops.colsum(dqt[:, :da], dbq)
+    ops.colsum(dqt[:, da:], dbkv)
+    assert maxrel(_np(dbq), dqq[:, :da].sum(0)) <= 2e-5 and maxrel(_np(dbkv), dqq[:, da:].sum(0)) <= 2e-5
+
+
 def test_gemm_tcgen05_split_k_deep():
     """Few output tiles and a very deep K (the dlogits W_out^T shape class): the launch is split along K,
     partials are reduced in split order, so two runs are bitwise equal and match the unsplit result."""

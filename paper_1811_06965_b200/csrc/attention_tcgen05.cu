@@ -9,9 +9,10 @@
 // maps [seq][row][col] zero-fill past the end of a sequence).
 //
 // forward  (one CTA = 128 query rows of one (sequence, head), 8 warps, 2 CTAs / SM):
-//   TMA Q, K, V -> S = Q K^T (M 128, N <= 256, K 64) in TMEM -> row max, P = exp2(..) as bf16 into
-//   swizzled K-major panels (overlaying Q / K, which are dead by then) -> O = P V (M 128, N 64,
-//   K <= 256; V is the MN-major B operand as it lies) -> O / l and the LSE stored directly.
+//   TMA Q, K, V -> S = Q K^T (M 128, N <= 256, K 64) in TMEM -> row max, P = exp2(..) written back into
+//   TENSOR MEMORY as packed bf16 pairs (tcgen05.st) over score columns the writing thread has already
+//   consumed -> O = P V with the A operand read from TMEM (M 128, N 64, K <= 256; V is the MN-major B
+//   operand as it lies) -> O / l and the LSE stored directly.  No shared-memory P panels, no proxy fence.
 // backward (one CTA = one (sequence, head), 8 compute warps + 1 control warp, 1 CTA / SM):
 //   for key block j, query block i (128 x 128 each):  S = Q_i K_j^T, dP = dO_i V_j^T  (TMEM)
 //   -> P = exp2(S - lse), dS = P (dP - D) as bf16 panels in shared memory
@@ -80,8 +81,12 @@ __device__ __forceinline__ uint32_t panel_addr(uint32_t panel, int r, int c) {
 // ---------------------------------------------------------------------------------------------
 // forward
 // ---------------------------------------------------------------------------------------------
-// shared memory (from a 1024-byte aligned base): Q [0,16K) | K [16K,48K) | pad [48K,64K) | V [64K,96K);
-// P (4 panels, 64 KB) overlays [0,64K) once the score product has retired.
+// shared memory (from a 1024-byte aligned base): Q [0,16K) | K [16K,48K) | pad [48K,64K) | V [64K,96K).
+// TMEM (256 columns): S in [0, N).  The thread pair of a row splits the 32-key chunks [0, split) / [split, nch); P chunk
+// c (16 columns of bf16 pairs) goes to column 16 c for the first half and to 32 split + 16 (c - split) for the second:
+// always inside score columns its own thread has already read in this pass (chunk c's P lies in chunk <= c of the same
+// thread; the next chunk's load, in flight, is never touched).  O accumulates once every thread is done, in 64 columns
+// clear of both P regions: [64, 128) when split = 4, else [192, 256).
 // 8 warps: warps w and w + 4 own TMEM lane quadrant w & 3 (32 query rows) and split the row's key
 // chunks (32 columns each) in two halves; the halves exchange row max and row sum through shared
 // memory.  TMEM read bandwidth (S is read twice: max, then exp) bounds the softmax, so each thread
@@ -110,7 +115,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
   __shared__ uint32_t tmem_base_smem;
   __shared__ float xm[2][128], xl[2][128];
   const uint32_t sb = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t sQ = sb, sK = sb + TILE, sV = sb + 4 * TILE, sP = sb;
+  const uint32_t sQ = sb, sK = sb + TILE, sV = sb + 4 * TILE;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int quad = warp & 3, chalf = warp >> 2;
   const int da = A * DH, seq = blockIdx.y / A, h = blockIdx.y - seq * A;
@@ -193,6 +198,9 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
   mx = fmaxf(xm[0][r_loc], xm[1][r_loc]);                // finite: key 0 is visible to every row
   const float ms = mx * sl2;
   float l = 0.f;
+  // where P chunk c lives in tensor memory (see the layout note above)
+  auto pcol = [&](int c) { return (uint32_t)(c < split ? c * 16 : 32 * split + (c - split) * 16); };
+  const uint32_t ocol = split == 4 ? 64u : 192u;          // 64 output columns clear of both P regions
   auto exp_chunk = [&](const uint32_t *r, int c) {
     float p[32];
 #pragma unroll
@@ -203,11 +211,10 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
     }
 #pragma unroll
     for (int j = 0; j < 32; ++j) l += p[j];
-    const uint32_t panel = sP + (uint32_t)(c >> 1) * TILE;
+    uint32_t pk[16];
 #pragma unroll
-    for (int q = 0; q < 4; ++q)
-      st_shared_v4(panel_addr(panel, r_loc, (c & 1) * 4 + q), pack2(p[8 * q], p[8 * q + 1]), pack2(p[8 * q + 2], p[8 * q + 3]),
-                   pack2(p[8 * q + 4], p[8 * q + 5]), pack2(p[8 * q + 6], p[8 * q + 7]));
+    for (int q = 0; q < 16; ++q) pk[q] = pack2(p[2 * q], p[2 * q + 1]);
+    tmem_st16(t_row + pcol(c), pk);
   };
   for (int c = c0; c < cv; c += 2) {
     tmem_ld_wait();
@@ -220,12 +227,13 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
     }
   }
   for (int c = max(cv, c0); c < c1; ++c) {                // chunks no row of this warp sees: P = 0
-    const uint32_t panel = sP + (uint32_t)(c >> 1) * TILE;
+    uint32_t pk[16];
 #pragma unroll
-    for (int q = 0; q < 4; ++q) st_shared_v4(panel_addr(panel, r_loc, (c & 1) * 4 + q), 0u, 0u, 0u, 0u);
+    for (int q = 0; q < 16; ++q) pk[q] = 0u;
+    tmem_st16(t_row + pcol(c), pk);
   }
+  tmem_st_wait();
   xl[chalf][r_loc] = l;
-  fence_proxy_async_smem();
   tcgen05_fence_before();
   __syncthreads();
 
@@ -236,12 +244,11 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
     const uint32_t id = idesc(0, 1, DH);
     // descriptors differ only in their (address >> 4) field: one base each, a constant added per k-step - the
     // N = 64 products retire in ~40 cycles, so the issuing thread must not spend longer than that per MMA
-    const uint64_t aP = desc_k(sP, 0), bV = desc_mn(sV, 0);
+    const uint64_t bV = desc_mn(sV, 0);
     const int nkk = N / 16;
 #pragma unroll
-    for (int kk = 0; kk < 16; ++kk)
-      if (kk < nkk)
-        umma_bf16(tmem, aP + (uint64_t)((kk >> 2) * (TILE >> 4) + (kk & 3) * 2), bV + (uint64_t)(kk * 128), id, kk ? 1u : 0u);
+    for (int kk = 0; kk < 16; ++kk)                       // 16 keys = 8 columns of P per k-step
+      if (kk < nkk) umma_bf16_ts(tmem + ocol, tmem + pcol(kk >> 1) + (kk & 1) * 8, bV + (uint64_t)(kk * 128), id, kk ? 1u : 0u);
     tcgen05_commit(bar_o);
   }
   __syncwarp();
@@ -249,7 +256,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
   mbar_wait(bar_o, 0, 0x24);
   tcgen05_fence_after();
   stamp(5);
-  tmem_ld32(t_row + chalf * 32, ra);                      // this thread's 32 of the row's 64 output columns
+  tmem_ld32(t_row + ocol + chalf * 32, ra);               // this thread's 32 of the row's 64 output columns
   tmem_ld_wait();
   if (row < S) {
     const float inv = 1.f / l;

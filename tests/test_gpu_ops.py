@@ -394,7 +394,7 @@ def test_layernorm_fwd_bwd(dtype, n, d):
 # -------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("dtype", ["fp32", "bf16"])
 @pytest.mark.parametrize("S,A,dh", [(16, 4, 16), (40, 3, 32), (256, 2, 64), (100, 2, 64), (129, 3, 64), (64, 1, 64),
-                                    (200, 2, 64), (3, 1, 64)])
+                                    (200, 2, 64), (192, 2, 64), (3, 1, 64)])
 @pytest.mark.parametrize("causal", [0, 1])
 @pytest.mark.parametrize("backend", [0, 2])       # 0: auto (tcgen05 for bf16, d_head 64, S <= 256); 2: legacy mma.sync
 def test_attention_fwd_bwd(dtype, S, A, dh, causal, backend):

@@ -103,15 +103,17 @@ def test_gemm_bf16_never_falls_back_silently():
         ops.gemm(A2, B2, C2, relu=True, bits_out=bits)
 
 
-@pytest.mark.parametrize("dtype", ["fp32", "bf16"])
-def test_gemm_on_column_views_of_a_packed_buffer(dtype):
+@pytest.mark.parametrize("dtype,T,d,da", [("fp32", 300, 192, 128), ("bf16", 300, 192, 128), ("bf16", 2048, 1024, 2048)],
+                         ids=["fp32-small", "bf16-small", "bf16-config5-microbatch"])
+def test_gemm_on_column_views_of_a_packed_buffer(dtype, T, d, da):
     """The cross-attention block of a decoder layer packs q2 | k2 | v2 side by side in ONE [T, 3 da]
     buffer so that the self-attention kernels serve it: GEMMs write column blocks of it (ldc = 3 da), read column
     blocks of its gradient as A (lda = 3 da, dgrad) and as B (ldb = 3 da, wgrad), the memory gradient accumulates in
     fp32 on top of another buffer (EPI_RESID, then EPI_ACCUM), column sums run over a block.  Every launch must touch
-    exactly its block: the rest of the buffer is filled with a sentinel and checked bit for bit."""
+    exactly its block: the rest of the buffer is filled with a sentinel and checked bit for bit.  Small case: ragged T
+    (two 256-row tiles, the second one partial); large case: the launches of one T(64,16384,32) decoder layer and
+    micro-batch (T_mb 2048, d 1024, d_a 2048), compared in full."""
     r = _rng(77)
-    T, d, da = 300, 192, 128                                  # ragged T: two 256-row tiles, the second one partial
     lp = torch.bfloat16 if dtype == "bf16" else torch.float32
     tol, cos = _tol(dtype)
     cxt, cxq = _lp(r.standard_normal((T, d)) * 0.5, dtype)

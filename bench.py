@@ -103,7 +103,7 @@ class ClockSampler:
         except Exception:
             self.p.kill()
             out = ""
-        sm, mx, reasons = [], [], set()
+        sm, mx, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for line in out.strip().splitlines():
             f = [x.strip() for x in line.split(",")]
@@ -112,13 +112,14 @@ class ClockSampler:
             try:
                 sm.append(float(f[0]))
                 mx.append(float(f[1]))
+                pw.append(float(f[2]))
             except ValueError:
                 continue
             for nm, v in zip(names, f[3:7]):
                 if v.lower().startswith("active"):
                     reasons.add(nm)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "samples": len(sm), "reasons": sorted(reasons)}
+                "power_w": float(np.median(pw)) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
 _T0 = time.perf_counter()
@@ -322,17 +323,20 @@ def run_ours(args, w, rank, world, local_rank):
     ids_h = [torch.tensor(a).pin_memory().numpy() for a in ids]
     s0 = eng.streams[0]
 
+    per_step = []
+
     def timed(fn, steps):
         barrier(world)
         torch.cuda.synchronize(dev)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(s0)                       # the engine starts and joins every step on stream 0
-        for _ in range(steps):
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+        evs[0].record(s0)                   # the engine starts and joins every step on stream 0
+        for i in range(steps):
             fn()                            # gradients keep accumulating (no apply in fwd+bwd)
-        e1.record(s0)
+            evs[i + 1].record(s0)           # also the end of step i: min / median / max over the K steps
         torch.cuda.synchronize(dev)
         barrier(world)
-        return max_over_ranks(e0.elapsed_time(e1), world)
+        per_step[:] = [evs[i].elapsed_time(evs[i + 1]) for i in range(steps)]
+        return max_over_ranks(evs[0].elapsed_time(evs[steps]), world)
 
     loss = None
     for i in range(args.warmup):
@@ -344,6 +348,7 @@ def run_ours(args, w, rank, world, local_rank):
     ms = timed(lambda: eng.step(*ids_d), args.steps)
     launches = (eng.launch_count() - l0)
     clocks = sampler.stop() if sampler else None
+    step_ms = sorted(per_step)
     progress("timed region done: %.1f ms/step" % (ms / args.steps))
     ms_e2e = timed(lambda: eng.step(*ids_h), args.steps)
     # two extra steps with per-launch CUDA events for the roofline of the dominant kernel class:
@@ -359,6 +364,18 @@ def run_ours(args, w, rank, world, local_rank):
     stats_conc = eng.kernel_stats()
     progress("per-launch timing steps done")
     eng.kernel_timing(False)
+    # gpipe_apply_sgd, timed separately (the metric is forward + backward): 18 B of traffic per parameter
+    ea0, ea1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n_param_flat = sum(r * c for r, c in eng.shapes.values())
+    if pipe_devices is None:
+        torch.cuda.synchronize(dev)
+        ea0.record(s0)
+        eng.apply_sgd(0.0)                   # lr = 0: same traffic, parameters unchanged
+        ea1.record(s0)
+        torch.cuda.synchronize(dev)
+        apply_ms = ea0.elapsed_time(ea1)
+    else:
+        apply_ms = None
     eng.zero_grads()
     peak_hbm = eng.peak_bytes()
     torch.cuda.synchronize(dev)
@@ -413,7 +430,9 @@ def run_ours(args, w, rank, world, local_rank):
                             if stats_conc else None,
                             "per_class": per_class(stats_conc)}}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": ms / args.steps,
+            "ms_per_step_min_median_max": [step_ms[0], step_ms[len(step_ms) // 2], step_ms[-1]] if step_ms else None,
+            "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "bf16" if w.dtype == "bf16" else "f32", "data": "synthetic",
             "config": {"workload": w.name, "L": w.n_layers, "n_enc": w.n_enc if w.n_dec else None, "n_dec": w.n_dec or None,
                        "d_model": w.d_model, "d_ffn": w.d_ffn,
@@ -429,6 +448,10 @@ def run_ours(args, w, rank, world, local_rank):
                                         "note": "formula: flops_per_step (DESIGN.md section 9); engine_count: sum of 2MNK / attention "
                                                 "FLOPs over every launch of one step, counted by the library (gpipe_kernel_stats)"},
             "frac_of_bf16_peak_executed": fl["executed"] / step_s / 1e12 / peaks["burst"],
+            "frac_of_sustained_executed": fl["executed"] / step_s / 1e12 / peaks["sustained"],
+            "frac_of_nominal_2250_executed": fl["executed"] / step_s / 1e12 / 2250.0,
+            "apply_sgd": {"ms": apply_ms, "gbs": (18.0 * n_param_flat / apply_ms / 1e6) if apply_ms else None,
+                          "note": "gpipe_apply_sgd timed separately (not part of tokens/s): 18 B per parameter"},
             "mfu_model_flops": fl["model"] / step_s / 1e12 / peaks["burst"],
             "peak_tflops_burst": peaks["burst"], "peak_tflops_sustained": peaks["sustained"],
             "peak_hbm_bytes": peak_hbm["total"], "peak_hbm_by_category": peak_hbm["by_category"],

@@ -188,8 +188,11 @@ int gpipe_cell_param_count(const gpipe_t *g, int k, int64_t *n_out);
  * the equal split; 1 <= K <= n_enc + n_dec.  gpipe_step_encdec: src, tgt, labels are HOST int32 [n_seqs, seq_len]
  * (labels[t] = the target id the decoder must predict at position t); gpipe_step_encdec_device: the same ids already
  * in HBM.  gpipe_step / gpipe_step_device on such a handle (and these on a plain handle) return GPIPE_EINVAL.
- * Every other call (apply, parameters, tracker, trace, graph, data-parallel apply) works unchanged; pipeline handles
- * (gpipe_create_pipeline) are not built for this model. */
+ * Every other call (apply, parameters, tracker, trace, graph, data-parallel apply) works unchanged.
+ * gpipe_create_pipeline_encdec / gpipe_plan_bytes_pipeline_encdec: the same model on the pipeline handle of
+ * gpipe_create_pipeline (one arena, stream and device per cell): BOTH members of the boundary pair and both of its
+ * gradient travel between neighbouring cells (store and forward: every cell keeps its own copy of the target embedding
+ * or of the memory and passes it on with its output). */
 typedef struct {
   int32_t n_enc, n_dec; /* >= 1 each                                                           */
   int32_t d_model, d_ffn, n_heads, d_head, vocab, seq_len, dtype;   /* as gpipe_layer_spec    */
@@ -200,6 +203,10 @@ int gpipe_plan_bytes_encdec(const gpipe_encdec_spec *spec, int K, int M, int rem
                             const int32_t *cell_lo, size_t *bytes_out);
 int gpipe_create_encdec(const gpipe_encdec_spec *spec, int K, int M, int remat, int64_t n_seqs,
                         const gpipe_env *env, const int32_t *cell_lo, gpipe_t **out);
+int gpipe_plan_bytes_pipeline_encdec(const gpipe_encdec_spec *spec, int K, int M, int remat, int64_t n_seqs,
+                                     const int32_t *cell_lo, size_t *bytes_out /* [K] */);
+int gpipe_create_pipeline_encdec(const gpipe_encdec_spec *spec, int K, int M, int remat, int64_t n_seqs,
+                                 const gpipe_cell_env *cells /* [K] */, const int32_t *cell_lo, int flags, gpipe_t **out);
 int gpipe_step_encdec(gpipe_t *g, const int32_t *src, const int32_t *tgt, const int32_t *labels, float *loss_out);
 int gpipe_step_encdec_device(gpipe_t *g, const int32_t *src_dev, const int32_t *tgt_dev, const int32_t *labels_dev,
                              float *loss_out);

@@ -91,6 +91,10 @@ def lib() -> C.CDLL:
                                           C.POINTER(C.c_size_t)]),
         "gpipe_create_encdec": (i32, [C.POINTER(EncDecSpec), i32, i32, i32, i64, C.POINTER(Env), C.POINTER(C.c_int32),
                                       C.POINTER(vp)]),
+        "gpipe_plan_bytes_pipeline_encdec": (i32, [C.POINTER(EncDecSpec), i32, i32, i32, i64, C.POINTER(C.c_int32),
+                                                   C.POINTER(C.c_size_t)]),
+        "gpipe_create_pipeline_encdec": (i32, [C.POINTER(EncDecSpec), i32, i32, i32, i64, C.POINTER(CellEnv),
+                                               C.POINTER(C.c_int32), i32, C.POINTER(vp)]),
         "gpipe_step_encdec": (i32, [vp, vp, vp, vp, C.POINTER(f32)]),
         "gpipe_step_encdec_device": (i32, [vp, vp, vp, vp, C.POINTER(f32)]),
         "gpipe_init_params": (i32, [vp, C.c_uint64, f32, i32]),
@@ -158,7 +162,8 @@ EXPORTED_SYMBOLS = [
     "gpipe_plan_bytes", "gpipe_create", "gpipe_destroy", "gpipe_layer_costs", "gpipe_partition_min_variance",
     "gpipe_create_partitioned", "gpipe_cell_range", "gpipe_plan_bytes_pipeline", "gpipe_create_pipeline",
     "gpipe_attach_optimizer_slots_cell", "gpipe_cell_param_count", "gpipe_init_params", "gpipe_init_params_scaled",
-    "gpipe_plan_bytes_encdec", "gpipe_create_encdec", "gpipe_step_encdec", "gpipe_step_encdec_device", "gpipe_step",
+    "gpipe_plan_bytes_encdec", "gpipe_create_encdec", "gpipe_plan_bytes_pipeline_encdec", "gpipe_create_pipeline_encdec",
+    "gpipe_step_encdec", "gpipe_step_encdec_device", "gpipe_step",
     "gpipe_step_device", "gpipe_apply_sgd", "gpipe_optimizer_slot_bytes", "gpipe_attach_optimizer_slots",
     "gpipe_apply_rmsprop", "gpipe_op_rmsprop", "gpipe_zero_grads", "gpipe_dp_shard", "gpipe_dp_layout",
     "gpipe_dp_apply_sgd", "gpipe_dp_apply_rmsprop", "gpipe_ipc_export", "gpipe_ipc_open", "gpipe_ipc_close", "gpipe_num_tensors",
@@ -574,7 +579,7 @@ class GPipeEncDec(GPipe):
     layers.  logit_clip: PAPER.md:174 (0 = off)."""
 
     def __init__(self, *, n_enc, n_dec, d_model, d_ffn, n_heads, d_head, vocab, seq_len, dtype, K, M, remat=True,
-                 n_seqs, ln_eps=1e-5, logit_clip=0.0, device="cuda:0", partition=None):
+                 n_seqs, ln_eps=1e-5, logit_clip=0.0, device="cuda:0", partition=None, devices=None, staged=False):
         import torch
         if not torch.cuda.is_available():
             raise GPipeError(-2, "no CUDA device: the GPipe path has no CPU fallback")
@@ -584,8 +589,30 @@ class GPipeEncDec(GPipe):
         self.spec = EncDecSpec(n_enc, n_dec, d_model, d_ffn, n_heads, d_head, vocab, seq_len, dt, ln_eps, logit_clip)
         self.K, self.M, self.remat, self.n_seqs, self.seq_len = K, M, bool(remat), n_seqs, seq_len
         self._h = C.c_void_p(None)
-        self.devices = None
+        self.devices = None if devices is None else [int(d) for d in devices]
         lo = (C.c_int32 * (K + 1))(*[int(v) for v in partition]) if partition is not None else None
+        if self.devices is not None:                       # gpipe_create_pipeline_encdec: one arena / stream / device per cell
+            if len(self.devices) != K:
+                raise ValueError("devices must list one CUDA device per cell")
+            self.device = torch.device("cuda", self.devices[0])
+            need = (C.c_size_t * K)()
+            _check(lib().gpipe_plan_bytes_pipeline_encdec(C.byref(self.spec), K, M, int(self.remat), n_seqs, lo, need))
+            self.arena, self.arenas, self.streams = None, [], []
+            cells = (CellEnv * K)()
+            for k, dev in enumerate(self.devices):
+                d = torch.device("cuda", dev)
+                with torch.cuda.device(d):
+                    a = torch.empty(int(need[k]) + 1024, dtype=torch.uint8, device=d)
+                    st = torch.cuda.Stream(device=d)
+                    torch.cuda.synchronize(d)
+                self.arenas.append(a)
+                self.streams.append(st)
+                cells[k] = CellEnv(dev, (a.data_ptr() + 1023) // 1024 * 1024, int(need[k]), st.cuda_stream)
+            with torch.cuda.device(self.device):
+                _check(lib().gpipe_create_pipeline_encdec(C.byref(self.spec), K, M, int(self.remat), n_seqs, cells, lo,
+                                                          PIPE_STAGED if staged else 0, C.byref(self._h)))
+            self._finish_init(K)
+            return
         with torch.cuda.device(self.device):
             nbytes = plan_bytes_encdec(self.spec, K, M, remat, n_seqs, partition)
             self.arena = torch.empty(nbytes + 1024, dtype=torch.uint8, device=self.device)

@@ -202,6 +202,34 @@ int gpipe_create_encdec(const gpipe_encdec_spec *spec, int K, int M, int remat, 
   return create_impl(&ls, K, M, remat, n_seqs, env, cell_lo, out, nullptr, 0, spec->n_dec, spec->logit_clip);
 }
 
+int gpipe_plan_bytes_pipeline_encdec(const gpipe_encdec_spec *spec, int K, int M, int remat, int64_t n_seqs,
+                                     const int32_t *cell_lo, size_t *bytes_out) {
+  if (!bytes_out) return fail(GPIPE_EINVAL, "bytes_out is NULL");
+  gpipe_layer_spec ls;
+  int rc = encdec_to_layer_spec(spec, &ls);
+  if (rc) return rc;
+  Engine e;
+  rc = configure(e, &ls, K, M, remat, n_seqs, cell_lo, spec->n_dec, spec->logit_clip);
+  if (rc) return rc;
+  e.n_arenas = K;
+  e.parena.assign(K, Arena());
+  if (K > 1) e.boundary_staged = 1;
+  std::string err;
+  rc = e.build_plan(true, err);
+  if (rc) return fail(rc, err);
+  for (int k = 0; k < K; ++k) bytes_out[k] = e.parena[k].used;
+  return GPIPE_OK;
+}
+
+int gpipe_create_pipeline_encdec(const gpipe_encdec_spec *spec, int K, int M, int remat, int64_t n_seqs,
+                                 const gpipe_cell_env *cells, const int32_t *cell_lo, int flags, gpipe_t **out) {
+  if (!cells) return fail(GPIPE_EINVAL, "cells is NULL");
+  gpipe_layer_spec ls;
+  int rc = encdec_to_layer_spec(spec, &ls);
+  if (rc) return rc;
+  return create_impl(&ls, K, M, remat, n_seqs, nullptr, cell_lo, out, cells, flags, spec->n_dec, spec->logit_clip);
+}
+
 int gpipe_cell_range(const gpipe_t *g, int k, int32_t *lo, int32_t *hi) {
   if (!g || k < 0 || k >= g->e.K) return fail(GPIPE_EINVAL, "handle is NULL or cell index out of range");
   if (lo) *lo = g->e.cell_lo[k];
@@ -274,7 +302,6 @@ static int create_impl(const gpipe_layer_spec *spec, int K, int M, int remat, in
   Engine &e = g->e;
   int rc = configure(e, spec, K, M, remat, n_seqs, cell_lo, n_dec, logit_clip);
   if (rc) { delete g; return rc; }
-  if (pipe && e.encdec()) { delete g; return fail(GPIPE_ENOTIMPL, "pipeline handles are not built for the encoder-decoder model"); }
   int dev = 0;
   cudaError_t ce = cudaGetDevice(&dev);
   if (ce != cudaSuccess) { delete g; return cuda_fail(ce, "gpipe_create: no usable CUDA device"); }
@@ -449,9 +476,14 @@ int gpipe_step_encdec(gpipe_t *g, const int32_t *src, const int32_t *tgt, const 
     if (src[i] < 0 || src[i] >= e.V || tgt[i] < 0 || tgt[i] >= e.V || labels[i] < 0 || labels[i] >= e.V)
       return fail(GPIPE_EINVAL, "source/target/label id outside [0, V) at flat index " + std::to_string(i));
   const size_t nb = (size_t)e.T_total * 4;
+  // both id sequences go where the embedding is (cell 0), the labels where the loss is (cell K-1)
+  const int kl = e.multi() ? e.K - 1 : 0;
+  API_CUDA(e.use(0), "gpipe_step_encdec");
   API_CUDA(cudaMemcpyAsync(e.tok_dev, src, nb, cudaMemcpyHostToDevice, e.streams[0]), "gpipe_step_encdec H2D");
   API_CUDA(cudaMemcpyAsync(e.tgt_dev, tgt, nb, cudaMemcpyHostToDevice, e.streams[0]), "gpipe_step_encdec H2D");
-  API_CUDA(cudaMemcpyAsync(e.lab_dev, labels, nb, cudaMemcpyHostToDevice, e.streams[0]), "gpipe_step_encdec H2D");
+  API_CUDA(e.use(kl), "gpipe_step_encdec");
+  API_CUDA(cudaMemcpyAsync(e.lab_dev, labels, nb, cudaMemcpyHostToDevice, e.streams[kl]), "gpipe_step_encdec H2D");
+  API_CUDA(e.use(0), "gpipe_step_encdec");
   return step_common(e, loss_out);
 }
 
@@ -460,18 +492,26 @@ int gpipe_step_encdec_device(gpipe_t *g, const int32_t *src_dev, const int32_t *
   if (!g || !src_dev || !tgt_dev || !labels_dev) return fail(GPIPE_EINVAL, "handle, src, tgt and labels are required");
   Engine &e = g->e;
   if (!e.encdec()) return fail(GPIPE_EINVAL, "not an encoder-decoder handle: use gpipe_step_device");
-  Ctx c0 = e.ctx(0);
+  const int kl = e.multi() ? e.K - 1 : 0;
   const size_t nb = (size_t)e.T_total * 4;
+  API_CUDA(e.use(0), "gpipe_step_encdec_device");
+  Ctx c0 = e.ctx(0);
   API_CUDA(cudaMemsetAsync(e.flag_dev, 0, 4, c0.stream), "gpipe_step_encdec_device");
   API_CUDA(cudaMemcpyAsync(e.tok_dev, src_dev, nb, cudaMemcpyDefault, c0.stream), "gpipe_step_encdec_device");
   API_CUDA(cudaMemcpyAsync(e.tgt_dev, tgt_dev, nb, cudaMemcpyDefault, c0.stream), "gpipe_step_encdec_device");
-  API_CUDA(cudaMemcpyAsync(e.lab_dev, labels_dev, nb, cudaMemcpyDefault, c0.stream), "gpipe_step_encdec_device");
   API_CUDA(check_ids(c0, e.tok_dev, e.T_total, e.V, e.flag_dev), "gpipe_step_encdec_device");
   API_CUDA(check_ids(c0, e.tgt_dev, e.T_total, e.V, e.flag_dev), "gpipe_step_encdec_device");
-  API_CUDA(check_ids(c0, e.lab_dev, e.T_total, e.V, e.flag_dev), "gpipe_step_encdec_device");
   API_CUDA(cudaMemcpyAsync(e.host_flag, e.flag_dev, 4, cudaMemcpyDeviceToHost, c0.stream), "gpipe_step_encdec_device");
+  API_CUDA(e.use(kl), "gpipe_step_encdec_device");
+  Ctx cl = e.ctx(kl);
+  if (e.multi()) API_CUDA(cudaMemsetAsync(e.flag_dev_last, 0, 4, cl.stream), "gpipe_step_encdec_device");
+  API_CUDA(cudaMemcpyAsync(e.lab_dev, labels_dev, nb, cudaMemcpyDefault, cl.stream), "gpipe_step_encdec_device");
+  API_CUDA(check_ids(cl, e.lab_dev, e.T_total, e.V, e.flag_dev_last), "gpipe_step_encdec_device");
+  API_CUDA(cudaMemcpyAsync(e.host_flag + 1, e.flag_dev_last, 4, cudaMemcpyDeviceToHost, cl.stream), "gpipe_step_encdec_device");
+  API_CUDA(cudaStreamSynchronize(cl.stream), "gpipe_step_encdec_device");
+  API_CUDA(e.use(0), "gpipe_step_encdec_device");
   API_CUDA(cudaStreamSynchronize(c0.stream), "gpipe_step_encdec_device");
-  if (e.host_flag[0]) return fail(GPIPE_EINVAL, "source/target/label id outside [0, V)");
+  if (e.host_flag[0] || e.host_flag[1]) return fail(GPIPE_EINVAL, "source/target/label id outside [0, V)");
   return step_common(e, loss_out);
 }
 

@@ -153,15 +153,26 @@ int Engine::build_plan(bool dry, std::string &err) {
   // encoder-decoder: the second member of the boundary pair.  One buffer per micro-batch serves every cell that
   // reads it (the hand-off is a pointer, as for x): the target embedding up to the transition cell, the memory
   // after it; its gradient travels through a two-entry ring like the gradient of x.
-  aux_tgt.assign(M, nullptr);
-  aux_mem.assign(M, nullptr);
+  aux_in.assign(K, std::vector<void *>(M, nullptr));
   if (encdec()) {
-    for (int m = 0; m < M && kt > 0; ++m) aux_tgt[m] = F32(Tm * d, GPIPE_CAT_BOUNDARY, kt);
-    for (int m = 0; m < M && kt < K - 1; ++m) aux_mem[m] = LP(Tm * d, GPIPE_CAT_BOUNDARY, kt);
+    for (int m = 0; m < M; ++m) {
+      void *tgt = nullptr, *mem_ = nullptr;
+      for (int k = 1; k < K; ++k) {
+        if (k <= kt) {
+          if (multi() || !tgt) tgt = F32(Tm * d, GPIPE_CAT_BOUNDARY, k);
+          aux_in[k][m] = tgt;
+        } else {
+          if (multi() || !mem_) mem_ = LP(Tm * d, GPIPE_CAT_BOUNDARY, k);
+          aux_in[k][m] = mem_;
+        }
+      }
+    }
   }
   for (int i = 0; i < 2; ++i) {
     dbound_aux[i].assign(K, nullptr);
+    dout_aux[i].assign(K, nullptr);
     for (int k = 1; k < K && encdec(); ++k) dbound_aux[i][k] = F32(Tm * d, GPIPE_CAT_BOUNDARY, k);
+    for (int k = 0; k + 1 < K && encdec(); ++k) dout_aux[i][k] = multi() ? F32(Tm * d, GPIPE_CAT_BOUNDARY, k) : dbound_aux[i][k + 1];
   }
   for (int i = 0; i < 2; ++i) {
     dbound[i].assign(K, nullptr);
@@ -212,8 +223,10 @@ int Engine::build_plan(bool dry, std::string &err) {
       Workspace &W_ = ws[k][w];
       const int cat = GPIPE_CAT_INTERIOR;
       if (k == 0) W_.x_emb = F32(Tm * d, cat, k);
+      // the target embedding as cell 0's own buffer: interior when cell 0 holds the transition, staging for the boundary
+      // transfer in a pipeline handle
+      if (k == 0 && encdec() && (kt == 0 || multi())) W_.aux_emb = F32(Tm * d, cat, k);
       if (encdec() && k == kt) {
-        if (k == 0) W_.aux_emb = F32(Tm * d, cat, k);
         W_.mem = LP(Tm * d, cat, k);
         W_.mean_e = F32(Tm, cat, k);
         W_.rstd_e = F32(Tm, cat, k);
@@ -342,15 +355,21 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
       // written once, in the forward pass, into the buffer cells 1..kt read; a replay of cell 0 needs it only when
       // cell 0 itself holds the transition (then it is interior and recomputed)
       const int32_t *tgt = tgt_dev + (int64_t)m * T_mb;
-      aux_x = kt == 0 ? w.aux_emb : aux_tgt[m];
-      if (kt == 0 || !replay)
+      aux_x = w.aux_emb ? w.aux_emb : (float *)aux_in[1][m];
+      if (kt == 0 || !replay) {
         GP_TRY(timed(k, KC_EMBED, 0, (double)T_mb * d * (lpb + 8), [&] { return embed_fwd(c, dt, tgt, W(i_emb), pe, aux_x, T_mb, S, d); }));
+        if (multi() && kt > 0)                              // pipeline: the second member of the boundary pair travels too
+          GP_TRY(peer_copy(1, aux_in[1][m], 0, aux_x, (size_t)T_mb * d * sizeof(float), c.stream));
+      }
     }
   } else {
     x = slot[k][m];
     if (encdec()) {
-      if (k <= kt) aux_x = aux_tgt[m];
-      else mem = aux_mem[m];
+      if (k <= kt) aux_x = (float *)aux_in[k][m];
+      else mem = aux_in[k][m];
+      // pipeline: store and forward - this cell's copy goes on to the next cell, unless this cell changes what aux is
+      if (multi() && !replay && k + 1 < K && k != kt)
+        GP_TRY(peer_copy(k + 1, aux_in[k + 1][m], k, aux_in[k][m], (size_t)T_mb * d * (k < kt ? sizeof(float) : lp_size(dt)), c.stream));
     }
   }
   int nl = cell_hi[k] - cell_lo[k];
@@ -362,8 +381,10 @@ cudaError_t Engine::forward_cell(int k, int m, bool replay) {
     if (encdec() && l == n_enc) {
       // encoder -> decoder: memory = LN_e(x_src) (reading B2); the stream switches to the target embedding.  The
       // forward pass writes the memory where the later cells read it; a replay (and a last cell) keeps it interior.
-      void *mdst = (!replay && kt < K - 1) ? aux_mem[m] : w.mem;
+      void *mdst = (!replay && kt < K - 1 && !multi()) ? aux_in[kt + 1][m] : w.mem;
       GP_TRY(tln(x, P(i_lne_g), P(i_lne_b), mdst, w.mean_e, w.rstd_e, nullptr, nullptr));
+      if (multi() && !replay && kt < K - 1)
+        GP_TRY(peer_copy(kt + 1, aux_in[kt + 1][m], kt, w.mem, (size_t)T_mb * d * lp_size(dt), c.stream));
       mem = mdst;
       x = aux_x;
     }
@@ -525,7 +546,7 @@ cudaError_t Engine::backward_cell(int k, int m) {
   // every decoder layer's cross-attention adds dkv W_kv^T to it (fp32) - the first one of the cell on top of what the
   // next cell handed down (nothing, in the last cell), the others in place.  In the encoder it is the gradient of the
   // target embedding and only travels down to cell 0.
-  const float *daux_in = (encdec() && k + 1 < K) ? dbound_aux[m & 1][k + 1] : nullptr;
+  const float *daux_in = (encdec() && k + 1 < K) ? dout_aux[m & 1][k] : nullptr;
   float *daux = nullptr;
   bool daux_started = false;
   if (encdec() && k >= kt) daux = k == kt ? s.daux : dbound_aux[m & 1][k];
@@ -533,7 +554,8 @@ cudaError_t Engine::backward_cell(int k, int m) {
   // the transition cell's own memory: interior when it was replayed (or no later cell reads it), else what F(kt, m)
   // wrote for the later cells (stored-activation mode, and the elided replay of the last micro-batch)
   const bool replayed = replay_runs(k, m);
-  if (encdec() && k >= kt) mem = k > kt ? (const void *)aux_mem[m] : (const void *)((replayed || kt == K - 1) ? w.mem : aux_mem[m]);
+  if (encdec() && k >= kt)
+    mem = k > kt ? (const void *)aux_in[k][m] : (const void *)((replayed || kt == K - 1 || multi()) ? w.mem : aux_in[kt + 1][m]);
   for (int i = nl - 1; i >= 0; --i) {
     int l = cell_lo[k] + i;
     const LayerParams &q = lp[l];
@@ -542,7 +564,7 @@ cudaError_t Engine::backward_cell(int k, int m) {
     // input of the layer: the previous layer's output, the cell's input - or, for the first decoder layer, the
     // target embedding
     const float *x_in = i > 0 ? w.layers[i - 1].x2 : (k == 0 ? w.x_emb : slot[k][m]);
-    if (trans) x_in = kt == 0 ? w.aux_emb : aux_tgt[m];
+    if (trans) x_in = kt == 0 ? w.aux_emb : (const float *)aux_in[kt][m];
     // FFN: dh = (dx W_2^T) * [h > 0] with db_1 += sum_t dh fused into the epilogue; dW_2 += h^T dx
     // (db_2 += sum_t dx was fused into the LayerNorm-backward kernel that produced dx)
     GP_TRY(dgrad(dxo, d, d, q.w_2, H, s.dh, b.hbits, G(q.b_1)));
@@ -615,7 +637,7 @@ cudaError_t Engine::backward_cell(int k, int m) {
       const float *x_src = i > 0 ? w.layers[i - 1].x2 : slot[k][m];
       GP_TRY(cast_to_lp(c, dt, daux, s.dc, T_mb * (int64_t)d));
       GP_TRY(tlnb(s.dc, x_src, w.mean_e, w.rstd_e, P(i_lne_g), nullptr, out, dt == GP_BF16 ? out_lp : nullptr,
-                  G(i_lne_g), G(i_lne_b), G(lp[l - 1].b_2)));
+                  G(i_lne_g), G(i_lne_b), (multi() && i == 0) ? nullptr : G(lp[l - 1].b_2)));
     } else {
       // its output is the FFN2 output gradient of the layer below (possibly in the previous cell):
       // db_2(l-1) += sum_t dx
@@ -641,6 +663,8 @@ cudaError_t Engine::backward_cell(int k, int m) {
     GP_TRY(peer_copy(k - 1, dout[m & 1][k - 1], k, dbound[m & 1][k], (size_t)T_mb * d * sizeof(float), c.stream));
     if (dt == GP_BF16)
       GP_TRY(peer_copy(k - 1, dout_lp[m & 1][k - 1], k, dbound_lp[m & 1][k], (size_t)T_mb * d * 2, c.stream));
+    if (encdec())
+      GP_TRY(peer_copy(k - 1, dout_aux[m & 1][k - 1], k, dbound_aux[m & 1][k], (size_t)T_mb * d * sizeof(float), c.stream));
   }
   return cudaSuccess;
 }

@@ -98,9 +98,13 @@ struct Engine {
   int kt = 0;                                          // the cell that holds layer n_enc (the transition)
   int i_lne_g = -1, i_lne_b = -1;
   int32_t *tgt_dev = nullptr;                          // target ids (cell 0 embeds both id sequences)
-  std::vector<float *> aux_tgt;                        // [M]: target embedding, read by cells 1..kt   (kt > 0)
-  std::vector<void *> aux_mem;                         // [M]: memory (lp), read by cells kt+1..K-1    (kt < K-1)
+  // aux_in[k][m], k = 1..K-1: the second member of cell k's input pair - the target embedding (fp32) for k <= kt, the
+  // memory (lp) for k > kt.  One arena: a single buffer per micro-batch serves every cell that reads it (the hand-off
+  // is a pointer, as for x).  Pipeline handle: each cell has its own copy in its own arena and forwards it to the
+  // next cell with the boundary transfer (store and forward: only neighbouring devices talk).
+  std::vector<std::vector<void *>> aux_in;
   std::vector<float *> dbound_aux[2];                  // [k]: gradient wrt the aux input of cell k (two-entry ring like dbound)
+  std::vector<float *> dout_aux[2];                    // [k]: gradient wrt the aux OUTPUT of cell k (= dbound_aux[k+1], or its local copy)
   int sm_count = 148;                                  // of the device the handle lives on (launch geometry)
   // The memory plan must not depend on the device (gpipe_plan_bytes is host-only): scratch whose size follows the
   // launch geometry is planned for this fixed SM-count bound and the launchers clamp to what was planned.

@@ -27,3 +27,17 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _library_matches_sources():
+    """The in-tree libgpipe_b200.so is rebuilt when its sources changed since it was built (stamp check; a no-op
+    otherwise), so the tests never run against a stale library."""
+    from paper_1811_06965_b200 import build
+    try:
+        build.build()
+    except Exception as ex:                      # no nvcc here: keep going only if a library exists at all
+        if not os.path.exists(build.OUT):
+            raise
+        import warnings
+        warnings.warn("could not rebuild libgpipe_b200.so (%s); testing the existing one" % ex)

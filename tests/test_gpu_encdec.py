@@ -303,3 +303,52 @@ def test_encdec_trace_is_the_gpipe_schedule_and_timing_modes_agree():
     for n in g_graph:
         assert np.array_equal(g_serial[n], g_graph[n]), n
     assert stats["attn_fwd"]["launches"] > 0 and stats["gemm_dgrad"]["flops"] > 0
+
+
+@pytest.mark.parametrize("staged", [False, True])
+@pytest.mark.parametrize("K,cell_lo", [(2, None), (3, [0, 1, 3, 4]), (4, None), (2, [0, 3, 4])])
+def test_encdec_on_the_pipeline_handle(K, cell_lo, staged):
+    """f1 x f4: the encoder-decoder model with one arena, stream and device per cell
+    (gpipe_create_pipeline_encdec; the test box has one GPU, so the cells share device 0).  BOTH members of the boundary
+    pair travel forward (store and forward: target embedding up to the transition cell, memory after it) and both
+    gradients travel back.  Against the oracle (<= 1e-4) and bitwise against the single-arena engine - except the FFN2
+    bias gradient of each non-final cell's last layer, which the owning cell sums with another kernel."""
+    import torch
+    w = _tiny(logit_clip=0.2)
+    params = gi.make_params(w, 1111, round_bf16=False)
+    ids = gi.make_tokens_encdec(w, 2112)
+    o, loss_ref = _oracle(w, params, ids, K=K, cell_lo=cell_lo)
+    with gp.from_workload(w, K=K, partition=cell_lo) as one:
+        one.set_params(params)
+        loss_one = one.step(*ids)
+        g_one = one.grads()
+        cells = one.cells
+    special = {"l%d.b_2" % (hi - 1) for (lo, hi) in cells[:-1]}
+    with gp.from_workload(w, K=K, partition=cell_lo, devices=[0] * K, staged=staged) as e:
+        assert e.cells == cells
+        e.set_params(params)
+        loss = e.step(*ids)
+        assert loss == loss_one and abs(loss - loss_ref) <= 1e-4 * abs(loss_ref)
+        for n in e.names:
+            g = e.get_grad(n)
+            assert maxrel(g, o.g[n]) <= 1e-4, n
+            if n in special:
+                assert maxrel(g, g_one[n]) <= 1e-6, n
+            else:
+                assert np.array_equal(g, g_one[n]), n
+        need = (gp.binding.C.c_size_t * K)()
+        lo = (gp.binding.C.c_int32 * (K + 1))(*cell_lo) if cell_lo else None
+        gp.binding._check(gp.lib().gpipe_plan_bytes_pipeline_encdec(gp.binding.C.byref(e.spec), K, w.M, 1, w.n_seqs, lo, need))
+        pk = e.peak_bytes()
+        assert pk["by_cell"] == [int(v) for v in need]
+        # graph capture / replay with device-resident ids, then the update cell by cell
+        dev_ids = [torch.tensor(a, device="cuda") for a in ids]
+        e.zero_grads()
+        l3 = [e.step(*dev_ids) for _ in range(3)]
+        assert l3[0] == l3[1] == l3[2] == loss and e.cuda_graph_state() == 2
+        e.zero_grads()
+        e.step(*ids)
+        e.apply_sgd(0.5)
+        o.apply_sgd(0.5)
+        for n in e.names:
+            assert maxrel(e.get_param(n), o.p[n]) <= 1e-5, n

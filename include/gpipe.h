@@ -201,6 +201,11 @@ typedef struct {
 } gpipe_encdec_spec;
 int gpipe_plan_bytes_encdec(const gpipe_encdec_spec *spec, int K, int M, int remat, int64_t n_seqs,
                             const int32_t *cell_lo, size_t *bytes_out);
+/* gpipe_layer_costs for this model ("estimated cost"): a decoder layer adds the cross-attention block's
+ * projections (2 * 4 d d_a FLOPs per token) and one unmasked attention over the seq_len memory positions.  The result
+ * feeds gpipe_partition_min_variance; layer_cost_out: host [n_enc + n_dec]. */
+int gpipe_layer_costs_encdec(const gpipe_encdec_spec *spec, int remat, double *layer_cost_out, double *embed_cost,
+                             double *head_cost);
 int gpipe_create_encdec(const gpipe_encdec_spec *spec, int K, int M, int remat, int64_t n_seqs,
                         const gpipe_env *env, const int32_t *cell_lo, gpipe_t **out);
 int gpipe_plan_bytes_pipeline_encdec(const gpipe_encdec_spec *spec, int K, int M, int remat, int64_t n_seqs,

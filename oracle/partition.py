@@ -66,3 +66,23 @@ def layer_costs(n_layers, d_model, d_ffn, n_heads, d_head, vocab, seq_len, causa
         costs.append(fwd + bwd + (fwd if remat else 0.0))
     head = f_v + 2.0 * f_v + (f_v if remat else 0.0)
     return costs, 0.0, head
+
+
+def layer_costs_encdec(n_enc, n_dec, d_model, d_ffn, n_heads, d_head, vocab, seq_len, remat) -> Tuple[List[float], float, float]:
+    """The same per-token FLOP model for the encoder-decoder T(L,H,A) (oracle/encdec_oracle.py, reading B1):
+    an encoder layer is the unmasked layer above; a decoder layer is the causal layer plus the cross-attention block -
+    q (d x d_a), k | v (d x 2 d_a) and output (d_a x d) projections, 2 * 4 d d_a FLOPs, and one unmasked attention over
+    the S memory positions, 4 S d_a."""
+    d, H, da, V, S = float(d_model), float(d_ffn), float(n_heads * d_head), float(vocab), float(seq_len)
+    f_g = 2.0 * (4.0 * d * da + 2.0 * d * H)
+    f_x = 2.0 * (4.0 * d * da)
+    f_v = 2.0 * d * V
+    costs = []
+    for l in range(n_enc + n_dec):
+        dec = l >= n_enc
+        g = f_g + (f_x if dec else 0.0)
+        a = 4.0 * S * da * ((S + 1.0) / (2.0 * S) if dec else 1.0) + (4.0 * S * da if dec else 0.0)
+        fwd, bwd = g + a, 2.0 * g + 2.5 * a
+        costs.append(fwd + bwd + (fwd if remat else 0.0))
+    head = f_v + 2.0 * f_v + (f_v if remat else 0.0)
+    return costs, 0.0, head

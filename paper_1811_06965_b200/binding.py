@@ -91,6 +91,8 @@ def lib() -> C.CDLL:
                                           C.POINTER(C.c_size_t)]),
         "gpipe_create_encdec": (i32, [C.POINTER(EncDecSpec), i32, i32, i32, i64, C.POINTER(Env), C.POINTER(C.c_int32),
                                       C.POINTER(vp)]),
+        "gpipe_layer_costs_encdec": (i32, [C.POINTER(EncDecSpec), i32, C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                           C.POINTER(C.c_double)]),
         "gpipe_plan_bytes_pipeline_encdec": (i32, [C.POINTER(EncDecSpec), i32, i32, i32, i64, C.POINTER(C.c_int32),
                                                    C.POINTER(C.c_size_t)]),
         "gpipe_create_pipeline_encdec": (i32, [C.POINTER(EncDecSpec), i32, i32, i32, i64, C.POINTER(CellEnv),
@@ -162,7 +164,7 @@ EXPORTED_SYMBOLS = [
     "gpipe_plan_bytes", "gpipe_create", "gpipe_destroy", "gpipe_layer_costs", "gpipe_partition_min_variance",
     "gpipe_create_partitioned", "gpipe_cell_range", "gpipe_plan_bytes_pipeline", "gpipe_create_pipeline",
     "gpipe_attach_optimizer_slots_cell", "gpipe_cell_param_count", "gpipe_init_params", "gpipe_init_params_scaled",
-    "gpipe_plan_bytes_encdec", "gpipe_create_encdec", "gpipe_plan_bytes_pipeline_encdec", "gpipe_create_pipeline_encdec",
+    "gpipe_plan_bytes_encdec", "gpipe_create_encdec", "gpipe_layer_costs_encdec", "gpipe_plan_bytes_pipeline_encdec", "gpipe_create_pipeline_encdec",
     "gpipe_step_encdec", "gpipe_step_encdec_device", "gpipe_step",
     "gpipe_step_device", "gpipe_apply_sgd", "gpipe_optimizer_slot_bytes", "gpipe_attach_optimizer_slots",
     "gpipe_apply_rmsprop", "gpipe_op_rmsprop", "gpipe_zero_grads", "gpipe_dp_shard", "gpipe_dp_layout",
@@ -216,6 +218,15 @@ def plan_bytes_encdec(spec: "EncDecSpec", K: int, M: int, remat: bool, n_seqs: i
     lo = (C.c_int32 * (K + 1))(*[int(v) for v in cell_lo]) if cell_lo is not None else None
     _check(lib().gpipe_plan_bytes_encdec(C.byref(spec), K, M, int(bool(remat)), n_seqs, lo, C.byref(out)))
     return int(out.value)
+
+
+def layer_costs_encdec(spec: "EncDecSpec", remat: bool) -> Tuple[List[float], float, float]:
+    """gpipe_layer_costs_encdec: (per-layer costs, embedding cost, head cost); host-only."""
+    L = spec.n_enc + spec.n_dec
+    arr = (C.c_double * max(L, 1))()
+    emb, head = C.c_double(0), C.c_double(0)
+    _check(lib().gpipe_layer_costs_encdec(C.byref(spec), int(bool(remat)), arr, C.byref(emb), C.byref(head)))
+    return [arr[i] for i in range(L)], emb.value, head.value
 
 
 def plan_bytes_pipeline(spec: LayerSpec, K: int, M: int, remat: bool, n_seqs: int, cell_lo=None) -> List[int]:
@@ -590,6 +601,11 @@ class GPipeEncDec(GPipe):
         self.K, self.M, self.remat, self.n_seqs, self.seq_len = K, M, bool(remat), n_seqs, seq_len
         self._h = C.c_void_p(None)
         self.devices = None if devices is None else [int(d) for d in devices]
+        if isinstance(partition, str):
+            if partition != "cost":
+                raise ValueError("partition must be None, 'cost' or a list of K+1 boundaries")
+            costs, c_emb, c_head = layer_costs_encdec(self.spec, self.remat)
+            partition = partition_min_variance(costs, c_emb, c_head, K)
         lo = (C.c_int32 * (K + 1))(*[int(v) for v in partition]) if partition is not None else None
         if self.devices is not None:                       # gpipe_create_pipeline_encdec: one arena / stream / device per cell
             if len(self.devices) != K:

@@ -178,6 +178,29 @@ static int encdec_to_layer_spec(const gpipe_encdec_spec *s, gpipe_layer_spec *ls
   return GPIPE_OK;
 }
 
+// the cost model of gpipe_layer_costs with the decoder layers' cross-attention block: + 2 (4 d d_a) GEMM FLOPs and one
+// unmasked attention over the S memory positions per token
+int gpipe_layer_costs_encdec(const gpipe_encdec_spec *spec, int remat, double *layer_cost_out, double *embed_cost,
+                             double *head_cost) {
+  gpipe_layer_spec ls;
+  int rc = encdec_to_layer_spec(spec, &ls);
+  if (rc) return rc;
+  Engine e;
+  rc = configure(e, &ls, 1, 1, remat, 1, nullptr, spec->n_dec, spec->logit_clip);
+  if (rc) return rc;
+  const double d = e.d, da = e.da, H = e.H, S = e.S, V = e.V;
+  const double Fg = 2.0 * (4.0 * d * da + 2.0 * d * H), Fx = 2.0 * (4.0 * d * da), Fv = 2.0 * d * V;
+  const double passes_g = 3.0 + (remat ? 1.0 : 0.0), passes_a = 3.5 + (remat ? 1.0 : 0.0);
+  for (int l = 0; l < ls.n_layers; ++l) {
+    const bool dec = e.is_dec(l);
+    const double Fa = 4.0 * S * da * (dec ? (S + 1.0) / (2.0 * S) : 1.0) + (dec ? 4.0 * S * da : 0.0);
+    if (layer_cost_out) layer_cost_out[l] = passes_g * (Fg + (dec ? Fx : 0.0)) + passes_a * Fa;
+  }
+  if (embed_cost) *embed_cost = 0.0;
+  if (head_cost) *head_cost = passes_g * Fv;
+  return GPIPE_OK;
+}
+
 int gpipe_plan_bytes_encdec(const gpipe_encdec_spec *spec, int K, int M, int remat, int64_t n_seqs, const int32_t *cell_lo,
                             size_t *bytes_out) {
   if (!bytes_out) return fail(GPIPE_EINVAL, "bytes_out is NULL");

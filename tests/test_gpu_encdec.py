@@ -352,3 +352,21 @@ def test_encdec_on_the_pipeline_handle(K, cell_lo, staged):
         o.apply_sgd(0.5)
         for n in e.names:
             assert maxrel(e.get_param(n), o.p[n]) <= 1e-5, n
+
+
+def test_encdec_cost_partition_changes_nothing_but_the_cut():
+    """partition="cost" (gpipe_layer_costs_encdec + gpipe_partition_min_variance): decoder layers cost more,
+    so the cut moves; per-token values do not depend on where the cuts are, so loss and every gradient are bitwise those
+    of the equal split."""
+    w = _tiny(3, 3, K=3, M=2)
+    params = gi.make_params(w, 1112, round_bf16=False)
+    ids = gi.make_tokens_encdec(w, 2113)
+    out = []
+    for part in (None, "cost"):
+        with gp.from_workload(w, partition=part) as e:
+            e.set_params(params)
+            out.append((e.step(*ids), e.grads(), e.cells))
+    assert out[0][2] == [(0, 2), (2, 4), (4, 6)] and out[1][2] != out[0][2] and out[1][2][-1][1] == 6
+    assert out[0][0] == out[1][0]
+    for n in out[0][1]:
+        assert np.array_equal(out[0][1][n], out[1][1][n]), n

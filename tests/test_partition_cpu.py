@@ -134,3 +134,33 @@ def test_bench_workload_partitions():
     assert sum(sizes) == 128 and sizes[-1] == 7 and max(sizes) == 9       # head = 1.5 layers: 7 layers + head
     eq = list(range(0, 129, 8))
     assert op.variance(op.cell_costs(c, b, emb, head)) < 0.5 * op.variance(op.cell_costs(c, eq, emb, head))
+
+
+def test_encdec_cost_model_and_partition():
+    """f2 on the f4 model: the library's encoder-decoder cost model equals the oracle's restatement of it; a decoder layer
+    costs more than an encoder layer by the cross-attention block (checked against the parameter counts: its four
+    projections hold 4 d d_a of the layer's weights), so the minimum-variance cut gives the decoder cells fewer layers."""
+    from oracle import encdec_oracle as eo
+    for (n_enc, n_dec, H, A) in [(6, 6, 8192, 16), (64, 64, 16384, 32), (2, 2, 256, 4)]:
+        spec = B.EncDecSpec(n_enc, n_dec, 1024, H, A, 64, 64000, 256, 1, 1e-5, 0.0)
+        for remat in (False, True):
+            c, emb, head = B.layer_costs_encdec(spec, remat)
+            rc, remb, rhead = op.layer_costs_encdec(n_enc, n_dec, 1024, H, A, 64, 64000, 256, remat)
+            assert emb == remb and abs(head - rhead) <= 1e-9 * rhead and np.allclose(c, rc, rtol=1e-12, atol=0)
+        # GEMM FLOPs per token and pass are 2 x the layer's matrix parameters: the cost difference between a decoder and an
+        # encoder layer, attention aside, must be 2 x the cross-attention block's matrix parameters x (3 passes)
+        c, _, _ = B.layer_costs_encdec(spec, False)
+        s = eo.EncDecSpec(n_enc, n_dec, 1024, H, A, 64, 64000, 256)
+        shapes = dict(eo.tensor_list(s))
+        cross = sum(shapes["l%d.%s" % (n_enc, n)][0] * shapes["l%d.%s" % (n_enc, n)][1] for n in ("w_q", "w_kv", "w_o2"))
+        da, S = A * 64, 256
+        attn_enc = 4.0 * S * da
+        attn_dec = 4.0 * S * da * (S + 1.0) / (2.0 * S) + 4.0 * S * da
+        assert abs((c[n_enc] - c[0]) - (3.0 * 2.0 * cross + 3.5 * (attn_dec - attn_enc))) <= 1e-9 * c[0]
+    spec = B.EncDecSpec(64, 64, 1024, 16384, 32, 64, 64000, 256, 1, 1e-5, 0.0)
+    c, emb, head = B.layer_costs_encdec(spec, True)
+    b = B.partition_min_variance(c, emb, head, 16)
+    sizes = [b[k + 1] - b[k] for k in range(16)]
+    assert sum(sizes) == 128 and max(sizes[:7]) >= max(sizes[9:]) and sizes[-1] < sizes[0]
+    eq = [8 * k for k in range(17)]
+    assert op.variance(op.cell_costs(c, b, emb, head)) < op.variance(op.cell_costs(c, eq, emb, head))

@@ -74,9 +74,12 @@ int gpipe_op_ln_bwd(void *stream, int dtype, const void *dy, const float *x, con
  * 2 = legacy mma.sync kernels (bf16, d_head 32 / 64; GPIPE_ENOTIMPL-style CUDA error otherwise). */
 int gpipe_op_attn_fwd(void *stream, int dtype, const void *qkv, void *o, float *lse, int n_seq, int S,
                       int A, int dh, int causal, int backend);
+/* colpart (optional; bf16, d_head 64, S <= 256, backend 0 only - GPIPE_ECUDA/invalid value otherwise): fp32
+ * [n_seq, 3*A*dh], row s = the column sums of the dqkv rows of sequence s as stored (the per-sequence partials of the
+ * bias gradient db_qkv), fused into the kernel's store path. */
 int gpipe_op_attn_bwd(void *stream, int dtype, const void *qkv, const void *o, const void *d_o,
                       const float *lse, void *dqkv, float *dvec, int n_seq, int S, int A, int dh,
-                      int causal, int backend);
+                      int causal, int backend, float *colpart);
 
 /* in place logits -> dlogits = (softmax - onehot) * inv_T; rowloss[t] = CE_t * inv_T.
  * clip > 0 ("we clip the logit predictions (softmax pre-activations) whenever their magnitude exceeds a

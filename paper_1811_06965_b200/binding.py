@@ -141,7 +141,7 @@ def lib() -> C.CDLL:
         "gpipe_op_ln_bwd_scratch_floats": (i64, [i32]),
         "gpipe_op_ln_bwd": (i32, [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, i32]),
         "gpipe_op_attn_fwd": (i32, [vp, i32, vp, vp, vp, i32, i32, i32, i32, i32, i32]),
-        "gpipe_op_attn_bwd": (i32, [vp, i32, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32]),
+        "gpipe_op_attn_bwd": (i32, [vp, i32, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp]),
         "gpipe_op_softmax_ce": (i32, [vp, i32, vp, vp, vp, i64, i32, f32, f32]),
         "gpipe_op_colsum_scratch_floats": (i64, [i64, i32]),
         "gpipe_op_colsum": (i32, [vp, i32, vp, i64, vp, vp, i64, i32]),

@@ -290,9 +290,11 @@ constexpr uint32_t C_S = 0, C_DP = 128, C_DV = 256, C_DK = 320, C_DQ = 384;
 __global__ void __launch_bounds__(BWD_THREADS, 1)
 attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_constant__ CUtensorMap map_do,
                    const bf16 *__restrict__ o, const bf16 *__restrict__ d_o, const float *__restrict__ lse,
-                   bf16 *__restrict__ dqkv, int S, int A, int causal, float scale, unsigned long long *tl) {
+                   bf16 *__restrict__ dqkv, float *__restrict__ colpart, int S, int A, int causal, float scale,
+                   unsigned long long *tl) {
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t bars[5];
+  __shared__ float cs_part[8][4][32];    // per-warp column sums of what it stored: [dV|dK cols 0-31, 32-63, dQ cols 0-31, 32-63]
   // optional timeline probe (attn_tc_set_timeline): 32 %globaltimer stamps per CTA
   auto stamp = [&](int slot) {
 #if GP_PROBES
@@ -443,7 +445,10 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
     // shared-memory transposer (80-byte rows) -> global with 4 lanes per 64-byte row segment: 8 lines per
     // store instruction instead of 32 (one lane per row costs 32 LSU cycles per instruction)
     const uint32_t xp = smem_u32(xpose) + (uint32_t)warp * (32 * 80);
-    auto store_acc = [&](uint32_t col, float mul, bf16 *dst_row0, int rows_valid) {
+    // column sums over this sequence's tokens of everything this warp stores (the bias gradient db_qkv = sum_t dqkv[t],
+    // fused here instead of a separate pass over dqkv): lane j holds column j
+    float cs_acc[4] = {0.f, 0.f, 0.f, 0.f};
+    auto store_acc = [&](uint32_t col, float mul, bf16 *dst_row0, int rows_valid, float &cs) {
       uint32_t rr[32];
       tmem_ld32(t_lane + col, rr);
       tmem_ld_wait();
@@ -463,14 +468,24 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
                      : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(xp + (uint32_t)r * 80u + (uint32_t)seg * 16u));
         if (r < rows_valid) *reinterpret_cast<uint4 *>(dst_row0 + (int64_t)r * (3 * da) + seg * 8) = v;
       }
+      if (colpart) {                                       // column `lane` of the 32 x 32 bf16 tile just staged, rows in order
+        float t = 0.f;
+        const int nr = rows_valid < 32 ? rows_valid : 32;
+        for (int r = 0; r < nr; ++r) {
+          unsigned short hv;
+          asm volatile("ld.shared.u16 %0, [%1];" : "=h"(hv) : "r"(xp + (uint32_t)r * 80u + (uint32_t)lane * 2u));
+          t += __uint_as_float((uint32_t)hv << 16);
+        }
+        cs += t;
+      }
       __syncwarp();
     };
     // dV_j (warps 0-3) / dK_j (warps 4-7): this warp's 32 key rows, 64 columns
     auto store_dvdk = [&](int j) {
       const int key0w = j * 128 + quad * 32;
       bf16 *dst = dqkv + ((int64_t)seq * S + key0w) * (3 * da) + (chalf ? da : 2 * da) + h * DH;
-      store_acc((chalf ? C_DK : C_DV), chalf ? scale : 1.f, dst, S - key0w);
-      store_acc((chalf ? C_DK : C_DV) + 32, chalf ? scale : 1.f, dst + 32, S - key0w);
+      store_acc((chalf ? C_DK : C_DV), chalf ? scale : 1.f, dst, S - key0w, cs_acc[0]);
+      store_acc((chalf ? C_DK : C_DV) + 32, chalf ? scale : 1.f, dst + 32, S - key0w, cs_acc[1]);
     };
     int n = 0;
     for (int j = 0; j < nblk; ++j) {
@@ -540,8 +555,27 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, const __grid_con
     if (chalf < nblk) {
       const int q0w = chalf * 128 + quad * 32;
       bf16 *dst = dqkv + ((int64_t)seq * S + q0w) * (3 * da) + h * DH;
-      store_acc(C_DQ + 64 * chalf, scale, dst, S - q0w);
-      store_acc(C_DQ + 64 * chalf + 32, scale, dst + 32, S - q0w);
+      store_acc(C_DQ + 64 * chalf, scale, dst, S - q0w, cs_acc[2]);
+      store_acc(C_DQ + 64 * chalf + 32, scale, dst + 32, S - q0w, cs_acc[3]);
+    }
+    if (colpart) {
+      // this (sequence, head)'s 3 x 64 column sums, summed over the warps in a fixed order: dQ from all eight warps (query
+      // block 0: warps 0-3, block 1: warps 4-7), dK from warps 4-7, dV from warps 0-3
+#pragma unroll
+      for (int i = 0; i < 4; ++i) cs_part[warp][i][lane] = cs_acc[i];
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      const int t = threadIdx.x;
+      if (t < 192) {
+        const int which = t >> 6, colh = (t >> 5) & 1, cl = t & 31;      // 0: q, 1: k, 2: v
+        float v = 0.f;
+        if (which == 0) {
+          for (int wq = 0; wq < 8; ++wq) v += cs_part[wq][2 + colh][cl];
+        } else {
+          const int w0 = which == 1 ? 4 : 0;
+          for (int wq = w0; wq < w0 + 4; ++wq) v += cs_part[wq][colh][cl];
+        }
+        colpart[(int64_t)seq * (3 * da) + which * da + h * DH + colh * 32 + cl] = v;
+      }
     }
     if (threadIdx.x == 0) stamp(31);
   }
@@ -653,7 +687,7 @@ cudaError_t attn_fwd_tc(const Ctx &c, const void *qkv, void *o, float *lse, int 
 }
 
 cudaError_t attn_bwd_tc(const Ctx &c, const void *qkv, const void *o, const void *d_o, const float *lse, void *dqkv,
-                        int n_seq, int S, int A, int causal) {
+                        float *colpart, int n_seq, int S, int A, int causal) {
   if (n_seq == 0) return cudaSuccess;
   const int da = A * fat::DH;
   CUtensorMap mq, md;
@@ -663,7 +697,8 @@ cudaError_t attn_bwd_tc(const Ctx &c, const void *qkv, const void *o, const void
     if (e != cudaSuccess) return e;
   }
   fat::attn_bwd_tc_kernel<<<n_seq * A, fat::BWD_THREADS, fat::BWD_SMEM, c.stream>>>(
-      mq, md, (const bf16 *)o, (const bf16 *)d_o, lse, (bf16 *)dqkv, S, A, causal, 1.f / sqrtf((float)fat::DH), fat::g_attn_tl);
+      mq, md, (const bf16 *)o, (const bf16 *)d_o, lse, (bf16 *)dqkv, colpart, S, A, causal, 1.f / sqrtf((float)fat::DH),
+      fat::g_attn_tl);
   GP_LAUNCH_CHECK(c);
 }
 

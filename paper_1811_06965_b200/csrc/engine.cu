@@ -282,6 +282,7 @@ int Engine::build_plan(bool dry, std::string &err) {
     {
       size_t rows = (Tm + 127) / 128;
       if (rows < (size_t)colsum_scratch_rows(T_mb)) rows = colsum_scratch_rows(T_mb);
+      if (rows < (size_t)nb) rows = (size_t)nb;             // the attention backward's per-sequence partials of db_qkv
       size_t cols = (size_t)(H > 3 * da ? H : 3 * da);
       if (cols < (size_t)d) cols = d;
       s.colsum_scratch = F32(rows * cols, cat, k);
@@ -498,6 +499,11 @@ cudaError_t Engine::backward_cell(int k, int m) {
       return ln_bwd(c, dt, dy_, x_, mu_, rs_, g_, dres_, dxo_, dxlp_, s.ln_partials, dg_, db_, cs_, T_mb, d);
     });
   };
+  // the attention backward's fused column sums: partial [nb, 3 da] (row stride 3 da) -> out[n] += sum over the nb sequences
+  const bool fused_cs = attn_bwd_fuses_colsum(dt, S, A, dh);
+  auto tred = [&](const float *part_, int n_, float *out_) -> cudaError_t {
+    return timed(k, KC_COLSUM, 0, (double)nb * n_ * 4.0, [&] { return colsum_reduce_partials(c, part_, (int)nb, n_, 3 * da, out_); });
+  };
   auto tcol = [&](const void *dy_, int64_t ld_, float *out_, int n_) -> cudaError_t {
     return timed(k, KC_COLSUM, 0, Td * n_ * lpb, [&] { return colsum_accum(c, dt, dy_, ld_, out_, s.colsum_scratch, T_mb, n_); });
   };
@@ -585,11 +591,16 @@ cudaError_t Engine::backward_cell(int k, int m) {
       GP_TRY(dgrad(dxo, d, d, q.w_o2, da, s.d_o, nullptr));
       GP_TRY(wgrad(b.o2, da, da, dxo, d, d, q.w_o2));
       GP_TRY(timed(k, KC_ATTN_BWD, 10.0 * Td * S * da, Td * 8.0 * da * lpb,
-                   [&] { return attn_bwd(c, dt, b.qkv2, b.o2, s.d_o, b.lse2, s.dqkv, s.dvec, (int)nb, S, A, dh, 0); }));
+                   [&] { return attn_bwd(c, dt, b.qkv2, b.o2, s.d_o, b.lse2, s.dqkv, s.dvec, (int)nb, S, A, dh, 0,
+                                         fused_cs ? s.colsum_scratch : nullptr); }));
+      if (fused_cs) {                                      // db_q, db_kv from the kernel's per-sequence column sums
+        GP_TRY(tred(s.colsum_scratch, da, G(q.b_q)));
+        GP_TRY(tred(s.colsum_scratch + da, 2 * da, G(q.b_kv)));
+      }
       // queries: dcx = dq2 W_q^T; dW_q += cx^T dq2; db_q += sum_t dq2
       GP_TRY(dgrad(s.dqkv, 3 * da, da, q.w_q, d, s.dc, nullptr));
       GP_TRY(wgrad(b.cx, d, d, s.dqkv, 3 * da, da, q.w_q));
-      GP_TRY(tcol(s.dqkv, 3 * da, G(q.b_q), da));
+      if (!fused_cs) GP_TRY(tcol(s.dqkv, 3 * da, G(q.b_q), da));
       // keys / values: dmem += dkv W_kv^T (fp32); dW_kv += mem^T dkv; db_kv += sum_t dkv
       {
         GemmArgs g{};
@@ -604,7 +615,7 @@ cudaError_t Engine::backward_cell(int k, int m) {
         daux_started = true;
       }
       GP_TRY(wgrad(mem, d, d, (const char *)s.dqkv + kv_off, 3 * da, 2 * da, q.w_kv));
-      GP_TRY(tcol((const char *)s.dqkv + kv_off, 3 * da, G(q.b_kv), 2 * da));
+      if (!fused_cs) GP_TRY(tcol((const char *)s.dqkv + kv_off, 3 * da, G(q.b_kv), 2 * da));
       // LN_x backward: dx1 = dx1c + LN_x'(dcx); db_o += sum_t dx1
       GP_TRY(tlnb(s.dc, b.x1, b.meanx, b.rstdx, P(q.lnx_g), dx, s.dx[cur],
                   dt == GP_BF16 ? s.dx_lp[cur] : nullptr, G(q.lnx_g), G(q.lnx_b), G(q.b_o)));
@@ -615,12 +626,16 @@ cudaError_t Engine::backward_cell(int k, int m) {
     // attention block: do = dx1 W_o^T; dW_o += o^T dx1
     GP_TRY(dgrad(dxo, d, d, q.w_o, da, s.d_o, nullptr));
     GP_TRY(wgrad(b.o, da, da, dxo, d, d, q.w_o));
+    // db_qkv += sum_t dqkv: the tcgen05 attention backward leaves per-sequence column sums of what it stores (one small
+    // reduction over the nb sequences follows); the other backends take the separate pass over dqkv
     GP_TRY(timed(k, KC_ATTN_BWD, 10.0 * Td * S * da * (causal[l] ? (S + 1.0) / (2.0 * S) : 1.0), Td * 8.0 * da * lpb,
-                 [&] { return attn_bwd(c, dt, b.qkv, b.o, s.d_o, b.lse, s.dqkv, s.dvec, (int)nb, S, A, dh, causal[l]); }));
-    // da = dqkv W_qkv^T; dW_qkv += a^T dqkv; db_qkv += sum_t dqkv
+                 [&] { return attn_bwd(c, dt, b.qkv, b.o, s.d_o, b.lse, s.dqkv, s.dvec, (int)nb, S, A, dh, causal[l],
+                                       fused_cs ? s.colsum_scratch : nullptr); }));
+    if (fused_cs) GP_TRY(tred(s.colsum_scratch, 3 * da, G(q.b_qkv)));
+    // da = dqkv W_qkv^T; dW_qkv += a^T dqkv
     GP_TRY(dgrad(s.dqkv, 3 * da, 3 * da, q.w_qkv, d, s.dc, nullptr));
     GP_TRY(wgrad(b.a, d, d, s.dqkv, 3 * da, 3 * da, q.w_qkv));
-    GP_TRY(tcol(s.dqkv, 3 * da, G(q.b_qkv), 3 * da));
+    if (!fused_cs) GP_TRY(tcol(s.dqkv, 3 * da, G(q.b_qkv), 3 * da));
     // LN1 backward: dx_in = dx1 + LN1'(da); the cell's first layer writes the boundary gradient
     float *out = s.dx[cur];
     void *out_lp = s.dx_lp[cur];

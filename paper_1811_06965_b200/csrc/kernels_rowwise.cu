@@ -400,11 +400,11 @@ colsum_stage1_kernel(const T *__restrict__ dy, int64_t ld, float *__restrict__ p
 }
 
 __global__ void __launch_bounds__(256)
-colsum_stage2_kernel(const float *__restrict__ partial, int R, int n, float *__restrict__ out) {
+colsum_stage2_kernel(const float *__restrict__ partial, int R, int n, int64_t ld, float *__restrict__ out) {
   int col = blockIdx.x * 256 + threadIdx.x;
   if (col >= n) return;
   float t = 0.f;
-  for (int r = 0; r < R; ++r) t += partial[(size_t)r * n + col];
+  for (int r = 0; r < R; ++r) t += partial[(size_t)r * ld + col];
   out[col] += t;
 }
 
@@ -413,9 +413,9 @@ int colsum_scratch_rows(int64_t n_tok) {
   return (int)(r < 1 ? 1 : (r > 32 ? 32 : r));
 }
 
-cudaError_t colsum_reduce_partials(const Ctx &c, const float *partial, int R, int n, float *out) {
+cudaError_t colsum_reduce_partials(const Ctx &c, const float *partial, int R, int n, int64_t ld, float *out) {
   if (n == 0) return cudaSuccess;
-  colsum_stage2_kernel<<<(n + 255) / 256, 256, 0, c.stream>>>(partial, R, n, out);
+  colsum_stage2_kernel<<<(n + 255) / 256, 256, 0, c.stream>>>(partial, R, n, ld, out);
   GP_LAUNCH_CHECK(c);
 }
 
@@ -432,7 +432,7 @@ cudaError_t colsum_accum(const Ctx &c, int dt, const void *dy, int64_t ld, float
   if (c.launches) ++*c.launches;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  return colsum_reduce_partials(c, scratch, R, n, out);
+  return colsum_reduce_partials(c, scratch, R, n, n, out);
 }
 
 template <typename T>

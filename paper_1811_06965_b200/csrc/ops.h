@@ -83,8 +83,8 @@ cudaError_t ln_bwd(const Ctx &c, int dt, const void *dy, const float *x, const f
 int colsum_scratch_rows(int64_t n_tok);
 cudaError_t colsum_accum(const Ctx &c, int dt, const void *dy, int64_t ld, float *out, float *scratch,
                          int64_t n_tok, int n);
-// out[n] += sum_r partial[r][n]
-cudaError_t colsum_reduce_partials(const Ctx &c, const float *partial, int R, int n, float *out);
+// out[n] += sum_r partial[r * ld + n], r = 0 .. R-1 in order
+cudaError_t colsum_reduce_partials(const Ctx &c, const float *partial, int R, int n, int64_t ld, float *out);
 // fp32 -> lp copy (the operand copy of a residual gradient)
 cudaError_t cast_to_lp(const Ctx &c, int dt, const float *src, void *dst, int64_t n);
 
@@ -94,9 +94,13 @@ cudaError_t cast_to_lp(const Ctx &c, int dt, const float *src, void *dst, int64_
 cudaError_t attn_fwd(const Ctx &c, int dt, const void *qkv, void *o, float *lse, int n_seq, int S,
                      int A, int dh, int causal);
 // dqkv: lp [n_seq*S, 3*da];  dvec: fp32 scratch [n_seq, A, S]
+// colpart (optional, only where attn_bwd_fuses_colsum() is true): fp32 [n_seq, 3*da], row s = sum over the tokens of
+// sequence s of the stored dqkv rows - the per-sequence partials of the bias gradient db_qkv (colsum_reduce_partials
+// adds them up), fused into the kernel's store path instead of a separate pass over dqkv.
+bool attn_bwd_fuses_colsum(int dt, int S, int A, int dh);
 cudaError_t attn_bwd(const Ctx &c, int dt, const void *qkv, const void *o, const void *d_o,
                      const float *lse, void *dqkv, float *dvec, int n_seq, int S, int A, int dh,
-                     int causal);
+                     int causal, float *colpart = nullptr);
 
 // ---- watchdog -------------------------------------------------------------------------------------
 // The tcgen05 kernels bound every mbarrier wait (tcgen05.cuh); a wait that times out records where it

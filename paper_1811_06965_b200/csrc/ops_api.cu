@@ -30,7 +30,7 @@ cudaError_t attn_bwd_mma(const Ctx &c, const void *qkv, const void *o, const voi
 bool attn_tc_supported(int dt, int S, int A, int dh);
 cudaError_t attn_fwd_tc(const Ctx &c, const void *qkv, void *o, float *lse, int n_seq, int S, int A, int causal);
 cudaError_t attn_bwd_tc(const Ctx &c, const void *qkv, const void *o, const void *d_o, const float *lse, void *dqkv,
-                        int n_seq, int S, int A, int causal);
+                        float *colpart, int n_seq, int S, int A, int causal);
 cudaError_t gemm_tc_set_watchdog(unsigned long long *mapped);
 cudaError_t attn_tc_set_watchdog(unsigned long long *mapped);
 
@@ -81,7 +81,7 @@ cudaError_t gemm(const Ctx &c, int dt, const GemmArgs &a) {
   if (c.gemm_backend != 1 && gemm_tc_supported(dt, a)) {
     cudaError_t e = gemm_tc(c, a);             // EPI_COLSUM: per-tile-row partial sums -> scratch
     if (e != cudaSuccess || !colsum) return e;
-    return colsum_reduce_partials(c, a.colsum_scratch, (a.M + 127) / 128, a.N, a.colsum_out);
+    return colsum_reduce_partials(c, a.colsum_scratch, (a.M + 127) / 128, a.N, a.N, a.colsum_out);
   }
   // bf16 operands belong on the tensor cores: a bf16 problem the tcgen05 kernel cannot take (unaligned base or
   // pitch, N % 32 != 0 with a ReLU pattern) is an error, never a silent ~50x slower SIMT launch.  The SIMT kernel
@@ -97,10 +97,12 @@ cudaError_t attn_fwd(const Ctx &c, int dt, const void *qkv, void *o, float *lse,
   if (attn_mma_supported(dt, S, A, dh)) return attn_fwd_mma(c, qkv, o, lse, n_seq, S, A, dh, causal);
   return attn_fwd_simt(c, dt, qkv, o, lse, n_seq, S, A, dh, causal);
 }
+bool attn_bwd_fuses_colsum(int dt, int S, int A, int dh) { return attn_use_tc() && attn_tc_supported(dt, S, A, dh); }
 cudaError_t attn_bwd(const Ctx &c, int dt, const void *qkv, const void *o, const void *d_o,
                      const float *lse, void *dqkv, float *dvec, int n_seq, int S, int A, int dh,
-                     int causal) {
-  if (attn_use_tc() && attn_tc_supported(dt, S, A, dh)) return attn_bwd_tc(c, qkv, o, d_o, lse, dqkv, n_seq, S, A, causal);
+                     int causal, float *colpart) {
+  if (attn_use_tc() && attn_tc_supported(dt, S, A, dh)) return attn_bwd_tc(c, qkv, o, d_o, lse, dqkv, colpart, n_seq, S, A, causal);
+  if (colpart) return cudaErrorInvalidValue;           // only the tcgen05 kernel fuses the column sums (attn_bwd_fuses_colsum)
   if (attn_mma_supported(dt, S, A, dh)) return attn_bwd_mma(c, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal);
   return attn_bwd_simt(c, dt, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal);
 }
@@ -186,12 +188,14 @@ int gpipe_op_attn_fwd(void *stream, int dtype, const void *qkv, void *o, float *
 }
 int gpipe_op_attn_bwd(void *stream, int dtype, const void *qkv, const void *o, const void *d_o,
                       const float *lse, void *dqkv, float *dvec, int n_seq, int S, int A, int dh,
-                      int causal, int backend) {
+                      int causal, int backend, float *colpart) {
   Ctx c = mk(stream);
   if (backend == 2 && !attn_mma_supported(dtype, S, A, dh)) return ret(cudaErrorNotSupported, "gpipe_op_attn_bwd");
+  if (colpart && (backend != 0 || !attn_bwd_fuses_colsum(dtype, S, A, dh)))
+    return ret(cudaErrorInvalidValue, "gpipe_op_attn_bwd: colpart needs the tcgen05 kernel (bf16, d_head 64, S <= 256, backend 0)");
   return ret(backend == 1   ? attn_bwd_simt(c, dtype, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal)
              : backend == 2 ? attn_bwd_mma(c, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal)
-                            : attn_bwd(c, dtype, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal),
+                            : attn_bwd(c, dtype, qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal, colpart),
              "gpipe_op_attn_bwd");
 }
 int gpipe_op_softmax_ce(void *stream, int dtype, void *logits, const int32_t *labels, float *rowloss,

@@ -91,9 +91,9 @@ def attn_fwd(qkv, o, lse, n_seq, S, A, dh, causal, backend=0):
     B._check(B.lib().gpipe_op_attn_fwd(_stream(), _dt(qkv), _p(qkv), _p(o), _p(lse), n_seq, S, A, dh, int(causal), backend))
 
 
-def attn_bwd(qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal, backend=0):
+def attn_bwd(qkv, o, d_o, lse, dqkv, dvec, n_seq, S, A, dh, causal, backend=0, colpart=None):
     B._check(B.lib().gpipe_op_attn_bwd(_stream(), _dt(qkv), _p(qkv), _p(o), _p(d_o), _p(lse), _p(dqkv), _p(dvec),
-                                       n_seq, S, A, dh, int(causal), backend))
+                                       n_seq, S, A, dh, int(causal), backend, _p(colpart)))
 
 
 def softmax_ce(logits, labels, rowloss, inv_T, clip=0.0):

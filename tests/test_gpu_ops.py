@@ -434,6 +434,35 @@ def test_attention_fwd_bwd(dtype, S, A, dh, causal, backend):
             assert cosine(got[:, blk * da:(blk + 1) * da], ref) >= (cos if dtype == "fp32" else 0.9999), name
 
 
+@pytest.mark.parametrize("S,A", [(256, 3), (200, 2), (100, 2), (64, 1)])
+@pytest.mark.parametrize("causal", [0, 1])
+def test_attention_backward_fused_column_sums(S, A, causal):
+    """db_qkv = sum_t dqkv[t]: the tcgen05 backward leaves, per sequence, the column sums of the dqkv
+    rows it stores.  They must equal the sums of the stored bf16 values (fp32 summation order aside), leave dqkv
+    unchanged bit for bit, and be refused by the backends that do not compute them."""
+    from paper_1811_06965_b200 import GPipeError
+    n_seq, dh = 3, 64
+    da = A * dh
+    r = _rng(900 + S + causal)
+    qkvt, _ = _lp(r.standard_normal((n_seq * S, 3 * da)), "bf16")
+    dot, _ = _lp(r.standard_normal((n_seq * S, da)), "bf16")
+    o = torch.empty((n_seq * S, da), device=DEV, dtype=torch.bfloat16)
+    lse = torch.empty((n_seq, A, S), device=DEV)
+    dvec = torch.empty((n_seq, A, S), device=DEV)
+    ops.attn_fwd(qkvt, o, lse, n_seq, S, A, dh, causal)
+    d0 = torch.empty((n_seq * S, 3 * da), device=DEV, dtype=torch.bfloat16)
+    d1 = torch.empty_like(d0)
+    part = torch.full((n_seq, 3 * da), 7.0, device=DEV)
+    ops.attn_bwd(qkvt, o, dot, lse, d0, dvec, n_seq, S, A, dh, causal)
+    ops.attn_bwd(qkvt, o, dot, lse, d1, dvec, n_seq, S, A, dh, causal, colpart=part)
+    assert torch.equal(d0, d1)
+    want = _np(d1).reshape(n_seq, S, 3 * da).sum(axis=1)
+    got = _np(part)
+    assert np.abs(got - want).max() <= 1e-5 * np.abs(want).max(), np.abs(got - want).max()
+    with pytest.raises(GPipeError):
+        ops.attn_bwd(qkvt, o, dot, lse, d1, dvec, n_seq, S, A, dh, causal, backend=1, colpart=part)
+
+
 @pytest.mark.parametrize("causal", [0, 1])
 def test_attention_bench_shape_sampled(causal):
     """The launch configuration bench.py times at config 5 (8 sequences x 32 heads, S 256, d_head 64: 512 forward

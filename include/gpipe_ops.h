@@ -41,7 +41,9 @@ extern "C" {
  * (tcgen05 tensor cores for bf16 - a bf16 problem the tensor-core kernel cannot take, i.e. an
  * unaligned base / row pitch or N % 32 != 0 with a ReLU pattern, fails with GPIPE_EINVAL; the SIMT
  * kernel for fp32), 1 = fp32-FMA SIMT kernel,
- * 2 = tcgen05 or fail with GPIPE_EINVAL.  colsum_out fp32 [N] / colsum_scratch fp32
+ * 2 = tcgen05 or fail with GPIPE_EINVAL, 3 = tcgen05 with 256 x 256 CTA-pair tiles only, 4 = tcgen05 with
+ * 256 x 512 CTA-pair tiles (N >= 512; flags 0, ACCUM | OUT_F32 or BIAS | RELU | BITS_OUT) or fail with
+ * GPIPE_EINVAL; backends 0 and 2 pick the tile from the shape (results are bitwise the same).  colsum_out fp32 [N] / colsum_scratch fp32
  * [gpipe_op_colsum_scratch_floats(M, N)] are only read with GPIPE_EPI_COLSUM.
  * workspace (device, may be NULL): gpipe_op_gemm_workspace_bytes(M, N, K) bytes that were ZERO before
  * their first use and are only ever used by launches on one stream at a time; with it, shapes

@@ -200,7 +200,13 @@ struct Engine {
   int build_inventory(std::string &err);
   int build_plan(bool dry, std::string &err);
   // -- helpers --
-  Ctx ctx(int k) { return Ctx{st(k), &launches, sm_count, gemm_backend, multi() ? cell_device[k] : device}; }
+  int cells_on_device(int k) const {
+    if (!multi()) return K;
+    int n = 0;
+    for (int j = 0; j < K; ++j) n += cell_device[j] == cell_device[k];
+    return n;
+  }
+  Ctx ctx(int k) { return Ctx{st(k), &launches, sm_count, gemm_backend, multi() ? cell_device[k] : device, cells_on_device(k)}; }
   int64_t rel(int i) const { return tensors[i].off - cell_off[tensors[i].cell]; }
   float *P(int i) const { return cmaster[tensors[i].cell] + rel(i); }  // fp32 master / vector param
   void *Wl(int i) const {                                              // bf16 working copy (bf16 mode)

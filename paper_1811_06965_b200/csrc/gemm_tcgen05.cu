@@ -65,7 +65,7 @@ struct Params {
   unsigned int *ws_cnt;         // [tile][rank][2]: arrivals, partials ready
 #if GP_PROBES
   unsigned long long *tl;       // optional timeline probe: 8 globaltimer stamps per CTA (gemm_tc_set_timeline)
-  int dbg;                      // GPIPE_GEMM_DBG: 1 = epilogue only drains TMEM, 2 = no TMA loads (results are garbage)
+  int dbg;                      // GPIPE_GEMM_DBG: 1 = epilogue only drains TMEM, 2 = no TMA loads, 4 = half of B's rows loaded (garbage results)
 #endif
 };
 #if GP_PROBES
@@ -100,14 +100,16 @@ __device__ __forceinline__ void tl_clock(const Params &, bool, int, int) {}
 template <int BN, int F> struct PairCfg {
   static constexpr int BNH = BN / 2;
   static constexpr uint32_t A_BYTES = 128 * BK * 2, B_BYTES = BNH * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;
-  static constexpr int STAGES = 5;
+  static constexpr int STAGES = BN == 256 ? 5 : 4;
   static constexpr int STG = 1;
-  static constexpr uint32_t BIAS_BYTES = (F < 0 || (F & EPI_BIAS)) ? 2 * BN * 4 : 0;
+  static constexpr uint32_t BIAS_BYTES = (BN == 256 && (F < 0 || (F & EPI_BIAS))) ? 2 * BN * 4 : 0;   // BN 512: bias from L1
   static constexpr uint32_t COLBUF_BYTES = (F < 0 || (F & EPI_COLSUM)) ? 4 * BN * 4 : 0;
   static constexpr uint32_t AUX_BYTES = BIAS_BYTES + COLBUF_BYTES;
   static constexpr uint32_t LIMIT = 227 * 1024 - 512;                // opt-in maximum minus the static barriers etc.
   static constexpr uint32_t STAGING_BYTES = 8 * STG * 4096;
-  static constexpr uint32_t TMEM_COLS = 2 * BN > 256 ? 512 : 256;
+  static constexpr uint32_t TMEM_COLS = 512;
+  static constexpr int NBLK = BN / 256;                               // 256-column accumulator blocks of one tile
+  static constexpr int NACC = 2 / NBLK;                               // accumulator stages in the 512 TMEM columns
   static constexpr size_t SMEM = (size_t)STAGES * STAGE_BYTES + STAGING_BYTES + AUX_BYTES + 1024;
   static_assert(SMEM <= LIMIT, "shared-memory budget");
 };
@@ -139,7 +141,9 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
   using Cfg = PairCfg<BN, F>;
   constexpr int NST = Cfg::STAGES, BNH = Cfg::BNH, STG = Cfg::STG;
   constexpr uint32_t A_BYTES = Cfg::A_BYTES, STAGE_BYTES = Cfg::STAGE_BYTES;
-  static_assert(BN == 256, "the epilogue splits the tile into two 128-column halves of four 32-column chunks");
+  static_assert(BN == 256 || (BN == 512 && F >= 0 && !SPLITK && !(F & EPI_COLSUM)),
+                "256 x 512: compile-time flags, unsplit, no column sums (shared-memory budget)");
+  constexpr int NBLK = Cfg::NBLK, NACC = Cfg::NACC;
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t bars[2 * NST + 4];
   __shared__ uint32_t tmem_base_smem;
@@ -214,7 +218,8 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
             if (++stage == NST) { stage = 0; phase ^= 1; }
             continue;
           }
-          if (rank == 0) mbar_expect_tx(full_bar(stage), 2 * STAGE_BYTES);
+          const bool half_b = GP_DBG(p, 4);            // probe: deliver only half of the B rows (25 % fewer bytes)
+          if (rank == 0) mbar_expect_tx(full_bar(stage), half_b ? 2 * (A_BYTES + Cfg::B_BYTES / 2) : 2 * STAGE_BYTES);
           const uint32_t fb = mapa_shared(full_bar(stage), 0);
           const int k0 = kb * BK;
           if (!p.a_mn_major) {
@@ -228,7 +233,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
             tma_load_2d_pair(sb, &map_b, fb, k0, n0);                          // box [BN/2 rows x 64 k]
           } else {
 #pragma unroll
-            for (int c = 0; c < BNH / 64; ++c)                                 // boxes [64 k x 64 n]
+            for (int c = 0; c < (half_b ? BNH / 128 : BNH / 64); ++c)          // boxes [64 k x 64 n]
               tma_load_2d_pair(sb + c * (BK * 128), &map_b, fb, n0 + c * 64, k0);
           }
           if (++stage == NST) { stage = 0; phase ^= 1; }
@@ -240,7 +245,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
     if (lane == 0 && rank == 0) {
       // instruction descriptor: D fp32, A/B bf16, majorness, N >> 3, M >> 4 (M = 256 over the pair)
       const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)p.a_mn_major << 15) |
-                             ((uint32_t)p.b_mn_major << 16) | ((uint32_t)(BN >> 3) << 17) |
+                             ((uint32_t)p.b_mn_major << 16) | ((uint32_t)(256 >> 3) << 17) |
                              ((uint32_t)(256 >> 4) << 24);
       // K-major: 8-row atoms 1024 B apart, +32 B per 16 k.  MN-major: 64-element chunks BK*128 B
       // apart (LBO), 8-k groups 1024 B apart (SBO), +2048 B per 16 k.
@@ -250,28 +255,69 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
       uint32_t phase = 0;
       int as = 0;
       uint32_t aphase = 0;
+      auto issue = [&](uint32_t d_tmem, int st, uint32_t b_off, bool fresh) {     // one K-block into one accumulator block
+        const uint32_t sa = smem_base + st * STAGE_BYTES, sb = sa + A_BYTES + b_off;
+#pragma unroll
+        for (int k = 0; k < BK / 16; ++k) {
+          const uint64_t ad = make_smem_desc(sa + k * a_kstep, a_lbo, a_sbo);
+          const uint64_t bd = make_smem_desc(sb + k * b_kstep, b_lbo, b_sbo);
+          umma_bf16_pair(d_tmem, ad, bd, idesc, (!fresh || k) ? 1u : 0u);
+        }
+      };
       for (int u = pair; u < num_units; u += num_pairs) {
         const int sp = u % splits;
         const int kb0 = sp * p.kb_per_split, kb1 = min(num_kb, kb0 + p.kb_per_split);
-        mbar_wait(tempty_bar(as), aphase ^ 1, 0x12);       // both CTAs' epilogues have drained this accumulator
-        tcgen05_fence_after();
-        const uint32_t d_tmem = tmem_base + (uint32_t)(as * BN);
-        for (int kb = kb0; kb < kb1; ++kb) {
-          mbar_wait(full_bar(stage), phase, 0x13);
+        if constexpr (NBLK == 1) {
+          mbar_wait(tempty_bar(as), aphase ^ 1, 0x12);       // both CTAs' epilogues have drained this accumulator
           tcgen05_fence_after();
-          if (u == pair && kb == kb0) tl_stamp(p, 2);  // first operands landed
-          const uint32_t sa = smem_base + stage * STAGE_BYTES, sb = sa + A_BYTES;
-#pragma unroll
-          for (int k = 0; k < BK / 16; ++k) {
-            const uint64_t ad = make_smem_desc(sa + k * a_kstep, a_lbo, a_sbo);
-            const uint64_t bd = make_smem_desc(sb + k * b_kstep, b_lbo, b_sbo);
-            umma_bf16_pair(d_tmem, ad, bd, idesc, (kb > kb0 || k) ? 1u : 0u);
+          const uint32_t d_tmem = tmem_base + (uint32_t)(as * BN);
+          for (int kb = kb0; kb < kb1; ++kb) {
+            mbar_wait(full_bar(stage), phase, 0x13);
+            tcgen05_fence_after();
+            if (u == pair && kb == kb0) tl_stamp(p, 2);  // first operands landed
+            issue(d_tmem, stage, 0u, kb == kb0);
+            tcgen05_commit_pair(empty_bar(stage), 3);  // frees this stage in both CTAs
+            if (++stage == NST) { stage = 0; phase ^= 1; }
           }
-          tcgen05_commit_pair(empty_bar(stage), 3);  // frees this stage in both CTAs
-          if (++stage == NST) { stage = 0; phase ^= 1; }
+          tcgen05_commit_pair(tfull_bar(as), 3);       // accumulator complete -> both epilogues
+          if (++as == 2) { as = 0; aphase ^= 1; }
+        } else {
+          // 256 x 512: one accumulator of two 256-column blocks (all 512 TMEM columns), block b = the tile columns
+          // [b*128, b*128+128) of each CTA's 256 B rows (16 KB into its B stage).  The epilogue of the previous tile
+          // drains block 0 first: the first `pre` K-blocks (what the ring holds) go into block 0 while block 1 is
+          // still being drained, then into block 1; after that both blocks per K-block.
+          const int nkb = kb1 - kb0, pre = nkb < NST ? nkb : NST;
+          mbar_wait(tempty_bar(0), aphase ^ 1, 0x12);
+          tcgen05_fence_after();
+          {
+            int st = stage;
+            uint32_t ph = phase;
+            for (int i = 0; i < pre; ++i) {
+              mbar_wait(full_bar(st), ph, 0x13);
+              tcgen05_fence_after();
+              if (u == pair && i == 0) tl_stamp(p, 2);
+              issue(tmem_base, st, 0u, i == 0);
+              if (++st == NST) { st = 0; ph ^= 1; }
+            }
+          }
+          mbar_wait(tempty_bar(1), aphase ^ 1, 0x15);
+          tcgen05_fence_after();
+          for (int i = 0; i < pre; ++i) {
+            issue(tmem_base + 256u, stage, 16384u, i == 0);
+            tcgen05_commit_pair(empty_bar(stage), 3);
+            if (++stage == NST) { stage = 0; phase ^= 1; }
+          }
+          for (int i = pre; i < nkb; ++i) {
+            mbar_wait(full_bar(stage), phase, 0x13);
+            tcgen05_fence_after();
+            issue(tmem_base, stage, 0u, false);
+            issue(tmem_base + 256u, stage, 16384u, false);
+            tcgen05_commit_pair(empty_bar(stage), 3);
+            if (++stage == NST) { stage = 0; phase ^= 1; }
+          }
+          tcgen05_commit_pair(tfull_bar(0), 3);
+          aphase ^= 1;
         }
-        tcgen05_commit_pair(tfull_bar(as), 3);       // accumulator complete -> both epilogues
-        if (++as == 2) { as = 0; aphase ^= 1; }
       }
       tl_stamp(p, 3);                                  // every MMA issued
     }
@@ -294,31 +340,36 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
       const int row0 = m0 + quad * 32, row = row0 + lane;
       const bool row_ok = row < p.M;
       float *bs = bias_s + (it & 1) * BN;
-      if (flags & EPI_BIAS) {
-        for (int i = et; i < BN; i += NUM_EPI_THREADS) bs[i] = (n0 + i < p.N) ? __ldg(p.bias + n0 + i) : 0.f;
+      if constexpr (BN == 256) {
+        if (flags & EPI_BIAS) {
+          for (int i = et; i < BN; i += NUM_EPI_THREADS) bs[i] = (n0 + i < p.N) ? __ldg(p.bias + n0 + i) : 0.f;
+        }
       }
-      // this row's ReLU-pattern words for this warp's four chunks (16 bytes), fetched before the wait
-      uint32_t mb0 = 0u, mb1 = 0u, mb2 = 0u, mb3 = 0u;
-      if ((flags & EPI_MASK) && row_ok) {
-        const uint32_t *mp = p.maskbits + (int64_t)row * p.ldmask + (n0 >> 5) + chalf * 4;
-        if (n0 + BN <= p.N && (p.ldmask & 3) == 0) {
-          const uint4 q = __ldg(reinterpret_cast<const uint4 *>(mp));
-          mb0 = q.x; mb1 = q.y; mb2 = q.z; mb3 = q.w;
-        } else {
-          const int cb = n0 + chalf * 128;
-          if (cb < p.N) mb0 = __ldg(mp);
-          if (cb + 32 < p.N) mb1 = __ldg(mp + 1);
-          if (cb + 64 < p.N) mb2 = __ldg(mp + 2);
-          if (cb + 96 < p.N) mb3 = __ldg(mp + 3);
+      // this row's ReLU-pattern words for this warp's chunks (16 bytes per 256-column block), fetched before the wait
+      uint4 mbq[NBLK];
+#pragma unroll
+      for (int jb = 0; jb < NBLK; ++jb) {
+        mbq[jb] = make_uint4(0u, 0u, 0u, 0u);
+        if ((flags & EPI_MASK) && row_ok) {
+          const uint32_t *mp = p.maskbits + (int64_t)row * p.ldmask + (n0 >> 5) + (chalf * NBLK + jb) * 4;
+          if (n0 + BN <= p.N && (p.ldmask & 3) == 0) {
+            mbq[jb] = __ldg(reinterpret_cast<const uint4 *>(mp));
+          } else {
+            const int cb = n0 + (chalf * NBLK + jb) * 128;
+            if (cb < p.N) mbq[jb].x = __ldg(mp);
+            if (cb + 32 < p.N) mbq[jb].y = __ldg(mp + 1);
+            if (cb + 64 < p.N) mbq[jb].z = __ldg(mp + 2);
+            if (cb + 96 < p.N) mbq[jb].w = __ldg(mp + 3);
+          }
         }
       }
       asm volatile("bar.sync 1, 256;" ::: "memory");       // bias_s visible; colbuf of the previous tile consumed
       mbar_wait(tfull_bar(as), aphase, 0x14);
       tcgen05_fence_after();
       if (it == 0 && et == 0) tl_stamp(p, 4);          // first accumulator complete
-      const uint32_t t_row = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(as * BN + chalf * 128);
+      const uint32_t t_row0 = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(as * 256 + chalf * 128);
       uint32_t rn[32];
-      tmem_ld32(t_row, rn);                              // first chunk in flight during the split-K handshake
+      tmem_ld32(t_row0, rn);                             // first chunk in flight during the split-K handshake
       // ---- split-K: am I the last of this (tile, rank)'s splits to finish? ----
       bool write_partial = false;
       if constexpr (SPLITK) if (splits > 1) {
@@ -342,12 +393,19 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
       float *part_row = p.ws_part + (((size_t)t * splits) * 2 + rank) * (size_t)(128 * BN) +
                         (size_t)(quad * 32 + lane) * 32;          // split 0 of this (tile, rank), chunk 0, this lane's row
       const size_t part_split_stride = (size_t)2 * 128 * BN;
+      // One 256-column accumulator block per outer iteration (256 x 512 tiles have two; TMEM block jb holds the
+      // tile columns jb*128 + [0, 128) of each CTA's half, so this warp's 4 * NBLK chunks are consecutive tile columns).
+#pragma unroll 1
+      for (int jb = 0; jb < NBLK; ++jb) {
+      const uint32_t t_row = t_row0 + (uint32_t)(jb * 256);
+      const uint32_t mb0 = jb ? mbq[NBLK - 1].x : mbq[0].x, mb1 = jb ? mbq[NBLK - 1].y : mbq[0].y,
+                     mb2 = jb ? mbq[NBLK - 1].z : mbq[0].z, mb3 = jb ? mbq[NBLK - 1].w : mbq[0].w;
       uint32_t wb0 = 0u, wb1 = 0u, wb2 = 0u, wb3 = 0u;     // EPI_BITS_OUT words of this row
-      // one 32-column chunk per iteration; NOT unrolled: the epilogue has to stay resident in the
-      // instruction cache next to the other warp roles
+      // one 32-column chunk per iteration; NOT unrolled in the run-time-flag kernel: the epilogue has to stay
+      // resident in the instruction cache next to the other warp roles
 #pragma unroll (F >= 0 ? 4 : 1)
       for (int cl = 0; cl < 4; ++cl) {
-        const int c = chalf * 4 + cl;
+        const int c = (chalf * NBLK + jb) * 4 + cl;
         const int col0 = n0 + c * 32;
         const bool col_ok = col0 < p.N;                      // uniform over the warp
         float4 rr[8];
@@ -374,6 +432,7 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
 #pragma unroll
         for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(rn[j]);
         if (cl < 3) tmem_ld32(t_row + (cl + 1) * 32, rn);    // next chunk: overlaps this chunk's arithmetic and staging
+        else if (jb + 1 < NBLK) tmem_ld32(t_row + 256, rn);
         const bool tlon = it == 0 && et == 0;
         tl_clock(p, tlon, cl, 0);
         if (!col_ok) continue;
@@ -412,10 +471,22 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
           for (int j = 0; j < 32; ++j) v[j] = acc[j];
         }
         if (flags & EPI_BIAS) {
+          if constexpr (BN == 256) {
 #pragma unroll
-          for (int j = 0; j < 32; j += 4) {
-            float4 b = *reinterpret_cast<const float4 *>(bs + c * 32 + j);
-            v[j] += b.x; v[j + 1] += b.y; v[j + 2] += b.z; v[j + 3] += b.w;
+            for (int j = 0; j < 32; j += 4) {
+              float4 b = *reinterpret_cast<const float4 *>(bs + c * 32 + j);
+              v[j] += b.x; v[j + 1] += b.y; v[j + 2] += b.z; v[j + 3] += b.w;
+            }
+          } else if (col0 + 32 <= p.N) {                     // warp-uniform 16-byte loads (the launcher checked alignment)
+            const float4 *bp = reinterpret_cast<const float4 *>(p.bias + col0);
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              const float4 b = __ldg(bp + j);
+              v[4 * j] += b.x; v[4 * j + 1] += b.y; v[4 * j + 2] += b.z; v[4 * j + 3] += b.w;
+            }
+          } else {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) v[j] += col0 + j < p.N ? __ldg(p.bias + col0 + j) : 0.f;
           }
         }
         if (flags & EPI_RELU) {
@@ -511,20 +582,13 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
           colbuf[quad * BN + c * 32 + lane] = v[0];
         }
       }
-      // every TMEM read of this accumulator stage has completed (tcgen05.wait::ld): release it
+      // every TMEM read of this accumulator block has completed (tcgen05.wait::ld): release it
       tcgen05_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive_cluster_relaxed(as ? tempty_leader1 : tempty_leader0);
-      if (++as == 2) { as = 0; aphase ^= 1; }
-      if (write_partial) {                                   // publish: all 8 warps' partial rows, then one ready tick
-        __threadfence();
-        asm volatile("bar.sync 2, 256;" ::: "memory");
-        if (et == 0) atomicAdd(p.ws_cnt + ((size_t)t * 2 + rank) * 2 + 1, 1u);
-        continue;
-      }
-      if ((flags & EPI_BITS_OUT) && row_ok) {              // this row's four pattern words: one 16-byte store
-        uint32_t *mp = p.maskbits + (int64_t)row * p.ldmask + (n0 >> 5) + chalf * 4;
-        const int cb = n0 + chalf * 128;
+      if (lane == 0) mbar_arrive_cluster_relaxed((NBLK == 1 ? as : jb) ? tempty_leader1 : tempty_leader0);
+      if ((flags & EPI_BITS_OUT) && row_ok && !write_partial) {   // this row's four pattern words: one 16-byte store
+        uint32_t *mp = p.maskbits + (int64_t)row * p.ldmask + (n0 >> 5) + (chalf * NBLK + jb) * 4;
+        const int cb = n0 + (chalf * NBLK + jb) * 128;
         if (cb + 128 <= p.N && (p.ldmask & 3) == 0) {
           *reinterpret_cast<uint4 *>(mp) = make_uint4(wb0, wb1, wb2, wb3);
         } else {
@@ -533,6 +597,14 @@ gemm_tcgen05_pair_kernel(const __grid_constant__ CUtensorMap map_a, const __grid
           if (cb + 64 < p.N) mp[2] = wb2;
           if (cb + 96 < p.N) mp[3] = wb3;
         }
+      }
+      }                                                      // jb
+      if (++as == NACC) { as = 0; aphase ^= 1; }
+      if (write_partial) {                                   // publish: all 8 warps' partial rows, then one ready tick
+        __threadfence();
+        asm volatile("bar.sync 2, 256;" ::: "memory");
+        if (et == 0) atomicAdd(p.ws_cnt + ((size_t)t * 2 + rank) * 2 + 1, 1u);
+        continue;
       }
       if (flags & EPI_COLSUM) {
         asm volatile("bar.sync 2, 256;" ::: "memory");
@@ -693,7 +765,11 @@ static cudaError_t launch_pair(const Ctx &c, const GemmArgs &a) {
   if (!a.transA) ok = get_map(a.A, 2, (uint64_t)a.K, (uint64_t)a.M, (uint64_t)a.lda, BK, 128, &ma);     // [M,K], K inner
   else ok = get_map(a.A, 2, (uint64_t)a.M, (uint64_t)a.K, (uint64_t)a.lda, 64, BK, &ma);                // [K,M], M inner
   if (!ok) return cudaErrorInvalidValue;
-  if (a.transB) ok = get_map(a.B, 2, (uint64_t)a.K, (uint64_t)a.N, (uint64_t)a.ldb, BK, Cfg::BNH, &mb);  // [N,K], K inner
+  int b_rows = Cfg::BNH;
+#if GP_PROBES
+  if (p.dbg & 4) b_rows /= 2;
+#endif
+  if (a.transB) ok = get_map(a.B, 2, (uint64_t)a.K, (uint64_t)a.N, (uint64_t)a.ldb, BK, b_rows, &mb);    // [N,K], K inner
   else ok = get_map(a.B, 2, (uint64_t)a.N, (uint64_t)a.K, (uint64_t)a.ldb, 64, BK, &mb);                // [K,N], N inner
   if (!ok) return cudaErrorInvalidValue;
   // C: boxes of 32 rows x 128 bytes (32 fp32 / 64 bf16 columns), written from swizzled staging
@@ -749,6 +825,39 @@ bool gemm_tc_supported(int dt, const GemmArgs &a) {
 // The epilogue combinations the engine launches get their own instantiation - the two that occur on few-tile,
 // deep-K shapes (plain bf16 output: dgrads; fp32 accumulate: FFN2 / out-projection forward, wgrads) also as a
 // split-K variant; anything else takes the run-time-flag kernel.
+// 256 x 512 pair tiles (BN = 512).  The full-grid GEMMs are bound by what the L2 can deliver to the SMs (DESIGN.md
+// "K1-K3"); a pair tile twice as wide needs (128 + 256) instead of 2 x (128 + 128) operand rows per 128 x 512 outputs of
+// a CTA - 25 % fewer delivered bytes per FLOP - at the price of the epilogue / main-loop overlap (one accumulator fills
+// all 512 TMEM columns; only the first ring's worth of K-blocks of the next tile overlaps the drain of block 1) and of
+// half as many, twice as long work units.  Results are bitwise those of the 256 x 256 tiles (same K order per output).
+// Measured (profiles/gemm_wide_r02.md): alone, the wgrads (K = T_mb = 2048, 256 tiles) run 66 us instead of 70-74, the
+// K = 1024 forward GEMMs 76 instead of 57 (16 K-blocks do not hide a 4 us drain), the 32-tile deep-K products twice as
+// long on half the SMs; in the step, with >= 8 cells in flight everything that can go wide should (config 5:
+// 1471 -> 1427 ms, config 4: 547 -> 532), with 2-4 cells only the >= 64-tile products with K >= 2048 (config 3:
+// 159.5 -> 157.7 ms, config 2 unchanged; all-wide there is 2-13 % SLOWER: nothing fills the SMs a 16-tile launch
+// leaves idle).  gemm_backend 3 forbids the wide tile, 4 forces it (the per-kernel tests).
+static bool wide_tile_supported(const GemmArgs &a) {
+  const bool flags_ok = a.flags == 0 || a.flags == (EPI_ACCUM | EPI_OUT_F32) ||
+                        a.flags == (EPI_BIAS | EPI_RELU | EPI_BITS_OUT);
+  return flags_ok && a.N >= 512 && (!(a.flags & EPI_BIAS) || ((uintptr_t)a.bias & 15) == 0);
+}
+static bool wide_tile(const Ctx &c, const GemmArgs &a, bool split) {
+  if (c.gemm_backend == 3 || split || !wide_tile_supported(a)) return false;
+  if (c.gemm_backend == 4) return true;
+  if (a.N % 512 || (a.flags & EPI_BIAS)) return false;
+  const int tiles = ((a.M + 255) / 256) * ((a.N + 255) / 256);
+#if GP_PROBES
+  // experiment knobs: GPIPE_GEMM_WIDE bit 0 plain bf16 output, bit 1 fp32 accumulate (default 3); MINK / MAXK / MINTILES
+  static const int wide = getenv("GPIPE_GEMM_WIDE") ? atoi(getenv("GPIPE_GEMM_WIDE")) : 3;
+  static const int mink = getenv("GPIPE_GEMM_WIDE_MINK") ? atoi(getenv("GPIPE_GEMM_WIDE_MINK")) : -1;
+  static const int maxk = getenv("GPIPE_GEMM_WIDE_MAXK") ? atoi(getenv("GPIPE_GEMM_WIDE_MAXK")) : 1 << 30;
+  static const int mintiles = getenv("GPIPE_GEMM_WIDE_MINTILES") ? atoi(getenv("GPIPE_GEMM_WIDE_MINTILES")) : -1;
+  if (!(wide & (a.flags == 0 ? 1 : 2)) || a.K > maxk) return false;
+  if (mink >= 0 || mintiles >= 0) return a.K >= mink && tiles >= mintiles;
+#endif
+  return c.streams >= 8 || (tiles >= 64 && a.K >= 2048);
+}
+
 cudaError_t gemm_tc(const Ctx &c, const GemmArgs &a) {
 #if GP_PROBES
   static const int generic_only = getenv("GPIPE_GEMM_GENERIC") ? atoi(getenv("GPIPE_GEMM_GENERIC")) : 0;
@@ -758,6 +867,14 @@ cudaError_t gemm_tc(const Ctx &c, const GemmArgs &a) {
   const int tiles = ((a.M + 255) / 256) * ((a.N + 255) / 256);
   const bool split = a.ws && tc::splitk_factor(tiles, (a.K + tc::BK - 1) / tc::BK, c.sm_count / 2) > 1 &&
                      a.ws_bytes >= gemm_splitk_ws_bytes(a.M, a.N, a.K, c.sm_count);
+  if (c.gemm_backend == 4 && !wide_tile(c, a, split)) return cudaErrorNotSupported;
+  if (wide_tile(c, a, split)) {
+    switch (a.flags) {
+      case 0: return tc::launch_pair<512, 0, false>(c, a);
+      case EPI_ACCUM | EPI_OUT_F32: return tc::launch_pair<512, EPI_ACCUM | EPI_OUT_F32, false>(c, a);
+      default: return tc::launch_pair<512, EPI_BIAS | EPI_RELU | EPI_BITS_OUT, false>(c, a);
+    }
+  }
   if (!generic_only) {
     switch (a.flags) {
       case 0: return split ? tc::launch_pair<256, 0, true>(c, a) : tc::launch_pair<256, 0, false>(c, a);

@@ -15,8 +15,11 @@ struct Ctx {
   cudaStream_t stream;
   int64_t *launches;   // host counter, incremented once per kernel launch
   int sm_count;
-  int gemm_backend;    // 0 = auto (tcgen05 for bf16, SIMT for fp32), 1 = force SIMT, 2 = tcgen05 or fail
+  int gemm_backend;    // 0 = auto (tcgen05 for bf16, SIMT for fp32), 1 = force SIMT, 2 = tcgen05 or fail,
+                       // 3 = tcgen05 with 256 x 256 pair tiles or fail, 4 = tcgen05 with 256 x 512 pair tiles or fail
   int device;          // CUDA device ordinal the stream belongs to (per-device function attributes)
+  int streams = 1;     // streams that share the GPU with this launch (the cells of a pipeline on this device):
+                       // with >= 8 the GEMMs take 256 x 512 pair tiles wherever they can (gemm_tcgen05.cu)
 };
 
 inline size_t lp_size(int dt) { return dt == GP_BF16 ? 2 : 4; }

@@ -86,7 +86,7 @@ cudaError_t gemm(const Ctx &c, int dt, const GemmArgs &a) {
   // bf16 operands belong on the tensor cores: a bf16 problem the tcgen05 kernel cannot take (unaligned base or
   // pitch, N % 32 != 0 with a ReLU pattern) is an error, never a silent ~50x slower SIMT launch.  The SIMT kernel
   // is the fp32 (TF32 off) path, or an explicit request (backend 1: the per-kernel tests).
-  if (c.gemm_backend == 2 || (dt == GP_BF16 && c.gemm_backend != 1)) return cudaErrorNotSupported;
+  if (c.gemm_backend >= 2 || (dt == GP_BF16 && c.gemm_backend != 1)) return cudaErrorNotSupported;
   cudaError_t e = gemm_simt(c, dt, a);
   if (e != cudaSuccess || !colsum) return e;
   return colsum_accum(c, dt, a.C, a.ldc, a.colsum_out, a.colsum_scratch, a.M, a.N);

@@ -82,6 +82,73 @@ def test_gemm_tcgen05_all_layouts(transA, transB):
         assert maxrel(_np(C), ref) <= 2 ** -7 and cosine(_np(C), ref) >= 0.99999, (M, N, K)
 
 
+# 256 x 512 pair tiles (backend 4; backend 3 = 256 x 256 only): several tiles, ragged tails in M, N (a half-empty last
+# tile, N % 32 != 0) and K, fewer and more K-blocks than the 4 ring stages, one K-block
+WIDE_SHAPES = [(512, 1024, 320), (304, 520, 200), (1024, 512, 1088), (264, 1032, 64), (256, 512, 64), (2048, 2048, 1024),
+               (704, 1536, 4160), (136, 3072, 2048)]
+
+
+@pytest.mark.parametrize("transA,transB", [(0, 0), (0, 1), (1, 0), (1, 1)])
+@pytest.mark.parametrize("epi", ["plain", "accum", "bias_relu_bits"])
+def test_gemm_tcgen05_wide_tile(transA, transB, epi):
+    """The 256 x 512 pair tile (one accumulator in all 512 TMEM columns, two MMAs per K step, accumulator blocks that
+    interleave the two CTAs' B halves) against the fp64 product of the same operands, and bit for bit against the
+    256 x 256 tile: every output is the same chain of MMAs over K in the same order."""
+    for (M, N, K) in WIDE_SHAPES:
+        if epi == "bias_relu_bits" and N % 32:
+            continue
+        r = _rng(M * 1000 + N + K + 7)
+        At, Aq = _lp(r.standard_normal((K, M) if transA else (M, K)) * 0.5, "bf16")
+        Bt, Bq = _lp(r.standard_normal((N, K) if transB else (K, N)) * 0.5, "bf16")
+        ref = (Aq.T if transA else Aq) @ (Bq.T if transB else Bq)
+        kw = dict(transA=bool(transA), transB=bool(transB), workspace=False)
+        c0 = r.standard_normal((M, N)).astype(np.float32)
+        bias = r.standard_normal(N).astype(np.float32)
+        out = {}
+        for backend in (3, 4):
+            if epi == "plain":
+                C = torch.empty((M, N), device=DEV, dtype=torch.bfloat16)
+                ops.gemm(At, Bt, C, backend=backend, **kw)
+                out[backend] = (C,)
+                if backend == 4:
+                    assert maxrel(_np(C), ref) <= 2 ** -7 and cosine(_np(C), ref) >= 0.99999, (M, N, K)
+            elif epi == "accum":
+                C = torch.tensor(c0, device=DEV)
+                ops.gemm(At, Bt, C, accumulate=True, backend=backend, **kw)
+                ops.gemm(At, Bt, C, accumulate=True, backend=backend, **kw)
+                out[backend] = (C,)
+                if backend == 4:
+                    assert maxrel(_np(C), c0 + 2 * ref) <= 2e-5, (M, N, K)
+            else:
+                C = torch.empty((M, N), device=DEV, dtype=torch.bfloat16)
+                bits = torch.zeros((M, N // 32), device=DEV, dtype=torch.int32)
+                ops.gemm(At, Bt, C, bias=torch.tensor(bias, device=DEV), relu=True, bits_out=bits, backend=backend, **kw)
+                out[backend] = (C, bits)
+                if backend == 4:
+                    want = np.maximum(ref + bias, 0)
+                    assert maxrel(_np(C), want) <= 2 ** -7 and cosine(_np(C), want) >= 0.99999, (M, N, K)
+                    assert np.array_equal(_unpack_mask(bits, M, N), _np(C) > 0)
+        for a, b in zip(out[3], out[4]):
+            assert torch.equal(a, b), (M, N, K, epi)
+
+
+def test_gemm_tcgen05_wide_tile_refuses_what_it_cannot_take():
+    """backend 4 never silently runs another kernel: N < 512 and the epilogues without a 256 x 512 instantiation
+    (bias alone, the ReLU-masked dgrad with column sums) are GPIPE_EINVAL."""
+    r = _rng(5)
+    At, _ = _lp(r.standard_normal((256, 128)), "bf16")
+    Bt, _ = _lp(r.standard_normal((128, 256)), "bf16")
+    C = torch.empty((256, 256), device=DEV, dtype=torch.bfloat16)
+    from paper_1811_06965_b200 import GPipeError
+    with pytest.raises(GPipeError):
+        ops.gemm(At, Bt, C, backend=4)
+    Bt, _ = _lp(r.standard_normal((128, 1024)), "bf16")
+    C = torch.empty((256, 1024), device=DEV, dtype=torch.bfloat16)
+    with pytest.raises(GPipeError):
+        ops.gemm(At, Bt, C, bias=torch.zeros(1024, device=DEV), backend=4)
+    ops.gemm(At, Bt, C, backend=4)
+
+
 def test_gemm_bf16_never_falls_back_silently():
     """A bf16 problem the tcgen05 kernel cannot take (row pitch not a multiple of 16 bytes; a ReLU pattern with
     N % 32 != 0) is GPIPE_EINVAL on the default backend, not a ~50x slower SIMT launch; backend 1 still runs it."""

@@ -65,6 +65,9 @@ def main():
     ap.add_argument("--reps", type=int, default=10)
     ap.add_argument("--json", default=None)
     ap.add_argument("--compare", action="store_true")
+    ap.add_argument("--gemm-backend", type=int, default=0,
+                    help="0: the launcher's own tile choice; 3: 256 x 256 pair tiles only; 4: 256 x 512 pair tiles only "
+                         "(shapes / epilogues the wide tile does not take are skipped)")
     args = ap.parse_args()
 
     import torch
@@ -132,8 +135,15 @@ def main():
             kw["workspace"] = ops.gemm_workspace(M, N, K, dev)
             if kw["workspace"] is None: kw["workspace"] = False
             sets.append((A, Bm, Cm, kw))
-        fns = [(lambda s=s: ops.gemm(s[0], s[1], s[2], transA=bool(tA), transB=bool(tB), **s[3])) for s in sets]
-        ms = time_it(fns, args.reps)
+        fns = [(lambda s=s: ops.gemm(s[0], s[1], s[2], transA=bool(tA), transB=bool(tB), backend=args.gemm_backend, **s[3]))
+               for s in sets]
+        try:
+            ms = time_it(fns, args.reps)
+        except Exception as e:                                 # backend 4 on a shape the wide tile does not take
+            if args.gemm_backend == 0:
+                raise
+            print("gemm   %-14s skipped (%s)" % (name, str(e).splitlines()[0][:60]), flush=True)
+            continue
         byts = per + (M * N * 4 if ep.get("resid") else 0) + (M * N * 4 if ep.get("accum") else 0) + \
             (M * N // 8 if ep.get("mask") or ep.get("bits") else 0)
         extra = {"M": M, "N": N, "K": K, "transA": tA, "transB": tB}

@@ -358,6 +358,44 @@ def test_gemm_tcgen05_bench_shapes_sampled(case):
         raise AssertionError(epi)
 
 
+# the launches of the list above that a handle with >= 8 cells (the bench workload: 16) sends to the 256 x 512 pair tile
+WIDE_BENCH_GEMMS = [c for c in BENCH_GEMMS if c[6] in ("plain_nows", "accum", "accum2") or (c[6] == "plain" and c[0] != "logits_dgrad")]
+
+
+@pytest.mark.parametrize("case", WIDE_BENCH_GEMMS, ids=[c[0] for c in WIDE_BENCH_GEMMS])
+def test_gemm_tcgen05_bench_shapes_wide_tile(case):
+    """The same full-size config-5 launches in the tile the 16-cell bench step actually runs them with: the
+    256 x 512 pair tile (backend 4) - plain bf16 output (logits, the dgrads of FFN1 / QKV / out-projection, the
+    unsplit dlogits W_out^T) and fp32 accumulate (FFN2 / out-projection forward, every wgrad).  24 sampled rows
+    against the fp64 product of the same operands, and the whole output bit for bit against the 256 x 256 tiles."""
+    name, M, N, K, tA, tB, epi = case
+    assert N % 512 == 0
+    r = _rng(sum(map(ord, name)) + 1)
+    At, Aq = _lp(r.standard_normal((K, M) if tA else (M, K), dtype=np.float32) * 0.5, "bf16")
+    Bt, Bq = _lp(r.standard_normal((N, K) if tB else (K, N), dtype=np.float32) * 0.5, "bf16")
+    rows = np.sort(r.choice(M, size=24, replace=False))
+    ref = (Aq.T[rows] if tA else Aq[rows]) @ (Bq.T if tB else Bq)
+    f32_tol = 1e-4 if K > 20000 else 2e-5
+    kw = dict(transA=bool(tA), transB=bool(tB), workspace=False)
+    out = {}
+    for backend in (4, 3):
+        if epi in ("plain", "plain_nows"):
+            C = torch.empty((M, N), device=DEV, dtype=torch.bfloat16)
+            ops.gemm(At, Bt, C, backend=backend, **kw)
+            if backend == 4:
+                assert maxrel(_np(C[rows]), ref) <= 2 ** -7 and cosine(_np(C[rows]), ref) >= 0.99999
+        else:
+            n_acc = 2 if epi == "accum2" else 1
+            c0 = r.standard_normal((M, N)).astype(np.float32) if backend == 4 else c0
+            C = torch.tensor(c0, device=DEV)
+            for _ in range(n_acc):
+                ops.gemm(At, Bt, C, accumulate=True, backend=backend, **kw)
+            if backend == 4:
+                assert maxrel(_np(C[rows]), c0[rows] + n_acc * ref) <= f32_tol
+        out[backend] = C
+    assert torch.equal(out[3], out[4])
+
+
 @pytest.mark.parametrize("dtype", ["fp32", "bf16"])
 @pytest.mark.parametrize("backend", [1, 0])
 def test_gemm_epilogues(dtype, backend):

@@ -100,14 +100,8 @@ __device__ __forceinline__ void tl_clock(const Params &, bool, int, int) {}
 template <int BN, int F> struct PairCfg {
   static constexpr int BNH = BN / 2;
   static constexpr uint32_t A_BYTES = 128 * BK * 2, B_BYTES = BNH * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;
-#ifndef GP_WIDE_STAGES
-#define GP_WIDE_STAGES 4
-#endif
-#ifndef GP_WIDE_STG
-#define GP_WIDE_STG 1
-#endif
-  static constexpr int STAGES = BN == 256 ? 5 : GP_WIDE_STAGES;
-  static constexpr int STG = BN == 256 ? 1 : GP_WIDE_STG;
+  static constexpr int STAGES = BN == 256 ? 5 : 4;   // BN 512 with 3 stages + a second staging buffer per warp: +8 ms per config-5 step
+  static constexpr int STG = 1;
   static constexpr uint32_t BIAS_BYTES = (BN == 256 && (F < 0 || (F & EPI_BIAS))) ? 2 * BN * 4 : 0;   // BN 512: bias from L1
   static constexpr uint32_t COLBUF_BYTES = (F < 0 || (F & EPI_COLSUM)) ? 4 * BN * 4 : 0;
   static constexpr uint32_t AUX_BYTES = BIAS_BYTES + COLBUF_BYTES;

@@ -539,6 +539,49 @@ def test_attention_fwd_bwd(dtype, S, A, dh, causal, backend):
             assert cosine(got[:, blk * da:(blk + 1) * da], ref) >= (cos if dtype == "fp32" else 0.9999), name
 
 
+@pytest.mark.parametrize("case", ["small", "large", "mixed_rows", "orthogonal_gap", "orthogonal_huge"])
+@pytest.mark.parametrize("causal", [0, 1])
+@pytest.mark.parametrize("S", [256, 200])
+def test_attention_forward_score_range(case, causal, S):
+    """softmax is invariant to the shift m in exp(s - m): whatever shift a kernel uses (the exact row maximum today; a
+    Cauchy-Schwarz bound |q_row| max_j |k_j| was measured in round 2), output and log-sum-exp
+    must match the oracle's plain definition over the whole range of scores: small and large (|s| ~ 100), rows of both
+    kinds inside one 128-row block, and q orthogonal to every k with norms far above the scores (where a norm-based
+    shift would underflow)."""
+    A, dh, n_seq = 2, 64, 2
+    da = A * dh
+    r = _rng(S + 7 * causal + len(case))
+    x = r.standard_normal((n_seq * S, 3 * da))
+    if case == "small":
+        x[:, :2 * da] *= 0.25
+    elif case == "large":
+        x[:, :2 * da] *= 3.0                              # |s| up to ~ 100
+    elif case == "mixed_rows":
+        x[40:72, :da] *= 4.0                              # 32 rows straddling two warps with 16x the scores
+        x[S + 130:S + 140, :da] *= 5.0
+    else:
+        c = 12.5 if case == "orthogonal_gap" else 40.0    # |q| |k| / sqrt(d_head) = 19.5 / 200, scores ~ 0
+        x[:, :2 * da] *= 0.01
+        for h in range(A):
+            x[:, h * dh] += c                             # q along e_0
+            x[:, da + h * dh + 1] += c                    # k along e_1
+    qkvt, qkvq = _lp(x, "bf16")
+    o = torch.empty((n_seq * S, da), device=DEV, dtype=torch.bfloat16)
+    lse = torch.empty((n_seq, A, S), device=DEV)
+    ops.attn_fwd(qkvt, o, lse, n_seq, S, A, dh, causal)
+    for b in range(n_seq):
+        rows = slice(b * S, (b + 1) * S)
+        q, k, v = qkvq[rows, :da], qkvq[rows, da:2 * da], qkvq[rows, 2 * da:]
+        o_ref, _ = go.attention_fwd(q, k, v, A, dh, causal)
+        assert maxrel(_np(o[rows]), o_ref) <= 2 ** -6, (case, b)
+        for h in range(A):
+            sc = (q[:, h * dh:(h + 1) * dh] @ k[:, h * dh:(h + 1) * dh].T) / math.sqrt(dh)
+            if causal:
+                sc = np.where(np.tril(np.ones((S, S), bool)), sc, -np.inf)
+            lse_ref = np.log(np.exp(sc - sc.max(1, keepdims=True)).sum(1)) + sc.max(1)
+            assert np.abs(_np(lse[b, h]) - lse_ref).max() <= 1e-4 * max(1.0, np.abs(lse_ref).max()), (case, b, h)
+
+
 @pytest.mark.parametrize("S,A", [(256, 3), (200, 2), (100, 2), (64, 1)])
 @pytest.mark.parametrize("causal", [0, 1])
 def test_attention_backward_fused_column_sums(S, A, causal):

@@ -93,6 +93,17 @@ int gpipe_op_softmax_ce(void *stream, int dtype, void *logits, const int32_t *la
 int64_t gpipe_op_colsum_scratch_floats(int64_t n_tok, int n);
 int gpipe_op_colsum(void *stream, int dtype, const void *dy, int64_t ld, float *out, float *scratch,
                     int64_t n_tok, int n);
+/* The same column sums for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): out[n] += sum_t dy[t,n] with the kernels' scratch in a file-scope
+ * __device__ array inside the library (2 MiB, held by every GPU that loads the library until the process exits)
+ * instead of a caller-owned buffer.  Same kernels, same summation order: results are bitwise those of gpipe_op_colsum.
+ * dy: device, dtype elements [n_tok, ld]; out: device fp32 [n], accumulated into; both caller-owned.  n <=
+ * GPIPE_COLSUM_STATIC_MAX_N, wider inputs return GPIPE_EINVAL (message names the limit).  The call allocates nothing
+ * (no cudaMalloc / cudaFree / allocating library routine) and runs on the current device.  All calls share the one
+ * array per device: calls that overlap on the GPU (different streams) race - serialise them, or use gpipe_op_colsum
+ * with one scratch buffer per stream.  Nothing in the array has to be cleared between calls. */
+#define GPIPE_COLSUM_STATIC_MAX_N 16384
+int gpipe_op_colsum_static(void *stream, int dtype, const void *dy, int64_t ld, float *out, int64_t n_tok, int n);
 /* x[t,:] = emb[tok[t],:] + pe[t mod S,:];  gemb[tok[t],:] += dx[t,:] */
 int gpipe_op_embed_fwd(void *stream, int dtype, const int32_t *tok, const void *emb, const float *pe,
                        float *x, int64_t n_tok, int S, int d);

@@ -145,6 +145,7 @@ def lib() -> C.CDLL:
         "gpipe_op_softmax_ce": (i32, [vp, i32, vp, vp, vp, i64, i32, f32, f32]),
         "gpipe_op_colsum_scratch_floats": (i64, [i64, i32]),
         "gpipe_op_colsum": (i32, [vp, i32, vp, i64, vp, vp, i64, i32]),
+        "gpipe_op_colsum_static": (i32, [vp, i32, vp, i64, vp, i64, i32]),
         "gpipe_op_embed_fwd": (i32, [vp, i32, vp, vp, vp, vp, i64, i32, i32]),
         "gpipe_op_embed_bwd": (i32, [vp, vp, vp, vp, i64, i32]),
         "gpipe_op_positional": (i32, [vp, vp, i32, i32]),
@@ -174,7 +175,7 @@ EXPORTED_SYMBOLS = [
     "gpipe_trace", "gpipe_launch_count", "gpipe_cuda_graph", "gpipe_cuda_graph_state", "gpipe_kernel_timing", "gpipe_kernel_stats", "gpipe_debug_read", "gpipe_last_error", "gpipe_version",
     "gpipe_op_gemm", "gpipe_op_gemm_workspace_bytes", "gpipe_op_ln_fwd", "gpipe_op_ln_bwd_scratch_floats", "gpipe_op_ln_bwd",
     "gpipe_op_attn_fwd", "gpipe_op_attn_bwd", "gpipe_op_softmax_ce", "gpipe_op_colsum",
-    "gpipe_op_colsum_scratch_floats",
+    "gpipe_op_colsum_scratch_floats", "gpipe_op_colsum_static",
     "gpipe_op_embed_fwd", "gpipe_op_embed_bwd", "gpipe_op_positional", "gpipe_op_sgd", "gpipe_op_dp_apply_sgd",
 ]
 

@@ -17,7 +17,7 @@ CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libgpipe_b200.so")
 OBJ = os.path.join(HERE, "build")
 SOURCES = ["api.cu", "engine.cu", "ops_api.cu", "kernels_rowwise.cu", "kernels_misc.cu",
-           "gemm_simt.cu", "attention_simt.cu", "attention_mma.cu", "attention_tcgen05.cu", "gemm_tcgen05.cu"]
+           "gemm_simt.cu", "attention_simt.cu", "attention_mma.cu", "attention_tcgen05.cu", "gemm_tcgen05.cu", "no_alloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]
 # extra compile flags, e.g. GPIPE_NVCC_EXTRA="-DGP_WATCHDOG=1" (bounded mbarrier waits with a diagnosis)

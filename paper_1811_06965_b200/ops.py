@@ -108,6 +108,16 @@ def colsum(dy, out):
     B._check(B.lib().gpipe_op_colsum(_stream(), _dt(dy), _p(dy), dy.stride(0), _p(out), _p(scratch), n, c))
 
 
+COLSUM_STATIC_MAX_N = 16384
+
+
+def colsum_static(dy, out):
+    """out[n] += sum_t dy[t, n] through gpipe_op_colsum_static: no device allocation anywhere (the scratch is a static
+    array inside the library); at most COLSUM_STATIC_MAX_N columns; calls that overlap on the GPU race on it."""
+    n, c = dy.shape
+    B._check(B.lib().gpipe_op_colsum_static(_stream(), _dt(dy), _p(dy), dy.stride(0), _p(out), n, c))
+
+
 def embed_fwd(tok, emb, pe, x, S):
     n, d = x.shape
     B._check(B.lib().gpipe_op_embed_fwd(_stream(), _dt(emb), _p(tok), _p(emb), _p(pe), _p(x), n, S, d))

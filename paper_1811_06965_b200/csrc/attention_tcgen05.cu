@@ -81,7 +81,10 @@ __device__ __forceinline__ uint32_t panel_addr(uint32_t panel, int r, int c) {
 // ---------------------------------------------------------------------------------------------
 // forward
 // ---------------------------------------------------------------------------------------------
-// shared memory (from a 1024-byte aligned base): Q [0,16K) | K [16K,48K) | pad [48K,64K) | V [64K,96K).
+// One CTA = one (sequence, head): its query blocks of 128 rows one after the other (qpb = 2; qpb = 1: one block per CTA),
+// K and V loaded once; the score product of block b + 1 is issued as soon as every thread holds block b's output in
+// registers, so the output stores run under it.
+// shared memory (from a 1024-byte aligned base): Q_0 [0,16K) | K [16K,48K) | Q_1 [48K,64K) | V [64K,96K).
 // TMEM (256 columns): S in [0, N).  The thread pair of a row splits the 32-key chunks [0, split) / [split, nch); P chunk
 // c (16 columns of bf16 pairs) goes to column 16 c for the first half and to 32 split + 16 (c - split) for the second:
 // always inside score columns its own thread has already read in this pass (chunk c's P lies in chunk <= c of the same
@@ -96,7 +99,7 @@ constexpr int FWD_THREADS = 256;
 
 __global__ void __launch_bounds__(FWD_THREADS, 2)
 attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict__ o, float *__restrict__ lse, int S,
-                   int A, int causal, float scale, unsigned long long *tl) {
+                   int A, int causal, float scale, int qpb, unsigned long long *tl) {
   extern __shared__ uint8_t smem_raw[];
   // optional timeline probe (attn_tc_set_timeline): 8 %globaltimer stamps per CTA, written by thread 0
   auto stamp = [&](int slot) {
@@ -111,7 +114,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
 #endif
   };
   stamp(0);
-  __shared__ __align__(8) uint64_t bars[4];
+  __shared__ __align__(8) uint64_t bars[5];
   __shared__ uint32_t tmem_base_smem;
   __shared__ float xm[2][128], xl[2][128];
   const uint32_t sb = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -119,15 +122,16 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int quad = warp & 3, chalf = warp >> 2;
   const int da = A * DH, seq = blockIdx.y / A, h = blockIdx.y - seq * A;
-  const int q0 = blockIdx.x * 128;
-  const int nk = causal ? min(S, q0 + 128) : S;          // keys this block can see
-  const int nkb = (nk + 127) >> 7;
-  const int N = (nk + 15) & ~15;                         // MMA N of the score product / K of P V
+  // this CTA's query blocks [qb0, qb1) of 128 rows (qpb per CTA: 1, or 2 = the whole (sequence, head) for S <= 256 with
+  // K and V loaded once) and the key tiles the last of them sees
+  const int qb0 = blockIdx.x * qpb, qb1 = min((S + 127) >> 7, qb0 + qpb);
+  const int nk_all = causal ? min(S, qb1 * 128) : S;
+  const int nkb_all = (nk_all + 127) >> 7;
   const uint32_t bar_qk = smem_u32(&bars[0]), bar_v = smem_u32(&bars[1]), bar_s = smem_u32(&bars[2]),
-                 bar_o = smem_u32(&bars[3]);
+                 bar_o = smem_u32(&bars[3]), bar_q1 = smem_u32(&bars[4]);
   if (threadIdx.x == 0) {
     tma_prefetch_desc(&map_qkv);
-    for (int i = 0; i < 4; ++i) mbar_init(bar_qk + 8 * i, 1);
+    for (int i = 0; i < 5; ++i) mbar_init(bar_qk + 8 * i, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {
@@ -140,20 +144,40 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
   const uint32_t tmem = tmem_base_smem;
 
   if (threadIdx.x == 0) {
-    mbar_expect_tx(bar_qk, (1 + nkb) * TILE);
-    tma_load_3d(sQ, &map_qkv, bar_qk, h * DH, q0, seq);
-    for (int b = 0; b < nkb; ++b) tma_load_3d(sK + b * TILE, &map_qkv, bar_qk, da + h * DH, b * 128, seq);
-    mbar_expect_tx(bar_v, nkb * TILE);
-    for (int b = 0; b < nkb; ++b) tma_load_3d(sV + b * TILE, &map_qkv, bar_v, 2 * da + h * DH, b * 128, seq);
-    mbar_wait(bar_qk, 0, 0x21);
+    mbar_expect_tx(bar_qk, (1 + nkb_all) * TILE);
+    tma_load_3d(sQ, &map_qkv, bar_qk, h * DH, qb0 * 128, seq);
+    for (int b = 0; b < nkb_all; ++b) tma_load_3d(sK + b * TILE, &map_qkv, bar_qk, da + h * DH, b * 128, seq);
+    mbar_expect_tx(bar_v, nkb_all * TILE);
+    for (int b = 0; b < nkb_all; ++b) tma_load_3d(sV + b * TILE, &map_qkv, bar_v, 2 * da + h * DH, b * 128, seq);
+    if (qb1 - qb0 > 1) {                                 // the second query block: into the 16 KB between K and V
+      mbar_expect_tx(bar_q1, TILE);
+      tma_load_3d(sb + 3 * TILE, &map_qkv, bar_q1, h * DH, (qb0 + 1) * 128, seq);
+    }
+  }
+  // S = Q_b K^T of query block b into TMEM columns [0, N_b) (thread 0): block qb0 before the loop, block b + 1 as soon as
+  // every thread holds block b's output in registers - its global stores then run under the next score product
+  auto issue_scores = [&](int b) {
+    const int it_ = b - qb0;
+    const int nk_ = causal ? min(S, b * 128 + 128) : S;
+    mbar_wait(it_ ? bar_q1 : bar_qk, 0, 0x21);
     tcgen05_fence_after();
-    stamp(1);
-    const uint32_t id = idesc(0, 0, N);
+    const uint32_t id = idesc(0, 0, (nk_ + 15) & ~15);
+    const uint32_t sQb = it_ ? sb + 3 * TILE : sQ;
 #pragma unroll
-    for (int ks = 0; ks < DH / 16; ++ks) umma_bf16(tmem, desc_k(sQ, ks), desc_k(sK, ks), id, ks ? 1u : 0u);
+    for (int ks = 0; ks < DH / 16; ++ks) umma_bf16(tmem, desc_k(sQb, ks), desc_k(sK, ks), id, ks ? 1u : 0u);
     tcgen05_commit(bar_s);
+  };
+  if (threadIdx.x == 0) {
+    issue_scores(qb0);
+    stamp(1);
   }
   __syncwarp();
+  for (int qb = qb0; qb < qb1; ++qb) {
+  const int it = qb - qb0;
+  const uint32_t par = (uint32_t)(it & 1);               // bar_s / bar_o complete once per query block
+  const int q0 = qb * 128;
+  const int nk = causal ? min(S, q0 + 128) : S;          // keys this block can see
+  const int N = (nk + 15) & ~15;                         // MMA N of the score product / K of P V
 
   // ---- softmax: this thread's row, this half's chunks ----
   const int r_loc = quad * 32 + lane, row = q0 + r_loc;
@@ -166,7 +190,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
   const int cv = min(c1, (kvis_w + 31) >> 5);                        // chunks [c0, cv) hold visible keys
   // chunk c needs per-element masking when it reaches past the first row's diagonal or past nk
   auto edge = [&](int c) { return c * 32 + 32 > nk || (causal && c * 32 + 31 > q0 + quad * 32); };
-  mbar_wait(bar_s, 0, 0x22);
+  mbar_wait(bar_s, par, 0x22);
   tcgen05_fence_after();
   stamp(2);
   uint32_t ra[32], rb[32];
@@ -253,11 +277,18 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
   }
   __syncwarp();
   l = xl[0][r_loc] + xl[1][r_loc];
-  mbar_wait(bar_o, 0, 0x24);
+  mbar_wait(bar_o, par, 0x24);
   tcgen05_fence_after();
   stamp(5);
   tmem_ld32(t_row + ocol + chalf * 32, ra);               // this thread's 32 of the row's 64 output columns
   tmem_ld_wait();
+  if (qb + 1 < qb1) {                                    // every thread has read its part of O: the columns are free
+    tcgen05_fence_before();
+    __syncthreads();
+    tcgen05_fence_after();
+    if (threadIdx.x == 0) issue_scores(qb + 1);
+    __syncwarp();
+  }
   if (row < S) {
     const float inv = 1.f / l;
     uint4 *dst = reinterpret_cast<uint4 *>(o + ((int64_t)seq * S + row) * da + h * DH + chalf * 32);
@@ -270,6 +301,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap map_qkv, bf16 *__restrict
     if (chalf == 0) lse[((int64_t)seq * A + h) * S + row] = mx * scale + logf(l);
   }
   stamp(6);
+  }                                                      // qb
   tcgen05_fence_before();
   __syncthreads();
   if (warp == 1) {
@@ -680,9 +712,15 @@ cudaError_t attn_fwd_tc(const Ctx &c, const void *qkv, void *o, float *lse, int 
     cudaError_t e = ensure_dyn_smem<fat::attn_fwd_tc_kernel>(fat::FWD_SMEM, c.device);
     if (e != cudaSuccess) return e;
   }
-  dim3 grid((S + 127) / 128, n_seq * A);
+  // One CTA per (sequence, head) walks both 128-row query blocks (S <= 256) with K and V loaded once: 256 CTAs of the
+  // config-5 micro-batch are ONE wave at two CTAs per SM (512 one-block CTAs were 1.73), and a third less operand
+  // traffic.  Alone the launch takes the same 20.5 us (two serial chains per CTA); in the step, where SM-time counts,
+  // config 5 measured 1406.3 / 1406.9 ms against 1415.3 / 1416.4 ms with one block per CTA (qpb = 1).
+  const int qpb = 2;
+  const int nqb = (S + 127) / 128;
+  dim3 grid((nqb + qpb - 1) / qpb, n_seq * A);
   fat::attn_fwd_tc_kernel<<<grid, fat::FWD_THREADS, fat::FWD_SMEM, c.stream>>>(mq, (bf16 *)o, lse, S, A, causal,
-                                                                              1.f / sqrtf((float)fat::DH), fat::g_attn_tl);
+                                                                              1.f / sqrtf((float)fat::DH), qpb, fat::g_attn_tl);
   GP_LAUNCH_CHECK(c);
 }
 

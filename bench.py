@@ -310,12 +310,13 @@ def run_ours(args, w, rank, world, local_rank):
     torch.cuda.reset_peak_memory_stats(dev)
     pipe_devices = [int(x) for x in args.pipeline_devices.split(",")] if args.pipeline_devices else None
     if w.n_dec:          # the encoder-decoder T(L,H,A): equal split, depth-scaled FFN init
-        eng = gp.from_workload(w, device=dev)
+        eng = gp.from_workload(w, device=dev, side_streams={'auto': None, 'on': True, 'off': False}[args.side_streams])
         eng.init_params(seed=1000 + rank, std=0.02, parity=False, ffn_scale=1.0 / w.n_layers)
         ids = gi.make_tokens_encdec(w, 2000 + rank)
     else:
         eng = gp.from_workload(w, device=dev, partition=None if args.partition == "equal" else args.partition,
-                               devices=pipe_devices, staged=bool(pipe_devices) and args.pipeline_staged)
+                               devices=pipe_devices, staged=bool(pipe_devices) and args.pipeline_staged,
+                               side_streams={'auto': None, 'on': True, 'off': False}[args.side_streams])
         eng.init_params(seed=1000 + rank, std=0.02, parity=False)
         ids = gi.make_tokens(w, 2000 + rank)
     progress("engine ready (%.1f GB arena)" % (eng.peak_bytes()["total"] / 1e9))
@@ -450,6 +451,7 @@ def run_ours(args, w, rank, world, local_rank):
                        "layers_per_cell": [hi - lo for lo, hi in eng.cells],
                        "parallelism": ("pipeline over devices %s%s" % (pipe_devices, " (staged boundary copies)" if args.pipeline_staged else ""))
                        if pipe_devices else ("replicas" if world > 1 else "1 GPU, K streams"),
+                       "side_streams": bool(getattr(eng, "side_streams", False)),
                        "l2": "inputs larger than L2 (activations+weights per step >> 126 MB)"},
             "loss": loss,
             "tflops_executed": fl["executed"] / step_s / 1e12, "tflops_model": fl["model"] / step_s / 1e12,
@@ -498,6 +500,9 @@ def main():
                          "(gpipe_create_pipeline; PAPER.md:65) from THIS process; ordinals may repeat")
     ap.add_argument("--pipeline-staged", action="store_true", help="force staged boundary copies when cells share a device")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--side-streams", choices=("auto", "on", "off"), default="auto",
+                    help="a second stream per cell for the weight-gradient GEMMs (gpipe_env.n_streams = 2K); auto: the "
+                         "binding's default (on for K <= 2)")
     ap.add_argument("--oracle-full", action="store_true",
                     help="cpu_baseline / --impl reference: one WHOLE oracle step of the workload instead of the bounded "
                          "sample (config 2: minutes; BASELINE.md section 3)")

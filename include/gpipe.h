@@ -88,7 +88,10 @@ typedef struct {
 typedef struct {
   void   *arena;        /* device, >= gpipe_plan_bytes(), 1024-byte aligned                    */
   size_t  arena_bytes;
-  void *const *streams; /* host array of n_streams cudaStream_t, one per cell (n_streams >= K) */
+  void *const *streams; /* host array of n_streams cudaStream_t, one per cell (n_streams >= K).
+                         * n_streams >= 2K: streams[K + k] is cell k's second stream - the weight-gradient
+                         * GEMMs of B(k,m) run there, beside the cell's dgrad / LayerNorm / attention chain
+                         * (same kernels, same accumulation order: bitwise the same gradients)          */
   int32_t n_streams;
 } gpipe_env;
 

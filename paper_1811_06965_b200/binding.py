@@ -267,7 +267,7 @@ class GPipe:
 
     def __init__(self, *, n_layers, d_model, d_ffn, n_heads, d_head, vocab, seq_len, dtype, K, M,
                  remat=True, n_seqs, causal=None, ln_eps=1e-5, device="cuda:0", partition=None, devices=None,
-                 staged=False):
+                 staged=False, side_streams=None):
         import torch
         if not torch.cuda.is_available():
             raise GPipeError(-2, "no CUDA device: the GPipe path has no CPU fallback")
@@ -278,6 +278,10 @@ class GPipe:
         self.K, self.M, self.remat, self.n_seqs, self.seq_len = K, M, bool(remat), n_seqs, seq_len
         self._h = C.c_void_p(None)
         self.devices = None if devices is None else [int(d) for d in devices]
+        # gpipe_env.n_streams = 2K: each cell's weight-gradient GEMMs run beside its dgrad / LayerNorm / attention chain.
+        # None: on for K <= 2 - with more cells on the GPU the other cells' kernels already fill the SMs a cell's
+        # narrow launches leave idle (measured: K 2 -3 %, K 4 +2 %, K 8 / 16 +-0.5 %)
+        self.side_streams = (K <= 2 if side_streams is None else bool(side_streams)) and devices is None
         if self.devices is not None:
             self._create_pipeline(torch, K, M, n_seqs, partition, staged)
         else:
@@ -318,9 +322,11 @@ class GPipe:
             nbytes = plan_bytes(self.spec, K, M, remat, n_seqs)
             self.arena = torch.empty(nbytes + 1024, dtype=torch.uint8, device=self.device)
             base = (self.arena.data_ptr() + 1023) // 1024 * 1024
-            self.streams = [torch.cuda.Stream(device=self.device) for _ in range(K)]
-            self._stream_arr = (C.c_void_p * K)(*[s.cuda_stream for s in self.streams])
-            env = Env(base, nbytes, C.cast(self._stream_arr, C.POINTER(C.c_void_p)), K)
+            ns = 2 * K if self.side_streams else K
+            self._all_streams = [torch.cuda.Stream(device=self.device) for _ in range(ns)]
+            self.streams = self._all_streams[:K]
+            self._stream_arr = (C.c_void_p * ns)(*[s.cuda_stream for s in self._all_streams])
+            env = Env(base, nbytes, C.cast(self._stream_arr, C.POINTER(C.c_void_p)), ns)
             torch.cuda.synchronize(self.device)
             if partition is None:
                 _check(lib().gpipe_create(C.byref(self.spec), K, M, int(self.remat), n_seqs, C.byref(env),
@@ -591,7 +597,8 @@ class GPipeEncDec(GPipe):
     layers.  logit_clip: PAPER.md:174 (0 = off)."""
 
     def __init__(self, *, n_enc, n_dec, d_model, d_ffn, n_heads, d_head, vocab, seq_len, dtype, K, M, remat=True,
-                 n_seqs, ln_eps=1e-5, logit_clip=0.0, device="cuda:0", partition=None, devices=None, staged=False):
+                 n_seqs, ln_eps=1e-5, logit_clip=0.0, device="cuda:0", partition=None, devices=None, staged=False,
+                 side_streams=None):
         import torch
         if not torch.cuda.is_available():
             raise GPipeError(-2, "no CUDA device: the GPipe path has no CPU fallback")
@@ -602,6 +609,7 @@ class GPipeEncDec(GPipe):
         self.K, self.M, self.remat, self.n_seqs, self.seq_len = K, M, bool(remat), n_seqs, seq_len
         self._h = C.c_void_p(None)
         self.devices = None if devices is None else [int(d) for d in devices]
+        self.side_streams = (K <= 2 if side_streams is None else bool(side_streams)) and devices is None
         if isinstance(partition, str):
             if partition != "cost":
                 raise ValueError("partition must be None, 'cost' or a list of K+1 boundaries")
@@ -634,9 +642,11 @@ class GPipeEncDec(GPipe):
             nbytes = plan_bytes_encdec(self.spec, K, M, remat, n_seqs, partition)
             self.arena = torch.empty(nbytes + 1024, dtype=torch.uint8, device=self.device)
             base = (self.arena.data_ptr() + 1023) // 1024 * 1024
-            self.streams = [torch.cuda.Stream(device=self.device) for _ in range(K)]
-            self._stream_arr = (C.c_void_p * K)(*[s.cuda_stream for s in self.streams])
-            env = Env(base, nbytes, C.cast(self._stream_arr, C.POINTER(C.c_void_p)), K)
+            ns = 2 * K if self.side_streams else K
+            self._all_streams = [torch.cuda.Stream(device=self.device) for _ in range(ns)]
+            self.streams = self._all_streams[:K]
+            self._stream_arr = (C.c_void_p * ns)(*[s.cuda_stream for s in self._all_streams])
+            env = Env(base, nbytes, C.cast(self._stream_arr, C.POINTER(C.c_void_p)), ns)
             torch.cuda.synchronize(self.device)
             _check(lib().gpipe_create_encdec(C.byref(self.spec), K, M, int(self.remat), n_seqs, C.byref(env), lo,
                                              C.byref(self._h)))

@@ -384,6 +384,11 @@ static int create_impl(const gpipe_layer_spec *spec, int K, int M, int remat, in
   if (rc) { cudaSetDevice(dev_entry); delete g; return rc; }
   e.streams.resize(K);
   for (int k = 0; k < K; ++k) e.streams[k] = (cudaStream_t)(pipe ? cells[k].stream : env->streams[k]);
+  if (!pipe && env->n_streams >= 2 * K) {                      // a second stream per cell: weight gradients beside the chain
+    e.side.resize(K);
+    for (int k = 0; k < K; ++k) e.side[k] = (cudaStream_t)env->streams[K + k];
+    e.side_tail.assign(K, nullptr);
+  }
   e.ev_f.assign(K, std::vector<cudaEvent_t>(e.M, nullptr));
   e.ev_b.assign(K, std::vector<cudaEvent_t>(e.M, nullptr));
   e.ev_done.assign(K, nullptr);

@@ -492,8 +492,38 @@ cudaError_t Engine::backward_cell(int k, int m) {
   int cur = 0;                // which ping-pong buffer the NEXT producer writes
   const double lpb = (double)lp_size(dt);
   const double Td = (double)T_mb;
+  // Side stream (engine.h): a weight-gradient GEMM goes to side[k] behind an event that orders it after everything
+  // the main stream has enqueued so far.  Its X operand is an interior activation (next written by the cell's next
+  // task, which waits for side_tail[k]); its dY operand is scratch of this task: `pend` holds, per such buffer, the
+  // event of the last side-stream GEMM reading it, and `guard` makes the main stream wait for it before a kernel
+  // that overwrites the buffer is enqueued.  The side stream is in-order, so one wait covers every earlier GEMM.
+  const bool sideon = side_active();
+  Ctx cside = c;
+  if (sideon) cside.stream = side[k];
+  struct Pend { const void *buf; cudaEvent_t ev; int seq; };
+  Pend pend[8];
+  int npend = 0, side_seq = 0, waited_seq = 0;
+  cudaEvent_t tail = nullptr;
+  auto guard = [&](const void *buf) -> cudaError_t {
+    if (!buf) return cudaSuccess;
+    for (int i = 0; i < npend; ++i)
+      if (pend[i].buf == buf) {
+        const int sq = pend[i].seq;
+        GP_TRY(cudaStreamWaitEvent(c.stream, pend[i].ev, 0));
+        if (sq > waited_seq) waited_seq = sq;
+        int n = 0;
+        for (int j = 0; j < npend; ++j)
+          if (pend[j].seq > waited_seq) pend[n++] = pend[j];
+        npend = n;
+        if (side_seq == waited_seq) tail = nullptr;
+        break;
+      }
+    return cudaSuccess;
+  };
   auto tlnb = [&](const void *dy_, const float *x_, const float *mu_, const float *rs_, const float *g_,
                   const float *dres_, float *dxo_, void *dxlp_, float *dg_, float *db_, float *cs_) -> cudaError_t {
+    GP_TRY(guard(dxo_));
+    GP_TRY(guard(dxlp_));
     double by = Td * d * (lpb + 4.0 + (dres_ ? 4.0 : 0.0) + 4.0 + (dxlp_ ? lpb : 0.0));
     return timed(k, KC_LN_BWD, 0, by, [&] {
       return ln_bwd(c, dt, dy_, x_, mu_, rs_, g_, dres_, dxo_, dxlp_, s.ln_partials, dg_, db_, cs_, T_mb, d);
@@ -508,14 +538,34 @@ cudaError_t Engine::backward_cell(int k, int m) {
     return timed(k, KC_COLSUM, 0, Td * n_ * lpb, [&] { return colsum_accum(c, dt, dy_, ld_, out_, s.colsum_scratch, T_mb, n_); });
   };
   auto wgrad = [&](const void *X, int64_t ldx, int Min, const void *dY, int64_t ldy, int Nout,
-                   int iw) -> cudaError_t {
+                   int iw, bool may_side = true) -> cudaError_t {
     GemmArgs g{};
     g.M = Min; g.N = Nout; g.K = (int)T_mb;
     g.A = X; g.lda = ldx; g.transA = 1; g.B = dY; g.ldb = ldy; g.transB = 0;
     g.C = G(iw); g.ldc = Nout; g.flags = EPI_ACCUM | EPI_OUT_F32;
     g.ws = s.splitk_ws; g.ws_bytes = splitk_ws_bytes;
     double by = ((double)g.M * g.K + (double)g.K * g.N) * lpb + (double)g.M * g.N * 8.0;
-    return timed(k, KC_GEMM_WGRAD, 2.0 * g.M * g.N * (double)g.K, by, [&] { return gemm(c, dt, g); });
+    // a split-K product needs the cell's one split-K workspace, which the main stream's GEMMs use: it stays there
+    if (!sideon || !may_side || (dt == GP_BF16 && gemm_splitk_ws_bytes(g.M, g.N, g.K, sm_count) != 0))
+      return timed(k, KC_GEMM_WGRAD, 2.0 * g.M * g.N * (double)g.K, by, [&] { return gemm(c, dt, g); });
+    cudaEvent_t fork = pool_event(), done = pool_event();
+    if (!fork || !done) return pool_err;
+    GP_TRY(cudaEventRecord(fork, c.stream));
+    GP_TRY(cudaStreamWaitEvent(cside.stream, fork, 0));
+    g.ws = nullptr; g.ws_bytes = 0;
+    GP_TRY(timed_on(cside.stream, KC_GEMM_WGRAD, 2.0 * g.M * g.N * (double)g.K, by, [&] { return gemm(cside, dt, g); }));
+    GP_TRY(cudaEventRecord(done, cside.stream));
+    tail = done;
+    ++side_seq;
+    int slot_i = npend;
+    for (int i = 0; i < npend; ++i)
+      if (pend[i].buf == dY) slot_i = i;
+    if (slot_i == npend) {
+      if (npend == 8) return cudaErrorUnknown;             // cannot happen: at most six distinct dY buffers per task
+      ++npend;
+    }
+    pend[slot_i] = Pend{dY, done, side_seq};
+    return cudaSuccess;
   };
   auto dgrad = [&](const void *dY, int64_t ldy, int Kout, int iw, int Nin, void *dX,
                    uint32_t *mask, float *colsum_to = nullptr) -> cudaError_t {
@@ -525,6 +575,7 @@ cudaError_t Engine::backward_cell(int k, int m) {
     g.C = dX; g.ldc = Nin; g.mask = mask; g.ldmask = (Nin + 31) / 32; g.flags = mask ? EPI_MASK : 0;
     if (colsum_to) { g.flags |= EPI_COLSUM; g.colsum_out = colsum_to; g.colsum_scratch = s.colsum_scratch; }
     g.ws = s.splitk_ws; g.ws_bytes = splitk_ws_bytes;
+    GP_TRY(guard(dX));
     double by = ((double)g.M * g.K + (double)g.K * g.N + (double)g.M * g.N) * lpb + (mask ? (double)g.M * g.N / 8.0 : 0.0);
     return timed(k, KC_GEMM_DGRAD, 2.0 * g.M * g.N * (double)g.K, by, [&] { return gemm(c, dt, g); });
   };
@@ -548,6 +599,7 @@ cudaError_t Engine::backward_cell(int k, int m) {
     // this cell does it itself
     if (multi() && nl > 0) GP_TRY(tcol(dxo, d, G(lp[cell_hi[k] - 1].b_2), d));
   }
+  const void *dxo_in = dxo;   // (a boundary-ring entry when k < K-1: the next cell overwrites it after this task's event)
   // encoder-decoder: gradient of the second member of the pair.  In the decoder it is the gradient of the memory:
   // every decoder layer's cross-attention adds dkv W_kv^T to it (fp32) - the first one of the cell on top of what the
   // next cell handed down (nothing, in the last cell), the others in place.  In the encoder it is the gradient of the
@@ -589,7 +641,8 @@ cudaError_t Engine::backward_cell(int k, int m) {
       // cross-attention block: do2 = dx1c W_o2^T; dW_o2 += o2^T dx1c; attention backward over [q2 | k2 | v2]
       const size_t kv_off = (size_t)da * lp_size(dt);
       GP_TRY(dgrad(dxo, d, d, q.w_o2, da, s.d_o, nullptr));
-      GP_TRY(wgrad(b.o2, da, da, dxo, d, d, q.w_o2));
+      GP_TRY(wgrad(b.o2, da, da, dxo, d, d, q.w_o2, false));      // the cross-attention block's three stay on the main stream
+      GP_TRY(guard(s.dqkv));
       GP_TRY(timed(k, KC_ATTN_BWD, 10.0 * Td * S * da, Td * 8.0 * da * lpb,
                    [&] { return attn_bwd(c, dt, b.qkv2, b.o2, s.d_o, b.lse2, s.dqkv, s.dvec, (int)nb, S, A, dh, 0,
                                          fused_cs ? s.colsum_scratch : nullptr); }));
@@ -599,7 +652,7 @@ cudaError_t Engine::backward_cell(int k, int m) {
       }
       // queries: dcx = dq2 W_q^T; dW_q += cx^T dq2; db_q += sum_t dq2
       GP_TRY(dgrad(s.dqkv, 3 * da, da, q.w_q, d, s.dc, nullptr));
-      GP_TRY(wgrad(b.cx, d, d, s.dqkv, 3 * da, da, q.w_q));
+      GP_TRY(wgrad(b.cx, d, d, s.dqkv, 3 * da, da, q.w_q, false));
       if (!fused_cs) GP_TRY(tcol(s.dqkv, 3 * da, G(q.b_q), da));
       // keys / values: dmem += dkv W_kv^T (fp32); dW_kv += mem^T dkv; db_kv += sum_t dkv
       {
@@ -614,7 +667,7 @@ cudaError_t Engine::backward_cell(int k, int m) {
         GP_TRY(timed(k, KC_GEMM_DGRAD, 2.0 * g.M * g.N * (double)g.K, by, [&] { return gemm(c, dt, g); }));
         daux_started = true;
       }
-      GP_TRY(wgrad(mem, d, d, (const char *)s.dqkv + kv_off, 3 * da, 2 * da, q.w_kv));
+      GP_TRY(wgrad(mem, d, d, (const char *)s.dqkv + kv_off, 3 * da, 2 * da, q.w_kv, false));
       if (!fused_cs) GP_TRY(tcol((const char *)s.dqkv + kv_off, 3 * da, G(q.b_kv), 2 * da));
       // LN_x backward: dx1 = dx1c + LN_x'(dcx); db_o += sum_t dx1
       GP_TRY(tlnb(s.dc, b.x1, b.meanx, b.rstdx, P(q.lnx_g), dx, s.dx[cur],
@@ -628,6 +681,7 @@ cudaError_t Engine::backward_cell(int k, int m) {
     GP_TRY(wgrad(b.o, da, da, dxo, d, d, q.w_o));
     // db_qkv += sum_t dqkv: the tcgen05 attention backward leaves per-sequence column sums of what it stores (one small
     // reduction over the nb sequences follows); the other backends take the separate pass over dqkv
+    GP_TRY(guard(s.dqkv));
     GP_TRY(timed(k, KC_ATTN_BWD, 10.0 * Td * S * da * (causal[l] ? (S + 1.0) / (2.0 * S) : 1.0), Td * 8.0 * da * lpb,
                  [&] { return attn_bwd(c, dt, b.qkv, b.o, s.d_o, b.lse, s.dqkv, s.dvec, (int)nb, S, A, dh, causal[l],
                                        fused_cs ? s.colsum_scratch : nullptr); }));
@@ -672,6 +726,10 @@ cudaError_t Engine::backward_cell(int k, int m) {
     else GP_TRY(timed(k, KC_EMBED, 0, Td * d * 12.0, [&] { return embed_bwd(c, tgt_dev + (int64_t)m * T_mb, daux_in, G(i_emb), T_mb, d); }));
   } else if (encdec() && k == 0) {                                     // cell 0 holds the transition
     GP_TRY(timed(k, KC_EMBED, 0, Td * d * 12.0, [&] { return embed_bwd(c, tgt_dev + (int64_t)m * T_mb, s.dtgt, G(i_emb), T_mb, d); }));
+  }
+  if (sideon) {
+    GP_TRY(guard(dxo_in));
+    side_tail[k] = tail;
   }
   if (multi() && k > 0) {
     // backward boundary transfer: the gradient wrt this cell's input becomes the previous cell's output gradient
@@ -718,6 +776,10 @@ cudaError_t Engine::enqueue_step() {
       GP_TRY(cudaEventRecord(r.e0, st(k)));
     }
     GP_TRY(use(k));
+    if (!side_tail.empty() && side_tail[k]) {              // the cell's weight-gradient GEMMs still read its interior
+      GP_TRY(cudaStreamWaitEvent(st(k), side_tail[k], 0));
+      side_tail[k] = nullptr;
+    }
     cudaError_t e = kind == 'B' ? backward_cell(k, m) : forward_cell(k, m, kind == 'R');
     if (e != cudaSuccess) return e;
     if (trace_on) {
@@ -762,6 +824,11 @@ cudaError_t Engine::enqueue_step() {
       GP_TRY(cudaEventRecord(ev_b[k][m], st(k)));
     }
   // join: the loss partials come back on the last cell's stream, and stream 0 waits for every cell
+  for (int k = 0; k < K && !side_tail.empty(); ++k)
+    if (side_tail[k]) {
+      GP_TRY(cudaStreamWaitEvent(st(k), side_tail[k], 0));
+      side_tail[k] = nullptr;
+    }
   GP_TRY(use(K - 1));
   GP_TRY(cudaMemcpyAsync(host_loss, loss_parts, sizeof(float) * M, cudaMemcpyDeviceToHost, st(K - 1)));
   for (int k = 1; k < K; ++k) {

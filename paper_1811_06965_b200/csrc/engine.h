@@ -141,6 +141,14 @@ struct Engine {
   std::vector<float *> dout[2];                        // pipeline: local copy of the gradient wrt cell k's OUTPUT
   std::vector<void *> dout_lp[2];
   std::vector<cudaStream_t> streams;
+  // Optional second stream per cell (single-arena handle with env->n_streams >= 2K): the weight-gradient GEMMs of
+  // B(k, m) have no consumer inside the task, so they run beside the dgrad / LayerNorm / attention chain of the same
+  // cell - what a cell's accelerator would do with them anyway when fewer than ~8 cells share the GPU.  Same kernels,
+  // same accumulation order (the side stream is in-order), hence bitwise the same gradients.  side_tail[k]: the last
+  // side-stream event cell k's main stream has not waited for yet (waited before the cell's next task / the join).
+  std::vector<cudaStream_t> side;
+  std::vector<cudaEvent_t> side_tail;
+  bool side_active() const { return !side.empty() && !serial && !multi() && !trace_on; }
   std::vector<std::vector<float *>> slot;              // slot[k][m], k = 1..K-1: input of cell k
   std::vector<float *> dbound[2];                      // dbound[i][k]: gradient wrt input of cell k
   std::vector<void *> dbound_lp[2];
@@ -183,17 +191,21 @@ struct Engine {
   KStat kstats[KC_NUM];
   cudaError_t resolve_kernel_timing();
   template <typename F>
-  cudaError_t timed(int k, int cls, double flops, double bytes, F &&fn) {
+  cudaError_t timed_on(cudaStream_t s, int cls, double flops, double bytes, F &&fn) {
     if (!ktiming_on) return fn();
     KRec r{cls, flops, bytes, pool_event(), pool_event()};
     if (!r.e0 || !r.e1) return pool_err;
-    cudaError_t e = cudaEventRecord(r.e0, st(k));
+    cudaError_t e = cudaEventRecord(r.e0, s);
     if (e != cudaSuccess) return e;
     e = fn();
     if (e != cudaSuccess) return e;
-    e = cudaEventRecord(r.e1, st(k));
+    e = cudaEventRecord(r.e1, s);
     krecs.push_back(r);
     return e;
+  }
+  template <typename F>
+  cudaError_t timed(int k, int cls, double flops, double bytes, F &&fn) {
+    return timed_on(st(k), cls, flops, bytes, static_cast<F &&>(fn));
   }
 
   // -- construction --

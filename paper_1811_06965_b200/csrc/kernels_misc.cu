@@ -26,6 +26,9 @@ template <> struct VecIO<float> {
     return make_uint4(__float_as_uint(v[0]), __float_as_uint(v[1]), __float_as_uint(v[2]),
                       __float_as_uint(v[3]));
   }
+  __device__ static float vmax(const uint4 &u) {
+    return fmaxf(fmaxf(__uint_as_float(u.x), __uint_as_float(u.y)), fmaxf(__uint_as_float(u.z), __uint_as_float(u.w)));
+  }
 };
 template <> struct VecIO<bf16> {
   static constexpr int W = 8;
@@ -45,14 +48,31 @@ template <> struct VecIO<bf16> {
     for (int i = 0; i < 4; ++i) h[i] = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]);
     return u;
   }
+  __device__ static float vmax(const uint4 &u) {           // the maximum is exact in any format: packed bf16 max
+    const __nv_bfloat162 *h = reinterpret_cast<const __nv_bfloat162 *>(&u);
+    const __nv_bfloat162 m = __hmax2(__hmax2(h[0], h[1]), __hmax2(h[2], h[3]));
+    return fmaxf(__low2float(m), __high2float(m));
+  }
 };
 
-template <typename T, int VPT>
+// 2^x on the special-function unit, one instruction (relative error 2^-22; results below 2^-126 flush to zero)
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+// Instruction budget (the row pass is issue-bound before it is HBM-bound: 131 M elements per config-5 micro-batch):
+// packed max in pass 1; per element one subtract, one multiply / FMA and one ex2 in passes 2 and 3 - the factors
+// 1/sum and 1/T go into the exponent of pass 3 (p / T = 2^((z - max) log2 e - log2 sum + log2 (1/T))); the label's
+// "- 1/T" is applied to its one vector; the clamp exists only in the CLIP instantiation.
+template <typename T, int VPT, bool CLIP>
 __global__ void __launch_bounds__(1024)
 softmax_ce_reg_kernel(T *__restrict__ logits, const int32_t *__restrict__ labels,
                       float *__restrict__ rowloss, int V, float inv_T, float clip) {
-  const float hi = clip > 0.f ? clip : INFINITY, lo = -hi;
+  const float hi = CLIP ? clip : INFINITY, lo = -hi;
   constexpr int W = VecIO<T>::W;
+  constexpr float L2E = 1.4426950408889634f;
   __shared__ float red[33];
   int64_t row = blockIdx.x;
   uint4 *z = reinterpret_cast<uint4 *>(logits + row * (int64_t)V);
@@ -64,14 +84,11 @@ softmax_ce_reg_kernel(T *__restrict__ logits, const int32_t *__restrict__ labels
     int j = threadIdx.x + i * blockDim.x;
     if (j < nvec) {
       raw[i] = z[j];
-      float v[W];
-      VecIO<T>::unpack(raw[i], v);
-#pragma unroll
-      for (int e = 0; e < W; ++e) mx = fmaxf(mx, v[e]);
+      mx = fmaxf(mx, VecIO<T>::vmax(raw[i]));
     }
   }
-  mx = fminf(block_max(mx, red), hi);    // max of the clamped row (the clamp is monotone; V >= 1 so mx >= lo after fmaxf below)
-  mx = fmaxf(mx, lo);
+  mx = block_max(mx, red);
+  if (CLIP) mx = fmaxf(fminf(mx, hi), lo);   // max of the clamped row (the clamp is monotone)
   float s = 0.f;
 #pragma unroll
   for (int i = 0; i < VPT; ++i) {
@@ -80,14 +97,20 @@ softmax_ce_reg_kernel(T *__restrict__ logits, const int32_t *__restrict__ labels
       float v[W];
       VecIO<T>::unpack(raw[i], v);
 #pragma unroll
-      for (int e = 0; e < W; ++e) s += expf(fminf(fmaxf(v[e], lo), hi) - mx);
+      for (int e = 0; e < W; ++e) {
+        const float x = CLIP ? fminf(fmaxf(v[e], lo), hi) : v[e];
+        s += ex2_approx((x - mx) * L2E);
+      }
     }
   }
   s = block_sum(s, red);
-  int lab = labels[row];
-  float inv = 1.f / s;
-  if (threadIdx.x == 0)
-    rowloss[row] = (logf(s) + mx - fminf(fmaxf(to_f<T>(logits[row * (int64_t)V + lab]), lo), hi)) * inv_T;
+  const int lab = labels[row];
+  const int jl = lab / W, el = lab - jl * W;
+  if (threadIdx.x == 0) {
+    const float zl = to_f<T>(logits[row * (int64_t)V + lab]);
+    rowloss[row] = (logf(s) + mx - (CLIP ? fminf(fmaxf(zl, lo), hi) : zl)) * inv_T;
+  }
+  const float c = log2f(inv_T) - log2f(s);
   __syncthreads();                       // z[lab] read before anyone overwrites it
 #pragma unroll
   for (int i = 0; i < VPT; ++i) {
@@ -97,9 +120,22 @@ softmax_ce_reg_kernel(T *__restrict__ logits, const int32_t *__restrict__ labels
       VecIO<T>::unpack(raw[i], v);
 #pragma unroll
       for (int e = 0; e < W; ++e) {
-        float p = expf(fminf(fmaxf(v[e], lo), hi) - mx) * inv;
-        if (j * W + e == lab) p -= 1.f;
-        v[e] = (v[e] >= lo && v[e] <= hi) ? p * inv_T : 0.f;
+        const float x = CLIP ? fminf(fmaxf(v[e], lo), hi) : v[e];
+        const float p = ex2_approx(fmaf(x - mx, L2E, c));
+        v[e] = (!CLIP || (v[e] >= lo && v[e] <= hi)) ? p : 0.f;
+      }
+      if (j == jl) {                       // the label's element: (p - 1) / T, or zero under an active clamp
+        if constexpr (CLIP) {
+          float r[W];
+          VecIO<T>::unpack(raw[i], r);
+#pragma unroll
+          for (int e = 0; e < W; ++e)
+            if (e == el && r[e] >= lo && r[e] <= hi) v[e] -= inv_T;
+        } else {
+#pragma unroll
+          for (int e = 0; e < W; ++e)
+            if (e == el) v[e] -= inv_T;
+        }
       }
       z[j] = VecIO<T>::pack(v);
     }
@@ -140,13 +176,17 @@ static cudaError_t softmax_ce_t(const Ctx &c, T *logits, const int32_t *labels, 
   unsigned grid = (unsigned)n_tok;
   int nvec = V / W;
   bool vec_ok = (V % W == 0);
-  if (vec_ok && nvec <= 256)
-    softmax_ce_reg_kernel<T, 1><<<grid, 256, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
-  else if (vec_ok && nvec <= 1024 * 4)
-    softmax_ce_reg_kernel<T, 4><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
-  else if (vec_ok && nvec <= 1024 * 8)
-    softmax_ce_reg_kernel<T, 8><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
-  else
+  const bool cl = clip > 0.f;
+  if (vec_ok && nvec <= 256) {
+    if (cl) softmax_ce_reg_kernel<T, 1, true><<<grid, 256, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
+    else softmax_ce_reg_kernel<T, 1, false><<<grid, 256, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
+  } else if (vec_ok && nvec <= 1024 * 4) {
+    if (cl) softmax_ce_reg_kernel<T, 4, true><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
+    else softmax_ce_reg_kernel<T, 4, false><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
+  } else if (vec_ok && nvec <= 1024 * 8) {
+    if (cl) softmax_ce_reg_kernel<T, 8, true><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
+    else softmax_ce_reg_kernel<T, 8, false><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
+  } else
     softmax_ce_3pass_kernel<T><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
   GP_LAUNCH_CHECK(c);
 }

@@ -66,36 +66,43 @@ __device__ __forceinline__ float ex2_approx(float x) {
 // packed max in pass 1; per element one subtract, one multiply / FMA and one ex2 in passes 2 and 3 - the factors
 // 1/sum and 1/T go into the exponent of pass 3 (p / T = 2^((z - max) log2 e - log2 sum + log2 (1/T))); the label's
 // "- 1/T" is applied to its one vector; the clamp exists only in the CLIP instantiation.
-template <typename T, int VPT, bool CLIP>
-__global__ void __launch_bounds__(1024)
+// Residency: a row of V = 64000 bf16 is 125 KB - as registers alone it takes a whole SM's register file, and then an SM
+// works on ONE row at a time with nothing to overlap its load, its two block-wide reductions and its store with.  So
+// a block is NT <= 512 threads and keeps VR vectors per thread in registers and VS more in shared memory (thread-
+// private slots, conflict-free): two blocks = two rows in flight per SM.
+template <typename T, int NT, int VR, int VS, bool CLIP>
+__global__ void __launch_bounds__(NT, NT == 512 ? 2 : 1)
 softmax_ce_reg_kernel(T *__restrict__ logits, const int32_t *__restrict__ labels,
                       float *__restrict__ rowloss, int V, float inv_T, float clip) {
   const float hi = CLIP ? clip : INFINITY, lo = -hi;
   constexpr int W = VecIO<T>::W;
   constexpr float L2E = 1.4426950408889634f;
+  extern __shared__ uint4 spill[];          // [VS][NT]
   __shared__ float red[33];
   int64_t row = blockIdx.x;
   uint4 *z = reinterpret_cast<uint4 *>(logits + row * (int64_t)V);
   int nvec = V / W;
-  uint4 raw[VPT];
+  uint4 raw[VR];
   float mx = -INFINITY;
 #pragma unroll
-  for (int i = 0; i < VPT; ++i) {
-    int j = threadIdx.x + i * blockDim.x;
+  for (int i = 0; i < VR + VS; ++i) {
+    int j = threadIdx.x + i * NT;
     if (j < nvec) {
-      raw[i] = z[j];
-      mx = fmaxf(mx, VecIO<T>::vmax(raw[i]));
+      const uint4 u = z[j];
+      if (i < VR) raw[i < VR ? i : 0] = u;
+      else spill[(i - VR) * NT + threadIdx.x] = u;
+      mx = fmaxf(mx, VecIO<T>::vmax(u));
     }
   }
   mx = block_max(mx, red);
   if (CLIP) mx = fmaxf(fminf(mx, hi), lo);   // max of the clamped row (the clamp is monotone)
   float s = 0.f;
 #pragma unroll
-  for (int i = 0; i < VPT; ++i) {
-    int j = threadIdx.x + i * blockDim.x;
+  for (int i = 0; i < VR + VS; ++i) {
+    int j = threadIdx.x + i * NT;
     if (j < nvec) {
       float v[W];
-      VecIO<T>::unpack(raw[i], v);
+      VecIO<T>::unpack(i < VR ? raw[i < VR ? i : 0] : spill[(i - VR) * NT + threadIdx.x], v);
 #pragma unroll
       for (int e = 0; e < W; ++e) {
         const float x = CLIP ? fminf(fmaxf(v[e], lo), hi) : v[e];
@@ -113,11 +120,12 @@ softmax_ce_reg_kernel(T *__restrict__ logits, const int32_t *__restrict__ labels
   const float c = log2f(inv_T) - log2f(s);
   __syncthreads();                       // z[lab] read before anyone overwrites it
 #pragma unroll
-  for (int i = 0; i < VPT; ++i) {
-    int j = threadIdx.x + i * blockDim.x;
+  for (int i = 0; i < VR + VS; ++i) {
+    int j = threadIdx.x + i * NT;
     if (j < nvec) {
+      const uint4 u = i < VR ? raw[i < VR ? i : 0] : spill[(i - VR) * NT + threadIdx.x];
       float v[W];
-      VecIO<T>::unpack(raw[i], v);
+      VecIO<T>::unpack(u, v);
 #pragma unroll
       for (int e = 0; e < W; ++e) {
         const float x = CLIP ? fminf(fmaxf(v[e], lo), hi) : v[e];
@@ -127,7 +135,7 @@ softmax_ce_reg_kernel(T *__restrict__ logits, const int32_t *__restrict__ labels
       if (j == jl) {                       // the label's element: (p - 1) / T, or zero under an active clamp
         if constexpr (CLIP) {
           float r[W];
-          VecIO<T>::unpack(raw[i], r);
+          VecIO<T>::unpack(u, r);
 #pragma unroll
           for (int e = 0; e < W; ++e)
             if (e == el && r[e] >= lo && r[e] <= hi) v[e] -= inv_T;
@@ -178,14 +186,18 @@ static cudaError_t softmax_ce_t(const Ctx &c, T *logits, const int32_t *labels, 
   bool vec_ok = (V % W == 0);
   const bool cl = clip > 0.f;
   if (vec_ok && nvec <= 256) {
-    if (cl) softmax_ce_reg_kernel<T, 1, true><<<grid, 256, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
-    else softmax_ce_reg_kernel<T, 1, false><<<grid, 256, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
-  } else if (vec_ok && nvec <= 1024 * 4) {
-    if (cl) softmax_ce_reg_kernel<T, 4, true><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
-    else softmax_ce_reg_kernel<T, 4, false><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
-  } else if (vec_ok && nvec <= 1024 * 8) {
-    if (cl) softmax_ce_reg_kernel<T, 8, true><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
-    else softmax_ce_reg_kernel<T, 8, false><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
+    if (cl) softmax_ce_reg_kernel<T, 256, 1, 0, true><<<grid, 256, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
+    else softmax_ce_reg_kernel<T, 256, 1, 0, false><<<grid, 256, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
+  } else if (vec_ok && nvec <= 512 * 8) {
+    if (cl) softmax_ce_reg_kernel<T, 512, 8, 0, true><<<grid, 512, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
+    else softmax_ce_reg_kernel<T, 512, 8, 0, false><<<grid, 512, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
+  } else if (vec_ok && nvec <= 512 * 16) {
+    constexpr size_t smem = (size_t)8 * 512 * sizeof(uint4);            // 64 KB: two blocks per SM
+    cudaError_t e = cl ? ensure_dyn_smem<softmax_ce_reg_kernel<T, 512, 8, 8, true>>(smem, c.device)
+                       : ensure_dyn_smem<softmax_ce_reg_kernel<T, 512, 8, 8, false>>(smem, c.device);
+    if (e != cudaSuccess) return e;
+    if (cl) softmax_ce_reg_kernel<T, 512, 8, 8, true><<<grid, 512, smem, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
+    else softmax_ce_reg_kernel<T, 512, 8, 8, false><<<grid, 512, smem, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
   } else
     softmax_ce_3pass_kernel<T><<<grid, 1024, 0, c.stream>>>(logits, labels, rowloss, V, inv_T, clip);
   GP_LAUNCH_CHECK(c);

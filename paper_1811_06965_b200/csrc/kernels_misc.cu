@@ -11,9 +11,9 @@ namespace gp {
 // Logit clipping ("we clip the logit predictions (softmax pre-activations) whenever their magnitude
 // exceeds a certain value"; reading B5): with clip > 0 the softmax sees z = min(max(logit, -clip), clip) and the
 // gradient is zero wherever the clamp is active (|logit| > clip); clip == 0 turns it off.
-// The row is read once from HBM into registers (VPT vectors of 8 (bf16) / 4 (fp32) elements per
-// thread) when it fits, so HBM traffic is one read + one write of the row; longer rows fall
-// back to three passes over global memory (L2-resident row).
+// The row is read once from HBM and kept on the SM - vectors of 8 (bf16) / 4 (fp32) elements, VR per thread in
+// registers and VS more in shared memory - when it fits (up to 8192 vectors), so HBM traffic is one read + one
+// write of the row; longer rows fall back to three passes over global memory (L2-resident row).
 // ---------------------------------------------------------------------------------------------
 template <typename T> struct VecIO;       // 16-byte vectors kept packed in registers
 template <> struct VecIO<float> {

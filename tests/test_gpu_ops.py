@@ -719,6 +719,37 @@ def test_softmax_ce_with_logit_clipping(dtype, n, V):
     assert torch.equal(z0, z1)
 
 
+@pytest.mark.parametrize("clip", [0.0, 2.5])
+@pytest.mark.parametrize("dtype,V", [("bf16", 64000), ("fp32", 32000), ("bf16", 32000)])
+def test_softmax_ce_label_positions(dtype, V, clip):
+    """The row lives on the SM as 16-byte vectors, vector j in slot j // 512 of thread j % 512: slots 0..7 are
+    registers, 8..15 shared memory (rows beyond 4096 vectors).  The label's -1/T goes to one element of one vector:
+    put it at the first / last element of the first register vector, across the register / shared-memory boundary
+    and at the row's last element, with and without the clamp (reading B5)."""
+    from oracle import encdec_oracle as eo
+    W = 8 if dtype == "bf16" else 4
+    nvec = V // W
+    pos = [0, W - 1, W, 511 * W + 3, 512 * W, min(4096, nvec) * W - 1, min(4096, nvec - 1) * W, (nvec - 1) * W, V - 1]
+    n = len(pos)
+    r = _rng(5 * V + n)
+    zt, zq = _lp(r.standard_normal((n, V)) * 3, dtype)
+    labels = np.asarray(pos, dtype=np.int32)
+    rowloss = torch.empty(n, device=DEV)
+    if clip > 0:
+        loss_ref, dl_ref, per_tok = eo.softmax_ce_clipped(zq.astype(np.float64), labels, 77, clip)
+    else:
+        loss_ref, dl_ref = go.softmax_ce(zq, labels, 77)
+    ops.softmax_ce(zt, torch.tensor(labels, device=DEV), rowloss, 1.0 / 77, clip)
+    got = _np(zt)
+    assert abs(float(rowloss.double().sum()) - loss_ref) <= 2e-5 * abs(loss_ref)
+    tol, cos = _tol(dtype)
+    assert maxrel(got, dl_ref) <= tol and cosine(got, dl_ref) >= cos
+    for t, v in enumerate(pos):                              # the label's own element, one by one
+        assert abs(got[t, v] - dl_ref[t, v]) <= tol * max(abs(dl_ref[t, v]), 1.0 / 77), (t, v)
+        if clip > 0:
+            assert (got[t, v] == 0) == (abs(zq[t, v]) > clip)
+
+
 @pytest.mark.parametrize("dtype", ["fp32", "bf16"])
 def test_colsum_embedding_sgd(dtype):
     r = _rng(11)
